@@ -1,0 +1,182 @@
+/* cfs.h -- C ABI of the B200-native Composable Function System (CFS) hot path.
+ *
+ * What it computes (arxiv/paper_2606_02226, "Composable function systems as a general-purpose
+ * rendering framework"; citations "PAPER L<n>" are lines of the paper's text, "DESIGN R<n>" are
+ * the readings listed in DESIGN.md where the paper is silent):
+ *
+ *   chaos game: every point picks one function of the generator IFS at
+ *   random each step and applies it; a COPY of the point (Fig. 1, L77 Fig. 2(B)) runs
+ *   through the ordered chain of later, possibly non-affine, transforms and
+ *   is splatted / histogrammed into the output image; colours show the function
+ *   that produced the point.  The generator may instead be a stored point cloud
+ *   (PAPER L25, L206).
+ *
+ * All kernels are hand-written CUDA for sm_100a.  There is no CPU fallback: every entry point
+ * that does work needs a CUDA device and returns CFS_ERR_CUDA without one.
+ *
+ * Conventions
+ *   - plain C types only; pointers named d_* are DEVICE pointers, h_* are HOST pointers.
+ *   - every call returns cfs_status; nothing throws, aborts or prints.  cfs_last_error() gives
+ *     a thread-local message for the last non-OK status on the calling thread.
+ *   - cfs_create copies everything it is given; the caller keeps ownership of its arrays.
+ *   - cfs_render / cfs_tonemap / cfs_trace / cfs_microbench are asynchronous on `cuda_stream`
+ *     (a cudaStream_t passed as void*; NULL = the legacy default stream) and never synchronise.
+ *     They allocate no device memory (only the output image lives in global
+ *     memory); tables travel in the kernel parameter block.
+ *   - images are caller-owned and caller-cleared (0 for HIST/RGBA, all-ones bytes for DEPTH);
+ *     renders ACCUMULATE, so frames, point sub-ranges and GPUs compose by sum / min.
+ */
+#ifndef CFS_H
+#define CFS_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define CFS_MAX_FUNCS 64
+#define CFS_MAX_CHAIN 8
+
+typedef struct cfs_system cfs_system; /* opaque, host-side, owned by the library */
+
+typedef enum {
+    CFS_OK = 0,
+    CFS_ERR_INVALID_ARG = 1,
+    CFS_ERR_UNSUPPORTED = 2,
+    CFS_ERR_CUDA = 3,
+    CFS_ERR_NOMEM = 4
+} cfs_status;
+
+/* generator: an IFS solved by the chaos game, or a stored cloud */
+typedef enum { CFS_GEN_IFS = 0, CFS_GEN_CLOUD = 1 } cfs_gen_kind;
+/* generator function types.  AFFINE params: dim 2: a00 a01 a10 a11 b0 b1;
+ * dim 3: a00..a22 row-major, then b0 b1 b2.  x' = fma(a00,x,fma(a01,y,b0)) etc. (DESIGN R4). */
+typedef enum { CFS_F_AFFINE = 0 } cfs_func_type;
+typedef struct { int32_t type; float prob; float params[12]; } cfs_func;
+
+/* chain transform types (applied to the copy, in order).  Effective parameter i of a step is
+ * (float)((double)p0[i] + (double)t*(double)p1[i]), resolved on the host once per render.
+ *   AFFINE      params as cfs_func AFFINE
+ *   SWIRL       r2 = x^2+y^2; (x,y) rotated by r2                         (BASELINE cfg 1)
+ *   SINUSOIDAL  (sin x, sin y), z kept                                    (BASELINE cfg 2)
+ *   ROTATE_Z    p[0] = angle; resolved on the host to an AFFINE rotation  (BASELINE cfg 2)
+ *   TWIST_Z     (x,y) rotated by p[0]*z                                   (BASELINE cfg 3)
+ *   BEND        (x,y) rotated by p[0]*x (input x)                         (DESIGN R6)
+ *   PINHOLE     p = (fov_y degrees, cam_z, near): d = z-cam_z; dropped unless d > near;
+ *               x' = (fx*x)*(1/d), y' = (fy*y)*(1/d), z' = d; fy = 1/tan(fov/2), fx = fy*H/W
+ *   STRETCH_COS x' = 2x, y' = y - cos x                                   (PAPER Eq. 2) */
+typedef enum {
+    CFS_T_AFFINE = 0, CFS_T_SWIRL = 1, CFS_T_SINUSOIDAL = 2, CFS_T_ROTATE_Z = 3,
+    CFS_T_TWIST_Z = 4, CFS_T_BEND = 5, CFS_T_PINHOLE = 6, CFS_T_STRETCH_COS = 7
+} cfs_xform_type;
+typedef struct { int32_t type; float p0[12]; float p1[12]; } cfs_xform;
+
+/* colour rule and output layer (BASELINE cfg 0-4) */
+typedef enum { CFS_COLOR_NONE = 0, CFS_COLOR_MAP_INDEX = 1, CFS_COLOR_POINT = 2 } cfs_color_rule;
+typedef enum {
+    CFS_OUT_HIST_U32 = 0,        /* uint32[H*W]: hits                                    */
+    CFS_OUT_RGBA_F32 = 1,        /* float[H*W*4]: sum of (r,g,b,1), 16-byte aligned      */
+    CFS_OUT_DEPTH_RGBA8_U64 = 2  /* uint64[H*W]: min of (bits(depth)<<32 | rgba8)        */
+} cfs_out_mode;
+
+/* splat-stage variant (BASELINE north_star: "two variants chosen by image size") */
+typedef enum {
+    CFS_VARIANT_AUTO = 0,        /* chosen from mode and image bytes                                  */
+    CFS_VARIANT_DIRECT = 1,      /* one L2 reduction per splat (red.global / atom.global.min.u64)     */
+    CFS_VARIANT_SHARED_HIST = 2, /* HIST only, W*H*4 <= cfs_shared_hist_max_bytes(): per-CTA shared   */
+                                 /* histogram, merged with red.global                                 */
+    CFS_VARIANT_WARP_AGG = 3     /* DIRECT + __match_any_sync aggregation of same-pixel hits (HIST)   */
+} cfs_variant;
+
+/* one 16-byte record of a stored cloud (BASELINE cfg 3); rgba8 = r | g<<8 | b<<16 | a<<24 */
+typedef struct { float x, y, z; uint32_t rgba8; } cfs_cloud_rec;
+
+/* cfs_create -- the generator IFS (per-function type id, parameters, selection probabilities),
+ * the ordered transform chain and the colouring rule (BASELINE north_star).
+ *   dim 2|3.  funcs/n_funcs: 1..CFS_MAX_FUNCS, ignored for CLOUD.  chain/n_chain: 0..CFS_MAX_CHAIN.
+ *   palette_rgba: n_funcs*4 floats (integer-valued 0..255 by convention, DESIGN R9), required for
+ *   MAP_INDEX, else NULL.  reuse != 0 selects Fig. 2(C) composition (chain output fed back).
+ * Errors: INVALID_ARG for bad dims/counts/types, prob < 0 / NaN / sum <= 0, rule mismatch
+ * (COLOR_POINT needs CLOUD; MAP_INDEX needs IFS + palette). Host only: no device work. */
+cfs_status cfs_create(cfs_system **out, int32_t dim, int32_t gen_kind,
+                      const cfs_func *funcs, int32_t n_funcs,
+                      const cfs_xform *chain, int32_t n_chain,
+                      int32_t color_rule, const float *palette_rgba, int32_t reuse);
+void cfs_destroy(cfs_system *sys);
+
+typedef struct {
+    uint64_t n_points;      /* 0 is a no-op                                                     */
+    uint64_t point_offset;  /* first global point id (sub-range renders, multi-GPU sharding)    */
+    uint64_t seed;          /* Philox key                                                       */
+    int32_t iterations;     /* >= 1; CLOUD: must be 1                                           */
+    int32_t burn_in;        /* 0 <= burn_in < iterations; CLOUD: 0                              */
+    int32_t width, height;  /* width*height <= 2^31-1                                           */
+    float xmin, xmax, ymin, ymax; /* closed bounds; row 0 is ymin (DESIGN R8)                   */
+    float t;                /* frame parameter                                                  */
+    int32_t out_mode;       /* cfs_out_mode                                                     */
+    int32_t variant;        /* cfs_variant                                                      */
+    int32_t reserved_;      /* must be 0                                                        */
+    void *d_image;          /* device, caller-owned, caller-cleared, accumulates                */
+    const void *d_cloud;    /* device, CLOUD only: record p of the WHOLE cloud is d_cloud[p]    */
+    uint64_t *d_counters;   /* optional device u64[2]: += in-bounds splats, += dropped splats   */
+} cfs_render_args;
+
+/* cfs_render -- the hot path: sampler + pick + map + chain + colour + splat, one kernel launch.
+ * Errors: INVALID_ARG, UNSUPPORTED (variant impossible for the mode
+ * or image), CUDA (launch failure; message holds the CUDA error string). */
+cfs_status cfs_render(const cfs_system *sys, const cfs_render_args *args, void *cuda_stream);
+
+/* cfs_render_host -- same path with HOST buffers (end-to-end entry point): copies h_cloud to the
+ * device (CLOUD), clears a device image, renders [point_offset, +n_points), copies the image to
+ * h_image (layout of out_mode) and the counters to h_counters (u64[2], optional); synchronises
+ * the stream before returning.  args->d_image/d_cloud/d_counters are ignored.  Scratch device
+ * buffers are cached in the system handle and freed by cfs_destroy. */
+cfs_status cfs_render_host(cfs_system *sys, const cfs_render_args *args, void *h_image,
+                           const cfs_cloud_rec *h_cloud, uint64_t *h_counters, void *cuda_stream);
+
+/* cfs_tonemap -- log-density tone map to RGBA8 (DESIGN R10; fractal-flame convention, PAPER L31,
+ * L208): n = count (HIST value / RGBA alpha), n_max = max n; n = 0 -> 0; L = log(1+n)/log(1+n_max);
+ * v_c = clamp(colour_scale * acc_c/n * L^(1/gamma), 0, 1) (HIST: v = L^(1/gamma)); alpha = L;
+ * byte = floor(255 v + 0.5).  DEPTH: out = low 32 bits, empty -> 0.
+ * d_scratch: >= 8 bytes of device memory (overwritten).  Two kernels on the stream. */
+cfs_status cfs_tonemap(const void *d_image, int32_t out_mode, int32_t width, int32_t height,
+                       float gamma, float colour_scale, uint32_t *d_rgba8_out, void *d_scratch,
+                       void *cuda_stream);
+
+/* cfs_trace -- parity instrument (same device functions as cfs_render, no splat): per point the
+ * pick sequence d_picks[n_points*iterations] (u8), the final generator state d_final_g[n*3],
+ * the final chain output d_final_q[n*3] and its alive flag d_alive[n] (u8).  Any may be NULL. */
+cfs_status cfs_trace(const cfs_system *sys, const cfs_render_args *args, uint8_t *d_picks,
+                     float *d_final_g, float *d_final_q, uint8_t *d_alive, void *cuda_stream);
+
+/* cfs_microbench -- roofline denominators measured in the same run (BASELINE north_star).
+ * Launches `blocks` x `threads` threads each doing `ops_per_thread` operations of `kind`;
+ * the caller times the stream.  Memory kinds address `footprint_bytes` of d_buf uniformly at
+ * random (hash of a per-thread counter); ALU kinds ignore d_buf except for one sink store. */
+typedef enum {
+    CFS_MB_RED_ADD_U32 = 0,     /* red.global.add.u32, random 4-byte bins                */
+    CFS_MB_RED_ADD_V4F32 = 1,   /* red.global.add.v4.f32, random 16-byte pixels          */
+    CFS_MB_ATOM_MIN_U64 = 2,    /* atom.global.min.u64 (result unused), random bins      */
+    CFS_MB_LD_U64 = 3,          /* ld.global.cg.u64 at random bins (depth pre-test)      */
+    CFS_MB_ATOMS_ADD_U32 = 4,   /* atom.shared.add.u32 over footprint_bytes of shared    */
+    CFS_MB_FFMA = 5,            /* dependent-chain FFMA x 8 independent chains           */
+    CFS_MB_IMAD_WIDE = 6,       /* 32x32->64 multiply chains (Philox core)               */
+    CFS_MB_LOP3 = 7,            /* 3-input logic chains                                  */
+    CFS_MB_MUFU = 8,            /* sin.approx chains                                     */
+    CFS_MB_STREAM_LD128 = 9     /* coalesced 128-bit loads over footprint_bytes          */
+} cfs_microbench_kind;
+cfs_status cfs_microbench(int32_t kind, void *d_buf, uint64_t footprint_bytes,
+                          uint64_t ops_per_thread, int32_t blocks, int32_t threads,
+                          void *cuda_stream);
+
+/* largest W*H*4 the SHARED_HIST variant accepts on the current device (0 without a device) */
+uint64_t cfs_shared_hist_max_bytes(void);
+/* kernels launched by this library on the calling thread since the last reset (bench accounting) */
+uint64_t cfs_launch_count(int32_t reset);
+const char *cfs_last_error(void);
+const char *cfs_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CFS_H */

@@ -1,0 +1,273 @@
+"""Thin ctypes binding of libcfs_b200.so (include/cfs.h) -- argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of csrc/; PyTorch is used for device memory
+and streams, nothing else.  There is no CPU fallback: if the library is missing or cannot be
+loaded this module raises at import of the first symbol.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libcfs_b200.so")
+
+CFS_OK, CFS_ERR_INVALID_ARG, CFS_ERR_UNSUPPORTED, CFS_ERR_CUDA, CFS_ERR_NOMEM = range(5)
+GEN = {"ifs": 0, "cloud": 1}
+F_TYPE = {"affine": 0}
+T_TYPE = {"affine": 0, "swirl": 1, "sinusoidal": 2, "rotate_z": 3, "twist_z": 4, "bend": 5,
+          "pinhole": 6, "stretch_cos": 7}
+COLOR = {"none": 0, "map_index": 1, "point": 2}
+OUT = {"hist_u32": 0, "rgba_f32": 1, "depth_u64": 2}
+VARIANT = {"auto": 0, "direct": 1, "shared_hist": 2, "warp_agg": 3}
+MB = {"red_add_u32": 0, "red_add_v4f32": 1, "atom_min_u64": 2, "ld_u64": 3, "atoms_add_u32": 4,
+      "ffma": 5, "imad_wide": 6, "lop3": 7, "mufu": 8, "stream_ld128": 9}
+EXPORTS = ["cfs_create", "cfs_destroy", "cfs_render", "cfs_render_host", "cfs_tonemap", "cfs_trace",
+           "cfs_microbench", "cfs_shared_hist_max_bytes", "cfs_launch_count", "cfs_last_error",
+           "cfs_version"]
+
+
+class CfsError(RuntimeError):
+    def __init__(self, status: int, message: str):
+        super().__init__(f"cfs status {status}: {message}")
+        self.status = status
+
+
+class cfs_func(C.Structure):
+    _fields_ = [("type", C.c_int32), ("prob", C.c_float), ("params", C.c_float * 12)]
+
+
+class cfs_xform(C.Structure):
+    _fields_ = [("type", C.c_int32), ("p0", C.c_float * 12), ("p1", C.c_float * 12)]
+
+
+class cfs_render_args(C.Structure):
+    _fields_ = [("n_points", C.c_uint64), ("point_offset", C.c_uint64), ("seed", C.c_uint64),
+                ("iterations", C.c_int32), ("burn_in", C.c_int32),
+                ("width", C.c_int32), ("height", C.c_int32),
+                ("xmin", C.c_float), ("xmax", C.c_float), ("ymin", C.c_float), ("ymax", C.c_float),
+                ("t", C.c_float), ("out_mode", C.c_int32), ("variant", C.c_int32),
+                ("reserved_", C.c_int32),
+                ("d_image", C.c_void_p), ("d_cloud", C.c_void_p), ("d_counters", C.c_void_p)]
+
+
+_lib = None
+
+
+def lib():
+    """Load the CUDA library (built in-tree by paper_2606_02226_b200.build). Fails loudly."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_2606_02226_b200.build` "
+                              "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        L.cfs_create.argtypes = [C.POINTER(C.c_void_p), C.c_int32, C.c_int32, C.POINTER(cfs_func), C.c_int32,
+                                 C.POINTER(cfs_xform), C.c_int32, C.c_int32, C.POINTER(C.c_float), C.c_int32]
+        L.cfs_create.restype = C.c_int
+        L.cfs_destroy.argtypes = [C.c_void_p]
+        L.cfs_destroy.restype = None
+        L.cfs_render.argtypes = [C.c_void_p, C.POINTER(cfs_render_args), C.c_void_p]
+        L.cfs_render.restype = C.c_int
+        L.cfs_render_host.argtypes = [C.c_void_p, C.POINTER(cfs_render_args), C.c_void_p, C.c_void_p,
+                                      C.c_void_p, C.c_void_p]
+        L.cfs_render_host.restype = C.c_int
+        L.cfs_tonemap.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_float, C.c_float,
+                                  C.c_void_p, C.c_void_p, C.c_void_p]
+        L.cfs_tonemap.restype = C.c_int
+        L.cfs_trace.argtypes = [C.c_void_p, C.POINTER(cfs_render_args), C.c_void_p, C.c_void_p, C.c_void_p,
+                                C.c_void_p, C.c_void_p]
+        L.cfs_trace.restype = C.c_int
+        L.cfs_microbench.argtypes = [C.c_int32, C.c_void_p, C.c_uint64, C.c_uint64, C.c_int32, C.c_int32,
+                                     C.c_void_p]
+        L.cfs_microbench.restype = C.c_int
+        L.cfs_shared_hist_max_bytes.argtypes = []
+        L.cfs_shared_hist_max_bytes.restype = C.c_uint64
+        L.cfs_launch_count.argtypes = [C.c_int32]
+        L.cfs_launch_count.restype = C.c_uint64
+        L.cfs_last_error.argtypes = []
+        L.cfs_last_error.restype = C.c_char_p
+        L.cfs_version.argtypes = []
+        L.cfs_version.restype = C.c_char_p
+        _lib = L
+    return _lib
+
+
+def _check(status: int):
+    if status != CFS_OK:
+        raise CfsError(status, lib().cfs_last_error().decode())
+
+
+def cfs_version() -> str:
+    return lib().cfs_version().decode()
+
+
+def cfs_last_error() -> str:
+    return lib().cfs_last_error().decode()
+
+
+def cfs_launch_count(reset: bool = False) -> int:
+    return int(lib().cfs_launch_count(1 if reset else 0))
+
+
+def cfs_shared_hist_max_bytes() -> int:
+    return int(lib().cfs_shared_hist_max_bytes())
+
+
+def _ptr(x) -> Optional[int]:
+    """Device/host pointer of a torch tensor, numpy array, int or None."""
+    if x is None:
+        return None
+    if isinstance(x, int):
+        return x
+    if isinstance(x, np.ndarray):
+        return x.ctypes.data
+    return x.data_ptr()
+
+
+def _stream(stream) -> Optional[int]:
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+    if isinstance(stream, int):
+        return stream
+    return stream.cuda_stream
+
+
+class System:
+    """Owner of a cfs_system handle (cfs_create / cfs_destroy)."""
+
+    def __init__(self, handle: int):
+        self.handle = handle
+
+    def close(self):
+        if self.handle:
+            lib().cfs_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def cfs_create(system) -> System:
+    """cfs_create from a description with the attributes of workloads.System."""
+    nf = len(system.funcs)
+    funcs = (cfs_func * max(1, nf))()
+    for j, f in enumerate(system.funcs):
+        funcs[j].type = F_TYPE[f.type] if isinstance(f.type, str) else int(f.type)
+        funcs[j].prob = float(f.prob)
+        for i, v in enumerate(f.params):
+            funcs[j].params[i] = float(v)
+    nc = len(system.chain)
+    chain = (cfs_xform * max(1, nc))()
+    for m, x in enumerate(system.chain):
+        chain[m].type = T_TYPE[x.type] if isinstance(x.type, str) else int(x.type)
+        for i, v in enumerate(x.p0):
+            chain[m].p0[i] = float(v)
+        for i, v in enumerate(x.p1):
+            chain[m].p1[i] = float(v)
+    pal = None
+    if system.palette is not None:
+        pal_arr = np.ascontiguousarray(system.palette, dtype=np.float32)
+        pal = pal_arr.ctypes.data_as(C.POINTER(C.c_float))
+    out = C.c_void_p()
+    _check(lib().cfs_create(C.byref(out), int(system.dim), GEN[system.gen] if isinstance(system.gen, str) else int(system.gen),
+                            funcs, nf, chain, nc,
+                            COLOR[system.color] if isinstance(system.color, str) else int(system.color),
+                            pal, 1 if getattr(system, "reuse", False) else 0))
+    return System(out.value)
+
+
+def make_args(render, d_image=None, d_cloud=None, d_counters=None, n_points=None, point_offset=None,
+              t=None, variant="auto") -> cfs_render_args:
+    a = cfs_render_args()
+    a.n_points = int(render.n_points if n_points is None else n_points)
+    a.point_offset = int(render.point_offset if point_offset is None else point_offset)
+    a.seed = int(render.seed)
+    a.iterations = int(render.iterations)
+    a.burn_in = int(render.burn_in)
+    a.width = int(render.width)
+    a.height = int(render.height)
+    a.xmin, a.xmax, a.ymin, a.ymax = [float(np.float32(v)) for v in render.bounds]
+    a.t = float(render.t if t is None else t)
+    a.out_mode = OUT[render.out_mode] if isinstance(render.out_mode, str) else int(render.out_mode)
+    a.variant = VARIANT[variant] if isinstance(variant, str) else int(variant)
+    a.reserved_ = 0
+    a.d_image = _ptr(d_image)
+    a.d_cloud = _ptr(d_cloud)
+    a.d_counters = _ptr(d_counters)
+    return a
+
+
+def cfs_render(sys: System, args: cfs_render_args, stream=None) -> None:
+    _check(lib().cfs_render(sys.handle, C.byref(args), _stream(stream)))
+
+
+def cfs_render_host(sys: System, args: cfs_render_args, h_image: np.ndarray, h_cloud: Optional[np.ndarray] = None,
+                    h_counters: Optional[np.ndarray] = None, stream=None) -> None:
+    _check(lib().cfs_render_host(sys.handle, C.byref(args), _ptr(h_image), _ptr(h_cloud), _ptr(h_counters),
+                                 _stream(stream)))
+
+
+def cfs_tonemap(d_image, out_mode, width: int, height: int, gamma: float, colour_scale: float, d_rgba8_out,
+                d_scratch, stream=None) -> None:
+    mode = OUT[out_mode] if isinstance(out_mode, str) else int(out_mode)
+    _check(lib().cfs_tonemap(_ptr(d_image), mode, int(width), int(height), float(gamma), float(colour_scale),
+                             _ptr(d_rgba8_out), _ptr(d_scratch), _stream(stream)))
+
+
+def cfs_trace(sys: System, args: cfs_render_args, d_picks=None, d_final_g=None, d_final_q=None, d_alive=None,
+              stream=None) -> None:
+    _check(lib().cfs_trace(sys.handle, C.byref(args), _ptr(d_picks), _ptr(d_final_g), _ptr(d_final_q),
+                           _ptr(d_alive), _stream(stream)))
+
+
+def cfs_microbench(kind, d_buf, footprint_bytes: int, ops_per_thread: int, blocks: int, threads: int,
+                   stream=None) -> None:
+    k = MB[kind] if isinstance(kind, str) else int(kind)
+    _check(lib().cfs_microbench(k, _ptr(d_buf), int(footprint_bytes), int(ops_per_thread), int(blocks),
+                                int(threads), _stream(stream)))
+
+
+# ------------------------------------------------------------------ device-memory helpers (torch)
+def new_image(render, device="cuda"):
+    """Cleared device image for a render: HIST int32 view of u32, RGBA float32[.,4], DEPTH int64 = -1."""
+    import torch
+    n = int(render.width) * int(render.height)
+    if render.out_mode == "hist_u32":
+        return torch.zeros(n, dtype=torch.int32, device=device)
+    if render.out_mode == "rgba_f32":
+        return torch.zeros((n, 4), dtype=torch.float32, device=device)
+    if render.out_mode == "depth_u64":
+        return torch.full((n,), -1, dtype=torch.int64, device=device)
+    raise ValueError(render.out_mode)
+
+
+def image_to_numpy(img, out_mode: str) -> np.ndarray:
+    a = img.detach().cpu().numpy()
+    if out_mode == "hist_u32":
+        return a.view(np.uint32)
+    if out_mode == "depth_u64":
+        return a.view(np.uint64)
+    return a
+
+
+def cloud_to_device(cloud: np.ndarray, device="cuda"):
+    """16-byte records -> device tensor (uint8 view; the kernel reads 128-bit records)."""
+    import torch
+    assert cloud.dtype.itemsize == 16 and cloud.flags.c_contiguous
+    return torch.from_numpy(cloud.view(np.uint8).reshape(-1, 16)).to(device)
+
+
+def shard_points(n_points: int, rank: int, world: int):
+    """Contiguous point range of `rank` (multi-GPU: points are independent units, DESIGN 'multi-GPU').
+    Returns (point_offset, n_points_local)."""
+    lo = (n_points * rank) // world
+    hi = (n_points * (rank + 1)) // world
+    return lo, hi - lo

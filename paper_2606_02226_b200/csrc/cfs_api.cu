@@ -1,0 +1,557 @@
+// cfs_api.cu -- C ABI of the CFS hot path (include/cfs.h): validation, host-side resolution of
+// tables and frame-dependent parameters, kernel selection and launch.  No CPU fallback.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/cfs.h"
+#include "cfs_microbench.cuh"
+#include "cfs_render.cuh"
+#include "cfs_tonemap.cuh"
+
+static_assert((int)CFS_T_AFFINE == (int)cfs::T_AFFINE && (int)CFS_T_SWIRL == (int)cfs::T_SWIRL &&
+              (int)CFS_T_SINUSOIDAL == (int)cfs::T_SINUSOIDAL && (int)CFS_T_ROTATE_Z == (int)cfs::T_ROTATE_Z &&
+              (int)CFS_T_TWIST_Z == (int)cfs::T_TWIST_Z && (int)CFS_T_BEND == (int)cfs::T_BEND &&
+              (int)CFS_T_PINHOLE == (int)cfs::T_PINHOLE && (int)CFS_T_STRETCH_COS == (int)cfs::T_STRETCH_COS,
+              "chain type ids");
+static_assert(CFS_MAX_FUNCS == cfs::kMaxFuncs && CFS_MAX_CHAIN == cfs::kMaxChain, "limits");
+static_assert(sizeof(cfs_cloud_rec) == 16, "cloud record is one 128-bit load");
+static_assert(sizeof(cfs::RenderParams) < 16 * 1024, "parameter block");
+
+namespace {
+
+thread_local char g_err[512] = "";
+thread_local uint64_t g_launches = 0;
+
+cfs_status fail(cfs_status st, const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return st;
+}
+
+cfs_status cuda_fail(cudaError_t e, const char *what)
+{
+    return fail(CFS_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+
+struct DeviceInfo { int ok = -1; int sms = 0; int smem_optin = 0; };
+
+const DeviceInfo &device_info()
+{
+    static thread_local DeviceInfo di;
+    if (di.ok < 0) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess) { di.ok = 0; cudaGetLastError(); return di; }
+        cudaDeviceGetAttribute(&di.sms, cudaDevAttrMultiProcessorCount, dev);
+        cudaDeviceGetAttribute(&di.smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+        di.ok = (di.sms > 0) ? 1 : 0;
+    }
+    return di;
+}
+
+}  // namespace
+
+// -------------------------------------------------------------------------------------------------
+struct cfs_system {
+    int32_t dim = 2, gen = 0, color = 0, reuse = 0;
+    std::vector<cfs_func> funcs;
+    std::vector<cfs_xform> chain;
+    std::vector<float> palette;
+    // pick tables (DESIGN R2)
+    uint32_t T[cfs::kMaxFuncs];
+    uint8_t lut[256];
+    int32_t n_thr = 0, pick_steps = 0, pick_shift = -1;
+    int32_t aff = cfs::AFF_GENERAL;
+    float coef[cfs::kMaxFuncs * 12];
+    uint32_t pal8[cfs::kMaxFuncs];
+    // scratch of cfs_render_host (device), cached
+    void *d_image = nullptr; size_t image_bytes = 0;
+    void *d_cloud = nullptr; size_t cloud_bytes = 0;
+    unsigned long long *d_counters = nullptr;
+};
+
+namespace {
+
+bool bad_float(float v) { return std::isnan(v) || std::isinf(v); }
+
+uint32_t pack_rgba8(const float *c)
+{
+    uint32_t out = 0;
+    for (int i = 0; i < 4; ++i) {
+        float v = floorf(c[i] + 0.5f);
+        if (!(v >= 0.0f)) v = 0.0f;
+        if (v > 255.0f) v = 255.0f;
+        out |= (uint32_t)v << (8 * i);
+    }
+    return out;
+}
+
+// thresholds, bucket table and the affine table form
+cfs_status build_tables(cfs_system *s)
+{
+    const int n = (int)s->funcs.size();
+    double total = 0.0;
+    for (int j = 0; j < n; ++j) {
+        const float p = s->funcs[j].prob;
+        if (!(p >= 0.0f) || std::isinf(p)) return fail(CFS_ERR_INVALID_ARG, "funcs[%d].prob must be finite and >= 0", j);
+        total += (double)p;
+    }
+    if (!(total > 0.0)) return fail(CFS_ERR_INVALID_ARG, "sum of probabilities must be > 0");
+    uint64_t T64[cfs::kMaxFuncs];
+    double c = 0.0;
+    for (int j = 0; j < n; ++j) {
+        c += (double)s->funcs[j].prob;
+        T64[j] = (uint64_t)floor(c / total * 4294967296.0);
+    }
+    s->n_thr = 0;
+    for (int j = 0; j < n - 1; ++j)
+        if (T64[j] < 4294967296ull) s->n_thr = j + 1;          // T is non-decreasing
+    for (int j = 0; j < cfs::kMaxFuncs; ++j) s->T[j] = (j < s->n_thr) ? (uint32_t)T64[j] : 0xFFFFFFFFu;
+    s->pick_steps = 0;
+    for (int b = 0; b < 256; ++b) {
+        const uint64_t lo = (uint64_t)b << 24, hi = lo + 0xFFFFFFull;
+        int below = 0, inside = 0;
+        for (int j = 0; j < s->n_thr; ++j) {
+            if (T64[j] <= lo) ++below;
+            else if (T64[j] <= hi) ++inside;
+        }
+        s->lut[b] = (uint8_t)below;
+        if (inside > s->pick_steps) s->pick_steps = inside;
+    }
+    // equal power-of-two thresholds: k = u >> shift
+    s->pick_shift = -1;
+    if (n >= 1 && (n & (n - 1)) == 0 && s->n_thr == n - 1) {
+        int lg = 0;
+        while ((1 << lg) < n) ++lg;
+        bool ok = true;
+        for (int j = 0; j < n - 1; ++j) ok = ok && (T64[j] == ((uint64_t)(j + 1) << (32 - lg)));
+        if (ok && lg >= 1) s->pick_shift = 32 - lg;
+        if (n == 1) { s->pick_shift = -1; }
+    }
+    // affine form: DIAG when every off-diagonal coefficient is exactly zero
+    bool diag = true;
+    for (int j = 0; j < n; ++j) {
+        const float *m = s->funcs[j].params;
+        if (s->dim == 2) diag = diag && m[1] == 0.0f && m[2] == 0.0f;
+        else diag = diag && m[1] == 0.0f && m[2] == 0.0f && m[3] == 0.0f && m[5] == 0.0f && m[6] == 0.0f && m[7] == 0.0f;
+    }
+    s->aff = diag ? cfs::AFF_DIAG : cfs::AFF_GENERAL;
+    memset(s->coef, 0, sizeof(s->coef));
+    for (int j = 0; j < n; ++j) {
+        const float *m = s->funcs[j].params;
+        if (s->dim == 2 && diag) {
+            float *r = s->coef + 4 * j;  r[0] = m[0]; r[1] = m[3]; r[2] = m[4]; r[3] = m[5];
+        } else if (s->dim == 2) {
+            float *r = s->coef + 8 * j;  r[0] = m[0]; r[1] = m[1]; r[2] = m[4]; r[4] = m[2]; r[5] = m[3]; r[6] = m[5];
+        } else if (diag) {
+            float *r = s->coef + 8 * j;  r[0] = m[0]; r[1] = m[4]; r[2] = m[8]; r[4] = m[9]; r[5] = m[10]; r[6] = m[11];
+        } else {
+            float *r = s->coef + 12 * j;
+            for (int row = 0; row < 3; ++row) {
+                r[4 * row + 0] = m[3 * row + 0]; r[4 * row + 1] = m[3 * row + 1];
+                r[4 * row + 2] = m[3 * row + 2]; r[4 * row + 3] = m[9 + row];
+            }
+        }
+    }
+    return CFS_OK;
+}
+
+}  // namespace
+
+extern "C" cfs_status cfs_create(cfs_system **out, int32_t dim, int32_t gen_kind, const cfs_func *funcs,
+                                 int32_t n_funcs, const cfs_xform *chain, int32_t n_chain,
+                                 int32_t color_rule, const float *palette_rgba, int32_t reuse)
+{
+    if (!out) return fail(CFS_ERR_INVALID_ARG, "out is NULL");
+    *out = nullptr;
+    if (dim != 2 && dim != 3) return fail(CFS_ERR_INVALID_ARG, "dim must be 2 or 3");
+    if (gen_kind != CFS_GEN_IFS && gen_kind != CFS_GEN_CLOUD) return fail(CFS_ERR_INVALID_ARG, "unknown generator kind %d", gen_kind);
+    if (n_chain < 0 || n_chain > CFS_MAX_CHAIN || (n_chain > 0 && !chain)) return fail(CFS_ERR_INVALID_ARG, "n_chain must be 0..%d", CFS_MAX_CHAIN);
+    if (color_rule < CFS_COLOR_NONE || color_rule > CFS_COLOR_POINT) return fail(CFS_ERR_INVALID_ARG, "unknown colour rule %d", color_rule);
+    cfs_system *s = new (std::nothrow) cfs_system();
+    if (!s) return fail(CFS_ERR_NOMEM, "out of host memory");
+    s->dim = dim; s->gen = gen_kind; s->color = color_rule; s->reuse = reuse ? 1 : 0;
+    cfs_status st = CFS_OK;
+    if (gen_kind == CFS_GEN_IFS) {
+        if (n_funcs < 1 || n_funcs > CFS_MAX_FUNCS || !funcs) st = fail(CFS_ERR_INVALID_ARG, "n_funcs must be 1..%d", CFS_MAX_FUNCS);
+        if (st == CFS_OK && color_rule == CFS_COLOR_POINT) st = fail(CFS_ERR_INVALID_ARG, "COLOR_POINT needs a CLOUD generator");
+        if (st == CFS_OK && color_rule == CFS_COLOR_MAP_INDEX && !palette_rgba) st = fail(CFS_ERR_INVALID_ARG, "COLOR_MAP_INDEX needs a palette");
+        for (int j = 0; st == CFS_OK && j < n_funcs; ++j) {
+            if (funcs[j].type != CFS_F_AFFINE) st = fail(CFS_ERR_INVALID_ARG, "funcs[%d]: unknown type %d", j, funcs[j].type);
+            const int np = (dim == 2) ? 6 : 12;
+            for (int i = 0; st == CFS_OK && i < np; ++i)
+                if (bad_float(funcs[j].params[i])) st = fail(CFS_ERR_INVALID_ARG, "funcs[%d].params[%d] is not finite", j, i);
+        }
+        if (st == CFS_OK) {
+            s->funcs.assign(funcs, funcs + n_funcs);
+            st = build_tables(s);
+        }
+        if (st == CFS_OK && color_rule == CFS_COLOR_MAP_INDEX) {
+            s->palette.assign(palette_rgba, palette_rgba + 4 * n_funcs);
+            for (int j = 0; j < n_funcs; ++j) s->pal8[j] = pack_rgba8(palette_rgba + 4 * j);
+        }
+    } else {
+        if (color_rule == CFS_COLOR_MAP_INDEX) st = fail(CFS_ERR_INVALID_ARG, "COLOR_MAP_INDEX needs an IFS generator");
+    }
+    for (int m = 0; st == CFS_OK && m < n_chain; ++m) {
+        if (chain[m].type < CFS_T_AFFINE || chain[m].type > CFS_T_STRETCH_COS) st = fail(CFS_ERR_INVALID_ARG, "chain[%d]: unknown type %d", m, chain[m].type);
+        for (int i = 0; st == CFS_OK && i < 12; ++i)
+            if (bad_float(chain[m].p0[i]) || bad_float(chain[m].p1[i])) st = fail(CFS_ERR_INVALID_ARG, "chain[%d] parameter %d is not finite", m, i);
+    }
+    if (st != CFS_OK) { delete s; return st; }
+    if (n_chain) s->chain.assign(chain, chain + n_chain);
+    *out = s;
+    return CFS_OK;
+}
+
+extern "C" void cfs_destroy(cfs_system *s)
+{
+    if (!s) return;
+    if (s->d_image) cudaFree(s->d_image);
+    if (s->d_cloud) cudaFree(s->d_cloud);
+    if (s->d_counters) cudaFree(s->d_counters);
+    delete s;
+}
+
+// -------------------------------------------------------------------------------------------------
+namespace {
+
+using cfs::RenderParams;
+
+// per-render host resolution: validation, chain parameters at t, pixel map, round keys
+cfs_status build_params(const cfs_system *s, const cfs_render_args *a, RenderParams *out, bool need_image)
+{
+    if (!s || !a) return fail(CFS_ERR_INVALID_ARG, "system or args is NULL");
+    if (a->reserved_ != 0) return fail(CFS_ERR_INVALID_ARG, "reserved_ must be 0");
+    if (a->iterations < 1) return fail(CFS_ERR_INVALID_ARG, "iterations must be >= 1");
+    if (a->burn_in < 0 || a->burn_in >= a->iterations) return fail(CFS_ERR_INVALID_ARG, "burn_in must be in [0, iterations)");
+    if (s->gen == CFS_GEN_CLOUD && (a->iterations != 1 || a->burn_in != 0)) return fail(CFS_ERR_INVALID_ARG, "CLOUD generator needs iterations = 1, burn_in = 0");
+    if (a->width < 1 || a->height < 1 || (int64_t)a->width * a->height > 2147483647ll) return fail(CFS_ERR_INVALID_ARG, "bad image size %d x %d", a->width, a->height);
+    if (bad_float(a->xmin) || bad_float(a->xmax) || bad_float(a->ymin) || bad_float(a->ymax) || !(a->xmax > a->xmin) || !(a->ymax > a->ymin))
+        return fail(CFS_ERR_INVALID_ARG, "bounds must be finite with max > min");
+    if (bad_float(a->t)) return fail(CFS_ERR_INVALID_ARG, "t is not finite");
+    if (a->out_mode < CFS_OUT_HIST_U32 || a->out_mode > CFS_OUT_DEPTH_RGBA8_U64) return fail(CFS_ERR_INVALID_ARG, "unknown out_mode %d", a->out_mode);
+    if (a->out_mode == CFS_OUT_RGBA_F32 && s->color == CFS_COLOR_NONE) return fail(CFS_ERR_INVALID_ARG, "RGBA output needs a colour rule");
+    if (a->out_mode == CFS_OUT_DEPTH_RGBA8_U64) {
+        if (s->color == CFS_COLOR_NONE || s->dim != 3) return fail(CFS_ERR_INVALID_ARG, "DEPTH output needs dim 3 and a colour rule");
+        if (s->chain.empty() || s->chain.back().type != CFS_T_PINHOLE) return fail(CFS_ERR_INVALID_ARG, "DEPTH output needs a chain ending in PINHOLE");
+    }
+    if (need_image && a->n_points && !a->d_image) return fail(CFS_ERR_INVALID_ARG, "d_image is NULL");
+    if (a->n_points && s->gen == CFS_GEN_CLOUD && !a->d_cloud) return fail(CFS_ERR_INVALID_ARG, "d_cloud is NULL");
+    if (a->out_mode == CFS_OUT_RGBA_F32 && ((uintptr_t)a->d_image & 15)) return fail(CFS_ERR_INVALID_ARG, "RGBA image must be 16-byte aligned");
+    if (a->out_mode == CFS_OUT_DEPTH_RGBA8_U64 && ((uintptr_t)a->d_image & 7)) return fail(CFS_ERR_INVALID_ARG, "DEPTH image must be 8-byte aligned");
+    if (s->gen == CFS_GEN_CLOUD && ((uintptr_t)a->d_cloud & 15)) return fail(CFS_ERR_INVALID_ARG, "cloud must be 16-byte aligned");
+
+    RenderParams &p = *out;
+    memset(&p, 0, sizeof(p));
+    p.n_points = a->n_points; p.point_offset = a->point_offset;
+    uint32_t k0 = (uint32_t)(a->seed & 0xFFFFFFFFu), k1 = (uint32_t)(a->seed >> 32);
+    for (int r = 0; r < 10; ++r) { p.rk[r][0] = k0; p.rk[r][1] = k1; k0 += 0x9E3779B9u; k1 += 0xBB67AE85u; }
+    p.iterations = a->iterations; p.burn_in = a->burn_in;
+    p.W = a->width; p.H = a->height;
+    p.xmin = a->xmin; p.xmax = a->xmax; p.ymin = a->ymin; p.ymax = a->ymax;
+    const double wx = (double)a->xmax - (double)a->xmin, wy = (double)a->ymax - (double)a->ymin;
+    p.sx = (float)((double)a->width / wx);  p.ox = (float)(-(double)a->xmin * (double)a->width / wx);
+    p.sy = (float)((double)a->height / wy); p.oy = (float)(-(double)a->ymin * (double)a->height / wy);
+    p.image = a->d_image; p.cloud = a->d_cloud; p.counters = (unsigned long long *)a->d_counters;
+    p.dim = s->dim; p.n_funcs = (int)s->funcs.size(); p.n_chain = (int)s->chain.size();
+    p.color_rule = s->color; p.reuse = s->reuse;
+    p.pick_shift = s->pick_shift; p.n_thr = s->n_thr; p.pick_steps = s->pick_steps;
+    memcpy(p.T, s->T, sizeof(p.T)); memcpy(p.lut, s->lut, sizeof(p.lut));
+    memcpy(p.coef, s->coef, sizeof(p.coef)); memcpy(p.pal8, s->pal8, sizeof(p.pal8));
+    if (!s->palette.empty()) memcpy(p.palette, s->palette.data(), s->palette.size() * sizeof(float));
+
+    // chain parameters at t: (float)((double)p0 + (double)t*(double)p1)
+    const double t = (double)a->t;
+    for (int m = 0; m < p.n_chain; ++m) {
+        const cfs_xform &x = s->chain[m];
+        cfs::ChainStep &st = p.chain[m];
+        st.type = x.type;
+        auto res = [&](int i) { return (float)((double)x.p0[i] + t * (double)x.p1[i]); };
+        switch (x.type) {
+        case CFS_T_AFFINE:
+            for (int i = 0; i < 12; ++i) st.p[i] = res(i);
+            break;
+        case CFS_T_ROTATE_Z: {   // resolved once per render to an AFFINE rotation (DESIGN R5)
+            const double th = (double)x.p0[0] + t * (double)x.p1[0];
+            const float c = (float)cos(th), sn = (float)sin(th);
+            st.type = CFS_T_AFFINE;
+            if (s->dim == 2) { st.p[0] = c; st.p[1] = -sn; st.p[2] = sn; st.p[3] = c; }
+            else { st.p[0] = c; st.p[1] = -sn; st.p[3] = sn; st.p[4] = c; st.p[8] = 1.0f; }
+            break;
+        }
+        case CFS_T_TWIST_Z:
+        case CFS_T_BEND:
+            st.p[0] = res(0);
+            break;
+        case CFS_T_PINHOLE: {
+            const double fov = (double)x.p0[0] + t * (double)x.p1[0];
+            const double f = 1.0 / tan(fov * (3.14159265358979323846 / 180.0) * 0.5);
+            st.p[0] = (float)(f * (double)a->height / (double)a->width);
+            st.p[1] = (float)f;
+            st.p[2] = res(1);
+            st.p[3] = res(2);
+            break;
+        }
+        default:
+            break;
+        }
+    }
+    return CFS_OK;
+}
+
+typedef void (*render_fn)(const RenderParams);
+
+template <int DIM, int GEN, int AFF>
+render_fn pick_splat(int splat)
+{
+    switch (splat) {
+    case cfs::SPLAT_HIST_DIRECT: return cfs::render_kernel<DIM, GEN, AFF, cfs::SPLAT_HIST_DIRECT>;
+    case cfs::SPLAT_HIST_SHARED: return cfs::render_kernel<DIM, GEN, AFF, cfs::SPLAT_HIST_SHARED>;
+    case cfs::SPLAT_HIST_WARPAGG: return cfs::render_kernel<DIM, GEN, AFF, cfs::SPLAT_HIST_WARPAGG>;
+    case cfs::SPLAT_RGBA: return cfs::render_kernel<DIM, GEN, AFF, cfs::SPLAT_RGBA>;
+    case cfs::SPLAT_DEPTH:
+        if (DIM == 3) return cfs::render_kernel<3, GEN, AFF, cfs::SPLAT_DEPTH>;
+        return nullptr;
+    default: return nullptr;
+    }
+}
+
+render_fn pick_kernel(int dim, int gen, int aff, int splat)
+{
+    if (gen == CFS_GEN_CLOUD) return dim == 2 ? pick_splat<2, 1, cfs::AFF_GENERAL>(splat) : pick_splat<3, 1, cfs::AFF_GENERAL>(splat);
+    if (dim == 2) return aff == cfs::AFF_DIAG ? pick_splat<2, 0, cfs::AFF_DIAG>(splat) : pick_splat<2, 0, cfs::AFF_GENERAL>(splat);
+    return aff == cfs::AFF_DIAG ? pick_splat<3, 0, cfs::AFF_DIAG>(splat) : pick_splat<3, 0, cfs::AFF_GENERAL>(splat);
+}
+
+render_fn pick_trace(int dim, int gen, int aff)
+{
+    if (gen == CFS_GEN_CLOUD) return dim == 2 ? cfs::trace_kernel<2, 1, cfs::AFF_GENERAL> : cfs::trace_kernel<3, 1, cfs::AFF_GENERAL>;
+    if (dim == 2) return aff == cfs::AFF_DIAG ? cfs::trace_kernel<2, 0, cfs::AFF_DIAG> : cfs::trace_kernel<2, 0, cfs::AFF_GENERAL>;
+    return aff == cfs::AFF_DIAG ? cfs::trace_kernel<3, 0, cfs::AFF_DIAG> : cfs::trace_kernel<3, 0, cfs::AFF_GENERAL>;
+}
+
+size_t shared_hist_limit(const DeviceInfo &di)
+{
+    const long lim = (long)di.smem_optin - (long)sizeof(cfs::SharedTables) - 1024;
+    return lim > 0 ? (size_t)lim : 0;
+}
+
+}  // namespace
+
+extern "C" uint64_t cfs_shared_hist_max_bytes(void)
+{
+    const DeviceInfo &di = device_info();
+    return di.ok == 1 ? shared_hist_limit(di) : 0;
+}
+
+extern "C" cfs_status cfs_render(const cfs_system *s, const cfs_render_args *a, void *stream)
+{
+    RenderParams p;
+    cfs_status st = build_params(s, a, &p, true);
+    if (st != CFS_OK) return st;
+    if (a->variant < CFS_VARIANT_AUTO || a->variant > CFS_VARIANT_WARP_AGG) return fail(CFS_ERR_INVALID_ARG, "unknown variant %d", a->variant);
+    const DeviceInfo &di = device_info();
+    if (di.ok != 1) return fail(CFS_ERR_CUDA, "no CUDA device (this library has no CPU fallback)");
+    const size_t hist_bytes = (size_t)a->width * a->height * 4;
+    int splat;
+    if (a->out_mode == CFS_OUT_RGBA_F32) splat = cfs::SPLAT_RGBA;
+    else if (a->out_mode == CFS_OUT_DEPTH_RGBA8_U64) splat = cfs::SPLAT_DEPTH;
+    else splat = cfs::SPLAT_HIST_DIRECT;
+    if (a->variant == CFS_VARIANT_SHARED_HIST || a->variant == CFS_VARIANT_WARP_AGG) {
+        if (a->out_mode != CFS_OUT_HIST_U32) return fail(CFS_ERR_UNSUPPORTED, "variant %d is for HIST_U32 output only", a->variant);
+        if (a->variant == CFS_VARIANT_SHARED_HIST && hist_bytes > shared_hist_limit(di))
+            return fail(CFS_ERR_UNSUPPORTED, "image of %zu bytes does not fit the per-CTA shared histogram (%zu)", hist_bytes, shared_hist_limit(di));
+        splat = (a->variant == CFS_VARIANT_SHARED_HIST) ? cfs::SPLAT_HIST_SHARED : cfs::SPLAT_HIST_WARPAGG;
+    } else if (a->variant == CFS_VARIANT_AUTO && a->out_mode == CFS_OUT_HIST_U32) {
+        // chosen by image size (DESIGN "splat variants"): small histograms are privatised per CTA
+        if (hist_bytes <= shared_hist_limit(di) && a->n_points * (uint64_t)(a->iterations - a->burn_in) >= (uint64_t)di.sms * (hist_bytes / 4))
+            splat = cfs::SPLAT_HIST_SHARED;
+    }
+    if (a->n_points == 0) return CFS_OK;
+    render_fn fn = pick_kernel(s->dim, s->gen, s->aff, splat);
+    if (!fn) return fail(CFS_ERR_UNSUPPORTED, "no kernel for dim %d / splat %d", s->dim, splat);
+
+    const int threads = cfs::kRenderThreads;
+    uint64_t blocks = (a->n_points + threads - 1) / threads;
+    size_t dyn = 0;
+    if (splat == cfs::SPLAT_HIST_SHARED) {
+        dyn = hist_bytes;
+        p.hist_bins = (uint32_t)(hist_bytes / 4);
+        cudaError_t e = cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
+        if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute");
+    }
+    // CLOUD and SHARED_HIST: persistent grid (resident CTAs x SMs), grid-stride over points: one
+    // histogram merge per CTA, short per-point work amortises the CTA prologue.  IFS + direct
+    // splats: one point per thread, CTAs handed out by the hardware scheduler -- measured faster
+    // than a persistent grid (P / resident threads is ~3.5 for configs[1]: the last static trip
+    // would run 46 % full; dynamic CTA hand-out has no such tail).
+    if (s->gen == CFS_GEN_CLOUD || splat == cfs::SPLAT_HIST_SHARED) {
+        int per_sm = 1;
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void *)fn, threads, dyn);
+        if (per_sm < 1) per_sm = 1;
+        const uint64_t cap = (uint64_t)di.sms * per_sm;
+        if (blocks > cap) blocks = cap;
+    } else if (blocks > (1u << 24)) {
+        blocks = 1u << 24;
+    }
+    fn<<<(unsigned)blocks, threads, dyn, (cudaStream_t)stream>>>(p);
+    ++g_launches;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "render kernel launch");
+    return CFS_OK;
+}
+
+extern "C" cfs_status cfs_trace(const cfs_system *s, const cfs_render_args *a, uint8_t *d_picks, float *d_final_g,
+                                float *d_final_q, uint8_t *d_alive, void *stream)
+{
+    RenderParams p;
+    cfs_status st = build_params(s, a, &p, false);
+    if (st != CFS_OK) return st;
+    if (device_info().ok != 1) return fail(CFS_ERR_CUDA, "no CUDA device (this library has no CPU fallback)");
+    if (a->n_points == 0) return CFS_OK;
+    p.tr_picks = d_picks; p.tr_g = d_final_g; p.tr_q = d_final_q; p.tr_alive = d_alive;
+    p.counters = nullptr;
+    render_fn fn = pick_trace(s->dim, s->gen, s->aff);
+    uint64_t blocks = (a->n_points + cfs::kRenderThreads - 1) / cfs::kRenderThreads;
+    if (blocks > (1u << 22)) blocks = 1u << 22;
+    fn<<<(unsigned)blocks, cfs::kRenderThreads, 0, (cudaStream_t)stream>>>(p);
+    ++g_launches;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "trace kernel launch");
+    return CFS_OK;
+}
+
+// -------------------------------------------------------------------------------------------------
+extern "C" cfs_status cfs_render_host(cfs_system *s, const cfs_render_args *a, void *h_image,
+                                      const cfs_cloud_rec *h_cloud, uint64_t *h_counters, void *stream)
+{
+    if (!s || !a) return fail(CFS_ERR_INVALID_ARG, "system or args is NULL");
+    if (!h_image) return fail(CFS_ERR_INVALID_ARG, "h_image is NULL");
+    if (a->width < 1 || a->height < 1 || (int64_t)a->width * a->height > 2147483647ll) return fail(CFS_ERR_INVALID_ARG, "bad image size");
+    if (a->out_mode < CFS_OUT_HIST_U32 || a->out_mode > CFS_OUT_DEPTH_RGBA8_U64) return fail(CFS_ERR_INVALID_ARG, "unknown out_mode %d", a->out_mode);
+    if (device_info().ok != 1) return fail(CFS_ERR_CUDA, "no CUDA device (this library has no CPU fallback)");
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t px = (size_t)a->width * a->height;
+    const size_t bytes = px * (a->out_mode == CFS_OUT_HIST_U32 ? 4 : a->out_mode == CFS_OUT_RGBA_F32 ? 16 : 8);
+    cudaError_t e;
+    if (s->image_bytes < bytes) {
+        if (s->d_image) cudaFree(s->d_image);
+        s->d_image = nullptr; s->image_bytes = 0;
+        if ((e = cudaMalloc(&s->d_image, bytes)) != cudaSuccess) return cuda_fail(e, "cudaMalloc(image)");
+        s->image_bytes = bytes;
+    }
+    if (!s->d_counters && (e = cudaMalloc((void **)&s->d_counters, 16)) != cudaSuccess) return cuda_fail(e, "cudaMalloc(counters)");
+    cfs_render_args r = *a;
+    r.d_image = s->d_image; r.d_counters = (uint64_t *)s->d_counters; r.d_cloud = nullptr;
+    if (s->gen == CFS_GEN_CLOUD && a->n_points) {
+        if (!h_cloud) return fail(CFS_ERR_INVALID_ARG, "h_cloud is NULL");
+        // only the rendered record range travels; the kernel indexes the WHOLE cloud by p
+        const size_t cb = (size_t)a->n_points * sizeof(cfs_cloud_rec);
+        if (s->cloud_bytes < cb) {
+            if (s->d_cloud) cudaFree(s->d_cloud);
+            s->d_cloud = nullptr; s->cloud_bytes = 0;
+            if ((e = cudaMalloc(&s->d_cloud, cb)) != cudaSuccess) return cuda_fail(e, "cudaMalloc(cloud)");
+            s->cloud_bytes = cb;
+        }
+        if ((e = cudaMemcpyAsync(s->d_cloud, h_cloud + a->point_offset, cb, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(e, "H2D cloud");
+        r.d_cloud = (const cfs_cloud_rec *)s->d_cloud - a->point_offset;
+    }
+    if ((e = cudaMemsetAsync(s->d_image, a->out_mode == CFS_OUT_DEPTH_RGBA8_U64 ? 0xFF : 0, bytes, st)) != cudaSuccess) return cuda_fail(e, "clear image");
+    if ((e = cudaMemsetAsync(s->d_counters, 0, 16, st)) != cudaSuccess) return cuda_fail(e, "clear counters");
+    cfs_status rs = cfs_render(s, &r, stream);
+    if (rs != CFS_OK) return rs;
+    if ((e = cudaMemcpyAsync(h_image, s->d_image, bytes, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(e, "D2H image");
+    if (h_counters && (e = cudaMemcpyAsync(h_counters, s->d_counters, 16, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(e, "D2H counters");
+    if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(e, "stream synchronize");
+    return CFS_OK;
+}
+
+extern "C" cfs_status cfs_tonemap(const void *d_image, int32_t out_mode, int32_t width, int32_t height, float gamma,
+                                  float colour_scale, uint32_t *d_out, void *d_scratch, void *stream)
+{
+    if (!d_image || !d_out) return fail(CFS_ERR_INVALID_ARG, "image or output is NULL");
+    if (width < 1 || height < 1 || (int64_t)width * height > 2147483647ll) return fail(CFS_ERR_INVALID_ARG, "bad image size");
+    if (out_mode < CFS_OUT_HIST_U32 || out_mode > CFS_OUT_DEPTH_RGBA8_U64) return fail(CFS_ERR_INVALID_ARG, "unknown out_mode %d", out_mode);
+    const DeviceInfo &di = device_info();
+    if (di.ok != 1) return fail(CFS_ERR_CUDA, "no CUDA device (this library has no CPU fallback)");
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t n = (size_t)width * height;
+    const int threads = cfs::kToneThreads;
+    size_t want = (n + threads - 1) / threads;
+    const unsigned grid_map = (unsigned)(want < (size_t)di.sms * 32 ? want : (size_t)di.sms * 32);
+    if (out_mode == CFS_OUT_DEPTH_RGBA8_U64) {
+        cfs::tone_depth_kernel<<<grid_map, threads, 0, st>>>((const unsigned long long *)d_image, n, d_out);
+        ++g_launches;
+    } else {
+        if (!(gamma > 0.0f) || bad_float(gamma) || bad_float(colour_scale)) return fail(CFS_ERR_INVALID_ARG, "gamma must be > 0 and finite");
+        if (!d_scratch) return fail(CFS_ERR_INVALID_ARG, "d_scratch is NULL");
+        if (out_mode == CFS_OUT_HIST_U32 && ((uintptr_t)d_image & 15)) return fail(CFS_ERR_INVALID_ARG, "HIST image must be 16-byte aligned for the tone map");
+        cudaError_t e = cudaMemsetAsync(d_scratch, 0, 8, st);
+        if (e != cudaSuccess) return cuda_fail(e, "clear scratch");
+        const unsigned grid_max = (unsigned)(want < (size_t)di.sms * 8 ? want : (size_t)di.sms * 8);
+        const float inv_gamma = 1.0f / gamma;
+        if (out_mode == CFS_OUT_HIST_U32) {
+            cfs::tone_max_kernel<0><<<grid_max, threads, 0, st>>>(d_image, n, (uint32_t *)d_scratch);
+            cfs::tone_map_kernel<0><<<grid_map, threads, 0, st>>>(d_image, n, (const uint32_t *)d_scratch, inv_gamma, colour_scale, d_out);
+        } else {
+            cfs::tone_max_kernel<1><<<grid_max, threads, 0, st>>>(d_image, n, (uint32_t *)d_scratch);
+            cfs::tone_map_kernel<1><<<grid_map, threads, 0, st>>>(d_image, n, (const uint32_t *)d_scratch, inv_gamma, colour_scale, d_out);
+        }
+        g_launches += 2;
+    }
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "tonemap kernel launch");
+    return CFS_OK;
+}
+
+extern "C" cfs_status cfs_microbench(int32_t kind, void *d_buf, uint64_t footprint, uint64_t ops, int32_t blocks,
+                                     int32_t threads, void *stream)
+{
+    if (!d_buf || blocks < 1 || threads < 32 || threads > 1024 || (threads & 31)) return fail(CFS_ERR_INVALID_ARG, "bad microbench launch shape");
+    const DeviceInfo &di = device_info();
+    if (di.ok != 1) return fail(CFS_ERR_CUDA, "no CUDA device (this library has no CPU fallback)");
+    cudaStream_t st = (cudaStream_t)stream;
+    auto bins = [&](size_t elem) -> uint32_t { const uint64_t b = footprint / elem; return (uint32_t)(b > 0xFFFFFFFFull ? 0xFFFFFFFFull : b); };
+    switch (kind) {
+    case CFS_MB_RED_ADD_U32:   if (!bins(4)) return fail(CFS_ERR_INVALID_ARG, "footprint too small");  cfs::mb_mem_kernel<0><<<blocks, threads, 0, st>>>(d_buf, bins(4), ops); break;
+    case CFS_MB_RED_ADD_V4F32: if (!bins(16)) return fail(CFS_ERR_INVALID_ARG, "footprint too small"); cfs::mb_mem_kernel<1><<<blocks, threads, 0, st>>>(d_buf, bins(16), ops); break;
+    case CFS_MB_ATOM_MIN_U64:  if (!bins(8)) return fail(CFS_ERR_INVALID_ARG, "footprint too small");  cfs::mb_mem_kernel<2><<<blocks, threads, 0, st>>>(d_buf, bins(8), ops); break;
+    case CFS_MB_LD_U64:        if (!bins(8)) return fail(CFS_ERR_INVALID_ARG, "footprint too small");  cfs::mb_mem_kernel<3><<<blocks, threads, 0, st>>>(d_buf, bins(8), ops); break;
+    case CFS_MB_ATOMS_ADD_U32: {
+        if (footprint < 4 || footprint > (uint64_t)di.smem_optin) return fail(CFS_ERR_INVALID_ARG, "shared footprint must be 4..%d bytes", di.smem_optin);
+        cudaError_t e = cudaFuncSetAttribute((const void *)cfs::mb_atoms_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)footprint);
+        if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute");
+        cfs::mb_atoms_kernel<<<blocks, threads, footprint, st>>>(d_buf, (uint32_t)(footprint / 4), ops);
+        break;
+    }
+    case CFS_MB_FFMA:      cfs::mb_alu_kernel<5><<<blocks, threads, 0, st>>>(d_buf, ops); break;
+    case CFS_MB_IMAD_WIDE: cfs::mb_alu_kernel<6><<<blocks, threads, 0, st>>>(d_buf, ops); break;
+    case CFS_MB_LOP3:      cfs::mb_alu_kernel<7><<<blocks, threads, 0, st>>>(d_buf, ops); break;
+    case CFS_MB_MUFU:      cfs::mb_alu_kernel<8><<<blocks, threads, 0, st>>>(d_buf, ops); break;
+    case CFS_MB_STREAM_LD128: cfs::mb_stream_kernel<<<blocks, threads, 0, st>>>(d_buf, footprint / 16); break;
+    default: return fail(CFS_ERR_INVALID_ARG, "unknown microbench kind %d", kind);
+    }
+    ++g_launches;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "microbench launch");
+    return CFS_OK;
+}
+
+extern "C" uint64_t cfs_launch_count(int32_t reset)
+{
+    const uint64_t v = g_launches;
+    if (reset) g_launches = 0;
+    return v;
+}
+
+extern "C" const char *cfs_last_error(void) { return g_err; }
+extern "C" const char *cfs_version(void) { return "cfs-b200 0.1 (sm_100a)"; }

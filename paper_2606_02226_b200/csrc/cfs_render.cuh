@@ -1,0 +1,202 @@
+// cfs_render.cuh -- the fused sampler + pick + map + chain + colour + splat kernel (sm_100a).
+//
+// One thread owns one point at a time ("a single point chooses a single function at
+// random every step"); the per-thread state is 3 floats of generator state, 3 of the copy and 4
+// Philox words ("less than ten floating-point values stored per thread").
+// Nothing but the output image is written to global memory.
+#pragma once
+#include "cfs_device.cuh"
+
+namespace cfs {
+
+constexpr int kRenderThreads = 256;
+
+// ---------------------------------------------------------------------------------------------
+// splat sinks (row 7).  Each returns nothing; `pix >= 0` is guaranteed by the caller.
+__device__ __forceinline__ void red_add_v4_f32(float *addr, float a, float b, float c, float d)
+{
+    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};"
+                 :: "l"(addr), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
+}
+
+__device__ __forceinline__ void red_add_u32(uint32_t *addr, uint32_t v)
+{
+    asm volatile("red.global.add.u32 [%0], %1;" :: "l"(addr), "r"(v) : "memory");
+}
+
+__device__ __forceinline__ void splat_hist_warpagg(uint32_t *hist, int pix, bool valid)
+{
+    // ballot/match aggregation of same-pixel hits before the atomic (BASELINE north_star).
+    const unsigned act = __ballot_sync(0xFFFFFFFFu, valid);
+    if (!valid) return;
+    const unsigned peers = __match_any_sync(act, pix);
+    const int leader = __ffs(peers) - 1;
+    if ((int)(threadIdx.x & 31) == leader) red_add_u32(hist + pix, (uint32_t)__popc(peers));
+}
+
+__device__ __forceinline__ void splat_depth(unsigned long long *buf, int pix, float depth, uint32_t rgba8)
+{
+    // key = bits(d) << 32 | rgba8; d > 0 so unsigned order = float order (DESIGN R8).
+    const unsigned long long key = ((unsigned long long)__float_as_uint(depth) << 32) | rgba8;
+    // The buffer only ever decreases, so a stale read can cause a redundant atomic but never a
+    // wrong skip; most splats of a solid are occluded and stop at this load.
+    const unsigned long long cur = __ldcg(buf + pix);
+    if (key < cur) atomicMin(buf + pix, key);
+}
+
+// ---------------------------------------------------------------------------------------------
+// the kernel
+template <int DIM, int GEN, int AFF, int SPLAT>
+__global__ void __launch_bounds__(kRenderThreads)
+render_kernel(const __grid_constant__ RenderParams prm)
+{
+    __shared__ SharedTables s;
+    extern __shared__ __align__(16) uint32_t s_hist[];   // SPLAT_HIST_SHARED only
+    if (GEN == 0) load_tables(s, prm);
+    if (SPLAT == SPLAT_HIST_SHARED)
+        for (uint32_t i = threadIdx.x; i < prm.hist_bins; i += blockDim.x) s_hist[i] = 0u;
+    __syncthreads();
+
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    uint32_t n_in = 0, n_drop = 0;
+
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; ; i += stride) {
+        // SPLAT_HIST_WARPAGG uses full-warp collectives inside: keep whole warps in the loop
+        const bool have = i < prm.n_points;
+        if (SPLAT == SPLAT_HIST_WARPAGG) { if (!__any_sync(0xFFFFFFFFu, have)) break; }
+        else if (!have) break;
+        const uint64_t p = prm.point_offset + i;
+        float gx, gy, gz = 0.0f;
+        uint32_t point_rgba8 = 0;
+
+        if (GEN == 1) {   // stored cloud: one coalesced 128-bit load per point (row 1)
+            float4 rec = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (have) rec = __ldcs(reinterpret_cast<const float4 *>(prm.cloud) + p);
+            gx = rec.x; gy = rec.y; gz = (DIM == 3) ? rec.z : 0.0f;
+            point_rgba8 = __float_as_uint(rec.w);
+        } else {
+            const U4 w = philox4x32_10((uint32_t)p, (uint32_t)(p >> 32), 0u, DOMAIN_INIT, prm);
+            gx = u24_to_pm1(w.x);
+            gy = u24_to_pm1(w.y);
+            if (DIM == 3) gz = u24_to_pm1(w.z);
+        }
+
+        U4 w = {0, 0, 0, 0};
+        for (int it = 0; it < prm.iterations; ++it) {
+            int k = 0;
+            if (GEN == 0) {
+                if ((it & 3) == 0)
+                    w = philox4x32_10((uint32_t)p, (uint32_t)(p >> 32), (uint32_t)it >> 2, DOMAIN_PICK, prm);
+                const uint32_t u = w.x;
+                w.x = w.y; w.y = w.z; w.z = w.w;        // word it&3 rotates into .x
+                k = pick_index(u, s, prm);
+                apply_gen<DIM, AFF>(k, s, gx, gy, gz);
+            }
+            if (it < prm.burn_in && !prm.reuse) continue;
+            float qx = gx, qy = gy, qz = gz;            // the copy of Fig. 2(B)
+            const bool alive = apply_chain<DIM>(prm, qx, qy, qz);
+            if (prm.reuse) {                            // Fig. 2(C): the same point is reused
+                gx = qx; gy = qy; gz = qz;
+                if (it < prm.burn_in) continue;
+            }
+            const int pix = (alive && have) ? pixel_index(prm, qx, qy) : -1;
+            if (SPLAT == SPLAT_HIST_WARPAGG) {
+                splat_hist_warpagg(reinterpret_cast<uint32_t *>(prm.image), pix, pix >= 0);
+                if (have) { if (pix >= 0) ++n_in; else ++n_drop; }
+                continue;
+            }
+            if (pix < 0) { ++n_drop; continue; }
+            ++n_in;
+            if (SPLAT == SPLAT_HIST_DIRECT) {
+                red_add_u32(reinterpret_cast<uint32_t *>(prm.image) + pix, 1u);
+            } else if (SPLAT == SPLAT_HIST_SHARED) {
+                atomicAdd(&s_hist[pix], 1u);
+            } else if (SPLAT == SPLAT_RGBA) {
+                float *dst = reinterpret_cast<float *>(prm.image) + 4 * (size_t)pix;
+                if (GEN == 1) {   // colour of the point record, integer-valued (DESIGN R9)
+                    red_add_v4_f32(dst, (float)(point_rgba8 & 0xFFu), (float)((point_rgba8 >> 8) & 0xFFu),
+                                   (float)((point_rgba8 >> 16) & 0xFFu), 1.0f);
+                } else {          // colour of the map applied in this iteration
+                    const float4 c = s.palette[k];
+                    red_add_v4_f32(dst, c.x, c.y, c.z, 1.0f);
+                }
+            } else if (SPLAT == SPLAT_DEPTH) {
+                splat_depth(reinterpret_cast<unsigned long long *>(prm.image), pix, qz,
+                            GEN == 1 ? point_rgba8 : s.pal8[k]);
+            }
+        }
+    }
+
+    if (SPLAT == SPLAT_HIST_SHARED) {   // merge the private histogram (red.global, non-zero bins only)
+        __syncthreads();
+        uint32_t *hist = reinterpret_cast<uint32_t *>(prm.image);
+        for (uint32_t i = threadIdx.x; i < prm.hist_bins; i += blockDim.x) {
+            const uint32_t v = s_hist[i];
+            if (v) red_add_u32(hist + i, v);
+        }
+    }
+    if (prm.counters) {   // block-level reduction: two atomics per CTA (same-address L2 atomics serialise)
+        __shared__ unsigned long long s_cnt[2][kRenderThreads / 32];
+        unsigned long long a = n_in, b = n_drop;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            a += __shfl_xor_sync(0xFFFFFFFFu, a, o);
+            b += __shfl_xor_sync(0xFFFFFFFFu, b, o);
+        }
+        if ((threadIdx.x & 31) == 0) { s_cnt[0][threadIdx.x >> 5] = a; s_cnt[1][threadIdx.x >> 5] = b; }
+        __syncthreads();
+        if (threadIdx.x < 2) {
+            unsigned long long v = 0;
+            for (int i = 0; i < kRenderThreads / 32; ++i) v += s_cnt[threadIdx.x][i];
+            if (v) atomicAdd(prm.counters + threadIdx.x, v);
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// parity instrument: same device functions, records instead of splatting (SURVEY 8(c) S10 i, ii)
+template <int DIM, int GEN, int AFF>
+__global__ void __launch_bounds__(kRenderThreads)
+trace_kernel(const __grid_constant__ RenderParams prm)
+{
+    __shared__ SharedTables s;
+    if (GEN == 0) load_tables(s, prm);
+    __syncthreads();
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < prm.n_points; i += stride) {
+        const uint64_t p = prm.point_offset + i;
+        float gx, gy, gz = 0.0f;
+        if (GEN == 1) {
+            const float4 rec = __ldcs(reinterpret_cast<const float4 *>(prm.cloud) + p);
+            gx = rec.x; gy = rec.y; gz = (DIM == 3) ? rec.z : 0.0f;
+        } else {
+            const U4 w = philox4x32_10((uint32_t)p, (uint32_t)(p >> 32), 0u, DOMAIN_INIT, prm);
+            gx = u24_to_pm1(w.x);
+            gy = u24_to_pm1(w.y);
+            if (DIM == 3) gz = u24_to_pm1(w.z);
+        }
+        float qx = 0.f, qy = 0.f, qz = 0.f;
+        bool alive = false;
+        U4 w = {0, 0, 0, 0};
+        for (int it = 0; it < prm.iterations; ++it) {
+            if (GEN == 0) {
+                if ((it & 3) == 0)
+                    w = philox4x32_10((uint32_t)p, (uint32_t)(p >> 32), (uint32_t)it >> 2, DOMAIN_PICK, prm);
+                const uint32_t u = w.x;
+                w.x = w.y; w.y = w.z; w.z = w.w;
+                const int k = pick_index(u, s, prm);
+                if (prm.tr_picks) prm.tr_picks[i * (uint64_t)prm.iterations + it] = (uint8_t)k;
+                apply_gen<DIM, AFF>(k, s, gx, gy, gz);
+            }
+            if (it < prm.burn_in && !prm.reuse) continue;
+            qx = gx; qy = gy; qz = gz;
+            alive = apply_chain<DIM>(prm, qx, qy, qz);
+            if (prm.reuse) { gx = qx; gy = qy; gz = qz; }
+        }
+        if (prm.tr_g) { prm.tr_g[3 * i] = gx; prm.tr_g[3 * i + 1] = gy; prm.tr_g[3 * i + 2] = gz; }
+        if (prm.tr_q) { prm.tr_q[3 * i] = qx; prm.tr_q[3 * i + 1] = qy; prm.tr_q[3 * i + 2] = qz; }
+        if (prm.tr_alive) prm.tr_alive[i] = alive ? 1 : 0;
+    }
+}
+
+}  // namespace cfs

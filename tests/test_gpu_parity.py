@@ -1,0 +1,359 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on
+the same seeded inputs.  Bars (BASELINE.json north_star / SURVEY 8(c) S10):
+  (i)   map-index sequences bit-exact;
+  (ii)  final float32 coordinates within 1e-4 absolute;
+  (iii) affine-only images (cfg 0; cfg 4 incl. pinhole and depth) bit-exact per pixel;
+  (iv)  otherwise normalised-density L1 <= 1e-3 on the count and on each colour channel;
+  (v)   counters: in-bounds + dropped = points x (iterations - burn_in).
+"""
+import math
+
+import numpy as np
+import pytest
+
+from paper_2606_02226_b200 import workloads as W
+from tests._gpu_util import density_l1, gpu_render, gpu_trace
+
+pytestmark = pytest.mark.gpu
+
+COORD_TOL = 1e-4
+L1_TOL = 1e-3
+
+
+@pytest.fixture(scope="module")
+def cfs():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2606_02226_b200 import cfs as mod
+    mod.lib()
+    return mod
+
+
+def _cloud_for(w, n):
+    return W.gaussian_mixture_cloud(n, w.cloud_seed) if w.system.gen == "cloud" else None
+
+
+# ------------------------------------------------------------------ (i), (ii): picks and coordinates
+@pytest.mark.parametrize("cfg", [0, 1, 2, 3, 4])
+def test_pick_sequences_and_coordinates(cfs, oracle, cfg):
+    w = W.config(cfg)
+    n = 1024 + 37                                   # several CTAs and a ragged tail
+    cloud = _cloud_for(w, n)
+    w = w.scaled(n_points=n)
+    for t in (w.frames[0], w.frames[len(w.frames) // 2]) if len(w.frames) > 1 else (w.frames[0],):
+        gp, gg, gq, ga = gpu_trace(cfs, w, t=t, cloud=cloud)
+        op, og, oq, oa = oracle.trace(w.system, w.render, cloud=cloud, t=t)
+        assert np.array_equal(gp, op)                               # (i) bit-exact
+        assert np.array_equal(gg, og)                               # affine generators: bit-equal
+        assert np.array_equal(ga, oa)
+        live = oa.astype(bool)
+        assert np.abs(gq[live].astype(np.float64) - oq[live]).max() <= COORD_TOL   # (ii)
+        if cfg in (0, 4):
+            assert np.array_equal(gq, oq)                           # affine + pinhole: bit-exact
+
+
+def test_point_offset_beyond_32_bits(cfs, oracle):
+    w = W.config(0).scaled(n_points=300, iterations=40)
+    off = (1 << 33) + 12345
+    gp, gg, _, _ = gpu_trace(cfs, w, point_offset=off)
+    op, og, _, _ = oracle.trace(w.system, w.render, point_offset=off)
+    assert np.array_equal(gp, op) and np.array_equal(gg, og)
+
+
+# ------------------------------------------------------------------ (iii): bit-exact images
+@pytest.mark.parametrize("variant", ["direct", "warp_agg", "auto"])
+def test_cfg0_histogram_bit_exact(cfs, oracle, variant):
+    w = W.config(0).scaled(n_points=4096 + 99)
+    g, gc = gpu_render(cfs, w, variant=variant)
+    o, oc, _ = oracle.render_parallel(w.system, w.render)
+    assert np.array_equal(g, o)
+    assert np.array_equal(gc, oc) and int(gc[0]) == w.render.n_points * 980 and int(gc[1]) == 0
+
+
+@pytest.mark.parametrize("size", [(64, 64), (200, 120), (224, 224)])
+@pytest.mark.parametrize("variant", ["shared_hist", "direct", "warp_agg", "auto"])
+def test_small_histograms_all_variants(cfs, oracle, size, variant):
+    """Per-CTA shared-memory privatised histogram (and the others) on images that fit shared memory;
+    bounds narrower than the attractor so that some splats are dropped."""
+    w = W.config(0).scaled(n_points=3000, iterations=200, width=size[0], height=size[1])
+    w = w.scaled(bounds=(-0.75, 1.0, -1.0, 0.5))
+    g, gc = gpu_render(cfs, w, variant=variant)
+    o, oc, _ = oracle.render_parallel(w.system, w.render)
+    assert np.array_equal(g, o) and np.array_equal(gc, oc)
+    assert int(gc[1]) > 0 and int(gc[0]) + int(gc[1]) == 3000 * 180
+
+
+def test_cfg0_full_size_bit_exact(cfs, oracle):
+    w = W.config(0)
+    g, gc = gpu_render(cfs, w)
+    o, oc, _ = oracle.render_parallel(w.system, w.render)
+    assert int(gc[0]) == 64225280 and int(g.sum(dtype=np.uint64)) == 64225280
+    assert np.array_equal(g, o)
+
+
+@pytest.mark.parametrize("n", [1, 31, 255, 256, 257, 5000])
+def test_cfg4_depth_bit_exact(cfs, oracle, n):
+    w = W.config(4).scaled(n_points=n, iterations=120, width=480, height=270)
+    g, gc = gpu_render(cfs, w)
+    o, oc = oracle.render(w.system, w.render)
+    assert np.array_equal(g, o) and np.array_equal(gc, oc)
+    assert int(gc[0]) == n * 100
+
+
+def test_cfg4_full_image_subrange_bit_exact(cfs, oracle):
+    """Full 3840x2160 buffer, bench launch shape, a point sub-range the oracle finishes in seconds;
+    sub-ranges compose by min into the full-range result."""
+    w = W.config(4).scaled(n_points=1 << 13)
+    g, gc = gpu_render(cfs, w)
+    o, oc, _ = oracle.render_parallel(w.system, w.render)
+    assert np.array_equal(g, o) and np.array_equal(gc, oc)
+    a, _ = gpu_render(cfs, w, n_points=5000, point_offset=0)
+    b, _ = gpu_render(cfs, w, n_points=(1 << 13) - 5000, point_offset=5000)
+    assert np.array_equal(np.minimum(a, b), g)
+
+
+# ------------------------------------------------------------------ (iv): density L1
+def _check_rgba(g, o, gc, oc):
+    assert np.array_equal(gc, oc)                                    # (v)
+    assert g[:, 3].astype(np.float64).sum() == o[:, 3].sum() == float(oc[0])
+    for ch in range(4):
+        assert density_l1(g[:, ch], o[:, ch]) <= L1_TOL
+
+
+def test_cfg1_swirl_rgba(cfs, oracle):
+    w = W.config(1).scaled(n_points=(1 << 14) + 5)
+    g, gc = gpu_render(cfs, w)
+    o, oc, _ = oracle.render_parallel(w.system, w.render)
+    _check_rgba(g, o, gc, oc)
+    assert int(gc[1]) == 0
+
+
+@pytest.mark.parametrize("frame", [0, 7, 15])
+def test_cfg2_animation_frames(cfs, oracle, frame):
+    w = W.config(2).scaled(n_points=(1 << 14) + 3)
+    t = w.frames[frame]
+    g, gc = gpu_render(cfs, w, t=t)
+    o, oc, _ = oracle.render_parallel(w.system, w.render, t=t)
+    _check_rgba(g, o, gc, oc)
+
+
+def test_cfg3_cloud(cfs, oracle):
+    w = W.config(3)
+    n = (1 << 18) + 11
+    cloud = W.gaussian_mixture_cloud(n, w.cloud_seed)
+    w = w.scaled(n_points=n)
+    g, gc = gpu_render(cfs, w, cloud=cloud)
+    o, oc, _ = oracle.render_parallel(w.system, w.render, cloud=cloud)
+    assert int(gc[0]) + int(gc[1]) == n
+    # a point within float rounding of the frustum edge may be dropped on one side only
+    assert abs(int(gc[0]) - int(oc[0])) <= 4
+    for ch in range(4):
+        assert density_l1(g[:, ch], o[:, ch]) <= L1_TOL
+    # sub-range of the whole cloud: record p is d_cloud[p]
+    a, _ = gpu_render(cfs, w, cloud=cloud, n_points=n - 1000, point_offset=1000)
+    b, _ = gpu_render(cfs, w, cloud=cloud, n_points=1000, point_offset=0)
+    assert np.array_equal(a + b, g)                                  # integer-valued sums: exact
+
+
+# ------------------------------------------------------------------ general tables and edge cases
+def test_general_pick_and_general_affine(cfs, oracle):
+    """Non-uniform probabilities incl. zero-probability maps (table + compare pick), non-diagonal
+    affine maps in 2-D and 3-D (general coefficient rows)."""
+    rng = np.random.default_rng(3)
+    funcs2 = []
+    probs = [0.05, 0.0, 0.4, 0.25, 0.3, 0.0, 1e-4]
+    for pr in probs:
+        th = rng.uniform(0, 2 * math.pi)
+        s = rng.uniform(0.2, 0.6)
+        funcs2.append(W.Func("affine", float(np.float32(pr)),
+                             [s * math.cos(th), -s * math.sin(th), s * math.sin(th), s * math.cos(th),
+                              rng.uniform(-0.4, 0.4), rng.uniform(-0.4, 0.4)]))
+    sys2 = W.System(2, "ifs", funcs2, [], "none")
+    w2 = W.Workload("gen2", sys2, W.Render(2000, 9, 64, 4, 300, 200, (-1, 1, -1, 1), "hist_u32"))
+    gp, gg, _, _ = gpu_trace(cfs, w2)
+    op, og, _, _ = oracle.trace(sys2, w2.render)
+    assert np.array_equal(gp, op) and np.array_equal(gg, og)
+    assert set(np.unique(gp)) <= {0, 2, 3, 4, 6}
+    g, gc = gpu_render(cfs, w2, variant="direct")
+    o, oc = oracle.render(sys2, w2.render)
+    assert np.array_equal(g, o) and np.array_equal(gc, oc)
+
+    funcs3 = []
+    for k in range(37):
+        A = rng.uniform(-0.35, 0.35, size=(3, 3))
+        b = rng.uniform(-0.5, 0.5, size=3)
+        funcs3.append(W.Func("affine", float(np.float32(rng.uniform(0.0, 1.0))), list(A.ravel()) + list(b)))
+    pal = W.palette_for(37)
+    sys3 = W.System(3, "ifs", funcs3, [W.PINHOLE], "map_index", pal)
+    w3 = W.Workload("gen3", sys3, W.Render(3000, 10, 50, 5, 160, 90, (-1, 1, -1, 1), "depth_u64"))
+    gp, gg, gq, ga = gpu_trace(cfs, w3)
+    op, og, oq, oa = oracle.trace(sys3, w3.render)
+    assert np.array_equal(gp, op) and np.array_equal(gg, og) and np.array_equal(gq, oq) and np.array_equal(ga, oa)
+    g, gc = gpu_render(cfs, w3)
+    o, oc = oracle.render(sys3, w3.render)
+    assert np.array_equal(g, o) and np.array_equal(gc, oc)
+
+
+def test_n64_funcs_and_single_func(cfs, oracle):
+    funcs = [W.Func("affine", float(np.float32(1 + (k % 5))), [0.5, 0, 0, 0.5, 0.5 * math.cos(k), 0.5 * math.sin(k)])
+             for k in range(64)]
+    sysm = W.System(2, "ifs", funcs, [], "map_index", W.palette_for(64))
+    w = W.Workload("n64", sysm, W.Render(1500, 4, 80, 8, 128, 128, (-1, 1, -1, 1), "rgba_f32"))
+    gp, _, _, _ = gpu_trace(cfs, w)
+    op, _, _, _ = oracle.trace(sysm, w.render)
+    assert np.array_equal(gp, op) and gp.max() == 63
+    g, gc = gpu_render(cfs, w)
+    o, oc = oracle.render(sysm, w.render)
+    assert np.array_equal(g.astype(np.float64), o) and np.array_equal(gc, oc)     # integer sums: exact
+    one = W.System(2, "ifs", funcs[:1], [], "none")
+    w1 = W.Workload("n1", one, W.Render(100, 4, 30, 0, 64, 64, (-1, 1, -1, 1), "hist_u32"))
+    g, _ = gpu_render(cfs, w1, variant="direct")
+    o, _ = oracle.render(one, w1.render)
+    assert np.array_equal(g, o)
+
+
+def test_reuse_composition_and_eq2(cfs, oracle):
+    """Fig. 2(C) reuse flag and the paper's Eq. 2 transform."""
+    chain = [W.Xform("stretch_cos"), W.Xform("affine", [0.4, 0, 0, 0.4, 0, 0.3])]
+    for reuse in (False, True):
+        sysr = W.System(2, "ifs", W.square_funcs(), chain, "map_index", W.palette_for(4), reuse=reuse)
+        w = W.Workload("reuse", sysr, W.Render(2000, 12, 60, 10, 256, 256, (-1.5, 1.5, -1.5, 1.5), "rgba_f32"))
+        gp, gg, gq, ga = gpu_trace(cfs, w)
+        op, og, oq, oa = oracle.trace(sysr, w.render)
+        assert np.array_equal(gp, op) and np.array_equal(ga, oa)
+        assert np.abs(gg.astype(np.float64) - og).max() <= COORD_TOL
+        assert np.abs(gq.astype(np.float64) - oq).max() <= COORD_TOL
+        g, gc = gpu_render(cfs, w)
+        o, oc = oracle.render(sysr, w.render)
+        assert np.array_equal(gc, oc)
+        for ch in range(4):
+            assert density_l1(g[:, ch], o[:, ch]) <= 4e-3      # 100k splats: a handful of edge flips
+
+
+def test_empty_and_accumulate(cfs, oracle):
+    import torch
+    w = W.config(0).scaled(n_points=0)
+    g, gc = gpu_render(cfs, w)
+    assert int(g.sum()) == 0 and int(gc.sum()) == 0
+    # accumulation into a caller-owned image: two sub-ranges into one buffer
+    w = W.config(0).scaled(n_points=700, iterations=50)
+    img = cfs.new_image(w.render)
+    gpu_render(cfs, w, n_points=300, point_offset=0, image=img, variant="direct")
+    g, _ = gpu_render(cfs, w, n_points=400, point_offset=300, image=img, variant="direct")
+    o, _ = oracle.render(w.system, w.render)
+    assert np.array_equal(g, o)
+    torch.cuda.synchronize()
+
+
+def test_invalid_arguments(cfs):
+    import torch
+    w = W.config(0).scaled(n_points=10)
+    sysh = cfs.cfs_create(w.system)
+    img = cfs.new_image(w.render)
+
+    def status(**kw):
+        r = w.scaled(**kw).render
+        try:
+            cfs.cfs_render(sysh, cfs.make_args(r, d_image=img))
+        except cfs.CfsError as e:
+            return e.status
+        return 0
+
+    assert status(iterations=0) == cfs.CFS_ERR_INVALID_ARG
+    assert status(burn_in=1000) == cfs.CFS_ERR_INVALID_ARG
+    assert status(burn_in=-1) == cfs.CFS_ERR_INVALID_ARG
+    assert status(bounds=(1.0, -1.0, -1.0, 1.0)) == cfs.CFS_ERR_INVALID_ARG
+    assert status(bounds=(float("nan"), 1.0, -1.0, 1.0)) == cfs.CFS_ERR_INVALID_ARG
+    assert status(width=0) == cfs.CFS_ERR_INVALID_ARG
+    assert status(width=65536, height=65536) == cfs.CFS_ERR_INVALID_ARG
+    assert status(out_mode="rgba_f32") == cfs.CFS_ERR_INVALID_ARG      # COLOR_NONE needs HIST
+    assert status(out_mode="depth_u64") == cfs.CFS_ERR_INVALID_ARG
+    with pytest.raises(cfs.CfsError) as ei:                            # shared variant on a 1 MiB image
+        cfs.cfs_render(sysh, cfs.make_args(w.render, d_image=img, variant="shared_hist"))
+    assert ei.value.status == cfs.CFS_ERR_UNSUPPORTED
+    with pytest.raises(cfs.CfsError):
+        cfs.cfs_render(sysh, cfs.make_args(w.render, d_image=None))
+    assert status() == 0
+    torch.cuda.synchronize()
+    sysh.close()
+    bad = W.System(2, "ifs", [W.Func("affine", -1.0, [0.5, 0, 0, 0.5, 0, 0])], [], "none")
+    with pytest.raises(cfs.CfsError):
+        cfs.cfs_create(bad)
+    with pytest.raises(cfs.CfsError):
+        cfs.cfs_create(W.System(2, "ifs", W.square_funcs(), [], "point"))
+    with pytest.raises(cfs.CfsError):
+        cfs.cfs_create(W.System(4, "ifs", W.square_funcs(), [], "none"))
+    with pytest.raises(cfs.CfsError):
+        cfs.cfs_create(W.System(3, "cloud", [], [], "map_index", W.palette_for(4)))
+
+
+# ------------------------------------------------------------------ tone map and host entry point
+@pytest.mark.parametrize("cfg", [0, 1, 4])
+def test_tonemap_matches_oracle(cfs, oracle, cfg):
+    import torch
+    w = W.config(cfg).scaled(n_points=1 << 13, iterations=200)
+    sysh = cfs.cfs_create(w.system)
+    img = cfs.new_image(w.render)
+    cfs.cfs_render(sysh, cfs.make_args(w.render, d_image=img))
+    n = w.render.width * w.render.height
+    out = torch.zeros(n, dtype=torch.int32, device="cuda")
+    scratch = torch.zeros(2, dtype=torch.int32, device="cuda")
+    cfs.cfs_tonemap(img, w.render.out_mode, w.render.width, w.render.height, 2.2, 1 / 255.0, out, scratch)
+    torch.cuda.synchronize()
+    got = out.cpu().numpy().view(np.uint32)
+    want = oracle.tonemap(cfs.image_to_numpy(img, w.render.out_mode), w.render.out_mode, w.render.width,
+                          w.render.height, 2.2, 1 / 255.0)
+    if cfg == 4:
+        assert np.array_equal(got, want)
+    else:
+        for sh in (0, 8, 16, 24):
+            d = np.abs(((got >> sh) & 0xFF).astype(np.int32) - ((want >> sh) & 0xFF).astype(np.int32))
+            assert d.max() <= 1
+        assert np.array_equal(got == 0, want == 0) and np.count_nonzero(got) > 1000
+    sysh.close()
+
+
+@pytest.mark.parametrize("cfg", [0, 3, 4])
+def test_render_host_entry_point(cfs, oracle, cfg):
+    """cfs_render_host: HOST buffers in and out (the end-to-end call bench.py times)."""
+    w = W.config(cfg)
+    n = 5000
+    cloud = _cloud_for(w, n + 100)
+    w = w.scaled(n_points=n, iterations=min(w.render.iterations, 60), burn_in=min(w.render.burn_in, 20),
+                 width=320, height=180)
+    npx = 320 * 180
+    h_img = {"hist_u32": np.empty(npx, np.uint32), "rgba_f32": np.empty((npx, 4), np.float32),
+             "depth_u64": np.empty(npx, np.uint64)}[w.render.out_mode]
+    h_ctr = np.zeros(2, np.uint64)
+    sysh = cfs.cfs_create(w.system)
+    off = 100 if cloud is not None else 0
+    cfs.cfs_render_host(sysh, cfs.make_args(w.render, point_offset=off), h_img, cloud, h_ctr)
+    o, oc = oracle.render(w.system, w.render, cloud=cloud, point_offset=off)
+    if cfg == 3:
+        for ch in range(4):
+            assert density_l1(h_img[:, ch], o[:, ch]) <= 4e-3
+    else:
+        assert np.array_equal(h_img, o)
+    assert np.array_equal(h_ctr, oc) or cfg == 3
+    sysh.close()
+
+
+# ------------------------------------------------------------------ full-size properties (bench launch shape)
+def test_cfg1_full_size_properties(cfs, oracle):
+    """BASELINE configs[1] as bench.py launches it: conservation (exact, every pixel count < 2^24),
+    colour sums = 255 x picks of each map, and sub-ranges compose; oracle parity on the first 2^15
+    points rendered into the full-size image."""
+    w = W.config(1)
+    g, gc = gpu_render(cfs, w)
+    P, S = w.render.n_points, w.render.n_points * 980
+    assert int(gc[0]) == S and int(gc[1]) == 0
+    assert g[:, 3].max() < 2 ** 24 and g[:, 3].astype(np.float64).sum() == S
+    col = g[:, :3].astype(np.float64).sum(axis=0) / 255.0            # map 0: R, 1: G, 2: B, 3: R+G
+    assert g[:, :3].max() < 2 ** 24 and np.all(col == np.round(col))
+    assert abs(col[2] / S - 0.25) < 1e-3 and abs(col[1] / S - 0.5) < 1e-3 and abs(col[0] / S - 0.5) < 1e-3
+    sub = w.scaled(n_points=1 << 15)
+    gs, gsc = gpu_render(cfs, sub)
+    o, oc, _ = oracle.render_parallel(sub.system, sub.render)
+    assert np.array_equal(gsc, oc)
+    for ch in range(4):
+        assert density_l1(gs[:, ch], o[:, ch]) <= L1_TOL
