@@ -390,7 +390,7 @@ def run_ours(args):
         line["workloads"] = wl
 
     # ---- the oracle timed beside it (reported baseline, never tuned)
-    n_cpu = 1 << 15
+    n_cpu = 1 << 17
     pi, dt, threads = oracle_sample(HEADLINE_CFG, n_cpu)
     line["cpu_baseline"] = {"value": pi / dt, "unit": UNIT, "cores": threads, "kind": "oracle",
                             "sample": f"first {n_cpu} points x {I} iterations of configs[{HEADLINE_CFG}], full image, "
@@ -402,6 +402,36 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_profile_cfg(args):
+    """Target of the ncu commands under profiles/: `--steps` cfs_render launches of configs[N] (one
+    frame, t = middle frame), 2 warm-ups, nothing else on the GPU.  Prints device time per launch."""
+    import torch
+    from paper_2606_02226_b200 import cfs
+    torch.cuda.set_device(0)
+    cfg = args.profile_cfg
+    w = W.config(cfg)
+    cloud = W.gaussian_mixture_cloud(w.render.n_points, w.cloud_seed) if w.system.gen == "cloud" else None
+    d_cloud = cfs.cloud_to_device(cloud) if cloud is not None else None
+    sysh = cfs.cfs_create(w.system)
+    img = cfs.new_image(w.render)
+    ctr = torch.zeros(2, dtype=torch.int64, device="cuda")
+    t = w.frames[len(w.frames) // 2]
+    rargs = cfs.make_args(w.render, d_image=img, d_cloud=d_cloud, d_counters=ctr, t=t, variant=args.variant)
+    ms = []
+    for i in range(2 + args.steps):
+        img.fill_(-1 if w.render.out_mode == "depth_u64" else 0)
+        e0, e1 = event_pair(torch)
+        e0.record()
+        cfs.cfs_render(sysh, rargs)
+        e1.record()
+        torch.cuda.synchronize()
+        if i >= 2:
+            ms.append(e0.elapsed_time(e1))
+    print(json.dumps({"profile_cfg": cfg, "workload": w.name, "variant": args.variant, "launch_ms": ms,
+                      "point_iterations_per_s": w.render.n_points * w.render.iterations / (min(ms) * 1e-3)}))
+    sysh.close()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -409,8 +439,13 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-workloads", action="store_true", help="skip the per-config side report")
+    ap.add_argument("--profile-cfg", type=int, default=None,
+                    help="only launch cfs_render of configs[N] --steps times (ncu target; no bench line)")
+    ap.add_argument("--variant", default="auto", help="splat variant for --profile-cfg")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.profile_cfg is not None:
+        run_profile_cfg(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)
