@@ -28,6 +28,7 @@ if ROOT not in sys.path:
 from paper_2606_02226_b200 import workloads as W  # noqa: E402  (inputs only, no arithmetic)
 
 HEADLINE_CFG = 1
+SINCOS = "sincosf (<= 2 ulp)"
 METRIC = "cfs_point_iterations_per_s"
 UNIT = "point-iterations/s"
 L2_FLUSH_BYTES = 256 << 20
@@ -146,7 +147,7 @@ def workload_config(w, n_gpus):
     r = w.render
     return {"workload": f"BASELINE configs[{HEADLINE_CFG}] {w.name}", "points_per_gpu": r.n_points,
             "iterations": r.iterations, "burn_in": r.burn_in, "image": f"{r.width}x{r.height} {r.out_mode}",
-            "chain": [x.type for x in w.system.chain], "n_funcs": len(w.system.funcs),
+            "chain": [x.type for x in w.system.chain], "n_funcs": len(w.system.funcs), "sincos": SINCOS,
             "parallelism": f"points sharded over {n_gpus} GPU(s), image all-reduce" if n_gpus > 1 else "1 GPU",
             "l2": "flushed between steps (256 MiB memset outside the per-step events); the 16 MiB image is "
                   "L2-resident by design"}
@@ -212,7 +213,7 @@ def roofline_for(cfg, w, rates, peaks, splats, seconds):
             "t_roof_ms": t_roof * 1e3, "t_ms": seconds * 1e3, "frac": t_roof / seconds}
 
 
-def time_workload(cfs, torch, cfg, flush, reps=5):
+def time_workload(cfs, torch, cfg, flush, reps=5, flags=0):
     """Median device time of one cfs_render of configs[cfg] (all frames for cfg 2)."""
     w = W.config(cfg)
     cloud = W.gaussian_mixture_cloud(w.render.n_points, w.cloud_seed) if w.system.gen == "cloud" else None
@@ -228,7 +229,7 @@ def time_workload(cfs, torch, cfg, flush, reps=5):
         ctr.zero_()
         for t in w.frames:
             img.fill_(-1 if w.render.out_mode == "depth_u64" else 0)
-            args = cfs.make_args(w.render, d_image=img, d_cloud=d_cloud, d_counters=ctr, t=t)
+            args = cfs.make_args(w.render, d_image=img, d_cloud=d_cloud, d_counters=ctr, t=t, flags=flags)
             e0, e1 = event_pair(torch)
             e0.record()
             cfs.cfs_render(sysh, args)
@@ -276,7 +277,8 @@ def run_ours(args):
     scratch = torch.zeros(2, dtype=torch.int32, device="cuda")
     flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device="cuda")
     # weak scaling: every rank renders its own P points of the global point-id space
-    rargs = cfs.make_args(r, d_image=img, d_counters=ctr, point_offset=rank * P)
+    flags = ["fast_trig"] if args.fast_trig else 0
+    rargs = cfs.make_args(r, d_image=img, d_counters=ctr, point_offset=rank * P, flags=flags)
 
     def step(timed):
         flush.zero_()                         # L2 flush, outside the events
@@ -321,7 +323,7 @@ def run_ours(args):
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
     h_img = torch.empty((r.width * r.height, 4), dtype=torch.float32).pin_memory()
     h_ctr = torch.zeros(2, dtype=torch.int64).pin_memory()
-    hargs = cfs.make_args(r, point_offset=rank * P)
+    hargs = cfs.make_args(r, point_offset=rank * P, flags=flags)
     for _ in range(2):
         cfs.cfs_render_host(sysh, hargs, h_img.numpy(), None, h_ctr.numpy())
     torch.cuda.synchronize()
@@ -378,7 +380,7 @@ def run_ours(args):
     if not args.no_workloads and world == 1:
         wl = {}
         for cfg in range(W.N_CONFIGS):
-            wk, sec, n_in, n_drop = time_workload(cfs, torch, cfg, flush)
+            wk, sec, n_in, n_drop = time_workload(cfs, torch, cfg, flush, flags=flags)
             pi = wk.point_iterations
             rf = roofline_for(cfg, wk, rates, peaks, n_in / len(wk.frames), sec / len(wk.frames))
             wl[f"cfg{cfg}"] = {"name": wk.name, "ms": sec * 1e3, "point_iterations_per_s": pi / sec,
@@ -416,7 +418,8 @@ def run_profile_cfg(args):
     img = cfs.new_image(w.render)
     ctr = torch.zeros(2, dtype=torch.int64, device="cuda")
     t = w.frames[len(w.frames) // 2]
-    rargs = cfs.make_args(w.render, d_image=img, d_cloud=d_cloud, d_counters=ctr, t=t, variant=args.variant)
+    rargs = cfs.make_args(w.render, d_image=img, d_cloud=d_cloud, d_counters=ctr, t=t, variant=args.variant,
+                          flags=["fast_trig"] if args.fast_trig else 0)
     ms = []
     for i in range(2 + args.steps):
         img.fill_(-1 if w.render.out_mode == "depth_u64" else 0)
@@ -442,7 +445,11 @@ def main():
     ap.add_argument("--profile-cfg", type=int, default=None,
                     help="only launch cfs_render of configs[N] --steps times (ncu target; no bench line)")
     ap.add_argument("--variant", default="auto", help="splat variant for --profile-cfg")
+    ap.add_argument("--fast-trig", action="store_true", help="CFS_FLAG_FAST_TRIG (MUFU sin/cos) on every render")
     args = ap.parse_args()
+    global SINCOS
+    if args.fast_trig:
+        SINCOS = "MUFU sin.approx/cos.approx (CFS_FLAG_FAST_TRIG)"
     if args.profile_cfg is not None:
         run_profile_cfg(args)
     elif args.impl == "reference":

@@ -88,6 +88,15 @@ typedef enum {
     CFS_VARIANT_WARP_AGG = 3     /* DIRECT + __match_any_sync aggregation of same-pixel hits (HIST)   */
 } cfs_variant;
 
+/* render flags.
+ *   FAST_TRIG: the non-affine chain steps evaluate sin/cos on the special-function unit (MUFU
+ *   sin.approx / cos.approx, absolute error ~2^-21 on [-pi, pi], growing with |argument|) instead
+ *   of the <= 2 ulp sincosf.  Within the 1e-4 coordinate tolerance of BASELINE north_star for the
+ *   bounded arguments of contractive systems; the default is the accurate evaluation.
+ *   INTERPRET_CHAIN: never use a kernel compiled for the chain's signature; run the chain
+ *   interpreter (same device functions, same results; for tests and comparisons). */
+typedef enum { CFS_FLAG_FAST_TRIG = 1, CFS_FLAG_INTERPRET_CHAIN = 2 } cfs_render_flags;
+
 /* one 16-byte record of a stored cloud (BASELINE cfg 3); rgba8 = r | g<<8 | b<<16 | a<<24 */
 typedef struct { float x, y, z; uint32_t rgba8; } cfs_cloud_rec;
 
@@ -115,7 +124,7 @@ typedef struct {
     float t;                /* frame parameter                                                  */
     int32_t out_mode;       /* cfs_out_mode                                                     */
     int32_t variant;        /* cfs_variant                                                      */
-    int32_t reserved_;      /* must be 0                                                        */
+    int32_t flags;          /* OR of cfs_render_flags; 0 = accurate sin/cos, compiled chain     */
     void *d_image;          /* device, caller-owned, caller-cleared, accumulates                */
     const void *d_cloud;    /* device, CLOUD only: record p of the WHOLE cloud is d_cloud[p]    */
     uint64_t *d_counters;   /* optional device u64[2]: += in-bounds splats, += dropped splats   */

@@ -10,6 +10,7 @@ from __future__ import annotations
 
 import glob
 import os
+from concurrent.futures import ThreadPoolExecutor
 import subprocess
 import sys
 
@@ -19,8 +20,9 @@ LIB = os.path.join(HERE, "libcfs_b200.so")
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
     "-fmad=false", "-prec-div=true", "-prec-sqrt=true",
-    "-Xcompiler", "-fPIC,-ffp-contract=off,-O2", "-shared",
+    "-Xcompiler", "-fPIC,-ffp-contract=off,-O2",
 ]
+OBJ_DIR = os.path.join(HERE, "build")
 
 
 def sources():
@@ -40,8 +42,19 @@ def build(force: bool = False, verbose: bool = False) -> str:
     nvcc = os.environ.get("NVCC") or "/usr/local/cuda/bin/nvcc"
     if not os.path.exists(nvcc):
         nvcc = "nvcc"
-    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + sources()
-    subprocess.run(cmd, check=True, cwd=CSRC)
+    os.makedirs(OBJ_DIR, exist_ok=True)
+    extra = ["-Xptxas", "-v"] if verbose else []
+
+    def compile_one(src):
+        obj = os.path.join(OBJ_DIR, os.path.basename(src)[:-3] + ".o")
+        subprocess.run([nvcc] + NVCC_FLAGS + extra + ["-c", "-o", obj, src], check=True, cwd=CSRC)
+        return obj
+
+    # the kernel translation units are independent: compile them side by side, then link
+    with ThreadPoolExecutor(max_workers=min(len(sources()), os.cpu_count() or 1)) as ex:
+        objs = list(ex.map(compile_one, sources()))
+    subprocess.run([nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB] + objs,
+                   check=True, cwd=CSRC)
     return LIB
 
 

@@ -22,6 +22,7 @@ T_TYPE = {"affine": 0, "swirl": 1, "sinusoidal": 2, "rotate_z": 3, "twist_z": 4,
           "pinhole": 6, "stretch_cos": 7}
 COLOR = {"none": 0, "map_index": 1, "point": 2}
 OUT = {"hist_u32": 0, "rgba_f32": 1, "depth_u64": 2}
+FLAGS = {"fast_trig": 1, "interpret_chain": 2}
 VARIANT = {"auto": 0, "direct": 1, "shared_hist": 2, "warp_agg": 3}
 MB = {"red_add_u32": 0, "red_add_v4f32": 1, "atom_min_u64": 2, "ld_u64": 3, "atoms_add_u32": 4,
       "ffma": 5, "imad_wide": 6, "lop3": 7, "mufu": 8, "stream_ld128": 9}
@@ -50,7 +51,7 @@ class cfs_render_args(C.Structure):
                 ("width", C.c_int32), ("height", C.c_int32),
                 ("xmin", C.c_float), ("xmax", C.c_float), ("ymin", C.c_float), ("ymax", C.c_float),
                 ("t", C.c_float), ("out_mode", C.c_int32), ("variant", C.c_int32),
-                ("reserved_", C.c_int32),
+                ("flags", C.c_int32),
                 ("d_image", C.c_void_p), ("d_cloud", C.c_void_p), ("d_counters", C.c_void_p)]
 
 
@@ -185,7 +186,7 @@ def cfs_create(system) -> System:
 
 
 def make_args(render, d_image=None, d_cloud=None, d_counters=None, n_points=None, point_offset=None,
-              t=None, variant="auto") -> cfs_render_args:
+              t=None, variant="auto", flags=0) -> cfs_render_args:
     a = cfs_render_args()
     a.n_points = int(render.n_points if n_points is None else n_points)
     a.point_offset = int(render.point_offset if point_offset is None else point_offset)
@@ -198,7 +199,7 @@ def make_args(render, d_image=None, d_cloud=None, d_counters=None, n_points=None
     a.t = float(render.t if t is None else t)
     a.out_mode = OUT[render.out_mode] if isinstance(render.out_mode, str) else int(render.out_mode)
     a.variant = VARIANT[variant] if isinstance(variant, str) else int(variant)
-    a.reserved_ = 0
+    a.flags = sum(FLAGS[f] for f in flags) if isinstance(flags, (tuple, list)) else int(flags)
     a.d_image = _ptr(d_image)
     a.d_cloud = _ptr(d_cloud)
     a.d_counters = _ptr(d_counters)

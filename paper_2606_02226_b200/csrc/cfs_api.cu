@@ -10,8 +10,9 @@
 #include <vector>
 
 #include "../../include/cfs.h"
+#include "cfs_device.cuh"
 #include "cfs_microbench.cuh"
-#include "cfs_render.cuh"
+#include "cfs_registry.h"
 #include "cfs_tonemap.cuh"
 
 static_assert((int)CFS_T_AFFINE == (int)cfs::T_AFFINE && (int)CFS_T_SWIRL == (int)cfs::T_SWIRL &&
@@ -67,7 +68,7 @@ struct cfs_system {
     std::vector<float> palette;
     // pick tables (DESIGN R2)
     uint32_t T[cfs::kMaxFuncs];
-    uint8_t lut[256];
+    uint32_t lut[256];
     int32_t n_thr = 0, pick_steps = 0, pick_shift = -1;
     int32_t aff = cfs::AFF_GENERAL;
     float coef[cfs::kMaxFuncs * 12];
@@ -119,11 +120,12 @@ cfs_status build_tables(cfs_system *s)
     for (int b = 0; b < 256; ++b) {
         const uint64_t lo = (uint64_t)b << 24, hi = lo + 0xFFFFFFull;
         int below = 0, inside = 0;
+        uint32_t t24 = 1u << 24;                                  // none
         for (int j = 0; j < s->n_thr; ++j) {
             if (T64[j] <= lo) ++below;
-            else if (T64[j] <= hi) ++inside;
+            else if (T64[j] <= hi) { if (!inside) t24 = (uint32_t)(T64[j] - lo); ++inside; }
         }
-        s->lut[b] = (uint8_t)below;
+        s->lut[b] = ((uint32_t)below << 25) | t24;
         if (inside > s->pick_steps) s->pick_steps = inside;
     }
     // equal power-of-two thresholds: k = u >> shift
@@ -230,7 +232,7 @@ using cfs::RenderParams;
 cfs_status build_params(const cfs_system *s, const cfs_render_args *a, RenderParams *out, bool need_image)
 {
     if (!s || !a) return fail(CFS_ERR_INVALID_ARG, "system or args is NULL");
-    if (a->reserved_ != 0) return fail(CFS_ERR_INVALID_ARG, "reserved_ must be 0");
+    if (a->flags & ~(CFS_FLAG_FAST_TRIG | CFS_FLAG_INTERPRET_CHAIN)) return fail(CFS_ERR_INVALID_ARG, "unknown flags 0x%x", a->flags);
     if (a->iterations < 1) return fail(CFS_ERR_INVALID_ARG, "iterations must be >= 1");
     if (a->burn_in < 0 || a->burn_in >= a->iterations) return fail(CFS_ERR_INVALID_ARG, "burn_in must be in [0, iterations)");
     if (s->gen == CFS_GEN_CLOUD && (a->iterations != 1 || a->burn_in != 0)) return fail(CFS_ERR_INVALID_ARG, "CLOUD generator needs iterations = 1, burn_in = 0");
@@ -263,7 +265,7 @@ cfs_status build_params(const cfs_system *s, const cfs_render_args *a, RenderPar
     p.sy = (float)((double)a->height / wy); p.oy = (float)(-(double)a->ymin * (double)a->height / wy);
     p.image = a->d_image; p.cloud = a->d_cloud; p.counters = (unsigned long long *)a->d_counters;
     p.dim = s->dim; p.n_funcs = (int)s->funcs.size(); p.n_chain = (int)s->chain.size();
-    p.color_rule = s->color; p.reuse = s->reuse;
+    p.color_rule = s->color; p.reuse = s->reuse; p.fast_trig = (a->flags & CFS_FLAG_FAST_TRIG) ? 1 : 0;
     p.pick_shift = s->pick_shift; p.n_thr = s->n_thr; p.pick_steps = s->pick_steps;
     memcpy(p.T, s->T, sizeof(p.T)); memcpy(p.lut, s->lut, sizeof(p.lut));
     memcpy(p.coef, s->coef, sizeof(p.coef)); memcpy(p.pal8, s->pal8, sizeof(p.pal8));
@@ -308,35 +310,40 @@ cfs_status build_params(const cfs_system *s, const cfs_render_args *a, RenderPar
     return CFS_OK;
 }
 
-typedef void (*render_fn)(const RenderParams);
+using cfs::render_fn;
 
-template <int DIM, int GEN, int AFF>
-render_fn pick_splat(int splat)
+// chain signature after host resolution (ROTATE_Z is an AFFINE by now)
+uint32_t chain_signature(const RenderParams &p)
 {
-    switch (splat) {
-    case cfs::SPLAT_HIST_DIRECT: return cfs::render_kernel<DIM, GEN, AFF, cfs::SPLAT_HIST_DIRECT>;
-    case cfs::SPLAT_HIST_SHARED: return cfs::render_kernel<DIM, GEN, AFF, cfs::SPLAT_HIST_SHARED>;
-    case cfs::SPLAT_HIST_WARPAGG: return cfs::render_kernel<DIM, GEN, AFF, cfs::SPLAT_HIST_WARPAGG>;
-    case cfs::SPLAT_RGBA: return cfs::render_kernel<DIM, GEN, AFF, cfs::SPLAT_RGBA>;
-    case cfs::SPLAT_DEPTH:
-        if (DIM == 3) return cfs::render_kernel<3, GEN, AFF, cfs::SPLAT_DEPTH>;
-        return nullptr;
-    default: return nullptr;
+    uint32_t sig = 0;
+    for (int m = 0; m < p.n_chain; ++m) sig |= (uint32_t)(p.chain[m].type + 1) << (4 * m);
+    return sig;
+}
+
+// the kernel compiled for this chain when there is one (and the caller did not ask for the
+// interpreter), else the interpreter; both evaluate the same device functions
+render_fn pick_kernel(const cfs_system *s, const RenderParams &p, int splat, int flags)
+{
+    const int trig = (flags & CFS_FLAG_FAST_TRIG) ? cfs::TRIG_FAST : cfs::TRIG_ACCURATE;
+    if (!(flags & CFS_FLAG_INTERPRET_CHAIN) && p.n_chain > 0 && !p.reuse) {
+        const uint32_t sig = chain_signature(p);
+        render_fn fn = (s->dim == 2) ? cfs::lookup_render_static2d(s->gen, s->aff, splat, sig, trig)
+                                     : cfs::lookup_render_static3d(s->gen, s->aff, splat, sig, trig);
+        if (fn) return fn;
     }
+    return cfs::lookup_render_generic(s->dim, s->gen, s->aff, splat);
 }
 
-render_fn pick_kernel(int dim, int gen, int aff, int splat)
+render_fn pick_trace(const cfs_system *s, const RenderParams &p, int flags)
 {
-    if (gen == CFS_GEN_CLOUD) return dim == 2 ? pick_splat<2, 1, cfs::AFF_GENERAL>(splat) : pick_splat<3, 1, cfs::AFF_GENERAL>(splat);
-    if (dim == 2) return aff == cfs::AFF_DIAG ? pick_splat<2, 0, cfs::AFF_DIAG>(splat) : pick_splat<2, 0, cfs::AFF_GENERAL>(splat);
-    return aff == cfs::AFF_DIAG ? pick_splat<3, 0, cfs::AFF_DIAG>(splat) : pick_splat<3, 0, cfs::AFF_GENERAL>(splat);
-}
-
-render_fn pick_trace(int dim, int gen, int aff)
-{
-    if (gen == CFS_GEN_CLOUD) return dim == 2 ? cfs::trace_kernel<2, 1, cfs::AFF_GENERAL> : cfs::trace_kernel<3, 1, cfs::AFF_GENERAL>;
-    if (dim == 2) return aff == cfs::AFF_DIAG ? cfs::trace_kernel<2, 0, cfs::AFF_DIAG> : cfs::trace_kernel<2, 0, cfs::AFF_GENERAL>;
-    return aff == cfs::AFF_DIAG ? cfs::trace_kernel<3, 0, cfs::AFF_DIAG> : cfs::trace_kernel<3, 0, cfs::AFF_GENERAL>;
+    const int trig = (flags & CFS_FLAG_FAST_TRIG) ? cfs::TRIG_FAST : cfs::TRIG_ACCURATE;
+    if (!(flags & CFS_FLAG_INTERPRET_CHAIN) && p.n_chain > 0 && !p.reuse) {
+        const uint32_t sig = chain_signature(p);
+        render_fn fn = (s->dim == 2) ? cfs::lookup_trace_static2d(s->gen, s->aff, sig, trig)
+                                     : cfs::lookup_trace_static3d(s->gen, s->aff, sig, trig);
+        if (fn) return fn;
+    }
+    return cfs::lookup_trace_generic(s->dim, s->gen, s->aff);
 }
 
 size_t shared_hist_limit(const DeviceInfo &di)
@@ -377,7 +384,7 @@ extern "C" cfs_status cfs_render(const cfs_system *s, const cfs_render_args *a, 
             splat = cfs::SPLAT_HIST_SHARED;
     }
     if (a->n_points == 0) return CFS_OK;
-    render_fn fn = pick_kernel(s->dim, s->gen, s->aff, splat);
+    render_fn fn = pick_kernel(s, p, splat, a->flags);
     if (!fn) return fail(CFS_ERR_UNSUPPORTED, "no kernel for dim %d / splat %d", s->dim, splat);
 
     const int threads = cfs::kRenderThreads;
@@ -420,7 +427,7 @@ extern "C" cfs_status cfs_trace(const cfs_system *s, const cfs_render_args *a, u
     if (a->n_points == 0) return CFS_OK;
     p.tr_picks = d_picks; p.tr_g = d_final_g; p.tr_q = d_final_q; p.tr_alive = d_alive;
     p.counters = nullptr;
-    render_fn fn = pick_trace(s->dim, s->gen, s->aff);
+    render_fn fn = pick_trace(s, p, a->flags);
     uint64_t blocks = (a->n_points + cfs::kRenderThreads - 1) / cfs::kRenderThreads;
     if (blocks > (1u << 22)) blocks = 1u << 22;
     fn<<<(unsigned)blocks, cfs::kRenderThreads, 0, (cudaStream_t)stream>>>(p);

@@ -10,9 +10,34 @@ namespace cfs {
 
 constexpr int kMaxFuncs = 64;
 constexpr int kMaxChain = 8;
+constexpr int kRenderThreads = 256;   // CTA size of the render / trace kernels
 
 // affine table forms (bit-identical results, DESIGN R4: fma(0,y,b) == b)
 enum AffForm : int { AFF_GENERAL = 0, AFF_DIAG = 1 };
+// transcendental evaluation of the non-affine chain steps: libdevice sincosf/sinf/cosf (<= 2 ulp)
+// or the MUFU special-function unit (sin.approx/cos.approx, abs. error ~2^-21 on [-pi, pi])
+enum TrigKind : int { TRIG_ACCURATE = 0, TRIG_FAST = 1, TRIG_RUNTIME = 2 /* prm.fast_trig decides (interpreter) */ };
+// chain signature: 4 bits per step, (type + 1) of step m in bits [4m, 4m+4), 0 terminates.
+// A kernel compiled for a signature has the chain unrolled with every parameter a fixed constant
+// operand; kChainGeneric selects the interpreter (unrolled to kMaxChain steps, warp-uniform switch).
+constexpr uint32_t kChainGeneric = 0xFFFFFFFFu;
+constexpr uint32_t chain_sig(int a = -1, int b = -1, int c = -1, int d = -1)
+{
+    return (uint32_t)(a + 1) | ((uint32_t)(b + 1) << 4) | ((uint32_t)(c + 1) << 8) | ((uint32_t)(d + 1) << 12);
+}
+// true when a step of the signature evaluates sin/cos (types 1 SWIRL, 2 SINUSOIDAL, 4 TWIST_Z,
+// 5 BEND, 7 STRETCH_COS); the generic signature may
+constexpr bool sig_has_trig(uint32_t sig)
+{
+    if (sig == kChainGeneric) return true;
+    for (int m = 0; m < 8; ++m) {
+        const int code = (int)((sig >> (4 * m)) & 15u);
+        if (code == 0) break;
+        const int t = code - 1;
+        if (t == 1 || t == 2 || t == 4 || t == 5 || t == 7) return true;
+    }
+    return false;
+}
 // splat variants compiled into the render kernel
 enum SplatKind : int {
     SPLAT_HIST_DIRECT = 0,   // red.global.add.u32
@@ -43,7 +68,7 @@ struct RenderParams {
     float *tr_g, *tr_q;
     uint8_t *tr_alive;
 
-    int32_t dim, n_funcs, n_chain, color_rule, reuse;
+    int32_t dim, n_funcs, n_chain, color_rule, reuse, fast_trig;
     int32_t pick_shift;          // >= 0: k = u >> pick_shift (equal power-of-two thresholds)
     int32_t n_thr;               // thresholds below 2^32 (k = #{j < n_thr : u >= T[j]})
     int32_t pick_steps;          // max thresholds inside one 2^24 bucket of u
@@ -52,7 +77,8 @@ struct RenderParams {
 
     ChainStep chain[kMaxChain];
     uint32_t T[kMaxFuncs];       // thresholds (u32), T[j >= n_thr] = 0xFFFFFFFF
-    uint8_t lut[256];            // lut[b] = #{j < n_thr : T[j] <= b << 24}
+    uint32_t lut[256];           // lut[b] = #{j < n_thr : T[j] <= b << 24} << 25 | t24, t24 = first
+                                 // threshold inside bucket b minus (b << 24), 2^24 if none
     float coef[kMaxFuncs * 12];  // GENERAL dim2: rows of 8 (a00 a01 b0 0 | a10 a11 b1 0);
                                  // GENERAL dim3: rows of 12 (a00 a01 a02 b0 | ... );
                                  // DIAG dim2: rows of 4 (sx sy bx by); DIAG dim3: rows of 8

@@ -4,15 +4,16 @@
 // random every step"); the per-thread state is 3 floats of generator state, 3 of the copy and 4
 // Philox words ("less than ten floating-point values stored per thread").
 // Nothing but the output image is written to global memory.
+//
+// Template axes: DIM 2|3, GEN 0 = IFS / 1 = stored cloud, AFF table form, SPLAT sink, SIG chain
+// signature (kChainGeneric = interpreter, else the chain is compiled in), TRIG sin/cos evaluation.
 #pragma once
 #include "cfs_device.cuh"
 
 namespace cfs {
 
-constexpr int kRenderThreads = 256;
-
 // ---------------------------------------------------------------------------------------------
-// splat sinks (row 7).  Each returns nothing; `pix >= 0` is guaranteed by the caller.
+// splat sinks (row 7).  `pix >= 0` is guaranteed by the caller.
 __device__ __forceinline__ void red_add_v4_f32(float *addr, float a, float b, float c, float d)
 {
     asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};"
@@ -44,9 +45,76 @@ __device__ __forceinline__ void splat_depth(unsigned long long *buf, int pix, fl
     if (key < cur) atomicMin(buf + pix, key);
 }
 
+// rows 5-7 for one generated point: copy -> chain -> pixel -> reduction.  `k` is the map applied
+// in this iteration (colour rule MAP_INDEX), `point_rgba8` the record colour (POINT).
+// Returns 1 when the splat was dropped (dead or out of bounds), else 0.  Fig. 2(C) reuse is a
+// run-time option of the interpreter kernels only (compiled chains are never used with it).
+template <int DIM, int GEN, int SPLAT, uint32_t SIG, int TRIG>
+__device__ __forceinline__ uint32_t chain_and_splat(const RenderParams &prm, const SharedTables &s, uint32_t *s_hist,
+                                                    float &gx, float &gy, float &gz, int k, uint32_t point_rgba8,
+                                                    bool have, bool past_burn_in)
+{
+    float qx = gx, qy = gy, qz = gz;            // the copy of Fig. 2(B)
+    const bool alive = apply_chain<DIM, SIG, TRIG>(prm, qx, qy, qz);
+    if (SIG == kChainGeneric && prm.reuse) {    // Fig. 2(C): the same point is reused
+        gx = qx; gy = qy; gz = qz;
+        if (!past_burn_in) return 0u;
+    }
+    const bool ok = alive && have && in_bounds(prm, qx, qy);
+    if (SPLAT == SPLAT_HIST_WARPAGG) {
+        splat_hist_warpagg(reinterpret_cast<uint32_t *>(prm.image), ok ? pixel_of(prm, qx, qy) : -1, ok);
+        return (have && !ok) ? 1u : 0u;
+    }
+    if (!ok) return 1u;
+    const int pix = pixel_of(prm, qx, qy);
+    if (SPLAT == SPLAT_HIST_DIRECT) {
+        red_add_u32(reinterpret_cast<uint32_t *>(prm.image) + pix, 1u);
+    } else if (SPLAT == SPLAT_HIST_SHARED) {
+        atomicAdd(&s_hist[pix], 1u);
+    } else if (SPLAT == SPLAT_RGBA) {
+        float *dst = reinterpret_cast<float *>(prm.image) + 4 * (size_t)pix;
+        if (GEN == 1) {   // colour of the point record, integer-valued (DESIGN R9)
+            red_add_v4_f32(dst, (float)(point_rgba8 & 0xFFu), (float)((point_rgba8 >> 8) & 0xFFu),
+                           (float)((point_rgba8 >> 16) & 0xFFu), 1.0f);
+        } else {          // colour of the map applied in this iteration
+            const float4 c = s.palette[k];
+            red_add_v4_f32(dst, c.x, c.y, c.z, 1.0f);
+        }
+    } else if (SPLAT == SPLAT_DEPTH) {
+        splat_depth(reinterpret_cast<unsigned long long *>(prm.image), pix, qz,
+                    GEN == 1 ? point_rgba8 : s.pal8[k]);
+    }
+    return 0u;
+}
+
+// four iterations served by one Philox block (DESIGN R1: word it & 3 of block it >> 2).
+// CHECKED = false: the caller guarantees burn_in <= it0 and it0 + 4 <= iterations, so the body
+// has no per-iteration tests (the steady state of a render); CHECKED = true handles burn-in
+// and the ragged last block.
+template <int DIM, int GEN, int AFF, int SPLAT, uint32_t SIG, int TRIG, bool CHECKED>
+__device__ __forceinline__ uint32_t iterate_block(const RenderParams &prm, const SharedTables &s, uint32_t *s_hist,
+                                                  uint32_t plo, uint32_t phi, int it0, float &gx, float &gy, float &gz,
+                                                  bool have)
+{
+    const U4 w = philox4x32_10(plo, phi, (uint32_t)it0 >> 2, DOMAIN_PICK, prm);
+    uint32_t dropped = 0;
+#pragma unroll(CHECKED ? 1 : 4)
+    for (int j = 0; j < 4; ++j) {
+        const int it = it0 + j;
+        if (CHECKED && it >= prm.iterations) break;
+        const uint32_t u = (j == 0) ? w.x : (j == 1) ? w.y : (j == 2) ? w.z : w.w;
+        const int k = pick_index(u, s, prm);
+        apply_gen<DIM, AFF>(k, s, gx, gy, gz);
+        const bool past = !CHECKED || it >= prm.burn_in;
+        if (past || (SIG == kChainGeneric && prm.reuse))
+            dropped += chain_and_splat<DIM, GEN, SPLAT, SIG, TRIG>(prm, s, s_hist, gx, gy, gz, k, 0u, have, past);
+    }
+    return dropped;
+}
+
 // ---------------------------------------------------------------------------------------------
 // the kernel
-template <int DIM, int GEN, int AFF, int SPLAT>
+template <int DIM, int GEN, int AFF, int SPLAT, uint32_t SIG, int TRIG>
 __global__ void __launch_bounds__(kRenderThreads)
 render_kernel(const __grid_constant__ RenderParams prm)
 {
@@ -58,6 +126,7 @@ render_kernel(const __grid_constant__ RenderParams prm)
     __syncthreads();
 
     const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    const int I = prm.iterations, B = prm.burn_in;
     uint32_t n_in = 0, n_drop = 0;
 
     for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; ; i += stride) {
@@ -67,64 +136,32 @@ render_kernel(const __grid_constant__ RenderParams prm)
         else if (!have) break;
         const uint64_t p = prm.point_offset + i;
         float gx, gy, gz = 0.0f;
-        uint32_t point_rgba8 = 0;
+        uint32_t dropped = 0;
 
-        if (GEN == 1) {   // stored cloud: one coalesced 128-bit load per point (row 1)
+        if (GEN == 1) {   // stored cloud: one coalesced 128-bit load per point (row 1), one splat
             float4 rec = make_float4(0.f, 0.f, 0.f, 0.f);
             if (have) rec = __ldcs(reinterpret_cast<const float4 *>(prm.cloud) + p);
             gx = rec.x; gy = rec.y; gz = (DIM == 3) ? rec.z : 0.0f;
-            point_rgba8 = __float_as_uint(rec.w);
+            dropped = chain_and_splat<DIM, GEN, SPLAT, SIG, TRIG>(prm, s, s_hist, gx, gy, gz, 0,
+                                                                  __float_as_uint(rec.w), have, true);
         } else {
-            const U4 w = philox4x32_10((uint32_t)p, (uint32_t)(p >> 32), 0u, DOMAIN_INIT, prm);
-            gx = u24_to_pm1(w.x);
-            gy = u24_to_pm1(w.y);
-            if (DIM == 3) gz = u24_to_pm1(w.z);
-        }
-
-        U4 w = {0, 0, 0, 0};
-        for (int it = 0; it < prm.iterations; ++it) {
-            int k = 0;
-            if (GEN == 0) {
-                if ((it & 3) == 0)
-                    w = philox4x32_10((uint32_t)p, (uint32_t)(p >> 32), (uint32_t)it >> 2, DOMAIN_PICK, prm);
-                const uint32_t u = w.x;
-                w.x = w.y; w.y = w.z; w.z = w.w;        // word it&3 rotates into .x
-                k = pick_index(u, s, prm);
-                apply_gen<DIM, AFF>(k, s, gx, gy, gz);
+            const uint32_t plo = (uint32_t)p, phi = (uint32_t)(p >> 32);
+            {
+                const U4 w = philox4x32_10(plo, phi, 0u, DOMAIN_INIT, prm);
+                gx = u24_to_pm1(w.x);
+                gy = u24_to_pm1(w.y);
+                if (DIM == 3) gz = u24_to_pm1(w.z);
             }
-            if (it < prm.burn_in && !prm.reuse) continue;
-            float qx = gx, qy = gy, qz = gz;            // the copy of Fig. 2(B)
-            const bool alive = apply_chain<DIM>(prm, qx, qy, qz);
-            if (prm.reuse) {                            // Fig. 2(C): the same point is reused
-                gx = qx; gy = qy; gz = qz;
-                if (it < prm.burn_in) continue;
-            }
-            const int pix = (alive && have) ? pixel_index(prm, qx, qy) : -1;
-            if (SPLAT == SPLAT_HIST_WARPAGG) {
-                splat_hist_warpagg(reinterpret_cast<uint32_t *>(prm.image), pix, pix >= 0);
-                if (have) { if (pix >= 0) ++n_in; else ++n_drop; }
-                continue;
-            }
-            if (pix < 0) { ++n_drop; continue; }
-            ++n_in;
-            if (SPLAT == SPLAT_HIST_DIRECT) {
-                red_add_u32(reinterpret_cast<uint32_t *>(prm.image) + pix, 1u);
-            } else if (SPLAT == SPLAT_HIST_SHARED) {
-                atomicAdd(&s_hist[pix], 1u);
-            } else if (SPLAT == SPLAT_RGBA) {
-                float *dst = reinterpret_cast<float *>(prm.image) + 4 * (size_t)pix;
-                if (GEN == 1) {   // colour of the point record, integer-valued (DESIGN R9)
-                    red_add_v4_f32(dst, (float)(point_rgba8 & 0xFFu), (float)((point_rgba8 >> 8) & 0xFFu),
-                                   (float)((point_rgba8 >> 16) & 0xFFu), 1.0f);
-                } else {          // colour of the map applied in this iteration
-                    const float4 c = s.palette[k];
-                    red_add_v4_f32(dst, c.x, c.y, c.z, 1.0f);
-                }
-            } else if (SPLAT == SPLAT_DEPTH) {
-                splat_depth(reinterpret_cast<unsigned long long *>(prm.image), pix, qz,
-                            GEN == 1 ? point_rgba8 : s.pal8[k]);
+            // blocks touching burn-in or the ragged end take the checked path, the rest the lean one
+            const int it_fast0 = min((B + 3) & ~3, I & ~3), it_fast1 = I & ~3;
+            for (int it0 = 0; it0 < I; it0 += 4) {
+                if (it0 >= it_fast0 && it0 < it_fast1)
+                    dropped += iterate_block<DIM, GEN, AFF, SPLAT, SIG, TRIG, false>(prm, s, s_hist, plo, phi, it0, gx, gy, gz, have);
+                else
+                    dropped += iterate_block<DIM, GEN, AFF, SPLAT, SIG, TRIG, true>(prm, s, s_hist, plo, phi, it0, gx, gy, gz, have);
             }
         }
+        if (have) { n_drop += dropped; n_in += (uint32_t)(I - B) - dropped; }
     }
 
     if (SPLAT == SPLAT_HIST_SHARED) {   // merge the private histogram (red.global, non-zero bins only)
@@ -155,7 +192,7 @@ render_kernel(const __grid_constant__ RenderParams prm)
 
 // ---------------------------------------------------------------------------------------------
 // parity instrument: same device functions, records instead of splatting (SURVEY 8(c) S10 i, ii)
-template <int DIM, int GEN, int AFF>
+template <int DIM, int GEN, int AFF, uint32_t SIG, int TRIG>
 __global__ void __launch_bounds__(kRenderThreads)
 trace_kernel(const __grid_constant__ RenderParams prm)
 {
@@ -190,7 +227,7 @@ trace_kernel(const __grid_constant__ RenderParams prm)
             }
             if (it < prm.burn_in && !prm.reuse) continue;
             qx = gx; qy = gy; qz = gz;
-            alive = apply_chain<DIM>(prm, qx, qy, qz);
+            alive = apply_chain<DIM, SIG, TRIG>(prm, qx, qy, qz);
             if (prm.reuse) { gx = qx; gy = qy; gz = qz; }
         }
         if (prm.tr_g) { prm.tr_g[3 * i] = gx; prm.tr_g[3 * i + 1] = gy; prm.tr_g[3 * i + 2] = gz; }

@@ -6,7 +6,7 @@ import numpy as np
 
 
 def gpu_render(cfs, w, t=None, cloud=None, variant="auto", n_points=None, point_offset=None, image=None,
-               want_counters=True):
+               want_counters=True, flags=0):
     """cfs_render through the binding. Returns (numpy image, counters[2])."""
     import torch
     sysh = cfs.cfs_create(w.system)
@@ -14,7 +14,7 @@ def gpu_render(cfs, w, t=None, cloud=None, variant="auto", n_points=None, point_
     ctr = torch.zeros(2, dtype=torch.int64, device="cuda") if want_counters else None
     d_cloud = cfs.cloud_to_device(cloud) if cloud is not None else None
     args = cfs.make_args(w.render, d_image=img, d_cloud=d_cloud, d_counters=ctr, t=t, variant=variant,
-                         n_points=n_points, point_offset=point_offset)
+                         n_points=n_points, point_offset=point_offset, flags=flags)
     cfs.cfs_render(sysh, args)
     torch.cuda.synchronize()
     out = cfs.image_to_numpy(img, w.render.out_mode)
@@ -23,7 +23,7 @@ def gpu_render(cfs, w, t=None, cloud=None, variant="auto", n_points=None, point_
     return out, c
 
 
-def gpu_trace(cfs, w, t=None, cloud=None, n_points=None, point_offset=None):
+def gpu_trace(cfs, w, t=None, cloud=None, n_points=None, point_offset=None, flags=0):
     import torch
     n = int(w.render.n_points if n_points is None else n_points)
     I = int(w.render.iterations)
@@ -33,7 +33,7 @@ def gpu_trace(cfs, w, t=None, cloud=None, n_points=None, point_offset=None):
     fq = torch.zeros((n, 3), dtype=torch.float32, device="cuda")
     al = torch.zeros(n, dtype=torch.uint8, device="cuda")
     d_cloud = cfs.cloud_to_device(cloud) if cloud is not None else None
-    args = cfs.make_args(w.render, d_cloud=d_cloud, t=t, n_points=n_points, point_offset=point_offset)
+    args = cfs.make_args(w.render, d_cloud=d_cloud, t=t, n_points=n_points, point_offset=point_offset, flags=flags)
     cfs.cfs_trace(sysh, args, picks, fg, fq, al)
     torch.cuda.synchronize()
     sysh.close()

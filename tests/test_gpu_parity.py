@@ -155,6 +155,55 @@ def test_cfg3_cloud(cfs, oracle):
     assert np.array_equal(a + b, g)                                  # integer-valued sums: exact
 
 
+# ------------------------------------------------------------------ compiled chains, interpreter, fast sin/cos
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4])
+def test_compiled_chain_equals_interpreter(cfs, oracle, cfg):
+    """A kernel compiled for the chain's signature and the chain interpreter evaluate the same device
+    functions: traces and images are bit-identical (integer-valued colour sums are order-free)."""
+    w = W.config(cfg)
+    n = 3000 + 77
+    cloud = _cloud_for(w, n)
+    w = w.scaled(n_points=n, iterations=min(w.render.iterations, 150), width=640, height=360)
+    t = w.frames[len(w.frames) // 2]
+    a = gpu_trace(cfs, w, t=t, cloud=cloud)
+    b = gpu_trace(cfs, w, t=t, cloud=cloud, flags=["interpret_chain"])
+    for x, y in zip(a, b):
+        assert np.array_equal(x, y)
+    ga, ca = gpu_render(cfs, w, t=t, cloud=cloud)
+    gb, cb = gpu_render(cfs, w, t=t, cloud=cloud, flags=["interpret_chain"])
+    assert np.array_equal(ga, gb) and np.array_equal(ca, cb)
+    o, oc, _ = oracle.render_parallel(w.system, w.render, cloud=cloud, t=t)
+    if cfg == 4:
+        assert np.array_equal(ga, o) and np.array_equal(ca, oc)
+    else:
+        for ch in range(4):
+            assert density_l1(ga[:, ch], o[:, ch]) <= 4e-3      # < 500k splats: a handful of edge flips
+
+
+@pytest.mark.parametrize("interp", [False, True])
+@pytest.mark.parametrize("cfg", [1, 2, 3])
+def test_fast_trig_within_tolerance(cfs, oracle, cfg, interp):
+    """CFS_FLAG_FAST_TRIG (MUFU sin/cos): pick sequences unchanged, coordinates within 1e-4 of the
+    oracle (BASELINE north_star), density L1 within 1e-3."""
+    flags = ["fast_trig"] + (["interpret_chain"] if interp else [])
+    w = W.config(cfg)
+    n = (1 << 14) + 5 if cfg != 3 else (1 << 18) + 11
+    cloud = _cloud_for(w, n)
+    w = w.scaled(n_points=n)
+    t = w.frames[len(w.frames) // 2]
+    nt = 1024 + 37
+    gp, gg, gq, ga = gpu_trace(cfs, w, t=t, cloud=cloud, n_points=nt, flags=flags)
+    op, og, oq, oa = oracle.trace(w.system, w.scaled(n_points=nt).render, cloud=cloud, t=t)
+    assert np.array_equal(gp, op) and np.array_equal(gg, og) and np.array_equal(ga, oa)
+    live = oa.astype(bool)
+    assert np.abs(gq[live].astype(np.float64) - oq[live]).max() <= COORD_TOL
+    g, gc = gpu_render(cfs, w, t=t, cloud=cloud, flags=flags)
+    o, oc, _ = oracle.render_parallel(w.system, w.render, cloud=cloud, t=t)
+    assert int(gc[0]) + int(gc[1]) == int(oc[0]) + int(oc[1]) and abs(int(gc[0]) - int(oc[0])) <= 4
+    for ch in range(4):
+        assert density_l1(g[:, ch], o[:, ch]) <= L1_TOL
+
+
 # ------------------------------------------------------------------ general tables and edge cases
 def test_general_pick_and_general_affine(cfs, oracle):
     """Non-uniform probabilities incl. zero-probability maps (table + compare pick), non-diagonal
