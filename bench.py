@@ -213,7 +213,18 @@ def roofline_for(cfg, w, rates, peaks, splats, seconds):
             "t_roof_ms": t_roof * 1e3, "t_ms": seconds * 1e3, "frac": t_roof / seconds}
 
 
-def time_workload(cfs, torch, cfg, flush, reps=5, flags=0):
+SCRATCH_CAP_BYTES = 8 << 30
+
+
+def make_scratch(cfs, torch, sysh, render):
+    """Scratch of the tile-binned variant (None when the variant cannot serve the workload)."""
+    need = cfs.cfs_binned_scratch_bytes(sysh, cfs.make_args(render))
+    if need == 0:
+        return None
+    return torch.empty(min(need, SCRATCH_CAP_BYTES), dtype=torch.uint8, device="cuda")
+
+
+def time_workload(cfs, torch, cfg, flush, reps=5, flags=0, variant="auto"):
     """Median device time of one cfs_render of configs[cfg] (all frames for cfg 2)."""
     w = W.config(cfg)
     cloud = W.gaussian_mixture_cloud(w.render.n_points, w.cloud_seed) if w.system.gen == "cloud" else None
@@ -221,6 +232,7 @@ def time_workload(cfs, torch, cfg, flush, reps=5, flags=0):
     sysh = cfs.cfs_create(w.system)
     img = cfs.new_image(w.render)
     ctr = torch.zeros(2, dtype=torch.int64, device="cuda")
+    scratch = make_scratch(cfs, torch, sysh, w.render) if variant != "direct" else None
     times = []
     n_rep = reps if cfg != 4 else 3
     for rep in range(n_rep + 2):
@@ -229,7 +241,8 @@ def time_workload(cfs, torch, cfg, flush, reps=5, flags=0):
         ctr.zero_()
         for t in w.frames:
             img.fill_(-1 if w.render.out_mode == "depth_u64" else 0)
-            args = cfs.make_args(w.render, d_image=img, d_cloud=d_cloud, d_counters=ctr, t=t, flags=flags)
+            args = cfs.make_args(w.render, d_image=img, d_cloud=d_cloud, d_counters=ctr, t=t, flags=flags,
+                                 variant=variant, d_scratch=scratch)
             e0, e1 = event_pair(torch)
             e0.record()
             cfs.cfs_render(sysh, args)
@@ -278,7 +291,9 @@ def run_ours(args):
     flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device="cuda")
     # weak scaling: every rank renders its own P points of the global point-id space
     flags = ["fast_trig"] if args.fast_trig else 0
-    rargs = cfs.make_args(r, d_image=img, d_counters=ctr, point_offset=rank * P, flags=flags)
+    scratch_t = make_scratch(cfs, torch, sysh, r) if args.variant != "direct" else None
+    rargs = cfs.make_args(r, d_image=img, d_counters=ctr, point_offset=rank * P, flags=flags, variant=args.variant,
+                          d_scratch=scratch_t)
 
     def step(timed):
         flush.zero_()                         # L2 flush, outside the events
@@ -380,7 +395,7 @@ def run_ours(args):
     if not args.no_workloads and world == 1:
         wl = {}
         for cfg in range(W.N_CONFIGS):
-            wk, sec, n_in, n_drop = time_workload(cfs, torch, cfg, flush, flags=flags)
+            wk, sec, n_in, n_drop = time_workload(cfs, torch, cfg, flush, flags=flags, variant=args.variant)
             pi = wk.point_iterations
             rf = roofline_for(cfg, wk, rates, peaks, n_in / len(wk.frames), sec / len(wk.frames))
             wl[f"cfg{cfg}"] = {"name": wk.name, "ms": sec * 1e3, "point_iterations_per_s": pi / sec,
@@ -418,8 +433,9 @@ def run_profile_cfg(args):
     img = cfs.new_image(w.render)
     ctr = torch.zeros(2, dtype=torch.int64, device="cuda")
     t = w.frames[len(w.frames) // 2]
+    scratch = make_scratch(cfs, torch, sysh, w.render) if args.variant in ("auto", "binned") else None
     rargs = cfs.make_args(w.render, d_image=img, d_cloud=d_cloud, d_counters=ctr, t=t, variant=args.variant,
-                          flags=["fast_trig"] if args.fast_trig else 0)
+                          flags=["fast_trig"] if args.fast_trig else 0, d_scratch=scratch)
     ms = []
     for i in range(2 + args.steps):
         img.fill_(-1 if w.render.out_mode == "depth_u64" else 0)
@@ -444,7 +460,7 @@ def main():
     ap.add_argument("--no-workloads", action="store_true", help="skip the per-config side report")
     ap.add_argument("--profile-cfg", type=int, default=None,
                     help="only launch cfs_render of configs[N] --steps times (ncu target; no bench line)")
-    ap.add_argument("--variant", default="auto", help="splat variant for --profile-cfg")
+    ap.add_argument("--variant", default="auto", help="splat variant: auto (tile bins for large renders, else direct), direct, binned, ...")
     ap.add_argument("--fast-trig", action="store_true", help="CFS_FLAG_FAST_TRIG (MUFU sin/cos) on every render")
     args = ap.parse_args()
     global SINCOS

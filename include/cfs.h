@@ -85,7 +85,11 @@ typedef enum {
     CFS_VARIANT_DIRECT = 1,      /* one L2 reduction per splat (red.global / atom.global.min.u64)     */
     CFS_VARIANT_SHARED_HIST = 2, /* HIST only, W*H*4 <= cfs_shared_hist_max_bytes(): per-CTA shared   */
                                  /* histogram, merged with red.global                                 */
-    CFS_VARIANT_WARP_AGG = 3     /* DIRECT + __match_any_sync aggregation of same-pixel hits (HIST)   */
+    CFS_VARIANT_WARP_AGG = 3,    /* DIRECT + __match_any_sync aggregation of same-pixel hits (HIST)   */
+    CFS_VARIANT_BINNED = 4       /* HIST, or RGBA + MAP_INDEX with <= 16 functions, IFS generator:    */
+                                 /* splats are partitioned by image tile through d_scratch (one       */
+                                 /* 4-byte record each), then every tile is accumulated in shared     */
+                                 /* memory and merged with red.global; no L2 atomic per splat         */
 } cfs_variant;
 
 /* render flags.
@@ -128,12 +132,22 @@ typedef struct {
     void *d_image;          /* device, caller-owned, caller-cleared, accumulates                */
     const void *d_cloud;    /* device, CLOUD only: record p of the WHOLE cloud is d_cloud[p]    */
     uint64_t *d_counters;   /* optional device u64[2]: += in-bounds splats, += dropped splats   */
+    void *d_scratch;        /* optional device scratch of the BINNED variant, caller-owned; its  */
+    uint64_t scratch_bytes; /* contents are garbage afterwards.  cfs_binned_scratch_bytes() is    */
+                            /* what renders all points in one chunk; less means more chunks       */
 } cfs_render_args;
 
-/* cfs_render -- the hot path: sampler + pick + map + chain + colour + splat, one kernel launch.
+/* cfs_render -- the hot path: sampler + pick + map + chain + colour + splat, one kernel launch
+ * (BINNED: a memset and two launches per chunk of points).
  * Errors: INVALID_ARG, UNSUPPORTED (variant impossible for the mode
  * or image), CUDA (launch failure; message holds the CUDA error string). */
 cfs_status cfs_render(const cfs_system *sys, const cfs_render_args *args, void *cuda_stream);
+
+/* bytes of d_scratch with which CFS_VARIANT_BINNED renders args->n_points in ONE chunk (pass 1 +
+ * pass 2); 0 when the variant cannot serve this system / output mode / image, or without a device.
+ * With scratch memory given, CFS_VARIANT_AUTO takes the binned path for large renders it can serve
+ * (at least one 1024-point CTA per SM and 2^27 splats) and the direct path otherwise. */
+uint64_t cfs_binned_scratch_bytes(const cfs_system *sys, const cfs_render_args *args);
 
 /* cfs_render_host -- same path with HOST buffers (end-to-end entry point): copies h_cloud to the
  * device (CLOUD), clears a device image, renders [point_offset, +n_points), copies the image to

@@ -23,11 +23,11 @@ T_TYPE = {"affine": 0, "swirl": 1, "sinusoidal": 2, "rotate_z": 3, "twist_z": 4,
 COLOR = {"none": 0, "map_index": 1, "point": 2}
 OUT = {"hist_u32": 0, "rgba_f32": 1, "depth_u64": 2}
 FLAGS = {"fast_trig": 1, "interpret_chain": 2}
-VARIANT = {"auto": 0, "direct": 1, "shared_hist": 2, "warp_agg": 3}
+VARIANT = {"auto": 0, "direct": 1, "shared_hist": 2, "warp_agg": 3, "binned": 4}
 MB = {"red_add_u32": 0, "red_add_v4f32": 1, "atom_min_u64": 2, "ld_u64": 3, "atoms_add_u32": 4,
       "ffma": 5, "imad_wide": 6, "lop3": 7, "mufu": 8, "stream_ld128": 9}
 EXPORTS = ["cfs_create", "cfs_destroy", "cfs_render", "cfs_render_host", "cfs_tonemap", "cfs_trace",
-           "cfs_microbench", "cfs_shared_hist_max_bytes", "cfs_launch_count", "cfs_last_error",
+           "cfs_microbench", "cfs_shared_hist_max_bytes", "cfs_binned_scratch_bytes", "cfs_launch_count", "cfs_last_error",
            "cfs_version"]
 
 
@@ -52,7 +52,8 @@ class cfs_render_args(C.Structure):
                 ("xmin", C.c_float), ("xmax", C.c_float), ("ymin", C.c_float), ("ymax", C.c_float),
                 ("t", C.c_float), ("out_mode", C.c_int32), ("variant", C.c_int32),
                 ("flags", C.c_int32),
-                ("d_image", C.c_void_p), ("d_cloud", C.c_void_p), ("d_counters", C.c_void_p)]
+                ("d_image", C.c_void_p), ("d_cloud", C.c_void_p), ("d_counters", C.c_void_p),
+                ("d_scratch", C.c_void_p), ("scratch_bytes", C.c_uint64)]
 
 
 _lib = None
@@ -87,6 +88,8 @@ def lib():
         L.cfs_microbench.restype = C.c_int
         L.cfs_shared_hist_max_bytes.argtypes = []
         L.cfs_shared_hist_max_bytes.restype = C.c_uint64
+        L.cfs_binned_scratch_bytes.argtypes = [C.c_void_p, C.POINTER(cfs_render_args)]
+        L.cfs_binned_scratch_bytes.restype = C.c_uint64
         L.cfs_launch_count.argtypes = [C.c_int32]
         L.cfs_launch_count.restype = C.c_uint64
         L.cfs_last_error.argtypes = []
@@ -186,7 +189,7 @@ def cfs_create(system) -> System:
 
 
 def make_args(render, d_image=None, d_cloud=None, d_counters=None, n_points=None, point_offset=None,
-              t=None, variant="auto", flags=0) -> cfs_render_args:
+              t=None, variant="auto", flags=0, d_scratch=None) -> cfs_render_args:
     a = cfs_render_args()
     a.n_points = int(render.n_points if n_points is None else n_points)
     a.point_offset = int(render.point_offset if point_offset is None else point_offset)
@@ -203,7 +206,13 @@ def make_args(render, d_image=None, d_cloud=None, d_counters=None, n_points=None
     a.d_image = _ptr(d_image)
     a.d_cloud = _ptr(d_cloud)
     a.d_counters = _ptr(d_counters)
+    a.d_scratch = _ptr(d_scratch)
+    a.scratch_bytes = 0 if d_scratch is None else int(d_scratch.numel() * d_scratch.element_size())
     return a
+
+
+def cfs_binned_scratch_bytes(sys: System, args: cfs_render_args) -> int:
+    return int(lib().cfs_binned_scratch_bytes(sys.handle, C.byref(args)))
 
 
 def cfs_render(sys: System, args: cfs_render_args, stream=None) -> None:

@@ -10,6 +10,7 @@
 #include <vector>
 
 #include "../../include/cfs.h"
+#include "cfs_bin.cuh"
 #include "cfs_device.cuh"
 #include "cfs_microbench.cuh"
 #include "cfs_registry.h"
@@ -77,6 +78,7 @@ struct cfs_system {
     void *d_image = nullptr; size_t image_bytes = 0;
     void *d_cloud = nullptr; size_t cloud_bytes = 0;
     unsigned long long *d_counters = nullptr;
+    void *d_scratch = nullptr; size_t scratch_bytes = 0;
 };
 
 namespace {
@@ -220,6 +222,7 @@ extern "C" void cfs_destroy(cfs_system *s)
     if (s->d_image) cudaFree(s->d_image);
     if (s->d_cloud) cudaFree(s->d_cloud);
     if (s->d_counters) cudaFree(s->d_counters);
+    if (s->d_scratch) cudaFree(s->d_scratch);
     delete s;
 }
 
@@ -354,34 +357,225 @@ size_t shared_hist_limit(const DeviceInfo &di)
 
 }  // namespace
 
+// ---- tile-binned variant: plan (tiles, staging rows, scratch layout, chunking) -------------------
+namespace {
+
+struct BinPlan {
+    cfs::BinParams bp;         // pointers filled from the scratch buffer
+    size_t smem_pass1, smem_pass2;
+    uint32_t grid1;            // persistent CTAs of pass 1
+    uint64_t chunk_points;     // points per (pass 1, pass 2) pair
+    size_t clear_bytes;        // ctrl + tile_n at the start of the scratch: zeroed per chunk
+};
+
+constexpr size_t kBinCtrlBytes = 256;
+constexpr size_t kBinBlockBytes = cfs::kBinBlockRecords * 4;
+
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+// tiles and staging rows; false when the variant cannot serve this system / image
+bool bin_shape(const cfs_system *s, const cfs_render_args *a, const DeviceInfo &di, BinPlan *pl, const char **why)
+{
+    if (s->gen != CFS_GEN_IFS) { *why = "binned variant needs an IFS generator"; return false; }
+    if (a->out_mode == CFS_OUT_DEPTH_RGBA8_U64) { *why = "binned variant serves HIST and RGBA output"; return false; }
+    uint32_t kbits = 0;
+    if (a->out_mode == CFS_OUT_RGBA_F32) {
+        if (s->color != CFS_COLOR_MAP_INDEX) { *why = "binned RGBA needs COLOR_MAP_INDEX"; return false; }
+        while ((1u << kbits) < (uint32_t)s->funcs.size()) ++kbits;
+        if (kbits > 4) { *why = "binned RGBA supports at most 16 functions"; return false; }
+    }
+    const uint64_t n_pix = (uint64_t)a->width * a->height;
+    if (n_pix > (1ull << 28)) { *why = "binned variant serves images up to 2^28 pixels"; return false; }
+    // pass 2 keeps (pixels per tile) << kbits counters in shared memory: at most 3 * 2^14 (192 KiB).
+    // Fewer, larger tiles leave longer staging rows in pass 1, hence fewer barriers; but at least
+    // 64 tiles so that one tile's arrivals per iteration stay small against a row.
+    int shift = 14 - (int)kbits;
+    uint32_t mul = 3;
+    auto tiles_for = [&](int sh, uint32_t m) { const uint64_t tp = (uint64_t)m << sh; return (n_pix + tp - 1) / tp; };
+    while (tiles_for(shift, mul) < 64 && (shift > 8 || mul == 3)) {
+        if (mul == 3) { mul = 1; ++shift; } else { mul = 3; shift -= 2; }     // 3*2^s -> 2^(s+1) -> 3*2^(s-1) ...
+    }
+    const uint64_t n_tiles = tiles_for(shift, mul);
+    if (n_tiles > (uint64_t)cfs::kBinThreads) { *why = "image has too many tiles for the binned variant"; return false; }
+    // pass 1 staging: cnt + rows of `cap` records per tile, next to the static tables
+    const long budget = (long)di.smem_optin - (long)sizeof(cfs::SharedTables) - 2048;
+    const long words = budget / 4 - (long)n_tiles - 4;
+    long cap = words / (long)n_tiles / 32 * 32;
+    if (cap > 1024) cap = 1024;
+    if (cap < 160) { *why = "image has too many tiles for the binned variant's staging rows"; return false; }
+    cfs::BinParams &b = pl->bp;
+    memset(&b, 0, sizeof(b));
+    b.n_tiles = (uint32_t)n_tiles; b.tile_pixels = mul << shift;
+    b.kbits = kbits; b.cap = (uint32_t)cap;
+    // division by tile_pixels as multiply-high + shift, exact for every pixel index of this image
+    {
+        const uint64_t d = b.tile_pixels;
+        bool found = false;
+        for (uint32_t l = 0; l < 32 && !found; ++l) {
+            const unsigned __int128 pw = (unsigned __int128)1 << (32 + l);
+            const unsigned __int128 m = (pw + d - 1) / d;
+            if (m >> 32) continue;
+            if ((unsigned __int128)n_pix * (m * d - pw) < pw) { b.magic = (uint32_t)m; b.mshift = l; found = true; }
+        }
+        if (!found) { *why = "no exact tile division for this image size"; return false; }
+    }
+    // flush check every E iterations, E the largest power of two whose expected arrivals per row
+    // (with 50 % + 32 records of slack) fit above a nearly full flush unit
+    const double per_it = (double)cfs::kBinThreads / (double)n_tiles;
+    const double room = (double)(cap - (long)cfs::kBinFlushRecords + 1);
+    uint32_t every = 32;
+    while (every > 4 && 1.5 * every * per_it + 32.0 > room) every >>= 1;
+    b.check_mask = every / 4 - 1;                      // in Philox blocks of 4 iterations
+    b.split = (uint32_t)((4 * (uint64_t)di.sms + n_tiles - 1) / n_tiles);
+    if (b.split < 1) b.split = 1;
+    pl->smem_pass1 = ((n_tiles + 3) / 4 * 4 + n_tiles * (size_t)cap) * 4;
+    pl->smem_pass2 = ((size_t)b.tile_pixels << kbits) * 4;
+    pl->grid1 = (uint32_t)di.sms;
+    return true;
+}
+
+// list capacity per (tile, pass-1 CTA): four times the even share of the pool
+uint64_t bin_lcap(const BinPlan &pl, uint64_t nb) { return 4 * nb / ((uint64_t)pl.bp.n_tiles * pl.grid1) + 8; }
+
+size_t bin_fixed_bytes(const BinPlan &pl)
+{
+    return kBinCtrlBytes + align_up((size_t)pl.bp.n_tiles * pl.grid1 * 4, 256) + 1024;
+}
+
+// scratch needed to render `points` points in one chunk
+uint64_t bin_scratch_for(const BinPlan &pl, uint64_t points, uint64_t splats_per_point)
+{
+    const uint64_t rec = points * splats_per_point;
+    // every (CTA, tile) holds one prefetched and one partial block; 12.5 % head-room for uneven tiles
+    const uint64_t nb = rec / cfs::kBinBlockRecords * 9 / 8 + 4 * ((uint64_t)pl.grid1 * pl.bp.n_tiles + 64);
+    return bin_fixed_bytes(pl) + align_up((size_t)((uint64_t)pl.bp.n_tiles * pl.grid1 * bin_lcap(pl, nb)) * 4, 256) +
+           nb * kBinBlockBytes + 1024;
+}
+
+// carve the scratch buffer; false when it is too small for even one wave of points
+bool bin_layout(BinPlan *pl, void *scratch, uint64_t bytes, uint64_t n_points, uint64_t splats_per_point, const char **why)
+{
+    cfs::BinParams &b = pl->bp;
+    uint8_t *base = (uint8_t *)align_up((size_t)scratch, 512);
+    if ((size_t)(base - (uint8_t *)scratch) >= bytes) { *why = "scratch too small"; return false; }
+    bytes -= (size_t)(base - (uint8_t *)scratch);
+    const uint64_t pairs = (uint64_t)pl->grid1 * b.n_tiles;
+    const size_t fixed = bin_fixed_bytes(*pl) + 32 * pairs + 1024;      // + the "+ 8" list entries of every pair
+    if (bytes <= fixed) { *why = "scratch too small"; return false; }
+    // per block: 2 KiB of records + 16 B of list capacity
+    uint64_t nb = (bytes - fixed) / (kBinBlockBytes + 16);
+    if (nb > (1u << 23) - 1) nb = (1u << 23) - 1;                 // record positions are 32-bit
+    const uint64_t partial = 2 * (pairs + 64);
+    if (nb < partial + partial / 2) { *why = "scratch too small for the binned variant (two blocks per CTA and tile)"; return false; }
+    const uint64_t lcap = bin_lcap(*pl, nb);
+    b.nb = (uint32_t)nb; b.lcap = (uint32_t)lcap; b.grid = pl->grid1;
+    b.ctrl = (uint32_t *)base;
+    b.tails = (uint32_t *)(base + kBinCtrlBytes);
+    uint8_t *q = base + kBinCtrlBytes + align_up((size_t)pairs * 4, 256);
+    pl->clear_bytes = (size_t)(q - base);
+    b.list = (uint32_t *)q;  q += align_up((size_t)(pairs * lcap) * 4, 256);
+    b.pool = (uint32_t *)align_up((size_t)q, 512);
+    // records one chunk may produce: the blocks left after the prefetched / partial ones, with head-room
+    const uint64_t rec_cap = (nb - partial) * 8 / 9 * cfs::kBinBlockRecords;
+    uint64_t cp = rec_cap / splats_per_point;
+    const uint64_t wave = (uint64_t)pl->grid1 * cfs::kBinThreads;
+    if (cp >= wave) cp = cp / wave * wave;                      // whole waves: no ragged trip inside a chunk
+    if (cp < cfs::kBinThreads) { *why = "scratch too small for one CTA of points"; return false; }
+    if (cp > n_points) cp = n_points;
+    pl->chunk_points = cp;
+    return true;
+}
+
+}  // namespace
+
+extern "C" uint64_t cfs_binned_scratch_bytes(const cfs_system *s, const cfs_render_args *a)
+{
+    const DeviceInfo &di = device_info();
+    if (!s || !a || di.ok != 1 || a->iterations <= a->burn_in || a->width < 1 || a->height < 1) return 0;
+    BinPlan pl;
+    const char *why = "";
+    if (!bin_shape(s, a, di, &pl, &why)) return 0;
+    return bin_scratch_for(pl, a->n_points, (uint64_t)(a->iterations - a->burn_in));
+}
+
 extern "C" uint64_t cfs_shared_hist_max_bytes(void)
 {
     const DeviceInfo &di = device_info();
     return di.ok == 1 ? shared_hist_limit(di) : 0;
 }
 
+namespace {
+
+// tile-binned render: per chunk of points, clear the bin heads, pass 1 (sample + bin), pass 2
+// (accumulate tiles in shared memory, merge).  `force`: the caller asked for this variant, so
+// report why it cannot run; otherwise return UNSUPPORTED quietly and let AUTO fall back.
+cfs_status render_binned(const cfs_system *s, const cfs_render_args *a, RenderParams &p, const DeviceInfo &di, cudaStream_t st)
+{
+    BinPlan pl;
+    const char *why = "";
+    if (!bin_shape(s, a, di, &pl, &why)) return fail(CFS_ERR_UNSUPPORTED, "%s", why);
+    if (!a->d_scratch) return fail(CFS_ERR_UNSUPPORTED, "binned variant needs d_scratch (see cfs_binned_scratch_bytes)");
+    const uint64_t spp = (uint64_t)(a->iterations - a->burn_in);
+    if (!bin_layout(&pl, a->d_scratch, a->scratch_bytes, a->n_points, spp, &why)) return fail(CFS_ERR_UNSUPPORTED, "%s", why);
+    render_fn fn1 = pick_kernel(s, p, cfs::SPLAT_BIN, a->flags);
+    if (!fn1) return fail(CFS_ERR_UNSUPPORTED, "no binned kernel for dim %d", s->dim);
+    render_fn fn2 = (a->out_mode == CFS_OUT_HIST_U32) ? cfs::bin_accumulate_kernel<0> : cfs::bin_accumulate_kernel<1>;
+    cudaError_t e;
+    if ((e = cudaFuncSetAttribute((const void *)fn1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem_pass1)) != cudaSuccess)
+        return cuda_fail(e, "cudaFuncSetAttribute(pass 1)");
+    if ((e = cudaFuncSetAttribute((const void *)fn2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem_pass2)) != cudaSuccess)
+        return cuda_fail(e, "cudaFuncSetAttribute(pass 2)");
+    p.bin = pl.bp;
+    const uint64_t total = a->n_points, first = a->point_offset;
+    for (uint64_t done = 0; done < total; done += pl.chunk_points) {
+        const uint64_t n = (total - done < pl.chunk_points) ? total - done : pl.chunk_points;
+        p.n_points = n;
+        p.point_offset = first + done;
+        if ((e = cudaMemsetAsync(pl.bp.ctrl, 0, pl.clear_bytes, st)) != cudaSuccess) return cuda_fail(e, "clear bin heads");
+        // always the full persistent grid: pass 2 reads the tail word of every (tile, CTA)
+        fn1<<<pl.grid1, cfs::kBinThreads, pl.smem_pass1, st>>>(p);
+        fn2<<<pl.bp.n_tiles * pl.bp.split, cfs::kBinThreads, pl.smem_pass2, st>>>(p);
+        g_launches += 2;
+        if ((e = cudaGetLastError()) != cudaSuccess) return cuda_fail(e, "binned render launch");
+    }
+    return CFS_OK;
+}
+
+}  // namespace
+
 extern "C" cfs_status cfs_render(const cfs_system *s, const cfs_render_args *a, void *stream)
 {
     RenderParams p;
     cfs_status st = build_params(s, a, &p, true);
     if (st != CFS_OK) return st;
-    if (a->variant < CFS_VARIANT_AUTO || a->variant > CFS_VARIANT_WARP_AGG) return fail(CFS_ERR_INVALID_ARG, "unknown variant %d", a->variant);
+    if (a->variant < CFS_VARIANT_AUTO || a->variant > CFS_VARIANT_BINNED) return fail(CFS_ERR_INVALID_ARG, "unknown variant %d", a->variant);
     const DeviceInfo &di = device_info();
     if (di.ok != 1) return fail(CFS_ERR_CUDA, "no CUDA device (this library has no CPU fallback)");
     const size_t hist_bytes = (size_t)a->width * a->height * 4;
+    const uint64_t n_splats = a->n_points * (uint64_t)(a->iterations - a->burn_in);
     int splat;
     if (a->out_mode == CFS_OUT_RGBA_F32) splat = cfs::SPLAT_RGBA;
     else if (a->out_mode == CFS_OUT_DEPTH_RGBA8_U64) splat = cfs::SPLAT_DEPTH;
     else splat = cfs::SPLAT_HIST_DIRECT;
+    if (a->variant == CFS_VARIANT_BINNED) {
+        if (a->n_points == 0) return CFS_OK;
+        return render_binned(s, a, p, di, (cudaStream_t)stream);
+    }
     if (a->variant == CFS_VARIANT_SHARED_HIST || a->variant == CFS_VARIANT_WARP_AGG) {
         if (a->out_mode != CFS_OUT_HIST_U32) return fail(CFS_ERR_UNSUPPORTED, "variant %d is for HIST_U32 output only", a->variant);
         if (a->variant == CFS_VARIANT_SHARED_HIST && hist_bytes > shared_hist_limit(di))
             return fail(CFS_ERR_UNSUPPORTED, "image of %zu bytes does not fit the per-CTA shared histogram (%zu)", hist_bytes, shared_hist_limit(di));
         splat = (a->variant == CFS_VARIANT_SHARED_HIST) ? cfs::SPLAT_HIST_SHARED : cfs::SPLAT_HIST_WARPAGG;
-    } else if (a->variant == CFS_VARIANT_AUTO && a->out_mode == CFS_OUT_HIST_U32) {
-        // chosen by image size (DESIGN "splat variants"): small histograms are privatised per CTA
-        if (hist_bytes <= shared_hist_limit(di) && a->n_points * (uint64_t)(a->iterations - a->burn_in) >= (uint64_t)di.sms * (hist_bytes / 4))
+    } else if (a->variant == CFS_VARIANT_AUTO) {
+        // chosen by image size and work (DESIGN "splat variants"): small histograms are privatised
+        // per CTA; big renders with scratch memory go through the tile bins; else direct L2 atomics
+        if (a->out_mode == CFS_OUT_HIST_U32 && hist_bytes <= shared_hist_limit(di) && n_splats >= (uint64_t)di.sms * (hist_bytes / 4)) {
             splat = cfs::SPLAT_HIST_SHARED;
+        } else if (a->d_scratch && a->n_points >= (uint64_t)di.sms * cfs::kBinThreads && n_splats >= (1ull << 27)) {
+            cfs_status bs = render_binned(s, a, p, di, (cudaStream_t)stream);
+            if (bs != CFS_ERR_UNSUPPORTED) return bs;
+            build_params(s, a, &p, true);      // restore what the attempt changed; fall through to direct
+        }
     }
     if (a->n_points == 0) return CFS_OK;
     render_fn fn = pick_kernel(s, p, splat, a->flags);
@@ -471,6 +665,19 @@ extern "C" cfs_status cfs_render_host(cfs_system *s, const cfs_render_args *a, v
         }
         if ((e = cudaMemcpyAsync(s->d_cloud, h_cloud + a->point_offset, cb, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(e, "H2D cloud");
         r.d_cloud = (const cfs_cloud_rec *)s->d_cloud - a->point_offset;
+    }
+    r.d_scratch = nullptr; r.scratch_bytes = 0;
+    if (a->variant == CFS_VARIANT_AUTO || a->variant == CFS_VARIANT_BINNED) {
+        // scratch of the tile-binned variant: enough for one chunk, at most 8 GiB (more chunks beyond)
+        uint64_t want = cfs_binned_scratch_bytes(s, &r);
+        if (want > (8ull << 30)) want = 8ull << 30;
+        if (want > s->scratch_bytes) {
+            if (s->d_scratch) cudaFree(s->d_scratch);
+            s->d_scratch = nullptr; s->scratch_bytes = 0;
+            if (cudaMalloc(&s->d_scratch, want) == cudaSuccess) s->scratch_bytes = want;
+            else cudaGetLastError();           // no scratch: AUTO renders directly
+        }
+        if (want && s->d_scratch) { r.d_scratch = s->d_scratch; r.scratch_bytes = s->scratch_bytes; }
     }
     if ((e = cudaMemsetAsync(s->d_image, a->out_mode == CFS_OUT_DEPTH_RGBA8_U64 ? 0xFF : 0, bytes, st)) != cudaSuccess) return cuda_fail(e, "clear image");
     if ((e = cudaMemsetAsync(s->d_counters, 0, 16, st)) != cudaSuccess) return cuda_fail(e, "clear counters");

@@ -1,0 +1,261 @@
+// cfs_bin.cuh -- tile-binned splat stage (sm_100a): the way past the L2 atomic rate.
+//
+// A direct splat costs one L2 reduction (row 7), and the L2 executes ~190 G of them per second
+// whatever their width (measured, cfs_microbench) -- 3x below what the sampler can generate.
+// Shared-memory privatisation removes that bound, but no BASELINE image fits one CTA's shared
+// memory (SURVEY 7 "hard parts" 1).  So the image is cut into tiles that do fit, and the splats
+// are partitioned by tile on their way through HBM:
+//
+//   pass 1 (render_kernel<..., SPLAT_BIN>): each splat becomes ONE 32-bit record
+//     (pixel-in-tile << kbits | colour index), appended with one shared-memory atomic to the CTA's
+//     staging row of its tile; full rows leave as 512-byte coalesced stores into 2 KiB pool blocks
+//     owned by (CTA, tile), so no global atomic is paid per splat -- one per 512 records.
+//   pass 2 (bin_accumulate_kernel): one CTA per (tile, part) walks the tile's block list with
+//     coalesced 128-bit loads and counts records with shared-memory atomics (the record IS the
+//     counter index), then merges its private tile into the image with one red.global per
+//     touched pixel: "per-CTA shared-memory privatised histograms merged with red.global"
+//     (BASELINE north_star), made to work for images of any size.
+//
+// Nothing here can lose a splat: a staging row, the block pool or a tile list running out sends
+// the affected records down the direct path (one L2 reduction each).
+#pragma once
+#include "cfs_device.cuh"
+
+namespace cfs {
+
+__device__ __forceinline__ void bin_red_add_v4_f32(float *addr, float a, float b, float c, float d)
+{
+    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};"
+                 :: "l"(addr), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
+}
+
+__device__ __forceinline__ void bin_red_add_u32(uint32_t *addr, uint32_t v)
+{
+    asm volatile("red.global.add.u32 [%0], %1;" :: "l"(addr), "r"(v) : "memory");
+}
+
+// shared-memory layout of pass 1 (dynamic): cnt[n_tiles] | pad to 16 B | buf[n_tiles][cap]
+__device__ __forceinline__ uint32_t bin_buf_offset(uint32_t n_tiles) { return (n_tiles + 3u) & ~3u; }
+
+// one record down the direct path (staging row full, or no pool block for the tile)
+__device__ __forceinline__ void bin_direct(const RenderParams &prm, const SharedTables &s, uint32_t tile, uint32_t rec)
+{
+    const uint32_t pix = tile * prm.bin.tile_pixels + (rec >> prm.bin.kbits);
+    if (prm.color_rule == 0) {
+        bin_red_add_u32(reinterpret_cast<uint32_t *>(prm.image) + pix, 1u);
+    } else {
+        const float4 c = s.palette[rec & ((1u << prm.bin.kbits) - 1u)];
+        bin_red_add_v4_f32(reinterpret_cast<float *>(prm.image) + 4 * (size_t)pix, c.x, c.y, c.z, 1.0f);
+    }
+}
+
+// values of the append fast path, derived once per thread (32-bit shared-window addresses, so
+// an access is one ATOMS / STS without generic-address arithmetic)
+struct BinRegs {
+    uint32_t cnt_addr, buf_addr;   // shared addresses of cnt[] and buf[][]
+    uint32_t cap, cap4;            // row capacity in records / bytes
+    uint32_t tp, magic, mshift;    // tile = umulhi(pix, magic) >> mshift == pix / tp for every pixel of the image
+    uint32_t nk, kmask;            // colour slots per pixel, and the mask that zeroes k for HIST
+    float sx, ox, sy, oy;          // pixel map (DESIGN R8)
+    int W, Wm1, Hm1;
+};
+
+__device__ __forceinline__ BinRegs bin_regs_init(const RenderParams &prm, uint32_t *sm)
+{
+    BinRegs r;
+    r.cnt_addr = (uint32_t)__cvta_generic_to_shared(sm);
+    r.buf_addr = r.cnt_addr + 4u * bin_buf_offset(prm.bin.n_tiles);
+    r.cap = prm.bin.cap; r.cap4 = 4u * prm.bin.cap;
+    r.tp = prm.bin.tile_pixels; r.magic = prm.bin.magic; r.mshift = prm.bin.mshift;
+    r.nk = 1u << prm.bin.kbits; r.kmask = r.nk - 1u;
+    r.sx = prm.sx; r.ox = prm.ox; r.sy = prm.sy; r.oy = prm.oy;
+    r.W = prm.W; r.Wm1 = prm.W - 1; r.Hm1 = prm.H - 1;
+    return r;
+}
+
+// pixel rule of cfs_device.cuh pixel_of(), operands from registers
+__device__ __forceinline__ int bin_pixel_of(const BinRegs &br, float x, float y)
+{
+    int px = __float2int_rd(__fmaf_rn(x, br.sx, br.ox));
+    int py = __float2int_rd(__fmaf_rn(y, br.sy, br.oy));
+    px = min(max(px, 0), br.Wm1);
+    py = min(max(py, 0), br.Hm1);
+    return py * br.W + px;
+}
+
+// row 7, binned: one shared-memory atomic + one shared store per splat
+__device__ __forceinline__ void bin_append(const RenderParams &prm, const SharedTables &s, const BinRegs &br, int pix, int k)
+{
+    const uint32_t tile = __umulhi((uint32_t)pix, br.magic) >> br.mshift;
+    const uint32_t rec = ((uint32_t)pix - tile * br.tp) * br.nk + ((uint32_t)k & br.kmask);
+    const uint32_t row = br.buf_addr + tile * br.cap4;
+    uint32_t slot;
+    asm volatile("atom.shared.add.u32 %0, [%1], 1;" : "=r"(slot) : "r"(br.cnt_addr + 4u * tile) : "memory");
+    if (slot < br.cap) asm volatile("st.shared.u32 [%0], %1;" :: "r"(row + 4u * slot), "r"(rec) : "memory");
+    else bin_direct(prm, s, tile, rec);
+}
+
+// Per-lane bin state of pass 1, kept in REGISTERS: lane l of warp w owns tile l * warps + w (so
+// n_tiles <= 32 * warps per CTA, and the rows to flush are spread over all warps of the CTA).  `next` is a pool block taken ahead of time: the global atomic
+// that hands it out is issued when the previous block is opened and its result is not needed
+// until that block is full, so its latency never sits between the two barriers of a flush.
+struct BinLane {
+    uint32_t pos;    // next record position in the pool (block * 512 + fill); 0 = no block yet
+    uint32_t next;   // prefetched block id
+    uint32_t nblk;   // blocks this CTA has listed for the tile
+};
+
+__device__ __forceinline__ void bin_lane_init(const RenderParams &prm, BinLane &bl)
+{
+    bl.pos = 0u; bl.nblk = 0u;
+    const uint32_t my_tile = (threadIdx.x & 31u) * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    bl.next = (my_tile < prm.bin.n_tiles) ? atomicAdd(&prm.bin.ctrl[0], 1u) + 1u : 0u;   // block 0 is never used
+}
+
+// Called by every thread of the CTA between two __syncthreads.  Rows holding >= kBinFlushRecords
+// records (any record when `final`) are written out by the owning warp, 512 bytes per store
+// instruction; the remainder moves to the row start.
+__device__ __forceinline__ void bin_flush(const RenderParams &prm, const SharedTables &s, uint32_t *sm, BinLane &bl, bool final)
+{
+    const BinParams &b = prm.bin;
+    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+    const uint32_t my_tile = lane * nwarps + warp;
+    uint32_t *s_cnt = sm, *s_buf = sm + bin_buf_offset(b.n_tiles);
+    if (warp >= b.n_tiles) return;                     // warp owns no tile (warp-uniform)
+    const bool valid = my_tile < b.n_tiles;
+    uint32_t mine = valid ? s_cnt[my_tile] : 0u;
+    unsigned todo = __ballot_sync(0xFFFFFFFFu, final ? mine > 0u : mine >= kBinFlushRecords);
+    const size_t list_base = ((size_t)my_tile * b.grid + blockIdx.x) * b.lcap;
+    while (todo) {
+        const int src = __ffs(todo) - 1;
+        todo &= todo - 1;
+        const uint32_t tile = (uint32_t)src * nwarps + warp;
+        uint32_t cnt = min(__shfl_sync(0xFFFFFFFFu, mine, src), b.cap);   // slots >= cap went direct
+        uint32_t *row = s_buf + tile * b.cap;
+        uint32_t *head = row;                            // a row may hold several flush units
+        while (cnt >= kBinFlushRecords || (final && cnt > 0u)) {
+            const uint32_t n = min(cnt, kBinFlushRecords);
+            if ((int)lane == src && (bl.pos & (kBinBlockRecords - 1u)) == 0u && bl.pos != kBinInvalid) {
+                // block full (or none yet): open the prefetched one, list it, prefetch another
+                if (bl.next < b.nb && bl.nblk < b.lcap) {
+                    b.list[list_base + bl.nblk] = bl.next;
+                    bl.pos = bl.next * kBinBlockRecords;
+                    ++bl.nblk;
+                    bl.next = atomicAdd(&b.ctrl[0], 1u) + 1u;
+                } else {
+                    bl.pos = kBinInvalid;              // pool or list exhausted: direct from now on
+                }
+            }
+            const uint32_t pos = __shfl_sync(0xFFFFFFFFu, bl.pos, src);
+            uint4 v = make_uint4(0u, 0u, 0u, 0u);
+            if (4u * lane < n) v = reinterpret_cast<const uint4 *>(head)[lane];    // never past the row
+            if (pos != kBinInvalid) {
+                if (4u * lane < n) reinterpret_cast<uint4 *>(b.pool + pos)[lane] = v;
+                if ((int)lane == src) bl.pos += n;
+            } else {
+                const uint32_t r[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+                for (int i = 0; i < 4; ++i)
+                    if (4u * lane + i < n) bin_direct(prm, s, tile, r[i]);
+                if (lane == 0) atomicAdd(&b.ctrl[1], n);
+            }
+            cnt -= n;
+            head += kBinFlushRecords;
+        }
+        if (cnt > 0u && head != row) {   // fewer than 128 records remain, at least 128 words up the row
+            uint4 m = make_uint4(0u, 0u, 0u, 0u);
+            if (4u * lane < cnt) m = reinterpret_cast<const uint4 *>(head)[lane];
+            __syncwarp();
+            if (4u * lane < cnt) reinterpret_cast<uint4 *>(row)[lane] = m;
+            __syncwarp();
+        }
+        if ((int)lane == src) mine = cnt;
+    }
+    if (valid) s_cnt[my_tile] = min(mine, b.cap);
+    if (final && valid) {
+        // blocks listed for (tile, CTA) and the fill of the last one (a full block reads 512)
+        uint32_t fill = 0u;
+        if (bl.nblk > 0u && bl.pos != kBinInvalid) {
+            fill = bl.pos & (kBinBlockRecords - 1u);
+            if (fill == 0u) fill = kBinBlockRecords;
+        } else if (bl.nblk > 0u) {
+            fill = kBinBlockRecords;                   // went invalid only after full blocks
+        }
+        b.tails[(size_t)my_tile * b.grid + blockIdx.x] = (bl.nblk << 10) | fill;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// pass 2.  MODE 0: HIST_U32 (kbits = 0).  MODE 1: RGBA_F32 + MAP_INDEX: counters per
+// (pixel, colour index); the pixel's sum is sum_k n_k * palette[k] (any summation order is a
+// correct result, DESIGN R8; exact for integer-valued palettes while every sum stays < 2^24).
+template <int MODE>
+__global__ void __launch_bounds__(kBinThreads)
+bin_accumulate_kernel(const __grid_constant__ RenderParams prm)
+{
+    extern __shared__ __align__(16) uint32_t acc[];
+    const BinParams &b = prm.bin;
+    const uint32_t tile = blockIdx.x / b.split, part = blockIdx.x % b.split;
+    const uint32_t n_ctr = b.tile_pixels << b.kbits;
+    for (uint32_t i = threadIdx.x; i < n_ctr; i += blockDim.x) acc[i] = 0u;
+    __syncthreads();
+
+    // CTA `part` takes blocks j = part (mod split) of every pass-1 CTA's list for this tile; its
+    // warps stripe over the pass-1 CTAs
+    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+    for (uint32_t c = warp; c < b.grid; c += nwarps) {
+        const uint32_t tail = b.tails[(size_t)tile * b.grid + c];
+        const uint32_t n_blk = tail >> 10, last_fill = tail & 1023u;
+        const uint32_t *list = b.list + ((size_t)tile * b.grid + c) * b.lcap;
+        for (uint32_t j = part; j < n_blk; j += b.split) {
+            const uint32_t blk = list[j];
+            const uint32_t fill = (j + 1u == n_blk) ? last_fill : kBinBlockRecords;
+            const uint4 *src = reinterpret_cast<const uint4 *>(b.pool + (size_t)blk * kBinBlockRecords);
+            uint4 v[4];
+#pragma unroll
+            for (int q = 0; q < 4; ++q)     // 4 x 512 B, issued together
+                v[q] = (q * 128u < fill) ? __ldcs(src + q * 32 + lane) : make_uint4(0u, 0u, 0u, 0u);
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const uint32_t base = q * 128u + 4u * lane;
+                if (base + 0u < fill) atomicAdd(&acc[v[q].x], 1u);
+                if (base + 1u < fill) atomicAdd(&acc[v[q].y], 1u);
+                if (base + 2u < fill) atomicAdd(&acc[v[q].z], 1u);
+                if (base + 3u < fill) atomicAdd(&acc[v[q].w], 1u);
+            }
+        }
+    }
+    __syncthreads();
+
+    // merge the private tile (red.global, touched pixels only)
+    const uint32_t n_pix_tile = b.tile_pixels;
+    const uint32_t pix0 = tile * b.tile_pixels, n_pix = (uint32_t)prm.W * (uint32_t)prm.H;
+    if (MODE == 0) {
+        uint32_t *hist = reinterpret_cast<uint32_t *>(prm.image);
+        for (uint32_t i = threadIdx.x; i < n_pix_tile; i += blockDim.x) {
+            const uint32_t c = acc[i];
+            if (c && pix0 + i < n_pix) bin_red_add_u32(hist + pix0 + i, c);
+        }
+    } else {
+        float *img = reinterpret_cast<float *>(prm.image);
+        const uint32_t nk = 1u << b.kbits;
+        for (uint32_t i = threadIdx.x; i < n_pix_tile; i += blockDim.x) {
+            float r = 0.f, g = 0.f, bl = 0.f, a = 0.f;
+            uint32_t any = 0u;
+            for (uint32_t k = 0; k < nk; ++k) {
+                const uint32_t c = acc[(i << b.kbits) + k];
+                if (c) {
+                    const float fc = (float)c;
+                    r = __fmaf_rn(fc, prm.palette[4 * k + 0], r);
+                    g = __fmaf_rn(fc, prm.palette[4 * k + 1], g);
+                    bl = __fmaf_rn(fc, prm.palette[4 * k + 2], bl);
+                    a = __fadd_rn(a, fc);
+                    any = 1u;
+                }
+            }
+            if (any && pix0 + i < n_pix) bin_red_add_v4_f32(img + 4 * (size_t)(pix0 + i), r, g, bl, a);
+        }
+    }
+}
+
+}  // namespace cfs

@@ -45,7 +45,33 @@ enum SplatKind : int {
     SPLAT_HIST_WARPAGG = 2,  // __match_any_sync aggregation, then red.global.add.u32
     SPLAT_RGBA = 3,          // red.global.add.v4.f32
     SPLAT_DEPTH = 4,         // ld.global.cg pre-test + atom.global.min.u64
-    SPLAT_NONE = 5           // trace kernel
+    SPLAT_NONE = 5,          // trace kernel
+    SPLAT_BIN = 6            // tile-binned: records partitioned by image tile into a block pool
+                             // (pass 1), accumulated per tile in shared memory (pass 2)
+};
+
+// tile-binned splat stage (DESIGN "binned variant").  A record is one uint32:
+// (pixel index inside the tile) << kbits | colour index, i.e. directly the index of the shared-
+// memory counter pass 2 increments.  The pool is a set of fixed-size blocks; a block belongs to
+// one (CTA, tile) while it is filled and is listed under its tile when it is allocated.
+constexpr uint32_t kBinBlockRecords = 512;     // records per pool block (2 KiB)
+constexpr uint32_t kBinFlushRecords = 128;     // records per flush: one 512-byte coalesced store
+constexpr uint32_t kBinInvalid = 0xFFFFFFFFu;  // tile has no block (pool or list exhausted): direct splats
+constexpr int kBinThreads = 1024;              // CTA size of both binned passes (one CTA per SM)
+
+struct BinParams {
+    uint32_t *pool;        // nb * kBinBlockRecords records
+    uint32_t *list;        // [n_tiles][grid][lcap] block ids listed by pass-1 CTA c for a tile
+    uint32_t *tails;       // [n_tiles][grid] (blocks listed) << 10 | records in the last block
+    uint32_t *ctrl;        // [0] = blocks handed out, [1] = records splatted directly (statistics)
+    uint32_t nb, lcap, n_tiles;
+    uint32_t grid;         // CTAs of pass 1
+    uint32_t tile_pixels;  // pixels per tile: 2^s or 3 * 2^s
+    uint32_t magic, mshift; // pix / tile_pixels == umulhi(pix, magic) >> mshift for every pixel of the image
+    uint32_t kbits;        // log2(colour slots per pixel): 0 = HIST, else ceil(log2 n_funcs)
+    uint32_t cap;          // staging records per tile in shared memory (multiple of 32, >= 160)
+    uint32_t check_mask;   // flush check after Philox block q (4 iterations) when ((q + 1) & check_mask) == 0
+    uint32_t split;        // pass 2: CTAs per tile
 };
 
 struct ChainStep {
@@ -74,6 +100,8 @@ struct RenderParams {
     int32_t pick_steps;          // max thresholds inside one 2^24 bucket of u
     uint32_t points_per_thread;  // shared-hist persistent grid
     uint32_t hist_bins;          // W*H (shared-hist variant)
+
+    BinParams bin;               // SPLAT_BIN only
 
     ChainStep chain[kMaxChain];
     uint32_t T[kMaxFuncs];       // thresholds (u32), T[j >= n_thr] = 0xFFFFFFFF

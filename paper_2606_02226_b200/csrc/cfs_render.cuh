@@ -8,6 +8,7 @@
 // Template axes: DIM 2|3, GEN 0 = IFS / 1 = stored cloud, AFF table form, SPLAT sink, SIG chain
 // signature (kChainGeneric = interpreter, else the chain is compiled in), TRIG sin/cos evaluation.
 #pragma once
+#include "cfs_bin.cuh"
 #include "cfs_device.cuh"
 
 namespace cfs {
@@ -52,7 +53,7 @@ __device__ __forceinline__ void splat_depth(unsigned long long *buf, int pix, fl
 template <int DIM, int GEN, int SPLAT, uint32_t SIG, int TRIG>
 __device__ __forceinline__ uint32_t chain_and_splat(const RenderParams &prm, const SharedTables &s, uint32_t *s_hist,
                                                     float &gx, float &gy, float &gz, int k, uint32_t point_rgba8,
-                                                    bool have, bool past_burn_in)
+                                                    bool have, bool past_burn_in, const BinRegs &br)
 {
     float qx = gx, qy = gy, qz = gz;            // the copy of Fig. 2(B)
     const bool alive = apply_chain<DIM, SIG, TRIG>(prm, qx, qy, qz);
@@ -66,7 +67,7 @@ __device__ __forceinline__ uint32_t chain_and_splat(const RenderParams &prm, con
         return (have && !ok) ? 1u : 0u;
     }
     if (!ok) return 1u;
-    const int pix = pixel_of(prm, qx, qy);
+    const int pix = (SPLAT == SPLAT_BIN) ? bin_pixel_of(br, qx, qy) : pixel_of(prm, qx, qy);
     if (SPLAT == SPLAT_HIST_DIRECT) {
         red_add_u32(reinterpret_cast<uint32_t *>(prm.image) + pix, 1u);
     } else if (SPLAT == SPLAT_HIST_SHARED) {
@@ -83,6 +84,8 @@ __device__ __forceinline__ uint32_t chain_and_splat(const RenderParams &prm, con
     } else if (SPLAT == SPLAT_DEPTH) {
         splat_depth(reinterpret_cast<unsigned long long *>(prm.image), pix, qz,
                     GEN == 1 ? point_rgba8 : s.pal8[k]);
+    } else if (SPLAT == SPLAT_BIN) {
+        bin_append(prm, s, br, pix, k);
     }
     return 0u;
 }
@@ -94,7 +97,7 @@ __device__ __forceinline__ uint32_t chain_and_splat(const RenderParams &prm, con
 template <int DIM, int GEN, int AFF, int SPLAT, uint32_t SIG, int TRIG, bool CHECKED>
 __device__ __forceinline__ uint32_t iterate_block(const RenderParams &prm, const SharedTables &s, uint32_t *s_hist,
                                                   uint32_t plo, uint32_t phi, int it0, float &gx, float &gy, float &gz,
-                                                  bool have)
+                                                  bool have, BinLane &bl, const BinRegs &br)
 {
     const U4 w = philox4x32_10(plo, phi, (uint32_t)it0 >> 2, DOMAIN_PICK, prm);
     uint32_t dropped = 0;
@@ -107,7 +110,12 @@ __device__ __forceinline__ uint32_t iterate_block(const RenderParams &prm, const
         apply_gen<DIM, AFF>(k, s, gx, gy, gz);
         const bool past = !CHECKED || it >= prm.burn_in;
         if (past || (SIG == kChainGeneric && prm.reuse))
-            dropped += chain_and_splat<DIM, GEN, SPLAT, SIG, TRIG>(prm, s, s_hist, gx, gy, gz, k, 0u, have, past);
+            dropped += chain_and_splat<DIM, GEN, SPLAT, SIG, TRIG>(prm, s, s_hist, gx, gy, gz, k, 0u, have, past, br);
+    }
+    if (SPLAT == SPLAT_BIN && ((((uint32_t)it0 >> 2) + 1u) & prm.bin.check_mask) == 0u) {   // CTA-uniform
+        __syncthreads();
+        bin_flush(prm, s, s_hist, bl, false);
+        __syncthreads();
     }
     return dropped;
 }
@@ -115,15 +123,27 @@ __device__ __forceinline__ uint32_t iterate_block(const RenderParams &prm, const
 // ---------------------------------------------------------------------------------------------
 // the kernel
 template <int DIM, int GEN, int AFF, int SPLAT, uint32_t SIG, int TRIG>
-__global__ void __launch_bounds__(kRenderThreads)
+__global__ void __launch_bounds__(SPLAT == SPLAT_BIN ? kBinThreads : kRenderThreads, SPLAT == SPLAT_BIN ? 1 : 0)
 render_kernel(const __grid_constant__ RenderParams prm)
 {
     __shared__ SharedTables s;
-    extern __shared__ __align__(16) uint32_t s_hist[];   // SPLAT_HIST_SHARED only
+    extern __shared__ __align__(16) uint32_t s_hist[];   // SPLAT_HIST_SHARED: histogram; SPLAT_BIN: staging
     if (GEN == 0) load_tables(s, prm);
     if (SPLAT == SPLAT_HIST_SHARED)
         for (uint32_t i = threadIdx.x; i < prm.hist_bins; i += blockDim.x) s_hist[i] = 0u;
+    BinLane bl = {0u, 0u, 0u};
+    BinRegs br = {};
+    __shared__ BinRegs s_br;
+    if (SPLAT == SPLAT_BIN) {
+        // through shared memory on purpose: values read back from memory stay in registers for the
+        // whole kernel, whereas values derived from the parameter block are re-derived (constant
+        // loads + shifts) at every use, ~10 extra instructions per splat
+        if (threadIdx.x == 0) s_br = bin_regs_init(prm, s_hist);   // cnt[] of the staging rows; this lane's tile state
+        for (uint32_t i = threadIdx.x; i < prm.bin.n_tiles; i += blockDim.x) s_hist[i] = 0u;
+        bin_lane_init(prm, bl);
+    }
     __syncthreads();
+    if (SPLAT == SPLAT_BIN) br = s_br;
 
     const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
     const int I = prm.iterations, B = prm.burn_in;
@@ -133,6 +153,7 @@ render_kernel(const __grid_constant__ RenderParams prm)
         // SPLAT_HIST_WARPAGG uses full-warp collectives inside: keep whole warps in the loop
         const bool have = i < prm.n_points;
         if (SPLAT == SPLAT_HIST_WARPAGG) { if (!__any_sync(0xFFFFFFFFu, have)) break; }
+        else if (SPLAT == SPLAT_BIN) { if (i - threadIdx.x >= prm.n_points) break; }   // whole CTAs: barriers inside
         else if (!have) break;
         const uint64_t p = prm.point_offset + i;
         float gx, gy, gz = 0.0f;
@@ -143,7 +164,7 @@ render_kernel(const __grid_constant__ RenderParams prm)
             if (have) rec = __ldcs(reinterpret_cast<const float4 *>(prm.cloud) + p);
             gx = rec.x; gy = rec.y; gz = (DIM == 3) ? rec.z : 0.0f;
             dropped = chain_and_splat<DIM, GEN, SPLAT, SIG, TRIG>(prm, s, s_hist, gx, gy, gz, 0,
-                                                                  __float_as_uint(rec.w), have, true);
+                                                                  __float_as_uint(rec.w), have, true, br);
         } else {
             const uint32_t plo = (uint32_t)p, phi = (uint32_t)(p >> 32);
             {
@@ -156,14 +177,18 @@ render_kernel(const __grid_constant__ RenderParams prm)
             const int it_fast0 = min((B + 3) & ~3, I & ~3), it_fast1 = I & ~3;
             for (int it0 = 0; it0 < I; it0 += 4) {
                 if (it0 >= it_fast0 && it0 < it_fast1)
-                    dropped += iterate_block<DIM, GEN, AFF, SPLAT, SIG, TRIG, false>(prm, s, s_hist, plo, phi, it0, gx, gy, gz, have);
+                    dropped += iterate_block<DIM, GEN, AFF, SPLAT, SIG, TRIG, false>(prm, s, s_hist, plo, phi, it0, gx, gy, gz, have, bl, br);
                 else
-                    dropped += iterate_block<DIM, GEN, AFF, SPLAT, SIG, TRIG, true>(prm, s, s_hist, plo, phi, it0, gx, gy, gz, have);
+                    dropped += iterate_block<DIM, GEN, AFF, SPLAT, SIG, TRIG, true>(prm, s, s_hist, plo, phi, it0, gx, gy, gz, have, bl, br);
             }
         }
         if (have) { n_drop += dropped; n_in += (uint32_t)(I - B) - dropped; }
     }
 
+    if (SPLAT == SPLAT_BIN) {           // write out what is left in the staging rows
+        __syncthreads();
+        bin_flush(prm, s, s_hist, bl, true);
+    }
     if (SPLAT == SPLAT_HIST_SHARED) {   // merge the private histogram (red.global, non-zero bins only)
         __syncthreads();
         uint32_t *hist = reinterpret_cast<uint32_t *>(prm.image);
@@ -173,7 +198,7 @@ render_kernel(const __grid_constant__ RenderParams prm)
         }
     }
     if (prm.counters) {   // block-level reduction: two atomics per CTA (same-address L2 atomics serialise)
-        __shared__ unsigned long long s_cnt[2][kRenderThreads / 32];
+        __shared__ unsigned long long s_cnt[2][32];
         unsigned long long a = n_in, b = n_drop;
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
@@ -184,7 +209,7 @@ render_kernel(const __grid_constant__ RenderParams prm)
         __syncthreads();
         if (threadIdx.x < 2) {
             unsigned long long v = 0;
-            for (int i = 0; i < kRenderThreads / 32; ++i) v += s_cnt[threadIdx.x][i];
+            for (int i = 0; i < (int)(blockDim.x >> 5); ++i) v += s_cnt[threadIdx.x][i];
             if (v) atomicAdd(prm.counters + threadIdx.x, v);
         }
     }

@@ -6,7 +6,7 @@ import numpy as np
 
 
 def gpu_render(cfs, w, t=None, cloud=None, variant="auto", n_points=None, point_offset=None, image=None,
-               want_counters=True, flags=0):
+               want_counters=True, flags=0, scratch_bytes=None):
     """cfs_render through the binding. Returns (numpy image, counters[2])."""
     import torch
     sysh = cfs.cfs_create(w.system)
@@ -15,6 +15,11 @@ def gpu_render(cfs, w, t=None, cloud=None, variant="auto", n_points=None, point_
     d_cloud = cfs.cloud_to_device(cloud) if cloud is not None else None
     args = cfs.make_args(w.render, d_image=img, d_cloud=d_cloud, d_counters=ctr, t=t, variant=variant,
                          n_points=n_points, point_offset=point_offset, flags=flags)
+    if variant == "binned" or scratch_bytes is not None:       # scratch of the tile-binned variant
+        nbytes = cfs.cfs_binned_scratch_bytes(sysh, args) if scratch_bytes is None else scratch_bytes
+        scratch = torch.empty(max(int(nbytes), 1), dtype=torch.uint8, device="cuda")
+        args = cfs.make_args(w.render, d_image=img, d_cloud=d_cloud, d_counters=ctr, t=t, variant=variant,
+                             n_points=n_points, point_offset=point_offset, flags=flags, d_scratch=scratch)
     cfs.cfs_render(sysh, args)
     torch.cuda.synchronize()
     out = cfs.image_to_numpy(img, w.render.out_mode)

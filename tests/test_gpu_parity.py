@@ -204,6 +204,77 @@ def test_fast_trig_within_tolerance(cfs, oracle, cfg, interp):
         assert density_l1(g[:, ch], o[:, ch]) <= L1_TOL
 
 
+# ------------------------------------------------------------------ tile-binned variant
+@pytest.mark.parametrize("n", [1, 1000, 1024, 5000 + 13])
+def test_binned_histogram_bit_exact(cfs, oracle, n):
+    """CFS_VARIANT_BINNED on the cfg 0 image: records through the block pool, tiles accumulated in
+    shared memory; identical per pixel to the oracle, counters included; ragged CTAs."""
+    w = W.config(0).scaled(n_points=n, iterations=300)
+    g, gc = gpu_render(cfs, w, variant="binned")
+    o, oc, _ = oracle.render_parallel(w.system, w.render)
+    assert np.array_equal(g, o) and np.array_equal(gc, oc)
+
+
+def test_binned_chunks_and_small_scratch(cfs, oracle):
+    """A scratch buffer far below the one-chunk size forces several (pass 1, pass 2) chunks; one that
+    cannot hold a partial block per (CTA, tile) is refused with UNSUPPORTED."""
+    w = W.config(0).scaled(n_points=150000, iterations=120)
+    sysh = cfs.cfs_create(w.system)
+    need = cfs.cfs_binned_scratch_bytes(sysh, cfs.make_args(w.render))
+    sysh.close()
+    assert need > (60 << 20)
+    o, oc, _ = oracle.render_parallel(w.system, w.render)
+    g, gc = gpu_render(cfs, w, variant="binned", scratch_bytes=need // 2)
+    assert np.array_equal(g, o) and np.array_equal(gc, oc)
+    with pytest.raises(cfs.CfsError) as ei:
+        gpu_render(cfs, w, variant="binned", scratch_bytes=1 << 20)
+    assert ei.value.status == cfs.CFS_ERR_UNSUPPORTED
+    g, gc = gpu_render(cfs, w, variant="auto", scratch_bytes=1 << 20)      # AUTO falls back to direct
+    assert np.array_equal(g, o)
+
+
+@pytest.mark.parametrize("cfg", [1, 2])
+def test_binned_rgba_equals_direct(cfs, oracle, cfg):
+    """Binned RGBA (counters per pixel and map, sum_k n_k * palette[k]) against the direct variant
+    on the same device functions: integer-valued colour sums below 2^24 are exact, so the images
+    are identical; and against the oracle within the density bar."""
+    w = W.config(cfg).scaled(n_points=(1 << 14) + 5)
+    t = w.frames[len(w.frames) // 2]
+    gb, cb = gpu_render(cfs, w, t=t, variant="binned")
+    gd, cd = gpu_render(cfs, w, t=t, variant="direct")
+    assert np.array_equal(gb, gd) and np.array_equal(cb, cd)
+    o, oc, _ = oracle.render_parallel(w.system, w.render, t=t)
+    _check_rgba(gb, o, cb, oc)
+
+
+def test_binned_hot_tile_overflow_and_limits(cfs, oracle):
+    """All splats in ONE pixel (one-hot probabilities: the point sits on the map's fixed point): the
+    staging row of that tile overflows constantly and the surplus takes the direct path; nothing
+    is lost.  16 maps use 4 colour bits; 17 maps and DEPTH output are refused."""
+    funcs = W.square_funcs(probs=[0.0, 0.0, 1.0, 0.0])
+    sys1 = W.System(2, "ifs", funcs, [], "map_index", W.palette_for(4))
+    # 400 x 160 splats x 255 < 2^24: the float sum is exact whatever the order of the additions
+    w = W.Workload("hot", sys1, W.Render(400, 5, 200, 40, 512, 512, (-1, 1, -1, 1), "rgba_f32"))
+    g, gc = gpu_render(cfs, w, variant="binned")
+    o, oc = oracle.render(sys1, w.render)
+    assert np.array_equal(g.astype(np.float64), o) and np.array_equal(gc, oc)
+    assert np.count_nonzero(g[:, 3]) == 1 and g[:, 3].sum() == 400 * 160
+
+    f16 = [W.Func("affine", float(np.float32(1 + (k % 3))), [0.5, 0, 0, 0.5, 0.5 * math.cos(k), 0.5 * math.sin(k)])
+           for k in range(17)]
+    s16 = W.System(2, "ifs", f16[:16], [], "map_index", W.palette_for(16))
+    w16 = W.Workload("n16", s16, W.Render(4000, 6, 90, 10, 300, 200, (-1, 1, -1, 1), "rgba_f32"))
+    g, gc = gpu_render(cfs, w16, variant="binned")
+    o, oc = oracle.render(s16, w16.render)
+    assert np.array_equal(g.astype(np.float64), o) and np.array_equal(gc, oc)
+    s17 = W.System(2, "ifs", f16, [], "map_index", W.palette_for(17))
+    w17 = W.Workload("n17", s17, w16.render)
+    for bad in (w17, W.config(4).scaled(n_points=100, iterations=30)):
+        with pytest.raises(cfs.CfsError) as ei:
+            gpu_render(cfs, bad, variant="binned", scratch_bytes=64 << 20)
+        assert ei.value.status == cfs.CFS_ERR_UNSUPPORTED
+
+
 # ------------------------------------------------------------------ general tables and edge cases
 def test_general_pick_and_general_affine(cfs, oracle):
     """Non-uniform probabilities incl. zero-probability maps (table + compare pick), non-diagonal
@@ -400,6 +471,16 @@ def test_cfg1_full_size_properties(cfs, oracle):
     col = g[:, :3].astype(np.float64).sum(axis=0) / 255.0            # map 0: R, 1: G, 2: B, 3: R+G
     assert g[:, :3].max() < 2 ** 24 and np.all(col == np.round(col))
     assert abs(col[2] / S - 0.25) < 1e-3 and abs(col[1] / S - 0.5) < 1e-3 and abs(col[0] / S - 0.5) < 1e-3
+    # the same render through the tile bins (AUTO picks them when scratch is given), in one chunk and
+    # in several; integer-valued sums below 2^24 are exact, so all three images are identical.
+    # A scratch too small for the bins makes AUTO fall back to the direct path.
+    sysh = cfs.cfs_create(w.system)
+    need = cfs.cfs_binned_scratch_bytes(sysh, cfs.make_args(w.render))
+    sysh.close()
+    assert need > (4 << 30)
+    for nbytes in (need, need // 3, 1 << 20):
+        gb, gbc = gpu_render(cfs, w, scratch_bytes=nbytes)
+        assert np.array_equal(gb, g) and np.array_equal(gbc, gc)
     sub = w.scaled(n_points=1 << 15)
     gs, gsc = gpu_render(cfs, sub)
     o, oc, _ = oracle.render_parallel(sub.system, sub.render)
