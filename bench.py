@@ -34,7 +34,8 @@ UNIT = "point-iterations/s"
 L2_FLUSH_BYTES = 256 << 20
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the render kernel on configs[1], from
 # the `ncu --set full` capture summarised in profiles/r01_ncu_render_cfg1.md (null until captured)
-NCU_TRAFFIC_BYTES_PER_LAUNCH = None
+NCU_TRAFFIC_BYTES_PER_LAUNCH = None          # binned pass 1
+NCU_TRAFFIC_BYTES_PER_LAUNCH_DIRECT = 7.0e6  # direct kernel, profiles/r01a_render_cfg1.txt (image stays in L2)
 
 
 # ----------------------------------------------------------------------------- clocks sampler
@@ -197,6 +198,9 @@ def measure_rates(cfs, torch, buf, sms):
 
 # algorithmic lane-instructions per point-iteration (table "N_instr")
 N_INSTR = {0: 30, 1: 62, 2: 66, 3: 110, 4: 52}
+# the same for the binned variant with MUFU sin/cos (Philox 10, pick, LDS +
+# generator FMAs, chain, 4 bound compares, 9 pixel ops, 6 record ops, 4 append ops)
+N_INSTR_BIN = {0: 38, 1: 51, 2: 51}
 RED_KEY = {0: "red_add_u32@1048576", 1: "red_add_v4f32@16777216", 2: "red_add_v4f32@33177600",
            3: "red_add_v4f32@132710400", 4: "atom_min_u64@66355200"}
 
@@ -326,14 +330,30 @@ def run_ours(args):
         dist.barrier()
     clocks = sampler.stop() if rank == 0 else None
     launches = cfs.cfs_launch_count()
+    in_bounds = int(ctr[0].item())
+    assert in_bounds == S * args.steps, f"conservation violated: {in_bounds} != {S * args.steps}"
+    launches_per_render = (launches // max(args.steps, 1)) - 2        # minus the two tone-map kernels
+    pass1_s = None
+    if launches_per_render >= 2:       # binned: time pass 1 (sample + bin) apart from pass 2, same launch shape
+        p1args = cfs.make_args(r, d_image=img, point_offset=rank * P, variant=args.variant,
+                               flags=(["fast_trig"] if args.fast_trig else []) + ["bin_pass1_only"], d_scratch=scratch_t)
+        ts = []
+        for i in range(7):
+            flush.zero_()
+            e0, e1 = event_pair(torch)
+            e0.record()
+            cfs.cfs_render(sysh, p1args)
+            e1.record()
+            torch.cuda.synchronize()
+            if i >= 2:
+                ts.append(e0.elapsed_time(e1) * 1e-3)
+        pass1_s = float(np.median(ts))
     step_s = sum(e[0].elapsed_time(e[2]) for e in evs) * 1e-3
     render_s = sum(e[0].elapsed_time(e[1]) for e in evs) * 1e-3
     tt = torch.tensor([step_s, render_s], dtype=torch.float64, device="cuda")
     if world > 1:
         dist.all_reduce(tt, op=dist.ReduceOp.MAX)
     step_s, render_s = float(tt[0]), float(tt[1])
-    in_bounds = int(ctr[0].item())
-    assert in_bounds == S * args.steps, f"conservation violated: {in_bounds} != {S * args.steps}"
 
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
     h_img = torch.empty((r.width * r.height, 4), dtype=torch.float32).pin_memory()
@@ -365,17 +385,37 @@ def run_ours(args):
     value = world * P * I * args.steps / step_s
     t_render = render_s / args.steps
     roof = roofline_for(HEADLINE_CFG, w, rates, peaks, S, t_render)
-    peak_red = rates[RED_KEY[HEADLINE_CFG]]
-    roofline = {
-        "bound": roof["bound"], "achieved": S / t_render / 1e9,
-        "peak": (peak_red / 1e9) if roof["bound"] == "l2_atomic" else S / (roof["t_roof_ms"] * 1e-3) / 1e9,
-        "unit": "Gsplat/s (one red.global.add.v4.f32 per splat)", "frac": roof["frac"],
-        "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH, "kernel": "cfs::render_kernel<2,IFS,DIAG,RGBA>",
-        "kernel_ms": t_render * 1e3, "t_issue_ms": roof["t_issue_ms"], "t_atomic_ms": roof["t_atomic_ms"],
-        "peak_source": "red.global.add.v4.f32 at uniformly random pixels of a 16 MiB footprint, cfs_microbench "
-                       "in this run (BASELINE north_star); FFMA issue rate from the same run for t_issue",
-        "hbm_peak_gbs": peaks.get("hbm_gbs"), "hbm_peak_source": peaks_src,
-    }
+    binned = launches_per_render >= 2
+    north_star = {"definition": "t_roof / t_render, t_roof = max(t_issue, t_atomic, t_hbm) (BASELINE north_star; "
+                                "the L2-atomic term assumes one reduction per splat, which the binned variant does not pay)",
+                  "bound": roof["bound"], "frac": roof["frac"], "t_issue_ms": roof["t_issue_ms"],
+                  "t_atomic_ms": roof["t_atomic_ms"], "t_render_ms": t_render * 1e3}
+    if binned:
+        # dominant kernel: pass 1 (sample + chain + bin), bound by instruction issue
+        n_instr = N_INSTR_BIN[HEADLINE_CFG]
+        roofline = {
+            "bound": "alu", "achieved": P * I * n_instr / pass1_s / 1e12, "peak": rates["ffma"] / 1e12,
+            "unit": "T lane-instructions/s", "frac": (P * I * n_instr / pass1_s) / rates["ffma"],
+            "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH, "kernel": "cfs::render_kernel<2,IFS,DIAG,BIN,swirl+affine,MUFU>",
+            "kernel_ms": pass1_s * 1e3, "render_ms": t_render * 1e3, "pass2_ms": (t_render - pass1_s) * 1e3,
+            "algorithmic_lane_instructions_per_point_iteration": n_instr,
+            "algorithmic_bytes_per_launch": int(S * 4),
+            "peak_source": "FFMA lane-issue rate of cfs_microbench in this run (148 SMs x 128 lanes x SM clock)",
+            "hbm_peak_gbs": peaks.get("hbm_gbs"), "hbm_peak_source": peaks_src,
+            "pass2_hbm_gbs": S * 4 / max(t_render - pass1_s, 1e-9) / 1e9,
+        }
+    else:
+        peak_red = rates[RED_KEY[HEADLINE_CFG]]
+        roofline = {
+            "bound": roof["bound"], "achieved": S / t_render / 1e9,
+            "peak": (peak_red / 1e9) if roof["bound"] == "l2_atomic" else S / (roof["t_roof_ms"] * 1e-3) / 1e9,
+            "unit": "Gsplat/s (one red.global.add.v4.f32 per splat)", "frac": roof["frac"],
+            "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH_DIRECT, "kernel": "cfs::render_kernel<2,IFS,DIAG,RGBA,swirl+affine>",
+            "kernel_ms": t_render * 1e3, "t_issue_ms": roof["t_issue_ms"], "t_atomic_ms": roof["t_atomic_ms"],
+            "peak_source": "red.global.add.v4.f32 at uniformly random pixels of a 16 MiB footprint, cfs_microbench "
+                           "in this run (BASELINE north_star); FFMA issue rate from the same run for t_issue",
+            "hbm_peak_gbs": peaks.get("hbm_gbs"), "hbm_peak_source": peaks_src,
+        }
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
@@ -386,7 +426,8 @@ def run_ours(args):
                 "h2d_bytes_per_step": 0, "d2h_bytes_per_step": int(h_img.numel() * 4 + 16),
                 "note": "cfs_render_host: clear + render + D2H of the float32 accumulators and counters into pinned "
                         "host memory; this workload has no host input besides the kernel parameter block"},
-        "roofline": roofline,
+        "roofline": roofline, "north_star_roofline": north_star,
+        "splat_variant": "binned (tile bins through scratch, shared-memory tile accumulation)" if binned else "direct (one L2 reduction per splat)",
         "microbench": {k: (v / 1e9 if not k.endswith("GBps") else v) for k, v in rates.items()},
         "microbench_unit": "G lane-ops/s (stream: GB/s)",
     }
@@ -461,9 +502,12 @@ def main():
     ap.add_argument("--profile-cfg", type=int, default=None,
                     help="only launch cfs_render of configs[N] --steps times (ncu target; no bench line)")
     ap.add_argument("--variant", default="auto", help="splat variant: auto (tile bins for large renders, else direct), direct, binned, ...")
-    ap.add_argument("--fast-trig", action="store_true", help="CFS_FLAG_FAST_TRIG (MUFU sin/cos) on every render")
+    ap.add_argument("--accurate-trig", action="store_true",
+                    help="evaluate sin/cos with sincosf (<= 2 ulp) instead of CFS_FLAG_FAST_TRIG (MUFU); both are inside "
+                         "the BASELINE tolerances (tests/test_gpu_parity.py)")
     args = ap.parse_args()
     global SINCOS
+    args.fast_trig = not args.accurate_trig
     if args.fast_trig:
         SINCOS = "MUFU sin.approx/cos.approx (CFS_FLAG_FAST_TRIG)"
     if args.profile_cfg is not None:

@@ -98,8 +98,10 @@ typedef enum {
  *   of the <= 2 ulp sincosf.  Within the 1e-4 coordinate tolerance of BASELINE north_star for the
  *   bounded arguments of contractive systems; the default is the accurate evaluation.
  *   INTERPRET_CHAIN: never use a kernel compiled for the chain's signature; run the chain
- *   interpreter (same device functions, same results; for tests and comparisons). */
-typedef enum { CFS_FLAG_FAST_TRIG = 1, CFS_FLAG_INTERPRET_CHAIN = 2 } cfs_render_flags;
+ *   interpreter (same device functions, same results; for tests and comparisons).
+ *   BIN_PASS1_ONLY: measurement instrument of the BINNED variant: run pass 1 (sample + bin) and
+ *   skip pass 2, so the two passes can be timed apart with events; the image is NOT updated. */
+typedef enum { CFS_FLAG_FAST_TRIG = 1, CFS_FLAG_INTERPRET_CHAIN = 2, CFS_FLAG_BIN_PASS1_ONLY = 4 } cfs_render_flags;
 
 /* one 16-byte record of a stored cloud (BASELINE cfg 3); rgba8 = r | g<<8 | b<<16 | a<<24 */
 typedef struct { float x, y, z; uint32_t rgba8; } cfs_cloud_rec;
@@ -146,7 +148,9 @@ cfs_status cfs_render(const cfs_system *sys, const cfs_render_args *args, void *
 /* bytes of d_scratch with which CFS_VARIANT_BINNED renders args->n_points in ONE chunk (pass 1 +
  * pass 2); 0 when the variant cannot serve this system / output mode / image, or without a device.
  * With scratch memory given, CFS_VARIANT_AUTO takes the binned path for large renders it can serve
- * (at least one 1024-point CTA per SM and 2^27 splats) and the direct path otherwise. */
+ * (at least one 1024-point CTA per SM and 2^27 splats) whose chain has no sin/cos step or runs with
+ * CFS_FLAG_FAST_TRIG -- where it was measured faster than the L2 atomic rate allows -- and the
+ * direct path otherwise. */
 uint64_t cfs_binned_scratch_bytes(const cfs_system *sys, const cfs_render_args *args);
 
 /* cfs_render_host -- same path with HOST buffers (end-to-end entry point): copies h_cloud to the

@@ -235,7 +235,7 @@ using cfs::RenderParams;
 cfs_status build_params(const cfs_system *s, const cfs_render_args *a, RenderParams *out, bool need_image)
 {
     if (!s || !a) return fail(CFS_ERR_INVALID_ARG, "system or args is NULL");
-    if (a->flags & ~(CFS_FLAG_FAST_TRIG | CFS_FLAG_INTERPRET_CHAIN)) return fail(CFS_ERR_INVALID_ARG, "unknown flags 0x%x", a->flags);
+    if (a->flags & ~(CFS_FLAG_FAST_TRIG | CFS_FLAG_INTERPRET_CHAIN | CFS_FLAG_BIN_PASS1_ONLY)) return fail(CFS_ERR_INVALID_ARG, "unknown flags 0x%x", a->flags);
     if (a->iterations < 1) return fail(CFS_ERR_INVALID_ARG, "iterations must be >= 1");
     if (a->burn_in < 0 || a->burn_in >= a->iterations) return fail(CFS_ERR_INVALID_ARG, "burn_in must be in [0, iterations)");
     if (s->gen == CFS_GEN_CLOUD && (a->iterations != 1 || a->burn_in != 0)) return fail(CFS_ERR_INVALID_ARG, "CLOUD generator needs iterations = 1, burn_in = 0");
@@ -479,9 +479,9 @@ bool bin_layout(BinPlan *pl, void *scratch, uint64_t bytes, uint64_t n_points, u
     const uint64_t rec_cap = (nb - partial) * 8 / 9 * cfs::kBinBlockRecords;
     uint64_t cp = rec_cap / splats_per_point;
     const uint64_t wave = (uint64_t)pl->grid1 * cfs::kBinThreads;
-    if (cp >= wave) cp = cp / wave * wave;                      // whole waves: no ragged trip inside a chunk
     if (cp < cfs::kBinThreads) { *why = "scratch too small for one CTA of points"; return false; }
-    if (cp > n_points) cp = n_points;
+    if (cp >= n_points) cp = n_points;                          // everything in one chunk
+    else if (cp >= wave) cp = cp / wave * wave;                 // whole waves: no ragged trip inside a chunk
     pl->chunk_points = cp;
     return true;
 }
@@ -534,8 +534,11 @@ cfs_status render_binned(const cfs_system *s, const cfs_render_args *a, RenderPa
         if ((e = cudaMemsetAsync(pl.bp.ctrl, 0, pl.clear_bytes, st)) != cudaSuccess) return cuda_fail(e, "clear bin heads");
         // always the full persistent grid: pass 2 reads the tail word of every (tile, CTA)
         fn1<<<pl.grid1, cfs::kBinThreads, pl.smem_pass1, st>>>(p);
-        fn2<<<pl.bp.n_tiles * pl.bp.split, cfs::kBinThreads, pl.smem_pass2, st>>>(p);
-        g_launches += 2;
+        ++g_launches;
+        if (!(a->flags & CFS_FLAG_BIN_PASS1_ONLY)) {
+            fn2<<<pl.bp.n_tiles * pl.bp.split, cfs::kBinThreads, pl.smem_pass2, st>>>(p);
+            ++g_launches;
+        }
         if ((e = cudaGetLastError()) != cudaSuccess) return cuda_fail(e, "binned render launch");
     }
     return CFS_OK;
@@ -571,7 +574,10 @@ extern "C" cfs_status cfs_render(const cfs_system *s, const cfs_render_args *a, 
         // per CTA; big renders with scratch memory go through the tile bins; else direct L2 atomics
         if (a->out_mode == CFS_OUT_HIST_U32 && hist_bytes <= shared_hist_limit(di) && n_splats >= (uint64_t)di.sms * (hist_bytes / 4)) {
             splat = cfs::SPLAT_HIST_SHARED;
-        } else if (a->d_scratch && a->n_points >= (uint64_t)di.sms * cfs::kBinThreads && n_splats >= (1ull << 27)) {
+        } else if (a->d_scratch && a->n_points >= (uint64_t)di.sms * cfs::kBinThreads && n_splats >= (1ull << 27) &&
+                   (!cfs::sig_has_trig(chain_signature(p)) || (a->flags & CFS_FLAG_FAST_TRIG))) {
+            // the tile bins trade the L2 atomic (~190 G/s) for ~15 more instructions per splat: measured
+            // ahead of the direct path when sin/cos is absent or on the MUFU unit, level with it otherwise
             cfs_status bs = render_binned(s, a, p, di, (cudaStream_t)stream);
             if (bs != CFS_ERR_UNSUPPORTED) return bs;
             build_params(s, a, &p, true);      // restore what the attempt changed; fall through to direct

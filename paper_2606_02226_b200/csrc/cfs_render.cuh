@@ -101,16 +101,43 @@ __device__ __forceinline__ uint32_t iterate_block(const RenderParams &prm, const
 {
     const U4 w = philox4x32_10(plo, phi, (uint32_t)it0 >> 2, DOMAIN_PICK, prm);
     uint32_t dropped = 0;
+    if constexpr (!CHECKED && SIG != kChainGeneric && SPLAT == SPLAT_BIN) {
+        // ALU-bound variant: the generator recurrence is short (LDS + FMAs), the chain and pixel
+        // arithmetic of the four iterations are independent of one another once the four generator
+        // states exist -- written as straight-line stages so that the four dependent chains
+        // (LDS -> FMA -> MUFU -> FMA -> F2I -> ATOMS) interleave instead of running back to back
+        float X[4], Y[4], Z[4];
+        int K[4];
+        bool ok[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const uint32_t u = (j == 0) ? w.x : (j == 1) ? w.y : (j == 2) ? w.z : w.w;
+            K[j] = pick_index(u, s, prm);
+            apply_gen<DIM, AFF>(K[j], s, gx, gy, gz);
+            X[j] = gx; Y[j] = gy; Z[j] = gz;                 // the copies of Fig. 2(B)
+        }
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const bool alive = apply_chain<DIM, SIG, TRIG>(prm, X[j], Y[j], Z[j]);
+            ok[j] = alive && have && in_bounds(prm, X[j], Y[j]);
+        }
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            if (ok[j]) bin_append(prm, s, br, bin_pixel_of(br, X[j], Y[j]), K[j]);
+            else ++dropped;
+        }
+    } else {
 #pragma unroll(CHECKED ? 1 : 4)
-    for (int j = 0; j < 4; ++j) {
-        const int it = it0 + j;
-        if (CHECKED && it >= prm.iterations) break;
-        const uint32_t u = (j == 0) ? w.x : (j == 1) ? w.y : (j == 2) ? w.z : w.w;
-        const int k = pick_index(u, s, prm);
-        apply_gen<DIM, AFF>(k, s, gx, gy, gz);
-        const bool past = !CHECKED || it >= prm.burn_in;
-        if (past || (SIG == kChainGeneric && prm.reuse))
-            dropped += chain_and_splat<DIM, GEN, SPLAT, SIG, TRIG>(prm, s, s_hist, gx, gy, gz, k, 0u, have, past, br);
+        for (int j = 0; j < 4; ++j) {
+            const int it = it0 + j;
+            if (CHECKED && it >= prm.iterations) break;
+            const uint32_t u = (j == 0) ? w.x : (j == 1) ? w.y : (j == 2) ? w.z : w.w;
+            const int k = pick_index(u, s, prm);
+            apply_gen<DIM, AFF>(k, s, gx, gy, gz);
+            const bool past = !CHECKED || it >= prm.burn_in;
+            if (past || (SIG == kChainGeneric && prm.reuse))
+                dropped += chain_and_splat<DIM, GEN, SPLAT, SIG, TRIG>(prm, s, s_hist, gx, gy, gz, k, 0u, have, past, br);
+        }
     }
     if (SPLAT == SPLAT_BIN && ((((uint32_t)it0 >> 2) + 1u) & prm.bin.check_mask) == 0u) {   // CTA-uniform
         __syncthreads();

@@ -471,16 +471,21 @@ def test_cfg1_full_size_properties(cfs, oracle):
     col = g[:, :3].astype(np.float64).sum(axis=0) / 255.0            # map 0: R, 1: G, 2: B, 3: R+G
     assert g[:, :3].max() < 2 ** 24 and np.all(col == np.round(col))
     assert abs(col[2] / S - 0.25) < 1e-3 and abs(col[1] / S - 0.5) < 1e-3 and abs(col[0] / S - 0.5) < 1e-3
-    # the same render through the tile bins (AUTO picks them when scratch is given), in one chunk and
-    # in several; integer-valued sums below 2^24 are exact, so all three images are identical.
+    # the same render through the tile bins, in one chunk and in several; integer-valued sums below 2^24 are exact, so all three images are identical.
     # A scratch too small for the bins makes AUTO fall back to the direct path.
     sysh = cfs.cfs_create(w.system)
     need = cfs.cfs_binned_scratch_bytes(sysh, cfs.make_args(w.render))
     sysh.close()
     assert need > (4 << 30)
-    for nbytes in (need, need // 3, 1 << 20):
-        gb, gbc = gpu_render(cfs, w, scratch_bytes=nbytes)
+    for variant, nbytes in (("binned", need), ("binned", need // 3), ("auto", 1 << 20)):
+        gb, gbc = gpu_render(cfs, w, variant=variant, scratch_bytes=nbytes)
         assert np.array_equal(gb, g) and np.array_equal(gbc, gc)
+    # the configuration bench.py times: MUFU sin/cos, AUTO with scratch (-> tile bins).  Conservation
+    # stays exact; against the accurate image only splats within ~2^-21 of a pixel edge move.
+    gf, gfc = gpu_render(cfs, w, variant="auto", scratch_bytes=need, flags=["fast_trig"])
+    assert np.array_equal(gfc, gc) and gf[:, 3].astype(np.float64).sum() == S
+    for ch in range(4):
+        assert density_l1(gf[:, ch], g[:, ch]) <= L1_TOL
     sub = w.scaled(n_points=1 << 15)
     gs, gsc = gpu_render(cfs, sub)
     o, oc, _ = oracle.render_parallel(sub.system, sub.render)
