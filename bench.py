@@ -34,8 +34,8 @@ UNIT = "point-iterations/s"
 L2_FLUSH_BYTES = 256 << 20
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the render kernel on configs[1], from
 # the `ncu --set full` capture summarised in profiles/r01_ncu_render_cfg1.md (null until captured)
-NCU_TRAFFIC_BYTES_PER_LAUNCH = None          # binned pass 1
-NCU_TRAFFIC_BYTES_PER_LAUNCH_DIRECT = 7.0e6  # direct kernel, profiles/r01a_render_cfg1.txt (image stays in L2)
+NCU_TRAFFIC_BYTES_PER_LAUNCH = 4.062e9       # binned pass 1: profiles/r01h_binned_cfg1.txt (0.001 GB read + 4.061 GB written)
+NCU_TRAFFIC_BYTES_PER_LAUNCH_DIRECT = 7.06e6 # direct kernel: profiles/r01h_direct_cfg1.txt (the image stays in L2)
 
 
 # ----------------------------------------------------------------------------- clocks sampler

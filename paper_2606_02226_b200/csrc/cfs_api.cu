@@ -44,7 +44,7 @@ cfs_status cuda_fail(cudaError_t e, const char *what)
     return fail(CFS_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
 }
 
-struct DeviceInfo { int ok = -1; int sms = 0; int smem_optin = 0; };
+struct DeviceInfo { int ok = -1; int sms = 0; int smem_optin = 0; int smem_sm = 0; };
 
 const DeviceInfo &device_info()
 {
@@ -54,6 +54,7 @@ const DeviceInfo &device_info()
         if (cudaGetDevice(&dev) != cudaSuccess) { di.ok = 0; cudaGetLastError(); return di; }
         cudaDeviceGetAttribute(&di.sms, cudaDevAttrMultiProcessorCount, dev);
         cudaDeviceGetAttribute(&di.smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+        cudaDeviceGetAttribute(&di.smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev);
         di.ok = (di.sms > 0) ? 1 : 0;
     }
     return di;
@@ -398,7 +399,9 @@ bool bin_shape(const cfs_system *s, const cfs_render_args *a, const DeviceInfo &
     const uint64_t n_tiles = tiles_for(shift, mul);
     if (n_tiles > (uint64_t)cfs::kBinThreads) { *why = "image has too many tiles for the binned variant"; return false; }
     // pass 1 staging: cnt + rows of `cap` records per tile, next to the static tables
-    const long budget = (long)di.smem_optin - (long)sizeof(cfs::SharedTables) - 2048;
+    // kBinCtasPerSm CTAs of pass 1 share the SM's shared memory (1 KiB per CTA is reserved by the system)
+    const long budget = ((long)di.smem_sm / cfs::kBinCtasPerSm < (long)di.smem_optin ? (long)di.smem_sm / cfs::kBinCtasPerSm : (long)di.smem_optin)
+                        - (long)sizeof(cfs::SharedTables) - 2048;
     const long words = budget / 4 - (long)n_tiles - 4;
     long cap = words / (long)n_tiles / 32 * 32;
     if (cap > 1024) cap = 1024;
@@ -430,7 +433,7 @@ bool bin_shape(const cfs_system *s, const cfs_render_args *a, const DeviceInfo &
     if (b.split < 1) b.split = 1;
     pl->smem_pass1 = ((n_tiles + 3) / 4 * 4 + n_tiles * (size_t)cap) * 4;
     pl->smem_pass2 = ((size_t)b.tile_pixels << kbits) * 4;
-    pl->grid1 = (uint32_t)di.sms;
+    pl->grid1 = (uint32_t)di.sms * cfs::kBinCtasPerSm;
     return true;
 }
 
@@ -536,7 +539,7 @@ cfs_status render_binned(const cfs_system *s, const cfs_render_args *a, RenderPa
         fn1<<<pl.grid1, cfs::kBinThreads, pl.smem_pass1, st>>>(p);
         ++g_launches;
         if (!(a->flags & CFS_FLAG_BIN_PASS1_ONLY)) {
-            fn2<<<pl.bp.n_tiles * pl.bp.split, cfs::kBinThreads, pl.smem_pass2, st>>>(p);
+            fn2<<<pl.bp.n_tiles * pl.bp.split, cfs::kBinAccThreads, pl.smem_pass2, st>>>(p);
             ++g_launches;
         }
         if ((e = cudaGetLastError()) != cudaSuccess) return cuda_fail(e, "binned render launch");
@@ -574,7 +577,7 @@ extern "C" cfs_status cfs_render(const cfs_system *s, const cfs_render_args *a, 
         // per CTA; big renders with scratch memory go through the tile bins; else direct L2 atomics
         if (a->out_mode == CFS_OUT_HIST_U32 && hist_bytes <= shared_hist_limit(di) && n_splats >= (uint64_t)di.sms * (hist_bytes / 4)) {
             splat = cfs::SPLAT_HIST_SHARED;
-        } else if (a->d_scratch && a->n_points >= (uint64_t)di.sms * cfs::kBinThreads && n_splats >= (1ull << 27) &&
+        } else if (a->d_scratch && a->n_points >= (uint64_t)di.sms * cfs::kBinCtasPerSm * cfs::kBinThreads && n_splats >= (1ull << 27) &&
                    (!cfs::sig_has_trig(chain_signature(p)) || (a->flags & CFS_FLAG_FAST_TRIG))) {
             // the tile bins trade the L2 atomic (~190 G/s) for ~15 more instructions per splat: measured
             // ahead of the direct path when sin/cos is absent or on the MUFU unit, level with it otherwise

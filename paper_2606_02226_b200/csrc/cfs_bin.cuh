@@ -190,7 +190,7 @@ __device__ __forceinline__ void bin_flush(const RenderParams &prm, const SharedT
 // (pixel, colour index); the pixel's sum is sum_k n_k * palette[k] (any summation order is a
 // correct result, DESIGN R8; exact for integer-valued palettes while every sum stays < 2^24).
 template <int MODE>
-__global__ void __launch_bounds__(kBinThreads)
+__global__ void __launch_bounds__(kBinAccThreads)
 bin_accumulate_kernel(const __grid_constant__ RenderParams prm)
 {
     extern __shared__ __align__(16) uint32_t acc[];

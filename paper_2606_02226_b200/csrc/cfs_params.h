@@ -57,7 +57,9 @@ enum SplatKind : int {
 constexpr uint32_t kBinBlockRecords = 512;     // records per pool block (2 KiB)
 constexpr uint32_t kBinFlushRecords = 128;     // records per flush: one 512-byte coalesced store
 constexpr uint32_t kBinInvalid = 0xFFFFFFFFu;  // tile has no block (pool or list exhausted): direct splats
-constexpr int kBinThreads = 1024;              // CTA size of both binned passes (one CTA per SM)
+constexpr int kBinThreads = 1024;              // CTA size of pass 1 and CTAs per SM.  Measured on configs[1]: 1 x 1024
+constexpr int kBinCtasPerSm = 1;               // threads 4.69 ms, 2 x 512 threads (half-length staging rows) 5.53 ms
+constexpr int kBinAccThreads = 1024;           // CTA size of pass 2 (one CTA per SM: the tile fills shared memory)
 
 struct BinParams {
     uint32_t *pool;        // nb * kBinBlockRecords records

@@ -105,7 +105,9 @@ __device__ __forceinline__ uint32_t iterate_block(const RenderParams &prm, const
         // ALU-bound variant: the generator recurrence is short (LDS + FMAs), the chain and pixel
         // arithmetic of the four iterations are independent of one another once the four generator
         // states exist -- written as straight-line stages so that the four dependent chains
-        // (LDS -> FMA -> MUFU -> FMA -> F2I -> ATOMS) interleave instead of running back to back
+        // (LDS -> FMA -> MUFU -> FMA -> F2I -> ATOMS) can interleave.  (The same staging of the four
+        // depth-buffer loads of SPLAT_DEPTH was measured slower, 324 vs 309 ms on configs[4]: that
+        // path is bound by the SM-to-L2 request rate, not by load latency.)
         float X[4], Y[4], Z[4];
         int K[4];
         bool ok[4];
@@ -150,7 +152,7 @@ __device__ __forceinline__ uint32_t iterate_block(const RenderParams &prm, const
 // ---------------------------------------------------------------------------------------------
 // the kernel
 template <int DIM, int GEN, int AFF, int SPLAT, uint32_t SIG, int TRIG>
-__global__ void __launch_bounds__(SPLAT == SPLAT_BIN ? kBinThreads : kRenderThreads, SPLAT == SPLAT_BIN ? 1 : 0)
+__global__ void __launch_bounds__(SPLAT == SPLAT_BIN ? kBinThreads : kRenderThreads, SPLAT == SPLAT_BIN ? kBinCtasPerSm : 0)
 render_kernel(const __grid_constant__ RenderParams prm)
 {
     __shared__ SharedTables s;
