@@ -86,6 +86,9 @@ typedef enum {
     CFS_VARIANT_SHARED_HIST = 2, /* HIST only, W*H*4 <= cfs_shared_hist_max_bytes(): per-CTA shared   */
                                  /* histogram, merged with red.global                                 */
     CFS_VARIANT_WARP_AGG = 3,    /* DIRECT + __match_any_sync aggregation of same-pixel hits (HIST)   */
+    CFS_VARIANT_CLUSTER_HIST = 5,/* HIST, IFS generator, W*H*4 <= 8 x (shared memory of a CTA): the histogram is   */
+                                 /* distributed over the shared memory of 8-CTA thread-block clusters, splats are */
+                                 /* red.shared::cluster through DSMEM, slices merged with red.global              */
     CFS_VARIANT_BINNED = 4       /* HIST, or RGBA + MAP_INDEX with <= 16 functions, IFS generator:    */
                                  /* splats are partitioned by image tile through d_scratch (one       */
                                  /* 4-byte record each), then every tile is accumulated in shared     */

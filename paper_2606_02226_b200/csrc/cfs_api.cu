@@ -509,6 +509,48 @@ extern "C" uint64_t cfs_shared_hist_max_bytes(void)
 
 namespace {
 
+// bins per CTA (log2) of the cluster histogram, or -1 when the image does not fit a cluster
+int cluster_slice_shift(size_t hist_bytes, const DeviceInfo &di)
+{
+    const size_t bins = hist_bytes / 4;
+    int shift = 8;
+    while (((size_t)cfs::kClusterSize << shift) < bins) ++shift;
+    const long lim = (long)di.smem_optin - (long)sizeof(cfs::SharedTables) - 2048;
+    return ((long)(4ull << shift) <= lim) ? shift : -1;
+}
+
+// histogram distributed over the shared memory of 8-CTA clusters (DSMEM reductions), one CTA per SM
+cfs_status render_cluster_hist(const cfs_system *s, const cfs_render_args *a, RenderParams &p, const DeviceInfo &di, cudaStream_t st)
+{
+    if (a->out_mode != CFS_OUT_HIST_U32 || s->gen != CFS_GEN_IFS) return fail(CFS_ERR_UNSUPPORTED, "cluster histogram needs HIST_U32 output and an IFS generator");
+    const size_t hist_bytes = (size_t)a->width * a->height * 4;
+    const int shift = cluster_slice_shift(hist_bytes, di);
+    if (shift < 0) return fail(CFS_ERR_UNSUPPORTED, "image of %zu bytes does not fit the shared memory of a %d-CTA cluster", hist_bytes, cfs::kClusterSize);
+    render_fn fn = pick_kernel(s, p, cfs::SPLAT_HIST_CLUSTER, a->flags);
+    if (!fn) return fail(CFS_ERR_UNSUPPORTED, "no cluster-histogram kernel for this system");
+    const size_t dyn = (size_t)4 << shift;
+    cudaError_t e = cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute");
+    p.hist_bins = (uint32_t)(hist_bytes / 4);
+    p.slice_shift = (uint32_t)shift;
+    cudaLaunchConfig_t cfg = {};
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = cfs::kClusterSize; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.blockDim = dim3(cfs::kClusterThreads); cfg.dynamicSmemBytes = dyn; cfg.stream = st; cfg.attrs = attr; cfg.numAttrs = 1;
+    cfg.gridDim = dim3(cfs::kClusterSize);
+    int max_clusters = 0;
+    e = cudaOccupancyMaxActiveClusters(&max_clusters, (const void *)fn, &cfg);
+    if (e != cudaSuccess || max_clusters < 1) { cudaGetLastError(); return fail(CFS_ERR_UNSUPPORTED, "no co-resident %d-CTA cluster with %zu bytes of shared memory", cfs::kClusterSize, dyn); }
+    uint64_t clusters = (a->n_points + (uint64_t)cfs::kClusterSize * cfs::kClusterThreads - 1) / ((uint64_t)cfs::kClusterSize * cfs::kClusterThreads);
+    if (clusters > (uint64_t)max_clusters) clusters = (uint64_t)max_clusters;     // persistent: grid-stride over points
+    cfg.gridDim = dim3((unsigned)(clusters * cfs::kClusterSize));
+    e = cudaLaunchKernelEx(&cfg, fn, p);
+    ++g_launches;
+    if (e != cudaSuccess) return cuda_fail(e, "cluster histogram launch");
+    return CFS_OK;
+}
+
 // tile-binned render: per chunk of points, clear the bin heads, pass 1 (sample + bin), pass 2
 // (accumulate tiles in shared memory, merge).  `force`: the caller asked for this variant, so
 // report why it cannot run; otherwise return UNSUPPORTED quietly and let AUTO fall back.
@@ -554,7 +596,7 @@ extern "C" cfs_status cfs_render(const cfs_system *s, const cfs_render_args *a, 
     RenderParams p;
     cfs_status st = build_params(s, a, &p, true);
     if (st != CFS_OK) return st;
-    if (a->variant < CFS_VARIANT_AUTO || a->variant > CFS_VARIANT_BINNED) return fail(CFS_ERR_INVALID_ARG, "unknown variant %d", a->variant);
+    if (a->variant < CFS_VARIANT_AUTO || a->variant > CFS_VARIANT_CLUSTER_HIST) return fail(CFS_ERR_INVALID_ARG, "unknown variant %d", a->variant);
     const DeviceInfo &di = device_info();
     if (di.ok != 1) return fail(CFS_ERR_CUDA, "no CUDA device (this library has no CPU fallback)");
     const size_t hist_bytes = (size_t)a->width * a->height * 4;
@@ -566,6 +608,10 @@ extern "C" cfs_status cfs_render(const cfs_system *s, const cfs_render_args *a, 
     if (a->variant == CFS_VARIANT_BINNED) {
         if (a->n_points == 0) return CFS_OK;
         return render_binned(s, a, p, di, (cudaStream_t)stream);
+    }
+    if (a->variant == CFS_VARIANT_CLUSTER_HIST) {
+        if (a->n_points == 0) return CFS_OK;
+        return render_cluster_hist(s, a, p, di, (cudaStream_t)stream);
     }
     if (a->variant == CFS_VARIANT_SHARED_HIST || a->variant == CFS_VARIANT_WARP_AGG) {
         if (a->out_mode != CFS_OUT_HIST_U32) return fail(CFS_ERR_UNSUPPORTED, "variant %d is for HIST_U32 output only", a->variant);

@@ -95,6 +95,26 @@ __device__ __forceinline__ void bin_append(const RenderParams &prm, const Shared
     else bin_direct(prm, s, tile, rec);
 }
 
+// The same as straight-line predicated code (no branch in the common case): the atomic and the store
+// carry predicates, `ok == false` leaves slot = 0xFFFFFFFF.  Returns the slot; the caller sends
+// records with cap <= slot < 0xFFFFFFFF down the direct path afterwards (rare).
+__device__ __forceinline__ uint32_t bin_try_append(const BinRegs &br, bool ok, uint32_t tile, uint32_t rec)
+{
+    uint32_t slot;
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\tmov.u32 %0, 0xffffffff;\n\t"
+                 "@p atom.shared.add.u32 %0, [%1], 1;\n\t}"
+                 : "=r"(slot) : "r"(br.cnt_addr + 4u * tile), "r"((uint32_t)ok) : "memory");
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.lt.u32 p, %2, %3;\n\t@p st.shared.u32 [%0], %1;\n\t}"
+                 :: "r"(br.buf_addr + tile * br.cap4 + 4u * slot), "r"(rec), "r"(slot), "r"(br.cap) : "memory");
+    return slot;
+}
+
+__device__ __forceinline__ void bin_record_of(const BinRegs &br, int pix, int k, uint32_t &tile, uint32_t &rec)
+{
+    tile = __umulhi((uint32_t)pix, br.magic) >> br.mshift;
+    rec = ((uint32_t)pix - tile * br.tp) * br.nk + ((uint32_t)k & br.kmask);
+}
+
 // Per-lane bin state of pass 1, kept in REGISTERS: lane l of warp w owns tile l * warps + w (so
 // n_tiles <= 32 * warps per CTA, and the rows to flush are spread over all warps of the CTA).  `next` is a pool block taken ahead of time: the global atomic
 // that hands it out is issued when the previous block is opened and its result is not needed

@@ -11,6 +11,8 @@ namespace cfs {
 constexpr int kMaxFuncs = 64;
 constexpr int kMaxChain = 8;
 constexpr int kRenderThreads = 256;   // CTA size of the render / trace kernels
+constexpr int kClusterThreads = 512;  // CTA size of the cluster-histogram variant (one CTA per SM, 16 warps)
+constexpr int kClusterSize = 8;       // CTAs per cluster (portable maximum)
 
 // affine table forms (bit-identical results, DESIGN R4: fma(0,y,b) == b)
 enum AffForm : int { AFF_GENERAL = 0, AFF_DIAG = 1 };
@@ -46,6 +48,8 @@ enum SplatKind : int {
     SPLAT_RGBA = 3,          // red.global.add.v4.f32
     SPLAT_DEPTH = 4,         // ld.global.cg pre-test + atom.global.min.u64
     SPLAT_NONE = 5,          // trace kernel
+    SPLAT_HIST_CLUSTER = 7,  // histogram distributed over the shared memory of a thread-block cluster
+                             // (red.shared::cluster.add.u32 through DSMEM), merged by red.global
     SPLAT_BIN = 6            // tile-binned: records partitioned by image tile into a block pool
                              // (pass 1), accumulated per tile in shared memory (pass 2)
 };
@@ -101,7 +105,8 @@ struct RenderParams {
     int32_t n_thr;               // thresholds below 2^32 (k = #{j < n_thr : u >= T[j]})
     int32_t pick_steps;          // max thresholds inside one 2^24 bucket of u
     uint32_t points_per_thread;  // shared-hist persistent grid
-    uint32_t hist_bins;          // W*H (shared-hist variant)
+    uint32_t hist_bins;          // W*H (shared-hist and cluster-hist variants)
+    uint32_t slice_shift;        // cluster-hist: bins per CTA = 1 << slice_shift, bin b lives in CTA rank b >> slice_shift
 
     BinParams bin;               // SPLAT_BIN only
 

@@ -26,6 +26,22 @@ __device__ __forceinline__ void red_add_u32(uint32_t *addr, uint32_t v)
     asm volatile("red.global.add.u32 [%0], %1;" :: "l"(addr), "r"(v) : "memory");
 }
 
+// cluster histogram: bin `pix` lives in the shared memory of CTA rank pix >> slice_shift of this
+// cluster; one remote shared-memory reduction through DSMEM, no L2 traffic
+__device__ __forceinline__ void splat_hist_cluster(uint32_t s_hist_addr, uint32_t slice_shift, int pix)
+{
+    const uint32_t rank = (uint32_t)pix >> slice_shift;
+    const uint32_t local = s_hist_addr + 4u * ((uint32_t)pix & ((1u << slice_shift) - 1u));
+    uint32_t remote;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(local), "r"(rank));
+    asm volatile("red.relaxed.cluster.shared::cluster.add.u32 [%0], 1;" :: "r"(remote) : "memory");
+}
+
+__device__ __forceinline__ void cluster_sync_all()
+{
+    asm volatile("barrier.cluster.arrive.release;\n\tbarrier.cluster.wait.acquire;" ::: "memory");
+}
+
 __device__ __forceinline__ void splat_hist_warpagg(uint32_t *hist, int pix, bool valid)
 {
     // ballot/match aggregation of same-pixel hits before the atomic (BASELINE north_star).
@@ -72,6 +88,8 @@ __device__ __forceinline__ uint32_t chain_and_splat(const RenderParams &prm, con
         red_add_u32(reinterpret_cast<uint32_t *>(prm.image) + pix, 1u);
     } else if (SPLAT == SPLAT_HIST_SHARED) {
         atomicAdd(&s_hist[pix], 1u);
+    } else if (SPLAT == SPLAT_HIST_CLUSTER) {
+        splat_hist_cluster((uint32_t)__cvta_generic_to_shared(s_hist), prm.slice_shift, pix);
     } else if (SPLAT == SPLAT_RGBA) {
         float *dst = reinterpret_cast<float *>(prm.image) + 4 * (size_t)pix;
         if (GEN == 1) {   // colour of the point record, integer-valued (DESIGN R9)
@@ -123,10 +141,19 @@ __device__ __forceinline__ uint32_t iterate_block(const RenderParams &prm, const
             const bool alive = apply_chain<DIM, SIG, TRIG>(prm, X[j], Y[j], Z[j]);
             ok[j] = alive && have && in_bounds(prm, X[j], Y[j]);
         }
+        uint32_t tile[4], rec[4], slot[4];
+        bool overflow = false;
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            if (ok[j]) bin_append(prm, s, br, bin_pixel_of(br, X[j], Y[j]), K[j]);
-            else ++dropped;
+        for (int j = 0; j < 4; ++j) {      // out-of-bounds coordinates are clamped by the pixel rule: always a valid tile
+            bin_record_of(br, bin_pixel_of(br, X[j], Y[j]), K[j], tile[j], rec[j]);
+            slot[j] = bin_try_append(br, ok[j], tile[j], rec[j]);
+            dropped += ok[j] ? 0u : 1u;
+            overflow = overflow || (slot[j] >= br.cap && slot[j] != 0xFFFFFFFFu);
+        }
+        if (overflow) {                    // staging row full: those records take the direct path
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+                if (slot[j] >= br.cap && slot[j] != 0xFFFFFFFFu) bin_direct(prm, s, tile[j], rec[j]);
         }
     } else {
 #pragma unroll(CHECKED ? 1 : 4)
@@ -152,7 +179,8 @@ __device__ __forceinline__ uint32_t iterate_block(const RenderParams &prm, const
 // ---------------------------------------------------------------------------------------------
 // the kernel
 template <int DIM, int GEN, int AFF, int SPLAT, uint32_t SIG, int TRIG>
-__global__ void __launch_bounds__(SPLAT == SPLAT_BIN ? kBinThreads : kRenderThreads, SPLAT == SPLAT_BIN ? kBinCtasPerSm : 0)
+__global__ void __launch_bounds__(SPLAT == SPLAT_BIN ? kBinThreads : SPLAT == SPLAT_HIST_CLUSTER ? kClusterThreads : kRenderThreads,
+                                  SPLAT == SPLAT_BIN ? kBinCtasPerSm : 0)
 render_kernel(const __grid_constant__ RenderParams prm)
 {
     __shared__ SharedTables s;
@@ -160,6 +188,10 @@ render_kernel(const __grid_constant__ RenderParams prm)
     if (GEN == 0) load_tables(s, prm);
     if (SPLAT == SPLAT_HIST_SHARED)
         for (uint32_t i = threadIdx.x; i < prm.hist_bins; i += blockDim.x) s_hist[i] = 0u;
+    if (SPLAT == SPLAT_HIST_CLUSTER) {   // this CTA's slice; nobody may touch a peer's slice before it is cleared
+        for (uint32_t i = threadIdx.x; i < (1u << prm.slice_shift); i += blockDim.x) s_hist[i] = 0u;
+        cluster_sync_all();
+    }
     BinLane bl = {0u, 0u, 0u};
     BinRegs br = {};
     __shared__ BinRegs s_br;
@@ -217,6 +249,17 @@ render_kernel(const __grid_constant__ RenderParams prm)
     if (SPLAT == SPLAT_BIN) {           // write out what is left in the staging rows
         __syncthreads();
         bin_flush(prm, s, s_hist, bl, true);
+    }
+    if (SPLAT == SPLAT_HIST_CLUSTER) {  // all peers done with my slice, then merge it (red.global, non-zero bins)
+        cluster_sync_all();
+        uint32_t rank;
+        asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(rank));
+        uint32_t *hist = reinterpret_cast<uint32_t *>(prm.image);
+        const uint32_t base = rank << prm.slice_shift;
+        for (uint32_t i = threadIdx.x; i < (1u << prm.slice_shift) && base + i < prm.hist_bins; i += blockDim.x) {
+            const uint32_t v = s_hist[i];
+            if (v) red_add_u32(hist + base + i, v);
+        }
     }
     if (SPLAT == SPLAT_HIST_SHARED) {   // merge the private histogram (red.global, non-zero bins only)
         __syncthreads();

@@ -16,6 +16,7 @@ render_fn select_splat(int splat)
     CFS_CASE(SPLAT_HIST_DIRECT)
     CFS_CASE(SPLAT_HIST_SHARED)
     CFS_CASE(SPLAT_HIST_WARPAGG)
+    if constexpr (GEN == 0) { CFS_CASE(SPLAT_HIST_CLUSTER) }
     CFS_CASE(SPLAT_RGBA)
     if constexpr (DIM == 3) { CFS_CASE(SPLAT_DEPTH) }
     if constexpr (GEN == 0) { CFS_CASE(SPLAT_BIN) }
@@ -40,7 +41,7 @@ render_fn select_trace(int gen, int aff)
     return trace_kernel<DIM, 0, AFF_GENERAL, SIG, TRIG>;
 }
 
-constexpr unsigned kSplatsAll = (1u << SPLAT_HIST_DIRECT) | (1u << SPLAT_HIST_SHARED) | (1u << SPLAT_HIST_WARPAGG) |
+constexpr unsigned kSplatsAll = (1u << SPLAT_HIST_DIRECT) | (1u << SPLAT_HIST_SHARED) | (1u << SPLAT_HIST_WARPAGG) | (1u << SPLAT_HIST_CLUSTER) |
                                 (1u << SPLAT_RGBA) | (1u << SPLAT_DEPTH) | (1u << SPLAT_BIN);
 constexpr unsigned kSplatsDirect = (1u << SPLAT_HIST_DIRECT) | (1u << SPLAT_RGBA) | (1u << SPLAT_DEPTH) | (1u << SPLAT_BIN);
 

@@ -61,7 +61,7 @@ def test_point_offset_beyond_32_bits(cfs, oracle):
 
 
 # ------------------------------------------------------------------ (iii): bit-exact images
-@pytest.mark.parametrize("variant", ["direct", "warp_agg", "auto"])
+@pytest.mark.parametrize("variant", ["direct", "warp_agg", "cluster_hist", "auto"])
 def test_cfg0_histogram_bit_exact(cfs, oracle, variant):
     w = W.config(0).scaled(n_points=4096 + 99)
     g, gc = gpu_render(cfs, w, variant=variant)
@@ -71,7 +71,7 @@ def test_cfg0_histogram_bit_exact(cfs, oracle, variant):
 
 
 @pytest.mark.parametrize("size", [(64, 64), (200, 120), (224, 224)])
-@pytest.mark.parametrize("variant", ["shared_hist", "direct", "warp_agg", "auto"])
+@pytest.mark.parametrize("variant", ["shared_hist", "direct", "warp_agg", "cluster_hist", "auto"])
 def test_small_histograms_all_variants(cfs, oracle, size, variant):
     """Per-CTA shared-memory privatised histogram (and the others) on images that fit shared memory;
     bounds narrower than the attractor so that some splats are dropped."""
