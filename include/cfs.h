@@ -156,6 +156,13 @@ cfs_status cfs_render(const cfs_system *sys, const cfs_render_args *args, void *
  * direct path otherwise. */
 uint64_t cfs_binned_scratch_bytes(const cfs_system *sys, const cfs_render_args *args);
 
+/* the tile plan of the BINNED variant for an image and a device shape, host arithmetic only (no device
+ * needed; test instrument): out = { tiles, pixels per tile, magic, shift (tile of pixel p =
+ * mulhi32(p, magic) >> shift), colour bits, staging records per tile, flush-check interval in
+ * iterations, pass-2 CTAs per tile }.  UNSUPPORTED when the variant cannot serve the image. */
+cfs_status cfs_binned_plan(int32_t width, int32_t height, int32_t out_mode, int32_t n_funcs, int32_t sms,
+                           int32_t smem_per_block_optin, uint32_t out[8]);
+
 /* cfs_render_host -- same path with HOST buffers (end-to-end entry point): copies h_cloud to the
  * device (CLOUD), clears a device image, renders [point_offset, +n_points), copies the image to
  * h_image (layout of out_mode) and the counters to h_counters (u64[2], optional); synchronises

@@ -27,7 +27,7 @@ VARIANT = {"auto": 0, "direct": 1, "shared_hist": 2, "warp_agg": 3, "binned": 4,
 MB = {"red_add_u32": 0, "red_add_v4f32": 1, "atom_min_u64": 2, "ld_u64": 3, "atoms_add_u32": 4,
       "ffma": 5, "imad_wide": 6, "lop3": 7, "mufu": 8, "stream_ld128": 9}
 EXPORTS = ["cfs_create", "cfs_destroy", "cfs_render", "cfs_render_host", "cfs_tonemap", "cfs_trace",
-           "cfs_microbench", "cfs_shared_hist_max_bytes", "cfs_binned_scratch_bytes", "cfs_launch_count", "cfs_last_error",
+           "cfs_microbench", "cfs_shared_hist_max_bytes", "cfs_binned_scratch_bytes", "cfs_binned_plan", "cfs_launch_count", "cfs_last_error",
            "cfs_version"]
 
 
@@ -90,6 +90,9 @@ def lib():
         L.cfs_shared_hist_max_bytes.restype = C.c_uint64
         L.cfs_binned_scratch_bytes.argtypes = [C.c_void_p, C.POINTER(cfs_render_args)]
         L.cfs_binned_scratch_bytes.restype = C.c_uint64
+        L.cfs_binned_plan.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32,
+                                      C.POINTER(C.c_uint32)]
+        L.cfs_binned_plan.restype = C.c_int
         L.cfs_launch_count.argtypes = [C.c_int32]
         L.cfs_launch_count.restype = C.c_uint64
         L.cfs_last_error.argtypes = []
@@ -213,6 +216,14 @@ def make_args(render, d_image=None, d_cloud=None, d_counters=None, n_points=None
 
 def cfs_binned_scratch_bytes(sys: System, args: cfs_render_args) -> int:
     return int(lib().cfs_binned_scratch_bytes(sys.handle, C.byref(args)))
+
+
+def cfs_binned_plan(width: int, height: int, out_mode, n_funcs: int, sms: int = 148, smem_optin: int = 232448) -> dict:
+    mode = OUT[out_mode] if isinstance(out_mode, str) else int(out_mode)
+    out = (C.c_uint32 * 8)()
+    _check(lib().cfs_binned_plan(int(width), int(height), mode, int(n_funcs), int(sms), int(smem_optin), out))
+    keys = ["n_tiles", "tile_pixels", "magic", "mshift", "kbits", "cap", "check_every", "split"]
+    return dict(zip(keys, [int(v) for v in out]))
 
 
 def cfs_render(sys: System, args: cfs_render_args, stream=None) -> None:

@@ -375,17 +375,18 @@ constexpr size_t kBinBlockBytes = cfs::kBinBlockRecords * 4;
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 // tiles and staging rows; false when the variant cannot serve this system / image
-bool bin_shape(const cfs_system *s, const cfs_render_args *a, const DeviceInfo &di, BinPlan *pl, const char **why)
+bool bin_shape_raw(int gen, int out_mode, int color, uint32_t n_funcs, int32_t width, int32_t height, const DeviceInfo &di,
+                   BinPlan *pl, const char **why)
 {
-    if (s->gen != CFS_GEN_IFS) { *why = "binned variant needs an IFS generator"; return false; }
-    if (a->out_mode == CFS_OUT_DEPTH_RGBA8_U64) { *why = "binned variant serves HIST and RGBA output"; return false; }
+    if (gen != CFS_GEN_IFS) { *why = "binned variant needs an IFS generator"; return false; }
+    if (out_mode == CFS_OUT_DEPTH_RGBA8_U64) { *why = "binned variant serves HIST and RGBA output"; return false; }
     uint32_t kbits = 0;
-    if (a->out_mode == CFS_OUT_RGBA_F32) {
-        if (s->color != CFS_COLOR_MAP_INDEX) { *why = "binned RGBA needs COLOR_MAP_INDEX"; return false; }
-        while ((1u << kbits) < (uint32_t)s->funcs.size()) ++kbits;
+    if (out_mode == CFS_OUT_RGBA_F32) {
+        if (color != CFS_COLOR_MAP_INDEX) { *why = "binned RGBA needs COLOR_MAP_INDEX"; return false; }
+        while ((1u << kbits) < n_funcs) ++kbits;
         if (kbits > 4) { *why = "binned RGBA supports at most 16 functions"; return false; }
     }
-    const uint64_t n_pix = (uint64_t)a->width * a->height;
+    const uint64_t n_pix = (uint64_t)width * height;
     if (n_pix > (1ull << 28)) { *why = "binned variant serves images up to 2^28 pixels"; return false; }
     // pass 2 keeps (pixels per tile) << kbits counters in shared memory: at most 3 * 2^14 (192 KiB).
     // Fewer, larger tiles leave longer staging rows in pass 1, hence fewer barriers; but at least
@@ -445,6 +446,11 @@ size_t bin_fixed_bytes(const BinPlan &pl)
     return kBinCtrlBytes + align_up((size_t)pl.bp.n_tiles * pl.grid1 * 4, 256) + 1024;
 }
 
+bool bin_shape(const cfs_system *s, const cfs_render_args *a, const DeviceInfo &di, BinPlan *pl, const char **why)
+{
+    return bin_shape_raw(s->gen, a->out_mode, s->color, (uint32_t)s->funcs.size(), a->width, a->height, di, pl, why);
+}
+
 // scratch needed to render `points` points in one chunk
 uint64_t bin_scratch_for(const BinPlan &pl, uint64_t points, uint64_t splats_per_point)
 {
@@ -490,6 +496,21 @@ bool bin_layout(BinPlan *pl, void *scratch, uint64_t bytes, uint64_t n_points, u
 }
 
 }  // namespace
+
+// host-only view of the plan (no device needed): lets the CPU tests check the tile arithmetic
+extern "C" cfs_status cfs_binned_plan(int32_t width, int32_t height, int32_t out_mode, int32_t n_funcs, int32_t sms,
+                                      int32_t smem_per_block_optin, uint32_t out[8])
+{
+    if (!out || width < 1 || height < 1 || sms < 1 || n_funcs < 1) return fail(CFS_ERR_INVALID_ARG, "bad plan arguments");
+    DeviceInfo di; di.ok = 1; di.sms = sms; di.smem_optin = smem_per_block_optin; di.smem_sm = smem_per_block_optin + 1024;
+    BinPlan pl;
+    const char *why = "";
+    if (!bin_shape_raw(CFS_GEN_IFS, out_mode, out_mode == CFS_OUT_RGBA_F32 ? CFS_COLOR_MAP_INDEX : CFS_COLOR_NONE, (uint32_t)n_funcs,
+                       width, height, di, &pl, &why)) return fail(CFS_ERR_UNSUPPORTED, "%s", why);
+    out[0] = pl.bp.n_tiles; out[1] = pl.bp.tile_pixels; out[2] = pl.bp.magic; out[3] = pl.bp.mshift;
+    out[4] = pl.bp.kbits; out[5] = pl.bp.cap; out[6] = 4u * (pl.bp.check_mask + 1u); out[7] = pl.bp.split;
+    return CFS_OK;
+}
 
 extern "C" uint64_t cfs_binned_scratch_bytes(const cfs_system *s, const cfs_render_args *a)
 {

@@ -227,21 +227,32 @@ bin_accumulate_kernel(const __grid_constant__ RenderParams prm)
         const uint32_t tail = b.tails[(size_t)tile * b.grid + c];
         const uint32_t n_blk = tail >> 10, last_fill = tail & 1023u;
         const uint32_t *list = b.list + ((size_t)tile * b.grid + c) * b.lcap;
-        for (uint32_t j = part; j < n_blk; j += b.split) {
-            const uint32_t blk = list[j];
-            const uint32_t fill = (j + 1u == n_blk) ? last_fill : kBinBlockRecords;
-            const uint4 *src = reinterpret_cast<const uint4 *>(b.pool + (size_t)blk * kBinBlockRecords);
-            uint4 v[4];
+        // two blocks (2 x 2 KiB, eight 128-bit loads per lane) in flight per warp before their atomics
+        for (uint32_t j = part; j < n_blk; j += 2u * b.split) {
+            uint4 v[2][4];
+            uint32_t fill[2];
 #pragma unroll
-            for (int q = 0; q < 4; ++q)     // 4 x 512 B, issued together
-                v[q] = (q * 128u < fill) ? __ldcs(src + q * 32 + lane) : make_uint4(0u, 0u, 0u, 0u);
+            for (int h = 0; h < 2; ++h) {
+                const uint32_t jj = j + (uint32_t)h * b.split;
+                fill[h] = 0u;
+                if (jj < n_blk) {
+                    fill[h] = (jj + 1u == n_blk) ? last_fill : kBinBlockRecords;
+                    const uint4 *src = reinterpret_cast<const uint4 *>(b.pool + (size_t)list[jj] * kBinBlockRecords);
 #pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                const uint32_t base = q * 128u + 4u * lane;
-                if (base + 0u < fill) atomicAdd(&acc[v[q].x], 1u);
-                if (base + 1u < fill) atomicAdd(&acc[v[q].y], 1u);
-                if (base + 2u < fill) atomicAdd(&acc[v[q].z], 1u);
-                if (base + 3u < fill) atomicAdd(&acc[v[q].w], 1u);
+                    for (int q = 0; q < 4; ++q)
+                        v[h][q] = (q * 128u < fill[h]) ? __ldcs(src + q * 32 + lane) : make_uint4(0u, 0u, 0u, 0u);
+                }
+            }
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const uint32_t base = q * 128u + 4u * lane;
+                    if (base + 0u < fill[h]) atomicAdd(&acc[v[h][q].x], 1u);
+                    if (base + 1u < fill[h]) atomicAdd(&acc[v[h][q].y], 1u);
+                    if (base + 2u < fill[h]) atomicAdd(&acc[v[h][q].z], 1u);
+                    if (base + 3u < fill[h]) atomicAdd(&acc[v[h][q].w], 1u);
+                }
             }
         }
     }

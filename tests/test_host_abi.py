@@ -1,0 +1,108 @@
+"""CPU-side checks of the C ABI (no compute): the library loads, exports every function
+include/cfs.h declares, validates arguments on the host, refuses to work without a device (there is
+no CPU fallback), and plans the tiles of the binned variant with exact integer arithmetic."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+from paper_2606_02226_b200 import build as cuda_build
+from paper_2606_02226_b200 import workloads as W
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def cfs():
+    cuda_build.build()                       # nvcc cross-compiles without a GPU
+    from paper_2606_02226_b200 import cfs as mod
+    mod.lib()
+    return mod
+
+
+def _declared_functions():
+    text = open(os.path.join(ROOT, "include", "cfs.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(cfs_[a-z0-9_]+)\s*\(", text)))
+
+
+def test_library_exports_every_declared_function(cfs):
+    names = _declared_functions()
+    assert {"cfs_create", "cfs_render", "cfs_tonemap", "cfs_destroy", "cfs_render_host", "cfs_trace",
+            "cfs_microbench", "cfs_binned_scratch_bytes", "cfs_binned_plan", "cfs_last_error"} <= set(names)
+    lib = C.CDLL(cfs.LIB_PATH)
+    for n in names:
+        assert hasattr(lib, n), f"{n} is declared in include/cfs.h but not exported"
+    assert set(cfs.EXPORTS) == set(names)                 # the Python binding carries the same names
+    assert "sm_100a" in cfs.cfs_version()
+
+
+def test_create_validates_on_the_host(cfs):
+    sysh = cfs.cfs_create(W.config(1).system)             # host only: no device work
+    sysh.close()
+    for bad in (W.System(4, "ifs", W.square_funcs(), [], "none"),
+                W.System(2, "ifs", [W.Func("affine", -1.0, [0.5, 0, 0, 0.5, 0, 0])], [], "none"),
+                W.System(2, "ifs", [W.Func("affine", 0.0, [0.5, 0, 0, 0.5, 0, 0])], [], "none"),
+                W.System(2, "ifs", W.square_funcs(), [], "point"),
+                W.System(2, "ifs", W.square_funcs(), [W.Xform("affine")] * 9, "none"),
+                W.System(2, "ifs", W.square_funcs(), [], "map_index", None)):
+        with pytest.raises(cfs.CfsError) as ei:
+            cfs.cfs_create(bad)
+        assert ei.value.status == cfs.CFS_ERR_INVALID_ARG and cfs.cfs_last_error()
+
+
+def test_no_cpu_fallback(cfs):
+    """Without a CUDA device every working call fails loudly with CFS_ERR_CUDA."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    w = W.config(0).scaled(n_points=16)
+    sysh = cfs.cfs_create(w.system)
+    img = np.zeros(512 * 512, np.uint32)
+    with pytest.raises(cfs.CfsError) as ei:
+        cfs.cfs_render(sysh, cfs.make_args(w.render, d_image=img), stream=0)
+    assert ei.value.status == cfs.CFS_ERR_CUDA and "no CPU fallback" in str(ei.value)
+    with pytest.raises(cfs.CfsError) as ei:
+        cfs.cfs_render_host(sysh, cfs.make_args(w.render), img, None, None, stream=0)
+    assert ei.value.status == cfs.CFS_ERR_CUDA
+    assert cfs.cfs_binned_scratch_bytes(sysh, cfs.make_args(w.render)) == 0
+    sysh.close()
+
+
+SIZES = [(512, 512), (1024, 1024), (1920, 1080), (3840, 2160), (64, 64), (200, 120), (1, 1), (4097, 3), (7, 9001),
+         (16384, 16384), (12288, 1), (333, 777)]
+
+
+@pytest.mark.parametrize("mode,n_funcs", [("hist_u32", 1), ("rgba_f32", 3), ("rgba_f32", 4), ("rgba_f32", 16)])
+@pytest.mark.parametrize("size", SIZES)
+def test_binned_plan_tile_arithmetic_is_exact(cfs, size, mode, n_funcs):
+    """tile(p) = mulhi32(p, magic) >> shift must equal p // tile_pixels for EVERY pixel of the image
+    (checked at all tile boundaries and on a random sample), and the plan must respect the shared-
+    memory budgets of both passes."""
+    wd, ht = size
+    n_pix = wd * ht
+    try:
+        pl = cfs.cfs_binned_plan(wd, ht, mode, n_funcs)
+    except cfs.CfsError as e:
+        assert e.status == cfs.CFS_ERR_UNSUPPORTED          # too many tiles for 160-record staging rows
+        kbits = 0 if mode == "hist_u32" else (n_funcs - 1).bit_length()
+        assert -(-n_pix // (3 << (14 - kbits))) > 300
+        return
+    tp, nt = pl["tile_pixels"], pl["n_tiles"]
+    assert nt == -(-n_pix // tp) and nt <= 1024
+    assert tp & (tp - 1) == 0 or (tp % 3 == 0 and (tp // 3) & (tp // 3 - 1) == 0)      # 2^s or 3 * 2^s
+    assert (tp << pl["kbits"]) * 4 <= 192 << 10                                        # pass 2 counters
+    assert (1 << pl["kbits"]) >= n_funcs or mode == "hist_u32"
+    assert pl["cap"] >= 160 and pl["cap"] % 32 == 0
+    assert (nt * pl["cap"] + nt + 4) * 4 <= 232448                                      # pass 1 staging rows
+    assert pl["check_every"] in (4, 8, 16, 32) and pl["split"] >= 1
+    edges = np.arange(0, nt + 1, dtype=np.uint64) * np.uint64(tp)
+    p = np.unique(np.concatenate([edges, edges[1:] - np.uint64(1), edges[:-1] + np.uint64(1),
+                                  np.random.default_rng(1).integers(0, n_pix, 4096, dtype=np.uint64),
+                                  np.array([0, n_pix - 1], dtype=np.uint64)]))
+    p = p[p < n_pix]
+    got = ((p * np.uint64(pl["magic"])) >> np.uint64(32)) >> np.uint64(pl["mshift"])
+    assert np.array_equal(got, p // np.uint64(tp))
+    assert pl["magic"] < 1 << 32
