@@ -399,10 +399,10 @@ def run_ours(args):
             "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH, "kernel": "cfs::render_kernel<2,IFS,DIAG,BIN,swirl+affine,MUFU>",
             "kernel_ms": pass1_s * 1e3, "render_ms": t_render * 1e3, "pass2_ms": (t_render - pass1_s) * 1e3,
             "algorithmic_lane_instructions_per_point_iteration": n_instr,
-            "algorithmic_bytes_per_launch": int(S * 4),
+            "algorithmic_bytes_per_launch": int(S * 2),      # one 16-bit record per splat
             "peak_source": "FFMA lane-issue rate of cfs_microbench in this run (148 SMs x 128 lanes x SM clock)",
             "hbm_peak_gbs": peaks.get("hbm_gbs"), "hbm_peak_source": peaks_src,
-            "pass2_hbm_gbs": S * 4 / max(t_render - pass1_s, 1e-9) / 1e9,
+            "pass2_hbm_gbs": S * 2 / max(t_render - pass1_s, 1e-9) / 1e9,
         }
     else:
         peak_red = rates[RED_KEY[HEADLINE_CFG]]

@@ -91,7 +91,7 @@ typedef enum {
                                  /* red.shared::cluster through DSMEM, slices merged with red.global              */
     CFS_VARIANT_BINNED = 4       /* HIST, or RGBA + MAP_INDEX with <= 16 functions, IFS generator:    */
                                  /* splats are partitioned by image tile through d_scratch (one       */
-                                 /* 4-byte record each), then every tile is accumulated in shared     */
+                                 /* 2-byte record each), then every tile is accumulated in shared     */
                                  /* memory and merged with red.global; no L2 atomic per splat         */
 } cfs_variant;
 

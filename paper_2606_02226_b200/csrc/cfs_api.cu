@@ -370,7 +370,7 @@ struct BinPlan {
 };
 
 constexpr size_t kBinCtrlBytes = 256;
-constexpr size_t kBinBlockBytes = cfs::kBinBlockRecords * 4;
+constexpr size_t kBinBlockBytes = cfs::kBinBlockRecords * 2;      // 16-bit records
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
@@ -403,10 +403,10 @@ bool bin_shape_raw(int gen, int out_mode, int color, uint32_t n_funcs, int32_t w
     // kBinCtasPerSm CTAs of pass 1 share the SM's shared memory (1 KiB per CTA is reserved by the system)
     const long budget = ((long)di.smem_sm / cfs::kBinCtasPerSm < (long)di.smem_optin ? (long)di.smem_sm / cfs::kBinCtasPerSm : (long)di.smem_optin)
                         - (long)sizeof(cfs::SharedTables) - 2048;
-    const long words = budget / 4 - (long)n_tiles - 4;
-    long cap = words / (long)n_tiles / 32 * 32;
-    if (cap > 1024) cap = 1024;
-    if (cap < 160) { *why = "image has too many tiles for the binned variant's staging rows"; return false; }
+    const long row_bytes = (budget - 4 * (long)n_tiles - 16) / (long)n_tiles;       // u32 cnt[] + u16 rows
+    long cap = row_bytes / 2 / 64 * 64;
+    if (cap > 4096) cap = 4096;
+    if (cap < 320) { *why = "image has too many tiles for the binned variant's staging rows"; return false; }
     cfs::BinParams &b = pl->bp;
     memset(&b, 0, sizeof(b));
     b.n_tiles = (uint32_t)n_tiles; b.tile_pixels = mul << shift;
@@ -424,15 +424,15 @@ bool bin_shape_raw(int gen, int out_mode, int color, uint32_t n_funcs, int32_t w
         if (!found) { *why = "no exact tile division for this image size"; return false; }
     }
     // flush check every E iterations, E the largest power of two whose expected arrivals per row
-    // (with 50 % + 32 records of slack) fit above a nearly full flush unit
+    // (with 25 % + 16 records of slack; measured on configs[1]: 6.36 / 5.36 / 4.72 / 4.60 ms at 4 / 8 / 16 / 32) fit above a nearly full flush unit
     const double per_it = (double)cfs::kBinThreads / (double)n_tiles;
     const double room = (double)(cap - (long)cfs::kBinFlushRecords + 1);
-    uint32_t every = 32;
-    while (every > 4 && 1.5 * every * per_it + 32.0 > room) every >>= 1;
+    uint32_t every = 64;
+    while (every > 4 && 1.25 * every * per_it + 16.0 > room) every >>= 1;
     b.check_mask = every / 4 - 1;                      // in Philox blocks of 4 iterations
     b.split = (uint32_t)((4 * (uint64_t)di.sms + n_tiles - 1) / n_tiles);
     if (b.split < 1) b.split = 1;
-    pl->smem_pass1 = ((n_tiles + 3) / 4 * 4 + n_tiles * (size_t)cap) * 4;
+    pl->smem_pass1 = (n_tiles + 3) / 4 * 4 * 4 + n_tiles * (size_t)cap * 2;
     pl->smem_pass2 = ((size_t)b.tile_pixels << kbits) * 4;
     pl->grid1 = (uint32_t)di.sms * cfs::kBinCtasPerSm;
     return true;
@@ -471,9 +471,9 @@ bool bin_layout(BinPlan *pl, void *scratch, uint64_t bytes, uint64_t n_points, u
     const uint64_t pairs = (uint64_t)pl->grid1 * b.n_tiles;
     const size_t fixed = bin_fixed_bytes(*pl) + 32 * pairs + 1024;      // + the "+ 8" list entries of every pair
     if (bytes <= fixed) { *why = "scratch too small"; return false; }
-    // per block: 2 KiB of records + 16 B of list capacity
+    // per block: 2 KiB of records (1024 x 16 bit) + 16 B of list capacity
     uint64_t nb = (bytes - fixed) / (kBinBlockBytes + 16);
-    if (nb > (1u << 23) - 1) nb = (1u << 23) - 1;                 // record positions are 32-bit
+    if (nb > (1u << 22) - 1) nb = (1u << 22) - 1;                 // record positions are 32-bit
     const uint64_t partial = 2 * (pairs + 64);
     if (nb < partial + partial / 2) { *why = "scratch too small for the binned variant (two blocks per CTA and tile)"; return false; }
     const uint64_t lcap = bin_lcap(*pl, nb);
@@ -483,7 +483,7 @@ bool bin_layout(BinPlan *pl, void *scratch, uint64_t bytes, uint64_t n_points, u
     uint8_t *q = base + kBinCtrlBytes + align_up((size_t)pairs * 4, 256);
     pl->clear_bytes = (size_t)(q - base);
     b.list = (uint32_t *)q;  q += align_up((size_t)(pairs * lcap) * 4, 256);
-    b.pool = (uint32_t *)align_up((size_t)q, 512);
+    b.pool = (uint16_t *)align_up((size_t)q, 512);
     // records one chunk may produce: the blocks left after the prefetched / partial ones, with head-room
     const uint64_t rec_cap = (nb - partial) * 8 / 9 * cfs::kBinBlockRecords;
     uint64_t cp = rec_cap / splats_per_point;

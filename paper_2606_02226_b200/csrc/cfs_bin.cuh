@@ -6,8 +6,8 @@
 // memory (SURVEY 7 "hard parts" 1).  So the image is cut into tiles that do fit, and the splats
 // are partitioned by tile on their way through HBM:
 //
-//   pass 1 (render_kernel<..., SPLAT_BIN>): each splat becomes ONE 32-bit record
-//     (pixel-in-tile << kbits | colour index), appended with one shared-memory atomic to the CTA's
+//   pass 1 (render_kernel<..., SPLAT_BIN>): each splat becomes ONE 16-bit record
+//     (pixel-in-tile * colour slots + colour index), appended with one shared-memory atomic to the CTA's
 //     staging row of its tile; full rows leave as 512-byte coalesced stores into 2 KiB pool blocks
 //     owned by (CTA, tile), so no global atomic is paid per splat -- one per 512 records.
 //   pass 2 (bin_accumulate_kernel): one CTA per (tile, part) walks the tile's block list with
@@ -34,7 +34,7 @@ __device__ __forceinline__ void bin_red_add_u32(uint32_t *addr, uint32_t v)
     asm volatile("red.global.add.u32 [%0], %1;" :: "l"(addr), "r"(v) : "memory");
 }
 
-// shared-memory layout of pass 1 (dynamic): cnt[n_tiles] | pad to 16 B | buf[n_tiles][cap]
+// shared-memory layout of pass 1 (dynamic): u32 cnt[n_tiles] | pad to 16 B | u16 buf[n_tiles][cap]
 __device__ __forceinline__ uint32_t bin_buf_offset(uint32_t n_tiles) { return (n_tiles + 3u) & ~3u; }
 
 // one record down the direct path (staging row full, or no pool block for the tile)
@@ -53,7 +53,7 @@ __device__ __forceinline__ void bin_direct(const RenderParams &prm, const Shared
 // an access is one ATOMS / STS without generic-address arithmetic)
 struct BinRegs {
     uint32_t cnt_addr, buf_addr;   // shared addresses of cnt[] and buf[][]
-    uint32_t cap, cap4;            // row capacity in records / bytes
+    uint32_t cap, cap2;            // row capacity in records / bytes
     uint32_t tp, magic, mshift;    // tile = umulhi(pix, magic) >> mshift == pix / tp for every pixel of the image
     uint32_t nk, kmask;            // colour slots per pixel, and the mask that zeroes k for HIST
     float sx, ox, sy, oy;          // pixel map (DESIGN R8)
@@ -65,7 +65,7 @@ __device__ __forceinline__ BinRegs bin_regs_init(const RenderParams &prm, uint32
     BinRegs r;
     r.cnt_addr = (uint32_t)__cvta_generic_to_shared(sm);
     r.buf_addr = r.cnt_addr + 4u * bin_buf_offset(prm.bin.n_tiles);
-    r.cap = prm.bin.cap; r.cap4 = 4u * prm.bin.cap;
+    r.cap = prm.bin.cap; r.cap2 = 2u * prm.bin.cap;
     r.tp = prm.bin.tile_pixels; r.magic = prm.bin.magic; r.mshift = prm.bin.mshift;
     r.nk = 1u << prm.bin.kbits; r.kmask = r.nk - 1u;
     r.sx = prm.sx; r.ox = prm.ox; r.sy = prm.sy; r.oy = prm.oy;
@@ -88,10 +88,10 @@ __device__ __forceinline__ void bin_append(const RenderParams &prm, const Shared
 {
     const uint32_t tile = __umulhi((uint32_t)pix, br.magic) >> br.mshift;
     const uint32_t rec = ((uint32_t)pix - tile * br.tp) * br.nk + ((uint32_t)k & br.kmask);
-    const uint32_t row = br.buf_addr + tile * br.cap4;
+    const uint32_t row = br.buf_addr + tile * br.cap2;
     uint32_t slot;
     asm volatile("atom.shared.add.u32 %0, [%1], 1;" : "=r"(slot) : "r"(br.cnt_addr + 4u * tile) : "memory");
-    if (slot < br.cap) asm volatile("st.shared.u32 [%0], %1;" :: "r"(row + 4u * slot), "r"(rec) : "memory");
+    if (slot < br.cap) asm volatile("st.shared.u16 [%0], %1;" :: "r"(row + 2u * slot), "h"((uint16_t)rec) : "memory");
     else bin_direct(prm, s, tile, rec);
 }
 
@@ -104,8 +104,8 @@ __device__ __forceinline__ uint32_t bin_try_append(const BinRegs &br, bool ok, u
     asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\tmov.u32 %0, 0xffffffff;\n\t"
                  "@p atom.shared.add.u32 %0, [%1], 1;\n\t}"
                  : "=r"(slot) : "r"(br.cnt_addr + 4u * tile), "r"((uint32_t)ok) : "memory");
-    asm volatile("{\n\t.reg .pred p;\n\tsetp.lt.u32 p, %2, %3;\n\t@p st.shared.u32 [%0], %1;\n\t}"
-                 :: "r"(br.buf_addr + tile * br.cap4 + 4u * slot), "r"(rec), "r"(slot), "r"(br.cap) : "memory");
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.lt.u32 p, %2, %3;\n\t@p st.shared.u16 [%0], %1;\n\t}"
+                 :: "r"(br.buf_addr + tile * br.cap2 + 2u * slot), "h"((uint16_t)rec), "r"(slot), "r"(br.cap) : "memory");
     return slot;
 }
 
@@ -140,7 +140,8 @@ __device__ __forceinline__ void bin_flush(const RenderParams &prm, const SharedT
     const BinParams &b = prm.bin;
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
     const uint32_t my_tile = lane * nwarps + warp;
-    uint32_t *s_cnt = sm, *s_buf = sm + bin_buf_offset(b.n_tiles);
+    uint32_t *s_cnt = sm;
+    uint16_t *s_buf = reinterpret_cast<uint16_t *>(sm + bin_buf_offset(b.n_tiles));
     if (warp >= b.n_tiles) return;                     // warp owns no tile (warp-uniform)
     const bool valid = my_tile < b.n_tiles;
     uint32_t mine = valid ? s_cnt[my_tile] : 0u;
@@ -151,8 +152,8 @@ __device__ __forceinline__ void bin_flush(const RenderParams &prm, const SharedT
         todo &= todo - 1;
         const uint32_t tile = (uint32_t)src * nwarps + warp;
         uint32_t cnt = min(__shfl_sync(0xFFFFFFFFu, mine, src), b.cap);   // slots >= cap went direct
-        uint32_t *row = s_buf + tile * b.cap;
-        uint32_t *head = row;                            // a row may hold several flush units
+        uint16_t *row = s_buf + tile * b.cap;
+        uint16_t *head = row;                            // a row may hold several flush units
         while (cnt >= kBinFlushRecords || (final && cnt > 0u)) {
             const uint32_t n = min(cnt, kBinFlushRecords);
             if ((int)lane == src && (bl.pos & (kBinBlockRecords - 1u)) == 0u && bl.pos != kBinInvalid) {
@@ -168,25 +169,25 @@ __device__ __forceinline__ void bin_flush(const RenderParams &prm, const SharedT
             }
             const uint32_t pos = __shfl_sync(0xFFFFFFFFu, bl.pos, src);
             uint4 v = make_uint4(0u, 0u, 0u, 0u);
-            if (4u * lane < n) v = reinterpret_cast<const uint4 *>(head)[lane];    // never past the row
+            if (8u * lane < n) v = reinterpret_cast<const uint4 *>(head)[lane];    // 8 records; never past the row
             if (pos != kBinInvalid) {
-                if (4u * lane < n) reinterpret_cast<uint4 *>(b.pool + pos)[lane] = v;
+                if (8u * lane < n) reinterpret_cast<uint4 *>(b.pool + pos)[lane] = v;
                 if ((int)lane == src) bl.pos += n;
             } else {
                 const uint32_t r[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
-                for (int i = 0; i < 4; ++i)
-                    if (4u * lane + i < n) bin_direct(prm, s, tile, r[i]);
+                for (int i = 0; i < 8; ++i)
+                    if (8u * lane + i < n) bin_direct(prm, s, tile, (r[i >> 1] >> (16 * (i & 1))) & 0xFFFFu);
                 if (lane == 0) atomicAdd(&b.ctrl[1], n);
             }
             cnt -= n;
             head += kBinFlushRecords;
         }
-        if (cnt > 0u && head != row) {   // fewer than 128 records remain, at least 128 words up the row
+        if (cnt > 0u && head != row) {   // fewer than 256 records remain, at least 256 records up the row
             uint4 m = make_uint4(0u, 0u, 0u, 0u);
-            if (4u * lane < cnt) m = reinterpret_cast<const uint4 *>(head)[lane];
+            if (8u * lane < cnt) m = reinterpret_cast<const uint4 *>(head)[lane];
             __syncwarp();
-            if (4u * lane < cnt) reinterpret_cast<uint4 *>(row)[lane] = m;
+            if (8u * lane < cnt) reinterpret_cast<uint4 *>(row)[lane] = m;
             __syncwarp();
         }
         if ((int)lane == src) mine = cnt;
@@ -201,7 +202,7 @@ __device__ __forceinline__ void bin_flush(const RenderParams &prm, const SharedT
         } else if (bl.nblk > 0u) {
             fill = kBinBlockRecords;                   // went invalid only after full blocks
         }
-        b.tails[(size_t)my_tile * b.grid + blockIdx.x] = (bl.nblk << 10) | fill;
+        b.tails[(size_t)my_tile * b.grid + blockIdx.x] = (bl.nblk << kBinTailShift) | fill;
     }
 }
 
@@ -225,9 +226,9 @@ bin_accumulate_kernel(const __grid_constant__ RenderParams prm)
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
     for (uint32_t c = warp; c < b.grid; c += nwarps) {
         const uint32_t tail = b.tails[(size_t)tile * b.grid + c];
-        const uint32_t n_blk = tail >> 10, last_fill = tail & 1023u;
+        const uint32_t n_blk = tail >> kBinTailShift, last_fill = tail & ((1u << kBinTailShift) - 1u);
         const uint32_t *list = b.list + ((size_t)tile * b.grid + c) * b.lcap;
-        // two blocks (2 x 2 KiB, eight 128-bit loads per lane) in flight per warp before their atomics
+        // two blocks (2 x 2 KiB = 2 x 1024 records, eight 128-bit loads per lane) in flight per warp
         for (uint32_t j = part; j < n_blk; j += 2u * b.split) {
             uint4 v[2][4];
             uint32_t fill[2];
@@ -240,18 +241,18 @@ bin_accumulate_kernel(const __grid_constant__ RenderParams prm)
                     const uint4 *src = reinterpret_cast<const uint4 *>(b.pool + (size_t)list[jj] * kBinBlockRecords);
 #pragma unroll
                     for (int q = 0; q < 4; ++q)
-                        v[h][q] = (q * 128u < fill[h]) ? __ldcs(src + q * 32 + lane) : make_uint4(0u, 0u, 0u, 0u);
+                        v[h][q] = (q * 256u < fill[h]) ? __ldcs(src + q * 32 + lane) : make_uint4(0u, 0u, 0u, 0u);
                 }
             }
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
 #pragma unroll
                 for (int q = 0; q < 4; ++q) {
-                    const uint32_t base = q * 128u + 4u * lane;
-                    if (base + 0u < fill[h]) atomicAdd(&acc[v[h][q].x], 1u);
-                    if (base + 1u < fill[h]) atomicAdd(&acc[v[h][q].y], 1u);
-                    if (base + 2u < fill[h]) atomicAdd(&acc[v[h][q].z], 1u);
-                    if (base + 3u < fill[h]) atomicAdd(&acc[v[h][q].w], 1u);
+                    const uint32_t base = q * 256u + 8u * lane;
+                    const uint32_t r[4] = {v[h][q].x, v[h][q].y, v[h][q].z, v[h][q].w};
+#pragma unroll
+                    for (int i = 0; i < 8; ++i)
+                        if (base + i < fill[h]) atomicAdd(&acc[(r[i >> 1] >> (16 * (i & 1))) & 0xFFFFu], 1u);
                 }
             }
         }

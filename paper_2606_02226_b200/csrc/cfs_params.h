@@ -54,28 +54,29 @@ enum SplatKind : int {
                              // (pass 1), accumulated per tile in shared memory (pass 2)
 };
 
-// tile-binned splat stage (DESIGN "binned variant").  A record is one uint32:
-// (pixel index inside the tile) << kbits | colour index, i.e. directly the index of the shared-
-// memory counter pass 2 increments.  The pool is a set of fixed-size blocks; a block belongs to
+// tile-binned splat stage (DESIGN "binned variant").  A record is one uint16:
+// (pixel index inside the tile) * colour slots + colour index, i.e. directly the index of the
+// shared-memory counter pass 2 increments (a tile has at most 3 * 2^14 = 49152 counters).  The pool is a set of fixed-size blocks; a block belongs to
 // one (CTA, tile) while it is filled and is listed under its tile when it is allocated.
-constexpr uint32_t kBinBlockRecords = 512;     // records per pool block (2 KiB)
-constexpr uint32_t kBinFlushRecords = 128;     // records per flush: one 512-byte coalesced store
+constexpr uint32_t kBinBlockRecords = 1024;    // records per pool block (2 KiB)
+constexpr uint32_t kBinFlushRecords = 256;     // records per flush: one 512-byte coalesced store
+constexpr uint32_t kBinTailShift = 11;         // tails word: blocks << 11 | records in the last block (<= 1024)
 constexpr uint32_t kBinInvalid = 0xFFFFFFFFu;  // tile has no block (pool or list exhausted): direct splats
 constexpr int kBinThreads = 1024;              // CTA size of pass 1 and CTAs per SM.  Measured on configs[1]: 1 x 1024
 constexpr int kBinCtasPerSm = 1;               // threads 4.69 ms, 2 x 512 threads (half-length staging rows) 5.53 ms
 constexpr int kBinAccThreads = 1024;           // CTA size of pass 2 (one CTA per SM: the tile fills shared memory)
 
 struct BinParams {
-    uint32_t *pool;        // nb * kBinBlockRecords records
+    uint16_t *pool;        // nb * kBinBlockRecords records
     uint32_t *list;        // [n_tiles][grid][lcap] block ids listed by pass-1 CTA c for a tile
-    uint32_t *tails;       // [n_tiles][grid] (blocks listed) << 10 | records in the last block
+    uint32_t *tails;       // [n_tiles][grid] (blocks listed) << kBinTailShift | records in the last block
     uint32_t *ctrl;        // [0] = blocks handed out, [1] = records splatted directly (statistics)
     uint32_t nb, lcap, n_tiles;
     uint32_t grid;         // CTAs of pass 1
     uint32_t tile_pixels;  // pixels per tile: 2^s or 3 * 2^s
     uint32_t magic, mshift; // pix / tile_pixels == umulhi(pix, magic) >> mshift for every pixel of the image
     uint32_t kbits;        // log2(colour slots per pixel): 0 = HIST, else ceil(log2 n_funcs)
-    uint32_t cap;          // staging records per tile in shared memory (multiple of 32, >= 160)
+    uint32_t cap;          // staging records per tile in shared memory (multiple of 64, >= 320)
     uint32_t check_mask;   // flush check after Philox block q (4 iterations) when ((q + 1) & check_mask) == 0
     uint32_t split;        // pass 2: CTAs per tile
 };
