@@ -283,9 +283,15 @@ cfs_status build_params(const cfs_system *s, const cfs_render_args *a, RenderPar
         st.type = x.type;
         auto res = [&](int i) { return (float)((double)x.p0[i] + t * (double)x.p1[i]); };
         switch (x.type) {
-        case CFS_T_AFFINE:
+        case CFS_T_AFFINE: {
             for (int i = 0; i < 12; ++i) st.p[i] = res(i);
+            // zero off-diagonals: the internal SCALE step, bit-identical because fma(0, y, b) == b
+            const bool diag = (s->dim == 2) ? (st.p[1] == 0.0f && st.p[2] == 0.0f)
+                                            : (st.p[1] == 0.0f && st.p[2] == 0.0f && st.p[3] == 0.0f && st.p[5] == 0.0f &&
+                                               st.p[6] == 0.0f && st.p[7] == 0.0f);
+            if (diag) st.type = cfs::T_SCALE;
             break;
+        }
         case CFS_T_ROTATE_Z: {   // resolved once per render to an AFFINE rotation (DESIGN R5)
             const double th = (double)x.p0[0] + t * (double)x.p1[0];
             const float c = (float)cos(th), sn = (float)sin(th);
@@ -403,7 +409,7 @@ bool bin_shape_raw(int gen, int out_mode, int color, uint32_t n_funcs, int32_t w
     // kBinCtasPerSm CTAs of pass 1 share the SM's shared memory (1 KiB per CTA is reserved by the system)
     const long budget = ((long)di.smem_sm / cfs::kBinCtasPerSm < (long)di.smem_optin ? (long)di.smem_sm / cfs::kBinCtasPerSm : (long)di.smem_optin)
                         - (long)sizeof(cfs::SharedTables) - 2048;
-    const long row_bytes = (budget - 4 * (long)n_tiles - 16) / (long)n_tiles;       // u32 cnt[] + u16 rows
+    const long row_bytes = (budget - 4 * (long)(n_tiles + cfs::kBinDummy) - 16) / (long)n_tiles;       // u32 cnt[] + u16 rows
     long cap = row_bytes / 2 / 64 * 64;
     if (cap > 4096) cap = 4096;
     if (cap < 320) { *why = "image has too many tiles for the binned variant's staging rows"; return false; }
@@ -432,7 +438,7 @@ bool bin_shape_raw(int gen, int out_mode, int color, uint32_t n_funcs, int32_t w
     b.check_mask = every / 4 - 1;                      // in Philox blocks of 4 iterations
     b.split = (uint32_t)((4 * (uint64_t)di.sms + n_tiles - 1) / n_tiles);
     if (b.split < 1) b.split = 1;
-    pl->smem_pass1 = (n_tiles + 3) / 4 * 4 * 4 + n_tiles * (size_t)cap * 2;
+    pl->smem_pass1 = (n_tiles + cfs::kBinDummy + 3) / 4 * 4 * 4 + n_tiles * (size_t)cap * 2;
     pl->smem_pass2 = ((size_t)b.tile_pixels << kbits) * 4;
     pl->grid1 = (uint32_t)di.sms * cfs::kBinCtasPerSm;
     return true;

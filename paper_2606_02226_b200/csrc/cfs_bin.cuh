@@ -34,8 +34,11 @@ __device__ __forceinline__ void bin_red_add_u32(uint32_t *addr, uint32_t v)
     asm volatile("red.global.add.u32 [%0], %1;" :: "l"(addr), "r"(v) : "memory");
 }
 
-// shared-memory layout of pass 1 (dynamic): u32 cnt[n_tiles] | pad to 16 B | u16 buf[n_tiles][cap]
-__device__ __forceinline__ uint32_t bin_buf_offset(uint32_t n_tiles) { return (n_tiles + 3u) & ~3u; }
+// shared-memory layout of pass 1 (dynamic): u32 cnt[n_tiles + kBinDummy] | pad to 16 B | u16 buf[n_tiles][cap].
+// cnt[n_tiles + lane] is lane's DUMMY counter: a dropped splat increments it instead of a tile's, so
+// the append is straight-line code (no branch around the atomic) and dropped splats of different
+// lanes never meet on one address.
+__device__ __forceinline__ uint32_t bin_buf_offset(uint32_t n_tiles) { return (n_tiles + kBinDummy + 3u) & ~3u; }
 
 // one record down the direct path (staging row full, or no pool block for the tile)
 __device__ __forceinline__ void bin_direct(const RenderParams &prm, const SharedTables &s, uint32_t tile, uint32_t rec)
@@ -54,7 +57,8 @@ __device__ __forceinline__ void bin_direct(const RenderParams &prm, const Shared
 struct BinRegs {
     uint32_t cnt_addr, buf_addr;   // shared addresses of cnt[] and buf[][]
     uint32_t cap, cap2;            // row capacity in records / bytes
-    uint32_t tp, magic, mshift;    // tile = umulhi(pix, magic) >> mshift == pix / tp for every pixel of the image
+    uint32_t dummy;                // index of this lane's dummy counter (n_tiles + lane)
+    uint32_t tp, ntp, magic, mshift; // tile = umulhi(pix, magic) >> mshift == pix / tp for every pixel of the image; ntp = -tp
     uint32_t nk, kmask;            // colour slots per pixel, and the mask that zeroes k for HIST
     float sx, ox, sy, oy;          // pixel map (DESIGN R8)
     int W, Wm1, Hm1;
@@ -66,7 +70,8 @@ __device__ __forceinline__ BinRegs bin_regs_init(const RenderParams &prm, uint32
     r.cnt_addr = (uint32_t)__cvta_generic_to_shared(sm);
     r.buf_addr = r.cnt_addr + 4u * bin_buf_offset(prm.bin.n_tiles);
     r.cap = prm.bin.cap; r.cap2 = 2u * prm.bin.cap;
-    r.tp = prm.bin.tile_pixels; r.magic = prm.bin.magic; r.mshift = prm.bin.mshift;
+    r.dummy = prm.bin.n_tiles;      // + lane, added by each thread after the broadcast
+    r.tp = prm.bin.tile_pixels; r.ntp = 0u - prm.bin.tile_pixels; r.magic = prm.bin.magic; r.mshift = prm.bin.mshift;
     r.nk = 1u << prm.bin.kbits; r.kmask = r.nk - 1u;
     r.sx = prm.sx; r.ox = prm.ox; r.sy = prm.sy; r.oy = prm.oy;
     r.W = prm.W; r.Wm1 = prm.W - 1; r.Hm1 = prm.H - 1;
@@ -74,13 +79,12 @@ __device__ __forceinline__ BinRegs bin_regs_init(const RenderParams &prm, uint32
 }
 
 // pixel rule of cfs_device.cuh pixel_of(), operands from registers
+// (the unsigned conversion saturates negative values to 0: the lower clamp costs nothing)
 __device__ __forceinline__ int bin_pixel_of(const BinRegs &br, float x, float y)
 {
-    int px = __float2int_rd(__fmaf_rn(x, br.sx, br.ox));
-    int py = __float2int_rd(__fmaf_rn(y, br.sy, br.oy));
-    px = min(max(px, 0), br.Wm1);
-    py = min(max(py, 0), br.Hm1);
-    return py * br.W + px;
+    const uint32_t px = min(__float2uint_rd(__fmaf_rn(x, br.sx, br.ox)), (uint32_t)br.Wm1);
+    const uint32_t py = min(__float2uint_rd(__fmaf_rn(y, br.sy, br.oy)), (uint32_t)br.Hm1);
+    return (int)(py * (uint32_t)br.W + px);
 }
 
 // row 7, binned: one shared-memory atomic + one shared store per splat
@@ -95,24 +99,23 @@ __device__ __forceinline__ void bin_append(const RenderParams &prm, const Shared
     else bin_direct(prm, s, tile, rec);
 }
 
-// The same as straight-line predicated code (no branch in the common case): the atomic and the store
-// carry predicates, `ok == false` leaves slot = 0xFFFFFFFF.  Returns the slot; the caller sends
-// records with cap <= slot < 0xFFFFFFFF down the direct path afterwards (rare).
-__device__ __forceinline__ uint32_t bin_try_append(const BinRegs &br, bool ok, uint32_t tile, uint32_t rec)
+// The same as straight-line code: the atomic is unconditional (a dropped splat takes the lane's
+// dummy counter), the store is predicated.  Returns true when the record found its row full and
+// has to go down the direct path (rare; the caller does that afterwards).
+__device__ __forceinline__ bool bin_try_append(const BinRegs &br, bool ok, uint32_t tile, uint32_t rec)
 {
+    const uint32_t t_eff = ok ? tile : br.dummy;
     uint32_t slot;
-    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\tmov.u32 %0, 0xffffffff;\n\t"
-                 "@p atom.shared.add.u32 %0, [%1], 1;\n\t}"
-                 : "=r"(slot) : "r"(br.cnt_addr + 4u * tile), "r"((uint32_t)ok) : "memory");
-    asm volatile("{\n\t.reg .pred p;\n\tsetp.lt.u32 p, %2, %3;\n\t@p st.shared.u16 [%0], %1;\n\t}"
-                 :: "r"(br.buf_addr + tile * br.cap2 + 2u * slot), "h"((uint16_t)rec), "r"(slot), "r"(br.cap) : "memory");
-    return slot;
+    asm volatile("atom.shared.add.u32 %0, [%1], 1;" : "=r"(slot) : "r"(br.cnt_addr + 4u * t_eff) : "memory");
+    const bool fits = ok && slot < br.cap;
+    if (fits) asm volatile("st.shared.u16 [%0], %1;" :: "r"(br.buf_addr + tile * br.cap2 + 2u * slot), "h"((uint16_t)rec) : "memory");
+    return ok && slot >= br.cap;
 }
 
 __device__ __forceinline__ void bin_record_of(const BinRegs &br, int pix, int k, uint32_t &tile, uint32_t &rec)
 {
     tile = __umulhi((uint32_t)pix, br.magic) >> br.mshift;
-    rec = ((uint32_t)pix - tile * br.tp) * br.nk + ((uint32_t)k & br.kmask);
+    rec = (tile * br.ntp + (uint32_t)pix) * br.nk + ((uint32_t)k & br.kmask);
 }
 
 // Per-lane bin state of pass 1, kept in REGISTERS: lane l of warp w owns tile l * warps + w (so

@@ -9,7 +9,7 @@ namespace cfs {
 namespace {
 
 #define CFS_STATIC_CHAINS(X) \
-    X(chain_sig(T_SWIRL, T_AFFINE))          /* BASELINE cfg 1 */ \
+    X(chain_sig(T_SWIRL, T_SCALE))           /* BASELINE cfg 1 */ \
     X(chain_sig(T_AFFINE, T_SINUSOIDAL))     /* BASELINE cfg 2 */ \
     X(chain_sig(T_STRETCH_COS, T_AFFINE))    /* PAPER Eq. 2    */
 

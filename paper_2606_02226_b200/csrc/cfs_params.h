@@ -61,6 +61,7 @@ enum SplatKind : int {
 constexpr uint32_t kBinBlockRecords = 1024;    // records per pool block (2 KiB)
 constexpr uint32_t kBinFlushRecords = 256;     // records per flush: one 512-byte coalesced store
 constexpr uint32_t kBinTailShift = 11;         // tails word: blocks << 11 | records in the last block (<= 1024)
+constexpr uint32_t kBinDummy = 32;             // dummy counters behind cnt[n_tiles]: one per lane, take the dropped splats
 constexpr uint32_t kBinInvalid = 0xFFFFFFFFu;  // tile has no block (pool or list exhausted): direct splats
 constexpr int kBinThreads = 1024;              // CTA size of pass 1 and CTAs per SM.  Measured on configs[1]: 1 x 1024
 constexpr int kBinCtasPerSm = 1;               // threads 4.69 ms, 2 x 512 threads (half-length staging rows) 5.53 ms

@@ -141,19 +141,18 @@ __device__ __forceinline__ uint32_t iterate_block(const RenderParams &prm, const
             const bool alive = apply_chain<DIM, SIG, TRIG>(prm, X[j], Y[j], Z[j]);
             ok[j] = alive && have && in_bounds(prm, X[j], Y[j]);
         }
-        uint32_t tile[4], rec[4], slot[4];
-        bool overflow = false;
+        uint32_t tile[4], rec[4];
+        bool over[4];
 #pragma unroll
         for (int j = 0; j < 4; ++j) {      // out-of-bounds coordinates are clamped by the pixel rule: always a valid tile
             bin_record_of(br, bin_pixel_of(br, X[j], Y[j]), K[j], tile[j], rec[j]);
-            slot[j] = bin_try_append(br, ok[j], tile[j], rec[j]);
-            dropped += ok[j] ? 0u : 1u;
-            overflow = overflow || (slot[j] >= br.cap && slot[j] != 0xFFFFFFFFu);
+            over[j] = bin_try_append(br, ok[j], tile[j], rec[j]);
         }
-        if (overflow) {                    // staging row full: those records take the direct path
+        dropped += 4u - ((uint32_t)ok[0] + (uint32_t)ok[1] + (uint32_t)ok[2] + (uint32_t)ok[3]);
+        if (over[0] || over[1] || over[2] || over[3]) {   // staging row full: those records take the direct path
 #pragma unroll
             for (int j = 0; j < 4; ++j)
-                if (slot[j] >= br.cap && slot[j] != 0xFFFFFFFFu) bin_direct(prm, s, tile[j], rec[j]);
+                if (over[j]) bin_direct(prm, s, tile[j], rec[j]);
         }
     } else {
 #pragma unroll(CHECKED ? 1 : 4)
@@ -200,11 +199,11 @@ render_kernel(const __grid_constant__ RenderParams prm)
         // whole kernel, whereas values derived from the parameter block are re-derived (constant
         // loads + shifts) at every use, ~10 extra instructions per splat
         if (threadIdx.x == 0) s_br = bin_regs_init(prm, s_hist);   // cnt[] of the staging rows; this lane's tile state
-        for (uint32_t i = threadIdx.x; i < prm.bin.n_tiles; i += blockDim.x) s_hist[i] = 0u;
+        for (uint32_t i = threadIdx.x; i < prm.bin.n_tiles + kBinDummy; i += blockDim.x) s_hist[i] = 0u;
         bin_lane_init(prm, bl);
     }
     __syncthreads();
-    if (SPLAT == SPLAT_BIN) br = s_br;
+    if (SPLAT == SPLAT_BIN) { br = s_br; br.dummy += threadIdx.x & 31u; }
 
     const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
     const int I = prm.iterations, B = prm.burn_in;
