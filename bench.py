@@ -201,6 +201,9 @@ N_INSTR = {0: 30, 1: 62, 2: 66, 3: 110, 4: 52}
 # the same for the binned variant with MUFU sin/cos (Philox 10, pick, LDS +
 # generator FMAs, chain, 4 bound compares, 9 pixel ops, 6 record ops, 4 append ops)
 N_INSTR_BIN = {0: 38, 1: 51, 2: 51}
+# hybrid (CFS_FLAG_BIN_HYBRID, what AUTO runs): every other splat skips the 6 record + 4 append operations and
+# pays a palette LDS + one red.global instead, i.e. 43 on those iterations: (51 + 43) / 2
+N_INSTR_HYB = {1: 47, 2: 47}
 RED_KEY = {0: "red_add_u32@1048576", 1: "red_add_v4f32@16777216", 2: "red_add_v4f32@33177600",
            3: "red_add_v4f32@132710400", 4: "atom_min_u64@66355200"}
 
@@ -392,17 +395,18 @@ def run_ours(args):
                   "t_atomic_ms": roof["t_atomic_ms"], "t_render_ms": t_render * 1e3}
     if binned:
         # dominant kernel: pass 1 (sample + chain + bin), bound by instruction issue
-        n_instr = N_INSTR_BIN[HEADLINE_CFG]
+        hybrid = args.variant == "auto"
+        n_instr = N_INSTR_HYB[HEADLINE_CFG] if hybrid else N_INSTR_BIN[HEADLINE_CFG]
         roofline = {
             "bound": "alu", "achieved": P * I * n_instr / pass1_s / 1e12, "peak": rates["ffma"] / 1e12,
             "unit": "T lane-instructions/s", "frac": (P * I * n_instr / pass1_s) / rates["ffma"],
             "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH, "kernel": "cfs::render_kernel<2,IFS,DIAG,BIN,swirl+affine,MUFU>",
             "kernel_ms": pass1_s * 1e3, "render_ms": t_render * 1e3, "pass2_ms": (t_render - pass1_s) * 1e3,
             "algorithmic_lane_instructions_per_point_iteration": n_instr,
-            "algorithmic_bytes_per_launch": int(S * 2),      # one 16-bit record per splat
+            "algorithmic_bytes_per_launch": int(S * 2) // (2 if hybrid else 1),      # one 16-bit record per binned splat
             "peak_source": "FFMA lane-issue rate of cfs_microbench in this run (148 SMs x 128 lanes x SM clock)",
             "hbm_peak_gbs": peaks.get("hbm_gbs"), "hbm_peak_source": peaks_src,
-            "pass2_hbm_gbs": S * 2 / max(t_render - pass1_s, 1e-9) / 1e9,
+            "pass2_hbm_gbs": (S * 2 // (2 if hybrid else 1)) / max(t_render - pass1_s, 1e-9) / 1e9,
         }
     else:
         peak_red = rates[RED_KEY[HEADLINE_CFG]]
@@ -427,7 +431,9 @@ def run_ours(args):
                 "note": "cfs_render_host: clear + render + D2H of the float32 accumulators and counters into pinned "
                         "host memory; this workload has no host input besides the kernel parameter block"},
         "roofline": roofline, "north_star_roofline": north_star,
-        "splat_variant": "binned (tile bins through scratch, shared-memory tile accumulation)" if binned else "direct (one L2 reduction per splat)",
+        "splat_variant": ("hybrid: every other splat straight to L2 (red.global), the rest through tile bins in scratch with shared-memory "
+                          "tile accumulation (CFS_FLAG_BIN_HYBRID, set by AUTO)" if args.variant == "auto" else
+                          "binned (tile bins through scratch, shared-memory tile accumulation)") if binned else "direct (one L2 reduction per splat)",
         "microbench": {k: (v / 1e9 if not k.endswith("GBps") else v) for k, v in rates.items()},
         "microbench_unit": "G lane-ops/s (stream: GB/s)",
     }

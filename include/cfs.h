@@ -103,8 +103,15 @@ typedef enum {
  *   INTERPRET_CHAIN: never use a kernel compiled for the chain's signature; run the chain
  *   interpreter (same device functions, same results; for tests and comparisons).
  *   BIN_PASS1_ONLY: measurement instrument of the BINNED variant: run pass 1 (sample + bin) and
- *   skip pass 2, so the two passes can be timed apart with events; the image is NOT updated. */
-typedef enum { CFS_FLAG_FAST_TRIG = 1, CFS_FLAG_INTERPRET_CHAIN = 2, CFS_FLAG_BIN_PASS1_ONLY = 4 } cfs_render_flags;
+ *   skip pass 2, so the two passes can be timed apart with events; the image is NOT updated
+ *   (with BIN_HYBRID it receives the direct half only).
+ *   BIN_HYBRID: the BINNED variant sends every other splat (iterations 0 and 2 of each Philox block
+ *   of four) straight to L2 with red.global and only the rest through the tile bins, so that the
+ *   L2 reduction units, the issue slots of pass 1 and the shared-memory atomics of pass 2 are all
+ *   busy.  Same image (HIST sums are exact; RGBA sums are order-free, DESIGN R8).  CFS_VARIANT_AUTO
+ *   sets it whenever it chooses the tile bins; CFS_VARIANT_BINNED takes it from the caller. */
+typedef enum { CFS_FLAG_FAST_TRIG = 1, CFS_FLAG_INTERPRET_CHAIN = 2, CFS_FLAG_BIN_PASS1_ONLY = 4,
+               CFS_FLAG_BIN_HYBRID = 0x100 } cfs_render_flags;
 
 /* one 16-byte record of a stored cloud (BASELINE cfg 3); rgba8 = r | g<<8 | b<<16 | a<<24 */
 typedef struct { float x, y, z; uint32_t rgba8; } cfs_cloud_rec;

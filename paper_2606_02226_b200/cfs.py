@@ -22,7 +22,7 @@ T_TYPE = {"affine": 0, "swirl": 1, "sinusoidal": 2, "rotate_z": 3, "twist_z": 4,
           "pinhole": 6, "stretch_cos": 7}
 COLOR = {"none": 0, "map_index": 1, "point": 2}
 OUT = {"hist_u32": 0, "rgba_f32": 1, "depth_u64": 2}
-FLAGS = {"fast_trig": 1, "interpret_chain": 2, "bin_pass1_only": 4}
+FLAGS = {"fast_trig": 1, "interpret_chain": 2, "bin_pass1_only": 4, "bin_hybrid": 0x100}
 VARIANT = {"auto": 0, "direct": 1, "shared_hist": 2, "warp_agg": 3, "binned": 4, "cluster_hist": 5}
 MB = {"red_add_u32": 0, "red_add_v4f32": 1, "atom_min_u64": 2, "ld_u64": 3, "atoms_add_u32": 4,
       "ffma": 5, "imad_wide": 6, "lop3": 7, "mufu": 8, "stream_ld128": 9}

@@ -236,7 +236,7 @@ using cfs::RenderParams;
 cfs_status build_params(const cfs_system *s, const cfs_render_args *a, RenderParams *out, bool need_image)
 {
     if (!s || !a) return fail(CFS_ERR_INVALID_ARG, "system or args is NULL");
-    if (a->flags & ~(CFS_FLAG_FAST_TRIG | CFS_FLAG_INTERPRET_CHAIN | CFS_FLAG_BIN_PASS1_ONLY)) return fail(CFS_ERR_INVALID_ARG, "unknown flags 0x%x", a->flags);
+    if (a->flags & ~(CFS_FLAG_FAST_TRIG | CFS_FLAG_INTERPRET_CHAIN | CFS_FLAG_BIN_PASS1_ONLY | CFS_FLAG_BIN_HYBRID)) return fail(CFS_ERR_INVALID_ARG, "unknown flags 0x%x", a->flags);
     if (a->iterations < 1) return fail(CFS_ERR_INVALID_ARG, "iterations must be >= 1");
     if (a->burn_in < 0 || a->burn_in >= a->iterations) return fail(CFS_ERR_INVALID_ARG, "burn_in must be in [0, iterations)");
     if (s->gen == CFS_GEN_CLOUD && (a->iterations != 1 || a->burn_in != 0)) return fail(CFS_ERR_INVALID_ARG, "CLOUD generator needs iterations = 1, burn_in = 0");
@@ -598,6 +598,7 @@ cfs_status render_binned(const cfs_system *s, const cfs_render_args *a, RenderPa
     if ((e = cudaFuncSetAttribute((const void *)fn2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem_pass2)) != cudaSuccess)
         return cuda_fail(e, "cudaFuncSetAttribute(pass 2)");
     p.bin = pl.bp;
+    p.bin.hybrid = ((a->flags & CFS_FLAG_BIN_HYBRID) || a->variant == CFS_VARIANT_AUTO) ? 1u : 0u;
     const uint64_t total = a->n_points, first = a->point_offset;
     for (uint64_t done = 0; done < total; done += pl.chunk_points) {
         const uint64_t n = (total - done < pl.chunk_points) ? total - done : pl.chunk_points;

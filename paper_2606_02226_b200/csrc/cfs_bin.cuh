@@ -52,6 +52,17 @@ __device__ __forceinline__ void bin_direct(const RenderParams &prm, const Shared
     }
 }
 
+// one splat down the direct path, from its image pixel and map index
+__device__ __forceinline__ void bin_direct_pix(const RenderParams &prm, const SharedTables &s, uint32_t pix, uint32_t k)
+{
+    if (prm.color_rule == 0) {
+        bin_red_add_u32(reinterpret_cast<uint32_t *>(prm.image) + pix, 1u);
+    } else {
+        const float4 c = s.palette[k];
+        bin_red_add_v4_f32(reinterpret_cast<float *>(prm.image) + 4 * (size_t)pix, c.x, c.y, c.z, 1.0f);
+    }
+}
+
 // values of the append fast path, derived once per thread (32-bit shared-window addresses, so
 // an access is one ATOMS / STS without generic-address arithmetic)
 struct BinRegs {

@@ -80,6 +80,7 @@ struct BinParams {
     uint32_t cap;          // staging records per tile in shared memory (multiple of 64, >= 320)
     uint32_t check_mask;   // flush check after Philox block q (4 iterations) when ((q + 1) & check_mask) == 0
     uint32_t split;        // pass 2: CTAs per tile
+    uint32_t hybrid;       // != 0: iterations 0 and 2 of every steady-state Philox block splat straight to L2
 };
 
 struct ChainStep {

@@ -108,6 +108,38 @@ __device__ __forceinline__ uint32_t chain_and_splat(const RenderParams &prm, con
     return 0u;
 }
 
+// rows 6-7 of the four iterations of one steady-state Philox block, binned.  HYBRID: iterations 0
+// and 2 of the block splat straight to L2 (red.global), 1 and 3 go through the tile bins -- pass 1 is
+// bound by instruction issue and pass 2 by shared-memory atomics while the L2 reduction units would
+// idle, so half of the splats are given to them (a direct splat costs ~5 instructions against ~16
+// for record + append, and pass 2 halves).  Any split is a correct result: HIST sums are exact,
+// RGBA sums are order-free (DESIGN R8).  Returns the number of dropped splats.
+template <bool HYBRID>
+__device__ __forceinline__ uint32_t bin_block_splat(const RenderParams &prm, const SharedTables &s, const BinRegs &br,
+                                                    const float (&X)[4], const float (&Y)[4], const int (&K)[4],
+                                                    const bool (&ok)[4])
+{
+    uint32_t tile[4], rec[4];
+    bool over[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {      // out-of-bounds coordinates are clamped by the pixel rule: always a valid tile
+        const int pix = bin_pixel_of(br, X[j], Y[j]);
+        over[j] = false;
+        if (HYBRID && (j & 1) == 0) {
+            if (ok[j]) bin_direct_pix(prm, s, (uint32_t)pix, (uint32_t)K[j]);
+        } else {
+            bin_record_of(br, pix, K[j], tile[j], rec[j]);
+            over[j] = bin_try_append(br, ok[j], tile[j], rec[j]);
+        }
+    }
+    if (over[0] || over[1] || over[2] || over[3]) {   // staging row full: those records take the direct path
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+            if (over[j]) bin_direct(prm, s, tile[j], rec[j]);
+    }
+    return 4u - ((uint32_t)ok[0] + (uint32_t)ok[1] + (uint32_t)ok[2] + (uint32_t)ok[3]);
+}
+
 // four iterations served by one Philox block (DESIGN R1: word it & 3 of block it >> 2).
 // CHECKED = false: the caller guarantees burn_in <= it0 and it0 + 4 <= iterations, so the body
 // has no per-iteration tests (the steady state of a render); CHECKED = true handles burn-in
@@ -141,19 +173,8 @@ __device__ __forceinline__ uint32_t iterate_block(const RenderParams &prm, const
             const bool alive = apply_chain<DIM, SIG, TRIG>(prm, X[j], Y[j], Z[j]);
             ok[j] = alive && have && in_bounds(prm, X[j], Y[j]);
         }
-        uint32_t tile[4], rec[4];
-        bool over[4];
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {      // out-of-bounds coordinates are clamped by the pixel rule: always a valid tile
-            bin_record_of(br, bin_pixel_of(br, X[j], Y[j]), K[j], tile[j], rec[j]);
-            over[j] = bin_try_append(br, ok[j], tile[j], rec[j]);
-        }
-        dropped += 4u - ((uint32_t)ok[0] + (uint32_t)ok[1] + (uint32_t)ok[2] + (uint32_t)ok[3]);
-        if (over[0] || over[1] || over[2] || over[3]) {   // staging row full: those records take the direct path
-#pragma unroll
-            for (int j = 0; j < 4; ++j)
-                if (over[j]) bin_direct(prm, s, tile[j], rec[j]);
-        }
+        if (prm.bin.hybrid) dropped += bin_block_splat<true>(prm, s, br, X, Y, K, ok);    // warp-uniform
+        else                dropped += bin_block_splat<false>(prm, s, br, X, Y, K, ok);
     } else {
 #pragma unroll(CHECKED ? 1 : 4)
         for (int j = 0; j < 4; ++j) {
@@ -207,6 +228,7 @@ render_kernel(const __grid_constant__ RenderParams prm)
 
     const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
     const int I = prm.iterations, B = prm.burn_in;
+    const int it_fast0 = min((B + 3) & ~3, I & ~3), it_fast1 = I & ~3;   // steady-state Philox blocks: [it_fast0, it_fast1)
     uint32_t n_in = 0, n_drop = 0;
 
     for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; ; i += stride) {
@@ -234,13 +256,16 @@ render_kernel(const __grid_constant__ RenderParams prm)
                 if (DIM == 3) gz = u24_to_pm1(w.z);
             }
             // blocks touching burn-in or the ragged end take the checked path, the rest the lean one
-            const int it_fast0 = min((B + 3) & ~3, I & ~3), it_fast1 = I & ~3;
-            for (int it0 = 0; it0 < I; it0 += 4) {
-                if (it0 >= it_fast0 && it0 < it_fast1)
-                    dropped += iterate_block<DIM, GEN, AFF, SPLAT, SIG, TRIG, false>(prm, s, s_hist, plo, phi, it0, gx, gy, gz, have, bl, br);
-                else
-                    dropped += iterate_block<DIM, GEN, AFF, SPLAT, SIG, TRIG, true>(prm, s, s_hist, plo, phi, it0, gx, gy, gz, have, bl, br);
-            }
+            int it0 = 0;
+#pragma unroll 1
+            for (; it0 < it_fast0; it0 += 4)
+                dropped += iterate_block<DIM, GEN, AFF, SPLAT, SIG, TRIG, true>(prm, s, s_hist, plo, phi, it0, gx, gy, gz, have, bl, br);
+#pragma unroll 1
+            for (; it0 < it_fast1; it0 += 4)
+                dropped += iterate_block<DIM, GEN, AFF, SPLAT, SIG, TRIG, false>(prm, s, s_hist, plo, phi, it0, gx, gy, gz, have, bl, br);
+#pragma unroll 1
+            for (; it0 < I; it0 += 4)
+                dropped += iterate_block<DIM, GEN, AFF, SPLAT, SIG, TRIG, true>(prm, s, s_hist, plo, phi, it0, gx, gy, gz, have, bl, br);
         }
         if (have) { n_drop += dropped; n_in += (uint32_t)(I - B) - dropped; }
     }

@@ -205,12 +205,14 @@ def test_fast_trig_within_tolerance(cfs, oracle, cfg, interp):
 
 
 # ------------------------------------------------------------------ tile-binned variant
+@pytest.mark.parametrize("hybrid", [False, True])
 @pytest.mark.parametrize("n", [1, 1000, 1024, 5000 + 13])
-def test_binned_histogram_bit_exact(cfs, oracle, n):
+def test_binned_histogram_bit_exact(cfs, oracle, n, hybrid):
     """CFS_VARIANT_BINNED on the cfg 0 image: records through the block pool, tiles accumulated in
-    shared memory; identical per pixel to the oracle, counters included; ragged CTAs."""
+    shared memory; identical per pixel to the oracle, counters included; ragged CTAs.  With
+    CFS_FLAG_BIN_HYBRID every other splat goes straight to L2 instead: same histogram."""
     w = W.config(0).scaled(n_points=n, iterations=300)
-    g, gc = gpu_render(cfs, w, variant="binned")
+    g, gc = gpu_render(cfs, w, variant="binned", flags=["bin_hybrid"] if hybrid else 0)
     o, oc, _ = oracle.render_parallel(w.system, w.render)
     assert np.array_equal(g, o) and np.array_equal(gc, oc)
 
@@ -233,14 +235,15 @@ def test_binned_chunks_and_small_scratch(cfs, oracle):
     assert np.array_equal(g, o)
 
 
+@pytest.mark.parametrize("hybrid", [False, True])
 @pytest.mark.parametrize("cfg", [1, 2])
-def test_binned_rgba_equals_direct(cfs, oracle, cfg):
+def test_binned_rgba_equals_direct(cfs, oracle, cfg, hybrid):
     """Binned RGBA (counters per pixel and map, sum_k n_k * palette[k]) against the direct variant
     on the same device functions: integer-valued colour sums below 2^24 are exact, so the images
     are identical; and against the oracle within the density bar."""
     w = W.config(cfg).scaled(n_points=(1 << 14) + 5)
     t = w.frames[len(w.frames) // 2]
-    gb, cb = gpu_render(cfs, w, t=t, variant="binned")
+    gb, cb = gpu_render(cfs, w, t=t, variant="binned", flags=["bin_hybrid"] if hybrid else 0)
     gd, cd = gpu_render(cfs, w, t=t, variant="direct")
     assert np.array_equal(gb, gd) and np.array_equal(cb, cd)
     o, oc, _ = oracle.render_parallel(w.system, w.render, t=t)
@@ -255,10 +258,11 @@ def test_binned_hot_tile_overflow_and_limits(cfs, oracle):
     sys1 = W.System(2, "ifs", funcs, [], "map_index", W.palette_for(4))
     # 400 x 160 splats x 255 < 2^24: the float sum is exact whatever the order of the additions
     w = W.Workload("hot", sys1, W.Render(400, 5, 200, 40, 512, 512, (-1, 1, -1, 1), "rgba_f32"))
-    g, gc = gpu_render(cfs, w, variant="binned")
     o, oc = oracle.render(sys1, w.render)
-    assert np.array_equal(g.astype(np.float64), o) and np.array_equal(gc, oc)
-    assert np.count_nonzero(g[:, 3]) == 1 and g[:, 3].sum() == 400 * 160
+    for flags in (0, ["bin_hybrid"]):
+        g, gc = gpu_render(cfs, w, variant="binned", flags=flags)
+        assert np.array_equal(g.astype(np.float64), o) and np.array_equal(gc, oc)
+        assert np.count_nonzero(g[:, 3]) == 1 and g[:, 3].sum() == 400 * 160
 
     f16 = [W.Func("affine", float(np.float32(1 + (k % 3))), [0.5, 0, 0, 0.5, 0.5 * math.cos(k), 0.5 * math.sin(k)])
            for k in range(17)]
