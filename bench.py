@@ -226,6 +226,8 @@ SCRATCH_CAP_BYTES = 8 << 30
 def make_scratch(cfs, torch, sysh, render):
     """Scratch of the tile-binned variant (None when the variant cannot serve the workload)."""
     need = cfs.cfs_binned_scratch_bytes(sysh, cfs.make_args(render))
+    if need == 0 and render.out_mode == "depth_u64":      # the Hi-Z map of the depth variant
+        need = cfs.cfs_hiz_scratch_bytes(render.width, render.height)
     if need == 0:
         return None
     return torch.empty(min(need, SCRATCH_CAP_BYTES), dtype=torch.uint8, device="cuda")

@@ -89,6 +89,10 @@ typedef enum {
     CFS_VARIANT_CLUSTER_HIST = 5,/* HIST, IFS generator, W*H*4 <= 8 x (shared memory of a CTA): the histogram is   */
                                  /* distributed over the shared memory of 8-CTA thread-block clusters, splats are */
                                  /* red.shared::cluster through DSMEM, slices merged with red.global              */
+    CFS_VARIANT_DEPTH_HIZ = 6,   /* DEPTH, IFS generator, needs d_scratch of cfs_hiz_scratch_bytes(): a coarse        */
+                                 /* conservative depth map (max of depth bits >> 16 per pixel block), rebuilt from   */
+                                 /* the image after the first slices of the points and held in shared memory, lets   */
+                                 /* occluded splats stop on the SM instead of paying a random L2 load; same image    */
     CFS_VARIANT_BINNED = 4       /* HIST, or RGBA + MAP_INDEX with <= 16 functions, IFS generator:    */
                                  /* splats are partitioned by image tile through d_scratch (one       */
                                  /* 2-byte record each), then every tile is accumulated in shared     */
@@ -162,6 +166,12 @@ cfs_status cfs_render(const cfs_system *sys, const cfs_render_args *args, void *
  * CFS_FLAG_FAST_TRIG -- where it was measured faster than the L2 atomic rate allows -- and the
  * direct path otherwise. */
 uint64_t cfs_binned_scratch_bytes(const cfs_system *sys, const cfs_render_args *args);
+
+/* bytes of d_scratch CFS_VARIANT_DEPTH_HIZ needs for a width x height depth image (host arithmetic,
+ * no device needed); 0 when the image is too large for a shared-memory Hi-Z map (> 96 KiB at
+ * 32 x 32-pixel blocks).  With that much scratch given, CFS_VARIANT_AUTO takes the Hi-Z path for
+ * DEPTH renders of an IFS generator with at least 2^27 splats. */
+uint64_t cfs_hiz_scratch_bytes(int32_t width, int32_t height);
 
 /* the tile plan of the BINNED variant for an image and a device shape, host arithmetic only (no device
  * needed; test instrument): out = { tiles, pixels per tile, magic, shift (tile of pixel p =

@@ -23,11 +23,11 @@ T_TYPE = {"affine": 0, "swirl": 1, "sinusoidal": 2, "rotate_z": 3, "twist_z": 4,
 COLOR = {"none": 0, "map_index": 1, "point": 2}
 OUT = {"hist_u32": 0, "rgba_f32": 1, "depth_u64": 2}
 FLAGS = {"fast_trig": 1, "interpret_chain": 2, "bin_pass1_only": 4, "bin_hybrid": 0x100}
-VARIANT = {"auto": 0, "direct": 1, "shared_hist": 2, "warp_agg": 3, "binned": 4, "cluster_hist": 5}
+VARIANT = {"auto": 0, "direct": 1, "shared_hist": 2, "warp_agg": 3, "binned": 4, "cluster_hist": 5, "depth_hiz": 6}
 MB = {"red_add_u32": 0, "red_add_v4f32": 1, "atom_min_u64": 2, "ld_u64": 3, "atoms_add_u32": 4,
       "ffma": 5, "imad_wide": 6, "lop3": 7, "mufu": 8, "stream_ld128": 9}
 EXPORTS = ["cfs_create", "cfs_destroy", "cfs_render", "cfs_render_host", "cfs_tonemap", "cfs_trace",
-           "cfs_microbench", "cfs_shared_hist_max_bytes", "cfs_binned_scratch_bytes", "cfs_binned_plan", "cfs_launch_count", "cfs_last_error",
+           "cfs_microbench", "cfs_shared_hist_max_bytes", "cfs_binned_scratch_bytes", "cfs_hiz_scratch_bytes", "cfs_binned_plan", "cfs_launch_count", "cfs_last_error",
            "cfs_version"]
 
 
@@ -90,6 +90,8 @@ def lib():
         L.cfs_shared_hist_max_bytes.restype = C.c_uint64
         L.cfs_binned_scratch_bytes.argtypes = [C.c_void_p, C.POINTER(cfs_render_args)]
         L.cfs_binned_scratch_bytes.restype = C.c_uint64
+        L.cfs_hiz_scratch_bytes.argtypes = [C.c_int32, C.c_int32]
+        L.cfs_hiz_scratch_bytes.restype = C.c_uint64
         L.cfs_binned_plan.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32,
                                       C.POINTER(C.c_uint32)]
         L.cfs_binned_plan.restype = C.c_int
@@ -216,6 +218,10 @@ def make_args(render, d_image=None, d_cloud=None, d_counters=None, n_points=None
 
 def cfs_binned_scratch_bytes(sys: System, args: cfs_render_args) -> int:
     return int(lib().cfs_binned_scratch_bytes(sys.handle, C.byref(args)))
+
+
+def cfs_hiz_scratch_bytes(width: int, height: int) -> int:
+    return int(lib().cfs_hiz_scratch_bytes(int(width), int(height)))
 
 
 def cfs_binned_plan(width: int, height: int, out_mode, n_funcs: int, sms: int = 148, smem_optin: int = 232448) -> dict:

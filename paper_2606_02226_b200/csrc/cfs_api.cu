@@ -11,6 +11,7 @@
 
 #include "../../include/cfs.h"
 #include "cfs_bin.cuh"
+#include "cfs_hiz.cuh"
 #include "cfs_device.cuh"
 #include "cfs_microbench.cuh"
 #include "cfs_registry.h"
@@ -271,6 +272,13 @@ cfs_status build_params(const cfs_system *s, const cfs_render_args *a, RenderPar
     p.dim = s->dim; p.n_funcs = (int)s->funcs.size(); p.n_chain = (int)s->chain.size();
     p.color_rule = s->color; p.reuse = s->reuse; p.fast_trig = (a->flags & CFS_FLAG_FAST_TRIG) ? 1 : 0;
     p.pick_shift = s->pick_shift; p.n_thr = s->n_thr; p.pick_steps = s->pick_steps;
+    {   // coefficient rows are replicated in shared memory (up to 8 copies) when more than 8 of them are in
+        // use: with fewer, every row already has a bank group of its own
+        const uint32_t rows_per_map = (s->aff == cfs::AFF_DIAG) ? (s->dim == 2 ? 1u : 2u) : (s->dim == 2 ? 2u : 3u);
+        p.coef_rows = (uint32_t)s->funcs.size() * rows_per_map;
+        p.coef_cshift = 0;
+        if (p.coef_rows > 8) while (p.coef_cshift < 3 && (p.coef_rows << (p.coef_cshift + 1)) <= (uint32_t)cfs::kCoefSlots) ++p.coef_cshift;
+    }
     memcpy(p.T, s->T, sizeof(p.T)); memcpy(p.lut, s->lut, sizeof(p.lut));
     memcpy(p.coef, s->coef, sizeof(p.coef)); memcpy(p.pal8, s->pal8, sizeof(p.pal8));
     if (!s->palette.empty()) memcpy(p.palette, s->palette.data(), s->palette.size() * sizeof(float));
@@ -382,7 +390,7 @@ size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 // tiles and staging rows; false when the variant cannot serve this system / image
 bool bin_shape_raw(int gen, int out_mode, int color, uint32_t n_funcs, int32_t width, int32_t height, const DeviceInfo &di,
-                   BinPlan *pl, const char **why)
+                   bool hybrid, BinPlan *pl, const char **why)
 {
     if (gen != CFS_GEN_IFS) { *why = "binned variant needs an IFS generator"; return false; }
     if (out_mode == CFS_OUT_DEPTH_RGBA8_U64) { *why = "binned variant serves HIST and RGBA output"; return false; }
@@ -429,12 +437,14 @@ bool bin_shape_raw(int gen, int out_mode, int color, uint32_t n_funcs, int32_t w
         }
         if (!found) { *why = "no exact tile division for this image size"; return false; }
     }
-    // flush check every E iterations, E the largest power of two whose expected arrivals per row
-    // (with 25 % + 16 records of slack; measured on configs[1]: 6.36 / 5.36 / 4.72 / 4.60 ms at 4 / 8 / 16 / 32) fit above a nearly full flush unit
-    const double per_it = (double)cfs::kBinThreads / (double)n_tiles;
+    // flush check every E iterations, E the largest power of two whose expected arrivals per row fit above a
+    // nearly full flush unit -- with a factor 2 for tiles that draw more than the even share (the swirled
+    // square of configs[1] covers 41 % of its image: before this factor every fifth warp-block found a full
+    // row, profiles/r01j) and 16 records of slack.  The hybrid stage bins every other splat only.
+    const double per_it = (double)cfs::kBinThreads / (double)n_tiles * (hybrid ? 0.5 : 1.0);
     const double room = (double)(cap - (long)cfs::kBinFlushRecords + 1);
     uint32_t every = 64;
-    while (every > 4 && 1.25 * every * per_it + 16.0 > room) every >>= 1;
+    while (every > 4 && 2.0 * every * per_it + 16.0 > room) every >>= 1;
     b.check_mask = every / 4 - 1;                      // in Philox blocks of 4 iterations
     b.split = (uint32_t)((4 * (uint64_t)di.sms + n_tiles - 1) / n_tiles);
     if (b.split < 1) b.split = 1;
@@ -454,7 +464,8 @@ size_t bin_fixed_bytes(const BinPlan &pl)
 
 bool bin_shape(const cfs_system *s, const cfs_render_args *a, const DeviceInfo &di, BinPlan *pl, const char **why)
 {
-    return bin_shape_raw(s->gen, a->out_mode, s->color, (uint32_t)s->funcs.size(), a->width, a->height, di, pl, why);
+    const bool hybrid = (a->flags & CFS_FLAG_BIN_HYBRID) || a->variant == CFS_VARIANT_AUTO;
+    return bin_shape_raw(s->gen, a->out_mode, s->color, (uint32_t)s->funcs.size(), a->width, a->height, di, hybrid, pl, why);
 }
 
 // scratch needed to render `points` points in one chunk
@@ -512,7 +523,7 @@ extern "C" cfs_status cfs_binned_plan(int32_t width, int32_t height, int32_t out
     BinPlan pl;
     const char *why = "";
     if (!bin_shape_raw(CFS_GEN_IFS, out_mode, out_mode == CFS_OUT_RGBA_F32 ? CFS_COLOR_MAP_INDEX : CFS_COLOR_NONE, (uint32_t)n_funcs,
-                       width, height, di, &pl, &why)) return fail(CFS_ERR_UNSUPPORTED, "%s", why);
+                       width, height, di, false, &pl, &why)) return fail(CFS_ERR_UNSUPPORTED, "%s", why);
     out[0] = pl.bp.n_tiles; out[1] = pl.bp.tile_pixels; out[2] = pl.bp.magic; out[3] = pl.bp.mshift;
     out[4] = pl.bp.kbits; out[5] = pl.bp.cap; out[6] = 4u * (pl.bp.check_mask + 1u); out[7] = pl.bp.split;
     return CFS_OK;
@@ -619,12 +630,94 @@ cfs_status render_binned(const cfs_system *s, const cfs_render_args *a, RenderPa
 
 }  // namespace
 
+// ---- Hi-Z depth variant: plan + phased render ---------------------------------------------------
+namespace {
+
+struct HizPlan { uint32_t shift, nbx, nby, n, n_pad; uint64_t bytes; };
+
+// smallest block (8, 16 or 32 pixels square) whose map fits kHizMaxBytes of shared memory
+bool hiz_plan(int32_t width, int32_t height, HizPlan *pl)
+{
+    if (width < 1 || height < 1) return false;
+    for (uint32_t sh = 3; sh <= 5; ++sh) {
+        const uint64_t nbx = ((uint64_t)width + (1u << sh) - 1) >> sh, nby = ((uint64_t)height + (1u << sh) - 1) >> sh;
+        const uint64_t n = nbx * nby, n_pad = (n + 7) / 8 * 8;
+        if (n_pad * 2 <= cfs::kHizMaxBytes) {
+            pl->shift = sh; pl->nbx = (uint32_t)nbx; pl->nby = (uint32_t)nby; pl->n = (uint32_t)n; pl->n_pad = (uint32_t)n_pad;
+            pl->bytes = n_pad * 2 + 256;         // + alignment slack
+            return true;
+        }
+    }
+    return false;
+}
+
+}  // namespace
+
+extern "C" uint64_t cfs_hiz_scratch_bytes(int32_t width, int32_t height)
+{
+    HizPlan pl;
+    return hiz_plan(width, height, &pl) ? pl.bytes : 0;
+}
+
+namespace {
+
+// Phases over disjoint point ranges (min is order-free, so any split gives the same image):
+//   [0, n0)      plain depth splats -- n0 sized so that the image holds ~64 splats per pixel,
+//   build Hi-Z,  [n0, 8 n0) behind it,  rebuild (tighter),  the rest behind that.
+cfs_status render_depth_hiz(const cfs_system *s, const cfs_render_args *a, RenderParams &p, const DeviceInfo &di, cudaStream_t st)
+{
+    (void)di;
+    if (a->out_mode != CFS_OUT_DEPTH_RGBA8_U64 || s->gen != CFS_GEN_IFS)
+        return fail(CFS_ERR_UNSUPPORTED, "Hi-Z variant serves DEPTH output of an IFS generator");
+    HizPlan pl;
+    if (!hiz_plan(a->width, a->height, &pl)) return fail(CFS_ERR_UNSUPPORTED, "image too large for a shared-memory Hi-Z map");
+    if (!a->d_scratch || a->scratch_bytes < pl.bytes)
+        return fail(CFS_ERR_UNSUPPORTED, "Hi-Z variant needs d_scratch of cfs_hiz_scratch_bytes() = %llu bytes", (unsigned long long)pl.bytes);
+    render_fn fn0 = pick_kernel(s, p, cfs::SPLAT_DEPTH, a->flags);
+    render_fn fn1 = pick_kernel(s, p, cfs::SPLAT_DEPTH_HIZ, a->flags);
+    if (!fn0 || !fn1) return fail(CFS_ERR_UNSUPPORTED, "no depth kernel for dim %d", s->dim);
+    uint16_t *hz = (uint16_t *)(((uintptr_t)a->d_scratch + 255) & ~(uintptr_t)255);
+    const size_t dyn = (size_t)pl.n_pad * 2;
+    cudaError_t e = cudaFuncSetAttribute((const void *)fn1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute");
+    p.hiz.hz = hz; p.hiz.shift = pl.shift; p.hiz.nbx = pl.nbx; p.hiz.nby = pl.nby; p.hiz.n_pad = pl.n_pad;
+    // the map's padding entries are read into shared memory but never indexed; clear them once
+    if ((e = cudaMemsetAsync(hz, 0xFF, dyn, st)) != cudaSuccess) return cuda_fail(e, "clear Hi-Z map");
+
+    const uint64_t P = a->n_points, spp = (uint64_t)(a->iterations - a->burn_in);
+    uint64_t n0 = (64ull * (uint64_t)a->width * (uint64_t)a->height + spp - 1) / spp;
+    n0 = (n0 + cfs::kHizThreads - 1) / cfs::kHizThreads * cfs::kHizThreads;
+    const uint64_t cuts[4] = {0, n0 < P ? n0 : P, 8 * n0 < P ? 8 * n0 : P, P};
+    const uint64_t off0 = p.point_offset;
+    for (int ph = 0; ph < 3; ++ph) {
+        const uint64_t lo = cuts[ph], hi = cuts[ph + 1];
+        if (hi <= lo) continue;
+        p.point_offset = off0 + lo; p.n_points = hi - lo;
+        if (ph == 0) {
+            uint64_t blocks = (p.n_points + cfs::kRenderThreads - 1) / cfs::kRenderThreads;
+            fn0<<<(unsigned)blocks, cfs::kRenderThreads, 0, st>>>(p);
+        } else {
+            const unsigned side = 1u << pl.shift;
+            cfs::hiz_build_kernel<<<pl.n, side * side, 0, st>>>((const unsigned long long *)a->d_image, a->width, a->height,
+                                                                  pl.shift, pl.nbx, hz);
+            ++g_launches;
+            uint64_t blocks = (p.n_points + cfs::kHizThreads - 1) / cfs::kHizThreads;
+            fn1<<<(unsigned)blocks, cfs::kHizThreads, dyn, st>>>(p);
+        }
+        ++g_launches;
+        if ((e = cudaGetLastError()) != cudaSuccess) return cuda_fail(e, "Hi-Z render launch");
+    }
+    return CFS_OK;
+}
+
+}  // namespace
+
 extern "C" cfs_status cfs_render(const cfs_system *s, const cfs_render_args *a, void *stream)
 {
     RenderParams p;
     cfs_status st = build_params(s, a, &p, true);
     if (st != CFS_OK) return st;
-    if (a->variant < CFS_VARIANT_AUTO || a->variant > CFS_VARIANT_CLUSTER_HIST) return fail(CFS_ERR_INVALID_ARG, "unknown variant %d", a->variant);
+    if (a->variant < CFS_VARIANT_AUTO || a->variant > CFS_VARIANT_DEPTH_HIZ) return fail(CFS_ERR_INVALID_ARG, "unknown variant %d", a->variant);
     const DeviceInfo &di = device_info();
     if (di.ok != 1) return fail(CFS_ERR_CUDA, "no CUDA device (this library has no CPU fallback)");
     const size_t hist_bytes = (size_t)a->width * a->height * 4;
@@ -641,6 +734,10 @@ extern "C" cfs_status cfs_render(const cfs_system *s, const cfs_render_args *a, 
         if (a->n_points == 0) return CFS_OK;
         return render_cluster_hist(s, a, p, di, (cudaStream_t)stream);
     }
+    if (a->variant == CFS_VARIANT_DEPTH_HIZ) {
+        if (a->n_points == 0) return CFS_OK;
+        return render_depth_hiz(s, a, p, di, (cudaStream_t)stream);
+    }
     if (a->variant == CFS_VARIANT_SHARED_HIST || a->variant == CFS_VARIANT_WARP_AGG) {
         if (a->out_mode != CFS_OUT_HIST_U32) return fail(CFS_ERR_UNSUPPORTED, "variant %d is for HIST_U32 output only", a->variant);
         if (a->variant == CFS_VARIANT_SHARED_HIST && hist_bytes > shared_hist_limit(di))
@@ -651,6 +748,10 @@ extern "C" cfs_status cfs_render(const cfs_system *s, const cfs_render_args *a, 
         // per CTA; big renders with scratch memory go through the tile bins; else direct L2 atomics
         if (a->out_mode == CFS_OUT_HIST_U32 && hist_bytes <= shared_hist_limit(di) && n_splats >= (uint64_t)di.sms * (hist_bytes / 4)) {
             splat = cfs::SPLAT_HIST_SHARED;
+        } else if (a->out_mode == CFS_OUT_DEPTH_RGBA8_U64 && s->gen == CFS_GEN_IFS && a->d_scratch && n_splats >= (1ull << 27) &&
+                   cfs_hiz_scratch_bytes(a->width, a->height) != 0 && a->scratch_bytes >= cfs_hiz_scratch_bytes(a->width, a->height)) {
+            // occluded splats stop at a shared-memory Hi-Z map instead of a random L2 load
+            return render_depth_hiz(s, a, p, di, (cudaStream_t)stream);
         } else if (a->d_scratch && a->n_points >= (uint64_t)di.sms * cfs::kBinCtasPerSm * cfs::kBinThreads && n_splats >= (1ull << 27) &&
                    (!cfs::sig_has_trig(chain_signature(p)) || (a->flags & CFS_FLAG_FAST_TRIG))) {
             // the tile bins trade the L2 atomic (~190 G/s) for ~15 more instructions per splat: measured

@@ -50,6 +50,7 @@ enum SplatKind : int {
     SPLAT_NONE = 5,          // trace kernel
     SPLAT_HIST_CLUSTER = 7,  // histogram distributed over the shared memory of a thread-block cluster
                              // (red.shared::cluster.add.u32 through DSMEM), merged by red.global
+    SPLAT_DEPTH_HIZ = 8,     // SPLAT_DEPTH behind a coarse conservative depth map (Hi-Z) held in shared memory
     SPLAT_BIN = 6            // tile-binned: records partitioned by image tile into a block pool
                              // (pass 1), accumulated per tile in shared memory (pass 2)
 };
@@ -66,6 +67,17 @@ constexpr uint32_t kBinInvalid = 0xFFFFFFFFu;  // tile has no block (pool or lis
 constexpr int kBinThreads = 1024;              // CTA size of pass 1 and CTAs per SM.  Measured on configs[1]: 1 x 1024
 constexpr int kBinCtasPerSm = 1;               // threads 4.69 ms, 2 x 512 threads (half-length staging rows) 5.53 ms
 constexpr int kBinAccThreads = 1024;           // CTA size of pass 2 (one CTA per SM: the tile fills shared memory)
+
+// Hi-Z pre-test of the depth splat (DESIGN "Hi-Z variant").  hz[by * nbx + bx] is an upper bound of
+// (depth bits >> 16) over the 2^shift x 2^shift pixel block (bx, by), taken from a snapshot of the
+// depth image; the image only decreases, so the bound stays valid for the rest of the render.
+constexpr int kHizThreads = 512;               // CTA size of the Hi-Z render kernel, two CTAs per SM
+constexpr int kHizCtasPerSm = 2;
+constexpr uint32_t kHizMaxBytes = 96 * 1024;   // per CTA, in shared memory
+struct HizParams {
+    const uint16_t *hz;    // nbx * nby entries (device)
+    uint32_t shift, nbx, nby, n_pad;   // n_pad = entries rounded up to a multiple of 8 (copied as 16-byte vectors)
+};
 
 struct BinParams {
     uint16_t *pool;        // nb * kBinBlockRecords records
@@ -107,11 +119,14 @@ struct RenderParams {
     int32_t pick_shift;          // >= 0: k = u >> pick_shift (equal power-of-two thresholds)
     int32_t n_thr;               // thresholds below 2^32 (k = #{j < n_thr : u >= T[j]})
     int32_t pick_steps;          // max thresholds inside one 2^24 bucket of u
+    uint32_t coef_rows;          // 16-byte coefficient rows in use (n_funcs x rows per map)
+    uint32_t coef_cshift;        // log2(copies of each coefficient row in shared memory), bank-conflict-free table reads
     uint32_t points_per_thread;  // shared-hist persistent grid
     uint32_t hist_bins;          // W*H (shared-hist and cluster-hist variants)
     uint32_t slice_shift;        // cluster-hist: bins per CTA = 1 << slice_shift, bin b lives in CTA rank b >> slice_shift
 
     BinParams bin;               // SPLAT_BIN only
+    HizParams hiz;               // SPLAT_DEPTH_HIZ only
 
     ChainStep chain[kMaxChain];
     uint32_t T[kMaxFuncs];       // thresholds (u32), T[j >= n_thr] = 0xFFFFFFFF

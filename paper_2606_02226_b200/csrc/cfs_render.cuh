@@ -83,6 +83,20 @@ __device__ __forceinline__ uint32_t chain_and_splat(const RenderParams &prm, con
         return (have && !ok) ? 1u : 0u;
     }
     if (!ok) return 1u;
+    if (SPLAT == SPLAT_DEPTH_HIZ) {
+        // Hi-Z pre-test in shared memory: a splat whose depth bits exceed the block's upper bound is
+        // certainly occluded (the bound comes from a snapshot of an image that only decreases), so
+        // it never leaves the SM.  ~95 % of the splats of a solid stop here (DESIGN "Hi-Z variant").
+        int px = __float2int_rd(__fmaf_rn(qx, prm.sx, prm.ox));
+        int py = __float2int_rd(__fmaf_rn(qy, prm.sy, prm.oy));
+        px = min(max(px, 0), prm.W - 1);
+        py = min(max(py, 0), prm.H - 1);
+        const uint16_t *hz = reinterpret_cast<const uint16_t *>(s_hist);
+        const uint32_t bound = hz[(uint32_t)(py >> prm.hiz.shift) * prm.hiz.nbx + (uint32_t)(px >> prm.hiz.shift)];
+        if ((__float_as_uint(qz) >> 16) > bound) return 0u;
+        splat_depth(reinterpret_cast<unsigned long long *>(prm.image), py * prm.W + px, qz, s.pal8[k]);
+        return 0u;
+    }
     const int pix = (SPLAT == SPLAT_BIN) ? bin_pixel_of(br, qx, qy) : pixel_of(prm, qx, qy);
     if (SPLAT == SPLAT_HIST_DIRECT) {
         red_add_u32(reinterpret_cast<uint32_t *>(prm.image) + pix, 1u);
@@ -165,7 +179,7 @@ __device__ __forceinline__ uint32_t iterate_block(const RenderParams &prm, const
         for (int j = 0; j < 4; ++j) {
             const uint32_t u = (j == 0) ? w.x : (j == 1) ? w.y : (j == 2) ? w.z : w.w;
             K[j] = pick_index(u, s, prm);
-            apply_gen<DIM, AFF>(K[j], s, gx, gy, gz);
+            apply_gen<DIM, AFF>(K[j], s, prm, gx, gy, gz);
             X[j] = gx; Y[j] = gy; Z[j] = gz;                 // the copies of Fig. 2(B)
         }
 #pragma unroll
@@ -182,7 +196,7 @@ __device__ __forceinline__ uint32_t iterate_block(const RenderParams &prm, const
             if (CHECKED && it >= prm.iterations) break;
             const uint32_t u = (j == 0) ? w.x : (j == 1) ? w.y : (j == 2) ? w.z : w.w;
             const int k = pick_index(u, s, prm);
-            apply_gen<DIM, AFF>(k, s, gx, gy, gz);
+            apply_gen<DIM, AFF>(k, s, prm, gx, gy, gz);
             const bool past = !CHECKED || it >= prm.burn_in;
             if (past || (SIG == kChainGeneric && prm.reuse))
                 dropped += chain_and_splat<DIM, GEN, SPLAT, SIG, TRIG>(prm, s, s_hist, gx, gy, gz, k, 0u, have, past, br);
@@ -199,8 +213,9 @@ __device__ __forceinline__ uint32_t iterate_block(const RenderParams &prm, const
 // ---------------------------------------------------------------------------------------------
 // the kernel
 template <int DIM, int GEN, int AFF, int SPLAT, uint32_t SIG, int TRIG>
-__global__ void __launch_bounds__(SPLAT == SPLAT_BIN ? kBinThreads : SPLAT == SPLAT_HIST_CLUSTER ? kClusterThreads : kRenderThreads,
-                                  SPLAT == SPLAT_BIN ? kBinCtasPerSm : 0)
+__global__ void __launch_bounds__(SPLAT == SPLAT_BIN ? kBinThreads : SPLAT == SPLAT_HIST_CLUSTER ? kClusterThreads :
+                                  SPLAT == SPLAT_DEPTH_HIZ ? kHizThreads : kRenderThreads,
+                                  SPLAT == SPLAT_BIN ? kBinCtasPerSm : SPLAT == SPLAT_DEPTH_HIZ ? kHizCtasPerSm : 0)
 render_kernel(const __grid_constant__ RenderParams prm)
 {
     __shared__ SharedTables s;
@@ -211,6 +226,11 @@ render_kernel(const __grid_constant__ RenderParams prm)
     if (SPLAT == SPLAT_HIST_CLUSTER) {   // this CTA's slice; nobody may touch a peer's slice before it is cleared
         for (uint32_t i = threadIdx.x; i < (1u << prm.slice_shift); i += blockDim.x) s_hist[i] = 0u;
         cluster_sync_all();
+    }
+    if (SPLAT == SPLAT_DEPTH_HIZ) {      // the Hi-Z map of this render phase: 16-byte vectors, L2 -> shared memory
+        const uint4 *src = reinterpret_cast<const uint4 *>(prm.hiz.hz);
+        uint4 *dst = reinterpret_cast<uint4 *>(s_hist);
+        for (uint32_t i = threadIdx.x; i < prm.hiz.n_pad / 8u; i += blockDim.x) dst[i] = __ldcg(src + i);
     }
     BinLane bl = {0u, 0u, 0u};
     BinRegs br = {};
@@ -344,7 +364,7 @@ trace_kernel(const __grid_constant__ RenderParams prm)
                 w.x = w.y; w.y = w.z; w.z = w.w;
                 const int k = pick_index(u, s, prm);
                 if (prm.tr_picks) prm.tr_picks[i * (uint64_t)prm.iterations + it] = (uint8_t)k;
-                apply_gen<DIM, AFF>(k, s, gx, gy, gz);
+                apply_gen<DIM, AFF>(k, s, prm, gx, gy, gz);
             }
             if (it < prm.burn_in && !prm.reuse) continue;
             qx = gx; qy = gy; qz = gz;

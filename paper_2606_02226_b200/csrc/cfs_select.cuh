@@ -19,6 +19,7 @@ render_fn select_splat(int splat)
     if constexpr (GEN == 0) { CFS_CASE(SPLAT_HIST_CLUSTER) }
     CFS_CASE(SPLAT_RGBA)
     if constexpr (DIM == 3) { CFS_CASE(SPLAT_DEPTH) }
+    if constexpr (DIM == 3 && GEN == 0) { CFS_CASE(SPLAT_DEPTH_HIZ) }
     if constexpr (GEN == 0) { CFS_CASE(SPLAT_BIN) }
 #undef CFS_CASE
     return nullptr;
@@ -42,7 +43,7 @@ render_fn select_trace(int gen, int aff)
 }
 
 constexpr unsigned kSplatsAll = (1u << SPLAT_HIST_DIRECT) | (1u << SPLAT_HIST_SHARED) | (1u << SPLAT_HIST_WARPAGG) | (1u << SPLAT_HIST_CLUSTER) |
-                                (1u << SPLAT_RGBA) | (1u << SPLAT_DEPTH) | (1u << SPLAT_BIN);
-constexpr unsigned kSplatsDirect = (1u << SPLAT_HIST_DIRECT) | (1u << SPLAT_RGBA) | (1u << SPLAT_DEPTH) | (1u << SPLAT_BIN);
+                                (1u << SPLAT_RGBA) | (1u << SPLAT_DEPTH) | (1u << SPLAT_BIN) | (1u << SPLAT_DEPTH_HIZ);
+constexpr unsigned kSplatsDirect = (1u << SPLAT_HIST_DIRECT) | (1u << SPLAT_RGBA) | (1u << SPLAT_DEPTH) | (1u << SPLAT_BIN) | (1u << SPLAT_DEPTH_HIZ);
 
 }  // namespace cfs
