@@ -40,17 +40,61 @@ NCU_TRAFFIC_BYTES_PER_LAUNCH_DIRECT = 7.06e6 # direct kernel: profiles/r01h_dire
 
 # ----------------------------------------------------------------------------- clocks sampler
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    """SM clock / power / throttle reasons DURING the timed region (B200_PROFILING.md recipe).  The timed
+    region of configs[1] lasts tens of milliseconds, shorter than one `nvidia-smi -lms` period, so the
+    samples come from NVML in a polling thread (the library nvidia-smi itself reads); nvidia-smi is the
+    fallback when NVML cannot be loaded."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
+    BITS = {"hw_slowdown": 0x8, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20, "sw_power_cap": 0x4}
 
-    def __init__(self, index: int):
-        self.rows = []
+    def __init__(self, index: int, uuid=None):
+        self.rows = []          # nvidia-smi lines
+        self.samples = []       # (sm_mhz, power_w, reasons bit mask) from NVML
         self.proc = None
+        self.thread = None
         self.index = index
+        self.stop_flag = threading.Event()
+        self.nvml = None
+        self.handle = None
+        self.sm_max = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            h = None
+            if uuid:
+                try:
+                    h = pynvml.nvmlDeviceGetHandleByUUID(("GPU-" + str(uuid)).encode())
+                except Exception:
+                    h = None
+            if h is None:
+                h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.nvml, self.handle = pynvml, h
+            self.sm_max = float(pynvml.nvmlDeviceGetMaxClockInfo(h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self.nvml = None
+
+    def _poll(self):
+        n, h = self.nvml, self.handle
+        while not self.stop_flag.is_set():
+            try:
+                sm = float(n.nvmlDeviceGetClockInfo(h, n.NVML_CLOCK_SM))
+                pw = n.nvmlDeviceGetPowerUsage(h) / 1000.0
+                try:
+                    rs = int(n.nvmlDeviceGetCurrentClocksEventReasons(h))
+                except Exception:
+                    rs = int(n.nvmlDeviceGetCurrentClocksThrottleReasons(h))
+                self.samples.append((sm, pw, rs))
+            except Exception:
+                pass
+            time.sleep(0.002)
 
     def start(self):
+        if self.nvml is not None:
+            self.thread = threading.Thread(target=self._poll, daemon=True)
+            self.thread.start()
+            return
         try:
             self.proc = subprocess.Popen(
                 ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
@@ -65,6 +109,18 @@ class ClockSampler:
             self.rows.append(line.strip())
 
     def stop(self):
+        if self.nvml is not None:
+            self.stop_flag.set()
+            if self.thread:
+                self.thread.join(timeout=1)
+            sm = [x[0] for x in self.samples]
+            pw = [x[1] for x in self.samples]
+            mask = 0
+            for x in self.samples:
+                mask |= x[2]
+            reasons = sorted(nm for nm, bit in self.BITS.items() if mask & bit)
+            return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": self.sm_max,
+                    "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": reasons, "source": "nvml"}
         if not self.proc:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
         self.proc.terminate()
@@ -86,7 +142,8 @@ class ClockSampler:
                 if v.lower().startswith("active"):
                     reasons.add(nm)
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons),
+                "source": "nvidia-smi"}
 
 
 # ----------------------------------------------------------------------------- reference arm (oracle)
@@ -226,8 +283,6 @@ SCRATCH_CAP_BYTES = 8 << 30
 def make_scratch(cfs, torch, sysh, render):
     """Scratch of the tile-binned variant (None when the variant cannot serve the workload)."""
     need = cfs.cfs_binned_scratch_bytes(sysh, cfs.make_args(render))
-    if need == 0 and render.out_mode == "depth_u64":      # the Hi-Z map of the depth variant
-        need = cfs.cfs_hiz_scratch_bytes(render.width, render.height)
     if need == 0:
         return None
     return torch.empty(min(need, SCRATCH_CAP_BYTES), dtype=torch.uint8, device="cuda")
@@ -326,7 +381,11 @@ def run_ours(args):
     if world > 1:
         dist.barrier()
     torch.cuda.synchronize()
-    sampler = ClockSampler(local)
+    try:
+        dev_uuid = torch.cuda.get_device_properties(local).uuid
+    except Exception:
+        dev_uuid = None
+    sampler = ClockSampler(local, dev_uuid)
     if rank == 0:
         sampler.start()
     evs = [step(True) for _ in range(args.steps)]

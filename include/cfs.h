@@ -169,8 +169,8 @@ uint64_t cfs_binned_scratch_bytes(const cfs_system *sys, const cfs_render_args *
 
 /* bytes of d_scratch CFS_VARIANT_DEPTH_HIZ needs for a width x height depth image (host arithmetic,
  * no device needed); 0 when the image is too large for a shared-memory Hi-Z map (> 96 KiB at
- * 32 x 32-pixel blocks).  With that much scratch given, CFS_VARIANT_AUTO takes the Hi-Z path for
- * DEPTH renders of an IFS generator with at least 2^27 splats. */
+ * 32 x 32-pixel blocks).  CFS_VARIANT_AUTO does not take this path: on configs[4] it was measured level
+ * with the direct one (the direct path is bound by the SM-to-L2 request rate, this one by instruction issue). */
 uint64_t cfs_hiz_scratch_bytes(int32_t width, int32_t height);
 
 /* the tile plan of the BINNED variant for an image and a device shape, host arithmetic only (no device

@@ -278,6 +278,7 @@ cfs_status build_params(const cfs_system *s, const cfs_render_args *a, RenderPar
         p.coef_rows = (uint32_t)s->funcs.size() * rows_per_map;
         p.coef_cshift = 0;
         if (p.coef_rows > 8) while (p.coef_cshift < 3 && (p.coef_rows << (p.coef_cshift + 1)) <= (uint32_t)cfs::kCoefSlots) ++p.coef_cshift;
+        p.coef_rstride = 16u << p.coef_cshift; p.coef_kstride = rows_per_map * p.coef_rstride;
     }
     memcpy(p.T, s->T, sizeof(p.T)); memcpy(p.lut, s->lut, sizeof(p.lut));
     memcpy(p.coef, s->coef, sizeof(p.coef)); memcpy(p.pal8, s->pal8, sizeof(p.pal8));
@@ -748,10 +749,10 @@ extern "C" cfs_status cfs_render(const cfs_system *s, const cfs_render_args *a, 
         // per CTA; big renders with scratch memory go through the tile bins; else direct L2 atomics
         if (a->out_mode == CFS_OUT_HIST_U32 && hist_bytes <= shared_hist_limit(di) && n_splats >= (uint64_t)di.sms * (hist_bytes / 4)) {
             splat = cfs::SPLAT_HIST_SHARED;
-        } else if (a->out_mode == CFS_OUT_DEPTH_RGBA8_U64 && s->gen == CFS_GEN_IFS && a->d_scratch && n_splats >= (1ull << 27) &&
-                   cfs_hiz_scratch_bytes(a->width, a->height) != 0 && a->scratch_bytes >= cfs_hiz_scratch_bytes(a->width, a->height)) {
-            // occluded splats stop at a shared-memory Hi-Z map instead of a random L2 load
-            return render_depth_hiz(s, a, p, di, (cudaStream_t)stream);
+        } else if (a->out_mode == CFS_OUT_DEPTH_RGBA8_U64) {
+            // direct: ld.cg pre-test + atom.min.  Measured at the SM-to-L2 request rate (one sector request per
+            // clock and SM, l1tex2xbar 98 % busy); CFS_VARIANT_DEPTH_HIZ removes that bound but lands on the
+            // issue rate at the same time (228.7 ms both on configs[4]), so AUTO keeps the path without scratch
         } else if (a->d_scratch && a->n_points >= (uint64_t)di.sms * cfs::kBinCtasPerSm * cfs::kBinThreads && n_splats >= (1ull << 27) &&
                    (!cfs::sig_has_trig(chain_signature(p)) || (a->flags & CFS_FLAG_FAST_TRIG))) {
             // the tile bins trade the L2 atomic (~190 G/s) for ~15 more instructions per splat: measured

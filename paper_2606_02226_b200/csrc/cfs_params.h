@@ -71,7 +71,7 @@ constexpr int kBinAccThreads = 1024;           // CTA size of pass 2 (one CTA pe
 // Hi-Z pre-test of the depth splat (DESIGN "Hi-Z variant").  hz[by * nbx + bx] is an upper bound of
 // (depth bits >> 16) over the 2^shift x 2^shift pixel block (bx, by), taken from a snapshot of the
 // depth image; the image only decreases, so the bound stays valid for the rest of the render.
-constexpr int kHizThreads = 512;               // CTA size of the Hi-Z render kernel, two CTAs per SM
+constexpr int kHizThreads = 768;               // CTA size of the Hi-Z render kernel, two CTAs per SM
 constexpr int kHizCtasPerSm = 2;
 constexpr uint32_t kHizMaxBytes = 96 * 1024;   // per CTA, in shared memory
 struct HizParams {
@@ -120,6 +120,7 @@ struct RenderParams {
     int32_t n_thr;               // thresholds below 2^32 (k = #{j < n_thr : u >= T[j]})
     int32_t pick_steps;          // max thresholds inside one 2^24 bucket of u
     uint32_t coef_rows;          // 16-byte coefficient rows in use (n_funcs x rows per map)
+    uint32_t coef_kstride, coef_rstride; // bytes between the first rows of two maps / between the rows of one map
     uint32_t coef_cshift;        // log2(copies of each coefficient row in shared memory), bank-conflict-free table reads
     uint32_t points_per_thread;  // shared-hist persistent grid
     uint32_t hist_bins;          // W*H (shared-hist and cluster-hist variants)

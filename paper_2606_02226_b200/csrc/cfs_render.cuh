@@ -67,7 +67,7 @@ __device__ __forceinline__ void splat_depth(unsigned long long *buf, int pix, fl
 // Returns 1 when the splat was dropped (dead or out of bounds), else 0.  Fig. 2(C) reuse is a
 // run-time option of the interpreter kernels only (compiled chains are never used with it).
 template <int DIM, int GEN, int SPLAT, uint32_t SIG, int TRIG>
-__device__ __forceinline__ uint32_t chain_and_splat(const RenderParams &prm, const SharedTables &s, uint32_t *s_hist,
+__device__ __forceinline__ uint32_t chain_and_splat(const RenderParams &prm, const SharedTables &s, const Sm &sm, uint32_t *s_hist,
                                                     float &gx, float &gy, float &gz, int k, uint32_t point_rgba8,
                                                     bool have, bool past_burn_in, const BinRegs &br)
 {
@@ -91,10 +91,10 @@ __device__ __forceinline__ uint32_t chain_and_splat(const RenderParams &prm, con
         int py = __float2int_rd(__fmaf_rn(qy, prm.sy, prm.oy));
         px = min(max(px, 0), prm.W - 1);
         py = min(max(py, 0), prm.H - 1);
-        const uint16_t *hz = reinterpret_cast<const uint16_t *>(s_hist);
-        const uint32_t bound = hz[(uint32_t)(py >> prm.hiz.shift) * prm.hiz.nbx + (uint32_t)(px >> prm.hiz.shift)];
+        const uint32_t bound = lds_u16(sm.dyn + 2u * ((uint32_t)(py >> prm.hiz.shift) * prm.hiz.nbx + (uint32_t)(px >> prm.hiz.shift)));
         if ((__float_as_uint(qz) >> 16) > bound) return 0u;
-        splat_depth(reinterpret_cast<unsigned long long *>(prm.image), py * prm.W + px, qz, s.pal8[k]);
+        splat_depth(reinterpret_cast<unsigned long long *>(prm.image), py * prm.W + px, qz,
+                    lds_u32(sm.tab + CFS_SM_OFF(pal8) + 4u * (uint32_t)k));
         return 0u;
     }
     const int pix = (SPLAT == SPLAT_BIN) ? bin_pixel_of(br, qx, qy) : pixel_of(prm, qx, qy);
@@ -110,12 +110,12 @@ __device__ __forceinline__ uint32_t chain_and_splat(const RenderParams &prm, con
             red_add_v4_f32(dst, (float)(point_rgba8 & 0xFFu), (float)((point_rgba8 >> 8) & 0xFFu),
                            (float)((point_rgba8 >> 16) & 0xFFu), 1.0f);
         } else {          // colour of the map applied in this iteration
-            const float4 c = s.palette[k];
+            const float4 c = lds_v4(sm.tab + CFS_SM_OFF(palette) + 16u * (uint32_t)k);
             red_add_v4_f32(dst, c.x, c.y, c.z, 1.0f);
         }
     } else if (SPLAT == SPLAT_DEPTH) {
         splat_depth(reinterpret_cast<unsigned long long *>(prm.image), pix, qz,
-                    GEN == 1 ? point_rgba8 : s.pal8[k]);
+                    GEN == 1 ? point_rgba8 : lds_u32(sm.tab + CFS_SM_OFF(pal8) + 4u * (uint32_t)k));
     } else if (SPLAT == SPLAT_BIN) {
         bin_append(prm, s, br, pix, k);
     }
@@ -159,7 +159,7 @@ __device__ __forceinline__ uint32_t bin_block_splat(const RenderParams &prm, con
 // has no per-iteration tests (the steady state of a render); CHECKED = true handles burn-in
 // and the ragged last block.
 template <int DIM, int GEN, int AFF, int SPLAT, uint32_t SIG, int TRIG, bool CHECKED>
-__device__ __forceinline__ uint32_t iterate_block(const RenderParams &prm, const SharedTables &s, uint32_t *s_hist,
+__device__ __forceinline__ uint32_t iterate_block(const RenderParams &prm, const SharedTables &s, const Sm &sm, uint32_t *s_hist,
                                                   uint32_t plo, uint32_t phi, int it0, float &gx, float &gy, float &gz,
                                                   bool have, BinLane &bl, const BinRegs &br)
 {
@@ -178,8 +178,8 @@ __device__ __forceinline__ uint32_t iterate_block(const RenderParams &prm, const
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
             const uint32_t u = (j == 0) ? w.x : (j == 1) ? w.y : (j == 2) ? w.z : w.w;
-            K[j] = pick_index(u, s, prm);
-            apply_gen<DIM, AFF>(K[j], s, prm, gx, gy, gz);
+            K[j] = pick_index(u, sm, prm);
+            apply_gen<DIM, AFF>(K[j], sm, prm, gx, gy, gz);
             X[j] = gx; Y[j] = gy; Z[j] = gz;                 // the copies of Fig. 2(B)
         }
 #pragma unroll
@@ -195,11 +195,11 @@ __device__ __forceinline__ uint32_t iterate_block(const RenderParams &prm, const
             const int it = it0 + j;
             if (CHECKED && it >= prm.iterations) break;
             const uint32_t u = (j == 0) ? w.x : (j == 1) ? w.y : (j == 2) ? w.z : w.w;
-            const int k = pick_index(u, s, prm);
-            apply_gen<DIM, AFF>(k, s, prm, gx, gy, gz);
+            const int k = pick_index(u, sm, prm);
+            apply_gen<DIM, AFF>(k, sm, prm, gx, gy, gz);
             const bool past = !CHECKED || it >= prm.burn_in;
             if (past || (SIG == kChainGeneric && prm.reuse))
-                dropped += chain_and_splat<DIM, GEN, SPLAT, SIG, TRIG>(prm, s, s_hist, gx, gy, gz, k, 0u, have, past, br);
+                dropped += chain_and_splat<DIM, GEN, SPLAT, SIG, TRIG>(prm, s, sm, s_hist, gx, gy, gz, k, 0u, have, past, br);
         }
     }
     if (SPLAT == SPLAT_BIN && ((((uint32_t)it0 >> 2) + 1u) & prm.bin.check_mask) == 0u) {   // CTA-uniform
@@ -232,6 +232,8 @@ render_kernel(const __grid_constant__ RenderParams prm)
         uint4 *dst = reinterpret_cast<uint4 *>(s_hist);
         for (uint32_t i = threadIdx.x; i < prm.hiz.n_pad / 8u; i += blockDim.x) dst[i] = __ldcg(src + i);
     }
+    __shared__ Sm s_sm;
+    sm_publish(&s_sm, s, s_hist);
     BinLane bl = {0u, 0u, 0u};
     BinRegs br = {};
     __shared__ BinRegs s_br;
@@ -245,6 +247,7 @@ render_kernel(const __grid_constant__ RenderParams prm)
     }
     __syncthreads();
     if (SPLAT == SPLAT_BIN) { br = s_br; br.dummy += threadIdx.x & 31u; }
+    const Sm sm = sm_read(&s_sm, prm);
 
     const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
     const int I = prm.iterations, B = prm.burn_in;
@@ -265,7 +268,7 @@ render_kernel(const __grid_constant__ RenderParams prm)
             float4 rec = make_float4(0.f, 0.f, 0.f, 0.f);
             if (have) rec = __ldcs(reinterpret_cast<const float4 *>(prm.cloud) + p);
             gx = rec.x; gy = rec.y; gz = (DIM == 3) ? rec.z : 0.0f;
-            dropped = chain_and_splat<DIM, GEN, SPLAT, SIG, TRIG>(prm, s, s_hist, gx, gy, gz, 0,
+            dropped = chain_and_splat<DIM, GEN, SPLAT, SIG, TRIG>(prm, s, sm, s_hist, gx, gy, gz, 0,
                                                                   __float_as_uint(rec.w), have, true, br);
         } else {
             const uint32_t plo = (uint32_t)p, phi = (uint32_t)(p >> 32);
@@ -279,13 +282,13 @@ render_kernel(const __grid_constant__ RenderParams prm)
             int it0 = 0;
 #pragma unroll 1
             for (; it0 < it_fast0; it0 += 4)
-                dropped += iterate_block<DIM, GEN, AFF, SPLAT, SIG, TRIG, true>(prm, s, s_hist, plo, phi, it0, gx, gy, gz, have, bl, br);
+                dropped += iterate_block<DIM, GEN, AFF, SPLAT, SIG, TRIG, true>(prm, s, sm, s_hist, plo, phi, it0, gx, gy, gz, have, bl, br);
 #pragma unroll 1
             for (; it0 < it_fast1; it0 += 4)
-                dropped += iterate_block<DIM, GEN, AFF, SPLAT, SIG, TRIG, false>(prm, s, s_hist, plo, phi, it0, gx, gy, gz, have, bl, br);
+                dropped += iterate_block<DIM, GEN, AFF, SPLAT, SIG, TRIG, false>(prm, s, sm, s_hist, plo, phi, it0, gx, gy, gz, have, bl, br);
 #pragma unroll 1
             for (; it0 < I; it0 += 4)
-                dropped += iterate_block<DIM, GEN, AFF, SPLAT, SIG, TRIG, true>(prm, s, s_hist, plo, phi, it0, gx, gy, gz, have, bl, br);
+                dropped += iterate_block<DIM, GEN, AFF, SPLAT, SIG, TRIG, true>(prm, s, sm, s_hist, plo, phi, it0, gx, gy, gz, have, bl, br);
         }
         if (have) { n_drop += dropped; n_in += (uint32_t)(I - B) - dropped; }
     }
@@ -339,7 +342,10 @@ trace_kernel(const __grid_constant__ RenderParams prm)
 {
     __shared__ SharedTables s;
     if (GEN == 0) load_tables(s, prm);
+    __shared__ Sm s_sm;
+    sm_publish(&s_sm, s, &s_sm);
     __syncthreads();
+    const Sm sm = sm_read(&s_sm, prm);
     const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
     for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < prm.n_points; i += stride) {
         const uint64_t p = prm.point_offset + i;
@@ -362,9 +368,9 @@ trace_kernel(const __grid_constant__ RenderParams prm)
                     w = philox4x32_10((uint32_t)p, (uint32_t)(p >> 32), (uint32_t)it >> 2, DOMAIN_PICK, prm);
                 const uint32_t u = w.x;
                 w.x = w.y; w.y = w.z; w.z = w.w;
-                const int k = pick_index(u, s, prm);
+                const int k = pick_index(u, sm, prm);
                 if (prm.tr_picks) prm.tr_picks[i * (uint64_t)prm.iterations + it] = (uint8_t)k;
-                apply_gen<DIM, AFF>(k, s, prm, gx, gy, gz);
+                apply_gen<DIM, AFF>(k, sm, prm, gx, gy, gz);
             }
             if (it < prm.burn_in && !prm.reuse) continue;
             qx = gx; qy = gy; qz = gz;

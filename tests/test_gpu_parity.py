@@ -279,6 +279,27 @@ def test_binned_hot_tile_overflow_and_limits(cfs, oracle):
         assert ei.value.status == cfs.CFS_ERR_UNSUPPORTED
 
 
+def test_depth_hiz_equals_direct_and_oracle(cfs, oracle):
+    """CFS_VARIANT_DEPTH_HIZ: occluded splats stop at a shared-memory Hi-Z map built from a snapshot of
+    the depth image.  The map is conservative (the image only decreases), so the image is identical per
+    pixel to the direct variant and to the oracle; sized so that all three phases run (plain slice, first
+    map, rebuilt map).  Without enough scratch the variant is refused."""
+    w = W.config(4).scaled(n_points=300000 + 7, iterations=100, width=256, height=144)
+    need = cfs.cfs_hiz_scratch_bytes(256, 144)
+    assert 0 < need < (1 << 20)
+    gh, ch = gpu_render(cfs, w, variant="depth_hiz", scratch_bytes=need)
+    gd, cd = gpu_render(cfs, w, variant="direct")
+    assert np.array_equal(gh, gd) and np.array_equal(ch, cd)
+    o, oc, _ = oracle.render_parallel(w.system, w.render)
+    assert np.array_equal(gh, o) and np.array_equal(ch, oc)
+    with pytest.raises(cfs.CfsError) as ei:
+        gpu_render(cfs, w, variant="depth_hiz", scratch_bytes=need // 2)
+    assert ei.value.status == cfs.CFS_ERR_UNSUPPORTED
+    with pytest.raises(cfs.CfsError) as ei:                          # not a depth render
+        gpu_render(cfs, W.config(1).scaled(n_points=100), variant="depth_hiz", scratch_bytes=need)
+    assert ei.value.status == cfs.CFS_ERR_UNSUPPORTED
+
+
 # ------------------------------------------------------------------ general tables and edge cases
 def test_general_pick_and_general_affine(cfs, oracle):
     """Non-uniform probabilities incl. zero-probability maps (table + compare pick), non-diagonal

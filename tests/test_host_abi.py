@@ -107,3 +107,14 @@ def test_binned_plan_tile_arithmetic_is_exact(cfs, size, mode, n_funcs):
     got = ((p * np.uint64(pl["magic"])) >> np.uint64(32)) >> np.uint64(pl["mshift"])
     assert np.array_equal(got, p // np.uint64(tp))
     assert pl["magic"] < 1 << 32
+
+
+def test_hiz_scratch_bytes_is_host_arithmetic(cfs):
+    """The Hi-Z map of CFS_VARIANT_DEPTH_HIZ: smallest 8/16/32-pixel block whose u16 map fits 96 KiB."""
+    for wd, ht, side in ((256, 144, 8), (1920, 1080, 8), (3840, 2160, 16), (7680, 4320, 32)):
+        n = -(-wd // side) * -(-ht // side)
+        assert (n + 7) // 8 * 8 * 2 <= 96 << 10
+        if side > 8:
+            assert -(-wd // (side // 2)) * -(-ht // (side // 2)) * 2 > 96 << 10
+        assert cfs.cfs_hiz_scratch_bytes(wd, ht) == (n + 7) // 8 * 8 * 2 + 256
+    assert cfs.cfs_hiz_scratch_bytes(16384, 16384) == 0 and cfs.cfs_hiz_scratch_bytes(0, 10) == 0
