@@ -33,8 +33,9 @@ METRIC = "cfs_point_iterations_per_s"
 UNIT = "point-iterations/s"
 L2_FLUSH_BYTES = 256 << 20
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the render kernel on configs[1], from
-# the `ncu --set full` capture summarised in profiles/r01_ncu_render_cfg1.md (null until captured)
-NCU_TRAFFIC_BYTES_PER_LAUNCH = 4.062e9       # binned pass 1: profiles/r01h_binned_cfg1.txt (0.001 GB read + 4.061 GB written)
+# the `ncu --set full` captures summarised in profiles/README.md
+NCU_TRAFFIC_BYTES_PER_LAUNCH = 0.989e9       # hybrid pass 1: profiles/r01j_hybrid_cfg1.txt (0.008 GB read + 0.982 GB written)
+NCU_TRAFFIC_BYTES_PER_LAUNCH_BINNED = 2.0e9  # pure bins (--variant binned): twice the records of the hybrid stage
 NCU_TRAFFIC_BYTES_PER_LAUNCH_DIRECT = 7.06e6 # direct kernel: profiles/r01h_direct_cfg1.txt (the image stays in L2)
 
 
@@ -461,7 +462,8 @@ def run_ours(args):
         roofline = {
             "bound": "alu", "achieved": P * I * n_instr / pass1_s / 1e12, "peak": rates["ffma"] / 1e12,
             "unit": "T lane-instructions/s", "frac": (P * I * n_instr / pass1_s) / rates["ffma"],
-            "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH, "kernel": "cfs::render_kernel<2,IFS,DIAG,BIN,swirl+affine,MUFU>",
+            "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH if hybrid else NCU_TRAFFIC_BYTES_PER_LAUNCH_BINNED,
+            "kernel": "cfs::render_kernel<2,IFS,DIAG,BIN,swirl+scale,%s>" % ("MUFU" if args.fast_trig else "sincosf"),
             "kernel_ms": pass1_s * 1e3, "render_ms": t_render * 1e3, "pass2_ms": (t_render - pass1_s) * 1e3,
             "algorithmic_lane_instructions_per_point_iteration": n_instr,
             "algorithmic_bytes_per_launch": int(S * 2) // (2 if hybrid else 1),      # one 16-bit record per binned splat
