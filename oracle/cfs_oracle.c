@@ -112,10 +112,32 @@ static void affine_apply(const float *m, int dim, float v[3])
     }
 }
 
+/* PAPER Eq. 1 (L49-58), the non-affine circle IFS: "functions to map the circle on to either the
+ * top or bottom half of itself" (L60).  As printed, with the reading of DESIGN R13:
+ *     r = sqrt(x^2 + y^2),  theta = atan(y/x) taken as the full-circle angle in [0, 2 pi),
+ *     theta_2 = pi (r + f_id)        [flag: pi (r^2 + f_id)],
+ *     r_2 = sqrt(theta / (2 pi)),
+ *     x_2 = r_2 cos theta_2,  y_2 = r_2 sin theta_2      (the source prints "r^2": a mangled r_2).
+ * Non-affine, hence tolerance-checked: evaluated in double on the float input, each output rounded
+ * once (DESIGN R5).  z is left alone. */
+static void circle_half_apply(const float *prm, float v[3])
+{
+    static const double PI = 3.14159265358979323846;
+    const double x = (double)v[0], y = (double)v[1];
+    const double fid = (double)prm[0];
+    const double r = sqrt(x * x + y * y);
+    double th = atan2(y, x);
+    if (th < 0.0) th += 2.0 * PI;
+    const double th2 = PI * ((prm[1] != 0.0f ? r * r : r) + fid);
+    const double r2 = sqrt(th / (2.0 * PI));
+    v[0] = (float)(r2 * cos(th2));
+    v[1] = (float)(r2 * sin(th2));
+}
+
 void orc_apply_func(const orc_func *f, int dim, float g[3])
 {
-    /* only ORC_F_AFFINE exists */
-    affine_apply(f->params, dim, g);
+    if (f->type == ORC_F_CIRCLE_HALF) circle_half_apply(f->params, g);
+    else affine_apply(f->params, dim, g);
 }
 
 /* ---------------------------------------------------------------- S6: chain transforms
@@ -303,7 +325,7 @@ static int run(const orc_system *s, const orc_render_args *a, int do_splat, uint
     if (s->gen_kind == ORC_GEN_IFS) {
         float prob[64];
         for (int j = 0; j < s->n_funcs; ++j) {
-            if (s->funcs[j].type != ORC_F_AFFINE) return -1;
+            if (s->funcs[j].type != ORC_F_AFFINE && !(s->funcs[j].type == ORC_F_CIRCLE_HALF && s->dim == 2)) return -1;
             prob[j] = s->funcs[j].prob;
         }
         if (orc_thresholds(prob, s->n_funcs, T)) return -1;

@@ -29,7 +29,7 @@ extern "C" {
 #endif
 
 enum { ORC_GEN_IFS = 0, ORC_GEN_CLOUD = 1 };
-enum { ORC_F_AFFINE = 0 };
+enum { ORC_F_AFFINE = 0, ORC_F_CIRCLE_HALF = 1 };
 enum {
     ORC_T_AFFINE = 0, ORC_T_SWIRL = 1, ORC_T_SINUSOIDAL = 2, ORC_T_ROTATE_Z = 3,
     ORC_T_TWIST_Z = 4, ORC_T_BEND = 5, ORC_T_PINHOLE = 6, ORC_T_STRETCH_COS = 7
@@ -39,7 +39,10 @@ enum { ORC_OUT_HIST_U32 = 0, ORC_OUT_RGBA = 1, ORC_OUT_DEPTH_U64 = 2 };
 enum { ORC_DOMAIN_PICK = 0, ORC_DOMAIN_INIT = 1 };
 
 /* generator function: AFFINE params, dim 2: a00 a01 a10 a11 b0 b1;
- * dim 3: a00..a22 row-major then b0 b1 b2. */
+ * dim 3: a00..a22 row-major then b0 b1 b2.
+ * CIRCLE_HALF (PAPER Eq. 1; dim 2 only): params[0] = f_id (0 -> top half, 1 -> bottom half of
+ * the unit disc), params[1] != 0 selects the r^2 reading of theta_2 (DESIGN R13).  PARITY UNPINNED
+ * beyond the invariants the paper states (L60): Eq. 1 is garbled in the source. */
 typedef struct { int32_t type; float prob; float params[12]; } orc_func;
 /* chain transform: effective parameter i = (float)((double)p0[i] + (double)t*(double)p1[i]) */
 typedef struct { int32_t type; float p0[12]; float p1[12]; } orc_xform;

@@ -19,7 +19,7 @@ import numpy as np
 
 from . import build as _build
 
-_F_TYPES = {"affine": 0}
+_F_TYPES = {"affine": 0, "circle_half": 1}
 _T_TYPES = {"affine": 0, "swirl": 1, "sinusoidal": 2, "rotate_z": 3, "twist_z": 4, "bend": 5,
             "pinhole": 6, "stretch_cos": 7}
 _COLORS = {"none": 0, "map_index": 1, "point": 2}

@@ -23,7 +23,7 @@ CLOUD_DTYPE = np.dtype([("x", "<f4"), ("y", "<f4"), ("z", "<f4"), ("rgba8", "<u4
 
 @dataclass
 class Func:
-    type: str            # "affine"
+    type: str            # "affine" | "circle_half" (PAPER Eq. 1: params = [f_id, r2_flag])
     prob: float
     params: Sequence[float]
 
@@ -99,6 +99,11 @@ def square_funcs(probs: Optional[Sequence[float]] = None) -> List[Func]:
 def sierpinski_vertices():
     h = math.sqrt(3.0) / 2.0
     return [(0.0, 1.0), (-h, -0.5), (h, -0.5)]
+
+
+def circle_funcs(r2_reading: bool = False) -> List[Func]:
+    """PAPER Eq. 1 (L47-60): the two maps sending the unit disc to its top (f_id 0) / bottom (f_id 1) half."""
+    return [Func("circle_half", 0.5, [float(fid), 1.0 if r2_reading else 0.0]) for fid in (0, 1)]
 
 
 def sierpinski_funcs(probs: Optional[Sequence[float]] = None) -> List[Func]:

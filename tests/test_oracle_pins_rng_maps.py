@@ -245,3 +245,65 @@ def test_pixel_rule_edges(oracle):
     b2 = (-16 / 9, 16 / 9, -1.0, 1.0)
     assert oracle.pixel(0.0, 0.0, b2, 1920, 1080) == 540 * 1920 + 960
     assert oracle.pixel(-1.7, 0.999, b2, 1920, 1080) == 1079 * 1920 + int(math.floor((-1.7 + 16 / 9) * 540))
+
+
+# ------------------------------------------------------------------ NEXT-1: PAPER Eq. 1, the circle IFS
+def _golden_eq1():
+    import os
+    rows = []
+    with open(os.path.join(os.path.dirname(__file__), "golden", "eq1_circle_half.txt")) as fh:
+        for ln in fh:
+            if ln.strip() and not ln.startswith("#"):
+                rows.append([float(v) for v in ln.split()])
+    return rows
+
+
+def test_circle_half_golden_values(oracle):
+    """Values worked by hand from the printed Eq. 1 (tests/golden/eq1_circle_half.txt)."""
+    rows = _golden_eq1()
+    assert len(rows) == 9
+    for x, y, fid, flag, ex, ey in rows:
+        g = oracle.apply_func(W.Func("circle_half", 0.5, [fid, flag]), 2, np.array([x, y, 0.0], dtype=np.float32))
+        assert abs(float(g[0]) - ex) < 2e-7 and abs(float(g[1]) - ey) < 2e-7, (x, y, fid, flag, g)
+
+
+@pytest.mark.parametrize("flag", [0.0, 1.0])
+def test_circle_half_invariants(oracle, flag):
+    """the maps send the disc "on to either the top or bottom half of itself": for r < 1 the
+    sign of y2 is decided by f_id alone and r2 < 1.  The map swaps the polar coordinates: the output radius
+    depends on the input ANGLE only, the output angle on the input RADIUS only."""
+    rng = np.random.default_rng(7)
+    for _ in range(300):
+        r, th = rng.uniform(0.01, 0.99), rng.uniform(0.01, 2 * math.pi - 0.01)
+        r_b, th_b = rng.uniform(0.01, 0.99), rng.uniform(0.01, 2 * math.pi - 0.01)
+        for fid in (0.0, 1.0):
+            f = W.Func("circle_half", 0.5, [fid, flag])
+            def m(rr, tt):
+                return oracle.apply_func(f, 2, np.array([rr * math.cos(tt), rr * math.sin(tt), 0.0], dtype=np.float32)).astype(np.float64)
+            a, b, c = m(r, th), m(r_b, th), m(r, th_b)
+            assert (a[1] >= 0) == (fid == 0.0) and np.hypot(a[0], a[1]) < 1.0
+            assert abs(np.hypot(a[0], a[1]) - np.hypot(b[0], b[1])) < 1e-6          # same angle -> same radius
+            assert abs(math.atan2(a[1], a[0]) - math.atan2(c[1], c[0])) < 1e-5      # same radius -> same angle
+
+
+def test_circle_half_r2_reading_has_uniform_invariant_density(oracle):
+    """In (s, u) = (r^2, theta / 2 pi) the r^2 reading is (s, u) -> (u, (s + f_id) / 2), which preserves
+    the uniform measure of the unit square, i.e. the uniform AREA measure of the disc: the chaos game's
+    histogram is flat over pixels wholly inside the disc (chi-square, one splat per point => i.i.d.)."""
+    sys_c = W.System(2, "ifs", W.circle_funcs(r2_reading=True), [], "none")
+    n, side = 400000, 32
+    r = W.Render(n, 1, 40, 39, side, side, (-1, 1, -1, 1), "hist_u32")
+    h, c = oracle.render(sys_c, r)
+    assert int(c[0]) == n
+    h = h.reshape(side, side).astype(np.float64)
+    edges = np.linspace(-1, 1, side + 1)
+    far = np.maximum(np.abs(edges[:-1]), np.abs(edges[1:]))
+    inside = (far[:, None] ** 2 + far[None, :] ** 2) < 1.0                  # all four corners inside the disc
+    exp = n * (2.0 / side) ** 2 / math.pi
+    chi2 = ((h[inside] - exp) ** 2 / exp).sum()
+    dof = int(inside.sum())
+    assert dof > 600 and abs(chi2 - dof) < 6 * math.sqrt(2 * dof), (chi2, dof)
+    # the as-printed reading (r, not r^2) is NOT uniform: same statistic, far outside the band
+    h2, _ = oracle.render(W.System(2, "ifs", W.circle_funcs(False), [], "none"), r)
+    h2 = h2.reshape(side, side).astype(np.float64)
+    assert ((h2[inside] - exp) ** 2 / exp).sum() > dof + 50 * math.sqrt(2 * dof)
