@@ -50,8 +50,14 @@ typedef enum {
 /* generator: an IFS solved by the chaos game, or a stored cloud */
 typedef enum { CFS_GEN_IFS = 0, CFS_GEN_CLOUD = 1 } cfs_gen_kind;
 /* generator function types.  AFFINE params: dim 2: a00 a01 a10 a11 b0 b1;
- * dim 3: a00..a22 row-major, then b0 b1 b2.  x' = fma(a00,x,fma(a01,y,b0)) etc. (DESIGN R4). */
-typedef enum { CFS_F_AFFINE = 0 } cfs_func_type;
+ * dim 3: a00..a22 row-major, then b0 b1 b2.  x' = fma(a00,x,fma(a01,y,b0)) etc. (DESIGN R4).
+ * CIRCLE_HALF (dim 2 only; every function of the generator must then be CIRCLE_HALF) is PAPER Eq. 1
+ * (L47-60), the non-affine circle IFS whose two maps send the unit disc to its top / bottom half:
+ * params[0] = f_id (0 or 1), params[1] != 0 selects the r^2 reading.  r = sqrt(x^2+y^2), theta = atan2(y,x)
+ * wrapped to [0, 2 pi), theta2 = pi (r + f_id) [flag: pi (r^2 + f_id)], r2 = sqrt(theta / 2 pi),
+ * (x', y') = (r2 cos theta2, r2 sin theta2) (DESIGN R13; the printed equation is garbled).  f_id is
+ * DATA (a table entry), so the two maps share one code path: no divergence from the random choice. */
+typedef enum { CFS_F_AFFINE = 0, CFS_F_CIRCLE_HALF = 1 } cfs_func_type;
 typedef struct { int32_t type; float prob; float params[12]; } cfs_func;
 
 /* chain transform types (applied to the copy, in order).  Effective parameter i of a step is

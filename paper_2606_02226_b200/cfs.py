@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libcfs_b200.so")
 
 CFS_OK, CFS_ERR_INVALID_ARG, CFS_ERR_UNSUPPORTED, CFS_ERR_CUDA, CFS_ERR_NOMEM = range(5)
 GEN = {"ifs": 0, "cloud": 1}
-F_TYPE = {"affine": 0}
+F_TYPE = {"affine": 0, "circle_half": 1}
 T_TYPE = {"affine": 0, "swirl": 1, "sinusoidal": 2, "rotate_z": 3, "twist_z": 4, "bend": 5,
           "pinhole": 6, "stretch_cos": 7}
 COLOR = {"none": 0, "map_index": 1, "point": 2}

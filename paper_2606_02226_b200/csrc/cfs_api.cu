@@ -149,11 +149,14 @@ cfs_status build_tables(cfs_system *s)
         if (s->dim == 2) diag = diag && m[1] == 0.0f && m[2] == 0.0f;
         else diag = diag && m[1] == 0.0f && m[2] == 0.0f && m[3] == 0.0f && m[5] == 0.0f && m[6] == 0.0f && m[7] == 0.0f;
     }
-    s->aff = diag ? cfs::AFF_DIAG : cfs::AFF_GENERAL;
+    const bool circle = n >= 1 && s->funcs[0].type == CFS_F_CIRCLE_HALF;     // all of them are (cfs_create)
+    s->aff = circle ? cfs::AFF_CIRCLE : diag ? cfs::AFF_DIAG : cfs::AFF_GENERAL;
     memset(s->coef, 0, sizeof(s->coef));
     for (int j = 0; j < n; ++j) {
         const float *m = s->funcs[j].params;
-        if (s->dim == 2 && diag) {
+        if (circle) {
+            float *r = s->coef + 4 * j;  r[0] = m[0]; r[1] = (m[1] != 0.0f) ? 1.0f : 0.0f;
+        } else if (s->dim == 2 && diag) {
             float *r = s->coef + 4 * j;  r[0] = m[0]; r[1] = m[3]; r[2] = m[4]; r[3] = m[5];
         } else if (s->dim == 2) {
             float *r = s->coef + 8 * j;  r[0] = m[0]; r[1] = m[1]; r[2] = m[4]; r[4] = m[2]; r[5] = m[3]; r[6] = m[5];
@@ -191,8 +194,12 @@ extern "C" cfs_status cfs_create(cfs_system **out, int32_t dim, int32_t gen_kind
         if (st == CFS_OK && color_rule == CFS_COLOR_POINT) st = fail(CFS_ERR_INVALID_ARG, "COLOR_POINT needs a CLOUD generator");
         if (st == CFS_OK && color_rule == CFS_COLOR_MAP_INDEX && !palette_rgba) st = fail(CFS_ERR_INVALID_ARG, "COLOR_MAP_INDEX needs a palette");
         for (int j = 0; st == CFS_OK && j < n_funcs; ++j) {
-            if (funcs[j].type != CFS_F_AFFINE) st = fail(CFS_ERR_INVALID_ARG, "funcs[%d]: unknown type %d", j, funcs[j].type);
-            const int np = (dim == 2) ? 6 : 12;
+            if (funcs[j].type != CFS_F_AFFINE && funcs[j].type != CFS_F_CIRCLE_HALF) st = fail(CFS_ERR_INVALID_ARG, "funcs[%d]: unknown type %d", j, funcs[j].type);
+            if (st == CFS_OK && funcs[j].type != funcs[0].type) st = fail(CFS_ERR_UNSUPPORTED, "funcs[%d]: AFFINE and CIRCLE_HALF maps cannot share a generator", j);
+            if (st == CFS_OK && funcs[j].type == CFS_F_CIRCLE_HALF && dim != 2) st = fail(CFS_ERR_INVALID_ARG, "CIRCLE_HALF is a 2-D map");
+            if (st == CFS_OK && funcs[j].type == CFS_F_CIRCLE_HALF && funcs[j].params[0] != 0.0f && funcs[j].params[0] != 1.0f)
+                st = fail(CFS_ERR_INVALID_ARG, "funcs[%d]: CIRCLE_HALF f_id must be 0 or 1", j);
+            const int np = (funcs[j].type == CFS_F_CIRCLE_HALF) ? 2 : (dim == 2) ? 6 : 12;
             for (int i = 0; st == CFS_OK && i < np; ++i)
                 if (bad_float(funcs[j].params[i])) st = fail(CFS_ERR_INVALID_ARG, "funcs[%d].params[%d] is not finite", j, i);
         }
@@ -274,7 +281,7 @@ cfs_status build_params(const cfs_system *s, const cfs_render_args *a, RenderPar
     p.pick_shift = s->pick_shift; p.n_thr = s->n_thr; p.pick_steps = s->pick_steps;
     {   // coefficient rows are replicated in shared memory (up to 8 copies) when more than 8 of them are in
         // use: with fewer, every row already has a bank group of its own
-        const uint32_t rows_per_map = (s->aff == cfs::AFF_DIAG) ? (s->dim == 2 ? 1u : 2u) : (s->dim == 2 ? 2u : 3u);
+        const uint32_t rows_per_map = (s->aff == cfs::AFF_CIRCLE) ? 1u : (s->aff == cfs::AFF_DIAG) ? (s->dim == 2 ? 1u : 2u) : (s->dim == 2 ? 2u : 3u);
         p.coef_rows = (uint32_t)s->funcs.size() * rows_per_map;
         p.coef_cshift = 0;
         if (p.coef_rows > 8) while (p.coef_cshift < 3 && (p.coef_rows << (p.coef_cshift + 1)) <= (uint32_t)cfs::kCoefSlots) ++p.coef_cshift;

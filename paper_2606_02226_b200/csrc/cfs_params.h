@@ -15,7 +15,7 @@ constexpr int kClusterThreads = 512;  // CTA size of the cluster-histogram varia
 constexpr int kClusterSize = 8;       // CTAs per cluster (portable maximum)
 
 // affine table forms (bit-identical results, DESIGN R4: fma(0,y,b) == b)
-enum AffForm : int { AFF_GENERAL = 0, AFF_DIAG = 1 };
+enum AffForm : int { AFF_GENERAL = 0, AFF_DIAG = 1, AFF_CIRCLE = 2 /* PAPER Eq. 1 maps: one row (f_id, r2 flag, -, -) per map */ };
 // transcendental evaluation of the non-affine chain steps: libdevice sincosf/sinf/cosf (<= 2 ulp)
 // or the MUFU special-function unit (sin.approx/cos.approx, abs. error ~2^-21 on [-pi, pi])
 enum TrigKind : int { TRIG_ACCURATE = 0, TRIG_FAST = 1, TRIG_RUNTIME = 2 /* prm.fast_trig decides (interpreter) */ };

@@ -30,6 +30,10 @@ template <int DIM, uint32_t SIG, int TRIG, unsigned SPLATS>
 render_fn select_render(int gen, int aff, int splat)
 {
     if (gen == 1) return select_splat<DIM, 1, AFF_GENERAL, SIG, TRIG, SPLATS>(splat);
+    if (aff == AFF_CIRCLE) {   // PAPER Eq. 1 generator: 2-D, chain interpreter only (no kernel per signature)
+        if constexpr (DIM == 2 && SIG == kChainGeneric) return select_splat<2, 0, AFF_CIRCLE, SIG, TRIG, SPLATS>(splat);
+        else return nullptr;
+    }
     if (aff == AFF_DIAG) return select_splat<DIM, 0, AFF_DIAG, SIG, TRIG, SPLATS>(splat);
     return select_splat<DIM, 0, AFF_GENERAL, SIG, TRIG, SPLATS>(splat);
 }
@@ -38,6 +42,10 @@ template <int DIM, uint32_t SIG, int TRIG>
 render_fn select_trace(int gen, int aff)
 {
     if (gen == 1) return trace_kernel<DIM, 1, AFF_GENERAL, SIG, TRIG>;
+    if (aff == AFF_CIRCLE) {
+        if constexpr (DIM == 2 && SIG == kChainGeneric) return trace_kernel<2, 0, AFF_CIRCLE, SIG, TRIG>;
+        else return nullptr;
+    }
     if (aff == AFF_DIAG) return trace_kernel<DIM, 0, AFF_DIAG, SIG, TRIG>;
     return trace_kernel<DIM, 0, AFF_GENERAL, SIG, TRIG>;
 }

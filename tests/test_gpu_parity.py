@@ -375,6 +375,49 @@ def test_reuse_composition_and_eq2(cfs, oracle):
             assert density_l1(g[:, ch], o[:, ch]) <= 4e-3      # 100k splats: a handful of edge flips
 
 
+@pytest.mark.parametrize("r2_reading", [False, True])
+@pytest.mark.parametrize("composition", ["A", "B", "C"])
+def test_eq1_circle_generator_fig2(cfs, oracle, r2_reading, composition):
+    """NEXT-1, the paper's own worked example (Fig. 2): the non-affine circle IFS of Eq. 1
+    alone (A), with Eq. 2 applied to a copy (B), and with the transformed point reused (C).  The maps are
+    non-affine and only contractive on average, so float32 and the double-evaluating oracle agree within
+    1e-4 on all but a sliver of points (those that passed within rounding of the angle cut or of r = 0);
+    pick sequences are bit-exact, counters conserve, densities agree."""
+    chain = [] if composition == "A" else [W.Xform("stretch_cos"), W.Xform("affine", [0.4, 0, 0, 0.4, 0, 0.3])]
+    sysc = W.System(2, "ifs", W.circle_funcs(r2_reading), chain, "map_index", W.palette_for(2),
+                    reuse=(composition == "C"))
+    w = W.Workload("eq1", sysc, W.Render(20000, 21, 60, 10, 256, 256, (-1.5, 1.5, -1.5, 1.5), "rgba_f32"))
+    gp, gg, gq, ga = gpu_trace(cfs, w)
+    op, og, oq, oa = oracle.trace(sysc, w.render)
+    assert np.array_equal(gp, op) and np.array_equal(ga, oa)
+    far_g = np.abs(gg.astype(np.float64) - og).max(axis=1) > COORD_TOL
+    far_q = np.abs(gq.astype(np.float64) - oq).max(axis=1) > COORD_TOL
+    assert far_g.mean() <= 2e-3 and far_q.mean() <= 2e-3, (far_g.mean(), far_q.mean())
+    if composition == "A":       # PAPER L60: f_id decides the half of the disc, and the point stays inside it
+        last = gp[:, -1]
+        assert np.all((gg[:, 1] >= 0) == (last == 0)) and np.all(np.hypot(gg[:, 0], gg[:, 1]) < 1.0 + 1e-6)
+    for variant in ("direct", "binned"):
+        g, gc = gpu_render(cfs, w, variant=variant, flags=["bin_hybrid"] if variant == "binned" else 0)
+        o, oc = oracle.render(sysc, w.render)
+        assert int(gc[0]) + int(gc[1]) == 20000 * 50 and abs(int(gc[0]) - int(oc[0])) <= 20
+        for ch in range(4):
+            if o[:, ch].sum() > 0:
+                assert density_l1(g[:, ch], o[:, ch]) <= 4e-3      # 1 M splats: edge flips + the sliver above
+
+
+def test_eq1_generator_validation(cfs):
+    f = W.circle_funcs()
+    with pytest.raises(cfs.CfsError) as ei:                      # mixed affine + circle
+        cfs.cfs_create(W.System(2, "ifs", [f[0], W.square_funcs()[0]], [], "none"))
+    assert ei.value.status == cfs.CFS_ERR_UNSUPPORTED
+    with pytest.raises(cfs.CfsError) as ei:                      # 3-D
+        cfs.cfs_create(W.System(3, "ifs", f, [], "none"))
+    assert ei.value.status == cfs.CFS_ERR_INVALID_ARG
+    with pytest.raises(cfs.CfsError) as ei:                      # f_id outside {0, 1}
+        cfs.cfs_create(W.System(2, "ifs", [W.Func("circle_half", 1.0, [2.0, 0.0])], [], "none"))
+    assert ei.value.status == cfs.CFS_ERR_INVALID_ARG
+
+
 def test_empty_and_accumulate(cfs, oracle):
     import torch
     w = W.config(0).scaled(n_points=0)
