@@ -17,8 +17,11 @@
  * uniform invariant density (chi-square), conservation, removed regions
  * (Sierpinski / carpet / Menger), word enumeration up to length 8, chain
  * invariants, depth buffer vs brute force, tone-map closed forms.
- * Parity unpinned: none of the functions below (the paper's Eq. 1 circle map is
- * not implemented here).
+ * Parity unpinned: the AS-PRINTED reading of the paper's Eq. 1 circle map
+ * (ORC_F_CIRCLE_HALF with params[1] == 0; DESIGN R13): the equation is garbled in
+ * the source, so beyond the invariants of PAPER L60, the polar-swap structure and
+ * nine hand-worked values nothing fixes it.  Its r^2 reading (params[1] != 0) is
+ * pinned by its closed-form uniform invariant density.  Everything else is pinned.
  */
 #ifndef CFS_ORACLE_H
 #define CFS_ORACLE_H
