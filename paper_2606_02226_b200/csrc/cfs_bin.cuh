@@ -52,17 +52,6 @@ __device__ __forceinline__ void bin_direct(const RenderParams &prm, const Shared
     }
 }
 
-// one splat down the direct path, from its image pixel and map index
-__device__ __forceinline__ void bin_direct_pix(const RenderParams &prm, const SharedTables &s, uint32_t pix, uint32_t k)
-{
-    if (prm.color_rule == 0) {
-        bin_red_add_u32(reinterpret_cast<uint32_t *>(prm.image) + pix, 1u);
-    } else {
-        const float4 c = s.palette[k];
-        bin_red_add_v4_f32(reinterpret_cast<float *>(prm.image) + 4 * (size_t)pix, c.x, c.y, c.z, 1.0f);
-    }
-}
-
 // values of the append fast path, derived once per thread (32-bit shared-window addresses, so
 // an access is one ATOMS / STS without generic-address arithmetic)
 struct BinRegs {
@@ -72,6 +61,7 @@ struct BinRegs {
     uint32_t tp, ntp, magic, mshift; // tile = umulhi(pix, magic) >> mshift == pix / tp for every pixel of the image; ntp = -tp
     uint32_t nk, kmask;            // colour slots per pixel, and the mask that zeroes k for HIST
     float sx, ox, sy, oy;          // pixel map (DESIGN R8)
+    float xmin, xmax, ymin, ymax;  // closed bounds (DESIGN R8)
     int W, Wm1, Hm1;
 };
 
@@ -85,8 +75,15 @@ __device__ __forceinline__ BinRegs bin_regs_init(const RenderParams &prm, uint32
     r.tp = prm.bin.tile_pixels; r.ntp = 0u - prm.bin.tile_pixels; r.magic = prm.bin.magic; r.mshift = prm.bin.mshift;
     r.nk = 1u << prm.bin.kbits; r.kmask = r.nk - 1u;
     r.sx = prm.sx; r.ox = prm.ox; r.sy = prm.sy; r.oy = prm.oy;
+    r.xmin = prm.xmin; r.xmax = prm.xmax; r.ymin = prm.ymin; r.ymax = prm.ymax;
     r.W = prm.W; r.Wm1 = prm.W - 1; r.Hm1 = prm.H - 1;
     return r;
+}
+
+// bounds rule of cfs_device.cuh in_bounds(), operands from registers
+__device__ __forceinline__ bool bin_in_bounds(const BinRegs &br, float x, float y)
+{
+    return (x >= br.xmin) && (x <= br.xmax) && (y >= br.ymin) && (y <= br.ymax);
 }
 
 // pixel rule of cfs_device.cuh pixel_of(), operands from registers

@@ -128,8 +128,8 @@ __device__ __forceinline__ uint32_t chain_and_splat(const RenderParams &prm, con
 // idle, so half of the splats are given to them (a direct splat costs ~5 instructions against ~16
 // for record + append, and pass 2 halves).  Any split is a correct result: HIST sums are exact,
 // RGBA sums are order-free (DESIGN R8).  Returns the number of dropped splats.
-template <bool HYBRID>
-__device__ __forceinline__ uint32_t bin_block_splat(const RenderParams &prm, const SharedTables &s, const BinRegs &br,
+template <bool HYBRID, bool RGBA>
+__device__ __forceinline__ uint32_t bin_block_splat(const RenderParams &prm, const SharedTables &s, const Sm &sm, const BinRegs &br,
                                                     const float (&X)[4], const float (&Y)[4], const int (&K)[4],
                                                     const bool (&ok)[4])
 {
@@ -139,8 +139,18 @@ __device__ __forceinline__ uint32_t bin_block_splat(const RenderParams &prm, con
     for (int j = 0; j < 4; ++j) {      // out-of-bounds coordinates are clamped by the pixel rule: always a valid tile
         const int pix = bin_pixel_of(br, X[j], Y[j]);
         over[j] = false;
-        if (HYBRID && (j & 1) == 0) {
-            if (ok[j]) bin_direct_pix(prm, s, (uint32_t)pix, (uint32_t)K[j]);
+        if (HYBRID && (j & 1) == 0) {  // straight to L2: one predicated reduction, no branch
+            if (RGBA) {
+                const float4 c = lds_v4(sm.tab + CFS_SM_OFF(palette) + 16u * (uint32_t)K[j]);
+                float *dst = reinterpret_cast<float *>(prm.image) + 4 * (size_t)(uint32_t)pix;
+                asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %4, 0;\n\t"
+                             "@p red.global.add.v4.f32 [%0], {%1, %2, %3, 0f3F800000};\n\t}"
+                             :: "l"(dst), "f"(c.x), "f"(c.y), "f"(c.z), "r"((uint32_t)ok[j]) : "memory");
+            } else {
+                uint32_t *dst = reinterpret_cast<uint32_t *>(prm.image) + (uint32_t)pix;
+                asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %1, 0;\n\t@p red.global.add.u32 [%0], 1;\n\t}"
+                             :: "l"(dst), "r"((uint32_t)ok[j]) : "memory");
+            }
         } else {
             bin_record_of(br, pix, K[j], tile[j], rec[j]);
             over[j] = bin_try_append(br, ok[j], tile[j], rec[j]);
@@ -185,10 +195,15 @@ __device__ __forceinline__ uint32_t iterate_block(const RenderParams &prm, const
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
             const bool alive = apply_chain<DIM, SIG, TRIG>(prm, X[j], Y[j], Z[j]);
-            ok[j] = alive && have && in_bounds(prm, X[j], Y[j]);
+            ok[j] = alive && have && bin_in_bounds(br, X[j], Y[j]);
         }
-        if (prm.bin.hybrid) dropped += bin_block_splat<true>(prm, s, br, X, Y, K, ok);    // warp-uniform
-        else                dropped += bin_block_splat<false>(prm, s, br, X, Y, K, ok);
+        // warp-uniform choice of one of four straight-line bodies (hybrid or pure bins, RGBA or HIST)
+        if (prm.bin.hybrid) {
+            if (prm.color_rule != 0) dropped += bin_block_splat<true, true>(prm, s, sm, br, X, Y, K, ok);
+            else                     dropped += bin_block_splat<true, false>(prm, s, sm, br, X, Y, K, ok);
+        } else {
+            dropped += bin_block_splat<false, false>(prm, s, sm, br, X, Y, K, ok);
+        }
     } else {
 #pragma unroll(CHECKED ? 1 : 4)
         for (int j = 0; j < 4; ++j) {
