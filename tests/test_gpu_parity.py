@@ -560,3 +560,59 @@ def test_cfg1_full_size_properties(cfs, oracle):
     assert np.array_equal(gsc, oc)
     for ch in range(4):
         assert density_l1(gs[:, ch], o[:, ch]) <= L1_TOL
+
+
+def test_cfg2_cfg3_cfg4_full_size_properties(cfs, oracle):
+    """The other BASELINE configs at full size, in the launch configuration bench.py's side report times
+    (AUTO with scratch + MUFU sin/cos): properties that hold at any size, and oracle parity on a sub-range
+    of the points rendered into the full-size image."""
+    # configs[2], middle frame: hybrid stage (tile bins + direct).  Exact conservation; identical to the
+    # direct variant under the same sin/cos evaluation (integer-valued sums below 2^24)
+    w = W.config(2)
+    t = w.frames[7]
+    S = w.render.n_points * 480
+    sysh = cfs.cfs_create(w.system)
+    need = cfs.cfs_binned_scratch_bytes(sysh, cfs.make_args(w.render))
+    sysh.close()
+    ga, gac = gpu_render(cfs, w, t=t, variant="auto", scratch_bytes=need, flags=["fast_trig"])
+    gd, gdc = gpu_render(cfs, w, t=t, variant="direct", flags=["fast_trig"])
+    assert int(gac[0]) == S and int(gac[1]) == 0 and ga[:, 3].astype(np.float64).sum() == S
+    assert ga[:, 3].max() < 2 ** 24 and np.array_equal(ga[:, 3], gd[:, 3]) and np.array_equal(gac, gdc)
+    small = gd[:, :3] < 2 ** 24          # hot pixels of the fractal exceed 2^24 in colour: there the order of
+    assert np.array_equal(ga[:, :3][small], gd[:, :3][small])          # the float32 additions shows (R8)
+    # beyond 2^24 every += 255 of the direct variant rounds (spacing 2, then 4): ~1e4 such additions drift by
+    # up to ~6e-4 relative, while the binned half adds n_k * palette[k] once per tile -- both are float32 sums
+    assert np.all(np.abs(ga[:, :3][~small] - gd[:, :3][~small]) <= 2e-3 * gd[:, :3][~small])
+    assert np.all(ga[np.abs(np.arange(ga.shape[0]) // 1920 - 539.5) > 0.8415 * 540 + 1, 3] == 0)   # |sin| <= sin 1
+    sub = w.scaled(n_points=1 << 14)
+    gs, gsc = gpu_render(cfs, sub, t=t, flags=["fast_trig"])
+    o, oc, _ = oracle.render_parallel(sub.system, sub.render, t=t)
+    assert np.array_equal(gsc, oc)
+    for ch in range(4):
+        assert density_l1(gs[:, ch], o[:, ch]) <= L1_TOL
+    # configs[3]: the whole 2^24-record cloud.  Every record is splatted or dropped; the alpha plane
+    # counts the splats and every colour sum is an integer (exact float32 sums below 2^24)
+    w = W.config(3)
+    cloud = W.gaussian_mixture_cloud(w.render.n_points, w.cloud_seed)
+    g, gc = gpu_render(cfs, w, cloud=cloud)
+    assert int(gc[0]) + int(gc[1]) == 1 << 24 and g[:, 3].astype(np.float64).sum() == int(gc[0])
+    assert g.max() < 2 ** 24 and np.all(g == np.round(g))
+    n_sub = 1 << 17
+    gs, gsc = gpu_render(cfs, w, cloud=cloud, n_points=n_sub)
+    o, oc, _ = oracle.render_parallel(w.system, w.render, cloud=cloud, n_points=n_sub)
+    assert abs(int(gsc[0]) - int(oc[0])) <= 4
+    for ch in range(4):
+        assert density_l1(gs[:, ch], o[:, ch]) <= L1_TOL
+    # configs[4]: min over all points <= min over any subset, with equality wherever the subset holds the
+    # winner; every key carries a depth in [3, 5] and one of the 20 palette entries
+    w = W.config(4)
+    g, gc = gpu_render(cfs, w)
+    assert int(gc[0]) == (1 << 26) * 980 and int(gc[1]) == 0
+    sub = w.scaled(n_points=1 << 12)
+    o, _, _ = oracle.render_parallel(sub.system, sub.render)
+    assert np.all(g <= o)
+    hit = g != np.uint64(0xFFFFFFFFFFFFFFFF)
+    depth = (g[hit] >> np.uint64(32)).astype(np.uint32).view(np.float32)
+    assert hit.sum() > 1_000_000 and depth.min() >= 3.0 - 1e-6 and depth.max() <= 5.0 + 1e-6
+    pal8 = set(int(v) for v in (g[hit] & np.uint64(0xFFFFFFFF)).astype(np.uint32)[:: 997])
+    assert len(pal8) <= 20
