@@ -311,9 +311,42 @@ static int validate(const orc_system *s, const orc_render_args *a)
     else if (a->out_mode == ORC_OUT_RGBA) { if (s->color_rule == ORC_COLOR_NONE) return -1; }
     else if (a->out_mode == ORC_OUT_DEPTH_U64) {
         if (s->color_rule == ORC_COLOR_NONE || s->dim != 3) return -1;
-        if (s->n_chain < 1 || s->chain[s->n_chain - 1].type != ORC_T_PINHOLE) return -1;
+        if (s->n_chain < 1) return -1;
+        for (int m = 0; m <= s->n_chain; ++m)        /* every branch ends in PINHOLE */
+            if ((m == s->n_chain || s->chain[m].type == ORC_T_BRANCH) && (m == 0 || s->chain[m - 1].type != ORC_T_PINHOLE)) return -1;
     } else return -1;
     return 0;
+}
+
+/* ---------------------------------------------------------------- S7 + S8: one splat */
+static void splat_one(const orc_system *s, const orc_render_args *a, const pixmap *pm, const float q[3], int alive,
+                      int k, uint32_t point_rgba8, uint64_t *n_in, uint64_t *n_drop)
+{
+    int64_t pix = alive ? pixel_of(pm, q[0], q[1], a->xmin, a->xmax, a->ymin, a->ymax, a->width, a->height) : -1;
+    if (pix < 0) { ++*n_drop; return; }
+    ++*n_in;
+    if (a->out_mode == ORC_OUT_HIST_U32) {
+        ((uint32_t *)a->image)[pix] += 1u;
+    } else if (a->out_mode == ORC_OUT_RGBA) {
+        double *acc = (double *)a->image + 4 * pix;
+        if (s->color_rule == ORC_COLOR_MAP_INDEX) {
+            const float *c = s->palette + 4 * k;
+            acc[0] += (double)c[0]; acc[1] += (double)c[1]; acc[2] += (double)c[2];
+        } else {
+            acc[0] += (double)(point_rgba8 & 0xFFu);
+            acc[1] += (double)((point_rgba8 >> 8) & 0xFFu);
+            acc[2] += (double)((point_rgba8 >> 16) & 0xFFu);
+        }
+        acc[3] += 1.0;
+    } else {
+        /* BJ cfg 4: nearest-point depth test via packed (float depth | rgba8) min */
+        uint32_t col = (s->color_rule == ORC_COLOR_MAP_INDEX) ? pack_rgba8(s->palette + 4 * k) : point_rgba8;
+        uint32_t dbits;
+        memcpy(&dbits, &q[2], 4);
+        uint64_t key = ((uint64_t)dbits << 32) | col;
+        uint64_t *buf = (uint64_t *)a->image + pix;
+        if (key < *buf) *buf = key;
+    }
 }
 
 /* ---------------------------------------------------------------- S1: the loop */
@@ -333,7 +366,12 @@ static int run(const orc_system *s, const orc_render_args *a, int do_splat, uint
     int ctype[8];
     float cprm[8][12];
     for (int m = 0; m < s->n_chain; ++m) {
-        if (s->chain[m].type < 0 || s->chain[m].type > ORC_T_STRETCH_COS) return -1;
+        if (s->chain[m].type < 0 || s->chain[m].type > ORC_T_BRANCH) return -1;
+        if (s->chain[m].type == ORC_T_BRANCH) {
+            if (s->reuse) return -1;              /* which branch would be fed back? */
+            ctype[m] = ORC_T_BRANCH;
+            continue;
+        }
         orc_resolve_xform(&s->chain[m], s->dim, a->t, a->width, a->height, &ctype[m], cprm[m]);
     }
     pixmap pm = make_pixmap(a->xmin, a->xmax, a->ymin, a->ymax, a->width, a->height);
@@ -359,42 +397,22 @@ static int run(const orc_system *s, const orc_render_args *a, int do_splat, uint
                 orc_apply_func(&s->funcs[k], s->dim, g);
             }
             if (it < a->burn_in && !s->reuse) continue;
-            /* PAPER L77 / Fig. 2(B): a copy of the point goes through the chain */
-            q[0] = g[0]; q[1] = g[1]; q[2] = g[2];
-            alive = 1;
-            for (int m = 0; m < s->n_chain && alive; ++m)
-                alive = orc_apply_xform(ctype[m], cprm[m], s->dim, q);
-            if (s->reuse) {                       /* Fig. 2(C): the same point is reused */
-                g[0] = q[0]; g[1] = q[1]; g[2] = q[2];
-                if (it < a->burn_in) continue;
-            }
-            if (!do_splat) continue;
-            int64_t pix = alive ? pixel_of(&pm, q[0], q[1], a->xmin, a->xmax, a->ymin, a->ymax,
-                                           a->width, a->height) : -1;
-            if (pix < 0) { ++n_drop; continue; }
-            ++n_in;
-            if (a->out_mode == ORC_OUT_HIST_U32) {
-                ((uint32_t *)a->image)[pix] += 1u;
-            } else if (a->out_mode == ORC_OUT_RGBA) {
-                double *acc = (double *)a->image + 4 * pix;
-                if (s->color_rule == ORC_COLOR_MAP_INDEX) {
-                    const float *c = s->palette + 4 * k;
-                    acc[0] += (double)c[0]; acc[1] += (double)c[1]; acc[2] += (double)c[2];
-                } else {
-                    acc[0] += (double)(point_rgba8 & 0xFFu);
-                    acc[1] += (double)((point_rgba8 >> 8) & 0xFFu);
-                    acc[2] += (double)((point_rgba8 >> 16) & 0xFFu);
+            /* PAPER L77 / Fig. 2(B): a copy of the point goes through the chain.  PAPER L192-198 ("many
+             * objects from a single primitive"): a chain may hold several BRANCHes; each is applied to its
+             * own copy of the generated point and splatted, so one point drives M splats per iteration. */
+            for (int m0 = 0; m0 <= s->n_chain; ) {
+                q[0] = g[0]; q[1] = g[1]; q[2] = g[2];
+                alive = 1;
+                int m = m0;
+                for (; m < s->n_chain && ctype[m] != ORC_T_BRANCH; ++m)
+                    if (alive) alive = orc_apply_xform(ctype[m], cprm[m], s->dim, q);
+                m0 = m + 1;                       /* past the BRANCH marker (or past the end) */
+                if (s->reuse) {                   /* Fig. 2(C): the same point is reused (single branch) */
+                    g[0] = q[0]; g[1] = q[1]; g[2] = q[2];
+                    if (it < a->burn_in) continue;
                 }
-                acc[3] += 1.0;
-            } else {
-                /* BJ cfg 4: nearest-point depth test via packed (float depth | rgba8) min */
-                uint32_t col = (s->color_rule == ORC_COLOR_MAP_INDEX) ? pack_rgba8(s->palette + 4 * k)
-                                                                      : point_rgba8;
-                uint32_t dbits;
-                memcpy(&dbits, &q[2], 4);
-                uint64_t key = ((uint64_t)dbits << 32) | col;
-                uint64_t *buf = (uint64_t *)a->image + pix;
-                if (key < *buf) *buf = key;
+                if (!do_splat) continue;
+                splat_one(s, a, &pm, q, alive, k, point_rgba8, &n_in, &n_drop);
             }
         }
         if (final_g) { final_g[3 * i] = g[0]; final_g[3 * i + 1] = g[1]; final_g[3 * i + 2] = g[2]; }

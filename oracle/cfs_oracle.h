@@ -35,7 +35,8 @@ enum { ORC_GEN_IFS = 0, ORC_GEN_CLOUD = 1 };
 enum { ORC_F_AFFINE = 0, ORC_F_CIRCLE_HALF = 1 };
 enum {
     ORC_T_AFFINE = 0, ORC_T_SWIRL = 1, ORC_T_SINUSOIDAL = 2, ORC_T_ROTATE_Z = 3,
-    ORC_T_TWIST_Z = 4, ORC_T_BEND = 5, ORC_T_PINHOLE = 6, ORC_T_STRETCH_COS = 7
+    ORC_T_TWIST_Z = 4, ORC_T_BEND = 5, ORC_T_PINHOLE = 6, ORC_T_STRETCH_COS = 7,
+    ORC_T_BRANCH = 8   /* not a transform: ends one branch of the chain and starts the next */
 };
 enum { ORC_COLOR_NONE = 0, ORC_COLOR_MAP_INDEX = 1, ORC_COLOR_POINT = 2 };
 enum { ORC_OUT_HIST_U32 = 0, ORC_OUT_RGBA = 1, ORC_OUT_DEPTH_U64 = 2 };

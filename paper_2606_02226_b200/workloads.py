@@ -30,7 +30,7 @@ class Func:
 
 @dataclass
 class Xform:
-    type: str            # affine|swirl|sinusoidal|rotate_z|twist_z|bend|pinhole|stretch_cos
+    type: str            # affine|swirl|sinusoidal|rotate_z|twist_z|bend|pinhole|stretch_cos|branch (separator)
     p0: Sequence[float] = ()
     p1: Sequence[float] = ()
 

@@ -373,3 +373,57 @@ def test_tonemap_closed_forms(oracle):
     buf[2] = (np.uint64(0x40800000) << np.uint64(32)) | np.uint64(0xFF112233)
     out = oracle.tonemap(buf, "depth_u64", 2, 2, 2.2, 1.0)
     assert list(out) == [0, 0, 0xFF112233, 0]
+
+
+# ------------------------------------------------------------------ NEXT-2: one-to-many splatting
+def _branches():
+    a = [W.Xform("affine", [0.5, 0, 0, 0.5, -0.4, 0.3])]
+    b = [W.Xform("swirl"), W.Xform("affine", [0.6, 0, 0, 0.6, 0.3, -0.2])]
+    c = []                                                   # the generated point itself
+    return [a, b, c]
+
+
+def _join(branches):
+    out = []
+    for i, br in enumerate(branches):
+        if i:
+            out.append(W.Xform("branch"))
+        out.extend(br)
+    return out
+
+
+@pytest.mark.parametrize("mode", ["hist_u32", "rgba_f32"])
+def test_branches_equal_the_sum_of_single_chain_renders(oracle, mode):
+    """"Many objects from a single primitive": every BRANCH of the chain gets its own
+    copy of the generated point.  The generator never sees the chain (Fig. 2(B)), so the M-branch image is
+    EXACTLY the sum of the M single-chain images -- which reduces this path to the pinned single-chain one.
+    Splats per point = M (I - B)."""
+    brs = _branches()
+    rule, pal = ("none", None) if mode == "hist_u32" else ("map_index", W.palette_for(4))
+    r = W.Render(3000, 5, 60, 10, 128, 128, (-1, 1, -1, 1), mode)
+    multi, mc = oracle.render(W.System(2, "ifs", W.square_funcs(), _join(brs), rule, pal), r)
+    total, n_in, n_drop = None, 0, 0
+    for br in brs:
+        img, c = oracle.render(W.System(2, "ifs", W.square_funcs(), br, rule, pal), r)
+        total = img.copy() if total is None else total + img
+        n_in += int(c[0]); n_drop += int(c[1])
+    assert np.array_equal(multi, total)
+    assert int(mc[0]) == n_in and int(mc[1]) == n_drop and n_in + n_drop == 3 * 3000 * 50
+    # a trailing BRANCH opens one more (empty) branch: the generated point itself
+    again, ac = oracle.render(W.System(2, "ifs", W.square_funcs(), _join(brs[:2]) + [W.Xform("branch")], rule, pal), r)
+    assert np.array_equal(again, multi) and np.array_equal(ac, mc)
+
+
+def test_branches_depth_is_the_min_of_single_chain_renders(oracle):
+    pin = W.Xform("pinhole", [60.0, -4.0, 1e-3])
+    brs = [[pin], [W.Xform("affine", [0.5, 0, 0, 0, 0.5, 0, 0, 0, 0.5, 0.3, 0.2, -1.0]), pin]]
+    r = W.Render(2000, 9, 50, 10, 160, 90, (-1, 1, -1, 1), "depth_u64")
+    pal = W.palette_for(20)
+    multi, mc = oracle.render(W.System(3, "ifs", W.menger_funcs(), _join(brs), "map_index", pal), r)
+    singles = [oracle.render(W.System(3, "ifs", W.menger_funcs(), br, "map_index", pal), r)[0] for br in brs]
+    assert np.array_equal(multi, np.minimum(singles[0], singles[1])) and int(mc[0]) + int(mc[1]) == 2 * 2000 * 40
+    with pytest.raises(ValueError):            # a branch that does not end in PINHOLE cannot feed a depth buffer
+        oracle.render(W.System(3, "ifs", W.menger_funcs(), _join([[pin], []]), "map_index", pal), r)
+    with pytest.raises(ValueError):            # reuse (Fig. 2(C)) has no meaning with several branches
+        oracle.render(W.System(2, "ifs", W.square_funcs(), _join(_branches()), "none", None, reuse=True),
+                      W.Render(10, 1, 20, 5, 32, 32, (-1, 1, -1, 1), "hist_u32"))
