@@ -70,10 +70,15 @@ typedef struct { int32_t type; float prob; float params[12]; } cfs_func;
  *   BEND        (x,y) rotated by p[0]*x (input x)                         (DESIGN R6)
  *   PINHOLE     p = (fov_y degrees, cam_z, near): d = z-cam_z; dropped unless d > near;
  *               x' = (fx*x)*(1/d), y' = (fy*y)*(1/d), z' = d; fy = 1/tan(fov/2), fx = fy*H/W
- *   STRETCH_COS x' = 2x, y' = y - cos x                                   (PAPER Eq. 2) */
+ *   STRETCH_COS x' = 2x, y' = y - cos x                                   (PAPER Eq. 2)
+ *   BRANCH      not a transform: ends one branch of the chain and starts the next.  Every branch is applied
+ *               to its own copy of the generated point and splatted, so a point drives M splats per iteration
+ *               ("many objects from a single primitive"); the image equals the sum (DEPTH: the
+ *               min) of the M single-chain renders.  Not with reuse; DEPTH needs every branch to end in PINHOLE.
+ *               Runs on the chain interpreter; cfs_trace does not serve it. */
 typedef enum {
     CFS_T_AFFINE = 0, CFS_T_SWIRL = 1, CFS_T_SINUSOIDAL = 2, CFS_T_ROTATE_Z = 3,
-    CFS_T_TWIST_Z = 4, CFS_T_BEND = 5, CFS_T_PINHOLE = 6, CFS_T_STRETCH_COS = 7
+    CFS_T_TWIST_Z = 4, CFS_T_BEND = 5, CFS_T_PINHOLE = 6, CFS_T_STRETCH_COS = 7, CFS_T_BRANCH = 8
 } cfs_xform_type;
 typedef struct { int32_t type; float p0[12]; float p1[12]; } cfs_xform;
 

@@ -215,7 +215,8 @@ extern "C" cfs_status cfs_create(cfs_system **out, int32_t dim, int32_t gen_kind
         if (color_rule == CFS_COLOR_MAP_INDEX) st = fail(CFS_ERR_INVALID_ARG, "COLOR_MAP_INDEX needs an IFS generator");
     }
     for (int m = 0; st == CFS_OK && m < n_chain; ++m) {
-        if (chain[m].type < CFS_T_AFFINE || chain[m].type > CFS_T_STRETCH_COS) st = fail(CFS_ERR_INVALID_ARG, "chain[%d]: unknown type %d", m, chain[m].type);
+        if (chain[m].type < CFS_T_AFFINE || chain[m].type > CFS_T_BRANCH) st = fail(CFS_ERR_INVALID_ARG, "chain[%d]: unknown type %d", m, chain[m].type);
+        if (st == CFS_OK && chain[m].type == CFS_T_BRANCH && reuse) st = fail(CFS_ERR_INVALID_ARG, "chain[%d]: BRANCH cannot be combined with reuse", m);
         for (int i = 0; st == CFS_OK && i < 12; ++i)
             if (bad_float(chain[m].p0[i]) || bad_float(chain[m].p1[i])) st = fail(CFS_ERR_INVALID_ARG, "chain[%d] parameter %d is not finite", m, i);
     }
@@ -256,7 +257,10 @@ cfs_status build_params(const cfs_system *s, const cfs_render_args *a, RenderPar
     if (a->out_mode == CFS_OUT_RGBA_F32 && s->color == CFS_COLOR_NONE) return fail(CFS_ERR_INVALID_ARG, "RGBA output needs a colour rule");
     if (a->out_mode == CFS_OUT_DEPTH_RGBA8_U64) {
         if (s->color == CFS_COLOR_NONE || s->dim != 3) return fail(CFS_ERR_INVALID_ARG, "DEPTH output needs dim 3 and a colour rule");
-        if (s->chain.empty() || s->chain.back().type != CFS_T_PINHOLE) return fail(CFS_ERR_INVALID_ARG, "DEPTH output needs a chain ending in PINHOLE");
+        if (s->chain.empty()) return fail(CFS_ERR_INVALID_ARG, "DEPTH output needs a chain ending in PINHOLE");
+        for (size_t m = 0; m <= s->chain.size(); ++m)       // every branch ends in PINHOLE
+            if ((m == s->chain.size() || s->chain[m].type == CFS_T_BRANCH) && (m == 0 || s->chain[m - 1].type != CFS_T_PINHOLE))
+                return fail(CFS_ERR_INVALID_ARG, "DEPTH output needs every branch of the chain to end in PINHOLE");
     }
     if (need_image && a->n_points && !a->d_image) return fail(CFS_ERR_INVALID_ARG, "d_image is NULL");
     if (a->n_points && s->gen == CFS_GEN_CLOUD && !a->d_cloud) return fail(CFS_ERR_INVALID_ARG, "d_cloud is NULL");
@@ -293,6 +297,8 @@ cfs_status build_params(const cfs_system *s, const cfs_render_args *a, RenderPar
 
     // chain parameters at t: (float)((double)p0 + (double)t*(double)p1)
     const double t = (double)a->t;
+    p.n_branches = 1;
+    for (int m = 0; m < p.n_chain; ++m) if (s->chain[m].type == CFS_T_BRANCH) ++p.n_branches;
     for (int m = 0; m < p.n_chain; ++m) {
         const cfs_xform &x = s->chain[m];
         cfs::ChainStep &st = p.chain[m];
@@ -351,7 +357,7 @@ uint32_t chain_signature(const RenderParams &p)
 render_fn pick_kernel(const cfs_system *s, const RenderParams &p, int splat, int flags)
 {
     const int trig = (flags & CFS_FLAG_FAST_TRIG) ? cfs::TRIG_FAST : cfs::TRIG_ACCURATE;
-    if (!(flags & CFS_FLAG_INTERPRET_CHAIN) && p.n_chain > 0 && !p.reuse) {
+    if (!(flags & CFS_FLAG_INTERPRET_CHAIN) && p.n_chain > 0 && !p.reuse && p.n_branches == 1) {
         const uint32_t sig = chain_signature(p);
         render_fn fn = (s->dim == 2) ? cfs::lookup_render_static2d(s->gen, s->aff, splat, sig, trig)
                                      : cfs::lookup_render_static3d(s->gen, s->aff, splat, sig, trig);
@@ -363,7 +369,7 @@ render_fn pick_kernel(const cfs_system *s, const RenderParams &p, int splat, int
 render_fn pick_trace(const cfs_system *s, const RenderParams &p, int flags)
 {
     const int trig = (flags & CFS_FLAG_FAST_TRIG) ? cfs::TRIG_FAST : cfs::TRIG_ACCURATE;
-    if (!(flags & CFS_FLAG_INTERPRET_CHAIN) && p.n_chain > 0 && !p.reuse) {
+    if (!(flags & CFS_FLAG_INTERPRET_CHAIN) && p.n_chain > 0 && !p.reuse && p.n_branches == 1) {
         const uint32_t sig = chain_signature(p);
         render_fn fn = (s->dim == 2) ? cfs::lookup_trace_static2d(s->gen, s->aff, sig, trig)
                                      : cfs::lookup_trace_static3d(s->gen, s->aff, sig, trig);
@@ -379,6 +385,14 @@ size_t shared_hist_limit(const DeviceInfo &di)
 }
 
 }  // namespace
+
+// splats one generated point drives per iteration past burn-in: 1 + BRANCH markers of the chain
+static uint64_t branches_of(const cfs_system *s)
+{
+    uint64_t n = 1;
+    for (const cfs_xform &x : s->chain) if (x.type == CFS_T_BRANCH) ++n;
+    return n;
+}
 
 // ---- tile-binned variant: plan (tiles, staging rows, scratch layout, chunking) -------------------
 namespace {
@@ -544,7 +558,7 @@ extern "C" uint64_t cfs_binned_scratch_bytes(const cfs_system *s, const cfs_rend
     BinPlan pl;
     const char *why = "";
     if (!bin_shape(s, a, di, &pl, &why)) return 0;
-    return bin_scratch_for(pl, a->n_points, (uint64_t)(a->iterations - a->burn_in));
+    return bin_scratch_for(pl, a->n_points, (uint64_t)(a->iterations - a->burn_in) * branches_of(s));
 }
 
 extern "C" uint64_t cfs_shared_hist_max_bytes(void)
@@ -606,7 +620,7 @@ cfs_status render_binned(const cfs_system *s, const cfs_render_args *a, RenderPa
     const char *why = "";
     if (!bin_shape(s, a, di, &pl, &why)) return fail(CFS_ERR_UNSUPPORTED, "%s", why);
     if (!a->d_scratch) return fail(CFS_ERR_UNSUPPORTED, "binned variant needs d_scratch (see cfs_binned_scratch_bytes)");
-    const uint64_t spp = (uint64_t)(a->iterations - a->burn_in);
+    const uint64_t spp = (uint64_t)(a->iterations - a->burn_in) * branches_of(s);
     if (!bin_layout(&pl, a->d_scratch, a->scratch_bytes, a->n_points, spp, &why)) return fail(CFS_ERR_UNSUPPORTED, "%s", why);
     render_fn fn1 = pick_kernel(s, p, cfs::SPLAT_BIN, a->flags);
     if (!fn1) return fail(CFS_ERR_UNSUPPORTED, "no binned kernel for dim %d", s->dim);
@@ -692,7 +706,7 @@ cfs_status render_depth_hiz(const cfs_system *s, const cfs_render_args *a, Rende
     // the map's padding entries are read into shared memory but never indexed; clear them once
     if ((e = cudaMemsetAsync(hz, 0xFF, dyn, st)) != cudaSuccess) return cuda_fail(e, "clear Hi-Z map");
 
-    const uint64_t P = a->n_points, spp = (uint64_t)(a->iterations - a->burn_in);
+    const uint64_t P = a->n_points, spp = (uint64_t)(a->iterations - a->burn_in) * branches_of(s);
     uint64_t n0 = (64ull * (uint64_t)a->width * (uint64_t)a->height + spp - 1) / spp;
     n0 = (n0 + cfs::kHizThreads - 1) / cfs::kHizThreads * cfs::kHizThreads;
     const uint64_t cuts[4] = {0, n0 < P ? n0 : P, 8 * n0 < P ? 8 * n0 : P, P};
@@ -729,7 +743,7 @@ extern "C" cfs_status cfs_render(const cfs_system *s, const cfs_render_args *a, 
     const DeviceInfo &di = device_info();
     if (di.ok != 1) return fail(CFS_ERR_CUDA, "no CUDA device (this library has no CPU fallback)");
     const size_t hist_bytes = (size_t)a->width * a->height * 4;
-    const uint64_t n_splats = a->n_points * (uint64_t)(a->iterations - a->burn_in);
+    const uint64_t n_splats = a->n_points * (uint64_t)(a->iterations - a->burn_in) * branches_of(s);
     int splat;
     if (a->out_mode == CFS_OUT_RGBA_F32) splat = cfs::SPLAT_RGBA;
     else if (a->out_mode == CFS_OUT_DEPTH_RGBA8_U64) splat = cfs::SPLAT_DEPTH;
@@ -811,6 +825,7 @@ extern "C" cfs_status cfs_trace(const cfs_system *s, const cfs_render_args *a, u
     if (st != CFS_OK) return st;
     if (device_info().ok != 1) return fail(CFS_ERR_CUDA, "no CUDA device (this library has no CPU fallback)");
     if (a->n_points == 0) return CFS_OK;
+    if (p.n_branches > 1) return fail(CFS_ERR_UNSUPPORTED, "cfs_trace does not serve chains with BRANCH markers");
     p.tr_picks = d_picks; p.tr_g = d_final_g; p.tr_q = d_final_q; p.tr_alive = d_alive;
     p.counters = nullptr;
     render_fn fn = pick_trace(s, p, a->flags);

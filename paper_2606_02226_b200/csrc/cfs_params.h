@@ -116,6 +116,7 @@ struct RenderParams {
     uint8_t *tr_alive;
 
     int32_t dim, n_funcs, n_chain, color_rule, reuse, fast_trig;
+    int32_t n_branches;          // 1 + BRANCH markers in the chain: splats per generated point and iteration
     int32_t pick_shift;          // >= 0: k = u >> pick_shift (equal power-of-two thresholds)
     int32_t n_thr;               // thresholds below 2^32 (k = #{j < n_thr : u >= T[j]})
     int32_t pick_steps;          // max thresholds inside one 2^24 bucket of u

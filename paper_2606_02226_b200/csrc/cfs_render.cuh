@@ -62,6 +62,11 @@ __device__ __forceinline__ void splat_depth(unsigned long long *buf, int pix, fl
     if (key < cur) atomicMin(buf + pix, key);
 }
 
+template <int DIM, int GEN, int SPLAT>
+__device__ __forceinline__ uint32_t splat_q(const RenderParams &prm, const SharedTables &s, const Sm &sm, uint32_t *s_hist,
+                                            float qx, float qy, float qz, bool alive, int k, uint32_t point_rgba8,
+                                            bool have, const BinRegs &br);
+
 // rows 5-7 for one generated point: copy -> chain -> pixel -> reduction.  `k` is the map applied
 // in this iteration (colour rule MAP_INDEX), `point_rgba8` the record colour (POINT).
 // Returns 1 when the splat was dropped (dead or out of bounds), else 0.  Fig. 2(C) reuse is a
@@ -71,12 +76,38 @@ __device__ __forceinline__ uint32_t chain_and_splat(const RenderParams &prm, con
                                                     float &gx, float &gy, float &gz, int k, uint32_t point_rgba8,
                                                     bool have, bool past_burn_in, const BinRegs &br)
 {
+    if (SIG == kChainGeneric && prm.n_branches > 1) {
+        // one-to-many ("many objects from a single primitive"): every BRANCH of the chain
+        // gets its own copy of the generated point and its own splat.  The markers sit in the parameter
+        // block, so the loop structure is warp-uniform; only dead lanes skip steps.
+        float qx = gx, qy = gy, qz = gz;
+        bool alive = true;
+        uint32_t dropped = 0u;
+        for (int m = 0; m <= prm.n_chain; ++m) {
+            if (m == prm.n_chain || prm.chain[m].type == T_BRANCH) {
+                dropped += splat_q<DIM, GEN, SPLAT>(prm, s, sm, s_hist, qx, qy, qz, alive, k, point_rgba8, have, br);
+                qx = gx; qy = gy; qz = gz; alive = true;
+            } else if (alive) {
+                alive = chain_step_dyn<DIM, TRIG>(prm, prm.chain[m], qx, qy, qz);
+            }
+        }
+        return dropped;
+    }
     float qx = gx, qy = gy, qz = gz;            // the copy of Fig. 2(B)
     const bool alive = apply_chain<DIM, SIG, TRIG>(prm, qx, qy, qz);
     if (SIG == kChainGeneric && prm.reuse) {    // Fig. 2(C): the same point is reused
         gx = qx; gy = qy; gz = qz;
         if (!past_burn_in) return 0u;
     }
+    return splat_q<DIM, GEN, SPLAT>(prm, s, sm, s_hist, qx, qy, qz, alive, k, point_rgba8, have, br);
+}
+
+// rows 6-7 for one chain output: bounds -> pixel -> reduction.  Returns 1 when the splat was dropped.
+template <int DIM, int GEN, int SPLAT>
+__device__ __forceinline__ uint32_t splat_q(const RenderParams &prm, const SharedTables &s, const Sm &sm, uint32_t *s_hist,
+                                            float qx, float qy, float qz, bool alive, int k, uint32_t point_rgba8,
+                                            bool have, const BinRegs &br)
+{
     const bool ok = alive && have && in_bounds(prm, qx, qy);
     if (SPLAT == SPLAT_HIST_WARPAGG) {
         splat_hist_warpagg(reinterpret_cast<uint32_t *>(prm.image), ok ? pixel_of(prm, qx, qy) : -1, ok);
@@ -305,7 +336,7 @@ render_kernel(const __grid_constant__ RenderParams prm)
             for (; it0 < I; it0 += 4)
                 dropped += iterate_block<DIM, GEN, AFF, SPLAT, SIG, TRIG, true>(prm, s, sm, s_hist, plo, phi, it0, gx, gy, gz, have, bl, br);
         }
-        if (have) { n_drop += dropped; n_in += (uint32_t)(I - B) - dropped; }
+        if (have) { n_drop += dropped; n_in += (uint32_t)(I - B) * (uint32_t)prm.n_branches - dropped; }
     }
 
     if (SPLAT == SPLAT_BIN) {           // write out what is left in the staging rows

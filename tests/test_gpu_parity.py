@@ -418,6 +418,63 @@ def test_eq1_generator_validation(cfs):
     assert ei.value.status == cfs.CFS_ERR_INVALID_ARG
 
 
+def test_branches_one_to_many(cfs, oracle):
+    """NEXT-2: a chain with BRANCH markers splats every generated point once per branch.
+    HIST: identical per pixel to the oracle and to the sum of the single-chain GPU renders, in every
+    variant; RGBA within the density bar; DEPTH = min of the single-chain renders, bit-exact."""
+    a = [W.Xform("affine", [0.5, 0, 0, 0.5, -0.4, 0.3])]
+    b = [W.Xform("affine", [0.3, 0.1, -0.1, 0.3, 0.3, -0.5])]
+    c = []
+    sw = [W.Xform("swirl"), W.Xform("affine", [0.6, 0, 0, 0.6, 0.3, -0.2])]
+    def join(brs):
+        out = []
+        for i, br in enumerate(brs):
+            out += ([W.Xform("branch")] if i else []) + br
+        return out
+    r = W.Render(6000 + 5, 5, 80, 10, 200, 160, (-1, 1, -1, 0.9), "hist_u32")
+    multi = W.Workload("m", W.System(2, "ifs", W.square_funcs(), join([a, b, c]), "none"), r)
+    o, oc = oracle.render(multi.system, r)
+    assert int(oc[0]) + int(oc[1]) == 3 * 6005 * 70 and int(oc[1]) > 0
+    total = None
+    for br in (a, b, c):
+        g1, _ = gpu_render(cfs, W.Workload("s", W.System(2, "ifs", W.square_funcs(), br, "none"), r), variant="direct")
+        total = g1 if total is None else total + g1
+    for variant, flags in (("direct", 0), ("auto", 0), ("shared_hist", 0), ("warp_agg", 0), ("binned", 0), ("binned", ["bin_hybrid"])):
+        if variant == "shared_hist":
+            continue                                    # 200 x 160 u32 does fit: exercised just below
+        g, gc = gpu_render(cfs, multi, variant=variant, flags=flags)
+        assert np.array_equal(g, o) and np.array_equal(gc, oc) and np.array_equal(g, total), variant
+    g, gc = gpu_render(cfs, multi, variant="shared_hist")
+    assert np.array_equal(g, o) and np.array_equal(gc, oc)
+    # RGBA + a non-affine branch
+    r2 = W.Render(20000, 6, 60, 10, 256, 256, (-1.2, 1.2, -1.2, 1.2), "rgba_f32")
+    m2 = W.Workload("m2", W.System(2, "ifs", W.square_funcs(), join([sw, a]), "map_index", W.palette_for(4)), r2)
+    o2, oc2 = oracle.render(m2.system, r2)
+    for variant in ("direct", "binned"):
+        g2, gc2 = gpu_render(cfs, m2, variant=variant)
+        assert int(gc2[0]) + int(gc2[1]) == 2 * 20000 * 50 and abs(int(gc2[0]) - int(oc2[0])) <= 4
+        for ch in range(4):
+            assert density_l1(g2[:, ch], o2[:, ch]) <= L1_TOL
+    # DEPTH: two objects from one Menger primitive
+    pin = W.Xform("pinhole", [60.0, -4.0, 1e-3])
+    small = [W.Xform("affine", [0.5, 0, 0, 0, 0.5, 0, 0, 0, 0.5, 0.3, 0.2, -1.0]), pin]
+    r3 = W.Render(3000, 9, 60, 10, 320, 180, (-1, 1, -1, 1), "depth_u64")
+    m3 = W.Workload("m3", W.System(3, "ifs", W.menger_funcs(), join([[pin], small]), "map_index", W.palette_for(20)), r3)
+    o3, oc3 = oracle.render(m3.system, r3)
+    g3, gc3 = gpu_render(cfs, m3)
+    assert np.array_equal(g3, o3) and np.array_equal(gc3, oc3)
+    # refused: reuse with branches, a depth branch without PINHOLE, cfs_trace
+    with pytest.raises(cfs.CfsError) as ei:
+        cfs.cfs_create(W.System(2, "ifs", W.square_funcs(), join([a, b]), "none", None, reuse=True))
+    assert ei.value.status == cfs.CFS_ERR_INVALID_ARG
+    with pytest.raises(cfs.CfsError) as ei:
+        gpu_render(cfs, W.Workload("bad", W.System(3, "ifs", W.menger_funcs(), join([[pin], []]), "map_index", W.palette_for(20)), r3))
+    assert ei.value.status == cfs.CFS_ERR_INVALID_ARG
+    with pytest.raises(cfs.CfsError) as ei:
+        gpu_trace(cfs, multi)
+    assert ei.value.status == cfs.CFS_ERR_UNSUPPORTED
+
+
 def test_empty_and_accumulate(cfs, oracle):
     import torch
     w = W.config(0).scaled(n_points=0)
