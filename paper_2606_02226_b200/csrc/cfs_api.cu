@@ -468,8 +468,21 @@ bool bin_shape_raw(int gen, int out_mode, int color, uint32_t n_funcs, int32_t w
     uint32_t every = 64;
     while (every > 4 && 2.0 * every * per_it + 16.0 > room) every >>= 1;
     b.check_mask = every / 4 - 1;                      // in Philox blocks of 4 iterations
-    b.split = (uint32_t)((4 * (uint64_t)di.sms + n_tiles - 1) / n_tiles);
-    if (b.split < 1) b.split = 1;
+    // pass 2 runs one CTA per SM (the tile fills shared memory) in waves of `sms` CTAs: among the splits
+    // that give 2.5 to 8 waves take the one whose last wave is fullest (configs[1]: 86 tiles x 7 = 4.07 waves
+    // ran as 5; x 5 = 2.9 waves runs as 3)
+    {
+        uint32_t best = 1;
+        double best_eff = 0.0;
+        for (uint32_t sp = 1; sp <= 64; ++sp) {
+            const double waves = (double)(n_tiles * sp) / (double)di.sms;
+            if (waves < 2.5 && sp < 64) continue;
+            const double eff = waves / std::ceil(waves);
+            if (eff > best_eff + 1e-9) { best_eff = eff; best = sp; }
+            if (waves >= 8.0) break;
+        }
+        b.split = best;
+    }
     pl->smem_pass1 = (n_tiles + cfs::kBinDummy + 3) / 4 * 4 * 4 + n_tiles * (size_t)cap * 2;
     pl->smem_pass2 = ((size_t)b.tile_pixels << kbits) * 4;
     pl->grid1 = (uint32_t)di.sms * cfs::kBinCtasPerSm;
