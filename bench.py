@@ -262,6 +262,9 @@ N_INSTR_BIN = {0: 38, 1: 51, 2: 51}
 # hybrid (CFS_FLAG_BIN_HYBRID, what AUTO runs): every other splat skips the 6 record + 4 append operations and
 # pays a palette LDS + one red.global instead, i.e. 43 on those iterations: (51 + 43) / 2
 N_INSTR_HYB = {1: 47, 2: 47}
+# with sincosf (--accurate-trig): the direct count of N_INSTR on direct iterations, + 8 (6 record + 4 append - 2) on binned ones
+N_INSTR_HYB_ACC = {1: 66, 2: 70}
+N_INSTR_BIN_ACC = {0: 38, 1: 70, 2: 74}
 RED_KEY = {0: "red_add_u32@1048576", 1: "red_add_v4f32@16777216", 2: "red_add_v4f32@33177600",
            3: "red_add_v4f32@132710400", 4: "atom_min_u64@66355200"}
 
@@ -458,7 +461,10 @@ def run_ours(args):
     if binned:
         # dominant kernel: pass 1 (sample + chain + bin), bound by instruction issue
         hybrid = args.variant == "auto"
-        n_instr = N_INSTR_HYB[HEADLINE_CFG] if hybrid else N_INSTR_BIN[HEADLINE_CFG]
+        if args.fast_trig:
+            n_instr = N_INSTR_HYB[HEADLINE_CFG] if hybrid else N_INSTR_BIN[HEADLINE_CFG]
+        else:
+            n_instr = N_INSTR_HYB_ACC[HEADLINE_CFG] if hybrid else N_INSTR_BIN_ACC[HEADLINE_CFG]
         roofline = {
             "bound": "alu", "achieved": P * I * n_instr / pass1_s / 1e12, "peak": rates["ffma"] / 1e12,
             "unit": "T lane-instructions/s", "frac": (P * I * n_instr / pass1_s) / rates["ffma"],

@@ -172,10 +172,9 @@ cfs_status cfs_render(const cfs_system *sys, const cfs_render_args *args, void *
 
 /* bytes of d_scratch with which CFS_VARIANT_BINNED renders args->n_points in ONE chunk (pass 1 +
  * pass 2); 0 when the variant cannot serve this system / output mode / image, or without a device.
- * With scratch memory given, CFS_VARIANT_AUTO takes the binned path for large renders it can serve
- * (at least one 1024-point CTA per SM and 2^27 splats) whose chain has no sin/cos step or runs with
- * CFS_FLAG_FAST_TRIG -- where it was measured faster than the L2 atomic rate allows -- and the
- * direct path otherwise. */
+ * With scratch memory given, CFS_VARIANT_AUTO takes the binned path in its hybrid form (CFS_FLAG_BIN_HYBRID)
+ * for large renders it can serve (at least one 1024-point CTA per SM and 2^27 splats) -- where it was
+ * measured faster than the L2 atomic rate allows -- and the direct path otherwise. */
 uint64_t cfs_binned_scratch_bytes(const cfs_system *sys, const cfs_render_args *args);
 
 /* bytes of d_scratch CFS_VARIANT_DEPTH_HIZ needs for a width x height depth image (host arithmetic,

@@ -787,10 +787,10 @@ extern "C" cfs_status cfs_render(const cfs_system *s, const cfs_render_args *a, 
             // direct: ld.cg pre-test + atom.min.  Measured at the SM-to-L2 request rate (one sector request per
             // clock and SM, l1tex2xbar 98 % busy); CFS_VARIANT_DEPTH_HIZ removes that bound but lands on the
             // issue rate at the same time (228.7 ms both on configs[4]), so AUTO keeps the path without scratch
-        } else if (a->d_scratch && a->n_points >= (uint64_t)di.sms * cfs::kBinCtasPerSm * cfs::kBinThreads && n_splats >= (1ull << 27) &&
-                   (!cfs::sig_has_trig(chain_signature(p)) || (a->flags & CFS_FLAG_FAST_TRIG))) {
-            // the tile bins trade the L2 atomic (~190 G/s) for ~15 more instructions per splat: measured
-            // ahead of the direct path when sin/cos is absent or on the MUFU unit, level with it otherwise
+        } else if (a->d_scratch && a->n_points >= (uint64_t)di.sms * cfs::kBinCtasPerSm * cfs::kBinThreads && n_splats >= (1ull << 27)) {
+            // the hybrid stage (every other splat direct, the rest through the tile bins) keeps issue slots, the
+            // L2 reduction path and HBM busy at once: measured ahead of the direct path with MUFU sin/cos
+            // (configs[1] 3.49 against 5.0 ms) and with sincosf (4.06 against 5.21 ms; configs[2] 172 against 197 ms)
             cfs_status bs = render_binned(s, a, p, di, (cudaStream_t)stream);
             if (bs != CFS_ERR_UNSUPPORTED) return bs;
             build_params(s, a, &p, true);      // restore what the attempt changed; fall through to direct

@@ -405,19 +405,6 @@ def test_eq1_circle_generator_fig2(cfs, oracle, r2_reading, composition):
                 assert density_l1(g[:, ch], o[:, ch]) <= 4e-3      # 1 M splats: edge flips + the sliver above
 
 
-def test_eq1_generator_validation(cfs):
-    f = W.circle_funcs()
-    with pytest.raises(cfs.CfsError) as ei:                      # mixed affine + circle
-        cfs.cfs_create(W.System(2, "ifs", [f[0], W.square_funcs()[0]], [], "none"))
-    assert ei.value.status == cfs.CFS_ERR_UNSUPPORTED
-    with pytest.raises(cfs.CfsError) as ei:                      # 3-D
-        cfs.cfs_create(W.System(3, "ifs", f, [], "none"))
-    assert ei.value.status == cfs.CFS_ERR_INVALID_ARG
-    with pytest.raises(cfs.CfsError) as ei:                      # f_id outside {0, 1}
-        cfs.cfs_create(W.System(2, "ifs", [W.Func("circle_half", 1.0, [2.0, 0.0])], [], "none"))
-    assert ei.value.status == cfs.CFS_ERR_INVALID_ARG
-
-
 def test_branches_one_to_many(cfs, oracle):
     """NEXT-2: a chain with BRANCH markers splats every generated point once per branch.
     HIST: identical per pixel to the oracle and to the sum of the single-chain GPU renders, in every

@@ -118,3 +118,26 @@ def test_hiz_scratch_bytes_is_host_arithmetic(cfs):
             assert -(-wd // (side // 2)) * -(-ht // (side // 2)) * 2 > 96 << 10
         assert cfs.cfs_hiz_scratch_bytes(wd, ht) == (n + 7) // 8 * 8 * 2 + 256
     assert cfs.cfs_hiz_scratch_bytes(16384, 16384) == 0 and cfs.cfs_hiz_scratch_bytes(0, 10) == 0
+
+
+def test_eq1_generator_validation(cfs):
+    f = W.circle_funcs()
+    with pytest.raises(cfs.CfsError) as ei:                      # mixed affine + circle
+        cfs.cfs_create(W.System(2, "ifs", [f[0], W.square_funcs()[0]], [], "none"))
+    assert ei.value.status == cfs.CFS_ERR_UNSUPPORTED
+    with pytest.raises(cfs.CfsError) as ei:                      # 3-D
+        cfs.cfs_create(W.System(3, "ifs", f, [], "none"))
+    assert ei.value.status == cfs.CFS_ERR_INVALID_ARG
+    with pytest.raises(cfs.CfsError) as ei:                      # f_id outside {0, 1}
+        cfs.cfs_create(W.System(2, "ifs", [W.Func("circle_half", 1.0, [2.0, 0.0])], [], "none"))
+    assert ei.value.status == cfs.CFS_ERR_INVALID_ARG
+
+
+def test_branch_marker_validation(cfs):
+    """CFS_T_BRANCH (one-to-many splatting) is checked on the host: not with reuse, known type ids only."""
+    a = [W.Xform("affine", [0.5, 0, 0, 0.5, 0, 0])]
+    ok = cfs.cfs_create(W.System(2, "ifs", W.square_funcs(), a + [W.Xform("branch")] + a, "none"))
+    ok.close()
+    with pytest.raises(cfs.CfsError) as ei:
+        cfs.cfs_create(W.System(2, "ifs", W.square_funcs(), a + [W.Xform("branch")] + a, "none", None, reuse=True))
+    assert ei.value.status == cfs.CFS_ERR_INVALID_ARG
