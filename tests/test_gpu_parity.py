@@ -520,7 +520,7 @@ def test_invalid_arguments(cfs):
 
 
 # ------------------------------------------------------------------ tone map and host entry point
-@pytest.mark.parametrize("cfg", [0, 1, 4])
+@pytest.mark.parametrize("cfg", [0, 1, 2, 4])
 def test_tonemap_matches_oracle(cfs, oracle, cfg):
     import torch
     w = W.config(cfg).scaled(n_points=1 << 13, iterations=200)
@@ -589,7 +589,8 @@ def test_cfg1_full_size_properties(cfs, oracle):
     need = cfs.cfs_binned_scratch_bytes(sysh, cfs.make_args(w.render))
     sysh.close()
     assert need > (2 << 30)                       # 2 bytes per splat + block lists
-    for variant, nbytes in (("binned", need), ("binned", need // 3), ("auto", 1 << 20)):
+    # AUTO with enough scratch runs the hybrid stage (every other splat direct), under sincosf as well.
+    for variant, nbytes in (("binned", need), ("binned", need // 3), ("auto", need), ("auto", 1 << 20)):
         gb, gbc = gpu_render(cfs, w, variant=variant, scratch_bytes=nbytes)
         assert np.array_equal(gb, g) and np.array_equal(gbc, gc)
     # the configuration bench.py times: MUFU sin/cos, AUTO with scratch (-> tile bins).  Conservation
