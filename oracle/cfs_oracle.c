@@ -53,6 +53,27 @@ uint32_t orc_pick_word(uint64_t seed, uint64_t p, uint32_t it)
     return w[it & 3];
 }
 
+/* "duplication" of an object by an on-the-fly PRNG (the stars of Fig. 4), no per-thread
+ * allocation.  The paper gives no rule; DESIGN R14 [PROPOSED]: a SCATTER step with parameters
+ * (D, rx, ry, rz) moves the copy onto one of D duplicates of the object,
+ *     d      = floor(w * D / 2^32),  w = word it&3 of Philox(seed; p lo, p hi, it>>2, AUX),
+ *     offset = (u(v0) rx, u(v1) ry, u(v2) rz),  v = Philox(seed; d, 0, 0, PLACE),  u = the 24-bit map of S4,
+ *     q     += offset          (one float multiply and one float add per coordinate; z only in 3-D).
+ * The D offsets are a pure function of (seed, d): nothing is stored. */
+void orc_scatter(uint64_t seed, uint64_t p, uint32_t it, const float *prm, int dim, float q[3])
+{
+    uint32_t w[4], v[4];
+    keyed_block(seed, p, it >> 2, ORC_DOMAIN_AUX, w);
+    const uint32_t D = (uint32_t)prm[0];
+    const uint32_t d = (uint32_t)(((uint64_t)w[it & 3] * (uint64_t)D) >> 32);
+    keyed_block(seed, (uint64_t)d, 0, ORC_DOMAIN_PLACE, v);
+    for (int c = 0; c < (dim == 3 ? 3 : 2); ++c) {
+        const float u = (float)(v[c] >> 8) * 0x1p-23f - 1.0f;
+        const float o = u * prm[1 + c];
+        q[c] = q[c] + o;
+    }
+}
+
 /* ---------------------------------------------------------------- S3: function pick
  * PAPER L17 "chooses a single function at random"; BJ "selection probabilities".
  * DESIGN R2: cumulative sums in double, T_j = floor(c_j / c_{n-1} * 2^32), T_{n-1} = 2^32,
@@ -366,7 +387,14 @@ static int run(const orc_system *s, const orc_render_args *a, int do_splat, uint
     int ctype[8];
     float cprm[8][12];
     for (int m = 0; m < s->n_chain; ++m) {
-        if (s->chain[m].type < 0 || s->chain[m].type > ORC_T_BRANCH) return -1;
+        if (s->chain[m].type < 0 || s->chain[m].type > ORC_T_SCATTER) return -1;
+        if (s->chain[m].type == ORC_T_SCATTER) {       /* parameters at t like any other step; D in [1, 2^20] */
+            for (int i = 0; i < 4; ++i)
+                cprm[m][i] = (float)((double)s->chain[m].p0[i] + (double)a->t * (double)s->chain[m].p1[i]);
+            if (!(cprm[m][0] >= 1.0f && cprm[m][0] <= 1048576.0f) || cprm[m][0] != (float)(uint32_t)cprm[m][0]) return -1;
+            ctype[m] = ORC_T_SCATTER;
+            continue;
+        }
         if (s->chain[m].type == ORC_T_BRANCH) {
             if (s->reuse) return -1;              /* which branch would be fed back? */
             ctype[m] = ORC_T_BRANCH;
@@ -405,7 +433,10 @@ static int run(const orc_system *s, const orc_render_args *a, int do_splat, uint
                 alive = 1;
                 int m = m0;
                 for (; m < s->n_chain && ctype[m] != ORC_T_BRANCH; ++m)
-                    if (alive) alive = orc_apply_xform(ctype[m], cprm[m], s->dim, q);
+                    if (alive) {
+                        if (ctype[m] == ORC_T_SCATTER) orc_scatter(a->seed, p, (uint32_t)it, cprm[m], s->dim, q);
+                        else alive = orc_apply_xform(ctype[m], cprm[m], s->dim, q);
+                    }
                 m0 = m + 1;                       /* past the BRANCH marker (or past the end) */
                 if (s->reuse) {                   /* Fig. 2(C): the same point is reused (single branch) */
                     g[0] = q[0]; g[1] = q[1]; g[2] = q[2];

@@ -36,11 +36,12 @@ enum { ORC_F_AFFINE = 0, ORC_F_CIRCLE_HALF = 1 };
 enum {
     ORC_T_AFFINE = 0, ORC_T_SWIRL = 1, ORC_T_SINUSOIDAL = 2, ORC_T_ROTATE_Z = 3,
     ORC_T_TWIST_Z = 4, ORC_T_BEND = 5, ORC_T_PINHOLE = 6, ORC_T_STRETCH_COS = 7,
-    ORC_T_BRANCH = 8   /* not a transform: ends one branch of the chain and starts the next */
+    ORC_T_BRANCH = 8,  /* not a transform: ends one branch of the chain and starts the next */
+    ORC_T_SCATTER = 9  /* PRNG-placed duplicates; p = (D, rx, ry, rz); DESIGN R14 */
 };
 enum { ORC_COLOR_NONE = 0, ORC_COLOR_MAP_INDEX = 1, ORC_COLOR_POINT = 2 };
 enum { ORC_OUT_HIST_U32 = 0, ORC_OUT_RGBA = 1, ORC_OUT_DEPTH_U64 = 2 };
-enum { ORC_DOMAIN_PICK = 0, ORC_DOMAIN_INIT = 1 };
+enum { ORC_DOMAIN_PICK = 0, ORC_DOMAIN_INIT = 1, ORC_DOMAIN_AUX = 2, ORC_DOMAIN_PLACE = 3 };
 
 /* generator function: AFFINE params, dim 2: a00 a01 a10 a11 b0 b1;
  * dim 3: a00..a22 row-major then b0 b1 b2.
@@ -84,6 +85,8 @@ int orc_thresholds(const float *prob, int n, uint64_t *T);
 int orc_pick(uint32_t u, const uint64_t *T, int n);
 /* pick of point p at iteration it (keyed word, then orc_pick) */
 uint32_t orc_pick_word(uint64_t seed, uint64_t p, uint32_t it);
+/* SCATTER step (DESIGN R14): q += the offset of the duplicate drawn for (seed, p, it); prm = (D, rx, ry, rz) */
+void orc_scatter(uint64_t seed, uint64_t p, uint32_t it, const float *prm, int dim, float q[3]);
 /* S4 */
 void orc_init_point(uint64_t seed, uint64_t p, int dim, float g[3]);
 /* S5 */

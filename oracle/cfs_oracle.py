@@ -21,7 +21,7 @@ from . import build as _build
 
 _F_TYPES = {"affine": 0, "circle_half": 1}
 _T_TYPES = {"affine": 0, "swirl": 1, "sinusoidal": 2, "rotate_z": 3, "twist_z": 4, "bend": 5,
-            "pinhole": 6, "stretch_cos": 7, "branch": 8}
+            "pinhole": 6, "stretch_cos": 7, "branch": 8, "scatter": 9}
 _COLORS = {"none": 0, "map_index": 1, "point": 2}
 _OUTS = {"hist_u32": 0, "rgba_f32": 1, "depth_u64": 2}
 _GENS = {"ifs": 0, "cloud": 1}

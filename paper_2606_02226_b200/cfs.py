@@ -19,7 +19,7 @@ CFS_OK, CFS_ERR_INVALID_ARG, CFS_ERR_UNSUPPORTED, CFS_ERR_CUDA, CFS_ERR_NOMEM = 
 GEN = {"ifs": 0, "cloud": 1}
 F_TYPE = {"affine": 0, "circle_half": 1}
 T_TYPE = {"affine": 0, "swirl": 1, "sinusoidal": 2, "rotate_z": 3, "twist_z": 4, "bend": 5,
-          "pinhole": 6, "stretch_cos": 7, "branch": 8}
+          "pinhole": 6, "stretch_cos": 7, "branch": 8, "scatter": 9}
 COLOR = {"none": 0, "map_index": 1, "point": 2}
 OUT = {"hist_u32": 0, "rgba_f32": 1, "depth_u64": 2}
 FLAGS = {"fast_trig": 1, "interpret_chain": 2, "bin_pass1_only": 4, "bin_hybrid": 0x100}

@@ -427,3 +427,43 @@ def test_branches_depth_is_the_min_of_single_chain_renders(oracle):
     with pytest.raises(ValueError):            # reuse (Fig. 2(C)) has no meaning with several branches
         oracle.render(W.System(2, "ifs", W.square_funcs(), _join(_branches()), "none", None, reuse=True),
                       W.Render(10, 1, 20, 5, 32, 32, (-1, 1, -1, 1), "hist_u32"))
+
+
+# ------------------------------------------------------------------ NEXT-2: PRNG-placed duplicates (DESIGN R14)
+def _u24(w):
+    return np.float32(np.float32(w >> 8) * np.float32(2.0 ** -23) - np.float32(1.0))
+
+
+def test_scatter_places_copies_by_philox(oracle):
+    """A SCATTER(D, rx, ry) step moves the copy onto duplicate d = floor(w D / 2^32), w = the AUX-domain word
+    of (seed, p, it); the offset of duplicate d is a pure function of (seed, d) in the PLACE domain.  Checked
+    per point against the pinned Philox (known-answer tests) with the keying written out here; the empty-chain
+    generator state must not move (Fig. 2(B)); duplicates are drawn uniformly (chi-square)."""
+    D, rx, ry = 5, 0.75, 0.5
+    seed, n, I = 0xABCDEF12345, 4000, 24
+    sys_s = W.System(2, "ifs", W.square_funcs(), [W.Xform("scatter", [D, rx, ry, 0.0])], "none")
+    r = W.Render(n, seed, I, 4, 64, 64, (-2, 2, -2, 2), "hist_u32")
+    _, g, q, alive = oracle.trace(sys_s, r)
+    _, g0, _, _ = oracle.trace(W.System(2, "ifs", W.square_funcs(), [], "none"), r)
+    assert np.array_equal(g, g0) and alive.all()
+    key = [seed & 0xFFFFFFFF, seed >> 32]
+    offs = []
+    for d in range(D):
+        v = oracle.philox4x32_10([d, 0, 0, 3], key)
+        offs.append((np.float32(_u24(v[0]) * np.float32(rx)), np.float32(_u24(v[1]) * np.float32(ry))))
+    assert len({(float(a), float(b)) for a, b in offs}) == D
+    it = I - 1
+    counts = np.zeros(D)
+    for p in range(n):
+        w = oracle.philox4x32_10([p, 0, it >> 2, 2], key)[it & 3]
+        d = (w * D) >> 32
+        counts[d] += 1
+        assert q[p, 0] == np.float32(g[p, 0] + offs[d][0]) and q[p, 1] == np.float32(g[p, 1] + offs[d][1]) and q[p, 2] == g[p, 2]
+    chi2 = ((counts - n / D) ** 2 / (n / D)).sum()
+    assert chi2 < 30.0                                                   # 4 dof
+    # D = 1: one copy; the offset is applied once per coordinate, z untouched in 2-D
+    one = W.System(2, "ifs", W.square_funcs(), [W.Xform("scatter", [1, rx, ry, 0.0])], "none")
+    _, g1, q1, _ = oracle.trace(one, r)
+    assert np.all(q1[:, 0] == (g1[:, 0] + offs[0][0]).astype(np.float32)) and np.all(q1[:, 1] == (g1[:, 1] + offs[0][1]).astype(np.float32))
+    with pytest.raises(ValueError):                                      # D must be a whole number in [1, 2^20]
+        oracle.trace(W.System(2, "ifs", W.square_funcs(), [W.Xform("scatter", [2.5, rx, ry, 0.0])], "none"), r)
