@@ -75,10 +75,17 @@ typedef struct { int32_t type; float prob; float params[12]; } cfs_func;
  *               to its own copy of the generated point and splatted, so a point drives M splats per iteration
  *               ("many objects from a single primitive"); the image equals the sum (DEPTH: the
  *               min) of the M single-chain renders.  Not with reuse; DEPTH needs every branch to end in PINHOLE.
- *               Runs on the chain interpreter; cfs_trace does not serve it. */
+ *               Runs on the chain interpreter; cfs_trace does not serve it.
+ *   SCATTER     p = (D, rx, ry, rz), D a whole number in [1, 2^20]: PRNG-placed duplicates of an object
+ *               (DESIGN R14).  The copy moves onto duplicate d = floor(w D / 2^32), w = word it & 3
+ *               of Philox(seed; point lo, point hi, it >> 2, domain 2); its offset is (u(v0) rx, u(v1) ry, u(v2) rz)
+ *               with v = Philox(seed; d, 0, 0, domain 3) and u the 24-bit map to [-1, 1) of the point init --
+ *               a pure function of (seed, d), nothing is stored.  Exact float32 (one multiply, one add per
+ *               coordinate).  Runs on the chain interpreter. */
 typedef enum {
     CFS_T_AFFINE = 0, CFS_T_SWIRL = 1, CFS_T_SINUSOIDAL = 2, CFS_T_ROTATE_Z = 3,
-    CFS_T_TWIST_Z = 4, CFS_T_BEND = 5, CFS_T_PINHOLE = 6, CFS_T_STRETCH_COS = 7, CFS_T_BRANCH = 8
+    CFS_T_TWIST_Z = 4, CFS_T_BEND = 5, CFS_T_PINHOLE = 6, CFS_T_STRETCH_COS = 7, CFS_T_BRANCH = 8,
+    CFS_T_SCATTER = 9
 } cfs_xform_type;
 typedef struct { int32_t type; float p0[12]; float p1[12]; } cfs_xform;
 

@@ -20,7 +20,8 @@
 static_assert((int)CFS_T_AFFINE == (int)cfs::T_AFFINE && (int)CFS_T_SWIRL == (int)cfs::T_SWIRL &&
               (int)CFS_T_SINUSOIDAL == (int)cfs::T_SINUSOIDAL && (int)CFS_T_ROTATE_Z == (int)cfs::T_ROTATE_Z &&
               (int)CFS_T_TWIST_Z == (int)cfs::T_TWIST_Z && (int)CFS_T_BEND == (int)cfs::T_BEND &&
-              (int)CFS_T_PINHOLE == (int)cfs::T_PINHOLE && (int)CFS_T_STRETCH_COS == (int)cfs::T_STRETCH_COS,
+              (int)CFS_T_PINHOLE == (int)cfs::T_PINHOLE && (int)CFS_T_STRETCH_COS == (int)cfs::T_STRETCH_COS &&
+              (int)CFS_T_BRANCH == (int)cfs::T_BRANCH && (int)CFS_T_SCATTER == (int)cfs::T_SCATTER,
               "chain type ids");
 static_assert(CFS_MAX_FUNCS == cfs::kMaxFuncs && CFS_MAX_CHAIN == cfs::kMaxChain, "limits");
 static_assert(sizeof(cfs_cloud_rec) == 16, "cloud record is one 128-bit load");
@@ -215,7 +216,7 @@ extern "C" cfs_status cfs_create(cfs_system **out, int32_t dim, int32_t gen_kind
         if (color_rule == CFS_COLOR_MAP_INDEX) st = fail(CFS_ERR_INVALID_ARG, "COLOR_MAP_INDEX needs an IFS generator");
     }
     for (int m = 0; st == CFS_OK && m < n_chain; ++m) {
-        if (chain[m].type < CFS_T_AFFINE || chain[m].type > CFS_T_BRANCH) st = fail(CFS_ERR_INVALID_ARG, "chain[%d]: unknown type %d", m, chain[m].type);
+        if (chain[m].type < CFS_T_AFFINE || chain[m].type > CFS_T_SCATTER) st = fail(CFS_ERR_INVALID_ARG, "chain[%d]: unknown type %d", m, chain[m].type);
         if (st == CFS_OK && chain[m].type == CFS_T_BRANCH && reuse) st = fail(CFS_ERR_INVALID_ARG, "chain[%d]: BRANCH cannot be combined with reuse", m);
         for (int i = 0; st == CFS_OK && i < 12; ++i)
             if (bad_float(chain[m].p0[i]) || bad_float(chain[m].p1[i])) st = fail(CFS_ERR_INVALID_ARG, "chain[%d] parameter %d is not finite", m, i);
@@ -325,6 +326,11 @@ cfs_status build_params(const cfs_system *s, const cfs_render_args *a, RenderPar
         case CFS_T_TWIST_Z:
         case CFS_T_BEND:
             st.p[0] = res(0);
+            break;
+        case CFS_T_SCATTER:
+            for (int i = 0; i < 4; ++i) st.p[i] = res(i);
+            if (!(st.p[0] >= 1.0f && st.p[0] <= 1048576.0f) || st.p[0] != (float)(uint32_t)st.p[0])
+                return fail(CFS_ERR_INVALID_ARG, "chain[%d]: SCATTER needs a whole number of duplicates in [1, 2^20]", m);
             break;
         case CFS_T_PINHOLE: {
             const double fov = (double)x.p0[0] + t * (double)x.p1[0];

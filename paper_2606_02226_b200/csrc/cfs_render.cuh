@@ -74,7 +74,7 @@ __device__ __forceinline__ uint32_t splat_q(const RenderParams &prm, const Share
 template <int DIM, int GEN, int SPLAT, uint32_t SIG, int TRIG>
 __device__ __forceinline__ uint32_t chain_and_splat(const RenderParams &prm, const SharedTables &s, const Sm &sm, uint32_t *s_hist,
                                                     float &gx, float &gy, float &gz, int k, uint32_t point_rgba8,
-                                                    bool have, bool past_burn_in, const BinRegs &br)
+                                                    bool have, bool past_burn_in, const BinRegs &br, const StepCtx &ctx)
 {
     if (SIG == kChainGeneric && prm.n_branches > 1) {
         // one-to-many ("many objects from a single primitive"): every BRANCH of the chain
@@ -88,13 +88,13 @@ __device__ __forceinline__ uint32_t chain_and_splat(const RenderParams &prm, con
                 dropped += splat_q<DIM, GEN, SPLAT>(prm, s, sm, s_hist, qx, qy, qz, alive, k, point_rgba8, have, br);
                 qx = gx; qy = gy; qz = gz; alive = true;
             } else if (alive) {
-                alive = chain_step_dyn<DIM, TRIG>(prm, prm.chain[m], qx, qy, qz);
+                alive = chain_step_dyn<DIM, TRIG>(prm, prm.chain[m], ctx, qx, qy, qz);
             }
         }
         return dropped;
     }
     float qx = gx, qy = gy, qz = gz;            // the copy of Fig. 2(B)
-    const bool alive = apply_chain<DIM, SIG, TRIG>(prm, qx, qy, qz);
+    const bool alive = apply_chain<DIM, SIG, TRIG>(prm, ctx, qx, qy, qz);
     if (SIG == kChainGeneric && prm.reuse) {    // Fig. 2(C): the same point is reused
         gx = qx; gy = qy; gz = qz;
         if (!past_burn_in) return 0u;
@@ -225,7 +225,7 @@ __device__ __forceinline__ uint32_t iterate_block(const RenderParams &prm, const
         }
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
-            const bool alive = apply_chain<DIM, SIG, TRIG>(prm, X[j], Y[j], Z[j]);
+            const bool alive = apply_chain<DIM, SIG, TRIG>(prm, StepCtx{plo, phi, it0 + j}, X[j], Y[j], Z[j]);
             ok[j] = alive && have && bin_in_bounds(br, X[j], Y[j]);
         }
         // warp-uniform choice of one of four straight-line bodies (hybrid or pure bins, RGBA or HIST)
@@ -245,7 +245,8 @@ __device__ __forceinline__ uint32_t iterate_block(const RenderParams &prm, const
             apply_gen<DIM, AFF>(k, sm, prm, gx, gy, gz);
             const bool past = !CHECKED || it >= prm.burn_in;
             if (past || (SIG == kChainGeneric && prm.reuse))
-                dropped += chain_and_splat<DIM, GEN, SPLAT, SIG, TRIG>(prm, s, sm, s_hist, gx, gy, gz, k, 0u, have, past, br);
+                dropped += chain_and_splat<DIM, GEN, SPLAT, SIG, TRIG>(prm, s, sm, s_hist, gx, gy, gz, k, 0u, have, past, br,
+                                                                       StepCtx{plo, phi, it});
         }
     }
     if (SPLAT == SPLAT_BIN && ((((uint32_t)it0 >> 2) + 1u) & prm.bin.check_mask) == 0u) {   // CTA-uniform
@@ -315,7 +316,8 @@ render_kernel(const __grid_constant__ RenderParams prm)
             if (have) rec = __ldcs(reinterpret_cast<const float4 *>(prm.cloud) + p);
             gx = rec.x; gy = rec.y; gz = (DIM == 3) ? rec.z : 0.0f;
             dropped = chain_and_splat<DIM, GEN, SPLAT, SIG, TRIG>(prm, s, sm, s_hist, gx, gy, gz, 0,
-                                                                  __float_as_uint(rec.w), have, true, br);
+                                                                  __float_as_uint(rec.w), have, true, br,
+                                                                  StepCtx{(uint32_t)p, (uint32_t)(p >> 32), 0});
         } else {
             const uint32_t plo = (uint32_t)p, phi = (uint32_t)(p >> 32);
             {
@@ -420,7 +422,7 @@ trace_kernel(const __grid_constant__ RenderParams prm)
             }
             if (it < prm.burn_in && !prm.reuse) continue;
             qx = gx; qy = gy; qz = gz;
-            alive = apply_chain<DIM, SIG, TRIG>(prm, qx, qy, qz);
+            alive = apply_chain<DIM, SIG, TRIG>(prm, StepCtx{(uint32_t)p, (uint32_t)(p >> 32), it}, qx, qy, qz);
             if (prm.reuse) { gx = qx; gy = qy; gz = qz; }
         }
         if (prm.tr_g) { prm.tr_g[3 * i] = gx; prm.tr_g[3 * i + 1] = gy; prm.tr_g[3 * i + 2] = gz; }

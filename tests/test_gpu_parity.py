@@ -462,6 +462,41 @@ def test_branches_one_to_many(cfs, oracle):
     assert ei.value.status == cfs.CFS_ERR_UNSUPPORTED
 
 
+def test_scatter_duplicates(cfs, oracle):
+    """NEXT-2 (DESIGN R14): PRNG-placed duplicates.  SCATTER is exact float32 arithmetic, so traced
+    coordinates and the histogram are identical to the oracle's, in 2-D and 3-D, alone and as one branch of a
+    one-to-many chain (an object plus a field of 64 small copies of it: the paper's "stars")."""
+    sc = W.Xform("scatter", [7, 0.6, 0.4, 0.0])
+    s2 = W.System(2, "ifs", W.square_funcs(), [W.Xform("affine", [0.25, 0, 0, 0.25, 0, 0]), sc], "none")
+    w = W.Workload("sc", s2, W.Render(5000 + 3, 0x1234567890, 61, 9, 192, 128, (-1, 1, -1, 1), "hist_u32"))
+    gp, gg, gq, ga = gpu_trace(cfs, w)
+    op, og, oq, oa = oracle.trace(s2, w.render)
+    assert np.array_equal(gp, op) and np.array_equal(gg, og) and np.array_equal(gq, oq) and np.array_equal(ga, oa)
+    o, oc = oracle.render(s2, w.render)
+    for variant in ("direct", "binned"):
+        g, gc = gpu_render(cfs, w, variant=variant)
+        assert np.array_equal(g, o) and np.array_equal(gc, oc)
+    stars = [W.Xform("affine", [0.03, 0, 0, 0.03, 0, 0]), W.Xform("scatter", [64, 0.95, 0.95, 0.0])]
+    planet = [W.Xform("affine", [0.4, 0, 0, 0.4, 0.1, -0.2])]
+    s3 = W.System(2, "ifs", W.square_funcs(), planet + [W.Xform("branch")] + stars, "map_index", W.palette_for(4))
+    w3 = W.Workload("sky", s3, W.Render(8000, 77, 60, 10, 256, 256, (-1, 1, -1, 1), "rgba_f32"))
+    o3, oc3 = oracle.render(s3, w3.render)
+    g3, gc3 = gpu_render(cfs, w3)
+    assert np.array_equal(g3.astype(np.float64), o3) and np.array_equal(gc3, oc3)      # integer sums < 2^24: exact
+    assert int(oc3[0]) + int(oc3[1]) == 2 * 8000 * 50
+    # 3-D: the z offset is applied too, before the projection
+    pin = W.Xform("pinhole", [60.0, -4.0, 1e-3])
+    s4 = W.System(3, "ifs", W.menger_funcs(), [W.Xform("affine", [0.2, 0, 0, 0, 0.2, 0, 0, 0, 0.2, 0, 0, 0]),
+                                                W.Xform("scatter", [9, 0.7, 0.7, 0.7]), pin], "map_index", W.palette_for(20))
+    w4 = W.Workload("sc3", s4, W.Render(3000, 5, 50, 10, 320, 180, (-1, 1, -1, 1), "depth_u64"))
+    o4, oc4 = oracle.render(s4, w4.render)
+    g4, gc4 = gpu_render(cfs, w4)
+    assert np.array_equal(g4, o4) and np.array_equal(gc4, oc4)
+    with pytest.raises(cfs.CfsError) as ei:
+        gpu_render(cfs, W.Workload("bad", W.System(2, "ifs", W.square_funcs(), [W.Xform("scatter", [0, 1, 1, 0])], "none"), w.render))
+    assert ei.value.status == cfs.CFS_ERR_INVALID_ARG
+
+
 def test_empty_and_accumulate(cfs, oracle):
     import torch
     w = W.config(0).scaled(n_points=0)
