@@ -228,6 +228,10 @@ def test_binned_chunks_and_small_scratch(cfs, oracle):
     o, oc, _ = oracle.render_parallel(w.system, w.render)
     g, gc = gpu_render(cfs, w, variant="binned", scratch_bytes=need * 2 // 3)       # two chunks
     assert np.array_equal(g, o) and np.array_equal(gc, oc)
+    g, gc = gpu_render(cfs, w, variant="binned", flags=["bin_hybrid"], scratch_bytes=need * 2 // 3)    # hybrid, in chunks
+    assert np.array_equal(g, o) and np.array_equal(gc, oc)
+    g, gc = gpu_render(cfs, w, variant="auto", scratch_bytes=need * 3 // 5)         # AUTO: hybrid, in chunks
+    assert np.array_equal(g, o) and np.array_equal(gc, oc)
     with pytest.raises(cfs.CfsError) as ei:
         gpu_render(cfs, w, variant="binned", scratch_bytes=1 << 20)
     assert ei.value.status == cfs.CFS_ERR_UNSUPPORTED
