@@ -192,7 +192,7 @@ uint64_t cfs_hiz_scratch_bytes(int32_t width, int32_t height);
 
 /* the tile plan of the BINNED variant for an image and a device shape, host arithmetic only (no device
  * needed; test instrument): out = { tiles, pixels per tile, magic, shift (tile of pixel p =
- * mulhi32(p, magic) >> shift), colour bits, staging records per tile, flush-check interval in
+ * mulhi32(p, magic) >> shift), colour slots per pixel, staging records per tile, flush-check interval in
  * iterations, pass-2 CTAs per tile }.  UNSUPPORTED when the variant cannot serve the image. */
 cfs_status cfs_binned_plan(int32_t width, int32_t height, int32_t out_mode, int32_t n_funcs, int32_t sms,
                            int32_t smem_per_block_optin, uint32_t out[8]);

@@ -422,23 +422,25 @@ bool bin_shape_raw(int gen, int out_mode, int color, uint32_t n_funcs, int32_t w
 {
     if (gen != CFS_GEN_IFS) { *why = "binned variant needs an IFS generator"; return false; }
     if (out_mode == CFS_OUT_DEPTH_RGBA8_U64) { *why = "binned variant serves HIST and RGBA output"; return false; }
-    uint32_t kbits = 0;
+    uint32_t nk = 1;                       // colour slots per pixel: 1 = HIST, else one per function
     if (out_mode == CFS_OUT_RGBA_F32) {
         if (color != CFS_COLOR_MAP_INDEX) { *why = "binned RGBA needs COLOR_MAP_INDEX"; return false; }
-        while ((1u << kbits) < n_funcs) ++kbits;
-        if (kbits > 4) { *why = "binned RGBA supports at most 16 functions"; return false; }
+        if (n_funcs > 16) { *why = "binned RGBA supports at most 16 functions"; return false; }
+        nk = n_funcs;
     }
     const uint64_t n_pix = (uint64_t)width * height;
     if (n_pix > (1ull << 28)) { *why = "binned variant serves images up to 2^28 pixels"; return false; }
-    // pass 2 keeps (pixels per tile) << kbits counters in shared memory: at most 3 * 2^14 (192 KiB).
-    // Fewer, larger tiles leave longer staging rows in pass 1, hence fewer barriers; but at least
-    // 64 tiles so that one tile's arrivals per iteration stay small against a row.
-    int shift = 14 - (int)kbits;
-    uint32_t mul = 3;
+    // pass 2 keeps (pixels per tile) x nk counters in shared memory: at most 3 * 2^14 (192 KiB), which is also
+    // what a 16-bit record can index.  Tile sizes are 2^s or 3 * 2^s pixels.  Fewer, larger tiles leave longer
+    // staging rows in pass 1, hence fewer barriers; but at least 64 tiles so that one tile's arrivals per
+    // iteration stay small against a row.
+    int shift = 15;
+    uint32_t mul = 1;
     auto tiles_for = [&](int sh, uint32_t m) { const uint64_t tp = (uint64_t)m << sh; return (n_pix + tp - 1) / tp; };
-    while (tiles_for(shift, mul) < 64 && (shift > 8 || mul == 3)) {
-        if (mul == 3) { mul = 1; ++shift; } else { mul = 3; shift -= 2; }     // 3*2^s -> 2^(s+1) -> 3*2^(s-1) ...
-    }
+    auto smaller = [&]() { if (mul == 3) { mul = 1; ++shift; } else { mul = 3; shift -= 2; } };   // 3*2^s -> 2^(s+1) -> 3*2^(s-1) ...
+    while ((((uint64_t)mul << shift) * nk > 49152u) && (shift > 8 || mul == 3)) smaller();
+    while (tiles_for(shift, mul) < 64 && (shift > 8 || mul == 3)) smaller();
+    if (((uint64_t)mul << shift) * nk > 49152u) { *why = "no tile size for this number of colour slots"; return false; }
     const uint64_t n_tiles = tiles_for(shift, mul);
     if (n_tiles > (uint64_t)cfs::kBinThreads) { *why = "image has too many tiles for the binned variant"; return false; }
     // pass 1 staging: cnt + rows of `cap` records per tile, next to the static tables
@@ -452,7 +454,7 @@ bool bin_shape_raw(int gen, int out_mode, int color, uint32_t n_funcs, int32_t w
     cfs::BinParams &b = pl->bp;
     memset(&b, 0, sizeof(b));
     b.n_tiles = (uint32_t)n_tiles; b.tile_pixels = mul << shift;
-    b.kbits = kbits; b.cap = (uint32_t)cap;
+    b.nk = nk; b.cap = (uint32_t)cap;
     // division by tile_pixels as multiply-high + shift, exact for every pixel index of this image
     {
         const uint64_t d = b.tile_pixels;
@@ -490,7 +492,7 @@ bool bin_shape_raw(int gen, int out_mode, int color, uint32_t n_funcs, int32_t w
         b.split = best;
     }
     pl->smem_pass1 = (n_tiles + cfs::kBinDummy + 3) / 4 * 4 * 4 + n_tiles * (size_t)cap * 2;
-    pl->smem_pass2 = ((size_t)b.tile_pixels << kbits) * 4;
+    pl->smem_pass2 = (size_t)b.tile_pixels * nk * 4;
     pl->grid1 = (uint32_t)di.sms * cfs::kBinCtasPerSm;
     return true;
 }
@@ -566,7 +568,7 @@ extern "C" cfs_status cfs_binned_plan(int32_t width, int32_t height, int32_t out
     if (!bin_shape_raw(CFS_GEN_IFS, out_mode, out_mode == CFS_OUT_RGBA_F32 ? CFS_COLOR_MAP_INDEX : CFS_COLOR_NONE, (uint32_t)n_funcs,
                        width, height, di, false, &pl, &why)) return fail(CFS_ERR_UNSUPPORTED, "%s", why);
     out[0] = pl.bp.n_tiles; out[1] = pl.bp.tile_pixels; out[2] = pl.bp.magic; out[3] = pl.bp.mshift;
-    out[4] = pl.bp.kbits; out[5] = pl.bp.cap; out[6] = 4u * (pl.bp.check_mask + 1u); out[7] = pl.bp.split;
+    out[4] = pl.bp.nk; out[5] = pl.bp.cap; out[6] = 4u * (pl.bp.check_mask + 1u); out[7] = pl.bp.split;
     return CFS_OK;
 }
 

@@ -43,11 +43,11 @@ __device__ __forceinline__ uint32_t bin_buf_offset(uint32_t n_tiles) { return (n
 // one record down the direct path (staging row full, or no pool block for the tile)
 __device__ __forceinline__ void bin_direct(const RenderParams &prm, const SharedTables &s, uint32_t tile, uint32_t rec)
 {
-    const uint32_t pix = tile * prm.bin.tile_pixels + (rec >> prm.bin.kbits);
+    const uint32_t pix = tile * prm.bin.tile_pixels + rec / prm.bin.nk;       // rare path: a real division is fine
     if (prm.color_rule == 0) {
         bin_red_add_u32(reinterpret_cast<uint32_t *>(prm.image) + pix, 1u);
     } else {
-        const float4 c = s.palette[rec & ((1u << prm.bin.kbits) - 1u)];
+        const float4 c = s.palette[rec % prm.bin.nk];
         bin_red_add_v4_f32(reinterpret_cast<float *>(prm.image) + 4 * (size_t)pix, c.x, c.y, c.z, 1.0f);
     }
 }
@@ -73,7 +73,7 @@ __device__ __forceinline__ BinRegs bin_regs_init(const RenderParams &prm, uint32
     r.cap = prm.bin.cap; r.cap2 = 2u * prm.bin.cap;
     r.dummy = prm.bin.n_tiles;      // + lane, added by each thread after the broadcast
     r.tp = prm.bin.tile_pixels; r.ntp = 0u - prm.bin.tile_pixels; r.magic = prm.bin.magic; r.mshift = prm.bin.mshift;
-    r.nk = 1u << prm.bin.kbits; r.kmask = r.nk - 1u;
+    r.nk = prm.bin.nk; r.kmask = (prm.color_rule == 0) ? 0u : 0xFFFFFFFFu;
     r.sx = prm.sx; r.ox = prm.ox; r.sy = prm.sy; r.oy = prm.oy;
     r.xmin = prm.xmin; r.xmax = prm.xmax; r.ymin = prm.ymin; r.ymax = prm.ymax;
     r.W = prm.W; r.Wm1 = prm.W - 1; r.Hm1 = prm.H - 1;
@@ -218,7 +218,7 @@ __device__ __forceinline__ void bin_flush(const RenderParams &prm, const SharedT
 }
 
 // ---------------------------------------------------------------------------------------------
-// pass 2.  MODE 0: HIST_U32 (kbits = 0).  MODE 1: RGBA_F32 + MAP_INDEX: counters per
+// pass 2.  MODE 0: HIST_U32 (nk = 1).  MODE 1: RGBA_F32 + MAP_INDEX: counters per
 // (pixel, colour index); the pixel's sum is sum_k n_k * palette[k] (any summation order is a
 // correct result, DESIGN R8; exact for integer-valued palettes while every sum stays < 2^24).
 template <int MODE>
@@ -228,7 +228,7 @@ bin_accumulate_kernel(const __grid_constant__ RenderParams prm)
     extern __shared__ __align__(16) uint32_t acc[];
     const BinParams &b = prm.bin;
     const uint32_t tile = blockIdx.x / b.split, part = blockIdx.x % b.split;
-    const uint32_t n_ctr = b.tile_pixels << b.kbits;
+    const uint32_t n_ctr = b.tile_pixels * b.nk;
     for (uint32_t i = threadIdx.x; i < n_ctr; i += blockDim.x) acc[i] = 0u;
     __syncthreads();
 
@@ -281,12 +281,12 @@ bin_accumulate_kernel(const __grid_constant__ RenderParams prm)
         }
     } else {
         float *img = reinterpret_cast<float *>(prm.image);
-        const uint32_t nk = 1u << b.kbits;
+        const uint32_t nk = b.nk;
         for (uint32_t i = threadIdx.x; i < n_pix_tile; i += blockDim.x) {
             float r = 0.f, g = 0.f, bl = 0.f, a = 0.f;
             uint32_t any = 0u;
             for (uint32_t k = 0; k < nk; ++k) {
-                const uint32_t c = acc[(i << b.kbits) + k];
+                const uint32_t c = acc[i * nk + k];
                 if (c) {
                     const float fc = (float)c;
                     r = __fmaf_rn(fc, prm.palette[4 * k + 0], r);

@@ -88,7 +88,7 @@ struct BinParams {
     uint32_t grid;         // CTAs of pass 1
     uint32_t tile_pixels;  // pixels per tile: 2^s or 3 * 2^s
     uint32_t magic, mshift; // pix / tile_pixels == umulhi(pix, magic) >> mshift for every pixel of the image
-    uint32_t kbits;        // log2(colour slots per pixel): 0 = HIST, else ceil(log2 n_funcs)
+    uint32_t nk;           // colour slots per pixel: 1 = HIST, else the number of functions (<= 16)
     uint32_t cap;          // staging records per tile in shared memory (multiple of 64, >= 320)
     uint32_t check_mask;   // flush check after Philox block q (4 iterations) when ((q + 1) & check_mask) == 0
     uint32_t split;        // pass 2: CTAs per tile

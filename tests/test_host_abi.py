@@ -87,17 +87,17 @@ def test_binned_plan_tile_arithmetic_is_exact(cfs, size, mode, n_funcs):
         pl = cfs.cfs_binned_plan(wd, ht, mode, n_funcs)
     except cfs.CfsError as e:
         assert e.status == cfs.CFS_ERR_UNSUPPORTED          # too many tiles for 320-record staging rows
-        kbits = 0 if mode == "hist_u32" else (n_funcs - 1).bit_length()
-        assert -(-n_pix // (3 << (14 - kbits))) > 300
+        nk = 1 if mode == "hist_u32" else n_funcs
+        assert -(-n_pix // (49152 // nk)) > 300
         return
     tp, nt = pl["tile_pixels"], pl["n_tiles"]
     assert nt == -(-n_pix // tp) and nt <= 1024
     assert tp & (tp - 1) == 0 or (tp % 3 == 0 and (tp // 3) & (tp // 3 - 1) == 0)      # 2^s or 3 * 2^s
-    assert (tp << pl["kbits"]) * 4 <= 192 << 10                                        # pass 2 counters
-    assert (1 << pl["kbits"]) >= n_funcs or mode == "hist_u32"
+    assert tp * pl["nk"] * 4 <= 192 << 10                                              # pass 2 counters
+    assert pl["nk"] == (1 if mode == "hist_u32" else n_funcs)
     assert pl["cap"] >= 320 and pl["cap"] % 64 == 0
     assert nt * pl["cap"] * 2 + (nt + 4) * 4 <= 232448                                  # pass 1 staging rows (u16)
-    assert (tp << pl["kbits"]) <= 1 << 16                                               # a record fits 16 bits
+    assert tp * pl["nk"] <= 1 << 16                                                     # a record fits 16 bits
     assert pl["check_every"] in (4, 8, 16, 32, 64) and pl["split"] >= 1
     edges = np.arange(0, nt + 1, dtype=np.uint64) * np.uint64(tp)
     p = np.unique(np.concatenate([edges, edges[1:] - np.uint64(1), edges[:-1] + np.uint64(1),
