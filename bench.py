@@ -371,7 +371,7 @@ def run_ours(args):
         cfs.cfs_render(sysh, rargs)
         ev[1].record()
         if world > 1:                          # the exchange step: one image all-reduce (sum)
-            dist.all_reduce(img, op=dist.ReduceOp.SUM)
+            cfs.allreduce_image(img, r.out_mode)
         cfs.cfs_tonemap(img, r.out_mode, r.width, r.height, 2.2, 1 / 255.0, out8, scratch)
         ev[2].record()
         return ev

@@ -298,3 +298,24 @@ def shard_points(n_points: int, rank: int, world: int):
     lo = (n_points * rank) // world
     hi = (n_points * (rank + 1)) // world
     return lo, hi - lo
+
+
+def allreduce_image(img, out_mode: str, group=None):
+    """The ONE exchange step of a sharded render (DESIGN 'multi-GPU'): every rank renders its point range
+    into a private image, then the images are combined in place -- sum for HIST / RGBA (uint32 sums wrap
+    like the int32 view they travel as), min over the unsigned 64-bit keys for DEPTH.  NCCL and gloo only
+    know a signed 64-bit MIN, and the empty key (all ones) is -1 there: the sign bit is flipped around
+    the reduction so that the signed order equals the unsigned one.  `img` is a torch tensor in the
+    library's layout (new_image), on any device the process group serves."""
+    import torch
+    import torch.distributed as dist
+    if out_mode == "depth_u64":
+        assert img.dtype == torch.int64
+        flip = torch.tensor(-(1 << 63), dtype=torch.int64, device=img.device)
+        img.bitwise_xor_(flip)
+        dist.all_reduce(img, op=dist.ReduceOp.MIN, group=group)
+        img.bitwise_xor_(flip)
+    else:
+        dist.all_reduce(img, op=dist.ReduceOp.SUM, group=group)
+    return img
+

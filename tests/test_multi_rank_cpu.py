@@ -41,21 +41,18 @@ def _worker(rank: int, world: int, port: int, cfg: int, n_points: int, out_dir: 
     w = W.config(cfg).scaled(n_points=n_points, iterations=60, width=96, height=64)
     off, n = cfs.shard_points(n_points, rank, world)
     img, ctr = cfs_oracle.render(w.system, w.render, n_points=n, point_offset=off)
+    # the binding's exchange step (cfs.allreduce_image), on CPU tensors in the library's layout
     if w.render.out_mode == "hist_u32":
-        t = torch.from_numpy(img.astype(np.int64))
-        dist.all_reduce(t, op=dist.ReduceOp.SUM)
-        red = t.numpy().astype(np.uint32)
+        t = torch.from_numpy(img.astype(np.uint32).view(np.int32).copy())
+        red = cfs.allreduce_image(t, "hist_u32").numpy().view(np.uint32)
     elif w.render.out_mode == "rgba_f32":
         t = torch.from_numpy(np.ascontiguousarray(img, dtype=np.float64))
-        dist.all_reduce(t, op=dist.ReduceOp.SUM)
-        red = t.numpy()
+        red = cfs.allreduce_image(t, "rgba_f32").numpy()
     else:
-        # depth keys are < 2^63 unless empty (all ones = -1 as int64): flip the sign bit so that the
-        # signed MIN of the int64 view orders like the unsigned keys (what ncclMin on int64 needs too)
-        flipped = (img ^ np.uint64(1 << 63)).view(np.int64)
-        t = torch.from_numpy(flipped.copy())
-        dist.all_reduce(t, op=dist.ReduceOp.MIN)
-        red = t.numpy().view(np.uint64) ^ np.uint64(1 << 63)
+        # depth keys are < 2^63 unless empty (all ones = -1 as int64): the helper flips the sign bit so that
+        # the signed MIN of the int64 view orders like the unsigned keys (what ncclMin on int64 needs too)
+        t = torch.from_numpy(img.view(np.int64).copy())
+        red = cfs.allreduce_image(t, "depth_u64").numpy().view(np.uint64)
     c = torch.from_numpy(np.asarray(ctr, dtype=np.int64).copy())
     dist.all_reduce(c, op=dist.ReduceOp.SUM)
     if rank == 0:
