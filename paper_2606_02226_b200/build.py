@@ -31,7 +31,7 @@ def sources():
 
 def _deps():
     root = os.path.dirname(HERE)
-    return (sources() + glob.glob(os.path.join(CSRC, "*.cuh")) + glob.glob(os.path.join(CSRC, "*.h"))
+    return (sources() + glob.glob(os.path.join(CSRC, "*.cuh")) + glob.glob(os.path.join(CSRC, "*.h")) + glob.glob(os.path.join(CSRC, "*.inc"))
             + glob.glob(os.path.join(root, "include", "*.h")))
 
 
