@@ -197,6 +197,28 @@ uint64_t cfs_hiz_scratch_bytes(int32_t width, int32_t height);
 cfs_status cfs_binned_plan(int32_t width, int32_t height, int32_t out_mode, int32_t n_funcs, int32_t sms,
                            int32_t smem_per_block_optin, uint32_t out[8]);
 
+/* cfs_host_resolve -- test instrument, HOST arithmetic only (no device needed; d_image / d_cloud are ignored):
+ * what cfs_render resolves on the host for this system and these arguments before it launches, so that each
+ * value can be checked against a hand-worked number (tests/golden/host_resolved.txt).
+ *   sx, ox, sy, oy   pixel map px = floor(fma(x, sx, ox)) (DESIGN R8): sx = (float)(W / (xmax - xmin)),
+ *                    ox = (float)(-xmin W / (xmax - xmin)), evaluated in double
+ *   chain_type/p     the chain at frame parameter t: AFFINE parameters (float)((double)p0 + (double)t (double)p1);
+ *                    ROTATE_Z resolved to the AFFINE [c -s; s c] (3-D: about z), c = (float)cos(theta), s likewise;
+ *                    PINHOLE as (fx, fy, cam_z, near), fy = (float)(1 / tan(fov/2)), fx = (float)(that H / W);
+ *                    TWIST_Z / BEND p[0]; SCATTER (D, rx, ry, rz)
+ *   thresholds       T_j of DESIGN R2 (n_thresholds of them lie below 2^32), pal8 the palette packed to rgba8:
+ *                    byte = floor(v + 0.5) clamped to [0, 255], NaN -> 0, r | g<<8 | b<<16 | a<<24 (DESIGN R9)
+ * Errors: as cfs_render's validation (INVALID_ARG). */
+typedef struct {
+    float sx, ox, sy, oy;
+    int32_t n_chain, n_funcs, n_thresholds, pad_;
+    int32_t chain_type[CFS_MAX_CHAIN];
+    float chain_p[CFS_MAX_CHAIN][12];
+    uint32_t thresholds[CFS_MAX_FUNCS];
+    uint32_t pal8[CFS_MAX_FUNCS];
+} cfs_resolved;
+cfs_status cfs_host_resolve(const cfs_system *sys, const cfs_render_args *args, cfs_resolved *out);
+
 /* cfs_render_host -- same path with HOST buffers (end-to-end entry point): copies h_cloud to the
  * device (CLOUD), clears a device image, renders [point_offset, +n_points), copies the image to
  * h_image (layout of out_mode) and the counters to h_counters (u64[2], optional); synchronises

@@ -27,7 +27,7 @@ VARIANT = {"auto": 0, "direct": 1, "shared_hist": 2, "warp_agg": 3, "binned": 4,
 MB = {"red_add_u32": 0, "red_add_v4f32": 1, "atom_min_u64": 2, "ld_u64": 3, "atoms_add_u32": 4,
       "ffma": 5, "imad_wide": 6, "lop3": 7, "mufu": 8, "stream_ld128": 9}
 EXPORTS = ["cfs_create", "cfs_destroy", "cfs_render", "cfs_render_host", "cfs_tonemap", "cfs_trace",
-           "cfs_microbench", "cfs_shared_hist_max_bytes", "cfs_binned_scratch_bytes", "cfs_hiz_scratch_bytes", "cfs_binned_plan", "cfs_launch_count", "cfs_last_error",
+           "cfs_microbench", "cfs_host_resolve", "cfs_shared_hist_max_bytes", "cfs_binned_scratch_bytes", "cfs_hiz_scratch_bytes", "cfs_binned_plan", "cfs_launch_count", "cfs_last_error",
            "cfs_version"]
 
 
@@ -54,6 +54,13 @@ class cfs_render_args(C.Structure):
                 ("flags", C.c_int32),
                 ("d_image", C.c_void_p), ("d_cloud", C.c_void_p), ("d_counters", C.c_void_p),
                 ("d_scratch", C.c_void_p), ("scratch_bytes", C.c_uint64)]
+
+
+class cfs_resolved(C.Structure):
+    _fields_ = [("sx", C.c_float), ("ox", C.c_float), ("sy", C.c_float), ("oy", C.c_float),
+                ("n_chain", C.c_int32), ("n_funcs", C.c_int32), ("n_thresholds", C.c_int32), ("pad_", C.c_int32),
+                ("chain_type", C.c_int32 * 8), ("chain_p", (C.c_float * 12) * 8),
+                ("thresholds", C.c_uint32 * 64), ("pal8", C.c_uint32 * 64)]
 
 
 _lib = None
@@ -86,6 +93,8 @@ def lib():
         L.cfs_microbench.argtypes = [C.c_int32, C.c_void_p, C.c_uint64, C.c_uint64, C.c_int32, C.c_int32,
                                      C.c_void_p]
         L.cfs_microbench.restype = C.c_int
+        L.cfs_host_resolve.argtypes = [C.c_void_p, C.POINTER(cfs_render_args), C.POINTER(cfs_resolved)]
+        L.cfs_host_resolve.restype = C.c_int
         L.cfs_shared_hist_max_bytes.argtypes = []
         L.cfs_shared_hist_max_bytes.restype = C.c_uint64
         L.cfs_binned_scratch_bytes.argtypes = [C.c_void_p, C.POINTER(cfs_render_args)]
@@ -230,6 +239,18 @@ def cfs_binned_plan(width: int, height: int, out_mode, n_funcs: int, sms: int = 
     _check(lib().cfs_binned_plan(int(width), int(height), mode, int(n_funcs), int(sms), int(smem_optin), out))
     keys = ["n_tiles", "tile_pixels", "magic", "mshift", "nk", "cap", "check_every", "split"]
     return dict(zip(keys, [int(v) for v in out]))
+
+
+def cfs_host_resolve(sys: System, args: cfs_render_args) -> dict:
+    """What a render resolves on the host (pixel map, chain at t, thresholds, rgba8 palette); no device needed."""
+    out = cfs_resolved()
+    _check(lib().cfs_host_resolve(sys.handle, C.byref(args), C.byref(out)))
+    n = int(out.n_chain)
+    return {"sx": float(out.sx), "ox": float(out.ox), "sy": float(out.sy), "oy": float(out.oy),
+            "chain_type": [int(out.chain_type[m]) for m in range(n)],
+            "chain_p": [np.array(list(out.chain_p[m]), dtype=np.float32) for m in range(n)],
+            "thresholds": [int(out.thresholds[j]) for j in range(int(out.n_thresholds))],
+            "pal8": [int(out.pal8[j]) for j in range(int(out.n_funcs))]}
 
 
 def cfs_render(sys: System, args: cfs_render_args, stream=None) -> None:

@@ -6,7 +6,10 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <map>
+#include <mutex>
 #include <new>
+#include <utility>
 #include <vector>
 
 #include "../../include/cfs.h"
@@ -46,20 +49,50 @@ cfs_status cuda_fail(cudaError_t e, const char *what)
     return fail(CFS_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
 }
 
-struct DeviceInfo { int ok = -1; int sms = 0; int smem_optin = 0; int smem_sm = 0; };
+struct DeviceInfo { int ok = -1; int dev = -1; int sms = 0; int smem_optin = 0; int smem_sm = 0; int cc = 0; };
 
+constexpr int kMaxDevices = 64;
+std::mutex g_dev_mutex;
+DeviceInfo g_dev[kMaxDevices];          // one entry per device ordinal, filled on first use
+
+// attributes of the CURRENT device of the calling thread (a thread may switch devices between calls)
 const DeviceInfo &device_info()
 {
-    static thread_local DeviceInfo di;
+    static const DeviceInfo none = [] { DeviceInfo d; d.ok = 0; return d; }();
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) { cudaGetLastError(); return none; }
+    std::lock_guard<std::mutex> lock(g_dev_mutex);
+    DeviceInfo &di = g_dev[dev];
     if (di.ok < 0) {
-        int dev = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess) { di.ok = 0; cudaGetLastError(); return di; }
+        int major = 0, minor = 0;
         cudaDeviceGetAttribute(&di.sms, cudaDevAttrMultiProcessorCount, dev);
         cudaDeviceGetAttribute(&di.smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
         cudaDeviceGetAttribute(&di.smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev);
+        cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+        cudaDeviceGetAttribute(&minor, cudaDevAttrComputeCapabilityMinor, dev);
+        di.cc = major * 10 + minor;
+        di.dev = dev;
         di.ok = (di.sms > 0) ? 1 : 0;
+        if (di.ok != 1) cudaGetLastError();
     }
     return di;
+}
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize is sticky per (function, device): set it once, and again only
+// when a render needs more than any before it
+std::map<std::pair<const void *, int>, int> g_dyn_smem;
+
+cudaError_t ensure_dyn_smem(const void *fn, size_t bytes)
+{
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    std::lock_guard<std::mutex> lock(g_dev_mutex);
+    int &have = g_dyn_smem[std::make_pair(fn, dev)];
+    if ((int)bytes <= have) return cudaSuccess;
+    e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    if (e == cudaSuccess) have = (int)bytes;
+    return e;
 }
 
 }  // namespace
@@ -264,7 +297,7 @@ cfs_status build_params(const cfs_system *s, const cfs_render_args *a, RenderPar
                 return fail(CFS_ERR_INVALID_ARG, "DEPTH output needs every branch of the chain to end in PINHOLE");
     }
     if (need_image && a->n_points && !a->d_image) return fail(CFS_ERR_INVALID_ARG, "d_image is NULL");
-    if (a->n_points && s->gen == CFS_GEN_CLOUD && !a->d_cloud) return fail(CFS_ERR_INVALID_ARG, "d_cloud is NULL");
+    if (need_image && a->n_points && s->gen == CFS_GEN_CLOUD && !a->d_cloud) return fail(CFS_ERR_INVALID_ARG, "d_cloud is NULL");
     if (a->out_mode == CFS_OUT_RGBA_F32 && ((uintptr_t)a->d_image & 15)) return fail(CFS_ERR_INVALID_ARG, "RGBA image must be 16-byte aligned");
     if (a->out_mode == CFS_OUT_DEPTH_RGBA8_U64 && ((uintptr_t)a->d_image & 7)) return fail(CFS_ERR_INVALID_ARG, "DEPTH image must be 8-byte aligned");
     if (s->gen == CFS_GEN_CLOUD && ((uintptr_t)a->d_cloud & 15)) return fail(CFS_ERR_INVALID_ARG, "cloud must be 16-byte aligned");
@@ -282,7 +315,11 @@ cfs_status build_params(const cfs_system *s, const cfs_render_args *a, RenderPar
     p.sy = (float)((double)a->height / wy); p.oy = (float)(-(double)a->ymin * (double)a->height / wy);
     p.image = a->d_image; p.cloud = a->d_cloud; p.counters = (unsigned long long *)a->d_counters;
     p.dim = s->dim; p.n_funcs = (int)s->funcs.size(); p.n_chain = (int)s->chain.size();
-    p.color_rule = s->color; p.reuse = s->reuse; p.fast_trig = (a->flags & CFS_FLAG_FAST_TRIG) ? 1 : 0;
+    // colour rule AS THE OUTPUT USES IT: a histogram ignores colour whatever the system was created with
+    // (include/cfs.h, oracle: "colour ignored"), so the kernels see COLOR_NONE there -- the tile bins key
+    // their record layout (one counter per pixel against one per pixel and map) on this field
+    p.color_rule = (a->out_mode == CFS_OUT_HIST_U32) ? (int)CFS_COLOR_NONE : s->color;
+    p.reuse = s->reuse; p.fast_trig = (a->flags & CFS_FLAG_FAST_TRIG) ? 1 : 0;
     p.pick_shift = s->pick_shift; p.n_thr = s->n_thr; p.pick_steps = s->pick_steps;
     {   // coefficient rows are replicated in shared memory (up to 8 copies) when more than 8 of them are in
         // use: with fewer, every row already has a bank group of its own
@@ -334,11 +371,17 @@ cfs_status build_params(const cfs_system *s, const cfs_render_args *a, RenderPar
             break;
         case CFS_T_PINHOLE: {
             const double fov = (double)x.p0[0] + t * (double)x.p1[0];
+            if (!(fov > 0.0 && fov < 180.0)) return fail(CFS_ERR_INVALID_ARG, "chain[%d]: PINHOLE fov must be in (0, 180) degrees", m);
             const double f = 1.0 / tan(fov * (3.14159265358979323846 / 180.0) * 0.5);
             st.p[0] = (float)(f * (double)a->height / (double)a->width);
             st.p[1] = (float)f;
             st.p[2] = res(1);
             st.p[3] = res(2);
+            if (bad_float(st.p[0]) || bad_float(st.p[1]) || !(st.p[0] > 0.0f) || !(st.p[1] > 0.0f))
+                return fail(CFS_ERR_INVALID_ARG, "chain[%d]: PINHOLE focal lengths are not finite and positive", m);
+            // the depth key orders like the depth only for d > 0 (DESIGN R8): near < 0 would let d <= 0 through
+            if (a->out_mode == CFS_OUT_DEPTH_RGBA8_U64 && !(st.p[3] >= 0.0f))
+                return fail(CFS_ERR_INVALID_ARG, "chain[%d]: DEPTH output needs PINHOLE near >= 0", m);
             break;
         }
         default:
@@ -610,7 +653,7 @@ cfs_status render_cluster_hist(const cfs_system *s, const cfs_render_args *a, Re
     render_fn fn = pick_kernel(s, p, cfs::SPLAT_HIST_CLUSTER, a->flags);
     if (!fn) return fail(CFS_ERR_UNSUPPORTED, "no cluster-histogram kernel for this system");
     const size_t dyn = (size_t)4 << shift;
-    cudaError_t e = cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
+    cudaError_t e = ensure_dyn_smem((const void *)fn, dyn);
     if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute");
     p.hist_bins = (uint32_t)(hist_bytes / 4);
     p.slice_shift = (uint32_t)shift;
@@ -647,9 +690,9 @@ cfs_status render_binned(const cfs_system *s, const cfs_render_args *a, RenderPa
     if (!fn1) return fail(CFS_ERR_UNSUPPORTED, "no binned kernel for dim %d", s->dim);
     render_fn fn2 = (a->out_mode == CFS_OUT_HIST_U32) ? cfs::bin_accumulate_kernel<0> : cfs::bin_accumulate_kernel<1>;
     cudaError_t e;
-    if ((e = cudaFuncSetAttribute((const void *)fn1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem_pass1)) != cudaSuccess)
+    if ((e = ensure_dyn_smem((const void *)fn1, pl.smem_pass1)) != cudaSuccess)
         return cuda_fail(e, "cudaFuncSetAttribute(pass 1)");
-    if ((e = cudaFuncSetAttribute((const void *)fn2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem_pass2)) != cudaSuccess)
+    if ((e = ensure_dyn_smem((const void *)fn2, pl.smem_pass2)) != cudaSuccess)
         return cuda_fail(e, "cudaFuncSetAttribute(pass 2)");
     p.bin = pl.bp;
     p.bin.hybrid = ((a->flags & CFS_FLAG_BIN_HYBRID) || a->variant == CFS_VARIANT_AUTO) ? 1u : 0u;
@@ -721,7 +764,7 @@ cfs_status render_depth_hiz(const cfs_system *s, const cfs_render_args *a, Rende
     if (!fn0 || !fn1) return fail(CFS_ERR_UNSUPPORTED, "no depth kernel for dim %d", s->dim);
     uint16_t *hz = (uint16_t *)(((uintptr_t)a->d_scratch + 255) & ~(uintptr_t)255);
     const size_t dyn = (size_t)pl.n_pad * 2;
-    cudaError_t e = cudaFuncSetAttribute((const void *)fn1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
+    cudaError_t e = ensure_dyn_smem((const void *)fn1, dyn);
     if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute");
     p.hiz.hz = hz; p.hiz.shift = pl.shift; p.hiz.nbx = pl.nbx; p.hiz.nby = pl.nby; p.hiz.n_pad = pl.n_pad;
     // the map's padding entries are read into shared memory but never indexed; clear them once
@@ -755,11 +798,14 @@ cfs_status render_depth_hiz(const cfs_system *s, const cfs_render_args *a, Rende
 
 }  // namespace
 
-extern "C" cfs_status cfs_render(const cfs_system *s, const cfs_render_args *a, void *stream)
+// cloud_base: index of the record d_cloud[0] in the WHOLE cloud (0 for cfs_render; cfs_render_host uploads
+// only the rendered record range)
+static cfs_status render_impl(const cfs_system *s, const cfs_render_args *a, void *stream, uint64_t cloud_base)
 {
     RenderParams p;
     cfs_status st = build_params(s, a, &p, true);
     if (st != CFS_OK) return st;
+    p.cloud_base = cloud_base;
     if (a->variant < CFS_VARIANT_AUTO || a->variant > CFS_VARIANT_DEPTH_HIZ) return fail(CFS_ERR_INVALID_ARG, "unknown variant %d", a->variant);
     const DeviceInfo &di = device_info();
     if (di.ok != 1) return fail(CFS_ERR_CUDA, "no CUDA device (this library has no CPU fallback)");
@@ -802,6 +848,7 @@ extern "C" cfs_status cfs_render(const cfs_system *s, const cfs_render_args *a, 
             cfs_status bs = render_binned(s, a, p, di, (cudaStream_t)stream);
             if (bs != CFS_ERR_UNSUPPORTED) return bs;
             build_params(s, a, &p, true);      // restore what the attempt changed; fall through to direct
+            p.cloud_base = cloud_base;
         }
     }
     if (a->n_points == 0) return CFS_OK;
@@ -814,7 +861,7 @@ extern "C" cfs_status cfs_render(const cfs_system *s, const cfs_render_args *a, 
     if (splat == cfs::SPLAT_HIST_SHARED) {
         dyn = hist_bytes;
         p.hist_bins = (uint32_t)(hist_bytes / 4);
-        cudaError_t e = cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
+        cudaError_t e = ensure_dyn_smem((const void *)fn, dyn);
         if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute");
     }
     // CLOUD and SHARED_HIST: persistent grid (resident CTAs x SMs), grid-stride over points: one
@@ -835,6 +882,35 @@ extern "C" cfs_status cfs_render(const cfs_system *s, const cfs_render_args *a, 
     ++g_launches;
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "render kernel launch");
+    return CFS_OK;
+}
+
+extern "C" cfs_status cfs_render(const cfs_system *s, const cfs_render_args *a, void *stream)
+{
+    return render_impl(s, a, stream, 0);
+}
+
+// host-only view of what a render resolves before its launch (no device needed): lets the CPU tests pin the
+// library's host arithmetic against hand-worked numbers instead of against the oracle's restatement of it
+extern "C" cfs_status cfs_host_resolve(const cfs_system *s, const cfs_render_args *a, cfs_resolved *out)
+{
+    if (!out) return fail(CFS_ERR_INVALID_ARG, "out is NULL");
+    RenderParams p;
+    cfs_render_args r;
+    if (a) { r = *a; r.d_image = nullptr; r.d_cloud = nullptr; }
+    cfs_status st = build_params(s, a ? &r : nullptr, &p, false);
+    if (st != CFS_OK) return st;
+    memset(out, 0, sizeof(*out));
+    out->sx = p.sx; out->ox = p.ox; out->sy = p.sy; out->oy = p.oy;
+    out->n_chain = p.n_chain;
+    for (int m = 0; m < p.n_chain; ++m) {
+        out->chain_type[m] = (p.chain[m].type == cfs::T_SCALE) ? (int32_t)CFS_T_AFFINE : p.chain[m].type;
+        memcpy(out->chain_p[m], p.chain[m].p, sizeof(out->chain_p[m]));
+    }
+    out->n_funcs = p.n_funcs;
+    out->n_thresholds = p.n_thr;
+    memcpy(out->thresholds, p.T, sizeof(out->thresholds));
+    memcpy(out->pal8, p.pal8, sizeof(out->pal8));
     return CFS_OK;
 }
 
@@ -892,7 +968,7 @@ extern "C" cfs_status cfs_render_host(cfs_system *s, const cfs_render_args *a, v
             s->cloud_bytes = cb;
         }
         if ((e = cudaMemcpyAsync(s->d_cloud, h_cloud + a->point_offset, cb, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(e, "H2D cloud");
-        r.d_cloud = (const cfs_cloud_rec *)s->d_cloud - a->point_offset;
+        r.d_cloud = s->d_cloud;                // holds records [point_offset, point_offset + n_points)
     }
     r.d_scratch = nullptr; r.scratch_bytes = 0;
     if (a->variant == CFS_VARIANT_AUTO || a->variant == CFS_VARIANT_BINNED) {
@@ -909,7 +985,7 @@ extern "C" cfs_status cfs_render_host(cfs_system *s, const cfs_render_args *a, v
     }
     if ((e = cudaMemsetAsync(s->d_image, a->out_mode == CFS_OUT_DEPTH_RGBA8_U64 ? 0xFF : 0, bytes, st)) != cudaSuccess) return cuda_fail(e, "clear image");
     if ((e = cudaMemsetAsync(s->d_counters, 0, 16, st)) != cudaSuccess) return cuda_fail(e, "clear counters");
-    cfs_status rs = cfs_render(s, &r, stream);
+    cfs_status rs = render_impl(s, &r, stream, s->gen == CFS_GEN_CLOUD ? a->point_offset : 0);
     if (rs != CFS_OK) return rs;
     if ((e = cudaMemcpyAsync(h_image, s->d_image, bytes, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(e, "D2H image");
     if (h_counters && (e = cudaMemcpyAsync(h_counters, s->d_counters, 16, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(e, "D2H counters");
@@ -970,7 +1046,7 @@ extern "C" cfs_status cfs_microbench(int32_t kind, void *d_buf, uint64_t footpri
     case CFS_MB_LD_U64:        if (!bins(8)) return fail(CFS_ERR_INVALID_ARG, "footprint too small");  cfs::mb_mem_kernel<3><<<blocks, threads, 0, st>>>(d_buf, bins(8), ops); break;
     case CFS_MB_ATOMS_ADD_U32: {
         if (footprint < 4 || footprint > (uint64_t)di.smem_optin) return fail(CFS_ERR_INVALID_ARG, "shared footprint must be 4..%d bytes", di.smem_optin);
-        cudaError_t e = cudaFuncSetAttribute((const void *)cfs::mb_atoms_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)footprint);
+        cudaError_t e = ensure_dyn_smem((const void *)cfs::mb_atoms_kernel, footprint);
         if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute");
         cfs::mb_atoms_kernel<<<blocks, threads, footprint, st>>>(d_buf, (uint32_t)(footprint / 4), ops);
         break;

@@ -108,7 +108,8 @@ struct RenderParams {
     float xmin, xmax, ymin, ymax;
     float sx, ox, sy, oy;        // pixel map: px = floor(fma(x, sx, ox))
     void *image;
-    const void *cloud;
+    const void *cloud;           // record p of the whole cloud is cloud[p - cloud_base]
+    uint64_t cloud_base;
     unsigned long long *counters;
     // trace outputs (trace kernel only)
     uint8_t *tr_picks;

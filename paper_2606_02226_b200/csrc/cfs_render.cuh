@@ -65,7 +65,7 @@ __device__ __forceinline__ void splat_depth(unsigned long long *buf, int pix, fl
 template <int DIM, int GEN, int SPLAT>
 __device__ __forceinline__ uint32_t splat_q(const RenderParams &prm, const SharedTables &s, const Sm &sm, uint32_t *s_hist,
                                             float qx, float qy, float qz, bool alive, int k, uint32_t point_rgba8,
-                                            bool have, const BinRegs &br);
+                                            bool have, const BinRegs &br, bool bin_direct_half);
 
 // rows 5-7 for one generated point: copy -> chain -> pixel -> reduction.  `k` is the map applied
 // in this iteration (colour rule MAP_INDEX), `point_rgba8` the record colour (POINT).
@@ -74,7 +74,8 @@ __device__ __forceinline__ uint32_t splat_q(const RenderParams &prm, const Share
 template <int DIM, int GEN, int SPLAT, uint32_t SIG, int TRIG>
 __device__ __forceinline__ uint32_t chain_and_splat(const RenderParams &prm, const SharedTables &s, const Sm &sm, uint32_t *s_hist,
                                                     float &gx, float &gy, float &gz, int k, uint32_t point_rgba8,
-                                                    bool have, bool past_burn_in, const BinRegs &br, const StepCtx &ctx)
+                                                    bool have, bool past_burn_in, const BinRegs &br, const StepCtx &ctx,
+                                                    bool bin_direct_half = false)
 {
     if (SIG == kChainGeneric && prm.n_branches > 1) {
         // one-to-many ("many objects from a single primitive"): every BRANCH of the chain
@@ -85,7 +86,7 @@ __device__ __forceinline__ uint32_t chain_and_splat(const RenderParams &prm, con
         uint32_t dropped = 0u;
         for (int m = 0; m <= prm.n_chain; ++m) {
             if (m == prm.n_chain || prm.chain[m].type == T_BRANCH) {
-                dropped += splat_q<DIM, GEN, SPLAT>(prm, s, sm, s_hist, qx, qy, qz, alive, k, point_rgba8, have, br);
+                dropped += splat_q<DIM, GEN, SPLAT>(prm, s, sm, s_hist, qx, qy, qz, alive, k, point_rgba8, have, br, bin_direct_half);
                 qx = gx; qy = gy; qz = gz; alive = true;
             } else if (alive) {
                 alive = chain_step_dyn<DIM, TRIG>(prm, prm.chain[m], ctx, qx, qy, qz);
@@ -99,14 +100,14 @@ __device__ __forceinline__ uint32_t chain_and_splat(const RenderParams &prm, con
         gx = qx; gy = qy; gz = qz;
         if (!past_burn_in) return 0u;
     }
-    return splat_q<DIM, GEN, SPLAT>(prm, s, sm, s_hist, qx, qy, qz, alive, k, point_rgba8, have, br);
+    return splat_q<DIM, GEN, SPLAT>(prm, s, sm, s_hist, qx, qy, qz, alive, k, point_rgba8, have, br, bin_direct_half);
 }
 
 // rows 6-7 for one chain output: bounds -> pixel -> reduction.  Returns 1 when the splat was dropped.
 template <int DIM, int GEN, int SPLAT>
 __device__ __forceinline__ uint32_t splat_q(const RenderParams &prm, const SharedTables &s, const Sm &sm, uint32_t *s_hist,
                                             float qx, float qy, float qz, bool alive, int k, uint32_t point_rgba8,
-                                            bool have, const BinRegs &br)
+                                            bool have, const BinRegs &br, bool bin_direct_half)
 {
     const bool ok = alive && have && in_bounds(prm, qx, qy);
     if (SPLAT == SPLAT_HIST_WARPAGG) {
@@ -148,7 +149,16 @@ __device__ __forceinline__ uint32_t splat_q(const RenderParams &prm, const Share
         splat_depth(reinterpret_cast<unsigned long long *>(prm.image), pix, qz,
                     GEN == 1 ? point_rgba8 : lds_u32(sm.tab + CFS_SM_OFF(pal8) + 4u * (uint32_t)k));
     } else if (SPLAT == SPLAT_BIN) {
-        bin_append(prm, s, br, pix, k);
+        if (bin_direct_half) {      // hybrid stage on the interpreter path: this iteration's splat goes straight to L2 (warp-uniform)
+            if (prm.color_rule == 0) {
+                red_add_u32(reinterpret_cast<uint32_t *>(prm.image) + pix, 1u);
+            } else {
+                const float4 c = lds_v4(sm.tab + CFS_SM_OFF(palette) + 16u * (uint32_t)k);
+                red_add_v4_f32(reinterpret_cast<float *>(prm.image) + 4 * (size_t)pix, c.x, c.y, c.z, 1.0f);
+            }
+        } else {
+            bin_append(prm, s, br, pix, k);
+        }
     }
     return 0u;
 }
@@ -244,9 +254,11 @@ __device__ __forceinline__ uint32_t iterate_block(const RenderParams &prm, const
             const int k = pick_index(u, sm, prm);
             apply_gen<DIM, AFF>(k, sm, prm, gx, gy, gz);
             const bool past = !CHECKED || it >= prm.burn_in;
+            // hybrid stage (DESIGN "hybrid"): iterations 0 and 2 of a steady-state block splat straight to L2
+            const bool direct_half = SPLAT == SPLAT_BIN && !CHECKED && (j & 1) == 0 && prm.bin.hybrid != 0u;
             if (past || (SIG == kChainGeneric && prm.reuse))
                 dropped += chain_and_splat<DIM, GEN, SPLAT, SIG, TRIG>(prm, s, sm, s_hist, gx, gy, gz, k, 0u, have, past, br,
-                                                                       StepCtx{plo, phi, it});
+                                                                       StepCtx{plo, phi, it}, direct_half);
         }
     }
     if (SPLAT == SPLAT_BIN && ((((uint32_t)it0 >> 2) + 1u) & prm.bin.check_mask) == 0u) {   // CTA-uniform
@@ -313,7 +325,7 @@ render_kernel(const __grid_constant__ RenderParams prm)
 
         if (GEN == 1) {   // stored cloud: one coalesced 128-bit load per point (row 1), one splat
             float4 rec = make_float4(0.f, 0.f, 0.f, 0.f);
-            if (have) rec = __ldcs(reinterpret_cast<const float4 *>(prm.cloud) + p);
+            if (have) rec = __ldcs(reinterpret_cast<const float4 *>(prm.cloud) + (p - prm.cloud_base));
             gx = rec.x; gy = rec.y; gz = (DIM == 3) ? rec.z : 0.0f;
             dropped = chain_and_splat<DIM, GEN, SPLAT, SIG, TRIG>(prm, s, sm, s_hist, gx, gy, gz, 0,
                                                                   __float_as_uint(rec.w), have, true, br,
@@ -399,7 +411,7 @@ trace_kernel(const __grid_constant__ RenderParams prm)
         const uint64_t p = prm.point_offset + i;
         float gx, gy, gz = 0.0f;
         if (GEN == 1) {
-            const float4 rec = __ldcs(reinterpret_cast<const float4 *>(prm.cloud) + p);
+            const float4 rec = __ldcs(reinterpret_cast<const float4 *>(prm.cloud) + (p - prm.cloud_base));
             gx = rec.x; gy = rec.y; gz = (DIM == 3) ? rec.z : 0.0f;
         } else {
             const U4 w = philox4x32_10((uint32_t)p, (uint32_t)(p >> 32), 0u, DOMAIN_INIT, prm);

@@ -161,7 +161,7 @@ def test_compiled_chain_equals_interpreter(cfs, oracle, cfg):
     """A kernel compiled for the chain's signature and the chain interpreter evaluate the same device
     functions: traces and images are bit-identical (integer-valued colour sums are order-free)."""
     w = W.config(cfg)
-    n = 3000 + 77
+    n = (1 << 17) + 77 if cfg == 3 else (1 << 14) + 77      # >= 2 M splats (cfg 3: 2^17 records): edge flips stay far below the bar
     cloud = _cloud_for(w, n)
     w = w.scaled(n_points=n, iterations=min(w.render.iterations, 150), width=640, height=360)
     t = w.frames[len(w.frames) // 2]
@@ -177,7 +177,7 @@ def test_compiled_chain_equals_interpreter(cfs, oracle, cfg):
         assert np.array_equal(ga, o) and np.array_equal(ca, oc)
     else:
         for ch in range(4):
-            assert density_l1(ga[:, ch], o[:, ch]) <= 4e-3      # < 500k splats: a handful of edge flips
+            assert density_l1(ga[:, ch], o[:, ch]) <= L1_TOL, (cfg, ch, density_l1(ga[:, ch], o[:, ch]))
 
 
 @pytest.mark.parametrize("interp", [False, True])
@@ -252,6 +252,58 @@ def test_binned_rgba_equals_direct(cfs, oracle, cfg, hybrid):
     assert np.array_equal(gb, gd) and np.array_equal(cb, cd)
     o, oc, _ = oracle.render_parallel(w.system, w.render, t=t)
     _check_rgba(gb, o, cb, oc)
+
+
+@pytest.mark.parametrize("cfg", [1, 2])
+def test_hist_output_of_a_coloured_system_through_the_bins(cfs, oracle, cfg):
+    """HIST_U32 output from a system created with COLOR_MAP_INDEX (colour ignored, include/cfs.h): the tile
+    bins must lay out ONE counter per pixel (round-1 ADVICE: they keyed on the colour rule and wrote 16-byte
+    reductions into a 4-byte histogram).  Every variant that can serve a histogram gives the same image as
+    the direct one, exactly; conservation exact; oracle within the density bar."""
+    w = W.config(cfg).scaled(n_points=(1 << 15) + 9, out_mode="hist_u32")
+    t = w.frames[len(w.frames) // 2]
+    gd, cd = gpu_render(cfs, w, t=t, variant="direct")
+    S = w.render.n_points * (w.render.iterations - w.render.burn_in)
+    assert int(cd[0]) == S and int(gd.sum(dtype=np.uint64)) == S
+    sysh = cfs.cfs_create(w.system)
+    need = cfs.cfs_binned_scratch_bytes(sysh, cfs.make_args(w.render))
+    sysh.close()
+    assert need > 0
+    for variant, flags in (("binned", 0), ("binned", ["bin_hybrid"]), ("auto", 0), ("binned", ["interpret_chain"]),
+                           ("binned", ["bin_hybrid", "interpret_chain"]), ("warp_agg", 0)):
+        g, c = gpu_render(cfs, w, t=t, variant=variant, flags=flags, scratch_bytes=need)
+        assert np.array_equal(g, gd) and np.array_equal(c, cd), (variant, flags)
+    o, oc, _ = oracle.render_parallel(w.system, w.render, t=t)
+    assert np.array_equal(cd, oc) and density_l1(gd, o) <= L1_TOL
+
+
+@pytest.mark.parametrize("cfg,n", [(1, 1 << 18), (2, 1 << 19)])
+def test_bench_launch_configuration_against_the_oracle(cfs, oracle, cfg, n):
+    """The EXACT configuration bench.py times -- variant AUTO with scratch (-> hybrid: every other splat
+    straight to L2, the rest through the tile bins) and CFS_FLAG_FAST_TRIG (MUFU sin/cos) -- on a point
+    sub-range large enough for AUTO's hybrid threshold, at full image size, DIRECTLY against the oracle:
+    counters equal, normalised-density L1 <= 1e-3 on the count and on every colour channel."""
+    import torch
+    w = W.config(cfg).scaled(n_points=n)
+    t = w.frames[len(w.frames) // 2]
+    sysh = cfs.cfs_create(w.system)
+    need = cfs.cfs_binned_scratch_bytes(sysh, cfs.make_args(w.render))
+    assert need > 0
+    scratch = torch.empty(need, dtype=torch.uint8, device="cuda")
+    img = cfs.new_image(w.render)
+    ctr = torch.zeros(2, dtype=torch.int64, device="cuda")
+    cfs.cfs_launch_count(reset=True)
+    cfs.cfs_render(sysh, cfs.make_args(w.render, d_image=img, d_counters=ctr, t=t, variant="auto",
+                                       flags=["fast_trig"], d_scratch=scratch))
+    torch.cuda.synchronize()
+    assert cfs.cfs_launch_count() == 2, "AUTO did not take the hybrid stage (pass 1 + pass 2 in one chunk)"
+    g, gc = img.cpu().numpy(), ctr.cpu().numpy().astype(np.uint64)
+    sysh.close()
+    o, oc, _ = oracle.render_parallel(w.system, w.render, t=t)
+    assert np.array_equal(gc, oc) and int(gc[1]) == 0
+    assert g[:, 3].astype(np.float64).sum() == o[:, 3].sum() == float(oc[0])
+    for ch in range(4):
+        assert density_l1(g[:, ch], o[:, ch]) <= L1_TOL, (cfg, ch, density_l1(g[:, ch], o[:, ch]))
 
 
 def test_binned_hot_tile_overflow_and_limits(cfs, oracle):
@@ -366,17 +418,17 @@ def test_reuse_composition_and_eq2(cfs, oracle):
     chain = [W.Xform("stretch_cos"), W.Xform("affine", [0.4, 0, 0, 0.4, 0, 0.3])]
     for reuse in (False, True):
         sysr = W.System(2, "ifs", W.square_funcs(), chain, "map_index", W.palette_for(4), reuse=reuse)
-        w = W.Workload("reuse", sysr, W.Render(2000, 12, 60, 10, 256, 256, (-1.5, 1.5, -1.5, 1.5), "rgba_f32"))
-        gp, gg, gq, ga = gpu_trace(cfs, w)
-        op, og, oq, oa = oracle.trace(sysr, w.render)
+        w = W.Workload("reuse", sysr, W.Render(40000, 12, 60, 10, 256, 256, (-1.5, 1.5, -1.5, 1.5), "rgba_f32"))
+        gp, gg, gq, ga = gpu_trace(cfs, w, n_points=2000)
+        op, og, oq, oa = oracle.trace(sysr, w.render, n_points=2000)
         assert np.array_equal(gp, op) and np.array_equal(ga, oa)
         assert np.abs(gg.astype(np.float64) - og).max() <= COORD_TOL
         assert np.abs(gq.astype(np.float64) - oq).max() <= COORD_TOL
         g, gc = gpu_render(cfs, w)
-        o, oc = oracle.render(sysr, w.render)
+        o, oc, _ = oracle.render_parallel(sysr, w.render)
         assert np.array_equal(gc, oc)
         for ch in range(4):
-            assert density_l1(g[:, ch], o[:, ch]) <= 4e-3      # 100k splats: a handful of edge flips
+            assert density_l1(g[:, ch], o[:, ch]) <= L1_TOL, (reuse, ch, density_l1(g[:, ch], o[:, ch]))
 
 
 @pytest.mark.parametrize("r2_reading", [False, True])
@@ -400,13 +452,16 @@ def test_eq1_circle_generator_fig2(cfs, oracle, r2_reading, composition):
     if composition == "A":       # f_id decides the half of the disc, and the point stays inside it
         last = gp[:, -1]
         assert np.all((gg[:, 1] >= 0) == (last == 0)) and np.all(np.hypot(gg[:, 0], gg[:, 1]) < 1.0 + 1e-6)
+    # density bar (iv) at 24 M splats on a 128 x 128 image: the few trajectories that float32 and double take apart
+    # (non-contractive maps) land on the same invariant density, so with ~1500 splats per pixel they no longer show
+    wd = W.Workload("eq1d", sysc, W.Render(480000, 21, 60, 10, 128, 128, (-1.5, 1.5, -1.5, 1.5), "rgba_f32"))
+    o, oc, _ = oracle.render_parallel(sysc, wd.render)
     for variant in ("direct", "binned"):
-        g, gc = gpu_render(cfs, w, variant=variant, flags=["bin_hybrid"] if variant == "binned" else 0)
-        o, oc = oracle.render(sysc, w.render)
-        assert int(gc[0]) + int(gc[1]) == 20000 * 50 and abs(int(gc[0]) - int(oc[0])) <= 20
+        g, gc = gpu_render(cfs, wd, variant=variant, flags=["bin_hybrid"] if variant == "binned" else 0)
+        assert int(gc[0]) + int(gc[1]) == 480000 * 50 and abs(int(gc[0]) - int(oc[0])) <= 480
         for ch in range(4):
             if o[:, ch].sum() > 0:
-                assert density_l1(g[:, ch], o[:, ch]) <= 4e-3      # 1 M splats: edge flips + the sliver above
+                assert density_l1(g[:, ch], o[:, ch]) <= L1_TOL, (variant, ch, density_l1(g[:, ch], o[:, ch]))
 
 
 def test_branches_one_to_many(cfs, oracle):
@@ -590,6 +645,9 @@ def test_render_host_entry_point(cfs, oracle, cfg):
     w = W.config(cfg)
     n = 5000
     cloud = _cloud_for(w, n + 100)
+    if cfg == 3:
+        n = 1 << 17                          # one splat per record: enough of them that an edge flip weighs 1.5e-5
+        cloud = _cloud_for(w, n + 100)
     w = w.scaled(n_points=n, iterations=min(w.render.iterations, 60), burn_in=min(w.render.burn_in, 20),
                  width=320, height=180)
     npx = 320 * 180
@@ -602,7 +660,7 @@ def test_render_host_entry_point(cfs, oracle, cfg):
     o, oc = oracle.render(w.system, w.render, cloud=cloud, point_offset=off)
     if cfg == 3:
         for ch in range(4):
-            assert density_l1(h_img[:, ch], o[:, ch]) <= 4e-3
+            assert density_l1(h_img[:, ch], o[:, ch]) <= L1_TOL, (ch, density_l1(h_img[:, ch], o[:, ch]))
     else:
         assert np.array_equal(h_img, o)
     assert np.array_equal(h_ctr, oc) or cfg == 3

@@ -1,0 +1,305 @@
+"""Pins that close the round-1 ledger (VERDICT "what's weak" 1, ADVICE "shared misreading").
+
+Every expected value here comes from mathematics or from a hand-worked fixture under tests/golden/
+-- never from the oracle's own formula, never from the CUDA library:
+  * 3-D affine maps with all nine coefficients distinct and quarter turns about x, y, z
+    (a row/column swap of the coefficient layout fails them), through the generator AND the chain;
+  * Fig. 2(C) `reuse`: the chain runs at EVERY iteration, burn-in included (DESIGN R11) -- the composed
+    affine map's fixed point from a linear solve, and a case that differs iff burn-in skips the chain;
+  * SCATTER in 3-D with rz != 0 (the z offset), keying written out against the known-answer-tested Philox;
+  * rgba8 packing (round half up, clamp, NaN -> 0) through a DEPTH render with a non-integer palette;
+  * the values the HOST resolves (pixel map, pinhole focal lengths, ROTATE_Z, rgba8) for BOTH sides,
+    each against tests/golden/host_resolved.txt (the library through cfs_host_resolve, no device needed).
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+
+from paper_2606_02226_b200 import workloads as W
+
+GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+
+
+def _golden_values(name):
+    out = {}
+    for ln in open(os.path.join(GOLDEN, name)):
+        ln = ln.split("#", 1)[0].strip()
+        if not ln:
+            continue
+        k, v = [s.strip() for s in ln.split("=")]
+        out[k] = int(v, 16) if v.lower().startswith("0x") else float(v)
+    return out
+
+
+def _affine3d_cases():
+    cases = []
+    for ln in open(os.path.join(GOLDEN, "affine3d_worked.txt")):
+        ln = ln.split("#", 1)[0].strip()
+        if not ln:
+            continue
+        m, v, want = [[float(t) for t in part.split()] for part in ln.split("|")]
+        assert len(m) == 12 and len(v) == 3 and len(want) == 3
+        cases.append((m, v, want))
+    assert len(cases) >= 5
+    return cases
+
+
+# ------------------------------------------------------------------ 3-D affine: coefficient layout
+def test_affine3d_worked_examples_generator_and_chain(oracle):
+    for m, v, want in _affine3d_cases():
+        got = oracle.apply_func(W.Func("affine", 1.0, m), 3, np.array(v, dtype=np.float32))
+        assert list(got.astype(np.float64)) == want, (m, v, list(got), want)
+        q, alive = oracle.apply_xform(W.Xform("affine", m), 3, np.array(v, dtype=np.float32))
+        assert alive and list(q.astype(np.float64)) == want
+
+
+def test_affine3d_fixed_point_of_a_full_matrix(oracle):
+    """A contraction with a FULL 3x3 matrix (all off-diagonals non-zero, not symmetric): one-hot
+    probabilities converge to (I - A)^-1 b from a linear solve; the transposed matrix has a different one."""
+    A = np.array([[0.30, -0.20, 0.10], [0.25, 0.15, -0.35], [-0.05, 0.40, 0.20]])
+    b = np.array([0.3, -0.2, 0.5])
+    fix = np.linalg.solve(np.eye(3) - A, b)
+    fix_t = np.linalg.solve(np.eye(3) - A.T, b)
+    assert np.abs(fix - fix_t).max() > 0.05
+    funcs = [W.Func("affine", 1.0, list(A.ravel()) + list(b)),
+             W.Func("affine", 0.0, [0.5, 0, 0, 0, 0.5, 0, 0, 0, 0.5, 0, 0, 0])]
+    sysm = W.System(3, "ifs", funcs, [W.PINHOLE], "map_index", W.palette_for(2))
+    r = W.Render(64, 7, 80, 10, 64, 64, (-1, 1, -1, 1), "depth_u64")
+    picks, g, _, _ = oracle.trace(sysm, r)
+    assert not picks.any()
+    assert np.abs(g.astype(np.float64) - fix).max() < 2e-6
+
+
+# ------------------------------------------------------------------ Fig. 2(C): reuse during burn-in
+def _composed_fixed_point(fA, fb, TA, Tb):
+    """g* with g* = T(f(g*)), f(p) = fA p + fb, T(q) = TA q + Tb: a 2x2 linear solve."""
+    M = TA @ fA
+    return np.linalg.solve(np.eye(2) - M, TA @ fb + Tb)
+
+
+@pytest.mark.parametrize("k", [0, 3])
+def test_reuse_feeds_the_chain_back_at_every_iteration_including_burn_in(oracle, k):
+    """PAPER L77, Fig. 2(C); DESIGN R11.  One-hot probabilities on square map k, chain = one affine
+    contraction T with a rotation part, reuse: every iteration is g <- T(f_k(g)), an affine contraction
+    whose fixed point a linear solve gives.  (i) long run: the final point IS that fixed point.
+    (ii) iterations = burn_in + 1: an implementation that skipped the chain while it < burn_in would
+    sit on f_k's own fixed point c_k after burn-in and splat T(f_k(c_k)) = T(c_k), a different pixel."""
+    probs = [0.0] * 4
+    probs[k] = 1.0
+    c = np.array([2 * (k & 1) - 1, 2 * (k >> 1) - 1], dtype=np.float64)
+    fA, fb = 0.5 * np.eye(2), 0.5 * c
+    TA = np.array([[0.5, -0.25], [0.25, 0.5]])
+    Tb = np.array([0.25, -0.125])
+    chain = [W.Xform("affine", [TA[0, 0], TA[0, 1], TA[1, 0], TA[1, 1], Tb[0], Tb[1]])]
+    sysr = W.System(2, "ifs", W.square_funcs(probs), chain, "none", reuse=True)
+    fix = _composed_fixed_point(fA, fb, TA, Tb)
+    skipped = TA @ c + Tb                       # what "no chain during burn-in" would splat
+    assert np.abs(fix - skipped).max() > 0.1
+    for I, B in ((90, 60), (61, 60)):
+        r = W.Render(32, 3, I, B, 256, 256, (-2, 2, -2, 2), "hist_u32")
+        picks, g, q, alive = oracle.trace(sysr, r)
+        assert np.all(picks == k) and alive.all()
+        assert np.abs(g.astype(np.float64) - np.append(fix, 0.0)).max() < 1e-6
+        assert np.array_equal(g, q)
+        img, ctr = oracle.render(sysr, r)
+        want_pix = oracle.pixel(fix[0], fix[1], r.bounds, 256, 256)
+        wrong_pix = oracle.pixel(skipped[0], skipped[1], r.bounds, 256, 256)
+        assert want_pix != wrong_pix
+        assert int(img[want_pix]) == 32 * (I - B) == int(ctr[0]) and int(img[wrong_pix]) == 0
+
+
+def test_reuse_burn_in_positions_are_not_splatted(oracle):
+    """With reuse the chain runs during burn-in but nothing is written: B = I - 1 leaves one splat per point."""
+    chain = [W.Xform("affine", [0.5, 0, 0, 0.5, 0.25, 0])]
+    sysr = W.System(2, "ifs", W.square_funcs(), chain, "none", reuse=True)
+    img, ctr = oracle.render(sysr, W.Render(500, 9, 40, 39, 64, 64, (-2, 2, -2, 2), "hist_u32"))
+    assert int(img.sum()) == 500 == int(ctr[0]) + int(ctr[1])
+
+
+# ------------------------------------------------------------------ SCATTER in 3-D (z offset)
+def _u24(w):
+    return np.float32(np.float32(w >> 8) * np.float32(2.0 ** -23) - np.float32(1.0))
+
+
+def test_scatter_3d_offsets_include_z(oracle):
+    """DESIGN R14 in 3-D: offset = (u(v0) rx, u(v1) ry, u(v2) rz), v = Philox(seed; d, 0, 0, PLACE = 3),
+    d = floor(w D / 2^32), w = word it & 3 of Philox(seed; p lo, p hi, it >> 2, AUX = 2).  Checked per
+    point and per coordinate against the known-answer-tested Philox; a 2-D-only implementation (z
+    untouched) or one that reuses v1 for z fails."""
+    D, rx, ry, rz = 6, 0.5, 0.25, 0.75
+    seed, n, I = 0x1234ABCD5678, 1500, 13
+    sc = W.Xform("scatter", [D, rx, ry, rz])
+    sys3 = W.System(3, "ifs", W.menger_funcs(), [sc], "none")
+    r = W.Render(n, seed, I, 3, 32, 32, (-3, 3, -3, 3), "hist_u32")
+    _, g, q, alive = oracle.trace(sys3, r)
+    _, g0, _, _ = oracle.trace(W.System(3, "ifs", W.menger_funcs(), [], "none"), r)
+    assert np.array_equal(g, g0) and alive.all()
+    key = [seed & 0xFFFFFFFF, seed >> 32]
+    offs = []
+    for d in range(D):
+        v = oracle.philox4x32_10([d, 0, 0, 3], key)
+        offs.append([np.float32(_u24(v[c]) * np.float32(s)) for c, s in enumerate((rx, ry, rz))])
+    assert len({float(o[2]) for o in offs}) == D and all(float(o[2]) != float(o[1]) for o in offs)
+    it = I - 1
+    for p in range(n):
+        w = oracle.philox4x32_10([p, 0, it >> 2, 2], key)[it & 3]
+        d = (w * D) >> 32
+        for c in range(3):
+            assert q[p, c] == np.float32(g[p, c] + offs[d][c]), (p, c)
+    # the global point id (lo AND hi word) keys the draw
+    off = (5 << 32) + 17
+    _, g5, q5, _ = oracle.trace(sys3, r, n_points=8, point_offset=off)
+    for i in range(8):
+        p = off + i
+        w = oracle.philox4x32_10([p & 0xFFFFFFFF, p >> 32, it >> 2, 2], key)[it & 3]
+        d = (w * D) >> 32
+        assert q5[i, 2] == np.float32(g5[i, 2] + offs[d][2])
+
+
+# ------------------------------------------------------------------ rgba8 packing through a DEPTH render
+PACK_CASES = [("pack_a", (0.49, 0.5, 254.5, 255.5)), ("pack_b", (-3.0, 300.0, float("nan"), 1.5)),
+              ("pack_c", (2.5, 254.49, 0.0, 127.5))]
+
+
+def _pack_system(entry):
+    pal = np.array([entry, (9, 9, 9, 9)], dtype=np.float32)
+    funcs = [W.Func("affine", 1.0, [0.5, 0, 0, 0, 0.5, 0, 0, 0, 0.5, 0, 0, 0]),
+             W.Func("affine", 0.0, [0.5, 0, 0, 0, 0.5, 0, 0, 0, 0.5, 0.5, 0, 0])]
+    return W.System(3, "ifs", funcs, [W.PINHOLE], "map_index", pal)
+
+
+@pytest.mark.parametrize("name,entry", PACK_CASES)
+def test_rgba8_packing_through_depth_render(oracle, name, entry):
+    """byte = floor(v + 0.5) clamped to [0, 255], NaN -> 0 (DESIGN R9): the colour half of every depth key."""
+    want = _golden_values("host_resolved.txt")[name]
+    r = W.Render(40, 11, 30, 5, 16, 16, (-1, 1, -1, 1), "depth_u64")
+    img, ctr = oracle.render(_pack_system(entry), r)
+    hit = img != oracle.DEPTH_EMPTY
+    assert hit.any() and int(ctr[0]) == 40 * 25
+    assert set(int(v) for v in (img[hit] & np.uint64(0xFFFFFFFF))) == {want}
+    # the depth half: every point sits near the origin, camera at z = -4 -> d close to 4
+    depth = (img[hit] >> np.uint64(32)).astype(np.uint32).view(np.float32)
+    assert np.all(np.abs(depth - 4.0) < 1.0)
+
+
+# ------------------------------------------------------------------ host-resolved values, both sides
+@pytest.fixture(scope="module")
+def cfs():
+    from paper_2606_02226_b200 import build as cuda_build
+    cuda_build.build()                       # nvcc cross-compiles without a GPU
+    from paper_2606_02226_b200 import cfs as mod
+    mod.lib()
+    return mod
+
+
+def test_host_resolved_pixel_map_library(cfs):
+    G = _golden_values("host_resolved.txt")
+    w1, w2 = W.config(1), W.config(2)
+    for w, tag, keys in ((w1, "cfg1", ("sx", "ox")), (w2, "cfg2", ("sx", "ox", "sy", "oy"))):
+        sysh = cfs.cfs_create(w.system)
+        res = cfs.cfs_host_resolve(sysh, cfs.make_args(w.render))
+        for k in keys:
+            assert res[k] == G[f"pixmap_{tag}_{k}"], (tag, k, res[k])
+        sysh.close()
+    asym = W.config(0).scaled(width=200, height=120, bounds=(-0.75, 1.0, -1.0, 0.5))
+    sysh = cfs.cfs_create(asym.system)
+    res = cfs.cfs_host_resolve(sysh, cfs.make_args(asym.render))
+    for k in ("sx", "ox", "sy", "oy"):
+        assert res[k] == G[f"pixmap_asym_{k}"], (k, res[k])
+    sysh.close()
+
+
+def test_host_resolved_pixel_map_oracle(oracle):
+    """The oracle's pixel rule against the golden coefficients: px = floor(fma(x, sx, ox)) evaluated HERE in
+    float32 from the golden sx, ox (numpy float32 multiply-add of exactly representable products is not
+    assumed: the probe points are chosen so that the unfused and fused results agree)."""
+    G = _golden_values("host_resolved.txt")
+    sx, ox = np.float32(G["pixmap_asym_sx"]), np.float32(G["pixmap_asym_ox"])
+    sy, oy = np.float32(G["pixmap_asym_sy"]), np.float32(G["pixmap_asym_oy"])
+    rng = np.random.default_rng(5)
+    n_checked = 0
+    for _ in range(4000):
+        x = np.float32(rng.uniform(-0.75, 1.0))
+        y = np.float32(rng.uniform(-1.0, 0.5))
+        fx = np.float64(x) * np.float64(sx) + np.float64(ox)          # exact in double (24 x 24-bit product)
+        fy = np.float64(y) * np.float64(sy) + np.float64(oy)
+        if abs(fx - round(fx)) < 1e-3 or abs(fy - round(fy)) < 1e-3:
+            continue                                                   # within float32 rounding of a pixel edge
+        want = int(min(max(math.floor(fy), 0), 119)) * 200 + int(min(max(math.floor(fx), 0), 199))
+        assert oracle.pixel(x, y, (-0.75, 1.0, -1.0, 0.5), 200, 120) == want
+        n_checked += 1
+    assert n_checked > 3000
+    # a wrong offset sign, a swapped W/H or a scale without the width would move these
+    assert oracle.pixel(-0.75, -1.0, (-0.75, 1.0, -1.0, 0.5), 200, 120) == 0
+    assert oracle.pixel(1.0, 0.5, (-0.75, 1.0, -1.0, 0.5), 200, 120) == 119 * 200 + 199
+    assert oracle.pixel(0.125, -0.25, (-0.75, 1.0, -1.0, 0.5), 200, 120) == 60 * 200 + 100
+
+
+def _resolved_chain(cfs, system, render, t):
+    sysh = cfs.cfs_create(system)
+    res = cfs.cfs_host_resolve(sysh, cfs.make_args(render, t=t))
+    sysh.close()
+    return res
+
+
+def test_host_resolved_pinhole_both_sides(cfs, oracle):
+    G = _golden_values("host_resolved.txt")
+    w = W.config(4)
+    res = _resolved_chain(cfs, w.system, w.render, 0.0)
+    assert res["chain_type"] == [6]
+    lib_p = res["chain_p"][0]
+    ty, orc_p = oracle.resolve_xform(W.PINHOLE, 3, 0.0, 3840, 2160)
+    for p in (lib_p, orc_p):
+        assert float(p[0]) == G["pinhole60_fx_3840x2160"] and float(p[1]) == G["pinhole60_fy"]
+        assert float(p[2]) == -4.0 and float(p[3]) == float(np.float32(1e-3))
+    ph90 = W.Xform("pinhole", [90.0, -2.0, 0.0])
+    sys90 = W.System(3, "ifs", W.menger_funcs(), [ph90], "map_index", W.palette_for(20))
+    res = _resolved_chain(cfs, sys90, w.scaled(width=1920, height=1080).render, 0.0)
+    ty, orc_p = oracle.resolve_xform(ph90, 3, 0.0, 1920, 1080)
+    for p in (res["chain_p"][0], orc_p):
+        assert abs(float(p[1]) - G["pinhole90_fy"]) <= 6e-8 and abs(float(p[0]) - G["pinhole90_fx_1920x1080"]) <= 4e-8
+
+
+def test_host_resolved_rotate_z_both_sides(cfs, oracle):
+    G = _golden_values("host_resolved.txt")
+    w = W.config(2)
+    rot = w.system.chain[0]
+    for t, tag in ((0.25, "quarter"), (float(np.float32(1.0 / 3.0)), "third")):
+        c, s = G[f"rotate_{tag}_c"], G[f"rotate_{tag}_s"]
+        res = _resolved_chain(cfs, w.system, w.render, t)
+        assert res["chain_type"][0] == 0                      # ROTATE_Z became an AFFINE
+        ty, orc_p = oracle.resolve_xform(rot, 2, t, 8, 8)
+        assert ty == 0
+        for p in (res["chain_p"][0], orc_p):                  # a00 a01 a10 a11 b0 b1 = c -s s c 0 0
+            assert [float(v) for v in p[:6]] == [c, -s, s, c, 0.0, 0.0], (tag, list(p[:6]))
+    # 3-D: about z, row-major 3x3
+    sys3 = W.System(3, "ifs", W.menger_funcs(), [rot, W.PINHOLE], "map_index", W.palette_for(20))
+    res = _resolved_chain(cfs, sys3, W.config(4).render, 0.25)
+    c, s = G["rotate_quarter_c"], G["rotate_quarter_s"]
+    ty, orc_p = oracle.resolve_xform(rot, 3, 0.25, 8, 8)
+    for p in (res["chain_p"][0], orc_p):
+        assert [float(v) for v in p[:12]] == [c, -s, 0.0, s, c, 0.0, 0.0, 0.0, 1.0, 0.0, 0.0, 0.0]
+
+
+@pytest.mark.parametrize("name,entry", PACK_CASES)
+def test_host_resolved_rgba8_library(cfs, name, entry):
+    want = _golden_values("host_resolved.txt")[name]
+    sysh = cfs.cfs_create(_pack_system(entry))
+    res = cfs.cfs_host_resolve(sysh, cfs.make_args(W.Render(1, 1, 2, 0, 16, 16, (-1, 1, -1, 1), "depth_u64")))
+    sysh.close()
+    assert res["pal8"][0] == want and res["pal8"][1] == 0x09090909
+
+
+def test_pinhole_arguments_are_validated(cfs):
+    """ADVICE: near < 0 with DEPTH output, fov outside (0, 180) -> INVALID_ARG (the depth key orders like
+    the depth only for d > 0)."""
+    r = W.Render(1, 1, 2, 0, 16, 16, (-1, 1, -1, 1), "depth_u64")
+    for bad in ([60.0, -4.0, -0.5], [0.0, -4.0, 1e-3], [180.0, -4.0, 1e-3], [360.0, -4.0, 1e-3], [-20.0, -4.0, 1e-3]):
+        sysb = W.System(3, "ifs", W.menger_funcs(), [W.Xform("pinhole", bad)], "map_index", W.palette_for(20))
+        sysh = cfs.cfs_create(sysb)
+        with pytest.raises(cfs.CfsError) as ei:
+            cfs.cfs_host_resolve(sysh, cfs.make_args(r))
+        assert ei.value.status == cfs.CFS_ERR_INVALID_ARG
+        sysh.close()
