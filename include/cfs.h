@@ -75,13 +75,13 @@ typedef struct { int32_t type; float prob; float params[12]; } cfs_func;
  *               to its own copy of the generated point and splatted, so a point drives M splats per iteration
  *               ("many objects from a single primitive"); the image equals the sum (DEPTH: the
  *               min) of the M single-chain renders.  Not with reuse; DEPTH needs every branch to end in PINHOLE.
- *               Runs on the chain interpreter; cfs_trace does not serve it.
+ *               Runs on the chain interpreter, or compiled in with CFS_FLAG_JIT; cfs_trace does not serve it.
  *   SCATTER     p = (D, rx, ry, rz), D a whole number in [1, 2^20]: PRNG-placed duplicates of an object
  *               (DESIGN R14).  The copy moves onto duplicate d = floor(w D / 2^32), w = word it & 3
  *               of Philox(seed; point lo, point hi, it >> 2, domain 2); its offset is (u(v0) rx, u(v1) ry, u(v2) rz)
  *               with v = Philox(seed; d, 0, 0, domain 3) and u the 24-bit map to [-1, 1) of the point init --
  *               a pure function of (seed, d), nothing is stored.  Exact float32 (one multiply, one add per
- *               coordinate).  Runs on the chain interpreter. */
+ *               coordinate).  Runs on the chain interpreter, or compiled in with CFS_FLAG_JIT. */
 typedef enum {
     CFS_T_AFFINE = 0, CFS_T_SWIRL = 1, CFS_T_SINUSOIDAL = 2, CFS_T_ROTATE_Z = 3,
     CFS_T_TWIST_Z = 4, CFS_T_BEND = 5, CFS_T_PINHOLE = 6, CFS_T_STRETCH_COS = 7, CFS_T_BRANCH = 8,
@@ -131,8 +131,16 @@ typedef enum {
  *   of four) straight to L2 with red.global and only the rest through the tile bins, so that the
  *   L2 reduction units, the issue slots of pass 1 and the shared-memory atomics of pass 2 are all
  *   busy.  Same image (HIST sums are exact; RGBA sums are order-free, DESIGN R8).  CFS_VARIANT_AUTO
- *   sets it whenever it chooses the tile bins; CFS_VARIANT_BINNED takes it from the caller. */
-typedef enum { CFS_FLAG_FAST_TRIG = 1, CFS_FLAG_INTERPRET_CHAIN = 2, CFS_FLAG_BIN_PASS1_ONLY = 4,
+ *   sets it whenever it chooses the tile bins; CFS_VARIANT_BINNED takes it from the caller.
+ *   JIT: run-time specialisation (the chain is spliced into one fused kernel at run time; here by
+ *   NVRTC).  The render uses a kernel compiled in this process for exactly this system -- dimension, generator
+ *   form, splat sink, the chain unrolled with every step's type fixed, BRANCH / SCATTER / reuse / the Eq. 1
+ *   generator included -- instead of the ahead-of-time kernels (which exist for the BASELINE chains only) or the
+ *   chain interpreter.  The first use of a kernel pays its compilation (cfs_specialize() does it ahead of the
+ *   render and reports the time; PAPER L200 quotes 0.745 s against 0.0215 s per frame for the paper's own
+ *   system); kernels are cached in the process and, when $CFS_JIT_CACHE names a directory, on disk.  Same
+ *   device functions, same results as the other two ways.  UNSUPPORTED when NVRTC cannot be loaded. */
+typedef enum { CFS_FLAG_FAST_TRIG = 1, CFS_FLAG_INTERPRET_CHAIN = 2, CFS_FLAG_BIN_PASS1_ONLY = 4, CFS_FLAG_JIT = 8,
                CFS_FLAG_BIN_HYBRID = 0x100 } cfs_render_flags;
 
 /* one 16-byte record of a stored cloud (BASELINE cfg 3); rgba8 = r | g<<8 | b<<16 | a<<24 */
@@ -176,6 +184,21 @@ typedef struct {
  * Errors: INVALID_ARG, UNSUPPORTED (variant impossible for the mode
  * or image), CUDA (launch failure; message holds the CUDA error string). */
 cfs_status cfs_render(const cfs_system *sys, const cfs_render_args *args, void *cuda_stream);
+
+/* cfs_specialize -- compile now (NVRTC, sm_100a) and cache every kernel a cfs_render of this system with these
+ * arguments and CFS_FLAG_JIT may launch (the direct sink of the output mode, the tile-bin pass 1 where the bins can
+ * serve, the Hi-Z kernel for DEPTH), so that no render pays for compilation.  *out_compile_ms (optional) receives
+ * the milliseconds this call spent compiling and loading (0 when everything was cached already).  Needs a
+ * CUDA device (the module is loaded into its context).  PAPER L37, L182, L200.
+ * Errors: INVALID_ARG as cfs_render; UNSUPPORTED when NVRTC cannot be loaded or the compilation fails (message). */
+cfs_status cfs_specialize(const cfs_system *sys, const cfs_render_args *args, double *out_compile_ms);
+/* cfs_jit_check -- test instrument, no device needed: compile the kernel a CFS_FLAG_JIT render of this system would
+ * use for one splat sink (splat_kind < 0: the direct sink of args->out_mode; 6: the tile-bin pass 1; 8: the Hi-Z
+ * depth kernel) to sm_100a SASS and drop it.  Outputs (optional): size of the cubin, milliseconds NVRTC took. */
+cfs_status cfs_jit_check(const cfs_system *sys, const cfs_render_args *args, int32_t splat_kind,
+                         uint64_t *out_cubin_bytes, double *out_ms);
+/* kernels compiled at run time by this process so far and the milliseconds that took (either may be NULL) */
+void cfs_jit_stats(uint64_t *out_kernels_compiled, double *out_total_ms);
 
 /* bytes of d_scratch with which CFS_VARIANT_BINNED renders args->n_points in ONE chunk (pass 1 +
  * pass 2); 0 when the variant cannot serve this system / output mode / image, or without a device.

@@ -22,12 +22,12 @@ T_TYPE = {"affine": 0, "swirl": 1, "sinusoidal": 2, "rotate_z": 3, "twist_z": 4,
           "pinhole": 6, "stretch_cos": 7, "branch": 8, "scatter": 9}
 COLOR = {"none": 0, "map_index": 1, "point": 2}
 OUT = {"hist_u32": 0, "rgba_f32": 1, "depth_u64": 2}
-FLAGS = {"fast_trig": 1, "interpret_chain": 2, "bin_pass1_only": 4, "bin_hybrid": 0x100}
+FLAGS = {"fast_trig": 1, "interpret_chain": 2, "bin_pass1_only": 4, "jit": 8, "bin_hybrid": 0x100}
 VARIANT = {"auto": 0, "direct": 1, "shared_hist": 2, "warp_agg": 3, "binned": 4, "cluster_hist": 5, "depth_hiz": 6}
 MB = {"red_add_u32": 0, "red_add_v4f32": 1, "atom_min_u64": 2, "ld_u64": 3, "atoms_add_u32": 4,
       "ffma": 5, "imad_wide": 6, "lop3": 7, "mufu": 8, "stream_ld128": 9}
 EXPORTS = ["cfs_create", "cfs_destroy", "cfs_render", "cfs_render_host", "cfs_tonemap", "cfs_trace",
-           "cfs_microbench", "cfs_host_resolve", "cfs_shared_hist_max_bytes", "cfs_binned_scratch_bytes", "cfs_hiz_scratch_bytes", "cfs_binned_plan", "cfs_launch_count", "cfs_last_error",
+           "cfs_microbench", "cfs_host_resolve", "cfs_specialize", "cfs_jit_check", "cfs_jit_stats", "cfs_shared_hist_max_bytes", "cfs_binned_scratch_bytes", "cfs_hiz_scratch_bytes", "cfs_binned_plan", "cfs_launch_count", "cfs_last_error",
            "cfs_version"]
 
 
@@ -95,6 +95,12 @@ def lib():
         L.cfs_microbench.restype = C.c_int
         L.cfs_host_resolve.argtypes = [C.c_void_p, C.POINTER(cfs_render_args), C.POINTER(cfs_resolved)]
         L.cfs_host_resolve.restype = C.c_int
+        L.cfs_specialize.argtypes = [C.c_void_p, C.POINTER(cfs_render_args), C.POINTER(C.c_double)]
+        L.cfs_specialize.restype = C.c_int
+        L.cfs_jit_check.argtypes = [C.c_void_p, C.POINTER(cfs_render_args), C.c_int32, C.POINTER(C.c_uint64), C.POINTER(C.c_double)]
+        L.cfs_jit_check.restype = C.c_int
+        L.cfs_jit_stats.argtypes = [C.POINTER(C.c_uint64), C.POINTER(C.c_double)]
+        L.cfs_jit_stats.restype = None
         L.cfs_shared_hist_max_bytes.argtypes = []
         L.cfs_shared_hist_max_bytes.restype = C.c_uint64
         L.cfs_binned_scratch_bytes.argtypes = [C.c_void_p, C.POINTER(cfs_render_args)]
@@ -251,6 +257,28 @@ def cfs_host_resolve(sys: System, args: cfs_render_args) -> dict:
             "chain_p": [np.array(list(out.chain_p[m]), dtype=np.float32) for m in range(n)],
             "thresholds": [int(out.thresholds[j]) for j in range(int(out.n_thresholds))],
             "pal8": [int(out.pal8[j]) for j in range(int(out.n_funcs))]}
+
+
+def cfs_specialize(sys: System, args: cfs_render_args) -> float:
+    """Compile (NVRTC) and cache the kernels a CFS_FLAG_JIT render of this system will launch; returns the
+    milliseconds spent compiling in this call (0.0 when they were cached)."""
+    ms = C.c_double(0.0)
+    _check(lib().cfs_specialize(sys.handle, C.byref(args), C.byref(ms)))
+    return float(ms.value)
+
+
+def cfs_jit_check(sys: System, args: cfs_render_args, splat_kind: int = -1):
+    """Compile-only (no device needed): (cubin bytes, milliseconds) of the kernel a CFS_FLAG_JIT render would use."""
+    nbytes, ms = C.c_uint64(0), C.c_double(0.0)
+    _check(lib().cfs_jit_check(sys.handle, C.byref(args), int(splat_kind), C.byref(nbytes), C.byref(ms)))
+    return int(nbytes.value), float(ms.value)
+
+
+def cfs_jit_stats():
+    """(kernels compiled at run time so far, milliseconds that took)."""
+    n, ms = C.c_uint64(0), C.c_double(0.0)
+    lib().cfs_jit_stats(C.byref(n), C.byref(ms))
+    return int(n.value), float(ms.value)
 
 
 def cfs_render(sys: System, args: cfs_render_args, stream=None) -> None:

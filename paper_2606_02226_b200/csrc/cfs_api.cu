@@ -6,6 +6,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <cstdlib>
 #include <map>
 #include <mutex>
 #include <new>
@@ -14,7 +15,9 @@
 
 #include "../../include/cfs.h"
 #include "cfs_bin.cuh"
+#include "cfs_cloud.cuh"
 #include "cfs_hiz.cuh"
+#include "cfs_jit.h"
 #include "cfs_device.cuh"
 #include "cfs_microbench.cuh"
 #include "cfs_registry.h"
@@ -279,7 +282,7 @@ using cfs::RenderParams;
 cfs_status build_params(const cfs_system *s, const cfs_render_args *a, RenderParams *out, bool need_image)
 {
     if (!s || !a) return fail(CFS_ERR_INVALID_ARG, "system or args is NULL");
-    if (a->flags & ~(CFS_FLAG_FAST_TRIG | CFS_FLAG_INTERPRET_CHAIN | CFS_FLAG_BIN_PASS1_ONLY | CFS_FLAG_BIN_HYBRID)) return fail(CFS_ERR_INVALID_ARG, "unknown flags 0x%x", a->flags);
+    if (a->flags & ~(CFS_FLAG_FAST_TRIG | CFS_FLAG_INTERPRET_CHAIN | CFS_FLAG_BIN_PASS1_ONLY | CFS_FLAG_JIT | CFS_FLAG_BIN_HYBRID)) return fail(CFS_ERR_INVALID_ARG, "unknown flags 0x%x", a->flags);
     if (a->iterations < 1) return fail(CFS_ERR_INVALID_ARG, "iterations must be >= 1");
     if (a->burn_in < 0 || a->burn_in >= a->iterations) return fail(CFS_ERR_INVALID_ARG, "burn_in must be in [0, iterations)");
     if (s->gen == CFS_GEN_CLOUD && (a->iterations != 1 || a->burn_in != 0)) return fail(CFS_ERR_INVALID_ARG, "CLOUD generator needs iterations = 1, burn_in = 0");
@@ -401,30 +404,100 @@ uint32_t chain_signature(const RenderParams &p)
     return sig;
 }
 
-// the kernel compiled for this chain when there is one (and the caller did not ask for the
-// interpreter), else the interpreter; both evaluate the same device functions
-render_fn pick_kernel(const cfs_system *s, const RenderParams &p, int splat, int flags)
+// A kernel to launch: an ahead-of-time instantiation linked into the library, or a run-time-compiled one
+// (cfs_jit.h).  Both are instantiations of the same templates.
+struct Kernel {
+    render_fn aot = nullptr;
+    cfs::JitKernel jit;
+    bool compiled_chain = false;     // the chain is compiled in (not the interpreter)
+    bool ok() const { return aot != nullptr || jit.func != nullptr; }
+};
+
+bool is_cloud_stream(const cfs_system *s, int splat)
 {
-    const int trig = (flags & CFS_FLAG_FAST_TRIG) ? cfs::TRIG_FAST : cfs::TRIG_ACCURATE;
-    if (!(flags & CFS_FLAG_INTERPRET_CHAIN) && p.n_chain > 0 && !p.reuse && p.n_branches == 1) {
-        const uint32_t sig = chain_signature(p);
-        render_fn fn = (s->dim == 2) ? cfs::lookup_render_static2d(s->gen, s->aff, splat, sig, trig)
-                                     : cfs::lookup_render_static3d(s->gen, s->aff, splat, sig, trig);
-        if (fn) return fn;
-    }
-    return cfs::lookup_render_generic(s->dim, s->gen, s->aff, splat);
+    return s->gen == CFS_GEN_CLOUD && (splat == cfs::SPLAT_HIST_DIRECT || splat == cfs::SPLAT_RGBA || splat == cfs::SPLAT_DEPTH);
 }
 
-render_fn pick_trace(const cfs_system *s, const RenderParams &p, int flags)
+// run-time compilation is used when the render asks for it (CFS_FLAG_JIT), or for every render of the process
+// when $CFS_FORCE_JIT is set (kernel development) -- never together with CFS_FLAG_INTERPRET_CHAIN
+bool wants_jit(int flags)
 {
-    const int trig = (flags & CFS_FLAG_FAST_TRIG) ? cfs::TRIG_FAST : cfs::TRIG_ACCURATE;
-    if (!(flags & CFS_FLAG_INTERPRET_CHAIN) && p.n_chain > 0 && !p.reuse && p.n_branches == 1) {
-        const uint32_t sig = chain_signature(p);
-        render_fn fn = (s->dim == 2) ? cfs::lookup_trace_static2d(s->gen, s->aff, sig, trig)
-                                     : cfs::lookup_trace_static3d(s->gen, s->aff, sig, trig);
-        if (fn) return fn;
+    if (flags & CFS_FLAG_INTERPRET_CHAIN) return false;
+    if (flags & CFS_FLAG_JIT) return true;
+    static const bool forced = [] { const char *e = getenv("CFS_FORCE_JIT"); return e && *e && *e != '0'; }();
+    return forced;
+}
+
+int trig_of(uint32_t sig, int flags)
+{
+    return ((flags & CFS_FLAG_FAST_TRIG) && cfs::sig_has_trig(sig)) ? cfs::TRIG_FAST : cfs::TRIG_ACCURATE;
+}
+
+// The kernel for this render and splat sink.  Order: run-time compiled (when asked for), the kernel compiled
+// ahead of time for the chain's signature when there is one, else the chain interpreter; all evaluate the
+// same device functions.  UNSUPPORTED + message when CFS_FLAG_JIT was given and compilation is impossible.
+cfs_status pick_kernel(const cfs_system *s, const RenderParams &p, int splat, int flags, Kernel *out)
+{
+    *out = Kernel();
+    const uint32_t sig = chain_signature(p);
+    if (wants_jit(flags) && splat != cfs::SPLAT_HIST_CLUSTER) {
+        const int opt = p.reuse ? cfs::OPT_REUSE : 0;
+        const std::string name = is_cloud_stream(s, splat)
+            ? cfs::jit_cloud_name(s->dim, splat, sig, trig_of(sig, flags), opt)
+            : cfs::jit_render_name(s->dim, s->gen, s->gen == CFS_GEN_CLOUD ? (int)cfs::AFF_GENERAL : s->aff, splat, sig, trig_of(sig, flags), opt);
+        std::string err;
+        if (cfs::jit_get(name, &out->jit, &err)) { out->compiled_chain = true; return CFS_OK; }
+        if (flags & CFS_FLAG_JIT) return fail(CFS_ERR_UNSUPPORTED, "%s", err.c_str());
+        *out = Kernel();                       // $CFS_FORCE_JIT only: fall back to what is linked in
     }
-    return cfs::lookup_trace_generic(s->dim, s->gen, s->aff);
+    if (!(flags & CFS_FLAG_INTERPRET_CHAIN) && p.n_chain > 0 && !p.reuse && p.n_branches == 1) {
+        const int trig = (flags & CFS_FLAG_FAST_TRIG) ? cfs::TRIG_FAST : cfs::TRIG_ACCURATE;
+        out->aot = (s->dim == 2) ? cfs::lookup_render_static2d(s->gen, s->aff, splat, sig, trig)
+                                 : cfs::lookup_render_static3d(s->gen, s->aff, splat, sig, trig);
+        if (out->aot) { out->compiled_chain = true; return CFS_OK; }
+    }
+    out->aot = cfs::lookup_render_generic(s->dim, s->gen, s->aff, splat);
+    if (!out->aot) return fail(CFS_ERR_UNSUPPORTED, "no kernel for dim %d / generator form %d / splat %d", s->dim, s->aff, splat);
+    return CFS_OK;
+}
+
+cfs_status pick_trace(const cfs_system *s, const RenderParams &p, int flags, Kernel *out)
+{
+    *out = Kernel();
+    const uint32_t sig = chain_signature(p);
+    if (wants_jit(flags) && !p.reuse) {
+        std::string err;
+        const std::string name = cfs::jit_trace_name(s->dim, s->gen, s->gen == CFS_GEN_CLOUD ? (int)cfs::AFF_GENERAL : s->aff, sig, trig_of(sig, flags));
+        if (cfs::jit_get(name, &out->jit, &err)) { out->compiled_chain = true; return CFS_OK; }
+        if (flags & CFS_FLAG_JIT) return fail(CFS_ERR_UNSUPPORTED, "%s", err.c_str());
+        *out = Kernel();
+    }
+    if (!(flags & CFS_FLAG_INTERPRET_CHAIN) && p.n_chain > 0 && !p.reuse && p.n_branches == 1) {
+        const int trig = (flags & CFS_FLAG_FAST_TRIG) ? cfs::TRIG_FAST : cfs::TRIG_ACCURATE;
+        out->aot = (s->dim == 2) ? cfs::lookup_trace_static2d(s->gen, s->aff, sig, trig)
+                                 : cfs::lookup_trace_static3d(s->gen, s->aff, sig, trig);
+        if (out->aot) { out->compiled_chain = true; return CFS_OK; }
+    }
+    out->aot = cfs::lookup_trace_generic(s->dim, s->gen, s->aff);
+    if (!out->aot) return fail(CFS_ERR_UNSUPPORTED, "no trace kernel for dim %d / generator form %d", s->dim, s->aff);
+    return CFS_OK;
+}
+
+// one launch of either kind; dynamic shared memory beyond the default is opted into once per kernel
+cfs_status launch(const Kernel &k, unsigned grid, unsigned block, size_t dyn, cudaStream_t st, const RenderParams &p, const char *what)
+{
+    if (k.jit.func) {
+        std::string err;
+        if (cfs::jit_launch(k.jit, grid, block, dyn, st, p, &err) != cudaSuccess) return fail(CFS_ERR_CUDA, "%s: %s", what, err.c_str());
+        ++g_launches;
+        return CFS_OK;
+    }
+    cudaError_t e;
+    if (dyn > 48 * 1024 && (e = ensure_dyn_smem((const void *)k.aot, dyn)) != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute");
+    k.aot<<<grid, block, dyn, st>>>(p);
+    ++g_launches;
+    if ((e = cudaGetLastError()) != cudaSuccess) return cuda_fail(e, what);
+    return CFS_OK;
 }
 
 size_t shared_hist_limit(const DeviceInfo &di)
@@ -650,8 +723,10 @@ cfs_status render_cluster_hist(const cfs_system *s, const cfs_render_args *a, Re
     const size_t hist_bytes = (size_t)a->width * a->height * 4;
     const int shift = cluster_slice_shift(hist_bytes, di);
     if (shift < 0) return fail(CFS_ERR_UNSUPPORTED, "image of %zu bytes does not fit the shared memory of a %d-CTA cluster", hist_bytes, cfs::kClusterSize);
-    render_fn fn = pick_kernel(s, p, cfs::SPLAT_HIST_CLUSTER, a->flags);
-    if (!fn) return fail(CFS_ERR_UNSUPPORTED, "no cluster-histogram kernel for this system");
+    Kernel kc;
+    cfs_status ks = pick_kernel(s, p, cfs::SPLAT_HIST_CLUSTER, a->flags, &kc);
+    if (ks != CFS_OK) return ks;
+    render_fn fn = kc.aot;
     const size_t dyn = (size_t)4 << shift;
     cudaError_t e = ensure_dyn_smem((const void *)fn, dyn);
     if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute");
@@ -686,14 +761,12 @@ cfs_status render_binned(const cfs_system *s, const cfs_render_args *a, RenderPa
     if (!a->d_scratch) return fail(CFS_ERR_UNSUPPORTED, "binned variant needs d_scratch (see cfs_binned_scratch_bytes)");
     const uint64_t spp = (uint64_t)(a->iterations - a->burn_in) * branches_of(s);
     if (!bin_layout(&pl, a->d_scratch, a->scratch_bytes, a->n_points, spp, &why)) return fail(CFS_ERR_UNSUPPORTED, "%s", why);
-    render_fn fn1 = pick_kernel(s, p, cfs::SPLAT_BIN, a->flags);
-    if (!fn1) return fail(CFS_ERR_UNSUPPORTED, "no binned kernel for dim %d", s->dim);
-    render_fn fn2 = (a->out_mode == CFS_OUT_HIST_U32) ? cfs::bin_accumulate_kernel<0> : cfs::bin_accumulate_kernel<1>;
+    Kernel k1;
+    cfs_status ks = pick_kernel(s, p, cfs::SPLAT_BIN, a->flags, &k1);
+    if (ks != CFS_OK) return ks;
+    Kernel k2;
+    k2.aot = (a->out_mode == CFS_OUT_HIST_U32) ? cfs::bin_accumulate_kernel<0> : cfs::bin_accumulate_kernel<1>;
     cudaError_t e;
-    if ((e = ensure_dyn_smem((const void *)fn1, pl.smem_pass1)) != cudaSuccess)
-        return cuda_fail(e, "cudaFuncSetAttribute(pass 1)");
-    if ((e = ensure_dyn_smem((const void *)fn2, pl.smem_pass2)) != cudaSuccess)
-        return cuda_fail(e, "cudaFuncSetAttribute(pass 2)");
     p.bin = pl.bp;
     p.bin.hybrid = ((a->flags & CFS_FLAG_BIN_HYBRID) || a->variant == CFS_VARIANT_AUTO) ? 1u : 0u;
     const uint64_t total = a->n_points, first = a->point_offset;
@@ -703,13 +776,9 @@ cfs_status render_binned(const cfs_system *s, const cfs_render_args *a, RenderPa
         p.point_offset = first + done;
         if ((e = cudaMemsetAsync(pl.bp.ctrl, 0, pl.clear_bytes, st)) != cudaSuccess) return cuda_fail(e, "clear bin heads");
         // always the full persistent grid: pass 2 reads the tail word of every (tile, CTA)
-        fn1<<<pl.grid1, cfs::kBinThreads, pl.smem_pass1, st>>>(p);
-        ++g_launches;
-        if (!(a->flags & CFS_FLAG_BIN_PASS1_ONLY)) {
-            fn2<<<pl.bp.n_tiles * pl.bp.split, cfs::kBinAccThreads, pl.smem_pass2, st>>>(p);
-            ++g_launches;
-        }
-        if ((e = cudaGetLastError()) != cudaSuccess) return cuda_fail(e, "binned render launch");
+        if ((ks = launch(k1, pl.grid1, cfs::kBinThreads, pl.smem_pass1, st, p, "binned render, pass 1")) != CFS_OK) return ks;
+        if (!(a->flags & CFS_FLAG_BIN_PASS1_ONLY) &&
+            (ks = launch(k2, pl.bp.n_tiles * pl.bp.split, cfs::kBinAccThreads, pl.smem_pass2, st, p, "binned render, pass 2")) != CFS_OK) return ks;
     }
     return CFS_OK;
 }
@@ -759,13 +828,13 @@ cfs_status render_depth_hiz(const cfs_system *s, const cfs_render_args *a, Rende
     if (!hiz_plan(a->width, a->height, &pl)) return fail(CFS_ERR_UNSUPPORTED, "image too large for a shared-memory Hi-Z map");
     if (!a->d_scratch || a->scratch_bytes < pl.bytes)
         return fail(CFS_ERR_UNSUPPORTED, "Hi-Z variant needs d_scratch of cfs_hiz_scratch_bytes() = %llu bytes", (unsigned long long)pl.bytes);
-    render_fn fn0 = pick_kernel(s, p, cfs::SPLAT_DEPTH, a->flags);
-    render_fn fn1 = pick_kernel(s, p, cfs::SPLAT_DEPTH_HIZ, a->flags);
-    if (!fn0 || !fn1) return fail(CFS_ERR_UNSUPPORTED, "no depth kernel for dim %d", s->dim);
+    Kernel k0, k1;
+    cfs_status ks;
+    if ((ks = pick_kernel(s, p, cfs::SPLAT_DEPTH, a->flags, &k0)) != CFS_OK) return ks;
+    if ((ks = pick_kernel(s, p, cfs::SPLAT_DEPTH_HIZ, a->flags, &k1)) != CFS_OK) return ks;
     uint16_t *hz = (uint16_t *)(((uintptr_t)a->d_scratch + 255) & ~(uintptr_t)255);
     const size_t dyn = (size_t)pl.n_pad * 2;
-    cudaError_t e = ensure_dyn_smem((const void *)fn1, dyn);
-    if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute");
+    cudaError_t e;
     p.hiz.hz = hz; p.hiz.shift = pl.shift; p.hiz.nbx = pl.nbx; p.hiz.nby = pl.nby; p.hiz.n_pad = pl.n_pad;
     // the map's padding entries are read into shared memory but never indexed; clear them once
     if ((e = cudaMemsetAsync(hz, 0xFF, dyn, st)) != cudaSuccess) return cuda_fail(e, "clear Hi-Z map");
@@ -781,17 +850,16 @@ cfs_status render_depth_hiz(const cfs_system *s, const cfs_render_args *a, Rende
         p.point_offset = off0 + lo; p.n_points = hi - lo;
         if (ph == 0) {
             uint64_t blocks = (p.n_points + cfs::kRenderThreads - 1) / cfs::kRenderThreads;
-            fn0<<<(unsigned)blocks, cfs::kRenderThreads, 0, st>>>(p);
+            if ((ks = launch(k0, (unsigned)blocks, cfs::kRenderThreads, 0, st, p, "Hi-Z render, plain slice")) != CFS_OK) return ks;
         } else {
             const unsigned side = 1u << pl.shift;
             cfs::hiz_build_kernel<<<pl.n, side * side, 0, st>>>((const unsigned long long *)a->d_image, a->width, a->height,
                                                                   pl.shift, pl.nbx, hz);
             ++g_launches;
             uint64_t blocks = (p.n_points + cfs::kHizThreads - 1) / cfs::kHizThreads;
-            fn1<<<(unsigned)blocks, cfs::kHizThreads, dyn, st>>>(p);
+            if ((e = cudaGetLastError()) != cudaSuccess) return cuda_fail(e, "Hi-Z build launch");
+            if ((ks = launch(k1, (unsigned)blocks, cfs::kHizThreads, dyn, st, p, "Hi-Z render")) != CFS_OK) return ks;
         }
-        ++g_launches;
-        if ((e = cudaGetLastError()) != cudaSuccess) return cuda_fail(e, "Hi-Z render launch");
     }
     return CFS_OK;
 }
@@ -852,8 +920,8 @@ static cfs_status render_impl(const cfs_system *s, const cfs_render_args *a, voi
         }
     }
     if (a->n_points == 0) return CFS_OK;
-    render_fn fn = pick_kernel(s, p, splat, a->flags);
-    if (!fn) return fail(CFS_ERR_UNSUPPORTED, "no kernel for dim %d / splat %d", s->dim, splat);
+    Kernel kn;
+    if ((st = pick_kernel(s, p, splat, a->flags, &kn)) != CFS_OK) return st;
 
     const int threads = cfs::kRenderThreads;
     uint64_t blocks = (a->n_points + threads - 1) / threads;
@@ -861,33 +929,102 @@ static cfs_status render_impl(const cfs_system *s, const cfs_render_args *a, voi
     if (splat == cfs::SPLAT_HIST_SHARED) {
         dyn = hist_bytes;
         p.hist_bins = (uint32_t)(hist_bytes / 4);
-        cudaError_t e = ensure_dyn_smem((const void *)fn, dyn);
-        if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute");
     }
     // CLOUD and SHARED_HIST: persistent grid (resident CTAs x SMs), grid-stride over points: one
     // histogram merge per CTA, short per-point work amortises the CTA prologue.  IFS + direct
     // splats: one point per thread, CTAs handed out by the hardware scheduler -- measured faster
     // than a persistent grid (P / resident threads is ~3.5 for configs[1]: the last static trip
     // would run 46 % full; dynamic CTA hand-out has no such tail).
+    if (is_cloud_stream(s, splat)) {
+        // the streaming cloud kernel (cfs_cloud.cuh): persistent CTAs, chunks of records through a shared-memory ring
+        const uint64_t n_chunks = (a->n_points + cfs::kCloudChunk - 1) / cfs::kCloudChunk;
+        uint64_t grid = (uint64_t)di.sms * cfs::kCloudCtasPerSm;
+        if (grid > n_chunks) grid = n_chunks;
+        return launch(kn, (unsigned)grid, cfs::kCloudThreads, cfs::kCloudSmemBytes, (cudaStream_t)stream, p, "cloud kernel launch");
+    }
     if (s->gen == CFS_GEN_CLOUD || splat == cfs::SPLAT_HIST_SHARED) {
+        // resident CTAs per SM: from the occupancy calculator for a linked kernel; a run-time-compiled one of the
+        // same template has the same shape -- the registers allow 8 x 256 threads, shared memory decides
         int per_sm = 1;
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void *)fn, threads, dyn);
+        if (kn.aot) {
+            if (dyn > 48 * 1024) ensure_dyn_smem((const void *)kn.aot, dyn);
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void *)kn.aot, threads, dyn);
+        } else {
+            per_sm = (int)((size_t)di.smem_sm / (dyn + sizeof(cfs::SharedTables) + 2048));
+            if (per_sm > 8) per_sm = 8;
+        }
         if (per_sm < 1) per_sm = 1;
         const uint64_t cap = (uint64_t)di.sms * per_sm;
         if (blocks > cap) blocks = cap;
     } else if (blocks > (1u << 24)) {
         blocks = 1u << 24;
     }
-    fn<<<(unsigned)blocks, threads, dyn, (cudaStream_t)stream>>>(p);
-    ++g_launches;
-    cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) return cuda_fail(e, "render kernel launch");
-    return CFS_OK;
+    return launch(kn, (unsigned)blocks, threads, dyn, (cudaStream_t)stream, p, "render kernel launch");
 }
 
 extern "C" cfs_status cfs_render(const cfs_system *s, const cfs_render_args *a, void *stream)
 {
     return render_impl(s, a, stream, 0);
+}
+
+extern "C" cfs_status cfs_specialize(const cfs_system *s, const cfs_render_args *a, double *out_ms)
+{
+    if (out_ms) *out_ms = 0.0;
+    RenderParams p;
+    cfs_render_args r;
+    if (a) { r = *a; r.d_image = nullptr; r.d_cloud = nullptr; r.flags = (r.flags | CFS_FLAG_JIT) & ~CFS_FLAG_INTERPRET_CHAIN; }
+    cfs_status st = build_params(s, a ? &r : nullptr, &p, false);
+    if (st != CFS_OK) return st;
+    const DeviceInfo &di = device_info();
+    if (di.ok != 1) return fail(CFS_ERR_CUDA, "no CUDA device (this library has no CPU fallback)");
+    int kinds[4], n = 0;
+    if (a->out_mode == CFS_OUT_RGBA_F32) kinds[n++] = cfs::SPLAT_RGBA;
+    else if (a->out_mode == CFS_OUT_DEPTH_RGBA8_U64) { kinds[n++] = cfs::SPLAT_DEPTH; if (s->gen == CFS_GEN_IFS) kinds[n++] = cfs::SPLAT_DEPTH_HIZ; }
+    else kinds[n++] = cfs::SPLAT_HIST_DIRECT;
+    BinPlan pl;
+    const char *why = "";
+    if (bin_shape(s, &r, di, &pl, &why)) kinds[n++] = cfs::SPLAT_BIN;
+    double ms = 0.0;
+    for (int i = 0; i < n; ++i) {
+        Kernel k;
+        if ((st = pick_kernel(s, p, kinds[i], r.flags, &k)) != CFS_OK) return st;
+        ms += k.jit.compile_ms;
+    }
+    if (out_ms) *out_ms = ms;
+    return CFS_OK;
+}
+
+// compile-only twin of cfs_specialize: no device needed (the cubin is built and dropped)
+extern "C" cfs_status cfs_jit_check(const cfs_system *s, const cfs_render_args *a, int32_t splat_kind, uint64_t *out_cubin_bytes, double *out_ms)
+{
+    RenderParams p;
+    cfs_render_args r;
+    if (a) { r = *a; r.d_image = nullptr; r.d_cloud = nullptr; }
+    cfs_status st = build_params(s, a ? &r : nullptr, &p, false);
+    if (st != CFS_OK) return st;
+    int splat = splat_kind;
+    if (splat < 0) splat = (a->out_mode == CFS_OUT_RGBA_F32) ? cfs::SPLAT_RGBA : (a->out_mode == CFS_OUT_DEPTH_RGBA8_U64) ? cfs::SPLAT_DEPTH : cfs::SPLAT_HIST_DIRECT;
+    const uint32_t sig = chain_signature(p);
+    const int opt = p.reuse ? cfs::OPT_REUSE : 0;
+    const std::string name = is_cloud_stream(s, splat)
+        ? cfs::jit_cloud_name(s->dim, splat, sig, trig_of(sig, a->flags), opt)
+        : cfs::jit_render_name(s->dim, s->gen, s->gen == CFS_GEN_CLOUD ? (int)cfs::AFF_GENERAL : s->aff, splat, sig, trig_of(sig, a->flags), opt);
+    std::string err;
+    size_t bytes = 0;
+    double ms = 0.0;
+    if (!cfs::jit_compile_only(name, &bytes, &ms, &err)) return fail(CFS_ERR_UNSUPPORTED, "%s", err.c_str());
+    if (out_cubin_bytes) *out_cubin_bytes = bytes;
+    if (out_ms) *out_ms = ms;
+    return CFS_OK;
+}
+
+extern "C" void cfs_jit_stats(uint64_t *out_n, double *out_ms)
+{
+    unsigned long long n = 0;
+    double ms = 0.0;
+    cfs::jit_stats(&n, &ms);
+    if (out_n) *out_n = n;
+    if (out_ms) *out_ms = ms;
 }
 
 // host-only view of what a render resolves before its launch (no device needed): lets the CPU tests pin the
@@ -925,14 +1062,11 @@ extern "C" cfs_status cfs_trace(const cfs_system *s, const cfs_render_args *a, u
     if (p.n_branches > 1) return fail(CFS_ERR_UNSUPPORTED, "cfs_trace does not serve chains with BRANCH markers");
     p.tr_picks = d_picks; p.tr_g = d_final_g; p.tr_q = d_final_q; p.tr_alive = d_alive;
     p.counters = nullptr;
-    render_fn fn = pick_trace(s, p, a->flags);
+    Kernel kt;
+    if ((st = pick_trace(s, p, a->flags, &kt)) != CFS_OK) return st;
     uint64_t blocks = (a->n_points + cfs::kRenderThreads - 1) / cfs::kRenderThreads;
     if (blocks > (1u << 22)) blocks = 1u << 22;
-    fn<<<(unsigned)blocks, cfs::kRenderThreads, 0, (cudaStream_t)stream>>>(p);
-    ++g_launches;
-    cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) return cuda_fail(e, "trace kernel launch");
-    return CFS_OK;
+    return launch(kt, (unsigned)blocks, cfs::kRenderThreads, 0, (cudaStream_t)stream, p, "trace kernel launch");
 }
 
 // -------------------------------------------------------------------------------------------------

@@ -15,8 +15,10 @@
 // splat cannot change the result.  Depths are positive floats, so their bit patterns order like
 // the values; an empty pixel (all ones) gives 0xFFFF, which culls nothing.
 #pragma once
+#ifndef __CUDACC_RTC__
 #include <cuda_runtime.h>
 #include <stdint.h>
+#endif
 
 #include "cfs_params.h"
 

@@ -4,7 +4,25 @@
 // arguments"): no device-side table allocation, launches are asynchronous and
 // graph-capturable.  ~5.5 KB, inside the 32 KB parameter space of sm_70+ / CUDA >= 12.1.
 #pragma once
+#ifdef __CUDACC_RTC__
+// run-time compilation (cfs_jit.cu): NVRTC has no host headers; the fixed-width types are spelled out
+typedef signed char int8_t;
+typedef unsigned char uint8_t;
+typedef short int16_t;
+typedef unsigned short uint16_t;
+typedef int int32_t;
+typedef unsigned int uint32_t;
+typedef long long int64_t;
+typedef unsigned long long uint64_t;
+#else
 #include <stdint.h>
+#endif
+
+#ifdef __CUDACC__
+#define CFS_HD __host__ __device__
+#else
+#define CFS_HD
+#endif
 
 namespace cfs {
 
@@ -23,13 +41,30 @@ enum TrigKind : int { TRIG_ACCURATE = 0, TRIG_FAST = 1, TRIG_RUNTIME = 2 /* prm.
 // A kernel compiled for a signature has the chain unrolled with every parameter a fixed constant
 // operand; kChainGeneric selects the interpreter (unrolled to kMaxChain steps, warp-uniform switch).
 constexpr uint32_t kChainGeneric = 0xFFFFFFFFu;
-constexpr uint32_t chain_sig(int a = -1, int b = -1, int c = -1, int d = -1)
+CFS_HD constexpr uint32_t chain_sig(int a = -1, int b = -1, int c = -1, int d = -1)
 {
     return (uint32_t)(a + 1) | ((uint32_t)(b + 1) << 4) | ((uint32_t)(c + 1) << 8) | ((uint32_t)(d + 1) << 12);
 }
+// type of step m of a signature, -1 past its end
+CFS_HD constexpr int sig_step(uint32_t sig, int m)
+{
+    return (sig == kChainGeneric || m < 0 || m >= kMaxChain) ? -1 : (int)((sig >> (4 * m)) & 15u) - 1;
+}
+// kernel options compiled in (template argument OPT of render_kernel / cloud_kernel)
+enum KernelOpt : int {
+    OPT_REUSE = 1          // Fig. 2(C): the chain output is fed back into the generator (compiled chains; the interpreter reads prm.reuse)
+};
+// true when the signature holds a BRANCH separator (type 8): one-to-many splatting
+CFS_HD constexpr bool sig_has_branch(uint32_t sig)
+{
+    if (sig == kChainGeneric) return false;
+    for (int m = 0; m < kMaxChain; ++m)
+        if (sig_step(sig, m) == 8) return true;
+    return false;
+}
 // true when a step of the signature evaluates sin/cos (types 1 SWIRL, 2 SINUSOIDAL, 4 TWIST_Z,
 // 5 BEND, 7 STRETCH_COS); the generic signature may
-constexpr bool sig_has_trig(uint32_t sig)
+CFS_HD constexpr bool sig_has_trig(uint32_t sig)
 {
     if (sig == kChainGeneric) return true;
     for (int m = 0; m < 8; ++m) {

@@ -67,16 +67,35 @@ __device__ __forceinline__ uint32_t splat_q(const RenderParams &prm, const Share
                                             float qx, float qy, float qz, bool alive, int k, uint32_t point_rgba8,
                                             bool have, const BinRegs &br, bool bin_direct_half);
 
+// one branch of a compiled one-to-many chain, then the branches after it: every branch gets its own
+// copy of the generated point and its own splat; the structure is fixed at compile time
+template <int DIM, int GEN, int SPLAT, uint32_t SIG, int TRIG, int M>
+__device__ __forceinline__ uint32_t branches_static(const RenderParams &prm, const SharedTables &s, const Sm &sm, uint32_t *s_hist,
+                                                    float gx, float gy, float gz, int k, uint32_t point_rgba8, bool have,
+                                                    const BinRegs &br, const StepCtx &ctx, bool bin_direct_half)
+{
+    float qx = gx, qy = gy, qz = gz;
+    const bool alive = chain_static<DIM, SIG, TRIG, M>(prm, ctx, qx, qy, qz);
+    uint32_t dropped = splat_q<DIM, GEN, SPLAT>(prm, s, sm, s_hist, qx, qy, qz, alive, k, point_rgba8, have, br, bin_direct_half);
+    constexpr int next = sig_next_branch(SIG, M);
+    if constexpr (next >= 0)
+        dropped += branches_static<DIM, GEN, SPLAT, SIG, TRIG, next>(prm, s, sm, s_hist, gx, gy, gz, k, point_rgba8, have, br, ctx, bin_direct_half);
+    return dropped;
+}
+
 // rows 5-7 for one generated point: copy -> chain -> pixel -> reduction.  `k` is the map applied
 // in this iteration (colour rule MAP_INDEX), `point_rgba8` the record colour (POINT).
-// Returns 1 when the splat was dropped (dead or out of bounds), else 0.  Fig. 2(C) reuse is a
-// run-time option of the interpreter kernels only (compiled chains are never used with it).
-template <int DIM, int GEN, int SPLAT, uint32_t SIG, int TRIG>
+// Returns the number of dropped splats (dead or out of bounds).  Fig. 2(C) reuse: a run-time option of the
+// interpreter (prm.reuse), a compile-time one (OPT_REUSE) of a kernel compiled for the chain.
+template <int DIM, int GEN, int SPLAT, uint32_t SIG, int TRIG, int OPT>
 __device__ __forceinline__ uint32_t chain_and_splat(const RenderParams &prm, const SharedTables &s, const Sm &sm, uint32_t *s_hist,
                                                     float &gx, float &gy, float &gz, int k, uint32_t point_rgba8,
                                                     bool have, bool past_burn_in, const BinRegs &br, const StepCtx &ctx,
                                                     bool bin_direct_half = false)
 {
+    if constexpr (SIG != kChainGeneric && sig_has_branch(SIG)) {
+        return branches_static<DIM, GEN, SPLAT, SIG, TRIG, 0>(prm, s, sm, s_hist, gx, gy, gz, k, point_rgba8, have, br, ctx, bin_direct_half);
+    }
     if (SIG == kChainGeneric && prm.n_branches > 1) {
         // one-to-many ("many objects from a single primitive"): every BRANCH of the chain
         // gets its own copy of the generated point and its own splat.  The markers sit in the parameter
@@ -96,7 +115,7 @@ __device__ __forceinline__ uint32_t chain_and_splat(const RenderParams &prm, con
     }
     float qx = gx, qy = gy, qz = gz;            // the copy of Fig. 2(B)
     const bool alive = apply_chain<DIM, SIG, TRIG>(prm, ctx, qx, qy, qz);
-    if (SIG == kChainGeneric && prm.reuse) {    // Fig. 2(C): the same point is reused
+    if ((SIG == kChainGeneric) ? (prm.reuse != 0) : ((OPT & OPT_REUSE) != 0)) {    // Fig. 2(C): the same point is reused
         gx = qx; gy = qy; gz = qz;
         if (!past_burn_in) return 0u;
     }
@@ -209,14 +228,15 @@ __device__ __forceinline__ uint32_t bin_block_splat(const RenderParams &prm, con
 // CHECKED = false: the caller guarantees burn_in <= it0 and it0 + 4 <= iterations, so the body
 // has no per-iteration tests (the steady state of a render); CHECKED = true handles burn-in
 // and the ragged last block.
-template <int DIM, int GEN, int AFF, int SPLAT, uint32_t SIG, int TRIG, bool CHECKED>
+template <int DIM, int GEN, int AFF, int SPLAT, uint32_t SIG, int TRIG, int OPT, bool CHECKED>
 __device__ __forceinline__ uint32_t iterate_block(const RenderParams &prm, const SharedTables &s, const Sm &sm, uint32_t *s_hist,
                                                   uint32_t plo, uint32_t phi, int it0, float &gx, float &gy, float &gz,
                                                   bool have, BinLane &bl, const BinRegs &br)
 {
     const U4 w = philox4x32_10(plo, phi, (uint32_t)it0 >> 2, DOMAIN_PICK, prm);
     uint32_t dropped = 0;
-    if constexpr (!CHECKED && SIG != kChainGeneric && SPLAT == SPLAT_BIN) {
+    constexpr bool kReuse = (SIG != kChainGeneric) && (OPT & OPT_REUSE) != 0;
+    if constexpr (!CHECKED && SIG != kChainGeneric && SPLAT == SPLAT_BIN && !sig_has_branch(SIG) && !kReuse) {
         // ALU-bound variant: the generator recurrence is short (LDS + FMAs), the chain and pixel
         // arithmetic of the four iterations are independent of one another once the four generator
         // states exist -- written as straight-line stages so that the four dependent chains
@@ -256,8 +276,8 @@ __device__ __forceinline__ uint32_t iterate_block(const RenderParams &prm, const
             const bool past = !CHECKED || it >= prm.burn_in;
             // hybrid stage (DESIGN "hybrid"): iterations 0 and 2 of a steady-state block splat straight to L2
             const bool direct_half = SPLAT == SPLAT_BIN && !CHECKED && (j & 1) == 0 && prm.bin.hybrid != 0u;
-            if (past || (SIG == kChainGeneric && prm.reuse))
-                dropped += chain_and_splat<DIM, GEN, SPLAT, SIG, TRIG>(prm, s, sm, s_hist, gx, gy, gz, k, 0u, have, past, br,
+            if (past || (SIG == kChainGeneric && prm.reuse) || kReuse)
+                dropped += chain_and_splat<DIM, GEN, SPLAT, SIG, TRIG, OPT>(prm, s, sm, s_hist, gx, gy, gz, k, 0u, have, past, br,
                                                                        StepCtx{plo, phi, it}, direct_half);
         }
     }
@@ -271,7 +291,7 @@ __device__ __forceinline__ uint32_t iterate_block(const RenderParams &prm, const
 
 // ---------------------------------------------------------------------------------------------
 // the kernel
-template <int DIM, int GEN, int AFF, int SPLAT, uint32_t SIG, int TRIG>
+template <int DIM, int GEN, int AFF, int SPLAT, uint32_t SIG, int TRIG, int OPT>
 __global__ void __launch_bounds__(SPLAT == SPLAT_BIN ? kBinThreads : SPLAT == SPLAT_HIST_CLUSTER ? kClusterThreads :
                                   SPLAT == SPLAT_DEPTH_HIZ ? kHizThreads : kRenderThreads,
                                   SPLAT == SPLAT_BIN ? kBinCtasPerSm : SPLAT == SPLAT_DEPTH_HIZ ? kHizCtasPerSm : 0)
@@ -327,7 +347,7 @@ render_kernel(const __grid_constant__ RenderParams prm)
             float4 rec = make_float4(0.f, 0.f, 0.f, 0.f);
             if (have) rec = __ldcs(reinterpret_cast<const float4 *>(prm.cloud) + (p - prm.cloud_base));
             gx = rec.x; gy = rec.y; gz = (DIM == 3) ? rec.z : 0.0f;
-            dropped = chain_and_splat<DIM, GEN, SPLAT, SIG, TRIG>(prm, s, sm, s_hist, gx, gy, gz, 0,
+            dropped = chain_and_splat<DIM, GEN, SPLAT, SIG, TRIG, OPT>(prm, s, sm, s_hist, gx, gy, gz, 0,
                                                                   __float_as_uint(rec.w), have, true, br,
                                                                   StepCtx{(uint32_t)p, (uint32_t)(p >> 32), 0});
         } else {
@@ -342,13 +362,13 @@ render_kernel(const __grid_constant__ RenderParams prm)
             int it0 = 0;
 #pragma unroll 1
             for (; it0 < it_fast0; it0 += 4)
-                dropped += iterate_block<DIM, GEN, AFF, SPLAT, SIG, TRIG, true>(prm, s, sm, s_hist, plo, phi, it0, gx, gy, gz, have, bl, br);
+                dropped += iterate_block<DIM, GEN, AFF, SPLAT, SIG, TRIG, OPT, true>(prm, s, sm, s_hist, plo, phi, it0, gx, gy, gz, have, bl, br);
 #pragma unroll 1
             for (; it0 < it_fast1; it0 += 4)
-                dropped += iterate_block<DIM, GEN, AFF, SPLAT, SIG, TRIG, false>(prm, s, sm, s_hist, plo, phi, it0, gx, gy, gz, have, bl, br);
+                dropped += iterate_block<DIM, GEN, AFF, SPLAT, SIG, TRIG, OPT, false>(prm, s, sm, s_hist, plo, phi, it0, gx, gy, gz, have, bl, br);
 #pragma unroll 1
             for (; it0 < I; it0 += 4)
-                dropped += iterate_block<DIM, GEN, AFF, SPLAT, SIG, TRIG, true>(prm, s, sm, s_hist, plo, phi, it0, gx, gy, gz, have, bl, br);
+                dropped += iterate_block<DIM, GEN, AFF, SPLAT, SIG, TRIG, OPT, true>(prm, s, sm, s_hist, plo, phi, it0, gx, gy, gz, have, bl, br);
         }
         if (have) { n_drop += dropped; n_in += (uint32_t)(I - B) * (uint32_t)prm.n_branches - dropped; }
     }

@@ -1,6 +1,7 @@
 // cfs_select.cuh -- run-time -> compile-time selection helpers shared by the kernel translation units
 #pragma once
 #include "cfs_registry.h"
+#include "cfs_cloud.cuh"
 #include "cfs_render.cuh"
 
 namespace cfs {
@@ -9,9 +10,15 @@ namespace cfs {
 template <int DIM, int GEN, int AFF, uint32_t SIG, int TRIG, unsigned SPLATS>
 render_fn select_splat(int splat)
 {
+    // a stored cloud with a direct sink streams through cloud_kernel (bulk-async record ring); the host
+    // launches it with its own shape (cfs_api.cu is_cloud_stream)
 #define CFS_CASE(K)                                                                   \
     if constexpr ((SPLATS >> K) & 1u) {                                               \
-        if (splat == K) return render_kernel<DIM, GEN, AFF, K, SIG, TRIG>;            \
+        if constexpr (GEN == 1 && (K == SPLAT_HIST_DIRECT || K == SPLAT_RGBA || K == SPLAT_DEPTH)) { \
+            if (splat == K) return cloud_kernel<DIM, K, SIG, TRIG, 0>;                   \
+        } else {                                                                      \
+            if (splat == K) return render_kernel<DIM, GEN, AFF, K, SIG, TRIG, 0>;        \
+        }                                                                             \
     }
     CFS_CASE(SPLAT_HIST_DIRECT)
     CFS_CASE(SPLAT_HIST_SHARED)

@@ -141,3 +141,26 @@ def test_branch_marker_validation(cfs):
     with pytest.raises(cfs.CfsError) as ei:
         cfs.cfs_create(W.System(2, "ifs", W.square_funcs(), a + [W.Xform("branch")] + a, "none", None, reuse=True))
     assert ei.value.status == cfs.CFS_ERR_INVALID_ARG
+
+
+def test_run_time_specialiser_compiles_without_a_device(cfs):
+    """NEXT-4: the kernel templates compile under NVRTC for sm_100a from the sources embedded in
+    the library -- the five BASELINE systems, and chains no ahead-of-time kernel exists for (BRANCH, SCATTER,
+    reuse, the Eq. 1 generator).  Compile-only: no device needed."""
+    for cfg in range(W.N_CONFIGS):
+        w = W.config(cfg)
+        sysh = cfs.cfs_create(w.system)
+        nbytes, ms = cfs.cfs_jit_check(sysh, cfs.make_args(w.render, flags=["fast_trig"]))
+        assert nbytes > 10000 and ms > 0.0
+        sysh.close()
+    br = [W.Xform("branch")]
+    chain = [W.Xform("swirl"), W.Xform("affine", [0.6, 0, 0, 0.6, 0.3, -0.2])] + br + \
+            [W.Xform("affine", [0.03, 0, 0, 0.03, 0, 0]), W.Xform("scatter", [64, 0.95, 0.95, 0.0])]
+    r = W.Render(1000, 3, 40, 10, 128, 128, (-1.2, 1.2, -1.2, 1.2), "rgba_f32")
+    for system in (W.System(2, "ifs", W.square_funcs(), chain, "map_index", W.palette_for(4)),
+                   W.System(2, "ifs", W.circle_funcs(True), [W.Xform("stretch_cos")], "map_index", W.palette_for(2), reuse=True)):
+        sysh = cfs.cfs_create(system)
+        for kind in (-1, 6):                       # direct sink and the tile-bin pass 1
+            nbytes, _ = cfs.cfs_jit_check(sysh, cfs.make_args(r), kind)
+            assert nbytes > 10000
+        sysh.close()
