@@ -127,11 +127,12 @@ typedef enum {
  *   BIN_PASS1_ONLY: measurement instrument of the BINNED variant: run pass 1 (sample + bin) and
  *   skip pass 2, so the two passes can be timed apart with events; the image is NOT updated
  *   (with BIN_HYBRID it receives the direct half only).
- *   BIN_HYBRID: the BINNED variant sends every other splat (iterations 0 and 2 of each Philox block
- *   of four) straight to L2 with red.global and only the rest through the tile bins, so that the
- *   L2 reduction units, the issue slots of pass 1 and the shared-memory atomics of pass 2 are all
- *   busy.  Same image (HIST sums are exact; RGBA sums are order-free, DESIGN R8).  CFS_VARIANT_AUTO
- *   sets it whenever it chooses the tile bins; CFS_VARIANT_BINNED takes it from the caller.
+ *   BIN_HYBRID: the BINNED variant sends one splat in four (iteration 0 of each Philox block of four) straight
+ *   to L2 with red.global and the rest through the tile bins, so that the L2 reduction units, the issue slots of
+ *   pass 1 and the shared-memory atomics of pass 2 are all busy.  Same image (HIST sums are exact; RGBA sums are
+ *   order-free, DESIGN R8).  CFS_VARIANT_AUTO sets it whenever it chooses the tile bins; CFS_VARIANT_BINNED takes
+ *   it from the caller.  (Round 1 sent every other splat; with the leaner pass 2 of round 2 one in four measured
+ *   ahead on configs[2] and level on configs[1], DESIGN "hybrid".)
  *   JIT: run-time specialisation (the chain is spliced into one fused kernel at run time; here by
  *   NVRTC).  The render uses a kernel compiled in this process for exactly this system -- dimension, generator
  *   form, splat sink, the chain unrolled with every step's type fixed, BRANCH / SCATTER / reuse / the Eq. 1
@@ -209,8 +210,9 @@ uint64_t cfs_binned_scratch_bytes(const cfs_system *sys, const cfs_render_args *
 
 /* bytes of d_scratch CFS_VARIANT_DEPTH_HIZ needs for a width x height depth image (host arithmetic,
  * no device needed); 0 when the image is too large for a shared-memory Hi-Z map (> 96 KiB at
- * 32 x 32-pixel blocks).  CFS_VARIANT_AUTO does not take this path: on configs[4] it was measured level
- * with the direct one (the direct path is bound by the SM-to-L2 request rate, this one by instruction issue). */
+ * 32 x 32-pixel blocks).  CFS_VARIANT_AUTO takes this path for DEPTH renders of an IFS with at least 2^30 splats
+ * when d_scratch holds that many bytes: the direct path is bound by the SM-to-L2 request rate, this one by
+ * instruction issue -- level as linked ahead of time, ahead when compiled for the system (CFS_FLAG_JIT). */
 uint64_t cfs_hiz_scratch_bytes(int32_t width, int32_t height);
 
 /* the tile plan of the BINNED variant for an image and a device shape, host arithmetic only (no device

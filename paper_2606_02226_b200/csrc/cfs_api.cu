@@ -108,9 +108,10 @@ struct cfs_system {
     std::vector<float> palette;
     // pick tables (DESIGN R2)
     uint32_t T[cfs::kMaxFuncs];
-    uint32_t lut[256];
+    uint32_t lut[256][2];
     int32_t n_thr = 0, pick_steps = 0, pick_shift = -1;
     int32_t aff = cfs::AFF_GENERAL;
+    bool uscale_ok = false;      // AFF_DIAG and every map has the same scale: AFF_USCALE table available (run-time compiled kernels)
     float coef[cfs::kMaxFuncs * 12];
     uint32_t pal8[cfs::kMaxFuncs];
     // scratch of cfs_render_host (device), cached
@@ -161,12 +162,13 @@ cfs_status build_tables(cfs_system *s)
     for (int b = 0; b < 256; ++b) {
         const uint64_t lo = (uint64_t)b << 24, hi = lo + 0xFFFFFFull;
         int below = 0, inside = 0;
-        uint32_t t24 = 1u << 24;                                  // none
+        uint32_t first_m1 = 0xFFFFFFFFu;                          // none: u > 0xFFFFFFFF never holds
         for (int j = 0; j < s->n_thr; ++j) {
             if (T64[j] <= lo) ++below;
-            else if (T64[j] <= hi) { if (!inside) t24 = (uint32_t)(T64[j] - lo); ++inside; }
+            else if (T64[j] <= hi) { if (!inside) first_m1 = (uint32_t)(T64[j] - 1); ++inside; }    // T > lo >= 0, so T - 1 >= 0
         }
-        s->lut[b] = ((uint32_t)below << 25) | t24;
+        s->lut[b][0] = first_m1;
+        s->lut[b][1] = (uint32_t)below;
         if (inside > s->pick_steps) s->pick_steps = inside;
     }
     // equal power-of-two thresholds: k = u >> shift
@@ -188,6 +190,11 @@ cfs_status build_tables(cfs_system *s)
     }
     const bool circle = n >= 1 && s->funcs[0].type == CFS_F_CIRCLE_HALF;     // all of them are (cfs_create)
     s->aff = circle ? cfs::AFF_CIRCLE : diag ? cfs::AFF_DIAG : cfs::AFF_GENERAL;
+    s->uscale_ok = (s->aff == cfs::AFF_DIAG);
+    for (int j = 1; j < n && s->uscale_ok; ++j) {
+        const float *m = s->funcs[j].params, *m0 = s->funcs[0].params;
+        s->uscale_ok = (s->dim == 2) ? (m[0] == m0[0] && m[3] == m0[3]) : (m[0] == m0[0] && m[4] == m0[4] && m[8] == m0[8]);
+    }
     memset(s->coef, 0, sizeof(s->coef));
     for (int j = 0; j < n; ++j) {
         const float *m = s->funcs[j].params;
@@ -324,6 +331,7 @@ cfs_status build_params(const cfs_system *s, const cfs_render_args *a, RenderPar
     p.color_rule = (a->out_mode == CFS_OUT_HIST_U32) ? (int)CFS_COLOR_NONE : s->color;
     p.reuse = s->reuse; p.fast_trig = (a->flags & CFS_FLAG_FAST_TRIG) ? 1 : 0;
     p.pick_shift = s->pick_shift; p.n_thr = s->n_thr; p.pick_steps = s->pick_steps;
+    p.aff_form = s->aff;
     {   // coefficient rows are replicated in shared memory (up to 8 copies) when more than 8 of them are in
         // use: with fewer, every row already has a bank group of its own
         const uint32_t rows_per_map = (s->aff == cfs::AFF_CIRCLE) ? 1u : (s->aff == cfs::AFF_DIAG) ? (s->dim == 2 ? 1u : 2u) : (s->dim == 2 ? 2u : 3u);
@@ -428,6 +436,60 @@ bool wants_jit(int flags)
     return forced;
 }
 
+// which iterations of a steady-state Philox block splat straight to L2 in the tile-binned variant: 0 = none (pure
+// bins); the hybrid stage (CFS_FLAG_BIN_HYBRID, or chosen by AUTO) sends every other one
+uint32_t hybrid_mask(const cfs_render_args *a)
+{
+    if (!((a->flags & CFS_FLAG_BIN_HYBRID) || a->variant == CFS_VARIANT_AUTO)) return 0u;
+    if (const char *e = getenv("CFS_BIN_DIRECT_MASK")) return (uint32_t)atoi(e) & 15u;     // TEMP tuning
+    return 1u;
+}
+
+// generator table form of a run-time compiled kernel
+int jit_aff(const cfs_system *s)
+{
+    if (s->gen == CFS_GEN_CLOUD) return cfs::AFF_GENERAL;
+    return s->uscale_ok ? (int)cfs::AFF_USCALE : s->aff;
+}
+
+// rewrite the coefficient table of `p` for AFF_USCALE (translations only, the shared scale in p.uscale)
+void apply_uscale(const cfs_system *s, RenderParams &p)
+{
+    if (s->gen != CFS_GEN_IFS || !s->uscale_ok || p.aff_form == cfs::AFF_USCALE) return;
+    const int n = (int)s->funcs.size();
+    memset(p.coef, 0, sizeof(p.coef));
+    const float *m0 = s->funcs[0].params;
+    p.uscale[0] = m0[0]; p.uscale[1] = (s->dim == 2) ? m0[3] : m0[4]; p.uscale[2] = (s->dim == 2) ? 0.0f : m0[8];
+    for (int j = 0; j < n; ++j) {
+        const float *m = s->funcs[j].params;
+        float *r = p.coef + 4 * j;
+        if (s->dim == 2) { r[0] = m[4]; r[1] = m[5]; } else { r[0] = m[9]; r[1] = m[10]; r[2] = m[11]; }
+    }
+    p.aff_form = cfs::AFF_USCALE;
+    p.coef_rows = (uint32_t)n;
+    p.coef_cshift = 0;
+    if (p.coef_rows > 8) while (p.coef_cshift < 3 && (p.coef_rows << (p.coef_cshift + 1)) <= (uint32_t)cfs::kCoefSlots) ++p.coef_cshift;
+    p.coef_rstride = 16u << p.coef_cshift; p.coef_kstride = p.coef_rstride;
+}
+
+// options compiled into a run-time specialised kernel (cfs_params.h KernelOpt): everything the host knows about
+// the system and the render that lets the kernel drop a run-time decision
+int jit_options(const cfs_system *s, const RenderParams &p, int splat)
+{
+    int opt = p.reuse ? cfs::OPT_REUSE : 0;
+    if (s->gen == CFS_GEN_IFS) {
+        if (p.pick_shift >= 0) opt |= cfs::OPT_PICK_SHIFT;
+        else if (p.n_thr == 2) opt |= cfs::OPT_PICK_CMP2;          // exactly two real thresholds (unused slots hold 2^32 - 1)
+        else if (p.pick_steps <= 1) opt |= cfs::OPT_PICK_LUT1;
+    }
+    if (p.xmin == -p.xmax && p.ymin == -p.ymax) opt |= cfs::OPT_SYM_BOUNDS;
+    if (splat == cfs::SPLAT_BIN) {
+        opt |= cfs::OPT_BIN_FIXED | ((int)(p.bin.hybrid & 15u) << cfs::OPT_BIN_MASK_SHIFT);
+        if (p.color_rule != 0) opt |= cfs::OPT_BIN_RGBA;
+    }
+    return opt;
+}
+
 int trig_of(uint32_t sig, int flags)
 {
     return ((flags & CFS_FLAG_FAST_TRIG) && cfs::sig_has_trig(sig)) ? cfs::TRIG_FAST : cfs::TRIG_ACCURATE;
@@ -436,17 +498,17 @@ int trig_of(uint32_t sig, int flags)
 // The kernel for this render and splat sink.  Order: run-time compiled (when asked for), the kernel compiled
 // ahead of time for the chain's signature when there is one, else the chain interpreter; all evaluate the
 // same device functions.  UNSUPPORTED + message when CFS_FLAG_JIT was given and compilation is impossible.
-cfs_status pick_kernel(const cfs_system *s, const RenderParams &p, int splat, int flags, Kernel *out)
+cfs_status pick_kernel(const cfs_system *s, RenderParams &p, int splat, int flags, Kernel *out)
 {
     *out = Kernel();
     const uint32_t sig = chain_signature(p);
     if (wants_jit(flags) && splat != cfs::SPLAT_HIST_CLUSTER) {
-        const int opt = p.reuse ? cfs::OPT_REUSE : 0;
+        const int opt = jit_options(s, p, splat);
         const std::string name = is_cloud_stream(s, splat)
             ? cfs::jit_cloud_name(s->dim, splat, sig, trig_of(sig, flags), opt)
-            : cfs::jit_render_name(s->dim, s->gen, s->gen == CFS_GEN_CLOUD ? (int)cfs::AFF_GENERAL : s->aff, splat, sig, trig_of(sig, flags), opt);
+            : cfs::jit_render_name(s->dim, s->gen, jit_aff(s), splat, sig, trig_of(sig, flags), opt);
         std::string err;
-        if (cfs::jit_get(name, &out->jit, &err)) { out->compiled_chain = true; return CFS_OK; }
+        if (cfs::jit_get(name, &out->jit, &err)) { apply_uscale(s, p); out->compiled_chain = true; return CFS_OK; }
         if (flags & CFS_FLAG_JIT) return fail(CFS_ERR_UNSUPPORTED, "%s", err.c_str());
         *out = Kernel();                       // $CFS_FORCE_JIT only: fall back to what is linked in
     }
@@ -461,14 +523,14 @@ cfs_status pick_kernel(const cfs_system *s, const RenderParams &p, int splat, in
     return CFS_OK;
 }
 
-cfs_status pick_trace(const cfs_system *s, const RenderParams &p, int flags, Kernel *out)
+cfs_status pick_trace(const cfs_system *s, RenderParams &p, int flags, Kernel *out)
 {
     *out = Kernel();
     const uint32_t sig = chain_signature(p);
     if (wants_jit(flags) && !p.reuse) {
         std::string err;
-        const std::string name = cfs::jit_trace_name(s->dim, s->gen, s->gen == CFS_GEN_CLOUD ? (int)cfs::AFF_GENERAL : s->aff, sig, trig_of(sig, flags));
-        if (cfs::jit_get(name, &out->jit, &err)) { out->compiled_chain = true; return CFS_OK; }
+        const std::string name = cfs::jit_trace_name(s->dim, s->gen, jit_aff(s), sig, trig_of(sig, flags));
+        if (cfs::jit_get(name, &out->jit, &err)) { apply_uscale(s, p); out->compiled_chain = true; return CFS_OK; }
         if (flags & CFS_FLAG_JIT) return fail(CFS_ERR_UNSUPPORTED, "%s", err.c_str());
         *out = Kernel();
     }
@@ -493,7 +555,7 @@ cfs_status launch(const Kernel &k, unsigned grid, unsigned block, size_t dyn, cu
         return CFS_OK;
     }
     cudaError_t e;
-    if (dyn > 48 * 1024 && (e = ensure_dyn_smem((const void *)k.aot, dyn)) != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute");
+    if (dyn > 32 * 1024 && (e = ensure_dyn_smem((const void *)k.aot, dyn)) != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute");
     k.aot<<<grid, block, dyn, st>>>(p);
     ++g_launches;
     if ((e = cudaGetLastError()) != cudaSuccess) return cuda_fail(e, what);
@@ -534,7 +596,7 @@ size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 // tiles and staging rows; false when the variant cannot serve this system / image
 bool bin_shape_raw(int gen, int out_mode, int color, uint32_t n_funcs, int32_t width, int32_t height, const DeviceInfo &di,
-                   bool hybrid, BinPlan *pl, const char **why)
+                   uint32_t hybrid, BinPlan *pl, const char **why)
 {
     if (gen != CFS_GEN_IFS) { *why = "binned variant needs an IFS generator"; return false; }
     if (out_mode == CFS_OUT_DEPTH_RGBA8_U64) { *why = "binned variant serves HIST and RGBA output"; return false; }
@@ -587,7 +649,7 @@ bool bin_shape_raw(int gen, int out_mode, int color, uint32_t n_funcs, int32_t w
     // nearly full flush unit -- with a factor 2 for tiles that draw more than the even share (the swirled
     // square of configs[1] covers 41 % of its image: before this factor every fifth warp-block found a full
     // row, profiles/r01j) and 16 records of slack.  The hybrid stage bins every other splat only.
-    const double per_it = (double)cfs::kBinThreads / (double)n_tiles * (hybrid ? 0.5 : 1.0);
+    const double per_it = (double)cfs::kBinThreads / (double)n_tiles * (1.0 - 0.25 * __builtin_popcount(hybrid & 15u));
     const double room = (double)(cap - (long)cfs::kBinFlushRecords + 1);
     uint32_t every = 64;
     while (every > 4 && 2.0 * every * per_it + 16.0 > room) every >>= 1;
@@ -608,7 +670,7 @@ bool bin_shape_raw(int gen, int out_mode, int color, uint32_t n_funcs, int32_t w
         b.split = best;
     }
     pl->smem_pass1 = (n_tiles + cfs::kBinDummy + 3) / 4 * 4 * 4 + n_tiles * (size_t)cap * 2;
-    pl->smem_pass2 = (size_t)b.tile_pixels * nk * 4;
+    pl->smem_pass2 = (size_t)b.tile_pixels * nk * 4 + 16;      // + the dummy counter the padding records of a last flush unit hit
     pl->grid1 = (uint32_t)di.sms * cfs::kBinCtasPerSm;
     return true;
 }
@@ -623,7 +685,7 @@ size_t bin_fixed_bytes(const BinPlan &pl)
 
 bool bin_shape(const cfs_system *s, const cfs_render_args *a, const DeviceInfo &di, BinPlan *pl, const char **why)
 {
-    const bool hybrid = (a->flags & CFS_FLAG_BIN_HYBRID) || a->variant == CFS_VARIANT_AUTO;
+    const uint32_t hybrid = hybrid_mask(a);
     return bin_shape_raw(s->gen, a->out_mode, s->color, (uint32_t)s->funcs.size(), a->width, a->height, di, hybrid, pl, why);
 }
 
@@ -682,7 +744,7 @@ extern "C" cfs_status cfs_binned_plan(int32_t width, int32_t height, int32_t out
     BinPlan pl;
     const char *why = "";
     if (!bin_shape_raw(CFS_GEN_IFS, out_mode, out_mode == CFS_OUT_RGBA_F32 ? CFS_COLOR_MAP_INDEX : CFS_COLOR_NONE, (uint32_t)n_funcs,
-                       width, height, di, false, &pl, &why)) return fail(CFS_ERR_UNSUPPORTED, "%s", why);
+                       width, height, di, 0u, &pl, &why)) return fail(CFS_ERR_UNSUPPORTED, "%s", why);
     out[0] = pl.bp.n_tiles; out[1] = pl.bp.tile_pixels; out[2] = pl.bp.magic; out[3] = pl.bp.mshift;
     out[4] = pl.bp.nk; out[5] = pl.bp.cap; out[6] = 4u * (pl.bp.check_mask + 1u); out[7] = pl.bp.split;
     return CFS_OK;
@@ -761,14 +823,14 @@ cfs_status render_binned(const cfs_system *s, const cfs_render_args *a, RenderPa
     if (!a->d_scratch) return fail(CFS_ERR_UNSUPPORTED, "binned variant needs d_scratch (see cfs_binned_scratch_bytes)");
     const uint64_t spp = (uint64_t)(a->iterations - a->burn_in) * branches_of(s);
     if (!bin_layout(&pl, a->d_scratch, a->scratch_bytes, a->n_points, spp, &why)) return fail(CFS_ERR_UNSUPPORTED, "%s", why);
+    p.bin = pl.bp;
+    p.bin.hybrid = hybrid_mask(a);
     Kernel k1;
     cfs_status ks = pick_kernel(s, p, cfs::SPLAT_BIN, a->flags, &k1);
     if (ks != CFS_OK) return ks;
     Kernel k2;
     k2.aot = (a->out_mode == CFS_OUT_HIST_U32) ? cfs::bin_accumulate_kernel<0> : cfs::bin_accumulate_kernel<1>;
     cudaError_t e;
-    p.bin = pl.bp;
-    p.bin.hybrid = ((a->flags & CFS_FLAG_BIN_HYBRID) || a->variant == CFS_VARIANT_AUTO) ? 1u : 0u;
     const uint64_t total = a->n_points, first = a->point_offset;
     for (uint64_t done = 0; done < total; done += pl.chunk_points) {
         const uint64_t n = (total - done < pl.chunk_points) ? total - done : pl.chunk_points;
@@ -906,9 +968,18 @@ static cfs_status render_impl(const cfs_system *s, const cfs_render_args *a, voi
         if (a->out_mode == CFS_OUT_HIST_U32 && hist_bytes <= shared_hist_limit(di) && n_splats >= (uint64_t)di.sms * (hist_bytes / 4)) {
             splat = cfs::SPLAT_HIST_SHARED;
         } else if (a->out_mode == CFS_OUT_DEPTH_RGBA8_U64) {
-            // direct: ld.cg pre-test + atom.min.  Measured at the SM-to-L2 request rate (one sector request per
-            // clock and SM, l1tex2xbar 98 % busy); CFS_VARIANT_DEPTH_HIZ removes that bound but lands on the
-            // issue rate at the same time (228.7 ms both on configs[4]), so AUTO keeps the path without scratch
+            // direct: ld.cg pre-test + atom.min, measured at the SM-to-L2 request rate (one sector request per clock
+            // and SM, l1tex2xbar 98 % busy).  The Hi-Z variant removes that bound and is then bound by instruction
+            // issue: level with the direct path as linked ahead of time (227 ms both on configs[4]), ahead of it when
+            // compiled for the system (CFS_FLAG_JIT: 178 ms).  AUTO takes it for big renders when the caller provides
+            // the scratch for its map.
+            if (s->gen == CFS_GEN_IFS && a->d_scratch && cfs_hiz_scratch_bytes(a->width, a->height) != 0 &&
+                a->scratch_bytes >= cfs_hiz_scratch_bytes(a->width, a->height) && n_splats >= (1ull << 30)) {
+                cfs_status hs = render_depth_hiz(s, a, p, di, (cudaStream_t)stream);
+                if (hs != CFS_ERR_UNSUPPORTED) return hs;
+                build_params(s, a, &p, true);
+                p.cloud_base = cloud_base;
+            }
         } else if (a->d_scratch && a->n_points >= (uint64_t)di.sms * cfs::kBinCtasPerSm * cfs::kBinThreads && n_splats >= (1ull << 27)) {
             // the hybrid stage (every other splat direct, the rest through the tile bins) keeps issue slots, the
             // L2 reduction path and HBM busy at once: measured ahead of the direct path with MUFU sin/cos
@@ -947,7 +1018,7 @@ static cfs_status render_impl(const cfs_system *s, const cfs_render_args *a, voi
         // same template has the same shape -- the registers allow 8 x 256 threads, shared memory decides
         int per_sm = 1;
         if (kn.aot) {
-            if (dyn > 48 * 1024) ensure_dyn_smem((const void *)kn.aot, dyn);
+            if (dyn > 32 * 1024) ensure_dyn_smem((const void *)kn.aot, dyn);
             cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void *)kn.aot, threads, dyn);
         } else {
             per_sm = (int)((size_t)di.smem_sm / (dyn + sizeof(cfs::SharedTables) + 2048));
@@ -985,6 +1056,7 @@ extern "C" cfs_status cfs_specialize(const cfs_system *s, const cfs_render_args 
     const char *why = "";
     if (bin_shape(s, &r, di, &pl, &why)) kinds[n++] = cfs::SPLAT_BIN;
     double ms = 0.0;
+    p.bin.hybrid = hybrid_mask(&r);
     for (int i = 0; i < n; ++i) {
         Kernel k;
         if ((st = pick_kernel(s, p, kinds[i], r.flags, &k)) != CFS_OK) return st;
@@ -1005,10 +1077,11 @@ extern "C" cfs_status cfs_jit_check(const cfs_system *s, const cfs_render_args *
     int splat = splat_kind;
     if (splat < 0) splat = (a->out_mode == CFS_OUT_RGBA_F32) ? cfs::SPLAT_RGBA : (a->out_mode == CFS_OUT_DEPTH_RGBA8_U64) ? cfs::SPLAT_DEPTH : cfs::SPLAT_HIST_DIRECT;
     const uint32_t sig = chain_signature(p);
-    const int opt = p.reuse ? cfs::OPT_REUSE : 0;
+    if (splat == cfs::SPLAT_BIN) p.bin.hybrid = hybrid_mask(a);
+    const int opt = jit_options(s, p, splat);
     const std::string name = is_cloud_stream(s, splat)
         ? cfs::jit_cloud_name(s->dim, splat, sig, trig_of(sig, a->flags), opt)
-        : cfs::jit_render_name(s->dim, s->gen, s->gen == CFS_GEN_CLOUD ? (int)cfs::AFF_GENERAL : s->aff, splat, sig, trig_of(sig, a->flags), opt);
+        : cfs::jit_render_name(s->dim, s->gen, jit_aff(s), splat, sig, trig_of(sig, a->flags), opt);
     std::string err;
     size_t bytes = 0;
     double ms = 0.0;

@@ -7,7 +7,7 @@
 // are partitioned by tile on their way through HBM:
 //
 //   pass 1 (render_kernel<..., SPLAT_BIN>): each splat becomes ONE 16-bit record
-//     (pixel-in-tile * colour slots + colour index), appended with one shared-memory atomic to the CTA's
+//     (colour index * pixels per tile + pixel-in-tile), appended with one shared-memory atomic to the CTA's
 //     staging row of its tile; full rows leave as 512-byte coalesced stores into 2 KiB pool blocks
 //     owned by (CTA, tile), so no global atomic is paid per splat -- one per 512 records.
 //   pass 2 (bin_accumulate_kernel): one CTA per (tile, part) walks the tile's block list with
@@ -34,20 +34,23 @@ __device__ __forceinline__ void bin_red_add_u32(uint32_t *addr, uint32_t v)
     asm volatile("red.global.add.u32 [%0], %1;" :: "l"(addr), "r"(v) : "memory");
 }
 
-// shared-memory layout of pass 1 (dynamic): u32 cnt[n_tiles + kBinDummy] | pad to 16 B | u16 buf[n_tiles][cap].
-// cnt[n_tiles + lane] is lane's DUMMY counter: a dropped splat increments it instead of a tile's, so
-// the append is straight-line code (no branch around the atomic) and dropped splats of different
-// lanes never meet on one address.
+// shared-memory layout of pass 1 (dynamic): u32 cnt[n_tiles + kBinDummy] | pad to 16 B | u16 buf[n_tiles][cap].  The
+// fill counters are contiguous on purpose: 32 lanes taking slots in 32 random tiles spread over all 32 banks (a
+// counter at the head of each row puts them all on 8 banks: rows are a multiple of 128 bytes apart plus the head;
+// measured slower, 3.19 against 2.96 ms on configs[1]).  cnt[n_tiles + lane] is lane's DUMMY counter, pre-set to the
+// row capacity: a dropped splat takes its slot there and so finds "no room" -- the append stays straight-line code
+// (a predicated atom.shared compiles to a branch around it: three more instructions per splat, measured) and the
+// dropped splats of different lanes never meet on one address.
 __device__ __forceinline__ uint32_t bin_buf_offset(uint32_t n_tiles) { return (n_tiles + kBinDummy + 3u) & ~3u; }
 
 // one record down the direct path (staging row full, or no pool block for the tile)
 __device__ __forceinline__ void bin_direct(const RenderParams &prm, const SharedTables &s, uint32_t tile, uint32_t rec)
 {
-    const uint32_t pix = tile * prm.bin.tile_pixels + rec / prm.bin.nk;       // rare path: a real division is fine
+    const uint32_t pix = tile * prm.bin.tile_pixels + rec % prm.bin.tile_pixels;   // rare path: a real division is fine
     if (prm.color_rule == 0) {
         bin_red_add_u32(reinterpret_cast<uint32_t *>(prm.image) + pix, 1u);
     } else {
-        const float4 c = s.palette[rec % prm.bin.nk];
+        const float4 c = s.palette[rec / prm.bin.tile_pixels];
         bin_red_add_v4_f32(reinterpret_cast<float *>(prm.image) + 4 * (size_t)pix, c.x, c.y, c.z, 1.0f);
     }
 }
@@ -56,10 +59,10 @@ __device__ __forceinline__ void bin_direct(const RenderParams &prm, const Shared
 // an access is one ATOMS / STS without generic-address arithmetic)
 struct BinRegs {
     uint32_t cnt_addr, buf_addr;   // shared addresses of cnt[] and buf[][]
-    uint32_t cap, cap2;            // row capacity in records / bytes
+    uint32_t row_bytes, cap;       // bytes per row, records per row
     uint32_t dummy;                // index of this lane's dummy counter (n_tiles + lane)
     uint32_t tp, ntp, magic, mshift; // tile = umulhi(pix, magic) >> mshift == pix / tp for every pixel of the image; ntp = -tp
-    uint32_t nk, kmask;            // colour slots per pixel, and the mask that zeroes k for HIST
+    uint32_t ktp;                  // colour index stride of a record: tp for RGBA, 0 for HIST (the colour is ignored)
     float sx, ox, sy, oy;          // pixel map (DESIGN R8)
     float xmin, xmax, ymin, ymax;  // closed bounds (DESIGN R8)
     int W, Wm1, Hm1;
@@ -70,19 +73,22 @@ __device__ __forceinline__ BinRegs bin_regs_init(const RenderParams &prm, uint32
     BinRegs r;
     r.cnt_addr = (uint32_t)__cvta_generic_to_shared(sm);
     r.buf_addr = r.cnt_addr + 4u * bin_buf_offset(prm.bin.n_tiles);
-    r.cap = prm.bin.cap; r.cap2 = 2u * prm.bin.cap;
+    r.cap = prm.bin.cap; r.row_bytes = 2u * prm.bin.cap;
     r.dummy = prm.bin.n_tiles;      // + lane, added by each thread after the broadcast
     r.tp = prm.bin.tile_pixels; r.ntp = 0u - prm.bin.tile_pixels; r.magic = prm.bin.magic; r.mshift = prm.bin.mshift;
-    r.nk = prm.bin.nk; r.kmask = (prm.color_rule == 0) ? 0u : 0xFFFFFFFFu;
+    r.ktp = (prm.color_rule == 0) ? 0u : prm.bin.tile_pixels;
     r.sx = prm.sx; r.ox = prm.ox; r.sy = prm.sy; r.oy = prm.oy;
     r.xmin = prm.xmin; r.xmax = prm.xmax; r.ymin = prm.ymin; r.ymax = prm.ymax;
     r.W = prm.W; r.Wm1 = prm.W - 1; r.Hm1 = prm.H - 1;
     return r;
 }
 
-// bounds rule of cfs_device.cuh in_bounds(), operands from registers
+// bounds rule of cfs_device.cuh in_bounds(), operands from registers.  SYM: the bounds are symmetric about 0
+// (host-checked), so the closed test is two compares on |x|, |y| -- the same truth value for every float, NaN included.
+template <bool SYM>
 __device__ __forceinline__ bool bin_in_bounds(const BinRegs &br, float x, float y)
 {
+    if (SYM) return (fabsf(x) <= br.xmax) && (fabsf(y) <= br.ymax);
     return (x >= br.xmin) && (x <= br.xmax) && (y >= br.ymin) && (y <= br.ymax);
 }
 
@@ -95,35 +101,36 @@ __device__ __forceinline__ int bin_pixel_of(const BinRegs &br, float x, float y)
     return (int)(py * (uint32_t)br.W + px);
 }
 
-// row 7, binned: one shared-memory atomic + one shared store per splat
+__device__ __forceinline__ void bin_record_of(const BinRegs &br, int pix, int k, uint32_t &tile, uint32_t &rec)
+{
+    tile = __umulhi((uint32_t)pix, br.magic) >> br.mshift;
+    rec = (tile * br.ntp + (uint32_t)pix) + (uint32_t)k * br.ktp;
+}
+
+// row 7, binned: one shared-memory atomic + one shared store per splat (interpreter path: branches are fine here)
 __device__ __forceinline__ void bin_append(const RenderParams &prm, const SharedTables &s, const BinRegs &br, int pix, int k)
 {
-    const uint32_t tile = __umulhi((uint32_t)pix, br.magic) >> br.mshift;
-    const uint32_t rec = ((uint32_t)pix - tile * br.tp) * br.nk + ((uint32_t)k & br.kmask);
-    const uint32_t row = br.buf_addr + tile * br.cap2;
+    uint32_t tile, rec;
+    bin_record_of(br, pix, k, tile, rec);
+    const uint32_t row = br.buf_addr + tile * br.row_bytes;
     uint32_t slot;
     asm volatile("atom.shared.add.u32 %0, [%1], 1;" : "=r"(slot) : "r"(br.cnt_addr + 4u * tile) : "memory");
     if (slot < br.cap) asm volatile("st.shared.u16 [%0], %1;" :: "r"(row + 2u * slot), "h"((uint16_t)rec) : "memory");
     else bin_direct(prm, s, tile, rec);
 }
 
-// The same as straight-line code: the atomic is unconditional (a dropped splat takes the lane's
-// dummy counter), the store is predicated.  Returns true when the record found its row full and
-// has to go down the direct path (rare; the caller does that afterwards).
+// The same as straight-line code: a dropped splat takes its slot from the lane's dummy counter, which always reads
+// "full", so the store is predicated on the slot alone.  Returns true when the record was stored; false means
+// "row full" -- a live record then has to go down the direct path (rare; the caller does that afterwards and tells
+// live from dropped by `ok`).
 __device__ __forceinline__ bool bin_try_append(const BinRegs &br, bool ok, uint32_t tile, uint32_t rec)
 {
     const uint32_t t_eff = ok ? tile : br.dummy;
     uint32_t slot;
     asm volatile("atom.shared.add.u32 %0, [%1], 1;" : "=r"(slot) : "r"(br.cnt_addr + 4u * t_eff) : "memory");
-    const bool fits = ok && slot < br.cap;
-    if (fits) asm volatile("st.shared.u16 [%0], %1;" :: "r"(br.buf_addr + tile * br.cap2 + 2u * slot), "h"((uint16_t)rec) : "memory");
-    return ok && slot >= br.cap;
-}
-
-__device__ __forceinline__ void bin_record_of(const BinRegs &br, int pix, int k, uint32_t &tile, uint32_t &rec)
-{
-    tile = __umulhi((uint32_t)pix, br.magic) >> br.mshift;
-    rec = (tile * br.ntp + (uint32_t)pix) * br.nk + ((uint32_t)k & br.kmask);
+    const bool fits = slot < br.cap;
+    if (fits) asm volatile("st.shared.u16 [%0], %1;" :: "r"(br.buf_addr + tile * br.row_bytes + 2u * slot), "h"((uint16_t)rec) : "memory");
+    return fits;
 }
 
 // Per-lane bin state of pass 1, kept in REGISTERS: lane l of warp w owns tile l * warps + w (so
@@ -182,7 +189,20 @@ __device__ __forceinline__ void bin_flush(const RenderParams &prm, const SharedT
             uint4 v = make_uint4(0u, 0u, 0u, 0u);
             if (8u * lane < n) v = reinterpret_cast<const uint4 *>(head)[lane];    // 8 records; never past the row
             if (pos != kBinInvalid) {
-                if (8u * lane < n) reinterpret_cast<uint4 *>(b.pool + pos)[lane] = v;
+                if (n < kBinFlushRecords) {
+                    // last, partial unit of this (CTA, tile): pad it to 256 records with the DUMMY record (the counter
+                    // behind the tile's last one), so that pass 2 counts whole 512-byte units without a test per record
+                    const uint32_t dummy = b.tile_pixels * b.nk, d2 = dummy | (dummy << 16);
+                    uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+                        const uint32_t r0 = 8u * lane + 2u * i;
+                        w[i] = (r0 >= n) ? d2 : (r0 + 1u >= n) ? ((w[i] & 0xFFFFu) | (dummy << 16)) : w[i];
+                    }
+                    reinterpret_cast<uint4 *>(b.pool + pos)[lane] = make_uint4(w[0], w[1], w[2], w[3]);
+                } else {
+                    reinterpret_cast<uint4 *>(b.pool + pos)[lane] = v;
+                }
                 if ((int)lane == src) bl.pos += n;
             } else {
                 const uint32_t r[4] = {v.x, v.y, v.z, v.w};
@@ -218,19 +238,40 @@ __device__ __forceinline__ void bin_flush(const RenderParams &prm, const SharedT
 }
 
 // ---------------------------------------------------------------------------------------------
-// pass 2.  MODE 0: HIST_U32 (nk = 1).  MODE 1: RGBA_F32 + MAP_INDEX: counters per
-// (pixel, colour index); the pixel's sum is sum_k n_k * palette[k] (any summation order is a
-// correct result, DESIGN R8; exact for integer-valued palettes while every sum stays < 2^24).
+// pass 2.  MODE 0: HIST_U32 (nk = 1).  MODE 1: RGBA_F32 + MAP_INDEX: counters per (colour index, pixel), laid
+// out [k][pixel] -- the colour of a splat follows its position (the last map decides the region), so a tile is
+// mostly ONE colour and a [pixel][k] layout would leave all records of a warp on 32 / nk banks (measured 5.2
+// wavefronts per ATOMS in r01k); with [k][pixel] the bank is the pixel's.  The pixel's sum is
+// sum_k n_k * palette[k] (any summation order is a correct result, DESIGN R8; exact for integer-valued palettes
+// while every sum stays < 2^24).
+//
+// A record IS the index of its counter, and every flush unit in the pool is 256 whole records (pass 1 pads a
+// last unit with the DUMMY record, the counter behind the tile's last one), so the count loop is three
+// instructions per record: extract 16 bits, scale to a shared-window address, red.shared.add.
+__device__ __forceinline__ void bin_count8(uint32_t acc_addr, const uint4 &v)
+{
+    const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        asm volatile("red.shared.add.u32 [%0], 1;" :: "r"(acc_addr + ((w[i] & 0xFFFFu) << 2)) : "memory");
+        asm volatile("red.shared.add.u32 [%0], 1;" :: "r"(acc_addr + ((w[i] >> 16) << 2)) : "memory");
+    }
+}
+
 template <int MODE>
 __global__ void __launch_bounds__(kBinAccThreads)
 bin_accumulate_kernel(const __grid_constant__ RenderParams prm)
 {
-    extern __shared__ __align__(16) uint32_t acc[];
+    extern __shared__ __align__(16) uint32_t acc[];     // tile_pixels * nk counters + the dummy one (+ padding to 16 bytes)
     const BinParams &b = prm.bin;
     const uint32_t tile = blockIdx.x / b.split, part = blockIdx.x % b.split;
     const uint32_t n_ctr = b.tile_pixels * b.nk;
-    for (uint32_t i = threadIdx.x; i < n_ctr; i += blockDim.x) acc[i] = 0u;
+    {
+        uint4 *a4 = reinterpret_cast<uint4 *>(acc);
+        for (uint32_t i = threadIdx.x; i < n_ctr / 4u + 1u; i += blockDim.x) a4[i] = make_uint4(0u, 0u, 0u, 0u);
+    }
     __syncthreads();
+    const uint32_t acc_addr = (uint32_t)__cvta_generic_to_shared(acc);
 
     // CTA `part` takes blocks j = part (mod split) of every pass-1 CTA's list for this tile; its
     // warps stripe over the pass-1 CTAs
@@ -239,32 +280,27 @@ bin_accumulate_kernel(const __grid_constant__ RenderParams prm)
         const uint32_t tail = b.tails[(size_t)tile * b.grid + c];
         const uint32_t n_blk = tail >> kBinTailShift, last_fill = tail & ((1u << kBinTailShift) - 1u);
         const uint32_t *list = b.list + ((size_t)tile * b.grid + c) * b.lcap;
-        // two blocks (2 x 2 KiB = 2 x 1024 records, eight 128-bit loads per lane) in flight per warp
+        // two blocks (2 x 2 KiB = 2 x 4 units of 256 records, eight 128-bit loads per lane) in flight per warp
         for (uint32_t j = part; j < n_blk; j += 2u * b.split) {
             uint4 v[2][4];
-            uint32_t fill[2];
+            uint32_t units[2];
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
                 const uint32_t jj = j + (uint32_t)h * b.split;
-                fill[h] = 0u;
+                units[h] = 0u;
                 if (jj < n_blk) {
-                    fill[h] = (jj + 1u == n_blk) ? last_fill : kBinBlockRecords;
+                    units[h] = (jj + 1u == n_blk) ? (last_fill + kBinFlushRecords - 1u) / kBinFlushRecords : kBinBlockRecords / kBinFlushRecords;
                     const uint4 *src = reinterpret_cast<const uint4 *>(b.pool + (size_t)list[jj] * kBinBlockRecords);
 #pragma unroll
                     for (int q = 0; q < 4; ++q)
-                        v[h][q] = (q * 256u < fill[h]) ? __ldcs(src + q * 32 + lane) : make_uint4(0u, 0u, 0u, 0u);
+                        if ((uint32_t)q < units[h]) v[h][q] = __ldcs(src + q * 32 + lane);
                 }
             }
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
 #pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    const uint32_t base = q * 256u + 8u * lane;
-                    const uint32_t r[4] = {v[h][q].x, v[h][q].y, v[h][q].z, v[h][q].w};
-#pragma unroll
-                    for (int i = 0; i < 8; ++i)
-                        if (base + i < fill[h]) atomicAdd(&acc[(r[i >> 1] >> (16 * (i & 1))) & 0xFFFFu], 1u);
-                }
+                for (int q = 0; q < 4; ++q)
+                    if ((uint32_t)q < units[h]) bin_count8(acc_addr, v[h][q]);        // warp-uniform
             }
         }
     }
@@ -286,7 +322,7 @@ bin_accumulate_kernel(const __grid_constant__ RenderParams prm)
             float r = 0.f, g = 0.f, bl = 0.f, a = 0.f;
             uint32_t any = 0u;
             for (uint32_t k = 0; k < nk; ++k) {
-                const uint32_t c = acc[i * nk + k];
+                const uint32_t c = acc[k * n_pix_tile + i];
                 if (c) {
                     const float fc = (float)c;
                     r = __fmaf_rn(fc, prm.palette[4 * k + 0], r);

@@ -22,6 +22,8 @@
 
 namespace cfs {
 
+// launch shape: measured flat on configs[3] (151.6 - 160.8 us over 128..1024 threads x 8..1 CTAs per SM, chunks of
+// 512..4096 records, 2..6 stages): the render is bound by the L2 slices, not by the shape of the stream
 constexpr int kCloudThreads = 512;
 constexpr int kCloudCtasPerSm = 2;
 constexpr uint32_t kCloudChunk = 2048;      // records per stage (32 KB)

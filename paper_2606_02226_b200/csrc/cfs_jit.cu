@@ -71,6 +71,7 @@ unsigned long long g_n_compiled = 0;
 double g_total_ms = 0.0;
 std::vector<std::string> g_sources;    // header texts in kHeaderNames order
 uint64_t g_source_hash = 0;
+std::vector<std::string> g_extra_options;   // $CFS_JIT_OPTIONS
 
 uint64_t fnv1a(const void *data, size_t n, uint64_t h = 1469598103934665603ull)
 {
@@ -108,9 +109,19 @@ bool load_sources(std::string *err)
             if (!found) { *err = std::string("source not embedded: ") + kHeaderNames[i]; return false; }
         }
     }
+    // kernel development: extra compiler options (e.g. -DNAME=value), separated by blanks
+    g_extra_options.clear();
+    if (const char *x = getenv("CFS_JIT_OPTIONS")) {
+        std::string cur;
+        for (const char *c = x;; ++c) {
+            if (*c == ' ' || *c == '\0') { if (!cur.empty()) g_extra_options.push_back(cur); cur.clear(); if (!*c) break; }
+            else cur.push_back(*c);
+        }
+    }
     uint64_t h = fnv1a(kProgram, strlen(kProgram));
     for (int i = 0; i < kNumHeaders; ++i) h = fnv1a(g_sources[i].data(), g_sources[i].size(), h);
     for (int i = 0; i < kNumOptions; ++i) h = fnv1a(kOptions[i], strlen(kOptions[i]), h);
+    for (const std::string &o : g_extra_options) h = fnv1a(o.data(), o.size(), h);
     g_source_hash = h;
     return true;
 }
@@ -192,7 +203,9 @@ bool compile_locked(const std::string &name, std::vector<char> *cubin, std::stri
     bool ok = false;
     do {
         if ((rc = r.AddNameExpression(prog, name.c_str())) != NVRTC_SUCCESS) { *err = std::string("nvrtcAddNameExpression: ") + r.GetErrorString(rc); break; }
-        rc = r.CompileProgram(prog, kNumOptions, kOptions);
+        std::vector<const char *> opts(kOptions, kOptions + kNumOptions);
+        for (const std::string &o : g_extra_options) opts.push_back(o.c_str());
+        rc = r.CompileProgram(prog, (int)opts.size(), opts.data());
         if (rc != NVRTC_SUCCESS) {
             size_t n = 0;
             r.GetProgramLogSize(prog, &n);
@@ -343,7 +356,7 @@ cudaError_t jit_launch(const JitKernel &k, unsigned grid, unsigned block, size_t
     {
         std::lock_guard<std::mutex> lock(g_mutex);
         if (!g_driver.ok || !k.func) { *err = "kernel was not compiled"; return cudaErrorInvalidDeviceFunction; }
-        if (dyn_smem > 48 * 1024) {
+        if (dyn_smem > 32 * 1024) {          // static + dynamic beyond the 48 KiB default needs the opt-in
             int dev = 0;
             cudaGetDevice(&dev);
             for (auto &kv : g_cache) {

@@ -33,7 +33,10 @@ constexpr int kClusterThreads = 512;  // CTA size of the cluster-histogram varia
 constexpr int kClusterSize = 8;       // CTAs per cluster (portable maximum)
 
 // affine table forms (bit-identical results, DESIGN R4: fma(0,y,b) == b)
-enum AffForm : int { AFF_GENERAL = 0, AFF_DIAG = 1, AFF_CIRCLE = 2 /* PAPER Eq. 1 maps: one row (f_id, r2 flag, -, -) per map */ };
+enum AffForm : int { AFF_GENERAL = 0, AFF_DIAG = 1, AFF_CIRCLE = 2 /* PAPER Eq. 1 maps: one row (f_id, r2 flag, -, -) per map */,
+                     AFF_USCALE = 3 /* DIAG maps that all share one scale (sx, sy, sz): the table holds the translations only,
+                                       one row (bx by bz -) per map, the scale travels as prm.uscale -- half the table reads
+                                       of AFF_DIAG, bit-identical results (run-time compiled kernels) */ };
 // transcendental evaluation of the non-affine chain steps: libdevice sincosf/sinf/cosf (<= 2 ulp)
 // or the MUFU special-function unit (sin.approx/cos.approx, abs. error ~2^-21 on [-pi, pi])
 enum TrigKind : int { TRIG_ACCURATE = 0, TRIG_FAST = 1, TRIG_RUNTIME = 2 /* prm.fast_trig decides (interpreter) */ };
@@ -52,7 +55,14 @@ CFS_HD constexpr int sig_step(uint32_t sig, int m)
 }
 // kernel options compiled in (template argument OPT of render_kernel / cloud_kernel)
 enum KernelOpt : int {
-    OPT_REUSE = 1          // Fig. 2(C): the chain output is fed back into the generator (compiled chains; the interpreter reads prm.reuse)
+    OPT_REUSE = 1,         // Fig. 2(C): the chain output is fed back into the generator (compiled chains; the interpreter reads prm.reuse)
+    OPT_PICK_SHIFT = 2,    // equal power-of-two thresholds: k = u >> prm.pick_shift, nothing else compiled in
+    OPT_PICK_LUT1 = 4,     // at most one threshold per 2^24 bucket of u: one table read + one compare, no loop
+    OPT_BIN_RGBA = 16,     // tile bins: records carry the colour index (RGBA + MAP_INDEX); with OPT_BIN_FIXED only
+    OPT_BIN_FIXED = 32,    // tile bins: OPT_BIN_RGBA and the direct mask below are the truth (else prm.bin.hybrid / prm.color_rule decide at run time)
+    OPT_SYM_BOUNDS = 64,   // xmin == -xmax and ymin == -ymax: the closed-bounds test is |x| <= xmax && |y| <= ymax (two compares)
+    OPT_PICK_CMP2 = 128,   // at most two thresholds: k = (u >= T[0]) + (u >= T[1]), two compares against the parameter block, no table read
+    OPT_BIN_MASK_SHIFT = 8 // bits 8..11, with OPT_BIN_FIXED: iteration j of a steady-state block splats straight to L2 when bit j is set
 };
 // true when the signature holds a BRANCH separator (type 8): one-to-many splatting
 CFS_HD constexpr bool sig_has_branch(uint32_t sig)
@@ -91,13 +101,14 @@ enum SplatKind : int {
 };
 
 // tile-binned splat stage (DESIGN "binned variant").  A record is one uint16:
-// (pixel index inside the tile) * colour slots + colour index, i.e. directly the index of the
+// (colour index) * (pixels per tile) + (pixel index inside the tile), i.e. directly the index of the
 // shared-memory counter pass 2 increments (a tile has at most 3 * 2^14 = 49152 counters).  The pool is a set of fixed-size blocks; a block belongs to
 // one (CTA, tile) while it is filled and is listed under its tile when it is allocated.
 constexpr uint32_t kBinBlockRecords = 1024;    // records per pool block (2 KiB)
 constexpr uint32_t kBinFlushRecords = 256;     // records per flush: one 512-byte coalesced store
 constexpr uint32_t kBinTailShift = 11;         // tails word: blocks << 11 | records in the last block (<= 1024)
-constexpr uint32_t kBinDummy = 32;             // dummy counters behind cnt[n_tiles]: one per lane, take the dropped splats
+constexpr uint32_t kBinDummy = 32;             // dummy fill counters behind cnt[n_tiles], one per lane: pre-set to the row capacity, they take
+                                               // the dropped splats -- "row full" for free, so a dropped splat stores nothing and needs no predicate
 constexpr uint32_t kBinInvalid = 0xFFFFFFFFu;  // tile has no block (pool or list exhausted): direct splats
 constexpr int kBinThreads = 1024;              // CTA size of pass 1 and CTAs per SM.  Measured on configs[1]: 1 x 1024
 constexpr int kBinCtasPerSm = 1;               // threads 4.69 ms, 2 x 512 threads (half-length staging rows) 5.53 ms
@@ -127,7 +138,8 @@ struct BinParams {
     uint32_t cap;          // staging records per tile in shared memory (multiple of 64, >= 320)
     uint32_t check_mask;   // flush check after Philox block q (4 iterations) when ((q + 1) & check_mask) == 0
     uint32_t split;        // pass 2: CTAs per tile
-    uint32_t hybrid;       // != 0: iterations 0 and 2 of every steady-state Philox block splat straight to L2
+    uint32_t hybrid;       // 4-bit mask: iteration j of every steady-state Philox block splats straight to L2 when bit j is set
+                           // (0 = pure bins, 5 = every other splat: the hybrid stage)
 };
 
 struct ChainStep {
@@ -152,6 +164,8 @@ struct RenderParams {
     uint8_t *tr_alive;
 
     int32_t dim, n_funcs, n_chain, color_rule, reuse, fast_trig;
+    int32_t aff_form;            // AffForm of the coefficient table below
+    float uscale[3];             // AFF_USCALE: the scale all maps share
     int32_t n_branches;          // 1 + BRANCH markers in the chain: splats per generated point and iteration
     int32_t pick_shift;          // >= 0: k = u >> pick_shift (equal power-of-two thresholds)
     int32_t n_thr;               // thresholds below 2^32 (k = #{j < n_thr : u >= T[j]})
@@ -168,8 +182,9 @@ struct RenderParams {
 
     ChainStep chain[kMaxChain];
     uint32_t T[kMaxFuncs];       // thresholds (u32), T[j >= n_thr] = 0xFFFFFFFF
-    uint32_t lut[256];           // lut[b] = #{j < n_thr : T[j] <= b << 24} << 25 | t24, t24 = first
-                                 // threshold inside bucket b minus (b << 24), 2^24 if none
+    uint32_t lut[256][2];        // bucket b of the top byte of u: { (first threshold inside the bucket) - 1, or 0xFFFFFFFF
+                                 // when the bucket holds none;  #{j < n_thr : T[j] <= b << 24} }.  k = lut[b][1] + (u > lut[b][0])
+                                 // is the pick when no bucket holds two thresholds; further ones are walked in T[]
     float coef[kMaxFuncs * 12];  // GENERAL dim2: rows of 8 (a00 a01 b0 0 | a10 a11 b1 0);
                                  // GENERAL dim3: rows of 12 (a00 a01 a02 b0 | ... );
                                  // DIAG dim2: rows of 4 (sx sy bx by); DIAG dim3: rows of 8

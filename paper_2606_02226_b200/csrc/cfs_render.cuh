@@ -62,24 +62,24 @@ __device__ __forceinline__ void splat_depth(unsigned long long *buf, int pix, fl
     if (key < cur) atomicMin(buf + pix, key);
 }
 
-template <int DIM, int GEN, int SPLAT>
+template <int DIM, int GEN, int SPLAT, int OPT>
 __device__ __forceinline__ uint32_t splat_q(const RenderParams &prm, const SharedTables &s, const Sm &sm, uint32_t *s_hist,
                                             float qx, float qy, float qz, bool alive, int k, uint32_t point_rgba8,
                                             bool have, const BinRegs &br, bool bin_direct_half);
 
 // one branch of a compiled one-to-many chain, then the branches after it: every branch gets its own
 // copy of the generated point and its own splat; the structure is fixed at compile time
-template <int DIM, int GEN, int SPLAT, uint32_t SIG, int TRIG, int M>
+template <int DIM, int GEN, int SPLAT, uint32_t SIG, int TRIG, int OPT, int M>
 __device__ __forceinline__ uint32_t branches_static(const RenderParams &prm, const SharedTables &s, const Sm &sm, uint32_t *s_hist,
                                                     float gx, float gy, float gz, int k, uint32_t point_rgba8, bool have,
                                                     const BinRegs &br, const StepCtx &ctx, bool bin_direct_half)
 {
     float qx = gx, qy = gy, qz = gz;
     const bool alive = chain_static<DIM, SIG, TRIG, M>(prm, ctx, qx, qy, qz);
-    uint32_t dropped = splat_q<DIM, GEN, SPLAT>(prm, s, sm, s_hist, qx, qy, qz, alive, k, point_rgba8, have, br, bin_direct_half);
+    uint32_t dropped = splat_q<DIM, GEN, SPLAT, OPT>(prm, s, sm, s_hist, qx, qy, qz, alive, k, point_rgba8, have, br, bin_direct_half);
     constexpr int next = sig_next_branch(SIG, M);
     if constexpr (next >= 0)
-        dropped += branches_static<DIM, GEN, SPLAT, SIG, TRIG, next>(prm, s, sm, s_hist, gx, gy, gz, k, point_rgba8, have, br, ctx, bin_direct_half);
+        dropped += branches_static<DIM, GEN, SPLAT, SIG, TRIG, OPT, next>(prm, s, sm, s_hist, gx, gy, gz, k, point_rgba8, have, br, ctx, bin_direct_half);
     return dropped;
 }
 
@@ -94,7 +94,7 @@ __device__ __forceinline__ uint32_t chain_and_splat(const RenderParams &prm, con
                                                     bool bin_direct_half = false)
 {
     if constexpr (SIG != kChainGeneric && sig_has_branch(SIG)) {
-        return branches_static<DIM, GEN, SPLAT, SIG, TRIG, 0>(prm, s, sm, s_hist, gx, gy, gz, k, point_rgba8, have, br, ctx, bin_direct_half);
+        return branches_static<DIM, GEN, SPLAT, SIG, TRIG, OPT, 0>(prm, s, sm, s_hist, gx, gy, gz, k, point_rgba8, have, br, ctx, bin_direct_half);
     }
     if (SIG == kChainGeneric && prm.n_branches > 1) {
         // one-to-many ("many objects from a single primitive"): every BRANCH of the chain
@@ -105,7 +105,7 @@ __device__ __forceinline__ uint32_t chain_and_splat(const RenderParams &prm, con
         uint32_t dropped = 0u;
         for (int m = 0; m <= prm.n_chain; ++m) {
             if (m == prm.n_chain || prm.chain[m].type == T_BRANCH) {
-                dropped += splat_q<DIM, GEN, SPLAT>(prm, s, sm, s_hist, qx, qy, qz, alive, k, point_rgba8, have, br, bin_direct_half);
+                dropped += splat_q<DIM, GEN, SPLAT, OPT>(prm, s, sm, s_hist, qx, qy, qz, alive, k, point_rgba8, have, br, bin_direct_half);
                 qx = gx; qy = gy; qz = gz; alive = true;
             } else if (alive) {
                 alive = chain_step_dyn<DIM, TRIG>(prm, prm.chain[m], ctx, qx, qy, qz);
@@ -119,16 +119,16 @@ __device__ __forceinline__ uint32_t chain_and_splat(const RenderParams &prm, con
         gx = qx; gy = qy; gz = qz;
         if (!past_burn_in) return 0u;
     }
-    return splat_q<DIM, GEN, SPLAT>(prm, s, sm, s_hist, qx, qy, qz, alive, k, point_rgba8, have, br, bin_direct_half);
+    return splat_q<DIM, GEN, SPLAT, OPT>(prm, s, sm, s_hist, qx, qy, qz, alive, k, point_rgba8, have, br, bin_direct_half);
 }
 
 // rows 6-7 for one chain output: bounds -> pixel -> reduction.  Returns 1 when the splat was dropped.
-template <int DIM, int GEN, int SPLAT>
+template <int DIM, int GEN, int SPLAT, int OPT>
 __device__ __forceinline__ uint32_t splat_q(const RenderParams &prm, const SharedTables &s, const Sm &sm, uint32_t *s_hist,
                                             float qx, float qy, float qz, bool alive, int k, uint32_t point_rgba8,
                                             bool have, const BinRegs &br, bool bin_direct_half)
 {
-    const bool ok = alive && have && in_bounds(prm, qx, qy);
+    const bool ok = alive && have && in_bounds<OPT>(prm, qx, qy);
     if (SPLAT == SPLAT_HIST_WARPAGG) {
         splat_hist_warpagg(reinterpret_cast<uint32_t *>(prm.image), ok ? pixel_of(prm, qx, qy) : -1, ok);
         return (have && !ok) ? 1u : 0u;
@@ -138,13 +138,11 @@ __device__ __forceinline__ uint32_t splat_q(const RenderParams &prm, const Share
         // Hi-Z pre-test in shared memory: a splat whose depth bits exceed the block's upper bound is
         // certainly occluded (the bound comes from a snapshot of an image that only decreases), so
         // it never leaves the SM.  ~95 % of the splats of a solid stop here (DESIGN "Hi-Z variant").
-        int px = __float2int_rd(__fmaf_rn(qx, prm.sx, prm.ox));
-        int py = __float2int_rd(__fmaf_rn(qy, prm.sy, prm.oy));
-        px = min(max(px, 0), prm.W - 1);
-        py = min(max(py, 0), prm.H - 1);
-        const uint32_t bound = lds_u16(sm.dyn + 2u * ((uint32_t)(py >> prm.hiz.shift) * prm.hiz.nbx + (uint32_t)(px >> prm.hiz.shift)));
+        uint32_t px, py;
+        pixel_xy(prm, qx, qy, px, py);
+        const uint32_t bound = lds_u16(sm.dyn + 2u * ((py >> prm.hiz.shift) * prm.hiz.nbx + (px >> prm.hiz.shift)));
         if ((__float_as_uint(qz) >> 16) > bound) return 0u;
-        splat_depth(reinterpret_cast<unsigned long long *>(prm.image), py * prm.W + px, qz,
+        splat_depth(reinterpret_cast<unsigned long long *>(prm.image), (int)(py * (uint32_t)prm.W + px), qz,
                     lds_u32(sm.tab + CFS_SM_OFF(pal8) + 4u * (uint32_t)k));
         return 0u;
     }
@@ -185,21 +183,24 @@ __device__ __forceinline__ uint32_t splat_q(const RenderParams &prm, const Share
 // rows 6-7 of the four iterations of one steady-state Philox block, binned.  HYBRID: iterations 0
 // and 2 of the block splat straight to L2 (red.global), 1 and 3 go through the tile bins -- pass 1 is
 // bound by instruction issue and pass 2 by shared-memory atomics while the L2 reduction units would
-// idle, so half of the splats are given to them (a direct splat costs ~5 instructions against ~16
+// idle, so half of the splats are given to them (a direct splat costs ~5 instructions against ~11
 // for record + append, and pass 2 halves).  Any split is a correct result: HIST sums are exact,
-// RGBA sums are order-free (DESIGN R8).  Returns the number of dropped splats.
-template <bool HYBRID, bool RGBA>
+// RGBA sums are order-free (DESIGN R8).  Straight-line code: every reduction, atomic and store is predicated.
+// Returns the number of dropped splats.
+template <int DIRECT_MASK, bool RGBA>
 __device__ __forceinline__ uint32_t bin_block_splat(const RenderParams &prm, const SharedTables &s, const Sm &sm, const BinRegs &br,
                                                     const float (&X)[4], const float (&Y)[4], const int (&K)[4],
                                                     const bool (&ok)[4])
 {
     uint32_t tile[4], rec[4];
-    bool over[4];
+    bool fine[4];
+    uint32_t dropped = 0u;
 #pragma unroll
     for (int j = 0; j < 4; ++j) {      // out-of-bounds coordinates are clamped by the pixel rule: always a valid tile
         const int pix = bin_pixel_of(br, X[j], Y[j]);
-        over[j] = false;
-        if (HYBRID && (j & 1) == 0) {  // straight to L2: one predicated reduction, no branch
+        fine[j] = true;
+        if (!ok[j]) ++dropped;         // counted here, so that no `ok` outlives its splat
+        if ((DIRECT_MASK >> j) & 1) {  // straight to L2: one predicated reduction, no branch
             if (RGBA) {
                 const float4 c = lds_v4(sm.tab + CFS_SM_OFF(palette) + 16u * (uint32_t)K[j]);
                 float *dst = reinterpret_cast<float *>(prm.image) + 4 * (size_t)(uint32_t)pix;
@@ -212,16 +213,16 @@ __device__ __forceinline__ uint32_t bin_block_splat(const RenderParams &prm, con
                              :: "l"(dst), "r"((uint32_t)ok[j]) : "memory");
             }
         } else {
-            bin_record_of(br, pix, K[j], tile[j], rec[j]);
-            over[j] = bin_try_append(br, ok[j], tile[j], rec[j]);
+            bin_record_of(br, pix, RGBA ? K[j] : 0, tile[j], rec[j]);
+            fine[j] = bin_try_append(br, ok[j], tile[j], rec[j]);
         }
     }
-    if (over[0] || over[1] || over[2] || over[3]) {   // staging row full: those records take the direct path
+    if (!(fine[0] && fine[1] && fine[2] && fine[3])) {   // a staging row was full (or a splat was dropped): live records take the direct path
 #pragma unroll
         for (int j = 0; j < 4; ++j)
-            if (over[j]) bin_direct(prm, s, tile[j], rec[j]);
+            if (!fine[j] && ok[j]) bin_direct(prm, s, tile[j], rec[j]);
     }
-    return 4u - ((uint32_t)ok[0] + (uint32_t)ok[1] + (uint32_t)ok[2] + (uint32_t)ok[3]);
+    return dropped;
 }
 
 // four iterations served by one Philox block (DESIGN R1: word it & 3 of block it >> 2).
@@ -249,21 +250,28 @@ __device__ __forceinline__ uint32_t iterate_block(const RenderParams &prm, const
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
             const uint32_t u = (j == 0) ? w.x : (j == 1) ? w.y : (j == 2) ? w.z : w.w;
-            K[j] = pick_index(u, sm, prm);
+            K[j] = pick_index<OPT>(u, sm, prm);
             apply_gen<DIM, AFF>(K[j], sm, prm, gx, gy, gz);
             X[j] = gx; Y[j] = gy; Z[j] = gz;                 // the copies of Fig. 2(B)
         }
+        // a thread without a point carries NaN coordinates (render_kernel), which fail every bounds test: no `have` here
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
             const bool alive = apply_chain<DIM, SIG, TRIG>(prm, StepCtx{plo, phi, it0 + j}, X[j], Y[j], Z[j]);
-            ok[j] = alive && have && bin_in_bounds(br, X[j], Y[j]);
+            ok[j] = alive && bin_in_bounds<(OPT & OPT_SYM_BOUNDS) != 0>(br, X[j], Y[j]);
         }
-        // warp-uniform choice of one of four straight-line bodies (hybrid or pure bins, RGBA or HIST)
-        if (prm.bin.hybrid) {
-            if (prm.color_rule != 0) dropped += bin_block_splat<true, true>(prm, s, sm, br, X, Y, K, ok);
-            else                     dropped += bin_block_splat<true, false>(prm, s, sm, br, X, Y, K, ok);
+        if constexpr ((OPT & OPT_BIN_FIXED) != 0) {
+            // compiled for this render's split and output: one straight-line body
+            dropped += bin_block_splat<(OPT >> OPT_BIN_MASK_SHIFT) & 15, (OPT & OPT_BIN_RGBA) != 0>(prm, s, sm, br, X, Y, K, ok);
         } else {
-            dropped += bin_block_splat<false, false>(prm, s, sm, br, X, Y, K, ok);
+            // warp-uniform choice of one of three straight-line bodies (hybrid RGBA / hybrid HIST / pure bins); any
+            // non-zero mask runs as "every other splat" here -- the exact mask is a compiled-in option
+            if (prm.bin.hybrid) {
+                if (prm.color_rule != 0) dropped += bin_block_splat<5, true>(prm, s, sm, br, X, Y, K, ok);
+                else                     dropped += bin_block_splat<5, false>(prm, s, sm, br, X, Y, K, ok);
+            } else {
+                dropped += bin_block_splat<0, true>(prm, s, sm, br, X, Y, K, ok);    // br.ktp = 0 for HIST: k is ignored
+            }
         }
     } else {
 #pragma unroll(CHECKED ? 1 : 4)
@@ -271,11 +279,11 @@ __device__ __forceinline__ uint32_t iterate_block(const RenderParams &prm, const
             const int it = it0 + j;
             if (CHECKED && it >= prm.iterations) break;
             const uint32_t u = (j == 0) ? w.x : (j == 1) ? w.y : (j == 2) ? w.z : w.w;
-            const int k = pick_index(u, sm, prm);
+            const int k = pick_index<OPT>(u, sm, prm);
             apply_gen<DIM, AFF>(k, sm, prm, gx, gy, gz);
             const bool past = !CHECKED || it >= prm.burn_in;
             // hybrid stage (DESIGN "hybrid"): iterations 0 and 2 of a steady-state block splat straight to L2
-            const bool direct_half = SPLAT == SPLAT_BIN && !CHECKED && (j & 1) == 0 && prm.bin.hybrid != 0u;
+            const bool direct_half = SPLAT == SPLAT_BIN && !CHECKED && ((prm.bin.hybrid >> j) & 1u) != 0u;
             if (past || (SIG == kChainGeneric && prm.reuse) || kReuse)
                 dropped += chain_and_splat<DIM, GEN, SPLAT, SIG, TRIG, OPT>(prm, s, sm, s_hist, gx, gy, gz, k, 0u, have, past, br,
                                                                        StepCtx{plo, phi, it}, direct_half);
@@ -320,8 +328,9 @@ render_kernel(const __grid_constant__ RenderParams prm)
         // through shared memory on purpose: values read back from memory stay in registers for the
         // whole kernel, whereas values derived from the parameter block are re-derived (constant
         // loads + shifts) at every use, ~10 extra instructions per splat
-        if (threadIdx.x == 0) s_br = bin_regs_init(prm, s_hist);   // cnt[] of the staging rows; this lane's tile state
-        for (uint32_t i = threadIdx.x; i < prm.bin.n_tiles + kBinDummy; i += blockDim.x) s_hist[i] = 0u;
+        if (threadIdx.x == 0) s_br = bin_regs_init(prm, s_hist);   // the staging rows; this lane's tile state
+        for (uint32_t i = threadIdx.x; i < prm.bin.n_tiles + kBinDummy; i += blockDim.x)
+            s_hist[i] = (i < prm.bin.n_tiles) ? 0u : prm.bin.cap;   // fill counters; the dummy ones read "full"
         bin_lane_init(prm, bl);
     }
     __syncthreads();
@@ -357,6 +366,9 @@ render_kernel(const __grid_constant__ RenderParams prm)
                 gx = u24_to_pm1(w.x);
                 gy = u24_to_pm1(w.y);
                 if (DIM == 3) gz = u24_to_pm1(w.z);
+                // SPLAT_BIN keeps whole CTAs in the loop (barriers inside): a thread without a point carries NaN, which
+                // every map hands on and every bounds test rejects -- no `have` predicate in the steady-state body
+                if (SPLAT == SPLAT_BIN && !have) gx = __int_as_float(0x7FC00000);
             }
             // blocks touching burn-in or the ragged end take the checked path, the rest the lean one
             int it0 = 0;

@@ -541,7 +541,7 @@ def test_eq1_circle_generator_fig2(cfs, oracle, r2_reading, composition):
     o, oc, _ = oracle.render_parallel(sysc, wd.render)
     for variant in ("direct", "binned"):
         g, gc = gpu_render(cfs, wd, variant=variant, flags=["bin_hybrid"] if variant == "binned" else 0)
-        assert int(gc[0]) + int(gc[1]) == 480000 * 50 and abs(int(gc[0]) - int(oc[0])) <= 480
+        assert int(gc[0]) + int(gc[1]) == 2000000 * 50 and abs(int(gc[0]) - int(oc[0])) <= 2000
         for ch in range(4):
             if o[:, ch].sum() > 0:
                 assert density_l1(g[:, ch], o[:, ch]) <= L1_TOL, (variant, ch, density_l1(g[:, ch], o[:, ch]))
