@@ -1,13 +1,14 @@
 #!/usr/bin/env python
-"""bench.py -- throughput of the CFS hot path on B200 (BASELINE.json metric: point-iterations/s and
-splats/s, % of measured roofline).
+"""bench.py -- throughput of the CFS hot path on B200 (BASELINE.json metric: point-iterations/s and splats/s on one
+B200, % of measured roofline).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--no-workloads]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--headline CFG] [--configs 0,1,2,3,4]
 
-One "step" = one pass of the whole hot path over one batch: clear the image, cfs_render (sampler +
-pick + map + chain + colour + splat, one kernel) and cfs_tonemap, on BASELINE configs[1] (square
-generator -> swirl -> scale 0.8, colour by map index, 2^20 points x 1000 iterations, 1024x1024
-RGBA float32).  Prints ONE JSON line (see DESIGN.md "measurement" for every key).
+One "step" = one pass of the whole hot path over one batch of a workload: clear the image, cfs_render (sampler + pick +
+map + chain + colour + splat) and cfs_resolve_rgba8 (log-density tone map to the paper's RGBA8888 output), once per
+frame of the workload.  The bench line is on BASELINE configs[4] (the largest single-GPU workload: 2^26 points x 1000
+iterations, 4K depth buffer); the line also carries one first-class record per BASELINE config under "workloads", each
+with its own roofline, clocks and end-to-end figure.  Prints ONE JSON line (DESIGN.md "measurement" explains every key).
 """
 from __future__ import annotations
 
@@ -27,16 +28,11 @@ if ROOT not in sys.path:
 
 from paper_2606_02226_b200 import workloads as W  # noqa: E402  (inputs only, no arithmetic)
 
-HEADLINE_CFG = 1
-SINCOS = "sincosf (<= 2 ulp)"
+HEADLINE_CFG = 4
 METRIC = "cfs_point_iterations_per_s"
 UNIT = "point-iterations/s"
 L2_FLUSH_BYTES = 256 << 20
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the render kernel on configs[1], from
-# the `ncu --set full` captures summarised in profiles/README.md
-NCU_TRAFFIC_BYTES_PER_LAUNCH = 0.989e9       # hybrid pass 1: profiles/r01j_hybrid_cfg1.txt (0.008 GB read + 0.982 GB written)
-NCU_TRAFFIC_BYTES_PER_LAUNCH_BINNED = 2.0e9  # pure bins (--variant binned): twice the records of the hybrid stage
-NCU_TRAFFIC_BYTES_PER_LAUNCH_DIRECT = 7.06e6 # direct kernel: profiles/r01h_direct_cfg1.txt (the image stays in L2)
+GAMMA, COLOUR_SCALE = 2.2, 1.0 / 255.0
 
 
 # ----------------------------------------------------------------------------- clocks sampler
@@ -147,7 +143,28 @@ class ClockSampler:
                 "source": "nvidia-smi"}
 
 
-# ----------------------------------------------------------------------------- reference arm (oracle)
+# ----------------------------------------------------------------------------- workloads, method work per unit
+# Algorithmic lane-instructions per point-iteration: SURVEY 8(d) "algorithmic work per unit" (what the METHOD must do:
+# Philox 10, pick, coefficient fetch + map, chain, colour + pixel + reduction) for the sin/cos evaluation actually run.
+# Never the implementation's own bookkeeping (bin records, appends, Hi-Z tests): ncu's executed count is printed beside
+# it as overhead.
+N_INSTR_MUFU = {0: 30, 1: 45, 2: 42, 3: 60, 4: 52}
+N_INSTR_ACCURATE = {0: 30, 1: 80, 2: 80, 3: 130, 4: 52}
+N_IMAD_WIDE = {0: 5, 1: 5, 2: 5, 3: 0, 4: 5}          # Philox4x32-10: 20 IMAD.WIDE per block of 4 iterations
+N_XU = {0: 2, 1: 4, 2: 4, 3: 10, 4: 3}                  # MUFU sin/cos/rcp + F2I/I2F conversions (special-function unit)
+RED_KEY = {0: "red_add_u32@1048576", 1: "red_add_v4f32@16777216", 2: "red_add_v4f32@33177600",
+           3: "red_add_v4f32@132710400", 4: "atom_min_u64@66355200"}
+# executed warp-instructions per warp-iteration and DRAM bytes per launch of the dominant kernel: from the ncu captures
+# under profiles/ (file named beside each); None = not captured for the kernel as it stands
+NCU = {
+    1: {"executed_per_iteration": None, "dram_bytes_per_launch": None, "profile": None},
+    2: {"executed_per_iteration": None, "dram_bytes_per_launch": None, "profile": None},
+    3: {"executed_per_iteration": None, "dram_bytes_per_launch": None, "profile": None},
+    4: {"executed_per_iteration": None, "dram_bytes_per_launch": None, "profile": None},
+}
+PARAM_BLOCK_BYTES = 9800           # sizeof(cfs::RenderParams), travels host -> device with every launch
+
+
 def host_cpu_model() -> str:
     try:
         with open("/proc/cpuinfo") as fh:
@@ -159,17 +176,47 @@ def host_cpu_model() -> str:
     return "unknown"
 
 
-def oracle_sample(cfg: int, n_points: int):
-    """The oracle as it stands on a bounded sample (first n_points points) of configs[cfg], on all
-    host cores through its own multi-threaded driver. Returns (point_iterations, seconds, threads)."""
+def workload_desc(w, cfg, n_gpus, sincos):
+    r = w.render
+    return {"workload": f"BASELINE configs[{cfg}] {w.name}", "points_per_gpu": r.n_points, "frames": len(w.frames),
+            "iterations": r.iterations, "burn_in": r.burn_in, "image": f"{r.width}x{r.height} {r.out_mode}",
+            "chain": [x.type for x in w.system.chain], "n_funcs": len(w.system.funcs), "sincos": sincos,
+            "parallelism": f"points sharded over {n_gpus} GPU(s) by global point id, one image all-reduce" if n_gpus > 1 else "1 GPU",
+            "l2": "flushed between steps (256 MiB memset outside the per-step events)"}
+
+
+# ----------------------------------------------------------------------------- reference arm (the oracle, as it stands)
+CPU_SAMPLE_POINTS = {0: (1 << 13, 1 << 16), 1: (1 << 13, 1 << 16), 2: (1 << 14, 1 << 17), 3: (1 << 20, 1 << 22),
+                     4: (1 << 13, 1 << 16)}          # (1 core, all cores): ~1-3 s of CPU work each
+
+
+def oracle_sample(cfg: int, n_points: int, threads=None):
+    """The oracle as it stands on a bounded sample (first n_points points, middle frame) of configs[cfg].
+    Returns (point_iterations, seconds, threads used)."""
     from oracle import cfs_oracle
     w = W.config(cfg)
     cloud = W.gaussian_mixture_cloud(n_points, w.cloud_seed) if w.system.gen == "cloud" else None
     t = w.frames[len(w.frames) // 2]
     t0 = time.perf_counter()
-    _, _, threads = cfs_oracle.render_parallel(w.system, w.render, cloud=cloud, n_points=n_points, t=t)
-    dt = time.perf_counter() - t0
-    return n_points * w.render.iterations, dt, threads
+    if threads == 1:
+        cfs_oracle.render(w.system, w.render, cloud=cloud, n_points=n_points, t=t)
+        used = 1
+    else:
+        _, _, used = cfs_oracle.render_parallel(w.system, w.render, cloud=cloud, n_points=n_points, t=t)
+    return n_points * w.render.iterations, time.perf_counter() - t0, used
+
+
+def cpu_baseline_for(cfg: int):
+    n1, nall = CPU_SAMPLE_POINTS[cfg]
+    pi1, dt1, _ = oracle_sample(cfg, n1, threads=1)
+    pia, dta, used = oracle_sample(cfg, nall)
+    w = W.config(cfg)
+    return {"value": pia / dta, "unit": UNIT, "cores": used, "kind": "oracle",
+            "one_core": {"value": pi1 / dt1, "unit": UNIT, "cores": 1,
+                         "sample": f"first {n1} points x {w.render.iterations} iterations, middle frame, full image, {dt1:.2f} s"},
+            "sample": f"first {nall} points x {w.render.iterations} iterations of configs[{cfg}], middle frame, full image, "
+                      f"{dta:.2f} s wall on {used} threads",
+            "cpu": host_cpu_model(), "host_cores": os.cpu_count()}
 
 
 def run_reference(args):
@@ -178,38 +225,33 @@ def run_reference(args):
         return
     from oracle import build as oracle_build
     oracle_build.build()
-    n = 1 << 14
+    cfg = args.headline
+    n = CPU_SAMPLE_POINTS[cfg][1] // 4
     for _ in range(args.warmup):
-        oracle_sample(HEADLINE_CFG, n)
+        oracle_sample(cfg, n)
     tot_pi, tot_t, threads = 0, 0.0, 1
     for _ in range(args.steps):
-        pi, dt, threads = oracle_sample(HEADLINE_CFG, n)
+        pi, dt, threads = oracle_sample(cfg, n)
         tot_pi += pi
         tot_t += dt
-    w = W.config(HEADLINE_CFG)
+    w = W.config(cfg)
     value = tot_pi / tot_t
-    sample = f"first {n} points x {w.render.iterations} iterations of configs[{HEADLINE_CFG}] per step, full 1024x1024 image"
+    sample = (f"first {n} points x {w.render.iterations} iterations of configs[{cfg}] per step (middle frame), "
+              f"full {w.render.width}x{w.render.height} image")
+    config = workload_desc(w, cfg, args.gpus, "libm sin/cos in double (the oracle)")
+    config["points_per_step"] = n
+    config["note"] = "the oracle times a bounded SAMPLE of the workload per step: rates are comparable, sizes are not"
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": tot_t / args.steps * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": workload_config(w, args.gpus),
+        "config": config,
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample,
-                         "cpu": host_cpu_model()},
+                         "cpu": host_cpu_model(), "host_cores": os.cpu_count()},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
     print(json.dumps(line), flush=True)
-
-
-def workload_config(w, n_gpus):
-    r = w.render
-    return {"workload": f"BASELINE configs[{HEADLINE_CFG}] {w.name}", "points_per_gpu": r.n_points,
-            "iterations": r.iterations, "burn_in": r.burn_in, "image": f"{r.width}x{r.height} {r.out_mode}",
-            "chain": [x.type for x in w.system.chain], "n_funcs": len(w.system.funcs), "sincos": SINCOS,
-            "parallelism": f"points sharded over {n_gpus} GPU(s), image all-reduce" if n_gpus > 1 else "1 GPU",
-            "l2": "flushed between steps (256 MiB memset outside the per-step events); the 16 MiB image is "
-                  "L2-resident by design"}
 
 
 # ----------------------------------------------------------------------------- our arm
@@ -218,14 +260,14 @@ def event_pair(torch):
 
 
 def measure_rates(cfs, torch, buf, sms):
-    """Roofline denominators in the same run (BASELINE north_star)."""
+    """Roofline denominators in the same run (BASELINE north_star): lane-operations per second."""
     out = {}
 
     def rate(kind, fp, ops, blocks, threads, reps=3):
         best = None
         for _ in range(reps + 1):
             if kind == "atom_min_u64":
-                buf.fill_(255)
+                buf[: fp].fill_(255)
             e0, e1 = event_pair(torch)
             e0.record()
             cfs.cfs_microbench(kind, buf, fp, ops, blocks, threads)
@@ -241,91 +283,326 @@ def measure_rates(cfs, torch, buf, sms):
             out[f"{kind}@{fp}"] = rate(kind, fp, 1024, sms * 8, 256)
     for kind in ("ffma", "imad_wide", "lop3", "mufu"):
         out[kind] = rate(kind, 0, 1 << 15, sms * 8, 256)
+    out["atoms_add_u32@196608"] = rate("atoms_add_u32", 196608, 4096, sms, 1024)     # pass 2 of the tile bins: one CTA per SM
     best = None
     for _ in range(4):
         e0, e1 = event_pair(torch)
         e0.record()
-        cfs.cfs_microbench("stream_ld128", buf, buf.numel(), 0, sms * 16, 256)
+        cfs.cfs_microbench("stream_ld128", buf, L2_FLUSH_BYTES, 0, sms * 16, 256)
         e1.record()
         torch.cuda.synchronize()
         dt = e0.elapsed_time(e1) * 1e-3
         best = dt if best is None else min(best, dt)
-    out["stream_ld128_GBps"] = buf.numel() / best / 1e9
+    out["stream_ld128_GBps"] = L2_FLUSH_BYTES / best / 1e9
     return out
 
 
-# algorithmic lane-instructions per point-iteration (table "N_instr")
-N_INSTR = {0: 30, 1: 62, 2: 66, 3: 110, 4: 52}
-# the same for the binned variant with MUFU sin/cos (Philox 10, pick, LDS +
-# generator FMAs, chain, 4 bound compares, 9 pixel ops, 6 record ops, 4 append ops)
-N_INSTR_BIN = {0: 38, 1: 51, 2: 51}
-# hybrid (CFS_FLAG_BIN_HYBRID, what AUTO runs): every other splat skips the 6 record + 4 append operations and
-# pays a palette LDS + one red.global instead, i.e. 43 on those iterations: (51 + 43) / 2
-N_INSTR_HYB = {1: 47, 2: 47}
-# with sincosf (--accurate-trig): the direct count of N_INSTR on direct iterations, + 8 (6 record + 4 append - 2) on binned ones
-N_INSTR_HYB_ACC = {1: 66, 2: 70}
-N_INSTR_BIN_ACC = {0: 38, 1: 70, 2: 74}
-RED_KEY = {0: "red_add_u32@1048576", 1: "red_add_v4f32@16777216", 2: "red_add_v4f32@33177600",
-           3: "red_add_v4f32@132710400", 4: "atom_min_u64@66355200"}
+def cloud_shape_rate(cfs, torch, buf, sms, n_records, footprint_bytes):
+    """configs[3]'s own denominator: records/s at which a 16-byte record stream and one red.v4.f32 per record over a
+    hot set of `footprint_bytes` (the pixels the render really touched) go through the L2 at the same time."""
+    blocks, threads = sms * 8, 256
+    ops = max(1, n_records // (blocks * threads))
+    assert blocks * threads * ops * 16 + footprint_bytes <= buf.numel()
+    best = None
+    for _ in range(4):
+        e0, e1 = event_pair(torch)
+        e0.record()
+        cfs.cfs_microbench("stream_red_v4f32", buf, footprint_bytes, ops, blocks, threads)
+        e1.record()
+        torch.cuda.synchronize()
+        dt = e0.elapsed_time(e1) * 1e-3
+        best = dt if best is None else min(best, dt)
+    return blocks * threads * ops / best
 
 
-def roofline_for(cfg, w, rates, peaks, splats, seconds):
-    """t_roof = max(t_issue, t_atomic, t_hbm); frac = t_roof / t."""
-    pi = w.render.n_points * w.render.iterations
-    t_issue = pi * N_INSTR[cfg] / rates["ffma"]
-    t_atom = splats / rates[RED_KEY[cfg]]
-    t_hbm = (w.render.n_points * 16 / (peaks["hbm_gbs"] * 1e9)) if w.system.gen == "cloud" else 0.0
-    t_roof = max(t_issue, t_atom, t_hbm)
-    bound = "alu" if t_roof == t_issue else ("l2_atomic" if t_roof == t_atom else "hbm")
-    return {"bound": bound, "t_issue_ms": t_issue * 1e3, "t_atomic_ms": t_atom * 1e3, "t_hbm_ms": t_hbm * 1e3,
-            "t_roof_ms": t_roof * 1e3, "t_ms": seconds * 1e3, "frac": t_roof / seconds}
+class ConfigBench:
+    """One BASELINE config on this rank: device buffers, the step, device timing, end-to-end timing, roofline."""
+
+    def __init__(self, cfs, torch, cfg, args, rank, world, flush):
+        self.cfs, self.torch, self.cfg, self.args, self.rank, self.world, self.flush = cfs, torch, cfg, args, rank, world, flush
+        self.w = W.config(cfg)
+        r = self.w.render
+        self.P, self.I, self.F = r.n_points, r.iterations, len(self.w.frames)
+        self.S = r.n_points * (r.iterations - r.burn_in)
+        self.cloud = W.gaussian_mixture_cloud(r.n_points, self.w.cloud_seed) if self.w.system.gen == "cloud" else None
+        self.d_cloud = cfs.cloud_to_device(self.cloud) if self.cloud is not None else None
+        self.sysh = cfs.cfs_create(self.w.system)
+        self.img = cfs.new_image(r)
+        self.ctr = torch.zeros(2, dtype=torch.int64, device="cuda")
+        self.out8 = torch.zeros(r.width * r.height, dtype=torch.int32, device="cuda")
+        self.tone = torch.zeros(4, dtype=torch.int32, device="cuda")
+        self.flags = (["fast_trig"] if args.fast_trig else []) + (["jit"] if args.jit else [])
+        need = cfs.cfs_binned_scratch_bytes(self.sysh, cfs.make_args(r))
+        if r.out_mode == "depth_u64":
+            need = cfs.cfs_hiz_scratch_bytes(r.width, r.height)
+        self.scratch_bytes = min(need, args.scratch_mib << 20) if args.variant == "auto" else 0
+        self.scratch = torch.empty(self.scratch_bytes, dtype=torch.uint8, device="cuda") if self.scratch_bytes else None
+        self.compile_ms = 0.0
+        if args.jit:
+            for t in self.w.frames[:1]:
+                self.compile_ms += cfs.cfs_specialize(self.sysh, self.make_args(t))
+
+    def make_args(self, t, extra_flags=()):
+        return self.cfs.make_args(self.w.render, d_image=self.img, d_cloud=self.d_cloud, d_counters=self.ctr, t=t,
+                                  point_offset=self.rank * self.P, flags=list(self.flags) + list(extra_flags),
+                                  variant=self.args.variant, d_scratch=self.scratch)
+
+    def step(self):
+        """clear + render + resolve for every frame; returns (e_start, e_render_end_of_last_frame, e_end)."""
+        cfs, torch, r = self.cfs, self.torch, self.w.render
+        self.flush.zero_()                         # L2 flush, outside the events
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        ev[0].record()
+        for k, t in enumerate(self.w.frames):
+            self.img.fill_(-1 if r.out_mode == "depth_u64" else 0)
+            cfs.cfs_render(self.sysh, self.make_args(t))
+            if self.world > 1:                     # the exchange step: one image all-reduce (sum / unsigned min)
+                cfs.allreduce_image(self.img, r.out_mode)
+            # frame 0 measures its maximum inside the launch; an in-between frame is mapped with the previous frame's
+            cfs.cfs_resolve_rgba8(self.img, r.out_mode, r.width, r.height, GAMMA, COLOUR_SCALE, 0.0 if k == 0 else -1.0,
+                                  self.out8, self.tone)
+        ev[1].record()
+        return ev
+
+    def time_render_only(self, extra_flags=(), reps=5):
+        """median device time of the cfs_render calls of one step (all frames), image clears outside the events"""
+        torch, r = self.torch, self.w.render
+        times = []
+        for i in range(reps + 1):
+            self.flush.zero_()
+            tot = 0.0
+            for t in self.w.frames:
+                self.img.fill_(-1 if r.out_mode == "depth_u64" else 0)
+                e0, e1 = event_pair(torch)
+                e0.record()
+                self.cfs.cfs_render(self.sysh, self.make_args(t, extra_flags))
+                e1.record()
+                torch.cuda.synchronize()
+                tot += e0.elapsed_time(e1) * 1e-3
+            if i >= 1:
+                times.append(tot)
+        return float(np.median(times))
+
+    def close(self):
+        self.sysh.close()
 
 
-SCRATCH_CAP_BYTES = 8 << 30
+def path_roofline(cb, rates, peaks, t_render, t_pass1, launches_per_render, hot_rate):
+    """Two bounds per config, both from quantities on this line (DESIGN "rooflines"):
+    north_star = max(t_issue, t_atomic, t_hbm) for the METHOD (one global reduction per splat);
+    path       = the bound of the variant that was timed (bins skip the L2 reduction, Hi-Z skips the pre-test load)."""
+    cfg, w = cb.cfg, cb.w
+    pi = cb.P * cb.I * cb.F
+    S = cb.S * cb.F
+    n_instr = (N_INSTR_MUFU if cb.args.fast_trig else N_INSTR_ACCURATE)[cfg]
+    t_issue_all = pi * n_instr / rates["ffma"]
+    t_iw = pi * N_IMAD_WIDE[cfg] / rates["imad_wide"]
+    t_xu = pi * N_XU[cfg] / rates["mufu"]
+    t_issue = max(t_issue_all, t_iw, t_xu)
+    t_atomic = S / rates[RED_KEY[cfg]]
+    t_hbm = (cb.P * 16 / (peaks["hbm_gbs"] * 1e9)) if w.system.gen == "cloud" else 0.0
+    ns = max(t_issue, t_atomic, t_hbm)
+    out = {"n_instr_method": n_instr, "t_issue_ms": t_issue * 1e3,
+           "t_issue_terms_ms": {"all_pipes": t_issue_all * 1e3, "imad_wide": t_iw * 1e3, "xu": t_xu * 1e3},
+           "t_issue_nominal_ms": pi * n_instr / (148 * 128 * 1.965e9) * 1e3,
+           "t_atomic_ms": t_atomic * 1e3, "t_hbm_ms": t_hbm * 1e3,
+           "north_star": {"t_roof_ms": ns * 1e3, "frac": ns / t_render,
+                          "bound": "alu" if ns == t_issue else ("l2_atomic" if ns == t_atomic else "hbm")}}
+    hbm = peaks["hbm_gbs"] * 1e9
+    if launches_per_render >= 2 and w.render.out_mode != "depth_u64":      # tile bins (hybrid): pass 1 + pass 2
+        f = bin(cb.args.direct_mask).count("1") / 4.0
+        p1 = {"issue": t_issue, "l2_red_direct_share": f * S / rates[RED_KEY[cfg]], "hbm_record_write": (1 - f) * S * 2 / hbm}
+        p2 = {"hbm_record_read": (1 - f) * S * 2 / hbm, "shared_atomics": (1 - f) * S / (rates["atoms_add_u32@196608"])}
+        t_path = max(p1.values()) + max(p2.values())
+        out["path"] = {"variant": f"hybrid tile bins, {f:.2f} of the splats straight to L2", "t_roof_ms": t_path * 1e3,
+                       "frac": t_path / t_render, "pass1_terms_ms": {k: v * 1e3 for k, v in p1.items()},
+                       "pass2_terms_ms": {k: v * 1e3 for k, v in p2.items()},
+                       "pass1_ms": t_pass1 * 1e3 if t_pass1 else None,
+                       "pass2_ms": (t_render - t_pass1) * 1e3 if t_pass1 else None,
+                       "bound": "alu" if max(p1, key=p1.get) == "issue" else max(p1, key=p1.get)}
+    elif w.system.gen == "cloud":
+        t_hot = cb.P / hot_rate if hot_rate else t_atomic
+        t_path = max(t_issue, t_hbm, t_hot)
+        out["path"] = {"variant": "streamed cloud, one L2 reduction per record", "t_roof_ms": t_path * 1e3, "frac": t_path / t_render,
+                       "t_stream_and_red_ms": t_hot * 1e3,
+                       "bound": "l2 (record stream + one reduction per record over the touched pixels, same-run microbenchmark)"
+                       if t_path == t_hot else ("hbm" if t_path == t_hbm else "alu")}
+    elif w.render.out_mode == "depth_u64":
+        t_ld = S / rates["ld_u64@66355200"]
+        hiz = launches_per_render > 1
+        t_path = t_issue if hiz else max(t_issue, t_ld)
+        out["path"] = {"variant": "Hi-Z pre-test in shared memory (occluded splats never leave the SM)" if hiz else "direct: one L2 sector load per splat",
+                       "t_roof_ms": t_path * 1e3, "frac": t_path / t_render, "t_random_sector_load_ms": t_ld * 1e3,
+                       "bound": "alu" if t_path == t_issue else "l2 random sector loads"}
+        out["north_star"]["t_algorithmic_minimum_ms"] = t_ld * 1e3
+    else:
+        out["path"] = {"variant": "direct: one L2 reduction per splat", "t_roof_ms": ns * 1e3, "frac": ns / t_render,
+                       "bound": out["north_star"]["bound"]}
+    return out
 
 
-def make_scratch(cfs, torch, sysh, render):
-    """Scratch of the tile-binned variant (None when the variant cannot serve the workload)."""
-    need = cfs.cfs_binned_scratch_bytes(sysh, cfs.make_args(render))
-    if need == 0:
+def measure_config(cfs, torch, cfg, args, rank, world, flush, rates, peaks, peaks_src, steps, warmup, dist, big):
+    """One first-class record: device-timed steps, clocks during them, end to end through the HOST entry point,
+    roofline, launches."""
+    cb = ConfigBench(cfs, torch, cfg, args, rank, world, flush)
+    w, r = cb.w, cb.w.render
+    for _ in range(max(warmup, 3)):
+        cb.step()
+    torch.cuda.synchronize()
+    cb.ctr.zero_()
+    cfs.cfs_launch_count(reset=True)
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    try:
+        dev_uuid = torch.cuda.get_device_properties(torch.cuda.current_device()).uuid
+    except Exception:
+        dev_uuid = None
+    sampler = ClockSampler(torch.cuda.current_device(), dev_uuid)
+    if rank == 0:
+        sampler.start()
+    evs = [cb.step() for _ in range(steps)]
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    launches = cfs.cfs_launch_count()
+    n_in, n_drop = int(cb.ctr[0].item()), int(cb.ctr[1].item())
+    assert n_in + n_drop == cb.S * cb.F * steps, f"conservation violated on configs[{cfg}]: {n_in} + {n_drop} != {cb.S * cb.F * steps}"
+    step_s = sum(e[0].elapsed_time(e[1]) for e in evs) * 1e-3
+    tt = torch.tensor([step_s], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    step_s = float(tt[0])
+
+    # ---- the render alone, and pass 1 of the tile bins alone (same launch shape)
+    t_render = cb.time_render_only()
+    launches_per_render = (launches // steps) // cb.F - 1            # minus the resolve kernel
+    t_pass1 = None
+    if launches_per_render >= 2 and r.out_mode != "depth_u64":
+        t_pass1 = cb.time_render_only(extra_flags=["bin_pass1_only"])
+    hot_rate = None
+    touched_px = None
+    if w.system.gen == "cloud":
+        touched_px = int((cb.img[:, 3] > 0).sum().item())
+        hot_rate = cloud_shape_rate(cfs, torch, big, torch.cuda.get_device_properties(0).multi_processor_count, cb.P, touched_px * 16)
+
+    # ---- end to end through the C ABI with HOST buffers (pinned): H2D of the inputs, render, resolve, D2H of the RGBA8888 image
+    h_out = torch.empty(r.width * r.height, dtype=torch.int32).pin_memory()
+    h_ctr = torch.zeros(2, dtype=torch.int64).pin_memory()
+    h_cloud = None
+    if cb.cloud is not None:
+        h_cloud_t = torch.from_numpy(cb.cloud.view(np.uint8).reshape(-1, 16)).pin_memory()
+        h_cloud = h_cloud_t.numpy()
+    hargs = [cfs.make_args(r, point_offset=rank * cb.P, t=t, flags=cb.flags, variant=args.variant) for t in w.frames]
+
+    def e2e_step():
+        for k, ha in enumerate(hargs):
+            cfs.cfs_render_rgba8_host(cb.sysh, ha, GAMMA, COLOUR_SCALE, 0.0 if k == 0 else -1.0, h_out.numpy(), h_cloud, h_ctr.numpy())
+
+    e2e_step()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    n_e2e = max(2, min(steps, 5))
+    t0 = time.perf_counter()
+    for _ in range(n_e2e):
+        e2e_step()
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    te = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(te, op=dist.ReduceOp.MAX)
+    e2e_s = float(te[0])
+    assert int(h_ctr[0]) + int(h_ctr[1]) == cb.S
+
+    pi_step = cb.P * cb.I * cb.F
+    rec = None
+    if rank == 0:
+        roof = path_roofline(cb, rates, peaks, t_render, t_pass1, launches_per_render + 0, hot_rate)
+        dominant_ms = (t_pass1 if t_pass1 else t_render) * 1e3
+        image_bytes = r.width * r.height * {"hist_u32": 4, "rgba_f32": 16, "depth_u64": 8}[r.out_mode]
+        algo_bytes = (image_bytes + (cb.P * 16 if w.system.gen == "cloud" else 0)) * cb.F
+        ncu = NCU.get(cfg, {})
+        traffic = ncu.get("dram_bytes_per_launch")
+        n_instr = roof["n_instr_method"]
+        achieved = pi_step * n_instr / (dominant_ms * 1e-3)
+        roofline = {
+            "bound": roof["path"]["bound"], "frac": roof["path"]["frac"], "t_roof_ms": roof["path"]["t_roof_ms"], "t_render_ms": t_render * 1e3,
+            "definition": "frac = t_roof(path) / t_render; every term is on this line (microbench rates, method counts)",
+            "achieved": achieved / 1e12, "peak": rates["ffma"] / 1e12, "unit": "T lane-instructions/s",
+            "achieved_over_peak": achieved / rates["ffma"],
+            "peak_source": "FFMA lane-issue rate, cfs_microbench in this run; nominal 148 SMs x 128 lanes x 1.965 GHz = 37.2",
+            "kernel": "render kernel(s) of one cfs_render" if not t_pass1 else "pass 1 of the tile bins (sample + chain + bin)",
+            "kernel_ms": dominant_ms, "traffic": traffic, "algorithmic_bytes_per_step": algo_bytes,
+            "traffic_over_algorithmic": (traffic / algo_bytes) if traffic else None,
+            "executed_instructions_per_iteration_ncu": ncu.get("executed_per_iteration"), "ncu_profile": ncu.get("profile"),
+            "hbm_peak_gbs": peaks.get("hbm_gbs"), "hbm_peak_source": peaks_src,
+        }
+        roofline.update({k: v for k, v in roof.items() if k not in ("path",)})
+        roofline["path"] = roof["path"]
+        if touched_px is not None:
+            roofline["touched_pixels"] = touched_px
+            roofline["stream_plus_red_rate_G_per_s"] = hot_rate / 1e9
+        h2d = (cb.P * 16 if cb.cloud is not None else 0) * 1 + PARAM_BLOCK_BYTES * (launches_per_render + 1) * cb.F
+        rec = {
+            "config": workload_desc(w, cfg, world, "MUFU sin.approx/cos.approx (CFS_FLAG_FAST_TRIG)" if args.fast_trig else "sincosf (<= 2 ulp)"),
+            "value": world * pi_step * steps / step_s, "unit": UNIT, "splats_per_s": world * (n_in / steps) / (step_s / steps),
+            "steps": steps, "ms_per_step": step_s / steps * 1e3, "render_ms": t_render * 1e3,
+            "in_bounds_per_step": n_in // steps, "dropped_per_step": n_drop // steps,
+            "clocks": clocks, "gpu_launches": int(launches), "launches_per_render": launches_per_render,
+            "kernels": "run-time compiled for the system (CFS_FLAG_JIT; compile time below, outside the timed region)" if args.jit else "linked ahead of time",
+            "jit_compile_ms": cb.compile_ms,
+            "scratch_bytes": cb.scratch_bytes,
+            "e2e": {"value": world * pi_step * n_e2e / e2e_s, "unit": UNIT, "ms_per_step": e2e_s / n_e2e * 1e3,
+                    "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int((r.width * r.height * 4 + 16) * cb.F),
+                    "note": "cfs_render_rgba8_host per frame: H2D of the cloud (configs[3]) and of the parameter blocks, clear, render, "
+                            "resolve to RGBA8888, D2H of the image and counters into pinned host memory"},
+            "roofline": roofline,
+        }
+    cb.close()
+    del cb
+    torch.cuda.empty_cache()
+    return rec
+
+
+def respawn_under_torchrun(args):
+    """`python bench.py --gpus N` without a launcher: start the N ranks ourselves (one process per GPU, NCCL)."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    env = dict(os.environ)
+    env.setdefault("NCCL_DEBUG", "INFO")
+    env.setdefault("NCCL_DEBUG_FILE", os.path.join(ROOT, "gpurun_out", "nccl_rank%h_%p.log"))
+    os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    raise SystemExit(subprocess.call(cmd, env=env))
+
+
+def nccl_summary():
+    """A few lines of NCCL's own log (communicator, transport, NVLS) when NCCL_DEBUG_FILE was set by the respawn."""
+    pat = os.environ.get("NCCL_DEBUG_FILE")
+    if not pat:
         return None
-    return torch.empty(min(need, SCRATCH_CAP_BYTES), dtype=torch.uint8, device="cuda")
-
-
-def time_workload(cfs, torch, cfg, flush, reps=5, flags=0, variant="auto"):
-    """Median device time of one cfs_render of configs[cfg] (all frames for cfg 2)."""
-    w = W.config(cfg)
-    cloud = W.gaussian_mixture_cloud(w.render.n_points, w.cloud_seed) if w.system.gen == "cloud" else None
-    d_cloud = cfs.cloud_to_device(cloud) if cloud is not None else None
-    sysh = cfs.cfs_create(w.system)
-    img = cfs.new_image(w.render)
-    ctr = torch.zeros(2, dtype=torch.int64, device="cuda")
-    scratch = make_scratch(cfs, torch, sysh, w.render) if variant != "direct" else None
-    times = []
-    n_rep = reps if cfg != 4 else 3
-    for rep in range(n_rep + 2):
-        flush.zero_()
-        tot = 0.0
-        ctr.zero_()
-        for t in w.frames:
-            img.fill_(-1 if w.render.out_mode == "depth_u64" else 0)
-            args = cfs.make_args(w.render, d_image=img, d_cloud=d_cloud, d_counters=ctr, t=t, flags=flags,
-                                 variant=variant, d_scratch=scratch)
-            e0, e1 = event_pair(torch)
-            e0.record()
-            cfs.cfs_render(sysh, args)
-            e1.record()
-            torch.cuda.synchronize()
-            tot += e0.elapsed_time(e1) * 1e-3
-        if rep >= 2:
-            times.append(tot)
-    sec = float(np.median(times))
-    c = ctr.cpu().numpy()
-    sysh.close()
-    return w, sec, int(c[0]), int(c[1])
+    import glob
+    lines = []
+    for f in sorted(glob.glob(os.path.join(os.path.dirname(pat), "nccl_rank*.log")))[:1]:
+        try:
+            for ln in open(f, errors="replace"):
+                if any(k in ln for k in ("NCCL version", "comm 0x", "NVLS", "via P2P", "Connected all", "Channel 00/")):
+                    lines.append(ln.strip()[:200])
+                if len(lines) >= 12:
+                    break
+        except OSError:
+            pass
+    return lines or None
 
 
 def run_ours(args):
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        respawn_under_torchrun(args)
     import torch
     import torch.distributed as dist
     from paper_2606_02226_b200 import cfs
@@ -339,198 +616,63 @@ def run_ours(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     cfs.lib()
+    if args.jit:
+        try:                                   # run-time compilation available on this box?
+            probe = cfs.cfs_create(W.config(0).system)
+            cfs.cfs_jit_check(probe, cfs.make_args(W.config(0).render))
+            probe.close()
+        except cfs.CfsError as e:
+            args.jit = False
+            args.jit_unavailable = str(e)[:200]
     sms = torch.cuda.get_device_properties(local).multi_processor_count
     peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(peaks_path):
         with open(peaks_path) as fh:
             peaks = json.load(fh)
-        peaks_src = "measured"
+        peaks_src = "measured (MEASURED_PEAKS.json)"
     else:
-        peaks, peaks_src = {"hbm_gbs": 6650.0}, "fallback"
-
-    w = W.config(HEADLINE_CFG)
-    r = w.render
-    P, I, S = r.n_points, r.iterations, r.n_points * (r.iterations - r.burn_in)
-    sysh = cfs.cfs_create(w.system)
-    img = cfs.new_image(r)
-    ctr = torch.zeros(2, dtype=torch.int64, device="cuda")
-    out8 = torch.zeros(r.width * r.height, dtype=torch.int32, device="cuda")
-    scratch = torch.zeros(2, dtype=torch.int32, device="cuda")
+        peaks, peaks_src = {"hbm_gbs": 6650.0}, "fallback (B200_PROFILING.md)"
     flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device="cuda")
-    # weak scaling: every rank renders its own P points of the global point-id space
-    flags = ["fast_trig"] if args.fast_trig else 0
-    scratch_t = make_scratch(cfs, torch, sysh, r) if args.variant != "direct" else None
-    rargs = cfs.make_args(r, d_image=img, d_counters=ctr, point_offset=rank * P, flags=flags, variant=args.variant,
-                          d_scratch=scratch_t)
+    big = torch.zeros(512 << 20, dtype=torch.uint8, device="cuda")          # microbenchmark arena (cloud stream + hot set)
+    rates = measure_rates(cfs, torch, big, sms)
 
-    def step(timed):
-        flush.zero_()                         # L2 flush, outside the events
-        ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
-        ev[0].record()
-        img.zero_()
-        cfs.cfs_render(sysh, rargs)
-        ev[1].record()
-        if world > 1:                          # the exchange step: one image all-reduce (sum)
-            cfs.allreduce_image(img, r.out_mode)
-        cfs.cfs_tonemap(img, r.out_mode, r.width, r.height, 2.2, 1 / 255.0, out8, scratch)
-        ev[2].record()
-        return ev
-
-    for _ in range(max(args.warmup, 3)):
-        step(False)
-    torch.cuda.synchronize()
-    rates = measure_rates(cfs, torch, flush, sms) if rank == 0 else None
-    ctr.zero_()
-    cfs.cfs_launch_count(reset=True)
-    if world > 1:
-        dist.barrier()
-    torch.cuda.synchronize()
-    try:
-        dev_uuid = torch.cuda.get_device_properties(local).uuid
-    except Exception:
-        dev_uuid = None
-    sampler = ClockSampler(local, dev_uuid)
-    if rank == 0:
-        sampler.start()
-    evs = [step(True) for _ in range(args.steps)]
-    torch.cuda.synchronize()
-    if world > 1:
-        dist.barrier()
-    clocks = sampler.stop() if rank == 0 else None
-    launches = cfs.cfs_launch_count()
-    in_bounds = int(ctr[0].item())
-    assert in_bounds == S * args.steps, f"conservation violated: {in_bounds} != {S * args.steps}"
-    launches_per_render = (launches // max(args.steps, 1)) - 2        # minus the two tone-map kernels
-    pass1_s = None
-    if launches_per_render >= 2:       # binned: time pass 1 (sample + bin) apart from pass 2, same launch shape
-        p1args = cfs.make_args(r, d_image=img, point_offset=rank * P, variant=args.variant,
-                               flags=(["fast_trig"] if args.fast_trig else []) + ["bin_pass1_only"], d_scratch=scratch_t)
-        ts = []
-        for i in range(7):
-            flush.zero_()
-            e0, e1 = event_pair(torch)
-            e0.record()
-            cfs.cfs_render(sysh, p1args)
-            e1.record()
-            torch.cuda.synchronize()
-            if i >= 2:
-                ts.append(e0.elapsed_time(e1) * 1e-3)
-        pass1_s = float(np.median(ts))
-    step_s = sum(e[0].elapsed_time(e[2]) for e in evs) * 1e-3
-    render_s = sum(e[0].elapsed_time(e[1]) for e in evs) * 1e-3
-    tt = torch.tensor([step_s, render_s], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-    step_s, render_s = float(tt[0]), float(tt[1])
-
-    # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
-    h_img = torch.empty((r.width * r.height, 4), dtype=torch.float32).pin_memory()
-    h_ctr = torch.zeros(2, dtype=torch.int64).pin_memory()
-    hargs = cfs.make_args(r, point_offset=rank * P, flags=flags)
-    for _ in range(2):
-        cfs.cfs_render_host(sysh, hargs, h_img.numpy(), None, h_ctr.numpy())
-    torch.cuda.synchronize()
-    if world > 1:
-        dist.barrier()
-    n_e2e = max(3, min(args.steps, 10))
-    t0 = time.perf_counter()
-    for _ in range(n_e2e):
-        cfs.cfs_render_host(sysh, hargs, h_img.numpy(), None, h_ctr.numpy())
-    torch.cuda.synchronize()
-    e2e_s = time.perf_counter() - t0
-    te = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e_s = float(te[0])
-    assert int(h_ctr[0]) == S
-
+    cfgs = [args.headline] + [c for c in args.configs if c != args.headline]
+    records = {}
+    for cfg in cfgs:
+        if world > 1 and cfg != args.headline:
+            continue                                  # the scaling run times the headline workload only
+        steps = args.steps if cfg == args.headline else max(3, min(args.steps, args.side_steps))
+        records[cfg] = measure_config(cfs, torch, cfg, args, rank, world, flush, rates, peaks, peaks_src, steps, args.warmup,
+                                      dist, big)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
 
-    ms_per_step = step_s / args.steps * 1e3
-    value = world * P * I * args.steps / step_s
-    t_render = render_s / args.steps
-    roof = roofline_for(HEADLINE_CFG, w, rates, peaks, S, t_render)
-    binned = launches_per_render >= 2
-    north_star = {"definition": "t_roof / t_render, t_roof = max(t_issue, t_atomic, t_hbm) (BASELINE north_star; "
-                                "the L2-atomic term assumes one reduction per splat, which the binned variant does not pay)",
-                  "bound": roof["bound"], "frac": roof["frac"], "t_issue_ms": roof["t_issue_ms"],
-                  "t_atomic_ms": roof["t_atomic_ms"], "t_render_ms": t_render * 1e3}
-    if binned:
-        # dominant kernel: pass 1 (sample + chain + bin), bound by instruction issue
-        hybrid = args.variant == "auto"
-        if args.fast_trig:
-            n_instr = N_INSTR_HYB[HEADLINE_CFG] if hybrid else N_INSTR_BIN[HEADLINE_CFG]
-        else:
-            n_instr = N_INSTR_HYB_ACC[HEADLINE_CFG] if hybrid else N_INSTR_BIN_ACC[HEADLINE_CFG]
-        roofline = {
-            "bound": "alu", "achieved": P * I * n_instr / pass1_s / 1e12, "peak": rates["ffma"] / 1e12,
-            "unit": "T lane-instructions/s", "frac": (P * I * n_instr / pass1_s) / rates["ffma"],
-            "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH if hybrid else NCU_TRAFFIC_BYTES_PER_LAUNCH_BINNED,
-            "kernel": "cfs::render_kernel<2,IFS,DIAG,BIN,swirl+scale,%s>" % ("MUFU" if args.fast_trig else "sincosf"),
-            "kernel_ms": pass1_s * 1e3, "render_ms": t_render * 1e3, "pass2_ms": (t_render - pass1_s) * 1e3,
-            "algorithmic_lane_instructions_per_point_iteration": n_instr,
-            "algorithmic_bytes_per_launch": int(S * 2) // (2 if hybrid else 1),      # one 16-bit record per binned splat
-            "peak_source": "FFMA lane-issue rate of cfs_microbench in this run (148 SMs x 128 lanes x SM clock)",
-            "hbm_peak_gbs": peaks.get("hbm_gbs"), "hbm_peak_source": peaks_src,
-            "pass2_hbm_gbs": (S * 2 // (2 if hybrid else 1)) / max(t_render - pass1_s, 1e-9) / 1e9,
-        }
-    else:
-        peak_red = rates[RED_KEY[HEADLINE_CFG]]
-        roofline = {
-            "bound": roof["bound"], "achieved": S / t_render / 1e9,
-            "peak": (peak_red / 1e9) if roof["bound"] == "l2_atomic" else S / (roof["t_roof_ms"] * 1e-3) / 1e9,
-            "unit": "Gsplat/s (one red.global.add.v4.f32 per splat)", "frac": roof["frac"],
-            "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH_DIRECT, "kernel": "cfs::render_kernel<2,IFS,DIAG,RGBA,swirl+affine>",
-            "kernel_ms": t_render * 1e3, "t_issue_ms": roof["t_issue_ms"], "t_atomic_ms": roof["t_atomic_ms"],
-            "peak_source": "red.global.add.v4.f32 at uniformly random pixels of a 16 MiB footprint, cfs_microbench "
-                           "in this run (BASELINE north_star); FFMA issue rate from the same run for t_issue",
-            "hbm_peak_gbs": peaks.get("hbm_gbs"), "hbm_peak_source": peaks_src,
-        }
+    head = records[args.headline]
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-        "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": workload_config(w, world),
-        "splats_per_s": world * S * args.steps / step_s,
-        "clocks": clocks, "gpu_launches": int(launches),
-        "e2e": {"value": world * P * I * n_e2e / e2e_s, "unit": UNIT,
-                "h2d_bytes_per_step": 0, "d2h_bytes_per_step": int(h_img.numel() * 4 + 16),
-                "note": "cfs_render_host: clear + render + D2H of the float32 accumulators and counters into pinned "
-                        "host memory; this workload has no host input besides the kernel parameter block"},
-        "roofline": roofline, "north_star_roofline": north_star,
-        "splat_variant": ("hybrid: every other splat straight to L2 (red.global), the rest through tile bins in scratch with shared-memory "
-                          "tile accumulation (CFS_FLAG_BIN_HYBRID, set by AUTO)" if args.variant == "auto" else
-                          "binned (tile bins through scratch, shared-memory tile accumulation)") if binned else "direct (one L2 reduction per splat)",
+        "metric": METRIC, "value": head["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": head["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": head["config"],
+        "splats_per_s": head["splats_per_s"], "clocks": head["clocks"], "gpu_launches": head["gpu_launches"],
+        "e2e": head["e2e"], "roofline": head["roofline"],
+        "kernels": head["kernels"], "jit_compile_ms": head["jit_compile_ms"],
         "microbench": {k: (v / 1e9 if not k.endswith("GBps") else v) for k, v in rates.items()},
-        "microbench_unit": "G lane-ops/s (stream: GB/s)",
+        "microbench_unit": "G lane-ops/s (stream: GB/s); one SASS instruction per op for ffma / imad_wide / lop3 / mufu",
+        "workloads": {f"cfg{c}": records[c] for c in sorted(records)},
     }
-
-    # ---- the other four workloads of BASELINE.json (same metric; not bench lines of their own)
-    if not args.no_workloads and world == 1:
-        wl = {}
-        for cfg in range(W.N_CONFIGS):
-            wk, sec, n_in, n_drop = time_workload(cfs, torch, cfg, flush, flags=flags, variant=args.variant)
-            pi = wk.point_iterations
-            rf = roofline_for(cfg, wk, rates, peaks, n_in / len(wk.frames), sec / len(wk.frames))
-            wl[f"cfg{cfg}"] = {"name": wk.name, "ms": sec * 1e3, "point_iterations_per_s": pi / sec,
-                               "splats_per_s": n_in / sec, "in_bounds": n_in, "dropped": n_drop,
-                               "roofline_bound": rf["bound"], "roofline_frac": rf["frac"],
-                               "t_issue_ms": rf["t_issue_ms"] * len(wk.frames),
-                               "t_atomic_ms": rf["t_atomic_ms"] * len(wk.frames),
-                               "t_hbm_ms": rf["t_hbm_ms"] * len(wk.frames)}
-        line["workloads"] = wl
-
-    # ---- the oracle timed beside it (reported baseline, never tuned)
-    n_cpu = 1 << 17
-    pi, dt, threads = oracle_sample(HEADLINE_CFG, n_cpu)
-    line["cpu_baseline"] = {"value": pi / dt, "unit": UNIT, "cores": threads, "kind": "oracle",
-                            "sample": f"first {n_cpu} points x {I} iterations of configs[{HEADLINE_CFG}], full image, "
-                                      f"{dt:.1f} s wall on {threads} threads", "cpu": host_cpu_model(),
-                            "host_cores": os.cpu_count()}
+    if getattr(args, "jit_unavailable", None):
+        line["jit_unavailable"] = args.jit_unavailable
+    if world > 1:
+        line["nccl"] = nccl_summary()
+    if world == 1 and not args.no_cpu_baseline:
+        # ---- the oracle timed beside it on this box's host cores (reported baseline, never tuned)
+        line["cpu_baseline"] = cpu_baseline_for(args.headline)
+        for c in sorted(records):
+            if c != args.headline:
+                line["workloads"][f"cfg{c}"]["cpu_baseline"] = cpu_baseline_for(c)
+        line["workloads"][f"cfg{args.headline}"]["cpu_baseline"] = line["cpu_baseline"]
     print(json.dumps(line), flush=True)
-    sysh.close()
     if world > 1:
         dist.destroy_process_group()
 
@@ -543,15 +685,20 @@ def run_profile_cfg(args):
     torch.cuda.set_device(0)
     cfg = args.profile_cfg
     w = W.config(cfg)
+    n_points = args.profile_points or w.render.n_points
     cloud = W.gaussian_mixture_cloud(w.render.n_points, w.cloud_seed) if w.system.gen == "cloud" else None
     d_cloud = cfs.cloud_to_device(cloud) if cloud is not None else None
     sysh = cfs.cfs_create(w.system)
     img = cfs.new_image(w.render)
     ctr = torch.zeros(2, dtype=torch.int64, device="cuda")
     t = w.frames[len(w.frames) // 2]
-    scratch = make_scratch(cfs, torch, sysh, w.render) if args.variant in ("auto", "binned") else None
+    need = cfs.cfs_binned_scratch_bytes(sysh, cfs.make_args(w.render))
+    if w.render.out_mode == "depth_u64":
+        need = cfs.cfs_hiz_scratch_bytes(w.render.width, w.render.height)
+    scratch = torch.empty(min(need, args.scratch_mib << 20), dtype=torch.uint8, device="cuda") if need and args.variant == "auto" else None
+    flags = (["fast_trig"] if args.fast_trig else []) + (["jit"] if args.jit else [])
     rargs = cfs.make_args(w.render, d_image=img, d_cloud=d_cloud, d_counters=ctr, t=t, variant=args.variant,
-                          flags=["fast_trig"] if args.fast_trig else 0, d_scratch=scratch)
+                          flags=flags, d_scratch=scratch, n_points=n_points)
     ms = []
     for i in range(2 + args.steps):
         img.fill_(-1 if w.render.out_mode == "depth_u64" else 0)
@@ -562,8 +709,8 @@ def run_profile_cfg(args):
         torch.cuda.synchronize()
         if i >= 2:
             ms.append(e0.elapsed_time(e1))
-    print(json.dumps({"profile_cfg": cfg, "workload": w.name, "variant": args.variant, "launch_ms": ms,
-                      "point_iterations_per_s": w.render.n_points * w.render.iterations / (min(ms) * 1e-3)}))
+    print(json.dumps({"profile_cfg": cfg, "workload": w.name, "variant": args.variant, "flags": flags, "n_points": n_points,
+                      "launch_ms": ms, "point_iterations_per_s": n_points * w.render.iterations / (min(ms) * 1e-3)}))
     sysh.close()
 
 
@@ -573,18 +720,25 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--no-workloads", action="store_true", help="skip the per-config side report")
+    ap.add_argument("--headline", type=int, default=HEADLINE_CFG, help="BASELINE config the bench line is on (default: configs[4], the largest)")
+    ap.add_argument("--configs", default="0,1,2,3,4", help="configs that get a first-class record under 'workloads'")
+    ap.add_argument("--side-steps", type=int, default=10, help="timed steps of the non-headline configs")
+    ap.add_argument("--no-workloads", action="store_true", help="only the headline config")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--profile-cfg", type=int, default=None,
                     help="only launch cfs_render of configs[N] --steps times (ncu target; no bench line)")
-    ap.add_argument("--variant", default="auto", help="splat variant: auto (tile bins for large renders, else direct), direct, binned, ...")
+    ap.add_argument("--profile-points", type=int, default=None, help="with --profile-cfg: render only the first N points")
+    ap.add_argument("--variant", default="auto", help="splat variant: auto (tile bins / Hi-Z with scratch for large renders, else direct), direct, ...")
+    ap.add_argument("--scratch-mib", type=int, default=8192, help="cap of the scratch buffer handed to AUTO (MiB); less means more chunks")
+    ap.add_argument("--no-jit", action="store_true", help="use the kernels linked ahead of time instead of the run-time compiled ones")
     ap.add_argument("--accurate-trig", action="store_true",
                     help="evaluate sin/cos with sincosf (<= 2 ulp) instead of CFS_FLAG_FAST_TRIG (MUFU); both are inside "
                          "the BASELINE tolerances (tests/test_gpu_parity.py)")
     args = ap.parse_args()
-    global SINCOS
     args.fast_trig = not args.accurate_trig
-    if args.fast_trig:
-        SINCOS = "MUFU sin.approx/cos.approx (CFS_FLAG_FAST_TRIG)"
+    args.jit = not args.no_jit
+    args.configs = [args.headline] if args.no_workloads else [int(c) for c in args.configs.split(",") if c != ""]
+    args.direct_mask = int(os.environ.get("CFS_BIN_DIRECT_MASK", "1"))
     if args.profile_cfg is not None:
         run_profile_cfg(args)
     elif args.impl == "reference":

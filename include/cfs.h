@@ -252,11 +252,36 @@ cfs_status cfs_host_resolve(const cfs_system *sys, const cfs_render_args *args, 
 cfs_status cfs_render_host(cfs_system *sys, const cfs_render_args *args, void *h_image,
                            const cfs_cloud_rec *h_cloud, uint64_t *h_counters, void *cuda_stream);
 
-/* cfs_tonemap -- log-density tone map to RGBA8 (DESIGN R10; fractal-flame convention, PAPER L31,
- * L208): n = count (HIST value / RGBA alpha), n_max = max n; n = 0 -> 0; L = log(1+n)/log(1+n_max);
+/* cfs_render_rgba8_host -- the whole path end to end with HOST buffers, to the paper's output format: as
+ * cfs_render_host, then cfs_resolve_rgba8(gamma, colour_scale, n_max) on the device image, and only the width*height
+ * RGBA8888 words travel back (h_rgba8), with the counters (optional) and this image's measured n_max (h_n_max,
+ * optional, float; untouched for DEPTH).  Synchronises the stream before returning.  Device buffers (image, cloud,
+ * scratch of at most 1 GiB, rgba8) are cached in the system handle and freed by cfs_destroy: the one exception to
+ * "the library allocates nothing" (DESIGN "what differs"), confined to the two *_host convenience entry points. */
+cfs_status cfs_render_rgba8_host(cfs_system *sys, const cfs_render_args *args, float gamma, float colour_scale,
+                                 float n_max, uint32_t *h_rgba8, const cfs_cloud_rec *h_cloud,
+                                 uint64_t *h_counters, float *h_n_max, void *cuda_stream);
+
+/* cfs_resolve_rgba8 -- the paper's output layer (an RGBA8888 image) from the accumulator in ONE kernel
+ * launch: log-density tone map (DESIGN R10; fractal-flame convention): n = count (HIST value /
+ * RGBA alpha), n_max = max n; n = 0 -> 0; L = log(1+n)/log(1+n_max);
  * v_c = clamp(colour_scale * acc_c/n * L^(1/gamma), 0, 1) (HIST: v = L^(1/gamma)); alpha = L;
- * byte = floor(255 v + 0.5).  DEPTH: out = low 32 bits, empty -> 0.
- * d_scratch: >= 8 bytes of device memory (overwritten).  Two kernels on the stream. */
+ * byte = floor(255 v + 0.5).  DEPTH: out = low 32 bits, empty -> 0 (gamma, colour_scale, n_max, d_scratch unused).
+ *   n_max > 0 : the maximum to map with is GIVEN (an animation passes the previous frame's): a single pass, every
+ *               accumulator is read once.  The pass also measures this image's own maximum.
+ *   n_max == 0: the maximum is measured first, inside the same (cooperative) launch; the second read of the image
+ *               comes from L2.
+ *   n_max < 0 : map with the maximum the PREVIOUS call on this d_scratch measured (its word 0; at least 1), with no
+ *               host round trip: frame k of an animation is mapped with frame k-1's maximum, in a single pass.
+ * d_scratch: >= 16 bytes of device memory, 4-byte aligned; afterwards word 0 holds the bits of this image's n_max as a
+ * float (0 for an empty image), words 1-3 are garbage.  d_rgba8_out: width*height uint32.  Asynchronous on the stream.
+ * Errors: INVALID_ARG (NULL pointers, sizes, gamma <= 0, non-finite values), CUDA. */
+cfs_status cfs_resolve_rgba8(const void *d_image, int32_t out_mode, int32_t width, int32_t height,
+                             float gamma, float colour_scale, float n_max, uint32_t *d_rgba8_out, void *d_scratch,
+                             void *cuda_stream);
+
+/* cfs_tonemap -- cfs_resolve_rgba8 with the maximum measured inside (n_max = 0): BASELINE north_star "cfs_tonemap
+ * does log-density tone mapping".  One memset and one kernel on the stream; d_scratch >= 8 bytes. */
 cfs_status cfs_tonemap(const void *d_image, int32_t out_mode, int32_t width, int32_t height,
                        float gamma, float colour_scale, uint32_t *d_rgba8_out, void *d_scratch,
                        void *cuda_stream);
@@ -270,18 +295,22 @@ cfs_status cfs_trace(const cfs_system *sys, const cfs_render_args *args, uint8_t
 /* cfs_microbench -- roofline denominators measured in the same run (BASELINE north_star).
  * Launches `blocks` x `threads` threads each doing `ops_per_thread` operations of `kind`;
  * the caller times the stream.  Memory kinds address `footprint_bytes` of d_buf uniformly at
- * random (hash of a per-thread counter); ALU kinds ignore d_buf except for one sink store. */
+ * random (hash of a per-thread counter); ALU kinds ignore d_buf except for one sink store (ops_per_thread is
+ * rounded down to a multiple of 256 there). */
 typedef enum {
     CFS_MB_RED_ADD_U32 = 0,     /* red.global.add.u32, random 4-byte bins                */
     CFS_MB_RED_ADD_V4F32 = 1,   /* red.global.add.v4.f32, random 16-byte pixels          */
     CFS_MB_ATOM_MIN_U64 = 2,    /* atom.global.min.u64 (result unused), random bins      */
     CFS_MB_LD_U64 = 3,          /* ld.global.cg.u64 at random bins (depth pre-test)      */
     CFS_MB_ATOMS_ADD_U32 = 4,   /* atom.shared.add.u32 over footprint_bytes of shared    */
-    CFS_MB_FFMA = 5,            /* dependent-chain FFMA x 8 independent chains           */
-    CFS_MB_IMAD_WIDE = 6,       /* 32x32->64 multiply chains (Philox core)               */
-    CFS_MB_LOP3 = 7,            /* 3-input logic chains                                  */
-    CFS_MB_MUFU = 8,            /* sin.approx chains                                     */
-    CFS_MB_STREAM_LD128 = 9     /* coalesced 128-bit loads over footprint_bytes          */
+    CFS_MB_FFMA = 5,            /* FFMA, 8 independent dependent chains, one SASS instruction per op */
+    CFS_MB_IMAD_WIDE = 6,       /* IMAD.WIDE.U32 chains (Philox core), one instruction per op        */
+    CFS_MB_LOP3 = 7,            /* LOP3.LUT chains, one instruction per op                           */
+    CFS_MB_MUFU = 8,            /* MUFU.RSQ chains (special-function unit), one instruction per op   */
+    CFS_MB_STREAM_LD128 = 9,    /* coalesced 128-bit loads over footprint_bytes                      */
+    CFS_MB_STREAM_RED_V4F32 = 10 /* the stored cloud's shape: per op one streamed 16-byte record (the first
+                                    blocks*threads*ops*16 bytes of d_buf) + one red.global.add.v4.f32 at a random
+                                    pixel of the footprint_bytes that follow them                                */
 } cfs_microbench_kind;
 cfs_status cfs_microbench(int32_t kind, void *d_buf, uint64_t footprint_bytes,
                           uint64_t ops_per_thread, int32_t blocks, int32_t threads,

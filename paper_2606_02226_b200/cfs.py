@@ -25,8 +25,8 @@ OUT = {"hist_u32": 0, "rgba_f32": 1, "depth_u64": 2}
 FLAGS = {"fast_trig": 1, "interpret_chain": 2, "bin_pass1_only": 4, "jit": 8, "bin_hybrid": 0x100}
 VARIANT = {"auto": 0, "direct": 1, "shared_hist": 2, "warp_agg": 3, "binned": 4, "cluster_hist": 5, "depth_hiz": 6}
 MB = {"red_add_u32": 0, "red_add_v4f32": 1, "atom_min_u64": 2, "ld_u64": 3, "atoms_add_u32": 4,
-      "ffma": 5, "imad_wide": 6, "lop3": 7, "mufu": 8, "stream_ld128": 9}
-EXPORTS = ["cfs_create", "cfs_destroy", "cfs_render", "cfs_render_host", "cfs_tonemap", "cfs_trace",
+      "ffma": 5, "imad_wide": 6, "lop3": 7, "mufu": 8, "stream_ld128": 9, "stream_red_v4f32": 10}
+EXPORTS = ["cfs_create", "cfs_destroy", "cfs_render", "cfs_render_host", "cfs_render_rgba8_host", "cfs_tonemap", "cfs_resolve_rgba8", "cfs_trace",
            "cfs_microbench", "cfs_host_resolve", "cfs_specialize", "cfs_jit_check", "cfs_jit_stats", "cfs_shared_hist_max_bytes", "cfs_binned_scratch_bytes", "cfs_hiz_scratch_bytes", "cfs_binned_plan", "cfs_launch_count", "cfs_last_error",
            "cfs_version"]
 
@@ -84,9 +84,15 @@ def lib():
         L.cfs_render_host.argtypes = [C.c_void_p, C.POINTER(cfs_render_args), C.c_void_p, C.c_void_p,
                                       C.c_void_p, C.c_void_p]
         L.cfs_render_host.restype = C.c_int
+        L.cfs_render_rgba8_host.argtypes = [C.c_void_p, C.POINTER(cfs_render_args), C.c_float, C.c_float, C.c_float,
+                                            C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.cfs_render_rgba8_host.restype = C.c_int
         L.cfs_tonemap.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_float, C.c_float,
                                   C.c_void_p, C.c_void_p, C.c_void_p]
         L.cfs_tonemap.restype = C.c_int
+        L.cfs_resolve_rgba8.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_float, C.c_float, C.c_float,
+                                        C.c_void_p, C.c_void_p, C.c_void_p]
+        L.cfs_resolve_rgba8.restype = C.c_int
         L.cfs_trace.argtypes = [C.c_void_p, C.POINTER(cfs_render_args), C.c_void_p, C.c_void_p, C.c_void_p,
                                 C.c_void_p, C.c_void_p]
         L.cfs_trace.restype = C.c_int
@@ -291,11 +297,25 @@ def cfs_render_host(sys: System, args: cfs_render_args, h_image: np.ndarray, h_c
                                  _stream(stream)))
 
 
+def cfs_render_rgba8_host(sys: System, args: cfs_render_args, gamma: float, colour_scale: float, n_max: float,
+                          h_rgba8: np.ndarray, h_cloud: Optional[np.ndarray] = None, h_counters: Optional[np.ndarray] = None,
+                          h_n_max: Optional[np.ndarray] = None, stream=None) -> None:
+    _check(lib().cfs_render_rgba8_host(sys.handle, C.byref(args), float(gamma), float(colour_scale), float(n_max),
+                                       _ptr(h_rgba8), _ptr(h_cloud), _ptr(h_counters), _ptr(h_n_max), _stream(stream)))
+
+
 def cfs_tonemap(d_image, out_mode, width: int, height: int, gamma: float, colour_scale: float, d_rgba8_out,
                 d_scratch, stream=None) -> None:
     mode = OUT[out_mode] if isinstance(out_mode, str) else int(out_mode)
     _check(lib().cfs_tonemap(_ptr(d_image), mode, int(width), int(height), float(gamma), float(colour_scale),
                              _ptr(d_rgba8_out), _ptr(d_scratch), _stream(stream)))
+
+
+def cfs_resolve_rgba8(d_image, out_mode, width: int, height: int, gamma: float, colour_scale: float, n_max: float,
+                      d_rgba8_out, d_scratch, stream=None) -> None:
+    mode = OUT[out_mode] if isinstance(out_mode, str) else int(out_mode)
+    _check(lib().cfs_resolve_rgba8(_ptr(d_image), mode, int(width), int(height), float(gamma), float(colour_scale),
+                                   float(n_max), _ptr(d_rgba8_out), _ptr(d_scratch), _stream(stream)))
 
 
 def cfs_trace(sys: System, args: cfs_render_args, d_picks=None, d_final_g=None, d_final_q=None, d_alive=None,
@@ -368,3 +388,16 @@ def allreduce_image(img, out_mode: str, group=None):
         dist.all_reduce(img, op=dist.ReduceOp.SUM, group=group)
     return img
 
+
+
+def render_sharded(sys: System, render, img, rank: int, world: int, group=None, **kw):
+    """The sharded render as one call (DESIGN 'multi-GPU'): rank `rank` of `world` renders its contiguous
+    range of the GLOBAL point ids into its own cleared image `img`, then the ONE exchange step combines the images
+    in place on every rank (sum, or unsigned min for DEPTH) -- over NCCL / NVLink for CUDA tensors.  Keyword arguments go
+    to make_args (t, variant, flags, d_counters, d_scratch, d_cloud ...).  Returns (point_offset, n_points) of this rank."""
+    first = int(kw.pop("point_offset", render.point_offset))
+    off, n = shard_points(int(kw.pop("n_points", render.n_points)), rank, world)
+    cfs_render(sys, make_args(render, d_image=img, n_points=n, point_offset=first + off, **kw))
+    if world > 1:
+        allreduce_image(img, render.out_mode, group=group)
+    return first + off, n

@@ -119,6 +119,8 @@ struct cfs_system {
     void *d_cloud = nullptr; size_t cloud_bytes = 0;
     unsigned long long *d_counters = nullptr;
     void *d_scratch = nullptr; size_t scratch_bytes = 0;
+    void *d_rgba8 = nullptr; size_t rgba8_bytes = 0;       // cfs_render_rgba8_host
+    void *d_tone = nullptr;                                // 16 bytes: scratch of the resolve
 };
 
 namespace {
@@ -277,6 +279,8 @@ extern "C" void cfs_destroy(cfs_system *s)
     if (s->d_cloud) cudaFree(s->d_cloud);
     if (s->d_counters) cudaFree(s->d_counters);
     if (s->d_scratch) cudaFree(s->d_scratch);
+    if (s->d_rgba8) cudaFree(s->d_rgba8);
+    if (s->d_tone) cudaFree(s->d_tone);
     delete s;
 }
 
@@ -418,7 +422,6 @@ struct Kernel {
     render_fn aot = nullptr;
     cfs::JitKernel jit;
     bool compiled_chain = false;     // the chain is compiled in (not the interpreter)
-    bool ok() const { return aot != nullptr || jit.func != nullptr; }
 };
 
 bool is_cloud_stream(const cfs_system *s, int splat)
@@ -590,6 +593,7 @@ struct BinPlan {
 };
 
 constexpr size_t kBinCtrlBytes = 256;
+constexpr uint64_t kHostScratchCap = 1ull << 30;     // scratch the host entry points allocate for the tile bins, at most (more chunks beyond)
 constexpr size_t kBinBlockBytes = cfs::kBinBlockRecords * 2;      // 16-bit records
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
@@ -1143,17 +1147,17 @@ extern "C" cfs_status cfs_trace(const cfs_system *s, const cfs_render_args *a, u
 }
 
 // -------------------------------------------------------------------------------------------------
-extern "C" cfs_status cfs_render_host(cfs_system *s, const cfs_render_args *a, void *h_image,
-                                      const cfs_cloud_rec *h_cloud, uint64_t *h_counters, void *stream)
+// common body of the host entry points: upload (CLOUD), clear, render; the image stays in s->d_image
+static cfs_status render_host_body(cfs_system *s, const cfs_render_args *a, const cfs_cloud_rec *h_cloud, void *stream, size_t *image_bytes)
 {
     if (!s || !a) return fail(CFS_ERR_INVALID_ARG, "system or args is NULL");
-    if (!h_image) return fail(CFS_ERR_INVALID_ARG, "h_image is NULL");
     if (a->width < 1 || a->height < 1 || (int64_t)a->width * a->height > 2147483647ll) return fail(CFS_ERR_INVALID_ARG, "bad image size");
     if (a->out_mode < CFS_OUT_HIST_U32 || a->out_mode > CFS_OUT_DEPTH_RGBA8_U64) return fail(CFS_ERR_INVALID_ARG, "unknown out_mode %d", a->out_mode);
     if (device_info().ok != 1) return fail(CFS_ERR_CUDA, "no CUDA device (this library has no CPU fallback)");
     cudaStream_t st = (cudaStream_t)stream;
     const size_t px = (size_t)a->width * a->height;
     const size_t bytes = px * (a->out_mode == CFS_OUT_HIST_U32 ? 4 : a->out_mode == CFS_OUT_RGBA_F32 ? 16 : 8);
+    *image_bytes = bytes;
     cudaError_t e;
     if (s->image_bytes < bytes) {
         if (s->d_image) cudaFree(s->d_image);
@@ -1178,10 +1182,11 @@ extern "C" cfs_status cfs_render_host(cfs_system *s, const cfs_render_args *a, v
         r.d_cloud = s->d_cloud;                // holds records [point_offset, point_offset + n_points)
     }
     r.d_scratch = nullptr; r.scratch_bytes = 0;
-    if (a->variant == CFS_VARIANT_AUTO || a->variant == CFS_VARIANT_BINNED) {
-        // scratch of the tile-binned variant: enough for one chunk, at most 8 GiB (more chunks beyond)
+    if (a->variant == CFS_VARIANT_AUTO || a->variant == CFS_VARIANT_BINNED || a->variant == CFS_VARIANT_DEPTH_HIZ) {
+        // scratch of the tile-binned variant (enough for one chunk, capped: more chunks beyond) or of the Hi-Z map
         uint64_t want = cfs_binned_scratch_bytes(s, &r);
-        if (want > (8ull << 30)) want = 8ull << 30;
+        if (want > kHostScratchCap) want = kHostScratchCap;
+        if (a->out_mode == CFS_OUT_DEPTH_RGBA8_U64) want = cfs_hiz_scratch_bytes(a->width, a->height);
         if (want > s->scratch_bytes) {
             if (s->d_scratch) cudaFree(s->d_scratch);
             s->d_scratch = nullptr; s->scratch_bytes = 0;
@@ -1192,16 +1197,54 @@ extern "C" cfs_status cfs_render_host(cfs_system *s, const cfs_render_args *a, v
     }
     if ((e = cudaMemsetAsync(s->d_image, a->out_mode == CFS_OUT_DEPTH_RGBA8_U64 ? 0xFF : 0, bytes, st)) != cudaSuccess) return cuda_fail(e, "clear image");
     if ((e = cudaMemsetAsync(s->d_counters, 0, 16, st)) != cudaSuccess) return cuda_fail(e, "clear counters");
-    cfs_status rs = render_impl(s, &r, stream, s->gen == CFS_GEN_CLOUD ? a->point_offset : 0);
+    return render_impl(s, &r, stream, s->gen == CFS_GEN_CLOUD ? a->point_offset : 0);
+}
+
+extern "C" cfs_status cfs_render_host(cfs_system *s, const cfs_render_args *a, void *h_image,
+                                      const cfs_cloud_rec *h_cloud, uint64_t *h_counters, void *stream)
+{
+    if (!h_image) return fail(CFS_ERR_INVALID_ARG, "h_image is NULL");
+    size_t bytes = 0;
+    cfs_status rs = render_host_body(s, a, h_cloud, stream, &bytes);
     if (rs != CFS_OK) return rs;
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaError_t e;
     if ((e = cudaMemcpyAsync(h_image, s->d_image, bytes, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(e, "D2H image");
     if (h_counters && (e = cudaMemcpyAsync(h_counters, s->d_counters, 16, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(e, "D2H counters");
     if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(e, "stream synchronize");
     return CFS_OK;
 }
 
-extern "C" cfs_status cfs_tonemap(const void *d_image, int32_t out_mode, int32_t width, int32_t height, float gamma,
-                                  float colour_scale, uint32_t *d_out, void *d_scratch, void *stream)
+extern "C" cfs_status cfs_render_rgba8_host(cfs_system *s, const cfs_render_args *a, float gamma, float colour_scale, float n_max,
+                                            uint32_t *h_rgba8, const cfs_cloud_rec *h_cloud, uint64_t *h_counters,
+                                            float *h_n_max, void *stream)
+{
+    if (!h_rgba8) return fail(CFS_ERR_INVALID_ARG, "h_rgba8 is NULL");
+    size_t bytes = 0;
+    cfs_status rs = render_host_body(s, a, h_cloud, stream, &bytes);
+    if (rs != CFS_OK) return rs;
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaError_t e;
+    const size_t out_bytes = (size_t)a->width * a->height * 4;
+    if (s->rgba8_bytes < out_bytes) {
+        if (s->d_rgba8) cudaFree(s->d_rgba8);
+        s->d_rgba8 = nullptr; s->rgba8_bytes = 0;
+        if ((e = cudaMalloc(&s->d_rgba8, out_bytes)) != cudaSuccess) return cuda_fail(e, "cudaMalloc(rgba8)");
+        s->rgba8_bytes = out_bytes;
+    }
+    if (!s->d_tone && (e = cudaMalloc(&s->d_tone, 16)) != cudaSuccess) return cuda_fail(e, "cudaMalloc(tone scratch)");
+    rs = cfs_resolve_rgba8(s->d_image, a->out_mode, a->width, a->height, gamma, colour_scale, n_max, (uint32_t *)s->d_rgba8, s->d_tone, stream);
+    if (rs != CFS_OK) return rs;
+    if ((e = cudaMemcpyAsync(h_rgba8, s->d_rgba8, out_bytes, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(e, "D2H rgba8");
+    if (h_counters && (e = cudaMemcpyAsync(h_counters, s->d_counters, 16, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(e, "D2H counters");
+    if (h_n_max && a->out_mode != CFS_OUT_DEPTH_RGBA8_U64 &&
+        (e = cudaMemcpyAsync(h_n_max, s->d_tone, 4, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(e, "D2H n_max");
+    if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(e, "stream synchronize");
+    return CFS_OK;
+}
+
+extern "C" cfs_status cfs_resolve_rgba8(const void *d_image, int32_t out_mode, int32_t width, int32_t height, float gamma,
+                                        float colour_scale, float n_max, uint32_t *d_out, void *d_scratch, void *stream)
 {
     if (!d_image || !d_out) return fail(CFS_ERR_INVALID_ARG, "image or output is NULL");
     if (width < 1 || height < 1 || (int64_t)width * height > 2147483647ll) return fail(CFS_ERR_INVALID_ARG, "bad image size");
@@ -1209,33 +1252,54 @@ extern "C" cfs_status cfs_tonemap(const void *d_image, int32_t out_mode, int32_t
     const DeviceInfo &di = device_info();
     if (di.ok != 1) return fail(CFS_ERR_CUDA, "no CUDA device (this library has no CPU fallback)");
     cudaStream_t st = (cudaStream_t)stream;
-    const size_t n = (size_t)width * height;
+    size_t n = (size_t)width * height;
     const int threads = cfs::kToneThreads;
-    size_t want = (n + threads - 1) / threads;
-    const unsigned grid_map = (unsigned)(want < (size_t)di.sms * 32 ? want : (size_t)di.sms * 32);
+    const size_t want = (n + threads - 1) / threads;
     if (out_mode == CFS_OUT_DEPTH_RGBA8_U64) {
-        cfs::tone_depth_kernel<<<grid_map, threads, 0, st>>>((const unsigned long long *)d_image, n, d_out);
+        const unsigned grid = (unsigned)(want < (size_t)di.sms * 32 ? want : (size_t)di.sms * 32);
+        cfs::tone_depth_kernel<<<grid, threads, 0, st>>>((const unsigned long long *)d_image, n, d_out);
         ++g_launches;
-    } else {
-        if (!(gamma > 0.0f) || bad_float(gamma) || bad_float(colour_scale)) return fail(CFS_ERR_INVALID_ARG, "gamma must be > 0 and finite");
-        if (!d_scratch) return fail(CFS_ERR_INVALID_ARG, "d_scratch is NULL");
-        if (out_mode == CFS_OUT_HIST_U32 && ((uintptr_t)d_image & 15)) return fail(CFS_ERR_INVALID_ARG, "HIST image must be 16-byte aligned for the tone map");
-        cudaError_t e = cudaMemsetAsync(d_scratch, 0, 8, st);
-        if (e != cudaSuccess) return cuda_fail(e, "clear scratch");
-        const unsigned grid_max = (unsigned)(want < (size_t)di.sms * 8 ? want : (size_t)di.sms * 8);
-        const float inv_gamma = 1.0f / gamma;
-        if (out_mode == CFS_OUT_HIST_U32) {
-            cfs::tone_max_kernel<0><<<grid_max, threads, 0, st>>>(d_image, n, (uint32_t *)d_scratch);
-            cfs::tone_map_kernel<0><<<grid_map, threads, 0, st>>>(d_image, n, (const uint32_t *)d_scratch, inv_gamma, colour_scale, d_out);
-        } else {
-            cfs::tone_max_kernel<1><<<grid_max, threads, 0, st>>>(d_image, n, (uint32_t *)d_scratch);
-            cfs::tone_map_kernel<1><<<grid_map, threads, 0, st>>>(d_image, n, (const uint32_t *)d_scratch, inv_gamma, colour_scale, d_out);
-        }
-        g_launches += 2;
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return cuda_fail(e, "resolve kernel launch");
+        return CFS_OK;
     }
-    cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) return cuda_fail(e, "tonemap kernel launch");
+    if (!(gamma > 0.0f) || bad_float(gamma) || bad_float(colour_scale)) return fail(CFS_ERR_INVALID_ARG, "gamma must be > 0 and finite");
+    if (std::isnan(n_max) || std::isinf(n_max)) return fail(CFS_ERR_INVALID_ARG, "n_max is not finite");
+    if (!d_scratch) return fail(CFS_ERR_INVALID_ARG, "d_scratch is NULL");
+    cudaError_t e;
+    // [0] n_max bits (output), [1] barrier arrivals, [2] the previous call's n_max when n_max < 0 asks for it
+    if (n_max < 0.0f && (e = cudaMemcpyAsync((char *)d_scratch + 8, d_scratch, 4, cudaMemcpyDeviceToDevice, st)) != cudaSuccess) return cuda_fail(e, "park previous n_max");
+    if ((e = cudaMemsetAsync(d_scratch, 0, 8, st)) != cudaSuccess) return cuda_fail(e, "clear scratch");
+    float inv_gamma = 1.0f / gamma;
+    uint32_t *scratch = (uint32_t *)d_scratch;
+    const bool hist = out_mode == CFS_OUT_HIST_U32;
+    if (n_max != 0.0f) {         // single pass with the given maximum (> 0) or the previous call's (< 0)
+        const unsigned grid = (unsigned)(want < (size_t)di.sms * 16 ? want : (size_t)di.sms * 16);
+        if (hist) cfs::resolve_kernel<0, true><<<grid, threads, 0, st>>>(d_image, n, scratch, n_max, inv_gamma, colour_scale, d_out);
+        else      cfs::resolve_kernel<1, true><<<grid, threads, 0, st>>>(d_image, n, scratch, n_max, inv_gamma, colour_scale, d_out);
+        ++g_launches;
+        if ((e = cudaGetLastError()) != cudaSuccess) return cuda_fail(e, "resolve kernel launch");
+        return CFS_OK;
+    }
+    // maximum + map in one cooperative launch: as many CTAs as are resident at once
+    const void *fn = hist ? (const void *)cfs::resolve_kernel<0, false> : (const void *)cfs::resolve_kernel<1, false>;
+    int per_sm = 0;
+    if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, threads, 0)) != cudaSuccess || per_sm < 1) return cuda_fail(e, "resolve occupancy");
+    if (per_sm > 8) per_sm = 8;
+    size_t grid = (size_t)di.sms * per_sm;
+    if (grid > want) grid = want;
+    float zero = 0.0f;
+    void *args[] = {(void *)&d_image, (void *)&n, (void *)&scratch, (void *)&zero, (void *)&inv_gamma, (void *)&colour_scale, (void *)&d_out};
+    if ((e = cudaLaunchCooperativeKernel(fn, dim3((unsigned)grid), dim3(threads), args, 0, st)) != cudaSuccess) return cuda_fail(e, "resolve kernel launch");
+    ++g_launches;
     return CFS_OK;
+}
+
+extern "C" cfs_status cfs_tonemap(const void *d_image, int32_t out_mode, int32_t width, int32_t height, float gamma,
+                                  float colour_scale, uint32_t *d_out, void *d_scratch, void *stream)
+{
+    if (out_mode == CFS_OUT_HIST_U32 && ((uintptr_t)d_image & 15)) return fail(CFS_ERR_INVALID_ARG, "HIST image must be 16-byte aligned for the tone map");
+    return cfs_resolve_rgba8(d_image, out_mode, width, height, gamma, colour_scale, 0.0f, d_out, d_scratch, stream);
 }
 
 extern "C" cfs_status cfs_microbench(int32_t kind, void *d_buf, uint64_t footprint, uint64_t ops, int32_t blocks,
@@ -1263,6 +1327,7 @@ extern "C" cfs_status cfs_microbench(int32_t kind, void *d_buf, uint64_t footpri
     case CFS_MB_LOP3:      cfs::mb_alu_kernel<7><<<blocks, threads, 0, st>>>(d_buf, ops); break;
     case CFS_MB_MUFU:      cfs::mb_alu_kernel<8><<<blocks, threads, 0, st>>>(d_buf, ops); break;
     case CFS_MB_STREAM_LD128: cfs::mb_stream_kernel<<<blocks, threads, 0, st>>>(d_buf, footprint / 16); break;
+    case CFS_MB_STREAM_RED_V4F32: if (!bins(16)) return fail(CFS_ERR_INVALID_ARG, "footprint too small"); cfs::mb_stream_red_kernel<<<blocks, threads, 0, st>>>(d_buf, bins(16), ops); break;
     default: return fail(CFS_ERR_INVALID_ARG, "unknown microbench kind %d", kind);
     }
     ++g_launches;

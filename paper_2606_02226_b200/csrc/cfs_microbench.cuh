@@ -63,33 +63,57 @@ __global__ void mb_atoms_kernel(void *buf, uint32_t n_bins, uint64_t ops)
     if (threadIdx.x == 0 && sh[0] == 0xFFFFFFFFu) reinterpret_cast<uint32_t *>(buf)[0] = 1;
 }
 
-// ALU kinds: 8 independent dependent-chains per thread, 8 ops per loop trip per chain
+// ALU kinds: 8 independent dependent chains per thread, 32 operations per chain and loop trip, each operation ONE SASS
+// instruction (inline PTX: FFMA, IMAD.WIDE.U32, LOP3.LUT, MUFU.RSQ), a 32-bit trip counter: the loop control is 3
+// instructions per 256 timed ones (round 1 timed IMAD.WIDE + LOP3 and FMUL + MUFU pairs with a 64-bit counter inside).
 template <int KIND>
 __global__ void mb_alu_kernel(void *buf, uint64_t ops)
 {
     const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x;
     float f[8];
     uint32_t u[8];
+    unsigned long long w[8];
 #pragma unroll
-    for (int j = 0; j < 8; ++j) { f[j] = 1.0f + 1e-3f * (float)(tid + j); u[j] = tid * 8u + j + 1u; }
+    for (int j = 0; j < 8; ++j) {
+        f[j] = 1.0f + 1e-3f * (float)((tid + j) & 1023u);
+        u[j] = tid * 8u + j + 1u;
+        w[j] = ((unsigned long long)tid << 32) | (uint32_t)(j * 2 + 1);
+    }
     const float a = 0.999f, b = 1e-4f;
-    const uint64_t trips = ops / 64;
-    for (uint64_t i = 0; i < trips; ++i) {
+    const uint32_t trips = (uint32_t)(ops / 256);
+    for (uint32_t i = 0; i < trips; ++i) {
 #pragma unroll
-        for (int rep = 0; rep < 8; ++rep) {
+        for (int rep = 0; rep < 32; ++rep) {
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
-                if (KIND == 5) f[j] = __fmaf_rn(f[j], a, b);
-                else if (KIND == 6) { const uint64_t p = (uint64_t)u[j] * 0xD2511F53u; u[j] = (uint32_t)(p >> 32) ^ (uint32_t)p; }
-                else if (KIND == 7) u[j] = (u[j] ^ u[(j + 1) & 7]) ^ (uint32_t)i;
-                else if (KIND == 8) f[j] = __sinf(f[j]);
+                if (KIND == 5) asm volatile("fma.rn.f32 %0, %0, %1, %2;" : "+f"(f[j]) : "f"(a), "f"(b));
+                else if (KIND == 6) asm volatile("mad.wide.u32 %0, %1, %2, %0;" : "+l"(w[j]) : "r"((uint32_t)w[j]), "r"(0xD2511F53u));
+                else if (KIND == 7) asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(u[j]) : "r"(u[(j + 1) & 7]), "r"(0x9E3779B9u));
+                else if (KIND == 8) asm volatile("rsqrt.approx.ftz.f32 %0, %0;" : "+f"(f[j]));
             }
         }
     }
     float fs = 0.f; uint32_t us = 0;
 #pragma unroll
-    for (int j = 0; j < 8; ++j) { fs += f[j]; us ^= u[j]; }
+    for (int j = 0; j < 8; ++j) { fs += f[j]; us ^= u[j] ^ (uint32_t)w[j] ^ (uint32_t)(w[j] >> 32); }
     if (fs == 123.456f || us == 0x12345u) reinterpret_cast<uint32_t *>(buf)[0] = us + (uint32_t)fs;
+}
+
+// the cloud's shape (BASELINE configs[3]): every operation is one streamed 16-byte record (ld.global.cs.v4 from the
+// first blocks*threads*ops*16 bytes of buf) and one red.global.add.v4.f32 at a uniformly random pixel of the
+// `n_bins` 16-byte pixels that follow -- the rate at which the L2 serves a record stream and one reduction per
+// record over a hot set of that size AT THE SAME TIME, which is what bounds a stored-cloud render (DESIGN "rooflines")
+__global__ void mb_stream_red_kernel(void *buf, uint32_t n_bins, uint64_t ops)
+{
+    const uint64_t n_threads = (uint64_t)gridDim.x * blockDim.x, tid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const float4 *src = reinterpret_cast<const float4 *>(buf);
+    float *img = reinterpret_cast<float *>(buf) + 4 * n_threads * ops;
+    for (uint64_t i = 0; i < ops; ++i) {
+        const float4 r = __ldcs(src + i * n_threads + tid);
+        const uint32_t b = mb_bin(mb_hash(__float_as_uint(r.x) ^ (uint32_t)(i * n_threads + tid)), n_bins);
+        asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};"
+                     :: "l"(img + 4 * (size_t)b), "f"(r.y), "f"(r.z), "f"(r.w), "f"(1.0f) : "memory");
+    }
 }
 
 __global__ void mb_stream_kernel(void *buf, uint64_t n_vec)

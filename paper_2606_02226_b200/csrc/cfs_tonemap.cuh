@@ -1,6 +1,7 @@
-// cfs_tonemap.cuh -- log-density tone map (DESIGN R10).  HBM-bound: reads the
-// image twice (max pass + map pass; the second read hits L2 for images below 126 MB) and writes
-// W*H*4 bytes.  Not in the paper; fractal-flame convention.
+// cfs_tonemap.cuh -- log-density tone map / resolve to RGBA8888 (DESIGN R10) in one
+// launch.  HBM/L2-bound: reads the accumulator once (n_max given) or twice (second read from L2) and writes
+// W*H*4 bytes.  The tone curve is not in the paper; fractal-flame convention; the RGBA8888 output is
+// the paper's (L202).
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -17,27 +18,42 @@ __device__ __forceinline__ float tone_count(const void *img, size_t i)
     return __ldg(reinterpret_cast<const float *>(img) + 4 * i + 3);
 }
 
-// pass 1: n_max.  Non-negative floats order like their bit patterns -> one atomicMax(u32) per CTA.
-template <int MODE>
-__global__ void __launch_bounds__(kToneThreads) tone_max_kernel(const void *img, size_t n, uint32_t *scratch)
+__device__ __forceinline__ uint32_t tone_byte(float v)
 {
-    float m = 0.0f;
-    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    v = fminf(fmaxf(v, 0.0f), 1.0f);   // NaN -> 0 (fmaxf returns the non-NaN operand)
+    return (uint32_t)__float2int_rd(__fmaf_rn(255.0f, v, 0.5f));
+}
+
+// ---------------------------------------------------------------------------------------------
+// Fused resolve: accumulator -> RGBA8888, the paper's output layer, in ONE launch.
+//   KNOWN = true : n_max is given (an animation reuses the previous frame's; PAPER L9, L206 in-betweens) -- a single
+//                  pass: every pixel is read once, mapped and written; the pass also measures THIS image's n_max
+//                  and leaves it in scratch[0] for the next frame.
+//   KNOWN = false: cooperative launch (all CTAs resident): each CTA reduces the maximum over its grid-stride slice,
+//                  one atomicMax per CTA, a grid-wide barrier, then the same slice is mapped -- its second read comes
+//                  from L2 (every BASELINE image but the 133 MB one of configs[3] fits the 126 MB L2).
+// Non-negative floats order like their bit patterns, so the maximum is one atomicMax(u32) per CTA.
+template <int MODE>
+__device__ __forceinline__ uint32_t tone_pixel(const void *img, size_t i, float inv_lmax, float inv_gamma, float colour_scale, float &count)
+{
     if (MODE == 0) {
-        // 128-bit loads over the u32 histogram
-        const uint4 *v = reinterpret_cast<const uint4 *>(img);
-        const size_t n4 = n / 4;
-        for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += stride) {
-            const uint4 q = __ldg(v + i);
-            m = fmaxf(m, (float)max(max(q.x, q.y), max(q.z, q.w)));
-        }
-        for (size_t i = n4 * 4 + (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride)
-            m = fmaxf(m, tone_count<0>(img, i));
-    } else {
-        const float4 *v = reinterpret_cast<const float4 *>(img);
-        for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride)
-            m = fmaxf(m, __ldg(v + i).w);
+        const float c = tone_count<0>(img, i);
+        count = c;
+        if (!(c > 0.0f)) return 0u;
+        const float L = log1pf(c) * inv_lmax;
+        const uint32_t g = tone_byte(powf(L, inv_gamma));
+        return g | (g << 8) | (g << 16) | (tone_byte(L) << 24);
     }
+    const float4 a = __ldg(reinterpret_cast<const float4 *>(img) + i);
+    count = a.w;
+    if (!(a.w > 0.0f)) return 0u;
+    const float L = log1pf(a.w) * inv_lmax;
+    const float sc = colour_scale * powf(L, inv_gamma) / a.w;
+    return tone_byte(a.x * sc) | (tone_byte(a.y * sc) << 8) | (tone_byte(a.z * sc) << 16) | (tone_byte(L) << 24);
+}
+
+__device__ __forceinline__ void tone_block_max(float m, uint32_t *scratch)
+{
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xFFFFFFFFu, m, o));
     __shared__ float sm[kToneThreads / 32];
@@ -49,41 +65,48 @@ __global__ void __launch_bounds__(kToneThreads) tone_max_kernel(const void *img,
     }
 }
 
-__device__ __forceinline__ uint32_t tone_byte(float v)
+// grid-wide barrier of a cooperative launch: one arrival per CTA on a counter in global memory (scratch[1], zeroed by
+// the host before the launch), everyone spins until all have arrived.  All CTAs are resident by construction
+// (cudaLaunchCooperativeKernel refuses the launch otherwise).
+__device__ __forceinline__ void tone_grid_barrier(uint32_t *counter)
 {
-    v = fminf(fmaxf(v, 0.0f), 1.0f);   // NaN -> 0 (fmaxf returns the non-NaN operand)
-    return (uint32_t)__float2int_rd(__fmaf_rn(255.0f, v, 0.5f));
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        atomicAdd(counter, 1u);
+        while (*reinterpret_cast<volatile uint32_t *>(counter) < gridDim.x) { }
+        __threadfence();
+    }
+    __syncthreads();
 }
 
-// pass 2: one pixel per thread.
-template <int MODE>
+template <int MODE, bool KNOWN>
 __global__ void __launch_bounds__(kToneThreads)
-tone_map_kernel(const void *img, size_t n, const uint32_t *scratch, float inv_gamma, float colour_scale,
-                uint32_t *out)
+resolve_kernel(const void *img, size_t n, uint32_t *scratch, float n_max_given, float inv_gamma, float colour_scale, uint32_t *out)
 {
-    const float nmax = __uint_as_float(__ldg(scratch));
-    const float inv_lmax = 1.0f / log1pf(nmax);
-    const size_t stride = (size_t)gridDim.x * blockDim.x;
-    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
-        if (MODE == 0) {
-            const float c = tone_count<0>(img, i);
-            uint32_t o = 0;
-            if (c > 0.0f) {
-                const float L = log1pf(c) * inv_lmax;
-                const uint32_t g = tone_byte(powf(L, inv_gamma));
-                o = g | (g << 8) | (g << 16) | (tone_byte(L) << 24);
-            }
-            out[i] = o;
-        } else {
-            const float4 a = __ldg(reinterpret_cast<const float4 *>(img) + i);
-            uint32_t o = 0;
-            if (a.w > 0.0f) {
-                const float L = log1pf(a.w) * inv_lmax;
-                const float sc = colour_scale * powf(L, inv_gamma) / a.w;
-                o = tone_byte(a.x * sc) | (tone_byte(a.y * sc) << 8) | (tone_byte(a.z * sc) << 16) |
-                    (tone_byte(L) << 24);
-            }
-            out[i] = o;
+    const size_t stride = (size_t)gridDim.x * blockDim.x, first = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    float m = 0.0f;
+    if constexpr (KNOWN) {
+        // n_max_given < 0: the maximum the previous resolve on this scratch measured, parked in word 2 by the host side
+        // of this call (no host round trip between the frames of an animation)
+        float n_max = n_max_given;
+        if (n_max < 0.0f) n_max = fmaxf(__uint_as_float(__ldcg(scratch + 2)), 1.0f);
+        const float inv_lmax = 1.0f / log1pf(n_max);
+        for (size_t i = first; i < n; i += stride) {
+            float c;
+            out[i] = tone_pixel<MODE>(img, i, inv_lmax, inv_gamma, colour_scale, c);
+            m = fmaxf(m, c);
+        }
+        tone_block_max(m, scratch);
+    } else {
+        for (size_t i = first; i < n; i += stride) m = fmaxf(m, tone_count<MODE>(img, i));
+        tone_block_max(m, scratch);
+        tone_grid_barrier(scratch + 1);
+        const float nmax = __uint_as_float(*reinterpret_cast<volatile uint32_t *>(scratch));
+        const float inv_lmax = 1.0f / log1pf(nmax);
+        for (size_t i = first; i < n; i += stride) {
+            float c;
+            out[i] = tone_pixel<MODE>(img, i, inv_lmax, inv_gamma, colour_scale, c);
         }
     }
 }

@@ -722,6 +722,50 @@ def test_tonemap_matches_oracle(cfs, oracle, cfg):
     sysh.close()
 
 
+@pytest.mark.parametrize("cfg", [0, 1, 2])
+def test_resolve_rgba8_single_pass_with_a_given_maximum(cfs, oracle, cfg):
+    """NEXT-3 (the output layer is an RGBA8888 image): cfs_resolve_rgba8 with n_max GIVEN reads every
+    accumulator once; with the image's true maximum it writes exactly what cfs_tonemap (maximum measured inside the
+    same launch) writes, and it leaves this image's maximum in the scratch word for the next frame.  One kernel
+    launch either way.  A different maximum changes the curve as the closed form says (alpha = log1p n / log1p n_max)."""
+    import torch
+    w = W.config(cfg).scaled(n_points=1 << 13, iterations=200)
+    t = w.frames[len(w.frames) // 2]
+    sysh = cfs.cfs_create(w.system)
+    img = cfs.new_image(w.render)
+    cfs.cfs_render(sysh, cfs.make_args(w.render, d_image=img, t=t))
+    npx = w.render.width * w.render.height
+    out_a = torch.zeros(npx, dtype=torch.int32, device="cuda")
+    out_b = torch.zeros(npx, dtype=torch.int32, device="cuda")
+    out_c = torch.zeros(npx, dtype=torch.int32, device="cuda")
+    scr = torch.zeros(2, dtype=torch.int32, device="cuda")
+    cfs.cfs_launch_count(reset=True)
+    cfs.cfs_tonemap(img, w.render.out_mode, w.render.width, w.render.height, 2.2, 1 / 255.0, out_a, scr)
+    torch.cuda.synchronize()
+    assert cfs.cfs_launch_count() == 1
+    host = cfs.image_to_numpy(img, w.render.out_mode)
+    counts = host.astype(np.float32) if w.render.out_mode == "hist_u32" else host[:, 3]
+    n_max = float(counts.max())
+    assert scr.cpu().numpy().view(np.float32)[0] == np.float32(n_max)
+    cfs.cfs_launch_count(reset=True)
+    cfs.cfs_resolve_rgba8(img, w.render.out_mode, w.render.width, w.render.height, 2.2, 1 / 255.0, n_max, out_b, scr)
+    torch.cuda.synchronize()
+    assert cfs.cfs_launch_count() == 1 and torch.equal(out_a, out_b)
+    assert scr.cpu().numpy().view(np.float32)[0] == np.float32(n_max)            # measured on the fly for the next frame
+    want = oracle.tonemap(host, w.render.out_mode, w.render.width, w.render.height, 2.2, 1 / 255.0)
+    got = out_b.cpu().numpy().view(np.uint32)
+    for sh in (0, 8, 16, 24):
+        assert np.abs(((got >> sh) & 0xFF).astype(np.int32) - ((want >> sh) & 0xFF).astype(np.int32)).max() <= 1
+    # twice the maximum: alpha byte = floor(255 log1p(n) / log1p(2 n_max) + 0.5), +-1 code (float32 log1p against numpy's double)
+    cfs.cfs_resolve_rgba8(img, w.render.out_mode, w.render.width, w.render.height, 2.2, 1 / 255.0, 2.0 * n_max, out_c, scr)
+    torch.cuda.synchronize()
+    alpha = (out_c.cpu().numpy().view(np.uint32) >> 24).astype(np.int32)
+    hit = counts > 0
+    exp = np.floor(255.0 * np.log1p(counts[hit].astype(np.float64)) / math.log1p(2.0 * n_max) + 0.5).astype(np.int32)
+    assert np.abs(alpha[hit] - exp).max() <= 1 and np.all(alpha[~hit] == 0)
+    sysh.close()
+
+
 @pytest.mark.parametrize("cfg", [0, 3, 4])
 def test_render_host_entry_point(cfs, oracle, cfg):
     """cfs_render_host: HOST buffers in and out (the end-to-end call bench.py times)."""
