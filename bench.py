@@ -566,6 +566,46 @@ def measure_config(cfs, torch, cfg, args, rank, world, flush, rates, peaks, peak
     return rec
 
 
+def fig4_like_record(cfs, torch, args, flush):
+    """NEXT-4 beside the paper's own experiment (0.745 s for one image including run-time compilation
+    against 0.0215 s per frame on an AMD 6700 XT): a scene with Fig. 4's structure (one circle primitive, four
+    branches, PRNG-placed stars; workloads.fig4_like) rendered by the chain interpreter and by the kernel NVRTC
+    compiles for it, with the compile time."""
+    w = W.fig4_like()
+    r = w.render
+    sysh = cfs.cfs_create(w.system)
+    img = cfs.new_image(r)
+    ctr = torch.zeros(2, dtype=torch.int64, device="cuda")
+    base = ["fast_trig"] if args.fast_trig else []
+    out = {"workload": w.name, "points": r.n_points, "iterations": r.iterations, "branches": 4,
+           "image": f"{r.width}x{r.height} {r.out_mode}", "paper": "PAPER L200: 0.745 s wall for one image incl. run-time "
+           "compilation, 0.0215 s per frame, AMD 6700 XT, OpenCL; point and iteration counts not stated (context, not a comparison)"}
+    compile_ms = None
+    for name, flags in (("interpreter", base + ["interpret_chain"]), ("jit", base + ["jit"])):
+        if name == "jit":
+            if not args.jit:
+                continue
+            compile_ms = cfs.cfs_specialize(sysh, cfs.make_args(r, flags=flags, variant="direct"))
+        ts = []
+        for i in range(5):
+            flush.zero_()
+            img.zero_()
+            ctr.zero_()
+            e0, e1 = event_pair(torch)
+            e0.record()
+            cfs.cfs_render(sysh, cfs.make_args(r, d_image=img, d_counters=ctr, flags=flags, variant="direct"))
+            e1.record()
+            torch.cuda.synchronize()
+            if i >= 2:
+                ts.append(e0.elapsed_time(e1))
+        ms = float(np.median(ts))
+        out[name] = {"ms_per_frame": ms, "point_iterations_per_s": r.n_points * r.iterations / (ms * 1e-3),
+                     "splats_per_s": int(ctr[0].item()) / (ms * 1e-3)}
+    out["jit_compile_ms"] = compile_ms
+    sysh.close()
+    return out
+
+
 def respawn_under_torchrun(args):
     """`python bench.py --gpus N` without a launcher: start the N ranks ourselves (one process per GPU, NCCL)."""
     import socket
@@ -663,6 +703,8 @@ def run_ours(args):
     }
     if getattr(args, "jit_unavailable", None):
         line["jit_unavailable"] = args.jit_unavailable
+    if world == 1 and not args.no_workloads:
+        line["fig4_like"] = fig4_like_record(cfs, torch, args, flush)
     if world > 1:
         line["nccl"] = nccl_summary()
     if world == 1 and not args.no_cpu_baseline:
@@ -738,7 +780,7 @@ def main():
     args.fast_trig = not args.accurate_trig
     args.jit = not args.no_jit
     args.configs = [args.headline] if args.no_workloads else [int(c) for c in args.configs.split(",") if c != ""]
-    args.direct_mask = int(os.environ.get("CFS_BIN_DIRECT_MASK", "1"))
+    args.direct_mask = 1          # the hybrid stage sends iteration 0 of every Philox block of four straight to L2 (csrc/cfs_api.cu hybrid_mask)
     if args.profile_cfg is not None:
         run_profile_cfg(args)
     elif args.impl == "reference":

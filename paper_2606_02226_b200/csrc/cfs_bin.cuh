@@ -112,6 +112,7 @@ __device__ __forceinline__ void bin_append(const RenderParams &prm, const Shared
 {
     uint32_t tile, rec;
     bin_record_of(br, pix, k, tile, rec);
+    CFS_CHECK(tile < prm.bin.n_tiles && rec < prm.bin.tile_pixels * prm.bin.nk);
     const uint32_t row = br.buf_addr + tile * br.row_bytes;
     uint32_t slot;
     asm volatile("atom.shared.add.u32 %0, [%1], 1;" : "=r"(slot) : "r"(br.cnt_addr + 4u * tile) : "memory");
@@ -126,6 +127,7 @@ __device__ __forceinline__ void bin_append(const RenderParams &prm, const Shared
 __device__ __forceinline__ bool bin_try_append(const BinRegs &br, bool ok, uint32_t tile, uint32_t rec)
 {
     const uint32_t t_eff = ok ? tile : br.dummy;
+    CFS_CHECK(tile <= br.dummy - (threadIdx.x & 31u) - 1u && rec <= 49152u && rec < (br.ktp ? 65536u : br.tp));
     uint32_t slot;
     asm volatile("atom.shared.add.u32 %0, [%1], 1;" : "=r"(slot) : "r"(br.cnt_addr + 4u * t_eff) : "memory");
     const bool fits = slot < br.cap;
@@ -237,6 +239,77 @@ __device__ __forceinline__ void bin_flush(const RenderParams &prm, const SharedT
     }
 }
 
+// The flush of the steady state, written for instruction count (the general bin_flush above costs ~340 warp-
+// instructions per call, ~10 per iteration at a 32-iteration interval: profiles/r02): every row holding >= 256
+// records loses its WHOLE 256-record units, one 512-byte coalesced store each (LDS.128 -> STG.128 through 32-bit
+// shared-window addresses), and the remainder (< 256 records, it sits >= 512 bytes up the row, so the move cannot
+// overlap itself) goes back to the row start.  A tile whose pool or list ran out hands the warp to the general flush.
+__device__ __forceinline__ uint4 bin_lds_u4(uint32_t a)
+{
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ void bin_sts_u4(uint32_t a, const uint4 &v)
+{
+    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" :: "r"(a), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+
+__device__ __forceinline__ void bin_flush_units(const RenderParams &prm, const SharedTables &s, uint32_t *sm, const BinRegs &br, BinLane &bl)
+{
+    const BinParams &b = prm.bin;
+    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+    if (warp >= b.n_tiles) return;                     // warp owns no tile (warp-uniform)
+    const uint32_t my_tile = lane * nwarps + warp;
+    const bool valid = my_tile < b.n_tiles;
+    if (__any_sync(0xFFFFFFFFu, valid && bl.pos == kBinInvalid)) { bin_flush(prm, s, sm, bl, false); return; }
+    uint32_t mine = 0u;
+    if (valid) asm volatile("ld.shared.u32 %0, [%1];" : "=r"(mine) : "r"(br.cnt_addr + 4u * my_tile));
+    mine = min(mine, br.cap);                          // slots >= cap went direct
+    unsigned todo = __ballot_sync(0xFFFFFFFFu, mine >= kBinFlushRecords);
+    if (todo == 0u) return;
+    const size_t list_base = ((size_t)my_tile * b.grid + blockIdx.x) * b.lcap;
+    char *pool_lane = reinterpret_cast<char *>(b.pool) + 16u * lane;
+    do {
+        const int src = __ffs(todo) - 1;
+        todo &= todo - 1;
+        const uint32_t cnt = __shfl_sync(0xFFFFFFFFu, mine, src);
+        const uint32_t units = cnt / kBinFlushRecords;
+        uint32_t row = br.buf_addr + ((uint32_t)src * nwarps + warp) * br.row_bytes + 16u * lane;
+        for (uint32_t u = 0; u < units; ++u, row += 2u * kBinFlushRecords) {
+            if ((int)lane == src && (bl.pos & (kBinBlockRecords - 1u)) == 0u) {
+                // block full (or none yet): open the prefetched one, list it, prefetch another
+                if (bl.next < b.nb && bl.nblk < b.lcap) {
+                    b.list[list_base + bl.nblk] = bl.next;
+                    bl.pos = bl.next * kBinBlockRecords;
+                    ++bl.nblk;
+                    bl.next = atomicAdd(&b.ctrl[0], 1u) + 1u;
+                } else {
+                    bl.pos = kBinInvalid;              // pool or list exhausted: direct from now on
+                }
+            }
+            const uint32_t pos = __shfl_sync(0xFFFFFFFFu, bl.pos, src);
+            const uint4 v = bin_lds_u4(row);
+            CFS_CHECK(pos == kBinInvalid || (pos >= kBinBlockRecords && pos + kBinFlushRecords <= (b.nb + 1u) * kBinBlockRecords));
+            CFS_CHECK(row + 16u <= br.buf_addr + b.n_tiles * br.row_bytes);
+            if (pos != kBinInvalid) {
+                *reinterpret_cast<uint4 *>(pool_lane + 2u * (size_t)pos) = v;
+                if ((int)lane == src) bl.pos += kBinFlushRecords;
+            } else {                                     // rare: this unit goes down the direct path
+                const uint32_t r[4] = {v.x, v.y, v.z, v.w};
+                const uint32_t tile = (uint32_t)src * nwarps + warp;
+#pragma unroll
+                for (int i = 0; i < 8; ++i) bin_direct(prm, s, tile, (r[i >> 1] >> (16 * (i & 1))) & 0xFFFFu);
+                if (lane == 0) atomicAdd(&b.ctrl[1], kBinFlushRecords);
+            }
+        }
+        const uint32_t rest = cnt % kBinFlushRecords;
+        if (8u * lane < rest) bin_sts_u4(row - units * 2u * kBinFlushRecords, bin_lds_u4(row));    // reads >= 512 B up, writes < 512 B: disjoint
+        if ((int)lane == src) mine = rest;
+    } while (todo);
+    if (valid) asm volatile("st.shared.u32 [%0], %1;" :: "r"(br.cnt_addr + 4u * my_tile), "r"(mine) : "memory");
+}
+
 // ---------------------------------------------------------------------------------------------
 // pass 2.  MODE 0: HIST_U32 (nk = 1).  MODE 1: RGBA_F32 + MAP_INDEX: counters per (colour index, pixel), laid
 // out [k][pixel] -- the colour of a splat follows its position (the last map decides the region), so a tile is
@@ -253,6 +326,7 @@ __device__ __forceinline__ void bin_count8(uint32_t acc_addr, const uint4 &v)
     const uint32_t w[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
+        CFS_CHECK((w[i] & 0xFFFFu) <= 49152u && (w[i] >> 16) <= 49152u);
         asm volatile("red.shared.add.u32 [%0], 1;" :: "r"(acc_addr + ((w[i] & 0xFFFFu) << 2)) : "memory");
         asm volatile("red.shared.add.u32 [%0], 1;" :: "r"(acc_addr + ((w[i] >> 16) << 2)) : "memory");
     }

@@ -100,6 +100,7 @@ cloud_kernel(const __grid_constant__ RenderParams prm)
     for (uint64_t c = blockIdx.x; c < n_chunks; c += gridDim.x) {
         mbar_wait(bar0 + 8u * stage, parity);
         const uint32_t n_rec = chunk_bytes(c) >> 4;
+        CFS_CHECK(stage < (uint32_t)kCloudStages && n_rec >= 1u && n_rec <= kCloudChunk);
         const uint32_t base = ring + stage * kCloudChunk * 16u;
         const uint64_t p0 = prm.point_offset + c * kCloudChunk;
         constexpr int kPer = kCloudChunk / kCloudThreads;      // independent records per thread: the ILP of the chain

@@ -117,7 +117,7 @@ constexpr int kBinAccThreads = 1024;           // CTA size of pass 2 (one CTA pe
 // Hi-Z pre-test of the depth splat (DESIGN "Hi-Z variant").  hz[by * nbx + bx] is an upper bound of
 // (depth bits >> 16) over the 2^shift x 2^shift pixel block (bx, by), taken from a snapshot of the
 // depth image; the image only decreases, so the bound stays valid for the rest of the render.
-constexpr int kHizThreads = 768;               // CTA size of the Hi-Z render kernel, two CTAs per SM
+constexpr int kHizThreads = 768;               // CTA size of the Hi-Z render kernel, two CTAs per SM (1024 x 1 measured 197 against 172 ms)
 constexpr int kHizCtasPerSm = 2;
 constexpr uint32_t kHizMaxBytes = 96 * 1024;   // per CTA, in shared memory
 struct HizParams {

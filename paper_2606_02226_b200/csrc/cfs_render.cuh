@@ -140,6 +140,7 @@ __device__ __forceinline__ uint32_t splat_q(const RenderParams &prm, const Share
         // it never leaves the SM.  ~95 % of the splats of a solid stop here (DESIGN "Hi-Z variant").
         uint32_t px, py;
         pixel_xy(prm, qx, qy, px, py);
+        CFS_CHECK((py >> prm.hiz.shift) * prm.hiz.nbx + (px >> prm.hiz.shift) < prm.hiz.nbx * prm.hiz.nby);
         const uint32_t bound = lds_u16(sm.dyn + 2u * ((py >> prm.hiz.shift) * prm.hiz.nbx + (px >> prm.hiz.shift)));
         if ((__float_as_uint(qz) >> 16) > bound) return 0u;
         splat_depth(reinterpret_cast<unsigned long long *>(prm.image), (int)(py * (uint32_t)prm.W + px), qz,
@@ -147,6 +148,7 @@ __device__ __forceinline__ uint32_t splat_q(const RenderParams &prm, const Share
         return 0u;
     }
     const int pix = (SPLAT == SPLAT_BIN) ? bin_pixel_of(br, qx, qy) : pixel_of(prm, qx, qy);
+    CFS_CHECK((uint32_t)pix < (uint32_t)prm.W * (uint32_t)prm.H);
     if (SPLAT == SPLAT_HIST_DIRECT) {
         red_add_u32(reinterpret_cast<uint32_t *>(prm.image) + pix, 1u);
     } else if (SPLAT == SPLAT_HIST_SHARED) {
@@ -198,6 +200,7 @@ __device__ __forceinline__ uint32_t bin_block_splat(const RenderParams &prm, con
 #pragma unroll
     for (int j = 0; j < 4; ++j) {      // out-of-bounds coordinates are clamped by the pixel rule: always a valid tile
         const int pix = bin_pixel_of(br, X[j], Y[j]);
+        CFS_CHECK((uint32_t)pix < (uint32_t)prm.W * (uint32_t)prm.H);
         fine[j] = true;
         if (!ok[j]) ++dropped;         // counted here, so that no `ok` outlives its splat
         if ((DIRECT_MASK >> j) & 1) {  // straight to L2: one predicated reduction, no branch
@@ -273,6 +276,48 @@ __device__ __forceinline__ uint32_t iterate_block(const RenderParams &prm, const
                 dropped += bin_block_splat<0, true>(prm, s, sm, br, X, Y, K, ok);    // br.ktp = 0 for HIST: k is ignored
             }
         }
+    } else if constexpr (!CHECKED && SIG != kChainGeneric && SPLAT == SPLAT_DEPTH_HIZ && !sig_has_branch(SIG) && !kReuse) {
+        // Hi-Z depth splats of a steady-state block in stages: the four chains, bounds tests and Hi-Z tests first, then the
+        // pre-test loads of the survivors back to back, then the compares -- one exposed L2 latency per block instead
+        // of four (the render is bound by instruction issue, and the sequential form spent a quarter of its stall
+        // samples waiting for each load in turn: profiles/r02c).
+        float X[4], Y[4], Z[4];
+        int K[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const uint32_t u = (j == 0) ? w.x : (j == 1) ? w.y : (j == 2) ? w.z : w.w;
+            K[j] = pick_index<OPT>(u, sm, prm);
+            apply_gen<DIM, AFF>(K[j], sm, prm, gx, gy, gz);
+            X[j] = gx; Y[j] = gy; Z[j] = gz;                 // the copies of Fig. 2(B)
+        }
+        unsigned long long *buf = reinterpret_cast<unsigned long long *>(prm.image);
+        uint32_t pix[4];
+        bool sv[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const bool alive = apply_chain<DIM, SIG, TRIG>(prm, StepCtx{plo, phi, it0 + j}, X[j], Y[j], Z[j]);
+            const bool ok = alive && in_bounds<OPT>(prm, X[j], Y[j]);
+            if (!ok) ++dropped;
+            uint32_t px, py;
+            pixel_xy(prm, X[j], Y[j], px, py);               // clamped: a valid pixel and block even for a dropped splat
+            CFS_CHECK((py >> prm.hiz.shift) * prm.hiz.nbx + (px >> prm.hiz.shift) < prm.hiz.nbx * prm.hiz.nby);
+            const uint32_t bound = lds_u16(sm.dyn + 2u * ((py >> prm.hiz.shift) * prm.hiz.nbx + (px >> prm.hiz.shift)));
+            sv[j] = ok && !((__float_as_uint(Z[j]) >> 16) > bound);
+            pix[j] = py * (uint32_t)prm.W + px;
+        }
+        unsigned long long cur[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {                        // the survivors' pre-test loads, all in flight together
+            cur[j] = 0ull;
+            if (sv[j]) cur[j] = __ldcg(buf + pix[j]);
+        }
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            if (sv[j] && __float_as_uint(Z[j]) <= (uint32_t)(cur[j] >> 32)) {      // else the key is larger whatever its colour
+                const unsigned long long key = ((unsigned long long)__float_as_uint(Z[j]) << 32) | lds_u32(sm.tab + CFS_SM_OFF(pal8) + 4u * (uint32_t)K[j]);
+                if (key < cur[j]) atomicMin(buf + pix[j], key);
+            }
+        }
     } else {
 #pragma unroll(CHECKED ? 1 : 4)
         for (int j = 0; j < 4; ++j) {
@@ -291,7 +336,7 @@ __device__ __forceinline__ uint32_t iterate_block(const RenderParams &prm, const
     }
     if (SPLAT == SPLAT_BIN && ((((uint32_t)it0 >> 2) + 1u) & prm.bin.check_mask) == 0u) {   // CTA-uniform
         __syncthreads();
-        bin_flush(prm, s, s_hist, bl, false);
+        bin_flush_units(prm, s, s_hist, br, bl);
         __syncthreads();
     }
     return dropped;
@@ -307,6 +352,7 @@ render_kernel(const __grid_constant__ RenderParams prm)
 {
     __shared__ SharedTables s;
     extern __shared__ __align__(16) uint32_t s_hist[];   // SPLAT_HIST_SHARED: histogram; SPLAT_BIN: staging
+    CFS_CHECK_ENTRY();
     if (GEN == 0) load_tables(s, prm);
     if (SPLAT == SPLAT_HIST_SHARED)
         for (uint32_t i = threadIdx.x; i < prm.hist_bins; i += blockDim.x) s_hist[i] = 0u;

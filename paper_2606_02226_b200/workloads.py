@@ -227,3 +227,23 @@ def config(i: int) -> Workload:
 
 
 N_CONFIGS = 5
+
+
+def fig4_like() -> Workload:
+    """A scene with the STRUCTURE of the paper's Fig. 4 (planet, ring, stars and comet, all from ONE
+    circle primitive; the paper prints none of its formulas, so the numbers here are this repo's): the Eq. 1 circle
+    generator (r^2 reading: uniform disc) drives four branches per iteration -- a planet (uniform scale), a ring
+    (the disc squashed and tilted), 64 stars (a tiny copy placed by the on-the-fly PRNG, L198) and a comet (a
+    stretched, sheared copy) -- into the paper's 1920 x 1080 frame (L202).  One-to-many splatting:
+    4 splats per point and iteration.  Used by bench.py to put numbers beside the paper's own (L200: compile time
+    against frame time) and by the run-time specialisation tests."""
+    c30, s30 = math.cos(math.radians(30.0)), math.sin(math.radians(30.0))
+    planet = [Xform("affine", [0.42, 0.0, 0.0, 0.42, 0.0, 0.0])]
+    ring = [Xform("affine", [0.95 * c30, -0.12 * s30, 0.95 * s30, 0.12 * c30, 0.0, 0.0])]
+    stars = [Xform("affine", [0.006, 0.0, 0.0, 0.006, 0.0, 0.0]), Xform("scatter", [64, 1.7, 0.95, 0.0])]
+    comet = [Xform("affine", [0.30, 0.06, -0.05, 0.05, 1.05, 0.55])]
+    chain = planet + [Xform("branch")] + ring + [Xform("branch")] + stars + [Xform("branch")] + comet
+    return Workload(
+        "fig4_like_planet_ring_stars_comet_1080p",
+        System(2, "ifs", circle_funcs(r2_reading=True), chain, "map_index", palette_for(2)),
+        Render(1 << 20, SEED_BASE + 0x40, 200, 20, 1920, 1080, (-16.0 / 9.0, 16.0 / 9.0, -1.0, 1.0), "rgba_f32"))

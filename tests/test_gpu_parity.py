@@ -885,3 +885,60 @@ def test_cfg2_cfg3_cfg4_full_size_properties(cfs, oracle):
     assert hit.sum() > 1_000_000 and depth.min() >= 3.0 - 1e-6 and depth.max() <= 5.0 + 1e-6
     pal8 = set(int(v) for v in (g[hit] & np.uint64(0xFFFFFFFF)).astype(np.uint32)[:: 997])
     assert len(pal8) <= 20
+
+
+# ------------------------------------------------------------------ bounds checks of our own (no compute-sanitizer on this pool)
+_CHECKED_RENDERS = r"""
+import sys, numpy as np, torch
+sys.path.insert(0, %(root)r)
+from paper_2606_02226_b200 import cfs, workloads as W
+from oracle import cfs_oracle as O
+from tests._gpu_util import gpu_render
+def same(w, variant, flags=0, scratch=None, cloud=None, exact=True):
+    g, c = gpu_render(cfs, w, variant=variant, flags=flags, scratch_bytes=scratch, cloud=cloud)
+    o, oc, _ = O.render_parallel(w.system, w.render, cloud=cloud)
+    assert np.array_equal(c, oc) or cloud is not None
+    if exact:
+        assert np.array_equal(g.astype(o.dtype), o), (w.name, variant)
+w0 = W.config(0).scaled(n_points=5000 + 13, iterations=300)
+for v, f in (("direct", 0), ("warp_agg", 0), ("binned", 0), ("binned", ["bin_hybrid"])):
+    same(w0, v, f)
+same(W.config(0).scaled(n_points=3000, iterations=200, width=200, height=120), "shared_hist")
+w0c = W.config(0).scaled(n_points=400000, iterations=120)
+sysh = cfs.cfs_create(w0c.system); need = cfs.cfs_binned_scratch_bytes(sysh, cfs.make_args(w0c.render)); sysh.close()
+same(w0c, "binned", ["bin_hybrid"], scratch=need * 2 // 3)                       # several chunks
+hot = W.Workload("hot", W.System(2, "ifs", W.square_funcs(probs=[0.0, 0.0, 1.0, 0.0]), [], "map_index", W.palette_for(4)),
+                 W.Render(400, 5, 200, 40, 512, 512, (-1, 1, -1, 1), "rgba_f32"))
+same(hot, "binned", ["bin_hybrid"])                                              # one pixel takes everything: rows overflow
+w1 = W.config(1).scaled(n_points=(1 << 14) + 5)
+gb, _ = gpu_render(cfs, w1, variant="binned", flags=["bin_hybrid", "fast_trig"])
+gd, _ = gpu_render(cfs, w1, variant="direct", flags=["fast_trig"])
+assert np.array_equal(gb, gd)
+w4 = W.config(4).scaled(n_points=300000 + 7, iterations=100, width=256, height=144)
+same(w4, "depth_hiz", scratch=cfs.cfs_hiz_scratch_bytes(256, 144))
+same(w4, "direct")
+w3 = W.config(3)
+cloud = W.gaussian_mixture_cloud((1 << 16) + 11, w3.cloud_seed)
+same(w3.scaled(n_points=(1 << 16) + 11), "auto", cloud=cloud, exact=False)
+print("checked renders ok; kernels compiled at run time:", cfs.cfs_jit_stats()[0])
+"""
+
+
+@pytest.mark.parametrize("selftest", [False, True])
+def test_device_bounds_checks(cfs, selftest):
+    """compute-sanitizer is closed on this pool, so the kernels carry bounds checks of their own (CFS_CHECK in csrc/:
+    staging rows, pool positions, tile / record / pixel / Hi-Z indices, ring stages), compiled in by -DCFS_CHECKS=1 for
+    run-time compiled kernels.  Here every splat variant renders in a fresh process with all kernels compiled under
+    the checks (a failed check traps and the render raises) and still matches the oracle; the negative control
+    (-DCFS_CHECK_SELFTEST=1: every kernel fails its first check) must fail."""
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = dict(os.environ, CFS_FORCE_JIT="1", CFS_JIT_OPTIONS="-DCFS_CHECKS=1" + (" -DCFS_CHECK_SELFTEST=1" if selftest else ""))
+    p = subprocess.run([sys.executable, "-c", _CHECKED_RENDERS % {"root": root}], env=env, capture_output=True, text=True, timeout=900)
+    if selftest:
+        assert p.returncode != 0, "the negative control rendered without tripping a check"
+    else:
+        assert p.returncode == 0, p.stdout[-2000:] + p.stderr[-4000:]
+        assert "checked renders ok" in p.stdout and not p.stdout.strip().endswith(": 0")
