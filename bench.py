@@ -771,7 +771,9 @@ def main():
                     help="only launch cfs_render of configs[N] --steps times (ncu target; no bench line)")
     ap.add_argument("--profile-points", type=int, default=None, help="with --profile-cfg: render only the first N points")
     ap.add_argument("--variant", default="auto", help="splat variant: auto (tile bins / Hi-Z with scratch for large renders, else direct), direct, ...")
-    ap.add_argument("--scratch-mib", type=int, default=8192, help="cap of the scratch buffer handed to AUTO (MiB); less means more chunks")
+    ap.add_argument("--scratch-mib", type=int, default=2048,
+                    help="cap of the scratch buffer handed to AUTO (MiB); less means more chunks (measured: 1 GiB +5 %%, 2 GiB +2 %% "
+                         "against one chunk on configs[1] and [2], DESIGN 'scratch')")
     ap.add_argument("--no-jit", action="store_true", help="use the kernels linked ahead of time instead of the run-time compiled ones")
     ap.add_argument("--accurate-trig", action="store_true",
                     help="evaluate sin/cos with sincosf (<= 2 ulp) instead of CFS_FLAG_FAST_TRIG (MUFU); both are inside "

@@ -359,24 +359,28 @@ def test_hist_output_of_a_coloured_system_through_the_bins(cfs, oracle, cfg):
     assert np.array_equal(cd, oc) and density_l1(gd, o) <= L1_TOL
 
 
+@pytest.mark.parametrize("jit", [False, True])
 @pytest.mark.parametrize("cfg,n", [(1, 1 << 18), (2, 1 << 19)])
-def test_bench_launch_configuration_against_the_oracle(cfs, oracle, cfg, n):
-    """The EXACT configuration bench.py times -- variant AUTO with scratch (-> hybrid: every other splat
-    straight to L2, the rest through the tile bins) and CFS_FLAG_FAST_TRIG (MUFU sin/cos) -- on a point
-    sub-range large enough for AUTO's hybrid threshold, at full image size, DIRECTLY against the oracle:
-    counters equal, normalised-density L1 <= 1e-3 on the count and on every colour channel."""
+def test_bench_launch_configuration_against_the_oracle(cfs, oracle, cfg, n, jit):
+    """The EXACT configuration bench.py times -- variant AUTO with scratch (-> hybrid: one splat in four straight to
+    L2, the rest through the tile bins), CFS_FLAG_FAST_TRIG (MUFU sin/cos) and the kernels compiled at run time for the
+    system (CFS_FLAG_JIT; also the linked ones) -- on a point sub-range large enough for AUTO's hybrid threshold, at
+    full image size, DIRECTLY against the oracle: counters equal, normalised-density L1 <= 1e-3 on the count and on
+    every colour channel."""
     import torch
     w = W.config(cfg).scaled(n_points=n)
     t = w.frames[len(w.frames) // 2]
+    flags = ["fast_trig"] + (["jit"] if jit else [])
     sysh = cfs.cfs_create(w.system)
     need = cfs.cfs_binned_scratch_bytes(sysh, cfs.make_args(w.render))
     assert need > 0
     scratch = torch.empty(need, dtype=torch.uint8, device="cuda")
     img = cfs.new_image(w.render)
     ctr = torch.zeros(2, dtype=torch.int64, device="cuda")
+    if jit:
+        cfs.cfs_specialize(sysh, cfs.make_args(w.render, t=t, variant="auto", flags=flags))
     cfs.cfs_launch_count(reset=True)
-    cfs.cfs_render(sysh, cfs.make_args(w.render, d_image=img, d_counters=ctr, t=t, variant="auto",
-                                       flags=["fast_trig"], d_scratch=scratch))
+    cfs.cfs_render(sysh, cfs.make_args(w.render, d_image=img, d_counters=ctr, t=t, variant="auto", flags=flags, d_scratch=scratch))
     torch.cuda.synchronize()
     assert cfs.cfs_launch_count() == 2, "AUTO did not take the hybrid stage (pass 1 + pass 2 in one chunk)"
     g, gc = img.cpu().numpy(), ctr.cpu().numpy().astype(np.uint64)
@@ -386,6 +390,38 @@ def test_bench_launch_configuration_against_the_oracle(cfs, oracle, cfg, n):
     assert g[:, 3].astype(np.float64).sum() == o[:, 3].sum() == float(oc[0])
     for ch in range(4):
         assert density_l1(g[:, ch], o[:, ch]) <= L1_TOL, (cfg, ch, density_l1(g[:, ch], o[:, ch]))
+
+
+def test_bench_launch_configuration_cfg3_cfg4_against_the_oracle(cfs, oracle):
+    """configs[3] and configs[4] as bench.py launches them (AUTO with scratch, MUFU sin/cos, run-time compiled kernels):
+    the streamed cloud on 2^20 records (L1 <= 1e-3 per channel), and the Menger depth render on 1.18 M points -- enough
+    splats for AUTO to take the Hi-Z variant (plain slice, map build, Hi-Z phase) -- bit for bit against the oracle,
+    full 4K images."""
+    import torch
+    flags = ["fast_trig", "jit"]
+    w = W.config(3)
+    n = 1 << 20
+    cloud = W.gaussian_mixture_cloud(n, w.cloud_seed)
+    w = w.scaled(n_points=n)
+    g, gc = gpu_render(cfs, w, cloud=cloud, variant="auto", flags=flags)
+    o, oc, _ = oracle.render_parallel(w.system, w.render, cloud=cloud)
+    assert int(gc[0]) + int(gc[1]) == n and abs(int(gc[0]) - int(oc[0])) <= 4
+    for ch in range(4):
+        assert density_l1(g[:, ch], o[:, ch]) <= L1_TOL, (3, ch, density_l1(g[:, ch], o[:, ch]))
+    w = W.config(4).scaled(n_points=(1 << 20) + (1 << 17) + 8)   # >= 2^30 splats: AUTO's threshold for the Hi-Z variant
+    sysh = cfs.cfs_create(w.system)
+    img = cfs.new_image(w.render)
+    ctr = torch.zeros(2, dtype=torch.int64, device="cuda")
+    scratch = torch.empty(cfs.cfs_hiz_scratch_bytes(w.render.width, w.render.height), dtype=torch.uint8, device="cuda")
+    cfs.cfs_specialize(sysh, cfs.make_args(w.render, variant="auto", flags=flags))
+    cfs.cfs_launch_count(reset=True)
+    cfs.cfs_render(sysh, cfs.make_args(w.render, d_image=img, d_counters=ctr, variant="auto", flags=flags, d_scratch=scratch))
+    torch.cuda.synchronize()
+    assert cfs.cfs_launch_count() in (3, 5), "AUTO did not take the Hi-Z depth variant"      # plain slice, map build, Hi-Z phase (+ rebuild, phase)
+    g, gc = cfs.image_to_numpy(img, "depth_u64"), ctr.cpu().numpy().astype(np.uint64)
+    sysh.close()
+    o, oc, _ = oracle.render_parallel(w.system, w.render)
+    assert np.array_equal(g, o) and np.array_equal(gc, oc)
 
 
 def test_binned_hot_tile_overflow_and_limits(cfs, oracle):
@@ -819,7 +855,7 @@ def test_cfg1_full_size_properties(cfs, oracle):
         assert np.array_equal(gb, g) and np.array_equal(gbc, gc)
     # the configuration bench.py times: MUFU sin/cos, AUTO with scratch (-> tile bins).  Conservation
     # stays exact; against the accurate image only splats within ~2^-21 of a pixel edge move.
-    gf, gfc = gpu_render(cfs, w, variant="auto", scratch_bytes=need, flags=["fast_trig"])
+    gf, gfc = gpu_render(cfs, w, variant="auto", scratch_bytes=need, flags=["fast_trig", "jit"])
     assert np.array_equal(gfc, gc) and gf[:, 3].astype(np.float64).sum() == S
     for ch in range(4):
         assert density_l1(gf[:, ch], g[:, ch]) <= L1_TOL
@@ -843,7 +879,7 @@ def test_cfg2_cfg3_cfg4_full_size_properties(cfs, oracle):
     sysh = cfs.cfs_create(w.system)
     need = cfs.cfs_binned_scratch_bytes(sysh, cfs.make_args(w.render))
     sysh.close()
-    ga, gac = gpu_render(cfs, w, t=t, variant="auto", scratch_bytes=need, flags=["fast_trig"])
+    ga, gac = gpu_render(cfs, w, t=t, variant="auto", scratch_bytes=need, flags=["fast_trig", "jit"])
     gd, gdc = gpu_render(cfs, w, t=t, variant="direct", flags=["fast_trig"])
     assert int(gac[0]) == S and int(gac[1]) == 0 and ga[:, 3].astype(np.float64).sum() == S
     assert ga[:, 3].max() < 2 ** 24 and np.array_equal(ga[:, 3], gd[:, 3]) and np.array_equal(gac, gdc)
@@ -863,11 +899,11 @@ def test_cfg2_cfg3_cfg4_full_size_properties(cfs, oracle):
     # counts the splats and every colour sum is an integer (exact float32 sums below 2^24)
     w = W.config(3)
     cloud = W.gaussian_mixture_cloud(w.render.n_points, w.cloud_seed)
-    g, gc = gpu_render(cfs, w, cloud=cloud)
+    g, gc = gpu_render(cfs, w, cloud=cloud, flags=["fast_trig", "jit"])
     assert int(gc[0]) + int(gc[1]) == 1 << 24 and g[:, 3].astype(np.float64).sum() == int(gc[0])
     assert g.max() < 2 ** 24 and np.all(g == np.round(g))
     n_sub = 1 << 17
-    gs, gsc = gpu_render(cfs, w, cloud=cloud, n_points=n_sub)
+    gs, gsc = gpu_render(cfs, w, cloud=cloud, n_points=n_sub, flags=["fast_trig", "jit"])
     o, oc, _ = oracle.render_parallel(w.system, w.render, cloud=cloud, n_points=n_sub)
     assert abs(int(gsc[0]) - int(oc[0])) <= 4
     for ch in range(4):
@@ -875,8 +911,10 @@ def test_cfg2_cfg3_cfg4_full_size_properties(cfs, oracle):
     # configs[4]: min over all points <= min over any subset, with equality wherever the subset holds the
     # winner; every key carries a depth in [3, 5] and one of the 20 palette entries
     w = W.config(4)
-    g, gc = gpu_render(cfs, w)
+    g, gc = gpu_render(cfs, w, variant="auto", flags=["jit"], scratch_bytes=cfs.cfs_hiz_scratch_bytes(3840, 2160))    # Hi-Z, as bench.py
     assert int(gc[0]) == (1 << 26) * 980 and int(gc[1]) == 0
+    gdir, gdc = gpu_render(cfs, w, variant="direct")          # the direct variant, linked kernel: the same image, bit for bit
+    assert np.array_equal(g, gdir) and np.array_equal(gc, gdc)
     sub = w.scaled(n_points=1 << 12)
     o, _, _ = oracle.render_parallel(sub.system, sub.render)
     assert np.all(g <= o)
