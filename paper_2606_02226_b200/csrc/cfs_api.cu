@@ -2,6 +2,7 @@
 // tables and frame-dependent parameters, kernel selection and launch.  No CPU fallback.
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -753,6 +754,18 @@ extern "C" cfs_status cfs_binned_plan(int32_t width, int32_t height, int32_t out
     return CFS_OK;
 }
 
+// records one point sends through the tile bins: its splats minus those the hybrid stage sends straight to L2
+// (iterations whose bit is set in the direct mask, in the steady-state Philox blocks only: the blocks touching
+// burn-in or the ragged end bin everything)
+static uint64_t binned_per_point(const cfs_system *s, const cfs_render_args *a)
+{
+    const uint64_t br = branches_of(s);
+    const int I = a->iterations, B = a->burn_in;
+    const int fast0 = std::min((B + 3) & ~3, I & ~3), fast1 = I & ~3;
+    const uint64_t direct = (uint64_t)__builtin_popcount(hybrid_mask(a)) * (uint64_t)((fast1 - fast0) / 4) * br;
+    return (uint64_t)(I - B) * br - direct;
+}
+
 extern "C" uint64_t cfs_binned_scratch_bytes(const cfs_system *s, const cfs_render_args *a)
 {
     const DeviceInfo &di = device_info();
@@ -760,7 +773,7 @@ extern "C" uint64_t cfs_binned_scratch_bytes(const cfs_system *s, const cfs_rend
     BinPlan pl;
     const char *why = "";
     if (!bin_shape(s, a, di, &pl, &why)) return 0;
-    return bin_scratch_for(pl, a->n_points, (uint64_t)(a->iterations - a->burn_in) * branches_of(s));
+    return bin_scratch_for(pl, a->n_points, binned_per_point(s, a));
 }
 
 extern "C" uint64_t cfs_shared_hist_max_bytes(void)
@@ -824,7 +837,7 @@ cfs_status render_binned(const cfs_system *s, const cfs_render_args *a, RenderPa
     const char *why = "";
     if (!bin_shape(s, a, di, &pl, &why)) return fail(CFS_ERR_UNSUPPORTED, "%s", why);
     if (!a->d_scratch) return fail(CFS_ERR_UNSUPPORTED, "binned variant needs d_scratch (see cfs_binned_scratch_bytes)");
-    const uint64_t spp = (uint64_t)(a->iterations - a->burn_in) * branches_of(s);
+    const uint64_t spp = binned_per_point(s, a);          // records per point that really go through the bins
     if (!bin_layout(&pl, a->d_scratch, a->scratch_bytes, a->n_points, spp, &why)) return fail(CFS_ERR_UNSUPPORTED, "%s", why);
     p.bin = pl.bp;
     p.bin.hybrid = hybrid_mask(a);
