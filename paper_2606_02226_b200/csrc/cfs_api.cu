@@ -475,6 +475,61 @@ void apply_uscale(const cfs_system *s, RenderParams &p)
     p.coef_rstride = 16u << p.coef_cshift; p.coef_kstride = p.coef_rstride;
 }
 
+// OPT_RCP_NORMAL: true when the host can PROVE that every live splat reaches each PINHOLE of the chain with a depth d in
+// [2^-126, 2^126), where the reciprocal's normal-range sequence is the correctly rounded one.  d > near holds for a
+// live splat, so near >= 2^-100 gives the lower end; the upper end needs a bound on |z|: an IFS of affine
+// contractions keeps its points inside the cube of half-width R = max(1, max_k |b_k| / (1 - |A_k|)) (infinity norms;
+// the initial point lies in [-1, 1)^3), and AFFINE / ROTATE_Z / TWIST_Z / BEND / SCATTER steps grow that bound by a
+// computable factor.  Anything else (a stored cloud, reuse, other steps): no proof, no option.
+bool depth_range_proved(const cfs_system *s, const RenderParams &p)
+{
+    if (s->gen != CFS_GEN_IFS || p.reuse || s->aff == cfs::AFF_CIRCLE) return false;
+    double R = 1.0;
+    for (const cfs_func &f : s->funcs) {
+        const float *m = f.params;
+        double na = 0.0, nb = 0.0;
+        const int d = s->dim;
+        for (int r = 0; r < d; ++r) {
+            double row = 0.0;
+            for (int c = 0; c < d; ++c) row += std::fabs((double)m[r * d + c]);
+            na = std::max(na, row);
+            nb = std::max(nb, std::fabs((double)m[d * d + r]));
+        }
+        if (!(na < 0.999)) return false;
+        R = std::max(R, nb / (1.0 - na));
+    }
+    bool any = false;
+    double Rb = R;                                   // bound inside the current branch
+    for (int m = 0; m < p.n_chain; ++m) {
+        const cfs::ChainStep &st = p.chain[m];
+        switch (st.type) {
+        case cfs::T_BRANCH: Rb = R; break;
+        case cfs::T_AFFINE: case cfs::T_SCALE: {
+            double na = 0.0, nb = 0.0;
+            const int d = s->dim;
+            for (int r = 0; r < d; ++r) {
+                double row = 0.0;
+                for (int c = 0; c < d; ++c) row += std::fabs((double)st.p[r * d + c]);
+                na = std::max(na, row);
+                nb = std::max(nb, std::fabs((double)st.p[d * d + r]));
+            }
+            Rb = na * Rb + nb;
+            break;
+        }
+        case cfs::T_TWIST_Z: case cfs::T_BEND: Rb *= 1.4142135623730951; break;      // (x, y) rotated: each at most sqrt(2) R
+        case cfs::T_SCATTER: Rb += std::max(std::fabs((double)st.p[1]), std::max(std::fabs((double)st.p[2]), std::fabs((double)st.p[3]))); break;
+        case cfs::T_PINHOLE:
+            if (!((double)st.p[3] >= 0x1p-100 && Rb + std::fabs((double)st.p[2]) < 0x1p100)) return false;
+            any = true;
+            Rb = 1e300;                              // nothing may follow a projection in this proof
+            break;
+        default: return false;
+        }
+        if (!(Rb < 1e300) && st.type != cfs::T_PINHOLE) return false;
+    }
+    return any;
+}
+
 // options compiled into a run-time specialised kernel (cfs_params.h KernelOpt): everything the host knows about
 // the system and the render that lets the kernel drop a run-time decision
 int jit_options(const cfs_system *s, const RenderParams &p, int splat)
@@ -486,6 +541,7 @@ int jit_options(const cfs_system *s, const RenderParams &p, int splat)
         else if (p.pick_steps <= 1) opt |= cfs::OPT_PICK_LUT1;
     }
     if (p.xmin == -p.xmax && p.ymin == -p.ymax) opt |= cfs::OPT_SYM_BOUNDS;
+    if (depth_range_proved(s, p)) opt |= cfs::OPT_RCP_NORMAL;
     if (splat == cfs::SPLAT_BIN) {
         opt |= cfs::OPT_BIN_FIXED | ((int)(p.bin.hybrid & 15u) << cfs::OPT_BIN_MASK_SHIFT);
         if (p.color_rule != 0) opt |= cfs::OPT_BIN_RGBA;

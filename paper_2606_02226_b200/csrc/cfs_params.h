@@ -62,6 +62,8 @@ enum KernelOpt : int {
     OPT_BIN_FIXED = 32,    // tile bins: OPT_BIN_RGBA and the direct mask below are the truth (else prm.bin.hybrid / prm.color_rule decide at run time)
     OPT_SYM_BOUNDS = 64,   // xmin == -xmax and ymin == -ymax: the closed-bounds test is |x| <= xmax && |y| <= ymax (two compares)
     OPT_PICK_CMP2 = 128,   // at most two thresholds: k = (u >= T[0]) + (u >= T[1]), two compares against the parameter block, no table read
+    OPT_RCP_NORMAL = 4096, // PINHOLE: the host has PROVED 2^-126 <= d < 2^126 for every live splat (bounded attractor, near >= 2^-100), so
+                           // 1/d is the four-instruction normal-range sequence of the correctly rounded reciprocal, without its range test
     OPT_BIN_MASK_SHIFT = 8 // bits 8..11, with OPT_BIN_FIXED: iteration j of a steady-state block splats straight to L2 when bit j is set
 };
 // true when the signature holds a BRANCH separator (type 8): one-to-many splatting

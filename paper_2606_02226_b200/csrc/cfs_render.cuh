@@ -75,7 +75,7 @@ __device__ __forceinline__ uint32_t branches_static(const RenderParams &prm, con
                                                     const BinRegs &br, const StepCtx &ctx, bool bin_direct_half)
 {
     float qx = gx, qy = gy, qz = gz;
-    const bool alive = chain_static<DIM, SIG, TRIG, M>(prm, ctx, qx, qy, qz);
+    const bool alive = chain_static<DIM, SIG, TRIG, M, OPT>(prm, ctx, qx, qy, qz);
     uint32_t dropped = splat_q<DIM, GEN, SPLAT, OPT>(prm, s, sm, s_hist, qx, qy, qz, alive, k, point_rgba8, have, br, bin_direct_half);
     constexpr int next = sig_next_branch(SIG, M);
     if constexpr (next >= 0)
@@ -114,7 +114,7 @@ __device__ __forceinline__ uint32_t chain_and_splat(const RenderParams &prm, con
         return dropped;
     }
     float qx = gx, qy = gy, qz = gz;            // the copy of Fig. 2(B)
-    const bool alive = apply_chain<DIM, SIG, TRIG>(prm, ctx, qx, qy, qz);
+    const bool alive = apply_chain<DIM, SIG, TRIG, OPT>(prm, ctx, qx, qy, qz);
     if ((SIG == kChainGeneric) ? (prm.reuse != 0) : ((OPT & OPT_REUSE) != 0)) {    // Fig. 2(C): the same point is reused
         gx = qx; gy = qy; gz = qz;
         if (!past_burn_in) return 0u;
@@ -260,7 +260,7 @@ __device__ __forceinline__ uint32_t iterate_block(const RenderParams &prm, const
         // a thread without a point carries NaN coordinates (render_kernel), which fail every bounds test: no `have` here
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
-            const bool alive = apply_chain<DIM, SIG, TRIG>(prm, StepCtx{plo, phi, it0 + j}, X[j], Y[j], Z[j]);
+            const bool alive = apply_chain<DIM, SIG, TRIG, OPT>(prm, StepCtx{plo, phi, it0 + j}, X[j], Y[j], Z[j]);
             ok[j] = alive && bin_in_bounds<(OPT & OPT_SYM_BOUNDS) != 0>(br, X[j], Y[j]);
         }
         if constexpr ((OPT & OPT_BIN_FIXED) != 0) {
@@ -295,7 +295,7 @@ __device__ __forceinline__ uint32_t iterate_block(const RenderParams &prm, const
         bool sv[4];
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
-            const bool alive = apply_chain<DIM, SIG, TRIG>(prm, StepCtx{plo, phi, it0 + j}, X[j], Y[j], Z[j]);
+            const bool alive = apply_chain<DIM, SIG, TRIG, OPT>(prm, StepCtx{plo, phi, it0 + j}, X[j], Y[j], Z[j]);
             const bool ok = alive && in_bounds<OPT>(prm, X[j], Y[j]);
             if (!ok) ++dropped;
             uint32_t px, py;

@@ -802,6 +802,88 @@ def test_resolve_rgba8_single_pass_with_a_given_maximum(cfs, oracle, cfg):
     sysh.close()
 
 
+def test_resolve_with_the_previous_frames_maximum_and_the_rgba8_host_entry(cfs, oracle):
+    """An animation (BASELINE configs[2]; PAPER L9, L206 in-betweens) resolved frame by frame: frame 0 measures its
+    maximum inside the launch (n_max = 0), frame k > 0 is mapped with frame k-1's maximum taken from the scratch word
+    on the device (n_max < 0: no host round trip) -- the same bytes as passing that maximum explicitly.  And the
+    end-to-end host entry (cfs_render_rgba8_host: H2D, clear, render, resolve, D2H of the RGBA8888 image only) returns
+    what the device calls produce."""
+    import torch
+    w = W.config(2).scaled(n_points=1 << 14, iterations=120)
+    r = w.render
+    npx = r.width * r.height
+    sysh = cfs.cfs_create(w.system)
+    img = cfs.new_image(r)
+    out = torch.zeros(npx, dtype=torch.int32, device="cuda")
+    ref = torch.zeros(npx, dtype=torch.int32, device="cuda")
+    scr = torch.zeros(4, dtype=torch.int32, device="cuda")
+    scr2 = torch.zeros(4, dtype=torch.int32, device="cuda")
+    prev_max = None
+    h_out = np.zeros(npx, dtype=np.uint32)
+    h_ctr = np.zeros(2, dtype=np.uint64)
+    h_max = np.zeros(1, dtype=np.float32)
+    for k, t in enumerate(w.frames[:4]):
+        img.zero_()
+        cfs.cfs_render(sysh, cfs.make_args(r, d_image=img, t=t, variant="direct"))
+        cfs.cfs_resolve_rgba8(img, r.out_mode, r.width, r.height, 2.2, 1 / 255.0, 0.0 if k == 0 else -1.0, out, scr)
+        cfs.cfs_resolve_rgba8(img, r.out_mode, r.width, r.height, 2.2, 1 / 255.0, 0.0 if k == 0 else prev_max, ref, scr2)
+        torch.cuda.synchronize()
+        assert torch.equal(out, ref), k
+        this_max = float(img[:, 3].max().item())
+        assert scr.cpu().numpy().view(np.float32)[0] == np.float32(this_max) == scr2.cpu().numpy().view(np.float32)[0]
+        # the host entry point, same frame, same maximum
+        cfs.cfs_render_rgba8_host(sysh, cfs.make_args(r, t=t, variant="direct"), 2.2, 1 / 255.0, 0.0 if k == 0 else prev_max,
+                                  h_out, None, h_ctr, h_max)
+        assert np.array_equal(h_out, out.cpu().numpy().view(np.uint32)) and h_max[0] == np.float32(this_max)
+        assert int(h_ctr[0]) + int(h_ctr[1]) == r.n_points * (r.iterations - r.burn_in)
+        prev_max = this_max
+    sysh.close()
+
+
+def test_render_and_resolve_replay_from_a_cuda_graph(cfs, oracle):
+    """cfs_render / cfs_resolve_rgba8 allocate nothing and never synchronise (include/cfs.h), so a frame -- clear, render
+    through the tile bins (memset + pass 1 + pass 2), resolve (memset + cooperative kernel) -- is captured once into a
+    CUDA graph and replayed; run-time compiled kernels are compiled before the capture (cfs_specialize).  Each replay
+    reproduces the eagerly rendered frame bit for bit."""
+    import torch
+    w = W.config(1).scaled(n_points=(1 << 15) + 3, iterations=200)
+    r = w.render
+    flags = ["fast_trig", "jit"]
+    sysh = cfs.cfs_create(w.system)
+    need = cfs.cfs_binned_scratch_bytes(sysh, cfs.make_args(r, variant="binned", flags=flags + ["bin_hybrid"]))
+    scratch = torch.empty(need, dtype=torch.uint8, device="cuda")
+    img = cfs.new_image(r)
+    out = torch.zeros(r.width * r.height, dtype=torch.int32, device="cuda")
+    tone = torch.zeros(4, dtype=torch.int32, device="cuda")
+    args = cfs.make_args(r, d_image=img, variant="binned", flags=flags + ["bin_hybrid"], d_scratch=scratch)
+    cfs.cfs_specialize(sysh, args)
+
+    def frame():
+        img.zero_()
+        cfs.cfs_render(sysh, args)
+        cfs.cfs_resolve_rgba8(img, r.out_mode, r.width, r.height, 2.2, 1 / 255.0, 0.0, out, tone)
+
+    frame()
+    torch.cuda.synchronize()
+    want_img, want_out = img.clone(), out.clone()
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        frame()                                   # warm-up on the capture stream
+    torch.cuda.current_stream().wait_stream(side)
+    torch.cuda.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        frame()
+    for _ in range(3):
+        img.fill_(7.0)
+        out.zero_()
+        graph.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(img, want_img) and torch.equal(out, want_out)
+    sysh.close()
+
+
 @pytest.mark.parametrize("cfg", [0, 3, 4])
 def test_render_host_entry_point(cfs, oracle, cfg):
     """cfs_render_host: HOST buffers in and out (the end-to-end call bench.py times)."""
