@@ -475,59 +475,82 @@ void apply_uscale(const cfs_system *s, RenderParams &p)
     p.coef_rstride = 16u << p.coef_cshift; p.coef_kstride = p.coef_rstride;
 }
 
-// OPT_RCP_NORMAL: true when the host can PROVE that every live splat reaches each PINHOLE of the chain with a depth d in
-// [2^-126, 2^126), where the reciprocal's normal-range sequence is the correctly rounded one.  d > near holds for a
-// live splat, so near >= 2^-100 gives the lower end; the upper end needs a bound on |z|: an IFS of affine
+// What the host can PROVE about a render and hand to a run-time compiled kernel as a dropped test.  An IFS of affine
 // contractions keeps its points inside the cube of half-width R = max(1, max_k |b_k| / (1 - |A_k|)) (infinity norms;
-// the initial point lies in [-1, 1)^3), and AFFINE / ROTATE_Z / TWIST_Z / BEND / SCATTER steps grow that bound by a
-// computable factor.  Anything else (a stored cloud, reuse, other steps): no proof, no option.
-bool depth_range_proved(const cfs_system *s, const RenderParams &p)
+// the initial point lies in [-1, 1)^3); AFFINE / ROTATE_Z / TWIST_Z / BEND / SWIRL / SINUSOIDAL / STRETCH_COS / SCATTER
+// steps change that bound by a computable amount, a PINHOLE turns it into a depth interval [d_min, d_max] and a bound on the projected
+// coordinates.  Hence: d in [2^-126, 2^126) at every PINHOLE (near >= 2^-100, |z| < 2^100), where the reciprocal's
+// normal-range sequence IS the correctly rounded one (OPT_RCP_NORMAL).  A stored cloud, reuse, the Eq. 1
+// generator or any other step: no proof, no option.
+// Returns the OPT_* bits proved for this render: OPT_RCP_NORMAL, and OPT_NO_DROP when moreover every splat of every
+// branch is alive (d > near at each PINHOLE) and lands strictly inside the image bounds, with a 1e-3 relative margin
+// against float rounding (the kernels' own CFS_CHECK re-tests both claims under -DCFS_CHECKS=1).
+int proved_options(const cfs_system *s, const RenderParams &p)
 {
-    if (s->gen != CFS_GEN_IFS || p.reuse || s->aff == cfs::AFF_CIRCLE) return false;
-    double R = 1.0;
-    for (const cfs_func &f : s->funcs) {
-        const float *m = f.params;
-        double na = 0.0, nb = 0.0;
-        const int d = s->dim;
+    if (s->gen != CFS_GEN_IFS || p.reuse || s->aff == cfs::AFF_CIRCLE) return 0;
+    const int d = s->dim;
+    auto norms = [d](const float *m, double *na, double *nb) {
+        *na = 0.0; *nb = 0.0;
         for (int r = 0; r < d; ++r) {
             double row = 0.0;
             for (int c = 0; c < d; ++c) row += std::fabs((double)m[r * d + c]);
-            na = std::max(na, row);
-            nb = std::max(nb, std::fabs((double)m[d * d + r]));
+            *na = std::max(*na, row);
+            *nb = std::max(*nb, std::fabs((double)m[d * d + r]));
         }
-        if (!(na < 0.999)) return false;
+    };
+    double R = 1.0;                                  // half-width of a cube that holds every generated point
+    for (const cfs_func &f : s->funcs) {
+        double na, nb;
+        norms(f.params, &na, &nb);
+        if (!(na < 0.999)) return 0;
         R = std::max(R, nb / (1.0 - na));
     }
-    bool any = false;
-    double Rb = R;                                   // bound inside the current branch
+    const double margin = 1.001;
+    const double bx = std::min(-(double)p.xmin, (double)p.xmax), by = std::min(-(double)p.ymin, (double)p.ymax);
+    bool rcp_ok = true, any_pinhole = false, no_drop = true;
+    double Rx = R, Ry = R, Rz = R;                   // per-axis bounds inside the current branch
+    bool projected = false;
+    auto end_branch = [&]() { if (!(Rx * margin < bx && Ry * margin < by)) no_drop = false; };
     for (int m = 0; m < p.n_chain; ++m) {
         const cfs::ChainStep &st = p.chain[m];
+        if (projected && st.type != cfs::T_BRANCH) return 0;      // nothing may follow a projection in this proof
         switch (st.type) {
-        case cfs::T_BRANCH: Rb = R; break;
+        case cfs::T_BRANCH: end_branch(); Rx = Ry = Rz = R; projected = false; break;
         case cfs::T_AFFINE: case cfs::T_SCALE: {
-            double na = 0.0, nb = 0.0;
-            const int d = s->dim;
-            for (int r = 0; r < d; ++r) {
-                double row = 0.0;
-                for (int c = 0; c < d; ++c) row += std::fabs((double)st.p[r * d + c]);
-                na = std::max(na, row);
-                nb = std::max(nb, std::fabs((double)st.p[d * d + r]));
+            double na, nb;
+            norms(st.p, &na, &nb);
+            const double Rm = std::max(Rx, std::max(Ry, d == 3 ? Rz : 0.0));
+            Rx = Ry = na * Rm + nb;
+            if (d == 3) Rz = Rx;
+            break;
+        }
+        case cfs::T_TWIST_Z: case cfs::T_BEND: case cfs::T_SWIRL: { const double r2 = std::sqrt(Rx * Rx + Ry * Ry); Rx = Ry = r2; break; }   // (x, y) rotated, z kept
+        case cfs::T_SINUSOIDAL: Rx = std::sin(std::min(Rx, 1.5707963267948966)); Ry = std::sin(std::min(Ry, 1.5707963267948966)); break;   // |sin| is increasing up to pi/2
+        case cfs::T_STRETCH_COS: Ry += 1.0; Rx *= 2.0; break;
+        case cfs::T_SCATTER: Rx += std::fabs((double)st.p[1]); Ry += std::fabs((double)st.p[2]); Rz += std::fabs((double)st.p[3]); break;
+        case cfs::T_PINHOLE: {
+            if (d != 3) return 0;
+            any_pinhole = true;
+            const double cam = (double)st.p[2], nearp = (double)st.p[3];
+            const double dmin = -Rz - cam, dmax = Rz - cam;
+            if (!(nearp >= 0x1p-100 && std::fabs(dmax) < 0x1p100 && std::fabs(dmin) < 0x1p100)) rcp_ok = false;
+            if (dmin > nearp * margin && dmin > 0x1p-100) {
+                Rx = (double)st.p[0] * Rx / dmin; Ry = (double)st.p[1] * Ry / dmin; Rz = dmax;
+            } else {
+                no_drop = false;                     // some splats may be behind the near plane
+                Rx = Ry = 1e300;
             }
-            Rb = na * Rb + nb;
+            projected = true;
             break;
         }
-        case cfs::T_TWIST_Z: case cfs::T_BEND: Rb *= 1.4142135623730951; break;      // (x, y) rotated: each at most sqrt(2) R
-        case cfs::T_SCATTER: Rb += std::max(std::fabs((double)st.p[1]), std::max(std::fabs((double)st.p[2]), std::fabs((double)st.p[3]))); break;
-        case cfs::T_PINHOLE:
-            if (!((double)st.p[3] >= 0x1p-100 && Rb + std::fabs((double)st.p[2]) < 0x1p100)) return false;
-            any = true;
-            Rb = 1e300;                              // nothing may follow a projection in this proof
-            break;
-        default: return false;
+        default: return 0;
         }
-        if (!(Rb < 1e300) && st.type != cfs::T_PINHOLE) return false;
     }
-    return any;
+    end_branch();
+    int opt = 0;
+    if (any_pinhole && rcp_ok) opt |= cfs::OPT_RCP_NORMAL;
+    if (no_drop) opt |= cfs::OPT_NO_DROP;
+    return opt;
 }
 
 // options compiled into a run-time specialised kernel (cfs_params.h KernelOpt): everything the host knows about
@@ -541,7 +564,7 @@ int jit_options(const cfs_system *s, const RenderParams &p, int splat)
         else if (p.pick_steps <= 1) opt |= cfs::OPT_PICK_LUT1;
     }
     if (p.xmin == -p.xmax && p.ymin == -p.ymax) opt |= cfs::OPT_SYM_BOUNDS;
-    if (depth_range_proved(s, p)) opt |= cfs::OPT_RCP_NORMAL;
+    opt |= proved_options(s, p);
     if (splat == cfs::SPLAT_BIN) {
         opt |= cfs::OPT_BIN_FIXED | ((int)(p.bin.hybrid & 15u) << cfs::OPT_BIN_MASK_SHIFT);
         if (p.color_rule != 0) opt |= cfs::OPT_BIN_RGBA;

@@ -64,6 +64,8 @@ enum KernelOpt : int {
     OPT_PICK_CMP2 = 128,   // at most two thresholds: k = (u >= T[0]) + (u >= T[1]), two compares against the parameter block, no table read
     OPT_RCP_NORMAL = 4096, // PINHOLE: the host has PROVED 2^-126 <= d < 2^126 for every live splat (bounded attractor, near >= 2^-100), so
                            // 1/d is the four-instruction normal-range sequence of the correctly rounded reciprocal, without its range test
+    OPT_NO_DROP = 8192,    // the host has PROVED (same bound, with a margin against rounding) that every splat is alive and inside the image
+                           // bounds: no near test, no bounds test, nothing to count as dropped
     OPT_BIN_MASK_SHIFT = 8 // bits 8..11, with OPT_BIN_FIXED: iteration j of a steady-state block splats straight to L2 when bit j is set
 };
 // true when the signature holds a BRANCH separator (type 8): one-to-many splatting

@@ -261,7 +261,13 @@ __device__ __forceinline__ uint32_t iterate_block(const RenderParams &prm, const
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
             const bool alive = apply_chain<DIM, SIG, TRIG, OPT>(prm, StepCtx{plo, phi, it0 + j}, X[j], Y[j], Z[j]);
-            ok[j] = alive && bin_in_bounds<(OPT & OPT_SYM_BOUNDS) != 0>(br, X[j], Y[j]);
+            if constexpr ((OPT & OPT_NO_DROP) != 0) {
+                // the host has proved every splat alive and in bounds: only a thread without a point (NaN) holds back
+                CFS_CHECK(!have || bin_in_bounds<false>(br, X[j], Y[j]));
+                ok[j] = have;
+            } else {
+                ok[j] = alive && bin_in_bounds<(OPT & OPT_SYM_BOUNDS) != 0>(br, X[j], Y[j]);
+            }
         }
         if constexpr ((OPT & OPT_BIN_FIXED) != 0) {
             // compiled for this render's split and output: one straight-line body
