@@ -94,10 +94,15 @@ __device__ __forceinline__ bool bin_in_bounds(const BinRegs &br, float x, float 
 
 // pixel rule of cfs_device.cuh pixel_of(), operands from registers
 // (the unsigned conversion saturates negative values to 0: the lower clamp costs nothing)
+// UNCLAMPED: the host has proved every splat inside the bounds with a margin (OPT_NO_DROP): the upper clamp cannot
+// bind; a thread without a point (NaN) converts to pixel 0 and stores nothing
+template <bool UNCLAMPED = false>
 __device__ __forceinline__ int bin_pixel_of(const BinRegs &br, float x, float y)
 {
-    const uint32_t px = min(__float2uint_rd(__fmaf_rn(x, br.sx, br.ox)), (uint32_t)br.Wm1);
-    const uint32_t py = min(__float2uint_rd(__fmaf_rn(y, br.sy, br.oy)), (uint32_t)br.Hm1);
+    uint32_t px = __float2uint_rd(__fmaf_rn(x, br.sx, br.ox));
+    uint32_t py = __float2uint_rd(__fmaf_rn(y, br.sy, br.oy));
+    CFS_CHECK(!UNCLAMPED || (px <= (uint32_t)br.Wm1 && py <= (uint32_t)br.Hm1));
+    if (!UNCLAMPED) { px = min(px, (uint32_t)br.Wm1); py = min(py, (uint32_t)br.Hm1); }
     return (int)(py * (uint32_t)br.W + px);
 }
 

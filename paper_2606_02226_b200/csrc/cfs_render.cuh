@@ -147,7 +147,7 @@ __device__ __forceinline__ uint32_t splat_q(const RenderParams &prm, const Share
                     lds_u32(sm.tab + CFS_SM_OFF(pal8) + 4u * (uint32_t)k));
         return 0u;
     }
-    const int pix = (SPLAT == SPLAT_BIN) ? bin_pixel_of(br, qx, qy) : pixel_of(prm, qx, qy);
+    const int pix = (SPLAT == SPLAT_BIN) ? bin_pixel_of(br, qx, qy) : pixel_of<OPT>(prm, qx, qy);
     CFS_CHECK((uint32_t)pix < (uint32_t)prm.W * (uint32_t)prm.H);
     if (SPLAT == SPLAT_HIST_DIRECT) {
         red_add_u32(reinterpret_cast<uint32_t *>(prm.image) + pix, 1u);
@@ -189,7 +189,7 @@ __device__ __forceinline__ uint32_t splat_q(const RenderParams &prm, const Share
 // for record + append, and pass 2 halves).  Any split is a correct result: HIST sums are exact,
 // RGBA sums are order-free (DESIGN R8).  Straight-line code: every reduction, atomic and store is predicated.
 // Returns the number of dropped splats.
-template <int DIRECT_MASK, bool RGBA>
+template <int DIRECT_MASK, bool RGBA, bool UNCLAMPED = false>
 __device__ __forceinline__ uint32_t bin_block_splat(const RenderParams &prm, const SharedTables &s, const Sm &sm, const BinRegs &br,
                                                     const float (&X)[4], const float (&Y)[4], const int (&K)[4],
                                                     const bool (&ok)[4])
@@ -199,7 +199,7 @@ __device__ __forceinline__ uint32_t bin_block_splat(const RenderParams &prm, con
     uint32_t dropped = 0u;
 #pragma unroll
     for (int j = 0; j < 4; ++j) {      // out-of-bounds coordinates are clamped by the pixel rule: always a valid tile
-        const int pix = bin_pixel_of(br, X[j], Y[j]);
+        const int pix = bin_pixel_of<UNCLAMPED>(br, X[j], Y[j]);
         CFS_CHECK((uint32_t)pix < (uint32_t)prm.W * (uint32_t)prm.H);
         fine[j] = true;
         if (!ok[j]) ++dropped;         // counted here, so that no `ok` outlives its splat
@@ -271,7 +271,7 @@ __device__ __forceinline__ uint32_t iterate_block(const RenderParams &prm, const
         }
         if constexpr ((OPT & OPT_BIN_FIXED) != 0) {
             // compiled for this render's split and output: one straight-line body
-            dropped += bin_block_splat<(OPT >> OPT_BIN_MASK_SHIFT) & 15, (OPT & OPT_BIN_RGBA) != 0>(prm, s, sm, br, X, Y, K, ok);
+            dropped += bin_block_splat<(OPT >> OPT_BIN_MASK_SHIFT) & 15, (OPT & OPT_BIN_RGBA) != 0, (OPT & OPT_NO_DROP) != 0>(prm, s, sm, br, X, Y, K, ok);
         } else {
             // warp-uniform choice of one of three straight-line bodies (hybrid RGBA / hybrid HIST / pure bins); any
             // non-zero mask runs as "every other splat" here -- the exact mask is a compiled-in option
@@ -305,7 +305,7 @@ __device__ __forceinline__ uint32_t iterate_block(const RenderParams &prm, const
             const bool ok = alive && in_bounds<OPT>(prm, X[j], Y[j]);
             if (!ok) ++dropped;
             uint32_t px, py;
-            pixel_xy(prm, X[j], Y[j], px, py);               // clamped: a valid pixel and block even for a dropped splat
+            pixel_xy<OPT>(prm, X[j], Y[j], px, py);          // clamped (or proved inside): a valid pixel and block even for a dropped splat
             CFS_CHECK((py >> prm.hiz.shift) * prm.hiz.nbx + (px >> prm.hiz.shift) < prm.hiz.nbx * prm.hiz.nby);
             const uint32_t bound = lds_u16(sm.dyn + 2u * ((py >> prm.hiz.shift) * prm.hiz.nbx + (px >> prm.hiz.shift)));
             sv[j] = ok && !((__float_as_uint(Z[j]) >> 16) > bound);
