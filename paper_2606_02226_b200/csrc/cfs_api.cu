@@ -170,7 +170,7 @@ cfs_status build_tables(cfs_system *s)
             if (T64[j] <= lo) ++below;
             else if (T64[j] <= hi) { if (!inside) first_m1 = (uint32_t)(T64[j] - 1); ++inside; }    // T > lo >= 0, so T - 1 >= 0
         }
-        s->lut[b][0] = first_m1;
+        s->lut[b][0] = ~first_m1;             // complemented: the device adds it to u and takes the carry (pick_index)
         s->lut[b][1] = (uint32_t)below;
         if (inside > s->pick_steps) s->pick_steps = inside;
     }

@@ -121,7 +121,7 @@ constexpr int kBinAccThreads = 1024;           // CTA size of pass 2 (one CTA pe
 // Hi-Z pre-test of the depth splat (DESIGN "Hi-Z variant").  hz[by * nbx + bx] is an upper bound of
 // (depth bits >> 16) over the 2^shift x 2^shift pixel block (bx, by), taken from a snapshot of the
 // depth image; the image only decreases, so the bound stays valid for the rest of the render.
-constexpr int kHizThreads = 768;               // CTA size of the Hi-Z render kernel, two CTAs per SM (1024 x 1 measured 197 against 172 ms)
+constexpr int kHizThreads = 576;               // CTA size of the Hi-Z render kernel, two CTAs per SM: 56 registers per thread, no spills (configs[4], ms: 512x2 132.3, 576x2 129.4, 640x2 130.8, 704x2 136.0, 768x2 135.2 with 40 registers and spills, 512x3 141.7, 1024x1 slower still)
 constexpr int kHizCtasPerSm = 2;
 constexpr uint32_t kHizMaxBytes = 96 * 1024;   // per CTA, in shared memory
 struct HizParams {
@@ -186,8 +186,9 @@ struct RenderParams {
 
     ChainStep chain[kMaxChain];
     uint32_t T[kMaxFuncs];       // thresholds (u32), T[j >= n_thr] = 0xFFFFFFFF
-    uint32_t lut[256][2];        // bucket b of the top byte of u: { (first threshold inside the bucket) - 1, or 0xFFFFFFFF
-                                 // when the bucket holds none;  #{j < n_thr : T[j] <= b << 24} }.  k = lut[b][1] + (u > lut[b][0])
+    uint32_t lut[256][2];        // bucket b of the top byte of u: { ~m, m = (first threshold inside the bucket) - 1, or 0xFFFFFFFF
+                                 // when the bucket holds none;  #{j < n_thr : T[j] <= b << 24} }.  k = lut[b][1] + (u > m),
+                                 // and u > m is the carry of u + ~m
                                  // is the pick when no bucket holds two thresholds; further ones are walked in T[]
     float coef[kMaxFuncs * 12];  // GENERAL dim2: rows of 8 (a00 a01 b0 0 | a10 a11 b1 0);
                                  // GENERAL dim3: rows of 12 (a00 a01 a02 b0 | ... );
