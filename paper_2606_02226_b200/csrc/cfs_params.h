@@ -114,8 +114,9 @@ constexpr uint32_t kBinTailShift = 11;         // tails word: blocks << 11 | rec
 constexpr uint32_t kBinDummy = 32;             // dummy fill counters behind cnt[n_tiles], one per lane: pre-set to the row capacity, they take
                                                // the dropped splats -- "row full" for free, so a dropped splat stores nothing and needs no predicate
 constexpr uint32_t kBinInvalid = 0xFFFFFFFFu;  // tile has no block (pool or list exhausted): direct splats
-constexpr int kBinThreads = 1024;              // CTA size of pass 1 and CTAs per SM.  Measured on configs[1]: 1 x 1024
-constexpr int kBinCtasPerSm = 1;               // threads 4.69 ms, 2 x 512 threads (half-length staging rows) 5.53 ms
+constexpr int kBinThreads = 1024;              // CTA size of pass 1 and CTAs per SM.  2 x 512 threads (half-length staging rows, one CTA computing
+constexpr int kBinCtasPerSm = 1;               // while the other is at its flush barrier) measured no better: configs[1] 2.97 against 2.95 ms, configs[2]
+                                               // 6.74 against 6.12 ms per frame -- the barrier stall of the flush is skew, which the slower warps fill
 constexpr int kBinAccThreads = 1024;           // CTA size of pass 2 (one CTA per SM: the tile fills shared memory)
 
 // Hi-Z pre-test of the depth splat (DESIGN "Hi-Z variant").  hz[by * nbx + bx] is an upper bound of

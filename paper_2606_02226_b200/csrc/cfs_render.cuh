@@ -340,7 +340,9 @@ __device__ __forceinline__ uint32_t iterate_block(const RenderParams &prm, const
                                                                        StepCtx{plo, phi, it}, direct_half);
         }
     }
-    if (SPLAT == SPLAT_BIN && ((((uint32_t)it0 >> 2) + 1u) & prm.bin.check_mask) == 0u) {   // CTA-uniform
+    // steady-state blocks are flushed by the caller, between runs of blocks (render_kernel): the run then is a loop
+    // of its own whose invariants -- the Philox round keys above all -- stay in uniform registers
+    if (CHECKED && SPLAT == SPLAT_BIN && ((((uint32_t)it0 >> 2) + 1u) & prm.bin.check_mask) == 0u) {   // CTA-uniform
         __syncthreads();
         bin_flush_units(prm, s, s_hist, br, bl);
         __syncthreads();
@@ -427,9 +429,26 @@ render_kernel(const __grid_constant__ RenderParams prm)
 #pragma unroll 1
             for (; it0 < it_fast0; it0 += 4)
                 dropped += iterate_block<DIM, GEN, AFF, SPLAT, SIG, TRIG, OPT, true>(prm, s, sm, s_hist, plo, phi, it0, gx, gy, gz, have, bl, br);
+            if (SPLAT == SPLAT_BIN) {
+                // runs of blocks up to the next flush boundary (CTA-uniform: every thread of the CTA is at the same it0)
+                const int mask = (int)prm.bin.check_mask;
 #pragma unroll 1
-            for (; it0 < it_fast1; it0 += 4)
-                dropped += iterate_block<DIM, GEN, AFF, SPLAT, SIG, TRIG, OPT, false>(prm, s, sm, s_hist, plo, phi, it0, gx, gy, gz, have, bl, br);
+                while (it0 < it_fast1) {
+                    const int stop = min(it_fast1, (((it0 >> 2) | mask) + 1) << 2);
+#pragma unroll 1
+                    for (; it0 < stop; it0 += 4)
+                        dropped += iterate_block<DIM, GEN, AFF, SPLAT, SIG, TRIG, OPT, false>(prm, s, sm, s_hist, plo, phi, it0, gx, gy, gz, have, bl, br);
+                    if (((it0 >> 2) & mask) == 0) {
+                        __syncthreads();
+                        bin_flush_units(prm, s, s_hist, br, bl);
+                        __syncthreads();
+                    }
+                }
+            } else {
+#pragma unroll 1
+                for (; it0 < it_fast1; it0 += 4)
+                    dropped += iterate_block<DIM, GEN, AFF, SPLAT, SIG, TRIG, OPT, false>(prm, s, sm, s_hist, plo, phi, it0, gx, gy, gz, have, bl, br);
+            }
 #pragma unroll 1
             for (; it0 < I; it0 += 4)
                 dropped += iterate_block<DIM, GEN, AFF, SPLAT, SIG, TRIG, OPT, true>(prm, s, sm, s_hist, plo, phi, it0, gx, gy, gz, have, bl, br);
