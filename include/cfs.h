@@ -231,12 +231,15 @@ cfs_status cfs_binned_plan(int32_t width, int32_t height, int32_t out_mode, int3
  *                    ROTATE_Z resolved to the AFFINE [c -s; s c] (3-D: about z), c = (float)cos(theta), s likewise;
  *                    PINHOLE as (fx, fy, cam_z, near), fy = (float)(1 / tan(fov/2)), fx = (float)(that H / W);
  *                    TWIST_Z / BEND p[0]; SCATTER (D, rx, ry, rz)
+ *   pick_form        how a kernel compiled for this system (CFS_FLAG_JIT) evaluates k = #{j : u >= T_j}: 0 table + walk,
+ *                    1 shift (equal power-of-two thresholds), 2 two compares, 3 table + one compare, 4 one multiply,
+ *                    k = (u n + n - 1) >> 32, taken only when T_j == floor((j + 1) 2^32 / n) for every j
  *   thresholds       T_j of DESIGN R2 (n_thresholds of them lie below 2^32), pal8 the palette packed to rgba8:
  *                    byte = floor(v + 0.5) clamped to [0, 255], NaN -> 0, r | g<<8 | b<<16 | a<<24 (DESIGN R9)
  * Errors: as cfs_render's validation (INVALID_ARG). */
 typedef struct {
     float sx, ox, sy, oy;
-    int32_t n_chain, n_funcs, n_thresholds, pad_;
+    int32_t n_chain, n_funcs, n_thresholds, pick_form;
     int32_t chain_type[CFS_MAX_CHAIN];
     float chain_p[CFS_MAX_CHAIN][12];
     uint32_t thresholds[CFS_MAX_FUNCS];

@@ -58,6 +58,7 @@ enum KernelOpt : int {
     OPT_REUSE = 1,         // Fig. 2(C): the chain output is fed back into the generator (compiled chains; the interpreter reads prm.reuse)
     OPT_PICK_SHIFT = 2,    // equal power-of-two thresholds: k = u >> prm.pick_shift, nothing else compiled in
     OPT_PICK_LUT1 = 4,     // at most one threshold per 2^24 bucket of u: one table read + one compare, no loop
+    OPT_PICK_MULHI = 8,    // equal thresholds T_j = floor((j + 1) 2^32 / n), n not a power of two: k = (u n + n - 1) >> 32 (64-bit product)
     OPT_BIN_RGBA = 16,     // tile bins: records carry the colour index (RGBA + MAP_INDEX); with OPT_BIN_FIXED only
     OPT_BIN_FIXED = 32,    // tile bins: OPT_BIN_RGBA and the direct mask below are the truth (else prm.bin.hybrid / prm.color_rule decide at run time)
     OPT_SYM_BOUNDS = 64,   // xmin == -xmax and ymin == -ymax: the closed-bounds test is |x| <= xmax && |y| <= ymax (two compares)

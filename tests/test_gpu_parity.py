@@ -206,6 +206,27 @@ def test_three_ways_to_run_a_chain_are_bit_identical(cfs, oracle, cfg, fast):
             assert np.array_equal(g, images["interpreter"][0]) and np.array_equal(c, images["interpreter"][1]), k
 
 
+@pytest.mark.parametrize("n", [5, 6, 7, 12, 20, 24])
+def test_map_pick_forms_agree_with_the_oracle(cfs, oracle, n):
+    """n equal maps: the run-time compiled kernel picks the map with one multiply (pick form 4; n = 6, 12, 24 have
+    thresholds that are exact integers, n = 5, 7, 20 none), the linked kernels read the table -- both bit-identical
+    to the oracle's threshold walk (DESIGN R2), picks traced and histograms rendered."""
+    funcs = [W.Func("affine", float(np.float32(1.0 / n)),
+                    [0.45, 0.0, 0.0, 0.45, 0.55 * math.cos(2 * math.pi * k / n), 0.55 * math.sin(2 * math.pi * k / n)]) for k in range(n)]
+    w = W.Workload("pick", W.System(2, "ifs", funcs), W.Render(6007, 31 + n, 96, 8, 160, 120, (-1.1, 1.1, -1.1, 1.1), "hist_u32"))
+    sysh = cfs.cfs_create(w.system)
+    form = cfs.cfs_host_resolve(sysh, cfs.make_args(w.render))["pick_form"]
+    sysh.close()
+    assert form == 4, (n, form)
+    o, oc, _ = oracle.render_parallel(w.system, w.render)
+    tr_ref = gpu_trace(cfs, w, flags=["interpret_chain"])
+    for flags in ([], ["jit"]):
+        g, c = gpu_render(cfs, w, variant="direct", flags=flags)
+        assert np.array_equal(g, o) and np.array_equal(c, oc), (n, flags)
+        for x, y in zip(gpu_trace(cfs, w, flags=flags), tr_ref):
+            assert np.array_equal(x, y), (n, flags)
+
+
 def test_jit_compiles_branch_scatter_reuse_and_the_eq1_generator(cfs, oracle):
     """The NEXT-1 / NEXT-2 systems have no ahead-of-time kernel; CFS_FLAG_JIT compiles their chain in (BRANCH
     structure, SCATTER draws, Fig. 2(C) reuse, the Eq. 1 generator) -- identical to the interpreter and, where

@@ -303,3 +303,60 @@ def test_pinhole_arguments_are_validated(cfs):
             cfs.cfs_host_resolve(sysh, cfs.make_args(r))
         assert ei.value.status == cfs.CFS_ERR_INVALID_ARG
         sysh.close()
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# The map pick as one multiply (pick_form 4 of cfs_host_resolve): k = (u n + n - 1) >> 32 must equal the definition
+# k = #{j : u >= T_j} (DESIGN R2) for EVERY u, with the library's own thresholds.  Checked at every threshold's
+# neighbourhood (the only places the two can part), at both ends of the range and at random u; and the library must
+# not offer the form when a threshold is not floor((j + 1) 2^32 / n).
+def _uniform_system(n, probs=None):
+    funcs = [W.Func("affine", float(np.float32(1.0 / n if probs is None else probs[k])), [0.5, 0.0, 0.0, 0.5, 0.0, 0.0])
+             for k in range(n)]
+    return W.System(dim=2, gen="ifs", funcs=funcs)
+
+
+@pytest.mark.parametrize("n", list(range(3, 65)))
+def test_multiply_pick_equals_the_threshold_count(cfs, n):
+    render = W.config(0).render
+    sysh = cfs.cfs_create(_uniform_system(n))
+    res = cfs.cfs_host_resolve(sysh, cfs.make_args(render))
+    sysh.close()
+    T = res["thresholds"]
+    assert len(T) == n - 1
+    if n & (n - 1) == 0:
+        assert res["pick_form"] == 1            # a power of two takes the shift
+        return
+    if n == 3:
+        assert res["pick_form"] == 2            # two thresholds: two compares
+        return
+    if res["pick_form"] != 4:                   # float32(1/n) summed in double missed an exact threshold: not offered
+        assert any(T[j] != ((j + 1) << 32) // n for j in range(n - 1))
+        return
+    assert all(T[j] == ((j + 1) << 32) // n for j in range(n - 1))
+    rng = np.random.default_rng(n)
+    us = {0, 1, (1 << 32) - 1, (1 << 32) - 2}
+    for t in T:
+        us.update((t - 1, t, t + 1))
+    us.update(int(v) for v in rng.integers(0, 1 << 32, size=2000, dtype=np.uint64))
+    for u in us:
+        want = sum(1 for t in T if u >= t)
+        got = (u * n + n - 1) >> 32
+        assert got == want, (n, u, got, want)
+
+
+def test_multiply_pick_is_not_offered_for_unequal_probabilities(cfs):
+    render = W.config(0).render
+    for probs in ([0.2, 0.2, 0.2, 0.2, 0.1, 0.1], [0.5, 0.25, 0.25], [0.3, 0.3, 0.4]):
+        sysh = cfs.cfs_create(_uniform_system(len(probs), probs))
+        res = cfs.cfs_host_resolve(sysh, cfs.make_args(render))
+        sysh.close()
+        assert res["pick_form"] != 4, probs
+    # configs[4] (20 equal maps) takes it, configs[2] (3 maps) the two compares, configs[0]/[1] (4 maps) the shift
+    forms = {}
+    for i in (0, 1, 2, 4):
+        w = W.config(i)
+        sysh = cfs.cfs_create(w.system)
+        forms[i] = cfs.cfs_host_resolve(sysh, cfs.make_args(w.render))["pick_form"]
+        sysh.close()
+    assert forms == {0: 1, 1: 1, 2: 2, 4: 4}, forms
