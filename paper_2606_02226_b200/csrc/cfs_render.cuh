@@ -319,7 +319,10 @@ __device__ __forceinline__ uint32_t iterate_block(const RenderParams &prm, const
         }
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
-            if (sv[j] && __float_as_uint(Z[j]) <= (uint32_t)(cur[j] >> 32)) {      // else the key is larger whatever its colour
+            // cur = 0 where no load was issued, and a live splat's depth bits are > 0 (d > near >= 0): under OPT_NO_DROP
+            // (every splat proved alive) the depth compare alone tells a candidate, without re-testing `sv`
+            CFS_CHECK((OPT & OPT_NO_DROP) == 0 || __float_as_uint(Z[j]) > 0u);
+            if (((OPT & OPT_NO_DROP) != 0 || sv[j]) && __float_as_uint(Z[j]) <= (uint32_t)(cur[j] >> 32)) {      // else the key is larger whatever its colour
                 const unsigned long long key = ((unsigned long long)__float_as_uint(Z[j]) << 32) | lds_u32(sm.tab + CFS_SM_OFF(pal8) + 4u * (uint32_t)K[j]);
                 if (key < cur[j]) atomicMin(buf + pix[j], key);
             }
