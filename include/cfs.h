@@ -234,6 +234,10 @@ cfs_status cfs_binned_plan(int32_t width, int32_t height, int32_t out_mode, int3
  *   pick_form        how a kernel compiled for this system (CFS_FLAG_JIT) evaluates k = #{j : u >= T_j}: 0 table + walk,
  *                    1 shift (equal power-of-two thresholds), 2 two compares, 3 table + one compare, 4 one multiply,
  *                    k = (u n + n - 1) >> 32, taken only when T_j == floor((j + 1) 2^32 / n) for every j
+ *   proved           what the host has PROVED about this render and compiles into a CFS_FLAG_JIT kernel as a dropped test
+ *                    (bounded attractor pushed through the chain, DESIGN "proved options"): bit 0 = every PINHOLE
+ *                    depth is a normal float (the reciprocal's short sequence is the correctly rounded one), bit 1 =
+ *                    every splat is alive and lands strictly inside the image (no bounds test, no drop count, no clamp)
  *   thresholds       T_j of DESIGN R2 (n_thresholds of them lie below 2^32), pal8 the palette packed to rgba8:
  *                    byte = floor(v + 0.5) clamped to [0, 255], NaN -> 0, r | g<<8 | b<<16 | a<<24 (DESIGN R9)
  * Errors: as cfs_render's validation (INVALID_ARG). */
@@ -244,6 +248,7 @@ typedef struct {
     float chain_p[CFS_MAX_CHAIN][12];
     uint32_t thresholds[CFS_MAX_FUNCS];
     uint32_t pal8[CFS_MAX_FUNCS];
+    int32_t proved, pad_;
 } cfs_resolved;
 cfs_status cfs_host_resolve(const cfs_system *sys, const cfs_render_args *args, cfs_resolved *out);
 

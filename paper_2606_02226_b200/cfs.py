@@ -60,7 +60,8 @@ class cfs_resolved(C.Structure):
     _fields_ = [("sx", C.c_float), ("ox", C.c_float), ("sy", C.c_float), ("oy", C.c_float),
                 ("n_chain", C.c_int32), ("n_funcs", C.c_int32), ("n_thresholds", C.c_int32), ("pick_form", C.c_int32),
                 ("chain_type", C.c_int32 * 8), ("chain_p", (C.c_float * 12) * 8),
-                ("thresholds", C.c_uint32 * 64), ("pal8", C.c_uint32 * 64)]
+                ("thresholds", C.c_uint32 * 64), ("pal8", C.c_uint32 * 64),
+                ("proved", C.c_int32), ("pad_", C.c_int32)]
 
 
 _lib = None
@@ -261,7 +262,7 @@ def cfs_host_resolve(sys: System, args: cfs_render_args) -> dict:
     return {"sx": float(out.sx), "ox": float(out.ox), "sy": float(out.sy), "oy": float(out.oy),
             "chain_type": [int(out.chain_type[m]) for m in range(n)],
             "chain_p": [np.array(list(out.chain_p[m]), dtype=np.float32) for m in range(n)],
-            "pick_form": int(out.pick_form),
+            "pick_form": int(out.pick_form), "proved": int(out.proved),
             "thresholds": [int(out.thresholds[j]) for j in range(int(out.n_thresholds))],
             "pal8": [int(out.pal8[j]) for j in range(int(out.n_funcs))]}
 

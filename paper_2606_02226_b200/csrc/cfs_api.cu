@@ -1220,6 +1220,7 @@ extern "C" cfs_status cfs_host_resolve(const cfs_system *s, const cfs_render_arg
     }
     out->n_funcs = p.n_funcs;
     out->n_thresholds = p.n_thr;
+    { const int po = proved_options(s, p); out->proved = ((po & cfs::OPT_RCP_NORMAL) ? 1 : 0) | ((po & cfs::OPT_NO_DROP) ? 2 : 0); }
     out->pick_form = (s->gen != CFS_GEN_IFS) ? 0 : (p.pick_shift >= 0) ? 1 : (p.n_thr == 2) ? 2 : s->pick_mulhi ? 4 : (p.pick_steps <= 1) ? 3 : 0;
     memcpy(out->thresholds, p.T, sizeof(out->thresholds));
     memcpy(out->pal8, p.pal8, sizeof(out->pal8));

@@ -227,6 +227,75 @@ def test_map_pick_forms_agree_with_the_oracle(cfs, oracle, n):
             assert np.array_equal(x, y), (n, flags)
 
 
+def _random_system(rng, dim):
+    """A random IFS of affine contractions with a random chain and random image bounds (sometimes generous enough for
+    the host to prove "no splat is dropped", sometimes not)."""
+    n = int(rng.integers(2, 8))
+    probs = rng.uniform(0.5, 1.5, n) if rng.random() < 0.5 else np.ones(n)
+    probs = probs / probs.sum()
+    funcs = []
+    for k in range(n):
+        if dim == 2:
+            sc, th = rng.uniform(0.2, 0.6), rng.uniform(0, 2 * math.pi)
+            A = sc * np.array([[math.cos(th), -math.sin(th)], [math.sin(th), math.cos(th)]])
+            if rng.random() < 0.3:
+                A = np.diag(rng.uniform(0.2, 0.7, 2))
+        else:
+            A = np.diag(rng.uniform(0.2, 0.6, 3)) + rng.uniform(-0.1, 0.1, (3, 3))
+        b = rng.uniform(-0.6, 0.6, dim)
+        funcs.append(W.Func("affine", float(np.float32(probs[k])), [float(v) for v in A.ravel()] + [float(v) for v in b]))
+    chain = []
+    for _ in range(int(rng.integers(0, 4))):
+        if dim == 2:
+            kind = rng.choice(["affine", "swirl", "sinusoidal", "stretch_cos", "scatter"])
+        else:
+            kind = rng.choice(["affine", "twist_z", "bend", "scatter"])
+        if kind == "affine":
+            M = rng.uniform(-0.7, 0.7, (dim, dim)) + np.eye(dim) * rng.uniform(0.3, 0.9)
+            chain.append(W.Xform("affine", [float(v) for v in M.ravel()] + [float(v) for v in rng.uniform(-0.3, 0.3, dim)]))
+        elif kind in ("twist_z", "bend"):
+            chain.append(W.Xform(kind, [float(rng.uniform(-3.0, 3.0))]))
+        elif kind == "scatter":
+            chain.append(W.Xform("scatter", [int(rng.integers(2, 40)), float(rng.uniform(0, 0.5)), float(rng.uniform(0, 0.5)),
+                                             float(rng.uniform(0, 0.5)) if dim == 3 else 0.0]))
+        else:
+            chain.append(W.Xform(kind))
+    if dim == 3:
+        chain.append(W.Xform("pinhole", [float(rng.uniform(40, 85)), -float(rng.uniform(2.0, 9.0)), float(rng.choice([1e-3, 0.1, 1.0]))]))
+    half = float(rng.choice([0.6, 1.2, 2.5, 6.0]))
+    bounds = (-half, half, -half * 0.75, half * 0.75) if rng.random() < 0.7 else (-half, half * 0.5, -half * 0.3, half)
+    out = "hist_u32" if dim == 2 else "depth_u64"
+    color, pal = ("none", None) if dim == 2 else ("map_index", W.palette_for(n))
+    return W.Workload("random", W.System(dim, "ifs", funcs, chain, color, pal),
+                      W.Render(int(rng.integers(1500, 4000)), int(rng.integers(1, 1 << 30)), 64, 8, 200, 150, bounds, out))
+
+
+def test_proved_options_are_sound_on_random_systems(cfs):
+    """What the host proves about a render (bounded attractor pushed through the chain: "every depth is a normal float",
+    "no splat is dropped") is compiled into the run-time specialised kernel as a DROPPED test.  On random systems the
+    specialised kernel must give the interpreter's image and counters to the last bit, whether the proof succeeded or
+    not -- an unsound proof shows as a splat that should have been dropped (or a clamp that should have bound)."""
+    rng = np.random.default_rng(20261105)
+    proved = {0: 0, 1: 0, 2: 0, 3: 0}
+    for i in range(36):
+        w = _random_system(rng, 2 if i % 2 == 0 else 3)
+        sysh = cfs.cfs_create(w.system)
+        proved[cfs.cfs_host_resolve(sysh, cfs.make_args(w.render))["proved"]] += 1
+        sysh.close()
+        ref, cref = gpu_render(cfs, w, variant="direct", flags=["interpret_chain"])
+        g, c = gpu_render(cfs, w, variant="direct", flags=["jit"])
+        assert np.array_equal(g, ref) and np.array_equal(c, cref), (i, w.system.chain, w.render.bounds)
+        if w.system.dim == 2:
+            g, c = gpu_render(cfs, w, variant="binned", flags=["jit", "bin_hybrid"])
+            assert np.array_equal(g, ref) and np.array_equal(c, cref), (i, "bins", w.system.chain, w.render.bounds)
+        else:
+            g, c = gpu_render(cfs, w, variant="depth_hiz", flags=["jit"],
+                              scratch_bytes=cfs.cfs_hiz_scratch_bytes(w.render.width, w.render.height))
+            assert np.array_equal(g, ref) and np.array_equal(c, cref), (i, "hiz", w.system.chain, w.render.bounds)
+    # both outcomes of the proof were exercised
+    assert proved[2] + proved[3] >= 5 and proved[0] + proved[1] >= 5, proved
+
+
 def test_jit_compiles_branch_scatter_reuse_and_the_eq1_generator(cfs, oracle):
     """The NEXT-1 / NEXT-2 systems have no ahead-of-time kernel; CFS_FLAG_JIT compiles their chain in (BRANCH
     structure, SCATTER draws, Fig. 2(C) reuse, the Eq. 1 generator) -- identical to the interpreter and, where
