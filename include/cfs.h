@@ -215,6 +215,26 @@ uint64_t cfs_binned_scratch_bytes(const cfs_system *sys, const cfs_render_args *
  * instruction issue -- level as linked ahead of time, ahead when compiled for the system (CFS_FLAG_JIT). */
 uint64_t cfs_hiz_scratch_bytes(int32_t width, int32_t height);
 
+/* cfs_render_depth_noalloc -- the Hi-Z depth render (CFS_VARIANT_DEPTH_HIZ) for callers that cannot allocate device
+ * memory (code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc): its scratch -- the
+ * Hi-Z map -- lives in a file-scope `static __device__` array of CFS_NOALLOC_SCRATCH_BYTES inside the library, which
+ * every GPU that loads the library holds until the process exits.  The call allocates nothing: no cudaMalloc /
+ * cudaFree, no run-time compilation or module load (CFS_FLAG_JIT and $CFS_FORCE_JIT are refused: INVALID_ARG; the
+ * kernels are the ones linked ahead of time), only a memset of the map and kernel launches on `cuda_stream`.
+ *   args  as for cfs_render: d_image (u64[width*height], cleared to 2^64 - 1 by the caller), d_counters (optional),
+ *         n_points, point_offset, ...; out_mode must be CFS_OUT_DEPTH_RGBA8_U64 and the system an IFS (UNSUPPORTED
+ *         otherwise); variant, d_scratch and scratch_bytes are IGNORED.
+ *   limit cfs_hiz_scratch_bytes(width, height) must be non-zero and <= CFS_NOALLOC_SCRATCH_BYTES -- i.e. at most
+ *         49152 blocks of 32 x 32 pixels, e.g. up to 7000 x 7000 -- else INVALID_ARG with both numbers in
+ *         cfs_last_error().
+ *   result identical, pixel for pixel and in the counters, to cfs_render with CFS_VARIANT_DEPTH_HIZ (and DIRECT).
+ * The array is SHARED by every call on a device and keeps the last call's contents; the call clears what it reads
+ * (the map is reset to "nothing culled" first), so a stale map cannot leak into a render -- but two calls that
+ * overlap on the GPU (different streams, no dependency) RACE on it: serialise them.  The first call on a device
+ * resolves the array's device address (cudaGetSymbolAddress) and lets CUDA load the kernels; make it before capture. */
+#define CFS_NOALLOC_SCRATCH_BYTES (96 * 1024 + 256)
+cfs_status cfs_render_depth_noalloc(const cfs_system *sys, const cfs_render_args *args, void *cuda_stream);
+
 /* the tile plan of the BINNED variant for an image and a device shape, host arithmetic only (no device
  * needed; test instrument): out = { tiles, pixels per tile, magic, shift (tile of pixel p =
  * mulhi32(p, magic) >> shift), colour slots per pixel, staging records per tile, flush-check interval in

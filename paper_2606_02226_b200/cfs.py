@@ -26,7 +26,7 @@ FLAGS = {"fast_trig": 1, "interpret_chain": 2, "bin_pass1_only": 4, "jit": 8, "b
 VARIANT = {"auto": 0, "direct": 1, "shared_hist": 2, "warp_agg": 3, "binned": 4, "cluster_hist": 5, "depth_hiz": 6}
 MB = {"red_add_u32": 0, "red_add_v4f32": 1, "atom_min_u64": 2, "ld_u64": 3, "atoms_add_u32": 4,
       "ffma": 5, "imad_wide": 6, "lop3": 7, "mufu": 8, "stream_ld128": 9, "stream_red_v4f32": 10}
-EXPORTS = ["cfs_create", "cfs_destroy", "cfs_render", "cfs_render_host", "cfs_render_rgba8_host", "cfs_tonemap", "cfs_resolve_rgba8", "cfs_trace",
+EXPORTS = ["cfs_create", "cfs_destroy", "cfs_render", "cfs_render_host", "cfs_render_depth_noalloc", "cfs_render_rgba8_host", "cfs_tonemap", "cfs_resolve_rgba8", "cfs_trace",
            "cfs_microbench", "cfs_host_resolve", "cfs_specialize", "cfs_jit_check", "cfs_jit_stats", "cfs_shared_hist_max_bytes", "cfs_binned_scratch_bytes", "cfs_hiz_scratch_bytes", "cfs_binned_plan", "cfs_launch_count", "cfs_last_error",
            "cfs_version"]
 
@@ -114,6 +114,8 @@ def lib():
         L.cfs_binned_scratch_bytes.restype = C.c_uint64
         L.cfs_hiz_scratch_bytes.argtypes = [C.c_int32, C.c_int32]
         L.cfs_hiz_scratch_bytes.restype = C.c_uint64
+        L.cfs_render_depth_noalloc.argtypes = [C.c_void_p, C.POINTER(cfs_render_args), C.c_void_p]
+        L.cfs_render_depth_noalloc.restype = C.c_int
         L.cfs_binned_plan.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32,
                                       C.POINTER(C.c_uint32)]
         L.cfs_binned_plan.restype = C.c_int
@@ -291,6 +293,15 @@ def cfs_jit_stats():
 
 def cfs_render(sys: System, args: cfs_render_args, stream=None) -> None:
     _check(lib().cfs_render(sys.handle, C.byref(args), _stream(stream)))
+
+
+NOALLOC_SCRATCH_BYTES = 96 * 1024 + 256      # CFS_NOALLOC_SCRATCH_BYTES of include/cfs.h
+
+
+def cfs_render_depth_noalloc(sys: System, args: cfs_render_args, stream=None) -> None:
+    """The Hi-Z depth render with its scratch inside the library (a static device array): allocates nothing.
+    DEPTH output of an IFS only; args.variant / d_scratch are ignored; calls that overlap on the GPU race."""
+    _check(lib().cfs_render_depth_noalloc(sys.handle, C.byref(args), _stream(stream)))
 
 
 def cfs_render_host(sys: System, args: cfs_render_args, h_image: np.ndarray, h_cloud: Optional[np.ndarray] = None,

@@ -1444,3 +1444,60 @@ extern "C" uint64_t cfs_launch_count(int32_t reset)
 
 extern "C" const char *cfs_last_error(void) { return g_err; }
 extern "C" const char *cfs_version(void) { return "cfs-b200 0.1 (sm_100a)"; }
+
+// ---- cfs_render_depth_noalloc: the Hi-Z depth render with its scratch inside the library ---------------------------
+// For callers that cannot allocate device memory (include/cfs.h has the contract).  The Hi-Z map lives in this
+// file-scope device array, which every GPU that loads the library holds until the process exits.  In HOST code the
+// name below is a host-side stand-in for the symbol, NOT a device address: a kernel handed `g_noalloc_scratch`
+// itself would fault (or, where the GPU can reach host memory, quietly use the wrong bytes).  The device address
+// is resolved with cudaGetSymbolAddress, once per device, with that device current, and only that pointer is
+// passed on.  Every call on a device shares the array; render_depth_hiz resets the map before it reads it, so the
+// last call's contents never reach a render -- but calls that overlap on the GPU race on it.
+static __device__ __align__(256) unsigned char g_noalloc_scratch[CFS_NOALLOC_SCRATCH_BYTES];
+static_assert(CFS_NOALLOC_SCRATCH_BYTES >= cfs::kHizMaxBytes + 256, "the built-in scratch must hold the largest Hi-Z map plus its alignment slack");
+
+namespace {
+
+std::mutex g_noalloc_mutex;
+void *g_noalloc_ptr[kMaxDevices];       // device address of g_noalloc_scratch per device ordinal; nullptr = not resolved yet
+
+cfs_status noalloc_scratch(void **out)
+{
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaGetDevice");
+    if (dev < 0 || dev >= kMaxDevices) return fail(CFS_ERR_UNSUPPORTED, "device ordinal %d beyond %d", dev, kMaxDevices);
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    if (!g_noalloc_ptr[dev]) {
+        void *ptr = nullptr;
+        e = cudaGetSymbolAddress(&ptr, g_noalloc_scratch);      // the address on the CURRENT device
+        if (e != cudaSuccess) return cuda_fail(e, "cudaGetSymbolAddress(built-in scratch)");
+        if (!ptr || ((uintptr_t)ptr & 255u) != 0) return fail(CFS_ERR_CUDA, "built-in scratch resolved to a bad address %p", ptr);
+        g_noalloc_ptr[dev] = ptr;
+    }
+    *out = g_noalloc_ptr[dev];
+    return CFS_OK;
+}
+
+}  // namespace
+
+extern "C" cfs_status cfs_render_depth_noalloc(const cfs_system *s, const cfs_render_args *a, void *stream)
+{
+    if (!s || !a) return fail(CFS_ERR_INVALID_ARG, "system or args is NULL");
+    if (wants_jit(a->flags))
+        return fail(CFS_ERR_INVALID_ARG, "cfs_render_depth_noalloc allocates nothing: CFS_FLAG_JIT / $CFS_FORCE_JIT compile and load a module, use cfs_render for that");
+    if (a->width >= 1 && a->height >= 1) {          // (a bad size is reported by the render's own validation below)
+        const uint64_t need = cfs_hiz_scratch_bytes(a->width, a->height);
+        if (need == 0 || need > (uint64_t)CFS_NOALLOC_SCRATCH_BYTES)
+            return fail(CFS_ERR_INVALID_ARG, "image %d x %d needs %llu bytes of Hi-Z scratch (0 = more than 49152 blocks of 32 x 32 pixels); the built-in scratch holds %d",
+                        a->width, a->height, (unsigned long long)need, (int)CFS_NOALLOC_SCRATCH_BYTES);
+    }
+    void *scratch = nullptr;
+    cfs_status st = noalloc_scratch(&scratch);
+    if (st != CFS_OK) return st;
+    cfs_render_args r = *a;
+    r.variant = CFS_VARIANT_DEPTH_HIZ;              // refuses anything but DEPTH output of an IFS (UNSUPPORTED)
+    r.d_scratch = scratch;
+    r.scratch_bytes = CFS_NOALLOC_SCRATCH_BYTES;
+    return render_impl(s, &r, stream, 0);
+}
