@@ -242,16 +242,24 @@ std::string cache_path(const std::string &name)
     return std::string(dir) + buf;
 }
 
-// disk cache file: u32 length of the lowered name, the name, the cubin
+// disk cache file: "CFSJ", u32 length of the lowered name, u64 cubin bytes, u64 FNV-1a of the cubin, the name, the cubin.
+// The driver loads a module from memory without a length, so a truncated or damaged image must be caught HERE: a file
+// whose sizes or checksum do not match is ignored (and rewritten after the compile).
+constexpr uint32_t kDiskMagic = 0x4A534643u;    // "CFSJ"
+struct DiskHeader { uint32_t magic, name_len; uint64_t cubin_bytes, cubin_hash; };
+
 bool disk_load(const std::string &path, std::vector<char> *cubin, std::string *lowered)
 {
     std::string all;
-    if (path.empty() || !read_file(path, &all) || all.size() < 8) return false;
-    uint32_t n = 0;
-    memcpy(&n, all.data(), 4);
-    if (n == 0 || (size_t)n + 4 >= all.size()) return false;
-    lowered->assign(all.data() + 4, n);
-    cubin->assign(all.begin() + 4 + n, all.end());
+    if (path.empty() || !read_file(path, &all) || all.size() < sizeof(DiskHeader)) return false;
+    DiskHeader h;
+    memcpy(&h, all.data(), sizeof(h));
+    if (h.magic != kDiskMagic || h.name_len == 0 || h.cubin_bytes == 0) return false;
+    if ((uint64_t)all.size() != sizeof(h) + (uint64_t)h.name_len + h.cubin_bytes) return false;
+    const char *body = all.data() + sizeof(h) + h.name_len;
+    if (fnv1a(body, (size_t)h.cubin_bytes, 0xcbf29ce484222325ull) != h.cubin_hash) return false;
+    lowered->assign(all.data() + sizeof(h), h.name_len);
+    cubin->assign(body, body + h.cubin_bytes);
     return true;
 }
 
@@ -263,8 +271,11 @@ void disk_store(const std::string &path, const std::vector<char> &cubin, const s
     const std::string tmp = path + ".tmp" + std::to_string((long)getpid());
     FILE *f = fopen(tmp.c_str(), "wb");
     if (!f) return;
-    const uint32_t n = (uint32_t)lowered.size();
-    const bool ok = fwrite(&n, 4, 1, f) == 1 && fwrite(lowered.data(), 1, n, f) == n && fwrite(cubin.data(), 1, cubin.size(), f) == cubin.size();
+    DiskHeader h;
+    h.magic = kDiskMagic; h.name_len = (uint32_t)lowered.size(); h.cubin_bytes = cubin.size();
+    h.cubin_hash = fnv1a(cubin.data(), cubin.size(), 0xcbf29ce484222325ull);
+    const bool ok = fwrite(&h, sizeof(h), 1, f) == 1 && fwrite(lowered.data(), 1, h.name_len, f) == h.name_len &&
+                    fwrite(cubin.data(), 1, cubin.size(), f) == cubin.size();
     fclose(f);
     if (ok) rename(tmp.c_str(), path.c_str());
     else unlink(tmp.c_str());

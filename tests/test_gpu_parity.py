@@ -1152,3 +1152,49 @@ def test_device_bounds_checks(cfs, selftest):
     else:
         assert p.returncode == 0, p.stdout[-2000:] + p.stderr[-4000:]
         assert "checked renders ok" in p.stdout and not p.stdout.strip().endswith(": 0")
+
+
+_CACHED_RENDER = """
+import sys, hashlib, numpy as np, torch
+sys.path.insert(0, %(root)r)
+from paper_2606_02226_b200 import cfs, workloads as W
+from tests._gpu_util import gpu_render
+cfs.lib()
+w = W.config(1).scaled(n_points=20011, iterations=60, width=200, height=160)
+g, c = gpu_render(cfs, w, variant="direct", flags=["jit", "fast_trig"])
+n, ms = cfs.cfs_jit_stats()
+print("RESULT", n, hashlib.sha256(g.tobytes()).hexdigest(), int(c[0]))
+"""
+
+
+def test_run_time_kernels_survive_processes_through_the_disk_cache(cfs, tmp_path):
+    """$CFS_JIT_CACHE: a kernel compiled for a system by one process is loaded, not compiled, by the next one (the
+    paper's own measurement has compilation at 35 x the frame time), keyed by kernel name and a hash of
+    the embedded sources; a damaged cache file is compiled afresh and replaced.  Same image every time."""
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = dict(os.environ, CFS_JIT_CACHE=str(tmp_path))
+    env.pop("CFS_FORCE_JIT", None)
+
+    def run():
+        p = subprocess.run([sys.executable, "-c", _CACHED_RENDER % {"root": root}], env=env, capture_output=True, text=True, timeout=600)
+        assert p.returncode == 0, p.stdout[-2000:] + p.stderr[-4000:]
+        line = [ln for ln in p.stdout.splitlines() if ln.startswith("RESULT")][-1].split()
+        return int(line[1]), line[2], int(line[3])
+
+    n1, h1, c1 = run()
+    files = sorted(os.listdir(tmp_path))
+    assert n1 == 1 and len(files) == 1, (n1, files)
+    n2, h2, c2 = run()
+    assert n2 == 0 and (h2, c2) == (h1, c1), "the second process compiled again or rendered something else"
+    path = os.path.join(tmp_path, files[0])
+    blob = bytearray(open(path, "rb").read())
+    for i in range(len(blob) // 2, len(blob) // 2 + 64):
+        blob[i] ^= 0x5A
+    open(path, "wb").write(bytes(blob[: len(blob) - 100]))       # damaged and truncated
+    n3, h3, c3 = run()
+    assert (h3, c3) == (h1, c1), "a damaged cache file changed the render"
+    n4, h4, c4 = run()
+    assert n3 == 1 and n4 == 0 and (h4, c4) == (h1, c1), (n3, n4)
