@@ -574,6 +574,8 @@ int jit_options(const cfs_system *s, const RenderParams &p, int splat)
     if (splat == cfs::SPLAT_BIN) {
         opt |= cfs::OPT_BIN_FIXED | ((int)(p.bin.hybrid & 15u) << cfs::OPT_BIN_MASK_SHIFT);
         if (p.color_rule != 0) opt |= cfs::OPT_BIN_RGBA;
+        // every chunk of this render is a whole number of pass-1 CTAs (bin_layout cuts chunks at multiples of kBinThreads)
+        if (p.n_points > 0 && p.n_points % (uint64_t)cfs::kBinThreads == 0) opt |= cfs::OPT_ALL_HAVE;
     }
     return opt;
 }
@@ -818,6 +820,7 @@ bool bin_layout(BinPlan *pl, void *scratch, uint64_t bytes, uint64_t n_points, u
     if (cp < cfs::kBinThreads) { *why = "scratch too small for one CTA of points"; return false; }
     if (cp >= n_points) cp = n_points;                          // everything in one chunk
     else if (cp >= wave) cp = cp / wave * wave;                 // whole waves: no ragged trip inside a chunk
+    else cp = cp / cfs::kBinThreads * cfs::kBinThreads;         // whole CTAs: only the render's last chunk can be ragged (OPT_ALL_HAVE)
     pl->chunk_points = cp;
     return true;
 }

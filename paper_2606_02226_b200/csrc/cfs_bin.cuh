@@ -51,7 +51,7 @@ __device__ __forceinline__ void bin_direct(const RenderParams &prm, const Shared
         bin_red_add_u32(reinterpret_cast<uint32_t *>(prm.image) + pix, 1u);
     } else {
         const float4 c = s.palette[rec / prm.bin.tile_pixels];
-        bin_red_add_v4_f32(reinterpret_cast<float *>(prm.image) + 4 * (size_t)pix, c.x, c.y, c.z, 1.0f);
+        bin_red_add_v4_f32(reinterpret_cast<float *>(prm.image) + 4 * (size_t)pix, c.x, c.y, c.z, c.w);   // c.w = 1 (load_tables)
     }
 }
 
@@ -125,21 +125,25 @@ __device__ __forceinline__ void bin_append(const RenderParams &prm, const Shared
     else bin_direct(prm, s, tile, rec);
 }
 
-// The same as straight-line code: a dropped splat takes its slot from the lane's dummy counter, which always reads
-// "full", so the store is predicated on the slot alone.  Returns true when the record was stored; false means
-// "row full" -- a live record then has to go down the direct path (rare; the caller does that afterwards and tells
-// live from dropped by `ok`).
-__device__ __forceinline__ bool bin_try_append(const BinRegs &br, bool ok, uint32_t tile, uint32_t rec)
+// The same as straight-line code, in two halves (the caller issues the atomics of a whole Philox block before the
+// first store, so their latencies overlap).  A dropped splat takes its slot from the lane's dummy counter, which always
+// reads "full", so the store is predicated on the slot alone.  bin_store_record returns true when the record was stored;
+// false means "row full" -- a live record then has to go down the direct path (rare; the caller does that afterwards
+// and tells live from dropped by `ok`).
+__device__ __forceinline__ uint32_t bin_take_slot(const BinRegs &br, bool ok, uint32_t tile, uint32_t rec)
 {
     const uint32_t t_eff = ok ? tile : br.dummy;
     CFS_CHECK(tile <= br.dummy - (threadIdx.x & 31u) - 1u && rec <= 49152u && rec < (br.ktp ? 65536u : br.tp));
     uint32_t slot;
     asm volatile("atom.shared.add.u32 %0, [%1], 1;" : "=r"(slot) : "r"(br.cnt_addr + 4u * t_eff) : "memory");
+    return slot;
+}
+__device__ __forceinline__ bool bin_store_record(const BinRegs &br, uint32_t tile, uint32_t rec, uint32_t slot)
+{
     const bool fits = slot < br.cap;
     if (fits) asm volatile("st.shared.u16 [%0], %1;" :: "r"(br.buf_addr + tile * br.row_bytes + 2u * slot), "h"((uint16_t)rec) : "memory");
     return fits;
 }
-
 // Per-lane bin state of pass 1, kept in REGISTERS: lane l of warp w owns tile l * warps + w (so
 // n_tiles <= 32 * warps per CTA, and the rows to flush are spread over all warps of the CTA).  `next` is a pool block taken ahead of time: the global atomic
 // that hands it out is issued when the previous block is opened and its result is not needed

@@ -67,6 +67,8 @@ enum KernelOpt : int {
                            // 1/d is the four-instruction normal-range sequence of the correctly rounded reciprocal, without its range test
     OPT_NO_DROP = 8192,    // the host has PROVED (same bound, with a margin against rounding) that every splat is alive and inside the image
                            // bounds: no near test, no bounds test, nothing to count as dropped
+    OPT_ALL_HAVE = 16384,  // tile bins: every chunk of the render is a whole number of CTAs (n_points a multiple of kBinThreads), so no
+                           // thread of pass 1 is ever without a point: no `have` predicate, select or dummy counter in the append
     OPT_BIN_MASK_SHIFT = 8 // bits 8..11, with OPT_BIN_FIXED: iteration j of a steady-state block splats straight to L2 when bit j is set
 };
 // true when the signature holds a BRANCH separator (type 8): one-to-many splatting

@@ -162,7 +162,7 @@ __device__ __forceinline__ uint32_t splat_q(const RenderParams &prm, const Share
                            (float)((point_rgba8 >> 16) & 0xFFu), 1.0f);
         } else {          // colour of the map applied in this iteration
             const float4 c = lds_v4(sm.tab + CFS_SM_OFF(palette) + 16u * (uint32_t)k);
-            red_add_v4_f32(dst, c.x, c.y, c.z, 1.0f);
+            red_add_v4_f32(dst, c.x, c.y, c.z, c.w);                    // c.w = 1 (load_tables)
         }
     } else if (SPLAT == SPLAT_DEPTH) {
         splat_depth(reinterpret_cast<unsigned long long *>(prm.image), pix, qz,
@@ -173,7 +173,7 @@ __device__ __forceinline__ uint32_t splat_q(const RenderParams &prm, const Share
                 red_add_u32(reinterpret_cast<uint32_t *>(prm.image) + pix, 1u);
             } else {
                 const float4 c = lds_v4(sm.tab + CFS_SM_OFF(palette) + 16u * (uint32_t)k);
-                red_add_v4_f32(reinterpret_cast<float *>(prm.image) + 4 * (size_t)pix, c.x, c.y, c.z, 1.0f);
+                red_add_v4_f32(reinterpret_cast<float *>(prm.image) + 4 * (size_t)pix, c.x, c.y, c.z, c.w);
             }
         } else {
             bin_append(prm, s, br, pix, k);
@@ -189,41 +189,64 @@ __device__ __forceinline__ uint32_t splat_q(const RenderParams &prm, const Share
 // for record + append, and pass 2 halves).  Any split is a correct result: HIST sums are exact,
 // RGBA sums are order-free (DESIGN R8).  Straight-line code: every reduction, atomic and store is predicated.
 // Returns the number of dropped splats.
-template <int DIRECT_MASK, bool RGBA, bool UNCLAMPED = false>
+template <int DIRECT_MASK, bool RGBA, bool UNCLAMPED = false, bool ALL_HAVE = false>
 __device__ __forceinline__ uint32_t bin_block_splat(const RenderParams &prm, const SharedTables &s, const Sm &sm, const BinRegs &br,
                                                     const float (&X)[4], const float (&Y)[4], const int (&K)[4],
                                                     const bool (&ok)[4])
 {
-    uint32_t tile[4], rec[4];
-    bool fine[4];
+    // In stages, so that the shared-memory atomics of the block are in flight TOGETHER: as one loop (record ->
+    // atomic -> store per splat) every store waited for its own atomic in turn, 7 % of the stall samples of pass 1
+    // (short scoreboard at the slot compare, profiles/r02 source view).  The asm statements are volatile, so their
+    // order here is their order in the kernel: reductions, then the atomics, then the stores.
+    // UNCLAMPED = OPT_NO_DROP: `ok` is `have` (nothing to count: the caller counts a thread without a point as
+    // nothing); ALL_HAVE: every thread has a point, so `ok` is true and every predicate below folds away.
+    int pix[4];
+    uint32_t tile[4] = {0u, 0u, 0u, 0u}, rec[4] = {0u, 0u, 0u, 0u}, slot[4] = {0u, 0u, 0u, 0u};
     uint32_t dropped = 0u;
 #pragma unroll
     for (int j = 0; j < 4; ++j) {      // out-of-bounds coordinates are clamped by the pixel rule: always a valid tile
-        const int pix = bin_pixel_of<UNCLAMPED>(br, X[j], Y[j]);
-        CFS_CHECK((uint32_t)pix < (uint32_t)prm.W * (uint32_t)prm.H);
-        fine[j] = true;
-        if (!ok[j]) ++dropped;         // counted here, so that no `ok` outlives its splat
-        if ((DIRECT_MASK >> j) & 1) {  // straight to L2: one predicated reduction, no branch
-            if (RGBA) {
-                const float4 c = lds_v4(sm.tab + CFS_SM_OFF(palette) + 16u * (uint32_t)K[j]);
-                float *dst = reinterpret_cast<float *>(prm.image) + 4 * (size_t)(uint32_t)pix;
-                asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %4, 0;\n\t"
-                             "@p red.global.add.v4.f32 [%0], {%1, %2, %3, 0f3F800000};\n\t}"
-                             :: "l"(dst), "f"(c.x), "f"(c.y), "f"(c.z), "r"((uint32_t)ok[j]) : "memory");
-            } else {
-                uint32_t *dst = reinterpret_cast<uint32_t *>(prm.image) + (uint32_t)pix;
+        pix[j] = bin_pixel_of<UNCLAMPED>(br, X[j], Y[j]);
+        CFS_CHECK((uint32_t)pix[j] < (uint32_t)prm.W * (uint32_t)prm.H);
+        CFS_CHECK(!ALL_HAVE || ok[j]);
+        if (!UNCLAMPED && !ok[j]) ++dropped;   // counted here, so that no `ok` outlives its splat
+    }
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        if (!((DIRECT_MASK >> j) & 1)) continue;   // straight to L2: one predicated reduction, no branch
+        if (RGBA) {
+            const float4 c = lds_v4(sm.tab + CFS_SM_OFF(palette) + 16u * (uint32_t)K[j]);     // (r, g, b, 1): load_tables
+            float *dst = reinterpret_cast<float *>(prm.image) + 4 * (size_t)(uint32_t)pix[j];
+            if (ALL_HAVE)
+                asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" :: "l"(dst), "f"(c.x), "f"(c.y), "f"(c.z), "f"(c.w) : "memory");
+            else
+                asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %5, 0;\n\t"
+                             "@p red.global.add.v4.f32 [%0], {%1, %2, %3, %4};\n\t}"
+                             :: "l"(dst), "f"(c.x), "f"(c.y), "f"(c.z), "f"(c.w), "r"((uint32_t)ok[j]) : "memory");
+        } else {
+            uint32_t *dst = reinterpret_cast<uint32_t *>(prm.image) + (uint32_t)pix[j];
+            if (ALL_HAVE)
+                asm volatile("red.global.add.u32 [%0], 1;" :: "l"(dst) : "memory");
+            else
                 asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %1, 0;\n\t@p red.global.add.u32 [%0], 1;\n\t}"
                              :: "l"(dst), "r"((uint32_t)ok[j]) : "memory");
-            }
-        } else {
-            bin_record_of(br, pix, RGBA ? K[j] : 0, tile[j], rec[j]);
-            fine[j] = bin_try_append(br, ok[j], tile[j], rec[j]);
         }
     }
-    if (!(fine[0] && fine[1] && fine[2] && fine[3])) {   // a staging row was full (or a splat was dropped): live records take the direct path
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {      // a slot in the staging row of the tile (a dropped splat: in the lane's dummy row, "full")
+        if ((DIRECT_MASK >> j) & 1) continue;
+        bin_record_of(br, pix[j], RGBA ? K[j] : 0, tile[j], rec[j]);
+        slot[j] = bin_take_slot(br, ALL_HAVE || ok[j], tile[j], rec[j]);
+    }
+    bool fine = true;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        if ((DIRECT_MASK >> j) & 1) continue;
+        fine &= bin_store_record(br, tile[j], rec[j], slot[j]);
+    }
+    if (!fine) {   // a staging row was full (or a splat was dropped): live records take the direct path
 #pragma unroll
         for (int j = 0; j < 4; ++j)
-            if (!fine[j] && ok[j]) bin_direct(prm, s, tile[j], rec[j]);
+            if (!((DIRECT_MASK >> j) & 1) && slot[j] >= br.cap && ok[j]) bin_direct(prm, s, tile[j], rec[j]);
     }
     return dropped;
 }
@@ -264,6 +287,7 @@ __device__ __forceinline__ uint32_t iterate_block(const RenderParams &prm, const
             if constexpr ((OPT & OPT_NO_DROP) != 0) {
                 // the host has proved every splat alive and in bounds: only a thread without a point (NaN) holds back
                 CFS_CHECK(!have || bin_in_bounds<false>(br, X[j], Y[j]));
+                CFS_CHECK((OPT & OPT_ALL_HAVE) == 0 || have);
                 ok[j] = have;
             } else {
                 ok[j] = alive && bin_in_bounds<(OPT & OPT_SYM_BOUNDS) != 0>(br, X[j], Y[j]);
@@ -271,7 +295,8 @@ __device__ __forceinline__ uint32_t iterate_block(const RenderParams &prm, const
         }
         if constexpr ((OPT & OPT_BIN_FIXED) != 0) {
             // compiled for this render's split and output: one straight-line body
-            dropped += bin_block_splat<(OPT >> OPT_BIN_MASK_SHIFT) & 15, (OPT & OPT_BIN_RGBA) != 0, (OPT & OPT_NO_DROP) != 0>(prm, s, sm, br, X, Y, K, ok);
+            dropped += bin_block_splat<(OPT >> OPT_BIN_MASK_SHIFT) & 15, (OPT & OPT_BIN_RGBA) != 0, (OPT & OPT_NO_DROP) != 0,
+                                       (OPT & OPT_NO_DROP) != 0 && (OPT & OPT_ALL_HAVE) != 0>(prm, s, sm, br, X, Y, K, ok);
         } else {
             // warp-uniform choice of one of three straight-line bodies (hybrid RGBA / hybrid HIST / pure bins); any
             // non-zero mask runs as "every other splat" here -- the exact mask is a compiled-in option
