@@ -450,6 +450,8 @@ bool wants_jit(int flags)
 uint32_t hybrid_mask(const cfs_render_args *a)
 {
     if (!((a->flags & CFS_FLAG_BIN_HYBRID) || a->variant == CFS_VARIANT_AUTO)) return 0u;
+    static const int forced = [] { const char *e = getenv("CFS_BIN_MASK"); return (e && *e) ? atoi(e) & 15 : -1; }();   // kernel development
+    if (forced >= 0) return (uint32_t)forced;
     return 1u;       // one splat in four: measured against 5 (every other), 0 (pure bins) and 7 on configs[1] and [2] (DESIGN "hybrid")
 }
 
