@@ -172,6 +172,7 @@ __device__ __forceinline__ void bin_flush(const RenderParams &prm, const SharedT
     uint32_t *s_cnt = sm;
     uint16_t *s_buf = reinterpret_cast<uint16_t *>(sm + bin_buf_offset(b.n_tiles));
     if (warp >= b.n_tiles) return;                     // warp owns no tile (warp-uniform)
+    if (final) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");   // units handed to the bulk-copy engine have landed
     const bool valid = my_tile < b.n_tiles;
     uint32_t mine = valid ? s_cnt[my_tile] : 0u;
     unsigned todo = __ballot_sync(0xFFFFFFFFu, final ? mine > 0u : mine >= kBinFlushRecords);
@@ -248,11 +249,6 @@ __device__ __forceinline__ void bin_flush(const RenderParams &prm, const SharedT
     }
 }
 
-// The flush of the steady state, written for instruction count (the general bin_flush above costs ~340 warp-
-// instructions per call, ~10 per iteration at a 32-iteration interval: profiles/r02): every row holding >= 256
-// records loses its WHOLE 256-record units, one 512-byte coalesced store each (LDS.128 -> STG.128 through 32-bit
-// shared-window addresses), and the remainder (< 256 records, it sits >= 512 bytes up the row, so the move cannot
-// overlap itself) goes back to the row start.  A tile whose pool or list ran out hands the warp to the general flush.
 __device__ __forceinline__ uint4 bin_lds_u4(uint32_t a)
 {
     uint4 v;
@@ -264,10 +260,20 @@ __device__ __forceinline__ void bin_sts_u4(uint32_t a, const uint4 &v)
     asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" :: "r"(a), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
 
+// The flush of the steady state (the general bin_flush above handles the last, padded units and tiles without a pool
+// block): every row holding >= 256 records loses its WHOLE 256-record units, each moved by the bulk-copy engine
+// (cp.async.bulk shared -> global, 512 bytes).  The lane that OWNS a tile issues its units by itself -- its pool
+// position is in its own registers, so nothing is shuffled and no lane loads or stores a record (round 2 first moved
+// them LDS.128 -> STG.128 through all 32 lanes: 10.8 % of the instructions of pass 1 and a tenth of its LSU
+// wavefronts; configs[2] 5.66 -> 5.47 ms per frame, configs[1] 2.757 -> 2.739 ms) -- then waits until the engine has
+// READ the rows (not for the writes to land; the final flush waits for those), and the warp moves the remainders
+// (< 256 records, >= 512 bytes up the row) back to the row start together.  A tile that cannot open a block keeps
+// its records and goes to the general flush at the next call.
 __device__ __forceinline__ void bin_flush_units(const RenderParams &prm, const SharedTables &s, uint32_t *sm, const BinRegs &br, BinLane &bl)
 {
     const BinParams &b = prm.bin;
-    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+    constexpr uint32_t nwarps = (uint32_t)kBinThreads / 32u;      // pass 1 is always launched with kBinThreads threads
+    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
     if (warp >= b.n_tiles) return;                     // warp owns no tile (warp-uniform)
     const uint32_t my_tile = lane * nwarps + warp;
     const bool valid = my_tile < b.n_tiles;
@@ -275,18 +281,17 @@ __device__ __forceinline__ void bin_flush_units(const RenderParams &prm, const S
     uint32_t mine = 0u;
     if (valid) asm volatile("ld.shared.u32 %0, [%1];" : "=r"(mine) : "r"(br.cnt_addr + 4u * my_tile));
     mine = min(mine, br.cap);                          // slots >= cap went direct
-    unsigned todo = __ballot_sync(0xFFFFFFFFu, mine >= kBinFlushRecords);
-    if (todo == 0u) return;
-    const size_t list_base = ((size_t)my_tile * b.grid + blockIdx.x) * b.lcap;
-    char *pool_lane = reinterpret_cast<char *>(b.pool) + 16u * lane;
-    do {
-        const int src = __ffs(todo) - 1;
-        todo &= todo - 1;
-        const uint32_t cnt = __shfl_sync(0xFFFFFFFFu, mine, src);
-        const uint32_t units = cnt / kBinFlushRecords;
-        uint32_t row = br.buf_addr + ((uint32_t)src * nwarps + warp) * br.row_bytes + 16u * lane;
-        for (uint32_t u = 0; u < units; ++u, row += 2u * kBinFlushRecords) {
-            if ((int)lane == src && (bl.pos & (kBinBlockRecords - 1u)) == 0u) {
+    uint32_t units = mine / kBinFlushRecords;          // whole units of MY tile
+    if (!__any_sync(0xFFFFFFFFu, units != 0u)) return;
+    const uint32_t my_row = br.buf_addr + my_tile * br.row_bytes;
+    if (units != 0u) {
+        // the records were written through the generic proxy (st.shared, before the barrier): order them before the
+        // async proxy's reads
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        const size_t list_base = ((size_t)my_tile * b.grid + blockIdx.x) * b.lcap;
+        uint32_t u = 0u, row = my_row;
+        for (; u < units; ++u, row += 2u * kBinFlushRecords) {
+            if ((bl.pos & (kBinBlockRecords - 1u)) == 0u) {
                 // block full (or none yet): open the prefetched one, list it, prefetch another
                 if (bl.next < b.nb && bl.nblk < b.lcap) {
                     b.list[list_base + bl.nblk] = bl.next;
@@ -294,29 +299,34 @@ __device__ __forceinline__ void bin_flush_units(const RenderParams &prm, const S
                     ++bl.nblk;
                     bl.next = atomicAdd(&b.ctrl[0], 1u) + 1u;
                 } else {
-                    bl.pos = kBinInvalid;              // pool or list exhausted: direct from now on
+                    bl.pos = kBinInvalid;              // pool or list exhausted: the general flush takes over at the next call
+                    break;
                 }
             }
-            const uint32_t pos = __shfl_sync(0xFFFFFFFFu, bl.pos, src);
-            const uint4 v = bin_lds_u4(row);
-            CFS_CHECK(pos == kBinInvalid || (pos >= kBinBlockRecords && pos + kBinFlushRecords <= (b.nb + 1u) * kBinBlockRecords));
-            CFS_CHECK(row + 16u <= br.buf_addr + b.n_tiles * br.row_bytes);
-            if (pos != kBinInvalid) {
-                *reinterpret_cast<uint4 *>(pool_lane + 2u * (size_t)pos) = v;
-                if ((int)lane == src) bl.pos += kBinFlushRecords;
-            } else {                                     // rare: this unit goes down the direct path
-                const uint32_t r[4] = {v.x, v.y, v.z, v.w};
-                const uint32_t tile = (uint32_t)src * nwarps + warp;
-#pragma unroll
-                for (int i = 0; i < 8; ++i) bin_direct(prm, s, tile, (r[i >> 1] >> (16 * (i & 1))) & 0xFFFFu);
-                if (lane == 0) atomicAdd(&b.ctrl[1], kBinFlushRecords);
-            }
+            CFS_CHECK(bl.pos >= kBinBlockRecords && bl.pos + kBinFlushRecords <= (b.nb + 1u) * kBinBlockRecords);
+            CFS_CHECK(row + 2u * kBinFlushRecords <= br.buf_addr + b.n_tiles * br.row_bytes);
+            asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
+                         :: "l"(b.pool + bl.pos), "r"(row), "n"(2 * kBinFlushRecords) : "memory");
+            bl.pos += kBinFlushRecords;
         }
-        const uint32_t rest = cnt % kBinFlushRecords;
-        if (8u * lane < rest) bin_sts_u4(row - units * 2u * kBinFlushRecords, bin_lds_u4(row));    // reads >= 512 B up, writes < 512 B: disjoint
-        if ((int)lane == src) mine = rest;
-    } while (todo);
-    if (valid) asm volatile("st.shared.u32 [%0], %1;" :: "r"(br.cnt_addr + 4u * my_tile), "r"(mine) : "memory");
+        units = u;                                     // units that really left
+        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");     // the rows have been read: their memory is free again
+    }
+    __syncwarp();
+    unsigned todo = __ballot_sync(0xFFFFFFFFu, units != 0u);
+    while (todo) {                                     // remainders (< one unit unless a pool ran out) back to the row start, 32 lanes together
+        const int src = __ffs(todo) - 1;
+        todo &= todo - 1;
+        const uint32_t cnt = __shfl_sync(0xFFFFFFFFu, mine, src), un = __shfl_sync(0xFFFFFFFFu, units, src);
+        const uint32_t rest = cnt - un * kBinFlushRecords;
+        const uint32_t row = br.buf_addr + ((uint32_t)src * nwarps + warp) * br.row_bytes + 16u * lane;
+        for (uint32_t off = 0u; off < rest; off += kBinFlushRecords) {     // reads >= 512 B above the writes of the same step
+            if (off + 8u * lane < rest) bin_sts_u4(row + 2u * off, bin_lds_u4(row + 2u * (off + un * kBinFlushRecords)));
+            __syncwarp();
+        }
+    }
+    if (valid) asm volatile("st.shared.u32 [%0], %1;" :: "r"(br.cnt_addr + 4u * my_tile), "r"(mine - units * kBinFlushRecords) : "memory");
 }
 
 // ---------------------------------------------------------------------------------------------
