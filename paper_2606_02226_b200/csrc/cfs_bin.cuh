@@ -161,83 +161,90 @@ __device__ __forceinline__ void bin_lane_init(const RenderParams &prm, BinLane &
     bl.next = (my_tile < prm.bin.n_tiles) ? atomicAdd(&prm.bin.ctrl[0], 1u) + 1u : 0u;   // block 0 is never used
 }
 
-// Called by every thread of the CTA between two __syncthreads.  Rows holding >= kBinFlushRecords
-// records (any record when `final`) are written out by the owning warp, 512 bytes per store
-// instruction; the remainder moves to the row start.
-__device__ __forceinline__ void bin_flush(const RenderParams &prm, const SharedTables &s, uint32_t *sm, BinLane &bl, bool final)
+// The staging records are written through the generic proxy (st.shared) and read by the bulk-copy engine (async
+// proxy): every WRITER orders its stores with this fence, then the threads synchronise, then one lane issues the copy
+// (render_kernel fences before the barrier that precedes bin_drain).
+__device__ __forceinline__ void bin_fence_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+// Called by every thread of the CTA between two __syncthreads: the owning warp DRAINS every staging row that holds at
+// least kBinDrainMin records (any record when `final`) into the (CTA, tile) pool block -- the WHOLE row, padded to a whole
+// 128-bit vector with the DUMMY record (the counter behind the tile's last one: pass 2 counts it without a test), moved
+// by the bulk-copy engine: one elected lane hands the row to cp.async.bulk (shared -> global, split where it crosses
+// into the next 2 KiB block), so no lane loads or stores a record and nothing stays behind -- no remainder to move, all
+// of a row's capacity serves the next interval.  The warp then waits until the engine has READ the rows (not for the
+// writes to land; the final drain waits for those).  A tile whose pool or list ran out sends its records down the
+// direct path.  (History: whole 256-record units through LDS.128 -> STG.128 by all 32 lanes, with the remainder carried,
+// were 10.8 % of the instructions of pass 1; the same units through the bulk engine 12 % less time on configs[2].)
+__device__ __forceinline__ void bin_drain(const RenderParams &prm, const SharedTables &s, const BinRegs &br, BinLane &bl, bool final)
 {
     const BinParams &b = prm.bin;
-    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
-    const uint32_t my_tile = lane * nwarps + warp;
-    uint32_t *s_cnt = sm;
-    uint16_t *s_buf = reinterpret_cast<uint16_t *>(sm + bin_buf_offset(b.n_tiles));
+    constexpr uint32_t nwarps = (uint32_t)kBinThreads / 32u;      // pass 1 is always launched with kBinThreads threads
+    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
     if (warp >= b.n_tiles) return;                     // warp owns no tile (warp-uniform)
-    if (final) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");   // units handed to the bulk-copy engine have landed
+    const uint32_t my_tile = lane * nwarps + warp;
     const bool valid = my_tile < b.n_tiles;
-    uint32_t mine = valid ? s_cnt[my_tile] : 0u;
-    unsigned todo = __ballot_sync(0xFFFFFFFFu, final ? mine > 0u : mine >= kBinFlushRecords);
-    const size_t list_base = ((size_t)my_tile * b.grid + blockIdx.x) * b.lcap;
-    while (todo) {
-        const int src = __ffs(todo) - 1;
-        todo &= todo - 1;
-        const uint32_t tile = (uint32_t)src * nwarps + warp;
-        uint32_t cnt = min(__shfl_sync(0xFFFFFFFFu, mine, src), b.cap);   // slots >= cap went direct
-        uint16_t *row = s_buf + tile * b.cap;
-        uint16_t *head = row;                            // a row may hold several flush units
-        while (cnt >= kBinFlushRecords || (final && cnt > 0u)) {
-            const uint32_t n = min(cnt, kBinFlushRecords);
-            if ((int)lane == src && (bl.pos & (kBinBlockRecords - 1u)) == 0u && bl.pos != kBinInvalid) {
-                // block full (or none yet): open the prefetched one, list it, prefetch another
-                if (bl.next < b.nb && bl.nblk < b.lcap) {
-                    b.list[list_base + bl.nblk] = bl.next;
-                    bl.pos = bl.next * kBinBlockRecords;
-                    ++bl.nblk;
-                    bl.next = atomicAdd(&b.ctrl[0], 1u) + 1u;
-                } else {
-                    bl.pos = kBinInvalid;              // pool or list exhausted: direct from now on
-                }
-            }
-            const uint32_t pos = __shfl_sync(0xFFFFFFFFu, bl.pos, src);
-            uint4 v = make_uint4(0u, 0u, 0u, 0u);
-            if (8u * lane < n) v = reinterpret_cast<const uint4 *>(head)[lane];    // 8 records; never past the row
-            if (pos != kBinInvalid) {
-                if (n < kBinFlushRecords) {
-                    // last, partial unit of this (CTA, tile): pad it to 256 records with the DUMMY record (the counter
-                    // behind the tile's last one), so that pass 2 counts whole 512-byte units without a test per record
-                    const uint32_t dummy = b.tile_pixels * b.nk, d2 = dummy | (dummy << 16);
-                    uint32_t w[4] = {v.x, v.y, v.z, v.w};
-#pragma unroll
-                    for (int i = 0; i < 4; ++i) {
-                        const uint32_t r0 = 8u * lane + 2u * i;
-                        w[i] = (r0 >= n) ? d2 : (r0 + 1u >= n) ? ((w[i] & 0xFFFFu) | (dummy << 16)) : w[i];
+    uint32_t mine = 0u;
+    if (valid) asm volatile("ld.shared.u32 %0, [%1];" : "=r"(mine) : "r"(br.cnt_addr + 4u * my_tile));
+    mine = min(mine, br.cap);                          // slots >= cap went direct
+    unsigned todo = __ballot_sync(0xFFFFFFFFu, final ? mine > 0u : mine >= b.drain_min);
+    if (todo != 0u) {
+        const size_t list_base = ((size_t)my_tile * b.grid + blockIdx.x) * b.lcap;
+        const uint32_t dummy = b.tile_pixels * b.nk;
+        do {
+            const int src = __ffs(todo) - 1;
+            todo &= todo - 1;
+            const uint32_t tile = (uint32_t)src * nwarps + warp;
+            const uint32_t cnt = __shfl_sync(0xFFFFFFFFu, mine, src);
+            const uint32_t cnt8 = (cnt + kBinGrain - 1u) & ~(kBinGrain - 1u);     // <= cap: cap is a multiple of 64
+            const uint32_t row = br.buf_addr + tile * br.row_bytes;
+            if (cnt + lane < cnt8)                                            // pad the last vector (at most 7 records)
+                asm volatile("st.shared.u16 [%0], %1;" :: "r"(row + 2u * (cnt + lane)), "h"((uint16_t)dummy) : "memory");
+            bin_fence_async();                                                // writers fence, then synchronise, then one lane issues
+            __syncwarp();
+            uint32_t left = cnt8, from = row;
+            do {
+                uint32_t pos = __shfl_sync(0xFFFFFFFFu, bl.pos, src);
+                if ((pos & (kBinBlockRecords - 1u)) == 0u) {                  // block full (or none yet); kBinInvalid ends in ones
+                    if ((int)lane == src) {    // open the prefetched block, list it, prefetch another
+                        if (bl.next < b.nb && bl.nblk < b.lcap) {
+                            b.list[list_base + bl.nblk] = bl.next;
+                            bl.pos = bl.next * kBinBlockRecords;
+                            ++bl.nblk;
+                            bl.next = atomicAdd(&b.ctrl[0], 1u) + 1u;
+                        } else {
+                            bl.pos = kBinInvalid;              // pool or list exhausted: direct from now on
+                        }
                     }
-                    reinterpret_cast<uint4 *>(b.pool + pos)[lane] = make_uint4(w[0], w[1], w[2], w[3]);
-                } else {
-                    reinterpret_cast<uint4 *>(b.pool + pos)[lane] = v;
+                    pos = __shfl_sync(0xFFFFFFFFu, bl.pos, src);
                 }
-                if ((int)lane == src) bl.pos += n;
-            } else {
-                const uint32_t r[4] = {v.x, v.y, v.z, v.w};
-#pragma unroll
-                for (int i = 0; i < 8; ++i)
-                    if (8u * lane + i < n) bin_direct(prm, s, tile, (r[i >> 1] >> (16 * (i & 1))) & 0xFFFFu);
-                if (lane == 0) atomicAdd(&b.ctrl[1], n);
-            }
-            cnt -= n;
-            head += kBinFlushRecords;
+                if (pos == kBinInvalid) {                                     // rare: the rest of the row goes down the direct path
+                    const uint32_t first = cnt8 - left;
+                    for (uint32_t i = first + lane; i < cnt; i += 32u) bin_direct(prm, s, tile, lds_u16(row + 2u * i));
+                    if (lane == 0u && cnt > first) atomicAdd(&b.ctrl[1], cnt - first);
+                    break;
+                }
+                const uint32_t seg = min(left, kBinBlockRecords - (pos & (kBinBlockRecords - 1u)));
+                CFS_CHECK(pos >= kBinBlockRecords && pos + seg <= (b.nb + 1u) * kBinBlockRecords && (pos & (kBinGrain - 1u)) == 0u && (seg & (kBinGrain - 1u)) == 0u);
+                CFS_CHECK(from + 2u * seg <= br.buf_addr + b.n_tiles * br.row_bytes);
+                if (lane == 0u)
+                    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
+                                 :: "l"(b.pool + pos), "r"(from), "r"(2u * seg) : "memory");
+                if ((int)lane == src) bl.pos = pos + seg;
+                from += 2u * seg;
+                left -= seg;
+            } while (left != 0u);
+            if ((int)lane == src) mine = 0u;
+        } while (todo != 0u);
+        if (lane == 0u) {
+            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+            if (final) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");          // the records have landed in the pool
+            else       asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");     // the rows have been read: their memory is free again
         }
-        if (cnt > 0u && head != row) {   // fewer than 256 records remain, at least 256 records up the row
-            uint4 m = make_uint4(0u, 0u, 0u, 0u);
-            if (8u * lane < cnt) m = reinterpret_cast<const uint4 *>(head)[lane];
-            __syncwarp();
-            if (8u * lane < cnt) reinterpret_cast<uint4 *>(row)[lane] = m;
-            __syncwarp();
-        }
-        if ((int)lane == src) mine = cnt;
+        __syncwarp();
     }
-    if (valid) s_cnt[my_tile] = min(mine, b.cap);
+    if (valid) asm volatile("st.shared.u32 [%0], %1;" :: "r"(br.cnt_addr + 4u * my_tile), "r"(mine) : "memory");
     if (final && valid) {
-        // blocks listed for (tile, CTA) and the fill of the last one (a full block reads 512)
+        // blocks listed for (tile, CTA) and the fill of the last one (a full block reads 1024)
         uint32_t fill = 0u;
         if (bl.nblk > 0u && bl.pos != kBinInvalid) {
             fill = bl.pos & (kBinBlockRecords - 1u);
@@ -249,86 +256,6 @@ __device__ __forceinline__ void bin_flush(const RenderParams &prm, const SharedT
     }
 }
 
-__device__ __forceinline__ uint4 bin_lds_u4(uint32_t a)
-{
-    uint4 v;
-    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a));
-    return v;
-}
-__device__ __forceinline__ void bin_sts_u4(uint32_t a, const uint4 &v)
-{
-    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" :: "r"(a), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
-}
-
-// The flush of the steady state (the general bin_flush above handles the last, padded units and tiles without a pool
-// block): every row holding >= 256 records loses its WHOLE 256-record units, each moved by the bulk-copy engine
-// (cp.async.bulk shared -> global, 512 bytes).  The lane that OWNS a tile issues its units by itself -- its pool
-// position is in its own registers, so nothing is shuffled and no lane loads or stores a record (round 2 first moved
-// them LDS.128 -> STG.128 through all 32 lanes: 10.8 % of the instructions of pass 1 and a tenth of its LSU
-// wavefronts; configs[2] 5.66 -> 5.47 ms per frame, configs[1] 2.757 -> 2.739 ms) -- then waits until the engine has
-// READ the rows (not for the writes to land; the final flush waits for those), and the warp moves the remainders
-// (< 256 records, >= 512 bytes up the row) back to the row start together.  A tile that cannot open a block keeps
-// its records and goes to the general flush at the next call.
-__device__ __forceinline__ void bin_flush_units(const RenderParams &prm, const SharedTables &s, uint32_t *sm, const BinRegs &br, BinLane &bl)
-{
-    const BinParams &b = prm.bin;
-    constexpr uint32_t nwarps = (uint32_t)kBinThreads / 32u;      // pass 1 is always launched with kBinThreads threads
-    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
-    if (warp >= b.n_tiles) return;                     // warp owns no tile (warp-uniform)
-    const uint32_t my_tile = lane * nwarps + warp;
-    const bool valid = my_tile < b.n_tiles;
-    if (__any_sync(0xFFFFFFFFu, valid && bl.pos == kBinInvalid)) { bin_flush(prm, s, sm, bl, false); return; }
-    uint32_t mine = 0u;
-    if (valid) asm volatile("ld.shared.u32 %0, [%1];" : "=r"(mine) : "r"(br.cnt_addr + 4u * my_tile));
-    mine = min(mine, br.cap);                          // slots >= cap went direct
-    uint32_t units = mine / kBinFlushRecords;          // whole units of MY tile
-    if (!__any_sync(0xFFFFFFFFu, units != 0u)) return;
-    const uint32_t my_row = br.buf_addr + my_tile * br.row_bytes;
-    if (units != 0u) {
-        // the records were written through the generic proxy (st.shared, before the barrier): order them before the
-        // async proxy's reads
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        const size_t list_base = ((size_t)my_tile * b.grid + blockIdx.x) * b.lcap;
-        uint32_t u = 0u, row = my_row;
-        for (; u < units; ++u, row += 2u * kBinFlushRecords) {
-            if ((bl.pos & (kBinBlockRecords - 1u)) == 0u) {
-                // block full (or none yet): open the prefetched one, list it, prefetch another
-                if (bl.next < b.nb && bl.nblk < b.lcap) {
-                    b.list[list_base + bl.nblk] = bl.next;
-                    bl.pos = bl.next * kBinBlockRecords;
-                    ++bl.nblk;
-                    bl.next = atomicAdd(&b.ctrl[0], 1u) + 1u;
-                } else {
-                    bl.pos = kBinInvalid;              // pool or list exhausted: the general flush takes over at the next call
-                    break;
-                }
-            }
-            CFS_CHECK(bl.pos >= kBinBlockRecords && bl.pos + kBinFlushRecords <= (b.nb + 1u) * kBinBlockRecords);
-            CFS_CHECK(row + 2u * kBinFlushRecords <= br.buf_addr + b.n_tiles * br.row_bytes);
-            asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
-                         :: "l"(b.pool + bl.pos), "r"(row), "n"(2 * kBinFlushRecords) : "memory");
-            bl.pos += kBinFlushRecords;
-        }
-        units = u;                                     // units that really left
-        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-        asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");     // the rows have been read: their memory is free again
-    }
-    __syncwarp();
-    unsigned todo = __ballot_sync(0xFFFFFFFFu, units != 0u);
-    while (todo) {                                     // remainders (< one unit unless a pool ran out) back to the row start, 32 lanes together
-        const int src = __ffs(todo) - 1;
-        todo &= todo - 1;
-        const uint32_t cnt = __shfl_sync(0xFFFFFFFFu, mine, src), un = __shfl_sync(0xFFFFFFFFu, units, src);
-        const uint32_t rest = cnt - un * kBinFlushRecords;
-        const uint32_t row = br.buf_addr + ((uint32_t)src * nwarps + warp) * br.row_bytes + 16u * lane;
-        for (uint32_t off = 0u; off < rest; off += kBinFlushRecords) {     // reads >= 512 B above the writes of the same step
-            if (off + 8u * lane < rest) bin_sts_u4(row + 2u * off, bin_lds_u4(row + 2u * (off + un * kBinFlushRecords)));
-            __syncwarp();
-        }
-    }
-    if (valid) asm volatile("st.shared.u32 [%0], %1;" :: "r"(br.cnt_addr + 4u * my_tile), "r"(mine - units * kBinFlushRecords) : "memory");
-}
-
 // ---------------------------------------------------------------------------------------------
 // pass 2.  MODE 0: HIST_U32 (nk = 1).  MODE 1: RGBA_F32 + MAP_INDEX: counters per (colour index, pixel), laid
 // out [k][pixel] -- the colour of a splat follows its position (the last map decides the region), so a tile is
@@ -337,8 +264,8 @@ __device__ __forceinline__ void bin_flush_units(const RenderParams &prm, const S
 // sum_k n_k * palette[k] (any summation order is a correct result, DESIGN R8; exact for integer-valued palettes
 // while every sum stays < 2^24).
 //
-// A record IS the index of its counter, and every flush unit in the pool is 256 whole records (pass 1 pads a
-// last unit with the DUMMY record, the counter behind the tile's last one), so the count loop is three
+// A record IS the index of its counter, and the pool holds whole 128-bit vectors of 8 records (pass 1 pads a
+// drained row with the DUMMY record, the counter behind the tile's last one), so the count loop is three
 // instructions per record: extract 16 bits, scale to a shared-window address, red.shared.add.
 __device__ __forceinline__ void bin_count8(uint32_t acc_addr, const uint4 &v)
 {
@@ -373,27 +300,28 @@ bin_accumulate_kernel(const __grid_constant__ RenderParams prm)
         const uint32_t tail = b.tails[(size_t)tile * b.grid + c];
         const uint32_t n_blk = tail >> kBinTailShift, last_fill = tail & ((1u << kBinTailShift) - 1u);
         const uint32_t *list = b.list + ((size_t)tile * b.grid + c) * b.lcap;
-        // two blocks (2 x 2 KiB = 2 x 4 units of 256 records, eight 128-bit loads per lane) in flight per warp
+        // two blocks (2 x 2 KiB, eight 128-bit loads per lane) in flight per warp; every block of a list is full except
+        // the last, whose fill is a whole number of 128-bit vectors (bin_drain pads with the DUMMY record)
         for (uint32_t j = part; j < n_blk; j += 2u * b.split) {
             uint4 v[2][4];
-            uint32_t units[2];
+            uint32_t nrec[2];
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
                 const uint32_t jj = j + (uint32_t)h * b.split;
-                units[h] = 0u;
+                nrec[h] = 0u;
                 if (jj < n_blk) {
-                    units[h] = (jj + 1u == n_blk) ? (last_fill + kBinFlushRecords - 1u) / kBinFlushRecords : kBinBlockRecords / kBinFlushRecords;
+                    nrec[h] = (jj + 1u == n_blk) ? last_fill : kBinBlockRecords;
                     const uint4 *src = reinterpret_cast<const uint4 *>(b.pool + (size_t)list[jj] * kBinBlockRecords);
 #pragma unroll
                     for (int q = 0; q < 4; ++q)
-                        if ((uint32_t)q < units[h]) v[h][q] = __ldcs(src + q * 32 + lane);
+                        if (kBinGrain * ((uint32_t)q * 32u + lane) < nrec[h]) v[h][q] = __ldcs(src + q * 32 + lane);
                 }
             }
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
 #pragma unroll
                 for (int q = 0; q < 4; ++q)
-                    if ((uint32_t)q < units[h]) bin_count8(acc_addr, v[h][q]);        // warp-uniform
+                    if (kBinGrain * ((uint32_t)q * 32u + lane) < nrec[h]) bin_count8(acc_addr, v[h][q]);
             }
         }
     }

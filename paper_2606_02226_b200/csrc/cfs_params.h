@@ -112,7 +112,8 @@ enum SplatKind : int {
 // shared-memory counter pass 2 increments (a tile has at most 3 * 2^14 = 49152 counters).  The pool is a set of fixed-size blocks; a block belongs to
 // one (CTA, tile) while it is filled and is listed under its tile when it is allocated.
 constexpr uint32_t kBinBlockRecords = 1024;    // records per pool block (2 KiB)
-constexpr uint32_t kBinFlushRecords = 256;     // records per flush: one 512-byte coalesced store
+constexpr uint32_t kBinGrain = 8;              // records per 128-bit vector: a drained row is padded to whole vectors with the DUMMY record
+constexpr uint32_t kBinDrainMin = 64;          // a row is drained when it holds at least this many records (a 128-byte store or longer)
 constexpr uint32_t kBinTailShift = 11;         // tails word: blocks << 11 | records in the last block (<= 1024)
 constexpr uint32_t kBinDummy = 32;             // dummy fill counters behind cnt[n_tiles], one per lane: pre-set to the row capacity, they take
                                                // the dropped splats -- "row full" for free, so a dropped splat stores nothing and needs no predicate
@@ -144,7 +145,8 @@ struct BinParams {
     uint32_t magic, mshift; // pix / tile_pixels == umulhi(pix, magic) >> mshift for every pixel of the image
     uint32_t nk;           // colour slots per pixel: 1 = HIST, else the number of functions (<= 16)
     uint32_t cap;          // staging records per tile in shared memory (multiple of 64, >= 320)
-    uint32_t check_mask;   // flush check after Philox block q (4 iterations) when ((q + 1) & check_mask) == 0
+    uint32_t drain_min;    // a staging row is drained when it holds at least this many records (multiple of 8)
+    uint32_t check_every;  // the staging rows are drained every check_every Philox blocks (4 iterations each) of the CTA
     uint32_t split;        // pass 2: CTAs per tile
     uint32_t hybrid;       // 4-bit mask: iteration j of every steady-state Philox block splats straight to L2 when bit j is set
                            // (0 = pure bins, 5 = every other splat: the hybrid stage)

@@ -243,10 +243,19 @@ __device__ __forceinline__ uint32_t bin_block_splat(const RenderParams &prm, con
         if ((DIRECT_MASK >> j) & 1) continue;
         fine &= bin_store_record(br, tile[j], rec[j], slot[j]);
     }
-    if (!fine) {   // a staging row was full (or a splat was dropped): live records take the direct path
+    if (!fine) {   // a staging row was full (or a splat was dropped): live records go straight to L2 -- the pixel and the
+                   // colour index are still in registers, so an overflow costs one reduction, not a division (rows of hot
+                   // tiles may overflow now and then: that is what lets the drain interval be long)
 #pragma unroll
-        for (int j = 0; j < 4; ++j)
-            if (!((DIRECT_MASK >> j) & 1) && slot[j] >= br.cap && ok[j]) bin_direct(prm, s, tile[j], rec[j]);
+        for (int j = 0; j < 4; ++j) {
+            if (((DIRECT_MASK >> j) & 1) || slot[j] < br.cap || !ok[j]) continue;
+            if (RGBA && br.ktp != 0u) {      // (the run-time test: kernels linked ahead of time run HIST renders through the RGBA body, ktp = 0)
+                const float4 c = lds_v4(sm.tab + CFS_SM_OFF(palette) + 16u * (uint32_t)K[j]);
+                bin_red_add_v4_f32(reinterpret_cast<float *>(prm.image) + 4 * (size_t)(uint32_t)pix[j], c.x, c.y, c.z, c.w);
+            } else {
+                bin_red_add_u32(reinterpret_cast<uint32_t *>(prm.image) + (uint32_t)pix[j], 1u);
+            }
+        }
     }
     return dropped;
 }
@@ -368,13 +377,8 @@ __device__ __forceinline__ uint32_t iterate_block(const RenderParams &prm, const
                                                                        StepCtx{plo, phi, it}, direct_half);
         }
     }
-    // steady-state blocks are flushed by the caller, between runs of blocks (render_kernel): the run then is a loop
-    // of its own whose invariants -- the Philox round keys above all -- stay in uniform registers
-    if (CHECKED && SPLAT == SPLAT_BIN && ((((uint32_t)it0 >> 2) + 1u) & prm.bin.check_mask) == 0u) {   // CTA-uniform
-        __syncthreads();
-        bin_flush_units(prm, s, s_hist, br, bl);
-        __syncthreads();
-    }
+    // the staging rows of SPLAT_BIN are drained by the caller, between runs of blocks (render_kernel): a run then is a
+    // loop of its own whose invariants -- the Philox round keys above all -- stay in uniform registers
     return dropped;
 }
 
@@ -423,6 +427,7 @@ render_kernel(const __grid_constant__ RenderParams prm)
     const int I = prm.iterations, B = prm.burn_in;
     const int it_fast0 = min((B + 3) & ~3, I & ~3), it_fast1 = I & ~3;   // steady-state Philox blocks: [it_fast0, it_fast1)
     uint32_t n_in = 0, n_drop = 0;
+    int until = (SPLAT == SPLAT_BIN) ? (int)prm.bin.check_every : 0;
 
     for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; ; i += stride) {
         // SPLAT_HIST_WARPAGG uses full-warp collectives inside: keep whole warps in the loop
@@ -454,39 +459,48 @@ render_kernel(const __grid_constant__ RenderParams prm)
             }
             // blocks touching burn-in or the ragged end take the checked path, the rest the lean one
             int it0 = 0;
-#pragma unroll 1
-            for (; it0 < it_fast0; it0 += 4)
-                dropped += iterate_block<DIM, GEN, AFF, SPLAT, SIG, TRIG, OPT, true>(prm, s, sm, s_hist, plo, phi, it0, gx, gy, gz, have, bl, br);
             if (SPLAT == SPLAT_BIN) {
-                // runs of blocks up to the next flush boundary (CTA-uniform: every thread of the CTA is at the same it0)
-                const int mask = (int)prm.bin.check_mask;
+                // every thread of the CTA is at the same it0 (whole CTAs in the loop), so `until` -- Philox blocks left
+                // before the staging rows are drained, counted across the points a thread renders -- is CTA-uniform
 #pragma unroll 1
-                while (it0 < it_fast1) {
-                    const int stop = min(it_fast1, (((it0 >> 2) | mask) + 1) << 2);
+                for (; it0 < it_fast0; it0 += 4) {
+                    dropped += iterate_block<DIM, GEN, AFF, SPLAT, SIG, TRIG, OPT, true>(prm, s, sm, s_hist, plo, phi, it0, gx, gy, gz, have, bl, br);
+                    if (--until == 0) { bin_fence_async(); __syncthreads(); bin_drain(prm, s, br, bl, false); __syncthreads(); until = (int)prm.bin.check_every; }
+                }
+#pragma unroll 1
+                while (it0 < it_fast1) {                   // runs of steady-state blocks up to the next drain
+                    const int run = min((it_fast1 - it0) >> 2, until);
+                    const int stop = it0 + 4 * run;
 #pragma unroll 1
                     for (; it0 < stop; it0 += 4)
                         dropped += iterate_block<DIM, GEN, AFF, SPLAT, SIG, TRIG, OPT, false>(prm, s, sm, s_hist, plo, phi, it0, gx, gy, gz, have, bl, br);
-                    if (((it0 >> 2) & mask) == 0) {
-                        __syncthreads();
-                        bin_flush_units(prm, s, s_hist, br, bl);
-                        __syncthreads();
-                    }
+                    until -= run;
+                    if (until == 0) { bin_fence_async(); __syncthreads(); bin_drain(prm, s, br, bl, false); __syncthreads(); until = (int)prm.bin.check_every; }
+                }
+#pragma unroll 1
+                for (; it0 < I; it0 += 4) {
+                    dropped += iterate_block<DIM, GEN, AFF, SPLAT, SIG, TRIG, OPT, true>(prm, s, sm, s_hist, plo, phi, it0, gx, gy, gz, have, bl, br);
+                    if (--until == 0) { bin_fence_async(); __syncthreads(); bin_drain(prm, s, br, bl, false); __syncthreads(); until = (int)prm.bin.check_every; }
                 }
             } else {
 #pragma unroll 1
+                for (; it0 < it_fast0; it0 += 4)
+                    dropped += iterate_block<DIM, GEN, AFF, SPLAT, SIG, TRIG, OPT, true>(prm, s, sm, s_hist, plo, phi, it0, gx, gy, gz, have, bl, br);
+#pragma unroll 1
                 for (; it0 < it_fast1; it0 += 4)
                     dropped += iterate_block<DIM, GEN, AFF, SPLAT, SIG, TRIG, OPT, false>(prm, s, sm, s_hist, plo, phi, it0, gx, gy, gz, have, bl, br);
-            }
 #pragma unroll 1
-            for (; it0 < I; it0 += 4)
-                dropped += iterate_block<DIM, GEN, AFF, SPLAT, SIG, TRIG, OPT, true>(prm, s, sm, s_hist, plo, phi, it0, gx, gy, gz, have, bl, br);
+                for (; it0 < I; it0 += 4)
+                    dropped += iterate_block<DIM, GEN, AFF, SPLAT, SIG, TRIG, OPT, true>(prm, s, sm, s_hist, plo, phi, it0, gx, gy, gz, have, bl, br);
+            }
         }
         if (have) { n_drop += dropped; n_in += (uint32_t)(I - B) * (uint32_t)prm.n_branches - dropped; }
     }
 
     if (SPLAT == SPLAT_BIN) {           // write out what is left in the staging rows
+        bin_fence_async();
         __syncthreads();
-        bin_flush(prm, s, s_hist, bl, true);
+        bin_drain(prm, s, br, bl, true);
     }
     if (SPLAT == SPLAT_HIST_CLUSTER) {  // all peers done with my slice, then merge it (red.global, non-zero bins)
         cluster_sync_all();
