@@ -236,9 +236,9 @@ uint64_t cfs_hiz_scratch_bytes(int32_t width, int32_t height);
 cfs_status cfs_render_depth_noalloc(const cfs_system *sys, const cfs_render_args *args, void *cuda_stream);
 
 /* the tile plan of the BINNED variant for an image and a device shape, host arithmetic only (no device
- * needed; test instrument): out = { tiles, pixels per tile, magic, shift (tile of pixel p =
- * mulhi32(p, magic) >> shift), colour slots per pixel, staging records per tile, flush-check interval in
- * iterations, pass-2 CTAs per tile }.  UNSUPPORTED when the variant cannot serve the image. */
+ * needed; test instrument): out = { tiles (a power of two), pixels per tile, shift, mask (the tiles are
+ * interleaved: pixel p belongs to tile p & mask and is its pixel p >> shift), colour slots per pixel, staging
+ * records per tile, drain interval in iterations, pass-2 CTAs per tile }.  UNSUPPORTED when the variant cannot serve the image. */
 cfs_status cfs_binned_plan(int32_t width, int32_t height, int32_t out_mode, int32_t n_funcs, int32_t sms,
                            int32_t smem_per_block_optin, uint32_t out[8]);
 

@@ -252,7 +252,7 @@ def cfs_binned_plan(width: int, height: int, out_mode, n_funcs: int, sms: int = 
     mode = OUT[out_mode] if isinstance(out_mode, str) else int(out_mode)
     out = (C.c_uint32 * 8)()
     _check(lib().cfs_binned_plan(int(width), int(height), mode, int(n_funcs), int(sms), int(smem_optin), out))
-    keys = ["n_tiles", "tile_pixels", "magic", "mshift", "nk", "cap", "check_every", "split"]
+    keys = ["n_tiles", "tile_pixels", "tile_shift", "tile_mask", "nk", "cap", "check_every", "split"]
     return dict(zip(keys, [int(v) for v in out]))
 
 

@@ -702,18 +702,17 @@ bool bin_shape_raw(int gen, int out_mode, int color, uint32_t n_funcs, int32_t w
     const uint64_t n_pix = (uint64_t)width * height;
     if (n_pix > (1ull << 28)) { *why = "binned variant serves images up to 2^28 pixels"; return false; }
     // pass 2 keeps (pixels per tile) x nk counters in shared memory: at most 3 * 2^14 (192 KiB), which is also
-    // what a 16-bit record can index.  Tile sizes are 2^s or 3 * 2^s pixels.  Fewer, larger tiles leave longer
-    // staging rows in pass 1, hence fewer barriers; but at least 64 tiles so that one tile's arrivals per
-    // iteration stay small against a row.
-    int shift = 15;
-    uint32_t mul = 1;
-    auto tiles_for = [&](int sh, uint32_t m) { const uint64_t tp = (uint64_t)m << sh; return (n_pix + tp - 1) / tp; };
-    auto smaller = [&]() { if (mul == 3) { mul = 1; ++shift; } else { mul = 3; shift -= 2; } };   // 3*2^s -> 2^(s+1) -> 3*2^(s-1) ...
-    while ((((uint64_t)mul << shift) * nk > 49152u) && (shift > 8 || mul == 3)) smaller();
-    while (tiles_for(shift, mul) < 64 && (shift > 8 || mul == 3)) smaller();
-    if (((uint64_t)mul << shift) * nk > 49152u) { *why = "no tile size for this number of colour slots"; return false; }
-    const uint64_t n_tiles = tiles_for(shift, mul);
-    if (n_tiles > (uint64_t)cfs::kBinThreads) { *why = "image has too many tiles for the binned variant"; return false; }
+    // what a 16-bit record can index.  Tiles are INTERLEAVED: with n_tiles = 2^t, pixel p belongs to tile p & (2^t - 1)
+    // and is its pixel p >> t -- every tile samples the whole image, so all tiles draw splats at the same rate
+    // whatever the attractor looks like (contiguous tiles drew up to 2.4 x the even share on configs[1], whose
+    // swirled square covers 41 % of the image, and the staging rows had to be sized and drained for the hottest one),
+    // and the tile / record arithmetic of a splat is an AND, a shift and a multiply-add.  The fewest tiles (at least
+    // 64) whose counters fit: longer staging rows, fewer drains.
+    uint32_t tshift = 6;
+    auto tp_for = [&](uint32_t t) { return (n_pix + (1ull << t) - 1) >> t; };
+    while (tshift < 10 && tp_for(tshift) * nk > 49152u) ++tshift;
+    if (tp_for(tshift) * nk > 49152u) { *why = "image has too many pixels (x colour slots) for 1024 tiles of 49152 counters"; return false; }
+    const uint64_t n_tiles = 1ull << tshift;
     // pass 1 staging: cnt + rows of `cap` records per tile, next to the static tables
     // kBinCtasPerSm CTAs of pass 1 share the SM's shared memory (1 KiB per CTA is reserved by the system)
     const long budget = ((long)di.smem_sm / cfs::kBinCtasPerSm < (long)di.smem_optin ? (long)di.smem_sm / cfs::kBinCtasPerSm : (long)di.smem_optin)
@@ -724,20 +723,9 @@ bool bin_shape_raw(int gen, int out_mode, int color, uint32_t n_funcs, int32_t w
     if (cap < 320) { *why = "image has too many tiles for the binned variant's staging rows"; return false; }
     cfs::BinParams &b = pl->bp;
     memset(&b, 0, sizeof(b));
-    b.n_tiles = (uint32_t)n_tiles; b.tile_pixels = mul << shift;
+    b.n_tiles = (uint32_t)n_tiles; b.tile_pixels = (uint32_t)tp_for(tshift);
+    b.tshift = tshift; b.tmask = (uint32_t)n_tiles - 1u;
     b.nk = nk; b.cap = (uint32_t)cap;
-    // division by tile_pixels as multiply-high + shift, exact for every pixel index of this image
-    {
-        const uint64_t d = b.tile_pixels;
-        bool found = false;
-        for (uint32_t l = 0; l < 32 && !found; ++l) {
-            const unsigned __int128 pw = (unsigned __int128)1 << (32 + l);
-            const unsigned __int128 m = (pw + d - 1) / d;
-            if (m >> 32) continue;
-            if ((unsigned __int128)n_pix * (m * d - pw) < pw) { b.magic = (uint32_t)m; b.mshift = l; found = true; }
-        }
-        if (!found) { *why = "no exact tile division for this image size"; return false; }
-    }
     // the rows are drained every E iterations (a multiple of 4: whole Philox blocks), E the largest value <= 128 whose
     // expected arrivals per row, times 1.9 for tiles that draw more than the even share, fit what a drained row has
     // free (a row keeps < drain_min records behind) with 16 records of slack.  Hotter rows overflow now and then; an
@@ -749,7 +737,7 @@ bool bin_shape_raw(int gen, int out_mode, int color, uint32_t n_funcs, int32_t w
     if (const char *x = getenv("CFS_BIN_DRAIN_MIN")) { const int v = atoi(x); if (v >= 8 && v <= 1024) b.drain_min = (uint32_t)v / 8 * 8; }   // kernel development
     const double room = (double)cap - (double)b.drain_min - 16.0;
     uint32_t every = 128;
-    while (every > 4 && 1.9 * every * per_it > room) every -= 4;
+    while (every > 4 && 1.25 * every * per_it > room) every -= 4;
     if (const char *x = getenv("CFS_BIN_EVERY")) { const int v = atoi(x); if (v >= 4 && v <= 4096) every = (uint32_t)v / 4 * 4; }   // kernel development
     b.check_every = every / 4;                         // in Philox blocks of 4 iterations
     // pass 2 runs one CTA per SM (the tile fills shared memory) in waves of `sms` CTAs: among the splits
@@ -844,7 +832,7 @@ extern "C" cfs_status cfs_binned_plan(int32_t width, int32_t height, int32_t out
     const char *why = "";
     if (!bin_shape_raw(CFS_GEN_IFS, out_mode, out_mode == CFS_OUT_RGBA_F32 ? CFS_COLOR_MAP_INDEX : CFS_COLOR_NONE, (uint32_t)n_funcs,
                        width, height, di, 0u, 1u, &pl, &why)) return fail(CFS_ERR_UNSUPPORTED, "%s", why);
-    out[0] = pl.bp.n_tiles; out[1] = pl.bp.tile_pixels; out[2] = pl.bp.magic; out[3] = pl.bp.mshift;
+    out[0] = pl.bp.n_tiles; out[1] = pl.bp.tile_pixels; out[2] = pl.bp.tshift; out[3] = pl.bp.tmask;
     out[4] = pl.bp.nk; out[5] = pl.bp.cap; out[6] = 4u * pl.bp.check_every; out[7] = pl.bp.split;
     return CFS_OK;
 }

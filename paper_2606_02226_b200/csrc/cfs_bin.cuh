@@ -46,7 +46,7 @@ __device__ __forceinline__ uint32_t bin_buf_offset(uint32_t n_tiles) { return (n
 // one record down the direct path (staging row full, or no pool block for the tile)
 __device__ __forceinline__ void bin_direct(const RenderParams &prm, const SharedTables &s, uint32_t tile, uint32_t rec)
 {
-    const uint32_t pix = tile * prm.bin.tile_pixels + rec % prm.bin.tile_pixels;   // rare path: a real division is fine
+    const uint32_t pix = ((rec % prm.bin.tile_pixels) << prm.bin.tshift) | tile;   // rare path: a real division is fine
     if (prm.color_rule == 0) {
         bin_red_add_u32(reinterpret_cast<uint32_t *>(prm.image) + pix, 1u);
     } else {
@@ -61,7 +61,7 @@ struct BinRegs {
     uint32_t cnt_addr, buf_addr;   // shared addresses of cnt[] and buf[][]
     uint32_t row_bytes, cap;       // bytes per row, records per row
     uint32_t dummy;                // index of this lane's dummy counter (n_tiles + lane)
-    uint32_t tp, ntp, magic, mshift; // tile = umulhi(pix, magic) >> mshift == pix / tp for every pixel of the image; ntp = -tp
+    uint32_t tmask, tshift;        // tile of pixel p = p & tmask, its pixel in the tile p >> tshift (interleaved tiles)
     uint32_t ktp;                  // colour index stride of a record: tp for RGBA, 0 for HIST (the colour is ignored)
     float sx, ox, sy, oy;          // pixel map (DESIGN R8)
     float xmin, xmax, ymin, ymax;  // closed bounds (DESIGN R8)
@@ -75,7 +75,7 @@ __device__ __forceinline__ BinRegs bin_regs_init(const RenderParams &prm, uint32
     r.buf_addr = r.cnt_addr + 4u * bin_buf_offset(prm.bin.n_tiles);
     r.cap = prm.bin.cap; r.row_bytes = 2u * prm.bin.cap;
     r.dummy = prm.bin.n_tiles;      // + lane, added by each thread after the broadcast
-    r.tp = prm.bin.tile_pixels; r.ntp = 0u - prm.bin.tile_pixels; r.magic = prm.bin.magic; r.mshift = prm.bin.mshift;
+    r.tmask = prm.bin.tmask; r.tshift = prm.bin.tshift;
     r.ktp = (prm.color_rule == 0) ? 0u : prm.bin.tile_pixels;
     r.sx = prm.sx; r.ox = prm.ox; r.sy = prm.sy; r.oy = prm.oy;
     r.xmin = prm.xmin; r.xmax = prm.xmax; r.ymin = prm.ymin; r.ymax = prm.ymax;
@@ -108,8 +108,8 @@ __device__ __forceinline__ int bin_pixel_of(const BinRegs &br, float x, float y)
 
 __device__ __forceinline__ void bin_record_of(const BinRegs &br, int pix, int k, uint32_t &tile, uint32_t &rec)
 {
-    tile = __umulhi((uint32_t)pix, br.magic) >> br.mshift;
-    rec = (tile * br.ntp + (uint32_t)pix) + (uint32_t)k * br.ktp;
+    tile = (uint32_t)pix & br.tmask;
+    rec = ((uint32_t)pix >> br.tshift) + (uint32_t)k * br.ktp;
 }
 
 // row 7, binned: one shared-memory atomic + one shared store per splat (interpreter path: branches are fine here)
@@ -133,7 +133,7 @@ __device__ __forceinline__ void bin_append(const RenderParams &prm, const Shared
 __device__ __forceinline__ uint32_t bin_take_slot(const BinRegs &br, bool ok, uint32_t tile, uint32_t rec)
 {
     const uint32_t t_eff = ok ? tile : br.dummy;
-    CFS_CHECK(tile <= br.dummy - (threadIdx.x & 31u) - 1u && rec <= 49152u && rec < (br.ktp ? 65536u : br.tp));
+    CFS_CHECK(tile <= br.dummy - (threadIdx.x & 31u) - 1u && rec <= 49152u);
     uint32_t slot;
     asm volatile("atom.shared.add.u32 %0, [%1], 1;" : "=r"(slot) : "r"(br.cnt_addr + 4u * t_eff) : "memory");
     return slot;
@@ -329,12 +329,13 @@ bin_accumulate_kernel(const __grid_constant__ RenderParams prm)
 
     // merge the private tile (red.global, touched pixels only)
     const uint32_t n_pix_tile = b.tile_pixels;
-    const uint32_t pix0 = tile * b.tile_pixels, n_pix = (uint32_t)prm.W * (uint32_t)prm.H;
+    const uint32_t n_pix = (uint32_t)prm.W * (uint32_t)prm.H, tshift = b.tshift;    // pixel i of the tile is image pixel (i << tshift) | tile
     if (MODE == 0) {
         uint32_t *hist = reinterpret_cast<uint32_t *>(prm.image);
         for (uint32_t i = threadIdx.x; i < n_pix_tile; i += blockDim.x) {
             const uint32_t c = acc[i];
-            if (c && pix0 + i < n_pix) bin_red_add_u32(hist + pix0 + i, c);
+            const uint32_t pix = (i << tshift) | tile;
+            if (c && pix < n_pix) bin_red_add_u32(hist + pix, c);
         }
     } else {
         float *img = reinterpret_cast<float *>(prm.image);
@@ -353,7 +354,8 @@ bin_accumulate_kernel(const __grid_constant__ RenderParams prm)
                     any = 1u;
                 }
             }
-            if (any && pix0 + i < n_pix) bin_red_add_v4_f32(img + 4 * (size_t)(pix0 + i), r, g, bl, a);
+            const uint32_t pix = (i << tshift) | tile;
+            if (any && pix < n_pix) bin_red_add_v4_f32(img + 4 * (size_t)pix, r, g, bl, a);
         }
     }
 }

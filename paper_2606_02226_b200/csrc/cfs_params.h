@@ -141,8 +141,8 @@ struct BinParams {
     uint32_t *ctrl;        // [0] = blocks handed out, [1] = records splatted directly (statistics)
     uint32_t nb, lcap, n_tiles;
     uint32_t grid;         // CTAs of pass 1
-    uint32_t tile_pixels;  // pixels per tile: 2^s or 3 * 2^s
-    uint32_t magic, mshift; // pix / tile_pixels == umulhi(pix, magic) >> mshift for every pixel of the image
+    uint32_t tile_pixels;  // pixels (counters per colour slot) of a tile: ceil(W H / n_tiles)
+    uint32_t tshift, tmask; // n_tiles = 2^tshift, tmask = n_tiles - 1: pixel p belongs to tile p & tmask and is its pixel p >> tshift (tiles are INTERLEAVED)
     uint32_t nk;           // colour slots per pixel: 1 = HIST, else the number of functions (<= 16)
     uint32_t cap;          // staging records per tile in shared memory (multiple of 64, >= 320)
     uint32_t drain_min;    // a staging row is drained when it holds at least this many records (multiple of 8)

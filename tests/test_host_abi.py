@@ -78,9 +78,9 @@ SIZES = [(512, 512), (1024, 1024), (1920, 1080), (3840, 2160), (64, 64), (200, 1
 @pytest.mark.parametrize("mode,n_funcs", [("hist_u32", 1), ("rgba_f32", 3), ("rgba_f32", 4), ("rgba_f32", 16)])
 @pytest.mark.parametrize("size", SIZES)
 def test_binned_plan_tile_arithmetic_is_exact(cfs, size, mode, n_funcs):
-    """tile(p) = mulhi32(p, magic) >> shift must equal p // tile_pixels for EVERY pixel of the image
-    (checked at all tile boundaries and on a random sample), and the plan must respect the shared-
-    memory budgets of both passes."""
+    """Interleaved tiles: pixel p belongs to tile p & mask and is its pixel p >> shift.  The map must be a
+    bijection between the pixels of the image and (tile, pixel in tile) pairs below the planned sizes, and
+    the plan must respect the shared-memory budgets of both passes."""
     wd, ht = size
     n_pix = wd * ht
     try:
@@ -88,25 +88,25 @@ def test_binned_plan_tile_arithmetic_is_exact(cfs, size, mode, n_funcs):
     except cfs.CfsError as e:
         assert e.status == cfs.CFS_ERR_UNSUPPORTED          # too many tiles for 320-record staging rows
         nk = 1 if mode == "hist_u32" else n_funcs
-        assert -(-n_pix // (49152 // nk)) > 300
+        assert -(-n_pix // (49152 // nk)) > 200
         return
-    tp, nt = pl["tile_pixels"], pl["n_tiles"]
-    assert nt == -(-n_pix // tp) and nt <= 1024
-    assert tp & (tp - 1) == 0 or (tp % 3 == 0 and (tp // 3) & (tp // 3 - 1) == 0)      # 2^s or 3 * 2^s
+    tp, nt, sh, mask = pl["tile_pixels"], pl["n_tiles"], pl["tile_shift"], pl["tile_mask"]
+    assert nt == 1 << sh and mask == nt - 1 and 64 <= nt <= 1024
+    assert tp == -(-n_pix // nt)                                                        # ceil(n_pix / n_tiles)
     assert tp * pl["nk"] * 4 <= 192 << 10                                              # pass 2 counters
     assert pl["nk"] == (1 if mode == "hist_u32" else n_funcs)
     assert pl["cap"] >= 320 and pl["cap"] % 64 == 0
     assert nt * pl["cap"] * 2 + (nt + 4) * 4 <= 232448                                  # pass 1 staging rows (u16)
     assert tp * pl["nk"] <= 1 << 16                                                     # a record fits 16 bits
     assert pl["check_every"] % 4 == 0 and 4 <= pl["check_every"] <= 128 and pl["split"] >= 1     # whole Philox blocks
-    edges = np.arange(0, nt + 1, dtype=np.uint64) * np.uint64(tp)
-    p = np.unique(np.concatenate([edges, edges[1:] - np.uint64(1), edges[:-1] + np.uint64(1),
+    p = np.unique(np.concatenate([np.arange(0, min(n_pix, 4 * nt), dtype=np.uint64),
                                   np.random.default_rng(1).integers(0, n_pix, 4096, dtype=np.uint64),
-                                  np.array([0, n_pix - 1], dtype=np.uint64)]))
+                                  np.array([0, n_pix - 1, max(n_pix - nt, 0), max(n_pix - nt - 1, 0)], dtype=np.uint64)]))
     p = p[p < n_pix]
-    got = ((p * np.uint64(pl["magic"])) >> np.uint64(32)) >> np.uint64(pl["mshift"])
-    assert np.array_equal(got, p // np.uint64(tp))
-    assert pl["magic"] < 1 << 32
+    tile, inner = p & np.uint64(mask), p >> np.uint64(sh)
+    assert tile.max() < nt and inner.max() < tp
+    assert np.array_equal((inner << np.uint64(sh)) | tile, p)                           # the inverse pass 2 uses
+    assert len(np.unique(tile * np.uint64(tp) + inner)) == len(p)                       # no two pixels share a counter
 
 
 def test_hiz_scratch_bytes_is_host_arithmetic(cfs):
