@@ -426,6 +426,25 @@ def test_binned_rgba_equals_direct(cfs, oracle, cfg, hybrid):
     _check_rgba(gb, o, cb, oc)
 
 
+@pytest.mark.parametrize("size,mode,jit", [((1000, 777), "rgba_f32", True), ((333, 555), "hist_u32", True), ((1921, 1079), "rgba_f32", False),
+                                           ((64, 64), "hist_u32", False), ((4099, 61), "rgba_f32", True)])
+def test_interleaved_tiles_on_awkward_image_sizes(cfs, oracle, size, mode, jit):
+    """The tiles of the binned variant are interleaved (pixel p in tile p & mask as its pixel p >> shift): images
+    whose pixel count is no multiple of the tile count, whose rows are no multiple of it, tiny and very wide ones --
+    binned (pure, hybrid, run-time compiled or linked) must equal the direct variant bit for bit (integer colour
+    sums), and the oracle on the histogram."""
+    wd, ht = size
+    w = W.config(1 if mode == "rgba_f32" else 0).scaled(n_points=(1 << 15) + 77, iterations=120, width=wd, height=ht)
+    flags = ["jit"] if jit else []
+    gd, cd = gpu_render(cfs, w, variant="direct")
+    for extra in ([], ["bin_hybrid"]):
+        gb, cb = gpu_render(cfs, w, variant="binned", flags=flags + extra)
+        assert np.array_equal(gb, gd) and np.array_equal(cb, cd), (size, mode, extra)
+    if mode == "hist_u32":           # the affine-only system of configs[0]: bit-exact against the oracle
+        o, oc, _ = oracle.render_parallel(w.system, w.render)
+        assert np.array_equal(gd, o) and np.array_equal(cd, oc)
+
+
 @pytest.mark.parametrize("cfg", [1, 2])
 def test_hist_output_of_a_coloured_system_through_the_bins(cfs, oracle, cfg):
     """HIST_U32 output from a system created with COLOR_MAP_INDEX (colour ignored, include/cfs.h): the tile
