@@ -237,11 +237,12 @@ __device__ __forceinline__ void bin_drain(const RenderParams &prm, const SharedT
         } while (todo != 0u);
         if (lane == 0u) {
             asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-            if (final) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");          // the records have landed in the pool
-            else       asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");     // the rows have been read: their memory is free again
+            asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");     // the rows have been read: their memory is free again
         }
         __syncwarp();
     }
+    if (final && lane == 0u) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");    // every record this warp handed over (now or in
+                                                                                          // an earlier drain) has landed in the pool
     if (valid) asm volatile("st.shared.u32 [%0], %1;" :: "r"(br.cnt_addr + 4u * my_tile), "r"(mine) : "memory");
     if (final && valid) {
         // blocks listed for (tile, CTA) and the fill of the last one (a full block reads 1024)
