@@ -268,14 +268,20 @@ __device__ __forceinline__ void bin_drain(const RenderParams &prm, const SharedT
 // A record IS the index of its counter, and the pool holds whole 128-bit vectors of 8 records (pass 1 pads a
 // drained row with the DUMMY record, the counter behind the tile's last one), so the count loop is three
 // instructions per record: extract 16 bits, scale to a shared-window address, red.shared.add.
+// Counter r lives at slot r ^ ((r >> 5) & 31): a permutation inside every aligned group of 32 counters that mixes
+// bits 5..9 of the index into the bank.  The bank of a record was (pixel >> t) mod 32 -- on configs[1] a function of
+// the coarse x position and y mod 4, and the swirled disc does not fill the x range evenly: 4.16 wavefronts per
+// red.shared against 3.5 for uniformly random banks (and 3.6 on configs[2]).  Two more ALU instructions per record
+// in a kernel that waits for the shared-memory pipe.
+__device__ __forceinline__ uint32_t bin_slot(uint32_t r) { return r ^ ((r >> 5) & 31u); }
 __device__ __forceinline__ void bin_count8(uint32_t acc_addr, const uint4 &v)
 {
     const uint32_t w[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
         CFS_CHECK((w[i] & 0xFFFFu) <= 49152u && (w[i] >> 16) <= 49152u);
-        asm volatile("red.shared.add.u32 [%0], 1;" :: "r"(acc_addr + ((w[i] & 0xFFFFu) << 2)) : "memory");
-        asm volatile("red.shared.add.u32 [%0], 1;" :: "r"(acc_addr + ((w[i] >> 16) << 2)) : "memory");
+        asm volatile("red.shared.add.u32 [%0], 1;" :: "r"(acc_addr + (bin_slot(w[i] & 0xFFFFu) << 2)) : "memory");
+        asm volatile("red.shared.add.u32 [%0], 1;" :: "r"(acc_addr + (bin_slot(w[i] >> 16) << 2)) : "memory");
     }
 }
 
@@ -283,13 +289,13 @@ template <int MODE>
 __global__ void __launch_bounds__(kBinAccThreads)
 bin_accumulate_kernel(const __grid_constant__ RenderParams prm)
 {
-    extern __shared__ __align__(16) uint32_t acc[];     // tile_pixels * nk counters + the dummy one (+ padding to 16 bytes)
+    extern __shared__ __align__(16) uint32_t acc[];     // tile_pixels * nk counters + the dummy one, rounded up to whole groups of 32 (bin_slot)
     const BinParams &b = prm.bin;
     const uint32_t tile = blockIdx.x / b.split, part = blockIdx.x % b.split;
     const uint32_t n_ctr = b.tile_pixels * b.nk;
     {
         uint4 *a4 = reinterpret_cast<uint4 *>(acc);
-        for (uint32_t i = threadIdx.x; i < n_ctr / 4u + 1u; i += blockDim.x) a4[i] = make_uint4(0u, 0u, 0u, 0u);
+        for (uint32_t i = threadIdx.x; i < (n_ctr + 32u) / 32u * 8u; i += blockDim.x) a4[i] = make_uint4(0u, 0u, 0u, 0u);
     }
     __syncthreads();
     const uint32_t acc_addr = (uint32_t)__cvta_generic_to_shared(acc);
@@ -334,7 +340,7 @@ bin_accumulate_kernel(const __grid_constant__ RenderParams prm)
     if (MODE == 0) {
         uint32_t *hist = reinterpret_cast<uint32_t *>(prm.image);
         for (uint32_t i = threadIdx.x; i < n_pix_tile; i += blockDim.x) {
-            const uint32_t c = acc[i];
+            const uint32_t c = acc[bin_slot(i)];
             const uint32_t pix = (i << tshift) | tile;
             if (c && pix < n_pix) bin_red_add_u32(hist + pix, c);
         }
@@ -345,7 +351,7 @@ bin_accumulate_kernel(const __grid_constant__ RenderParams prm)
             float r = 0.f, g = 0.f, bl = 0.f, a = 0.f;
             uint32_t any = 0u;
             for (uint32_t k = 0; k < nk; ++k) {
-                const uint32_t c = acc[k * n_pix_tile + i];
+                const uint32_t c = acc[bin_slot(k * n_pix_tile + i)];
                 if (c) {
                     const float fc = (float)c;
                     r = __fmaf_rn(fc, prm.palette[4 * k + 0], r);
