@@ -718,7 +718,7 @@ bool bin_shape_raw(int gen, int out_mode, int color, uint32_t n_funcs, int32_t w
     const long budget = ((long)di.smem_sm / cfs::kBinCtasPerSm < (long)di.smem_optin ? (long)di.smem_sm / cfs::kBinCtasPerSm : (long)di.smem_optin)
                         - (long)sizeof(cfs::SharedTables) - 2048;
     const long row_bytes = (budget - 4 * (long)(n_tiles + cfs::kBinDummy) - 16) / (long)n_tiles;       // u32 cnt[] + u16 rows
-    long cap = row_bytes / 2 / 64 * 64;
+    long cap = (row_bytes - (long)cfs::kBinRowPad) / 2 / 64 * 64;
     if (cap > 4096) cap = 4096;
     if (cap < 320) { *why = "image has too many tiles for the binned variant's staging rows"; return false; }
     cfs::BinParams &b = pl->bp;
@@ -755,7 +755,7 @@ bool bin_shape_raw(int gen, int out_mode, int color, uint32_t n_funcs, int32_t w
         }
         b.split = best;
     }
-    pl->smem_pass1 = (n_tiles + cfs::kBinDummy + 3) / 4 * 4 * 4 + n_tiles * (size_t)cap * 2;
+    pl->smem_pass1 = (n_tiles + cfs::kBinDummy + 3) / 4 * 4 * 4 + n_tiles * ((size_t)cap * 2 + cfs::kBinRowPad);
     pl->smem_pass2 = ((size_t)b.tile_pixels * nk + 32) / 32 * 32 * 4;      // + the dummy counter the padding records of a last flush unit hit
     pl->grid1 = (uint32_t)di.sms * cfs::kBinCtasPerSm;
     return true;

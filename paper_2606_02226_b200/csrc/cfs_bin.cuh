@@ -73,7 +73,7 @@ __device__ __forceinline__ BinRegs bin_regs_init(const RenderParams &prm, uint32
     BinRegs r;
     r.cnt_addr = (uint32_t)__cvta_generic_to_shared(sm);
     r.buf_addr = r.cnt_addr + 4u * bin_buf_offset(prm.bin.n_tiles);
-    r.cap = prm.bin.cap; r.row_bytes = 2u * prm.bin.cap;
+    r.cap = prm.bin.cap; r.row_bytes = 2u * prm.bin.cap + kBinRowPad;
     r.dummy = prm.bin.n_tiles;      // + lane, added by each thread after the broadcast
     r.tmask = prm.bin.tmask; r.tshift = prm.bin.tshift;
     r.ktp = (prm.color_rule == 0) ? 0u : prm.bin.tile_pixels;

@@ -115,6 +115,9 @@ constexpr uint32_t kBinBlockRecords = 1024;    // records per pool block (2 KiB)
 constexpr uint32_t kBinGrain = 8;              // records per 128-bit vector: a drained row is padded to whole vectors with the DUMMY record
 constexpr uint32_t kBinDrainMin = 64;          // a row is drained when it holds at least this many records (a 128-byte store or longer)
 constexpr uint32_t kBinTailShift = 11;         // tails word: blocks << 11 | records in the last block (<= 1024)
+constexpr uint32_t kBinRowPad = 16;            // bytes between two staging rows beyond their records: rows 2 * cap bytes long would all start on bank 0, and
+                                               // with interleaved tiles all rows fill in step, so the stores of a warp met on a few banks (4.15 wavefronts
+                                               // per STS); 16 bytes of skew per row spread them (rows stay 16-byte aligned for the bulk copy)
 constexpr uint32_t kBinDummy = 32;             // dummy fill counters behind cnt[n_tiles], one per lane: pre-set to the row capacity, they take
                                                // the dropped splats -- "row full" for free, so a dropped splat stores nothing and needs no predicate
 constexpr uint32_t kBinInvalid = 0xFFFFFFFFu;  // tile has no block (pool or list exhausted): direct splats
