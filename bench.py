@@ -157,7 +157,7 @@ RED_KEY = {0: "red_add_u32@1048576", 1: "red_add_v4f32@16777216", 2: "red_add_v4
 # executed warp-instructions per warp-iteration and DRAM bytes per launch of the dominant kernel: from the ncu captures
 # under profiles/ (file named beside each); None = not captured for the kernel as it stands
 NCU = {
-    1: {"executed_per_iteration": 48.9, "dram_bytes_per_launch": 1.516e9, "profile": "profiles/r02_hybrid_cfg1.txt",
+    1: {"executed_per_iteration": 48.9, "dram_bytes_per_launch": 1.517e9, "profile": "profiles/r02_hybrid_cfg1.txt",
         "scope": "pass 1 of one cfs_render (all 2^20 points in one chunk): 1.507 GB of 16-bit records written + 0.009 GB read; pass 2 reads them back (1.564 GB)"},
     2: {"executed_per_iteration": 49.2, "dram_bytes_per_launch": 1.710e9, "profile": "profiles/r02_hybrid_cfg2.txt",
         "scope": "pass 1 of the first of two chunks of one frame (2 424 832 of 2^22 points at the 2 GiB scratch cap): 1.706 GB of records written"},
