@@ -346,9 +346,9 @@ class ConfigBench:
             for t in self.w.frames[:1]:
                 self.compile_ms += cfs.cfs_specialize(self.sysh, self.make_args(t))
 
-    def make_args(self, t, extra_flags=()):
+    def make_args(self, t, extra_flags=(), flags=None):
         return self.cfs.make_args(self.w.render, d_image=self.img, d_cloud=self.d_cloud, d_counters=self.ctr, t=t,
-                                  point_offset=self.rank * self.P, flags=list(self.flags) + list(extra_flags),
+                                  point_offset=self.rank * self.P, flags=list(self.flags if flags is None else flags) + list(extra_flags),
                                   variant=self.args.variant, d_scratch=self.scratch)
 
     def step(self):
@@ -368,7 +368,7 @@ class ConfigBench:
         ev[1].record()
         return ev
 
-    def time_render_only(self, extra_flags=(), reps=5):
+    def time_render_only(self, extra_flags=(), reps=5, flags=None):
         """median device time of the cfs_render calls of one step (all frames), image clears outside the events"""
         torch, r = self.torch, self.w.render
         times = []
@@ -379,7 +379,7 @@ class ConfigBench:
                 self.img.fill_(-1 if r.out_mode == "depth_u64" else 0)
                 e0, e1 = event_pair(torch)
                 e0.record()
-                self.cfs.cfs_render(self.sysh, self.make_args(t, extra_flags))
+                self.cfs.cfs_render(self.sysh, self.make_args(t, extra_flags, flags))
                 e1.record()
                 torch.cuda.synchronize()
                 tot += e0.elapsed_time(e1) * 1e-3
@@ -485,6 +485,11 @@ def measure_config(cfs, torch, cfg, args, rank, world, flush, rates, peaks, peak
     t_pass1 = None
     if launches_per_render >= 2 and r.out_mode != "depth_u64":
         t_pass1 = cb.time_render_only(extra_flags=["bin_pass1_only"])
+    # the same render with the accurate sin/cos (libdevice sincosf, <= 2 ulp) beside the MUFU figure (the first repetition,
+    # which compiles the kernel when it is a run-time compiled one, is not timed)
+    t_render_sincosf = None
+    if args.fast_trig and any(x.type in ("swirl", "sinusoidal", "twist_z", "bend", "stretch_cos") for x in w.system.chain):
+        t_render_sincosf = cb.time_render_only(reps=3, flags=[f for f in cb.flags if f != "fast_trig"])
     hot_rate = None
     touched_px = None
     if w.system.gen == "cloud":
@@ -554,6 +559,7 @@ def measure_config(cfs, torch, cfg, args, rank, world, flush, rates, peaks, peak
             "config": workload_desc(w, cfg, world, "MUFU sin.approx/cos.approx (CFS_FLAG_FAST_TRIG)" if args.fast_trig else "sincosf (<= 2 ulp)"),
             "value": world * pi_step * steps / step_s, "unit": UNIT, "splats_per_s": world * (n_in / steps) / (step_s / steps),
             "steps": steps, "ms_per_step": step_s / steps * 1e3, "render_ms": t_render * 1e3,
+            "render_ms_sincosf": None if t_render_sincosf is None else t_render_sincosf * 1e3,
             "in_bounds_per_step": n_in // steps, "dropped_per_step": n_drop // steps,
             "clocks": clocks, "gpu_launches": int(launches), "launches_per_render": launches_per_render,
             "kernels": "run-time compiled for the system (CFS_FLAG_JIT; compile time below, outside the timed region)" if args.jit else "linked ahead of time",
