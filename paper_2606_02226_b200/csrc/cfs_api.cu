@@ -756,7 +756,7 @@ bool bin_shape_raw(int gen, int out_mode, int color, uint32_t n_funcs, int32_t w
         b.split = best;
     }
     pl->smem_pass1 = (n_tiles + cfs::kBinDummy + 3) / 4 * 4 * 4 + n_tiles * ((size_t)cap * 2 + cfs::kBinRowPad);
-    pl->smem_pass2 = ((size_t)b.tile_pixels * nk + 32) / 32 * 32 * 4;      // + the dummy counter the padding records of a last flush unit hit
+    pl->smem_pass2 = ((size_t)b.tile_pixels * nk + 32) / 32 * 32 * 4;      // + the dummy counter the padding records of a drained row hit, in whole groups of 32 (bin_slot)
     pl->grid1 = (uint32_t)di.sms * cfs::kBinCtasPerSm;
     return true;
 }

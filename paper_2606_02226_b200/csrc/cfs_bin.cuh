@@ -3,13 +3,15 @@
 // A direct splat costs one L2 reduction (row 7), and the L2 executes ~190 G of them per second
 // whatever their width (measured, cfs_microbench) -- 3x below what the sampler can generate.
 // Shared-memory privatisation removes that bound, but no BASELINE image fits one CTA's shared
-// memory (SURVEY 7 "hard parts" 1).  So the image is cut into tiles that do fit, and the splats
-// are partitioned by tile on their way through HBM:
+// memory (SURVEY 7 "hard parts" 1).  So the image is cut into tiles that do fit -- INTERLEAVED ones: with 2^t tiles,
+// pixel p belongs to tile p & (2^t - 1) as its pixel p >> t, so every tile samples the whole image and all tiles draw
+// splats at the same rate -- and the splats are partitioned by tile on their way through HBM:
 //
 //   pass 1 (render_kernel<..., SPLAT_BIN>): each splat becomes ONE 16-bit record
 //     (colour index * pixels per tile + pixel-in-tile), appended with one shared-memory atomic to the CTA's
-//     staging row of its tile; full rows leave as 512-byte coalesced stores into 2 KiB pool blocks
-//     owned by (CTA, tile), so no global atomic is paid per splat -- one per 512 records.
+//     staging row of its tile; every ~100 iterations the rows are drained by the bulk-copy engine (cp.async.bulk
+//     shared -> global) into 2 KiB pool blocks owned by (CTA, tile), so no global atomic is paid per splat -- one
+//     per 1024 records.
 //   pass 2 (bin_accumulate_kernel): one CTA per (tile, part) walks the tile's block list with
 //     coalesced 128-bit loads and counts records with shared-memory atomics (the record IS the
 //     counter index), then merges its private tile into the image with one red.global per
